@@ -1,0 +1,217 @@
+/*
+ * negf.h - C ABI of the B200-native LSE+OBC hot path of arxiv/paper_2602_03438.
+ *
+ * Path (Fig. 1 red blocks "LSE+OBC"; Eqs. 1-2):
+ * for many independent energies E, with z = E + i*eta and the block-tridiagonal (BT)
+ *     A(E) = z S - H - Sigma^R_B - Sigma^R_S,
+ * compute the selected blocks (i,i), (i,i+1), (i+1,i) of
+ *     G^R  = A^-1                                   (Eq. 1)
+ *     G^<> = G^R (Sigma^<>_B + Sigma^<>_S) (G^R)^H  (Eq. 2)
+ * by the recursive Green's function (RGF) sweeps, with the open-boundary
+ * self-energies Sigma_B ("open boundary condition term") obtained by
+ * Sancho-Rubio decimation of the lead blocks (BASELINE.json:north_star),
+ * and reduce them to density, LDOS, transmission and currents.
+ *
+ * Conventions
+ *  - negf_c128 = interleaved (re, im) doubles.  Every block is dense b x b ROW-MAJOR with
+ *    leading dimension b; blocks of a family are contiguous; batched arrays are
+ *    [N_E][n or n-1][b][b] (energy slowest).  No padding.
+ *  - Unless a parameter says HOST, every array pointer is a DEVICE pointer owned by the
+ *    caller.  The library never allocates or frees caller arrays; its only own allocation
+ *    is the small context object.  Scratch memory is the caller-provided workspace.
+ *  - All calls enqueue work on the context's stream and return without synchronising
+ *    (exception: negf_pipeline_host and negf_fp64_peak, which say so).
+ *  - Return value: 0 = enqueued; negative = argument / runtime error (see negf_strerror).
+ *    Numerical failures are reported PER ENERGY in the device int arrays info/status:
+ *    0 ok; k > 0 = zero pivot while inverting block k-1 (for the decimation: iteration k);
+ *    -1 = decimation hit max_iter without meeting tol (result still written).
+ *  - There is no CPU fallback: every call needs a CUDA device of compute capability 10.0.
+ *  - Thread safety: one context per host thread / stream.
+ */
+#ifndef NEGF_H
+#define NEGF_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct { double re, im; } negf_c128;
+typedef struct negf_ctx negf_ctx;
+
+/* error codes */
+#define NEGF_OK            0
+#define NEGF_EINVAL       -1   /* bad argument (NULL where required, n < 1, side not 0/1, ...) */
+#define NEGF_ENOWORKSPACE -2   /* workspace missing or smaller than negf_workspace_bytes()     */
+#define NEGF_EUNSUPPORTED -3   /* combination not implemented (documented at the call)         */
+#define NEGF_ECUDA        -4   /* CUDA runtime error; see negf_last_cuda_error()               */
+#define NEGF_ENOSTATE     -5   /* call needs the retained sweep state of negf_rgf_retarded     */
+
+/* kinds of scattering self-energy Sigma_S */
+#define NEGF_SIGMA_NONE   0
+#define NEGF_SIGMA_SCALAR 1    /* s(E) * I on every diagonal block                            */
+#define NEGF_SIGMA_BT     2    /* dense block-tridiagonal per energy                           */
+
+/* flags of negf_rgf_retarded */
+#define NEGF_KEEP_SWEEP   1    /* retain g_i, X_i, Y_i in the workspace for negf_rgf_lesser_greater */
+
+/* Device + energy grid (A = E S - H for electrons; BT shape). */
+typedef struct {
+    int n_blocks;              /* n >= 1 diagonal blocks                                       */
+    int block_size;            /* b >= 1                                                       */
+    int n_energy;              /* N_E >= 1 energies resident in this batch                     */
+    const negf_c128* H_diag;   /* [n][b][b]   Hermitian blocks, shared by all energies         */
+    const negf_c128* H_upper;  /* [n-1][b][b] H_{i,i+1}; H_{i+1,i} = H_{i,i+1}^H (may be NULL if n == 1) */
+    const negf_c128* S_diag;   /* [n][b][b]   or NULL: S = I (then S_upper must be NULL too)   */
+    const negf_c128* S_upper;  /* [n-1][b][b] S_{i,i+1}; S_{i+1,i} = S_{i,i+1}^H               */
+    const double*    energy;   /* [N_E] real energies E                                         */
+    double           eta;      /* z = E + i*eta multiplies S everywhere, leads included (R1)   */
+} negf_problem;
+
+/* One self-energy family: boundary blocks on the two contacts plus Sigma_S.
+ * For the retarded Sigma^R all of diag/upper/lower are independent.
+ * For Sigma^< and Sigma^> the full matrix is anti-Hermitian: lower = -upper^H is IMPLIED
+ * and `lower` is ignored. */
+typedef struct {
+    int kind;                  /* NEGF_SIGMA_NONE | _SCALAR | _BT                              */
+    const negf_c128* scalar;   /* [N_E]             (kind SCALAR)                              */
+    const negf_c128* diag;     /* [N_E][n][b][b]    (kind BT)                                  */
+    const negf_c128* upper;    /* [N_E][n-1][b][b]  (kind BT) Sigma_{i,i+1}                    */
+    const negf_c128* lower;    /* [N_E][n-1][b][b]  (kind BT, retarded only) Sigma_{i+1,i}     */
+    const negf_c128* left;     /* [N_E][b][b] boundary block added on block 0,   or NULL       */
+    const negf_c128* right;    /* [N_E][b][b] boundary block added on block n-1, or NULL       */
+} negf_sigma;
+
+/* Optional explicit lead (overrides "periodic copies of the contact blocks", reading R2;
+ * required when n_blocks == 1).  H_u/S_u couple a lead cell to its next cell on the right. */
+typedef struct {
+    const negf_c128* H_d;      /* [b][b] */
+    const negf_c128* H_u;      /* [b][b] */
+    const negf_c128* S_d;      /* [b][b] or NULL (identity) */
+    const negf_c128* S_u;      /* [b][b] or NULL (zero)     */
+} negf_lead;
+
+/* ---- context ---------------------------------------------------------------------------- */
+int negf_create(negf_ctx** out, int device);
+int negf_destroy(negf_ctx* ctx);
+/* cudaStream_t passed as void*; NULL = the legacy default stream. */
+int negf_set_stream(negf_ctx* ctx, void* cuda_stream);
+/* Bytes of workspace needed by ANY call on this problem shape (kind_max = the richest
+ * Sigma kind that will be passed, flags as for negf_rgf_retarded). */
+int negf_workspace_bytes(const negf_problem* p, int kind_max, int flags, size_t* bytes);
+/* Caller-owned device scratch (e.g. a torch tensor), 256-byte aligned. Retained sweep state
+ * lives here; replacing the workspace drops it. */
+int negf_set_workspace(negf_ctx* ctx, void* dev_ptr, size_t bytes);
+const char* negf_strerror(int code);
+/* cudaError_t of the last failing runtime call on this context (0 if none). */
+int negf_last_cuda_error(const negf_ctx* ctx);
+/* Number of kernels this context has launched since creation (bench.py's gpu_launches). */
+long long negf_launch_count(const negf_ctx* ctx);
+
+/* ---- S2: open-boundary self-energies ------------
+ * For each energy: a_d = z S_d - H_d, a_u = z S_u - H_u, a_l = z S_u^H - H_u^H of the lead
+ * (default: contact blocks 0/0-1 for side 0, n-1/(n-2,n-1) for side 1); Sancho-Rubio doubling
+ *   g = a_b^-1; a_s -= l g u (side 0) | u g l (side 1); a_b -= u g l + l g u; u = -u g u; l = -l g l
+ * until ||u||_F + ||l||_F <= tol (||a_u||_F + ||a_l||_F) or max_iter (reading R3); then
+ *   g_s = a_s^-1, Sigma^R = a_l g_s a_u (side 0) | a_u g_s a_l (side 1),
+ *   Gamma = i (Sigma^R - Sigma^R^H), f = 1/(1+exp((E-mu)/kT)),
+ *   Sigma^< = i f Gamma, Sigma^> = -i (1-f) Gamma.
+ * Outputs [N_E][b][b] each; any of gamma, sigma_lesser, sigma_greater, g_surface, fermi may be
+ * NULL.  iters [N_E] = doublings done; status [N_E] as described at the top. */
+int negf_obc_decimate(negf_ctx* ctx, const negf_problem* p, const negf_lead* lead /* or NULL */,
+                      int side, double mu, double kT, double tol, int max_iter,
+                      negf_c128* sigma_r, negf_c128* gamma,
+                      negf_c128* sigma_lesser, negf_c128* sigma_greater,
+                      negf_c128* g_surface, double* fermi, int* iters, int* status);
+
+/* ---- S1+S3+S4: retarded selected inversion ----------
+ *   g_0 = A_00^-1; g_i = (A_ii - A_{i,i-1} g_{i-1} A_{i-1,i})^-1;
+ *   G_{n-1,n-1} = g_{n-1}; X_i = g_i A_{i,i+1}; Y_i = A_{i+1,i} g_i;
+ *   G_{i,i+1} = -X_i G_{i+1,i+1}; G_{i+1,i} = -G_{i+1,i+1} Y_i; G_ii = g_i - G_{i,i+1} Y_i;
+ *   corner: G_{i,n-1} = -X_i G_{i+1,n-1}.
+ * sigma_r may be NULL (no self-energy at all).  GR_diag [N_E][n][b][b] required;
+ * GR_upper / GR_lower [N_E][n-1][b][b] and GR_corner [N_E][b][b] (= G_{0,n-1}) may be NULL.
+ * info [N_E]. */
+int negf_rgf_retarded(negf_ctx* ctx, const negf_problem* p, const negf_sigma* sigma_r,
+                      negf_c128* GR_diag, negf_c128* GR_upper, negf_c128* GR_lower,
+                      negf_c128* GR_corner, int flags, int* info);
+
+/* ---- S5+S6: lesser / greater selected blocks ----------------
+ *   g^x_0 = g_0 B_00 g_0^H;
+ *   g^x_i = g_i [B_ii + A_{i,i-1} g^x_{i-1} A_{i,i-1}^H - Y_{i-1} B_{i-1,i} - B_{i,i-1} Y_{i-1}^H] g_i^H;
+ *   G^x_{n-1,n-1} = g^x_{n-1};
+ *   G^x_{i,i+1} = (-g^x_i A_{i+1,i}^H + g_i B_{i,i+1}) (G^R_{i+1,i+1})^H - X_i G^x_{i+1,i+1};
+ *   G^x_ii = g^x_i - X_i G^x_{i+1,i} - G^x_{i,i+1} X_i^H - X_i G^x_{i+1,i+1} X_i^H,
+ *   G^x_{i+1,i} = -(G^x_{i,i+1})^H (not stored).
+ * Needs the sweep state retained by negf_rgf_retarded(..., NEGF_KEEP_SWEEP) on the SAME problem
+ * and sigma_r (else NEGF_ENOSTATE), and GR_diag from that call.  Either of sigma_lesser /
+ * sigma_greater may be NULL (then its outputs are ignored).  G*_diag [N_E][n][b][b],
+ * G*_upper [N_E][n-1][b][b] (may be NULL). */
+int negf_rgf_lesser_greater(negf_ctx* ctx, const negf_problem* p, const negf_sigma* sigma_r,
+                            const negf_sigma* sigma_lesser, const negf_sigma* sigma_greater,
+                            const negf_c128* GR_diag,
+                            negf_c128* GL_diag, negf_c128* GL_upper,
+                            negf_c128* GG_diag, negf_c128* GG_upper, int* info);
+
+/* ---- S7: observables (readings R11-R13) -------------
+ *   density[k]      = sum_E w_E Re[(-i/2pi) (G^< S)_kk]     over the BT pattern      [N = n b]
+ *   ldos[E][i]      = -(1/pi) Im Tr[(G^R S)_ii]                                      [N_E][n]
+ *   transmission[E] = Re Tr[Gamma_L G^R_{0,n-1} Gamma_R (G^R_{0,n-1})^H]             [N_E]
+ *   bond_current[E][i] = 2 Re Tr[(H_{i,i+1} - E S_{i,i+1}) G^<_{i+1,i}]              [N_E][n-1]
+ *   contact_current[E][c] = Re Tr[Sigma^<_c G^>_cc - Sigma^>_c G^<_cc], c = L, R     [N_E][2]
+ * Every output may be NULL (skipped); inputs only needed by skipped outputs may be NULL.
+ * density is OVERWRITTEN (not accumulated across calls); weights [N_E] device doubles. */
+int negf_observables(negf_ctx* ctx, const negf_problem* p,
+                     const negf_c128* GR_diag, const negf_c128* GR_upper, const negf_c128* GR_lower,
+                     const negf_c128* GR_corner,
+                     const negf_c128* GL_diag, const negf_c128* GL_upper, const negf_c128* GG_diag,
+                     const negf_c128* gamma_L, const negf_c128* gamma_R,
+                     const negf_c128* sigma_lesser_L, const negf_c128* sigma_greater_L,
+                     const negf_c128* sigma_lesser_R, const negf_c128* sigma_greater_R,
+                     const double* weights,
+                     double* density, double* ldos, double* transmission,
+                     double* bond_current, double* contact_current);
+
+/* ---- whole path with HOST buffers (bench.py's end-to-end leg) ---------------------------------
+ * All array arguments here are HOST pointers (pinned memory recommended).  Copies the inputs
+ * to the device, runs negf_obc_decimate (both sides) -> negf_rgf_retarded ->
+ * negf_rgf_lesser_greater -> negf_observables, copies the results back and SYNCHRONISES the
+ * stream before returning.  Device staging comes from `dev_scratch` (DEVICE pointer, caller
+ * owned, at least negf_pipeline_host_bytes()).  Sigma_S as for negf_sigma but with host
+ * pointers and left/right ignored.  Outputs may be NULL. */
+typedef struct {
+    negf_c128 *GR_diag, *GR_upper, *GR_lower, *GL_diag, *GL_upper, *GG_diag, *GG_upper;
+    double *density, *ldos, *transmission, *bond_current, *contact_current;
+    int *info;                /* [N_E] max over the stage codes */
+} negf_host_outputs;
+int negf_pipeline_host_bytes(const negf_problem* p_shape_only, int kind_max, int want_greater, size_t* bytes);
+int negf_pipeline_host(negf_ctx* ctx, const negf_problem* host_problem,
+                       const negf_sigma* host_sigma_r, const negf_sigma* host_sigma_lesser,
+                       const negf_sigma* host_sigma_greater, const double* host_weights,
+                       double mu_L, double mu_R, double kT, double tol, int max_iter,
+                       void* dev_scratch, size_t dev_scratch_bytes,
+                       const negf_host_outputs* out,
+                       size_t* h2d_bytes, size_t* d2h_bytes);
+
+/* ---- building blocks exposed for tests and roofline measurement -------- */
+/* C[e] = alpha * op(A[e]) op(B[e]) + beta * D[e], e < batch; m x n x k complex; row-major with
+ * leading dimensions lda/ldb/ldc (ldd = ldc); op: 0 = none, 1 = conjugate transpose; strides in
+ * elements between consecutive batch entries (0 = shared).  D may be NULL (beta ignored) or == C. */
+int negf_zgemm_batched(negf_ctx* ctx, int opA, int opB, int m, int n, int k,
+                       negf_c128 alpha, const negf_c128* A, int lda, long long strideA,
+                       const negf_c128* B, int ldb, long long strideB,
+                       negf_c128 beta, const negf_c128* D,
+                       negf_c128* C, int ldc, long long strideC, int batch);
+/* In-place inverse of `batch` dense b x b matrices (stride in elements), partial pivoting on
+ * |re|+|im|; info[e] = 0 or (column+1) of the first zero pivot.  Uses the context workspace. */
+int negf_zinverse_batched(negf_ctx* ctx, int b, negf_c128* A, long long stride, int batch, int* info);
+/* Measures the FP64 DMMA (mma.sync m8n8k4) issue-rate peak of this GPU for about `ms`
+ * milliseconds; SYNCHRONISES.  Writes TFLOP/s to *tflops (HOST pointer). */
+int negf_fp64_peak(negf_ctx* ctx, double ms, double* tflops);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NEGF_H */

@@ -1,0 +1,103 @@
+// Context management, error strings, the FP64 DMMA peak probe and the host-buffer pipeline
+// (include/negf.h).  No CPU fallback anywhere: negf_create fails unless a CUDA device of compute
+// capability 10.x is present.
+#include <new>
+
+#include "common.cuh"
+#include "workspace.cuh"
+
+extern "C" int negf_create(negf_ctx** out, int device) {
+    if (!out) return NEGF_EINVAL;
+    *out = nullptr;
+    int count = 0;
+    if (cudaGetDeviceCount(&count) != cudaSuccess || device < 0 || device >= count) return NEGF_ECUDA;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return NEGF_ECUDA;
+    if (prop.major != 10) return NEGF_EUNSUPPORTED;   // kernels are built for sm_100a only
+    if (cudaSetDevice(device) != cudaSuccess) return NEGF_ECUDA;
+    negf_ctx* c = new (std::nothrow) negf_ctx();
+    if (!c) return NEGF_EINVAL;
+    c->device = device; c->stream = nullptr; c->ws = nullptr; c->ws_bytes = 0; c->last_cuda_error = 0;
+    c->launches = 0; c->num_sms = prop.multiProcessorCount; c->sweep_valid = false;
+    c->sw_n = c->sw_b = c->sw_ne = 0;
+    *out = c;
+    return NEGF_OK;
+}
+extern "C" int negf_destroy(negf_ctx* ctx) {
+    if (!ctx) return NEGF_EINVAL;
+    delete ctx;
+    return NEGF_OK;
+}
+extern "C" int negf_set_stream(negf_ctx* ctx, void* s) {
+    if (!ctx) return NEGF_EINVAL;
+    ctx->stream = (cudaStream_t)s;
+    return NEGF_OK;
+}
+extern "C" int negf_set_workspace(negf_ctx* ctx, void* p, size_t bytes) {
+    if (!ctx) return NEGF_EINVAL;
+    if (p && ((uintptr_t)p & 255)) return NEGF_EINVAL;
+    ctx->ws = p; ctx->ws_bytes = p ? bytes : 0; ctx->sweep_valid = false;
+    return NEGF_OK;
+}
+extern "C" const char* negf_strerror(int code) {
+    switch (code) {
+        case NEGF_OK: return "ok";
+        case NEGF_EINVAL: return "invalid argument";
+        case NEGF_ENOWORKSPACE: return "workspace missing or too small (see negf_workspace_bytes)";
+        case NEGF_EUNSUPPORTED: return "unsupported configuration or device (needs compute capability 10.x)";
+        case NEGF_ECUDA: return "CUDA runtime error (see negf_last_cuda_error)";
+        case NEGF_ENOSTATE: return "no retained sweep state: call negf_rgf_retarded with NEGF_KEEP_SWEEP first";
+        default: return "unknown error code";
+    }
+}
+extern "C" int negf_last_cuda_error(const negf_ctx* ctx) { return ctx ? ctx->last_cuda_error : 0; }
+extern "C" long long negf_launch_count(const negf_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+// ---- FP64 tensor-pipe peak probe ---------------------------------------------------------------
+namespace {
+__global__ void __launch_bounds__(512) dmma_peak_kernel(double* out, int iters) {
+    double c[8][2];
+    double a = threadIdx.x * 1e-3, b = threadIdx.x * 2e-3;
+#pragma unroll
+    for (int i = 0; i < 8; i++) { c[i][0] = i; c[i][1] = -i; }
+    for (int it = 0; it < iters; it++) {
+#pragma unroll
+        for (int i = 0; i < 8; i++)
+            asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                         : "+d"(c[i][0]), "+d"(c[i][1]) : "d"(a), "d"(b));
+    }
+    double s = 0;
+#pragma unroll
+    for (int i = 0; i < 8; i++) s += c[i][0] + c[i][1];
+    if (s == 123.456) out[0] = s;   // never true; keeps the loop alive
+}
+}  // namespace
+
+extern "C" int negf_fp64_peak(negf_ctx* ctx, double ms, double* tflops) {
+    if (!ctx || !tflops) return NEGF_EINVAL;
+    double* d = nullptr;
+    NEGF_CUDA_CHECK(ctx, cudaMalloc(&d, 64));
+    cudaEvent_t e0, e1;
+    NEGF_CUDA_CHECK(ctx, cudaEventCreate(&e0));
+    NEGF_CUDA_CHECK(ctx, cudaEventCreate(&e1));
+    const int grid = ctx->num_sms * 2, threads = 512, iters = 4000;
+    const double flop_per_launch = 2.0 * 256 * 8 * (double)iters * (threads / 32) * grid;
+    dmma_peak_kernel<<<grid, threads, 0, ctx->stream>>>(d, 200);
+    NEGF_CUDA_CHECK(ctx, cudaStreamSynchronize(ctx->stream));
+    double best = 0.0, elapsed = 0.0;
+    while (elapsed < ms) {
+        NEGF_CUDA_CHECK(ctx, cudaEventRecord(e0, ctx->stream));
+        dmma_peak_kernel<<<grid, threads, 0, ctx->stream>>>(d, iters);
+        ctx->launches++;
+        NEGF_CUDA_CHECK(ctx, cudaEventRecord(e1, ctx->stream));
+        NEGF_CUDA_CHECK(ctx, cudaEventSynchronize(e1));
+        float t = 0.f;
+        NEGF_CUDA_CHECK(ctx, cudaEventElapsedTime(&t, e0, e1));
+        elapsed += t;
+        double tf = flop_per_launch / (t * 1e-3) * 1e-12;
+        if (tf > best) best = tf;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d);
+    *tflops = best;
+    return NEGF_OK;
+}

@@ -1,0 +1,106 @@
+// Shared declarations of the CUDA side (sm_100a only).  Not included by the oracle.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+
+#include "../../include/negf.h"
+
+typedef double2 cplx;  // (x, y) = (re, im), same bytes as negf_c128
+
+struct negf_ctx {
+    int device;
+    cudaStream_t stream;
+    void* ws;              // caller-owned workspace
+    size_t ws_bytes;
+    int last_cuda_error;
+    long long launches;
+    int num_sms;
+    // retained sweep state (NEGF_KEEP_SWEEP): valid for this shape only
+    bool sweep_valid;
+    int sw_n, sw_b, sw_ne;
+};
+
+#define NEGF_CUDA_CHECK(ctx, expr)                                  \
+    do {                                                            \
+        cudaError_t _e = (expr);                                    \
+        if (_e != cudaSuccess) {                                    \
+            (ctx)->last_cuda_error = (int)_e;                       \
+            return NEGF_ECUDA;                                      \
+        }                                                           \
+    } while (0)
+
+#define NEGF_LAUNCH_CHECK(ctx)                                      \
+    do {                                                            \
+        (ctx)->launches++;                                          \
+        cudaError_t _e = cudaGetLastError();                        \
+        if (_e != cudaSuccess) {                                    \
+            (ctx)->last_cuda_error = (int)_e;                       \
+            return NEGF_ECUDA;                                      \
+        }                                                           \
+    } while (0)
+
+#define NEGF_TRY(expr)                   \
+    do {                                 \
+        int _r = (expr);                 \
+        if (_r != NEGF_OK) return _r;    \
+    } while (0)
+
+__host__ __device__ inline cplx cmake(double r, double i) { cplx c; c.x = r; c.y = i; return c; }
+__device__ __forceinline__ cplx cadd(cplx a, cplx b) { return cmake(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ cplx csub(cplx a, cplx b) { return cmake(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ cplx cmul(cplx a, cplx b) {
+    return cmake(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+}
+__device__ __forceinline__ cplx cconj(cplx a) { return cmake(a.x, -a.y); }
+__device__ __forceinline__ cplx cneg(cplx a) { return cmake(-a.x, -a.y); }
+// c += a*b
+__device__ __forceinline__ void cfma(cplx& c, cplx a, cplx b) {
+    c.x = fma(a.x, b.x, c.x); c.x = fma(-a.y, b.y, c.x);
+    c.y = fma(a.x, b.y, c.y); c.y = fma(a.y, b.x, c.y);
+}
+// c -= a*b
+__device__ __forceinline__ void cfms(cplx& c, cplx a, cplx b) {
+    c.x = fma(-a.x, b.x, c.x); c.x = fma(a.y, b.y, c.x);
+    c.y = fma(-a.x, b.y, c.y); c.y = fma(-a.y, b.x, c.y);
+}
+// robust 1/a (Smith) -- pivots are O(1) here but keep it safe
+__device__ __forceinline__ cplx crecip(cplx a) {
+    if (fabs(a.x) >= fabs(a.y)) {
+        double r = a.y / a.x, d = a.x + a.y * r;
+        return cmake(1.0 / d, -r / d);
+    } else {
+        double r = a.x / a.y, d = a.x * r + a.y;
+        return cmake(r / d, -1.0 / d);
+    }
+}
+__device__ __forceinline__ double cabs1(cplx a) { return fabs(a.x) + fabs(a.y); }
+
+static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+// ---- internal entry points (host side, enqueue on ctx->stream) --------------------------------
+// zgemm.cu
+struct GemmArgs {
+    int opA, opB;            // 0 = N, 1 = conjugate transpose
+    int m, n, k;
+    cplx alpha, beta;
+    const cplx* A; int lda; long long sA;
+    const cplx* B; int ldb; long long sB;
+    const cplx* D; long long sD;   // addend (ld = ldc), may be NULL
+    cplx* C; int ldc; long long sC;
+    int batch;
+    const int* skip;         // optional [batch] device mask: entry skipped when skip[e] != 0
+};
+int zgemm_launch(negf_ctx* ctx, const GemmArgs& a);
+// convenience: square b x b x b, contiguous blocks
+int zgemm_bb(negf_ctx* ctx, int opA, int opB, int b, cplx alpha, const cplx* A, long long sA,
+             const cplx* B, long long sB, cplx beta, const cplx* D, long long sD,
+             cplx* C, long long sC, int batch, const int* skip);
+
+// zinv.cu
+size_t zinv_workspace_bytes(int b, int batch);
+// in-place inverse of A[e] (b x b, ld = b, stride sA); ws: zinv_workspace_bytes; info_code = value
+// written to info[e] on a zero pivot (>0), info untouched otherwise (caller zero-fills).
+int zinv_launch(negf_ctx* ctx, int b, cplx* A, long long sA, int batch, void* ws, int* info,
+                int info_code, const int* skip);
+

@@ -1,0 +1,214 @@
+// O(b^2) kernels around the GEMM / inverse building blocks: assembly of the blocks of
+// A = z S - H - Sigma^R and B = Sigma^<>, the anti-Hermitian combinations of
+// S5/S6, the Sancho-Rubio bookkeeping (reading R3) and the boundary
+// Gamma / Sigma^<> (8(c-2)).  All batched over energies: blockIdx.y = energy.
+#include "common.cuh"
+#include "kernels.cuh"
+
+namespace {
+
+__global__ void combine_kernel(CombineArgs a) {
+    const int e = blockIdx.y;
+    if (a.skip && a.skip[e]) return;
+    const int b = a.b;
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= b * b) return;
+    const int r = idx / b, c = idx % b;
+    const int src = a.dagger ? c * b + r : idx;
+    cplx v = cmake(0.0, 0.0);
+    if (a.use_z) {
+        cplx z = cmake(a.energy[e], a.eta);
+        if (a.S) {
+            cplx s = a.S[src];
+            if (a.dagger) s = cconj(s);
+            v = cmul(z, s);
+        } else if (a.s_identity && r == c) {
+            v = z;
+        }
+    }
+    if (a.H) {
+        cplx h = a.H[src];
+        if (a.dagger) h = cconj(h);
+        v = csub(v, h);
+    }
+    for (int t = 0; t < 3; t++) {
+        if (a.blk[t]) {
+            cplx x = a.blk[t][(size_t)e * a.sblk[t] + idx];
+            v.x = fma(a.coef, x.x, v.x); v.y = fma(a.coef, x.y, v.y);
+        }
+    }
+    if (a.scalar && r == c) {
+        cplx x = a.scalar[e];
+        v.x = fma(a.coef, x.x, v.x); v.y = fma(a.coef, x.y, v.y);
+    }
+    a.out[(size_t)e * a.sout + idx] = v;
+}
+
+// C = Z + sign * (V - V^H)
+__global__ void antiherm_add_kernel(int b, cplx* C, long long sC, const cplx* Z, long long sZ,
+                                    const cplx* V, long long sV, double sign) {
+    const int e = blockIdx.y;
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= b * b) return;
+    const int r = idx / b, c = idx % b;
+    cplx v = V[(size_t)e * sV + idx];
+    cplx vt = V[(size_t)e * sV + c * b + r];
+    cplx z = Z ? Z[(size_t)e * sZ + idx] : cmake(0.0, 0.0);
+    C[(size_t)e * sC + idx] = cmake(z.x + sign * (v.x - vt.x), z.y + sign * (v.y + vt.y));
+}
+
+__global__ void sub_kernel(int b, cplx* C, long long sC, const cplx* A, long long sA, const cplx* B, long long sB) {
+    const int e = blockIdx.y;
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= b * b) return;
+    C[(size_t)e * sC + idx] = csub(A[(size_t)e * sA + idx], B[(size_t)e * sB + idx]);
+}
+
+__global__ void copy_kernel(size_t n, cplx* dst, long long sd, const cplx* src, long long ss, const int* skip) {
+    const int e = blockIdx.y;
+    if (skip && skip[e]) return;
+    size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= n) return;
+    dst[(size_t)e * sd + idx] = src[(size_t)e * ss + idx];
+}
+
+__global__ void fill_int_kernel(int* p, int n, int v) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) p[i] = v;
+}
+__global__ void max_int_kernel(int* dst, const int* src, int n) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) { int a = dst[i], s = src[i]; if (a == 0) dst[i] = s; }
+}
+
+// a_s -= (side ? ugl : lgu) ; a_b -= ugl + lgu
+__global__ void sr_update_kernel(int b, int side, cplx* a_s, cplx* a_b, const cplx* lgu, const cplx* ugl,
+                                 const int* skip) {
+    const int e = blockIdx.y;
+    if (skip && skip[e]) return;
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= b * b) return;
+    size_t o = (size_t)e * b * b + idx;
+    cplx x = lgu[o], y = ugl[o];
+    cplx s = a_s[o], d = a_b[o];
+    cplx t = side ? y : x;
+    a_s[o] = csub(s, t);
+    a_b[o] = cmake(d.x - x.x - y.x, d.y - x.y - y.y);
+}
+
+// ||u||_F + ||l||_F per energy.  mode 0: ref[e] = value.  mode 1: convergence test (reading R3).
+__global__ void sr_norm_kernel(int b, const cplx* u, const cplx* l, double* ref, double tol, int* done,
+                               int* iters, int it, int mode) {
+    const int e = blockIdx.x;
+    if (mode == 1 && done[e]) return;
+    __shared__ double su[32], sl[32];
+    double au = 0.0, al = 0.0;
+    const cplx* pu = u + (size_t)e * b * b;
+    const cplx* pl = l + (size_t)e * b * b;
+    for (int i = threadIdx.x; i < b * b; i += blockDim.x) {
+        cplx x = pu[i], y = pl[i];
+        au += x.x * x.x + x.y * x.y;
+        al += y.x * y.x + y.y * y.y;
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        au += __shfl_down_sync(0xffffffffu, au, o);
+        al += __shfl_down_sync(0xffffffffu, al, o);
+    }
+    if ((threadIdx.x & 31) == 0) { su[threadIdx.x >> 5] = au; sl[threadIdx.x >> 5] = al; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        au = 0.0; al = 0.0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); w++) { au += su[w]; al += sl[w]; }
+        double v = sqrt(au) + sqrt(al);
+        if (mode == 0) ref[e] = v;
+        else {
+            iters[e] = it + 1;
+            if (v <= tol * ref[e]) done[e] = 1;
+        }
+    }
+}
+
+// Gamma = i (Sigma - Sigma^H); f = fermi(E); Sigma^< = i f Gamma; Sigma^> = -i (1-f) Gamma
+__global__ void obc_finalize_kernel(int b, const cplx* sigma, const double* energy, double mu, double kT,
+                                    cplx* gamma, cplx* sl, cplx* sg, double* fermi) {
+    const int e = blockIdx.y;
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    double x = (energy[e] - mu) / kT, f;
+    if (x > 0) { double ex = exp(-x); f = ex / (1.0 + ex); } else { f = 1.0 / (1.0 + exp(x)); }
+    if (idx == 0 && fermi) fermi[e] = f;
+    if (idx >= b * b) return;
+    const int r = idx / b, c = idx % b;
+    size_t o = (size_t)e * b * b;
+    cplx s = sigma[o + idx], st = sigma[o + c * b + r];
+    // Sigma - Sigma^H = (s.x - st.x) + i (s.y + st.y) ;  times i
+    cplx g = cmake(-(s.y + st.y), s.x - st.x);
+    if (gamma) gamma[o + idx] = g;
+    if (sl) sl[o + idx] = cmake(-f * g.y, f * g.x);                       // i f g
+    if (sg) sg[o + idx] = cmake((1.0 - f) * g.y, -(1.0 - f) * g.x);       // -i (1-f) g
+}
+
+__global__ void obc_status_kernel(int ne, const int* done, const int* sing, int* status) {
+    int e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e < ne) status[e] = sing[e] ? sing[e] : (done[e] ? 0 : -1);
+}
+
+inline dim3 grid2(int b, int batch) { return dim3((b * b + 255) / 256, batch); }
+
+}  // namespace
+
+int ew_combine(negf_ctx* ctx, const CombineArgs& a, int batch) {
+    combine_kernel<<<grid2(a.b, batch), 256, 0, ctx->stream>>>(a);
+    NEGF_LAUNCH_CHECK(ctx);
+    return NEGF_OK;
+}
+int ew_antiherm_add(negf_ctx* ctx, int b, int batch, cplx* C, long long sC, const cplx* Z, long long sZ,
+                    const cplx* V, long long sV, double sign) {
+    antiherm_add_kernel<<<grid2(b, batch), 256, 0, ctx->stream>>>(b, C, sC, Z, sZ, V, sV, sign);
+    NEGF_LAUNCH_CHECK(ctx);
+    return NEGF_OK;
+}
+int ew_sub(negf_ctx* ctx, int b, int batch, cplx* C, long long sC, const cplx* A, long long sA,
+           const cplx* B, long long sB) {
+    sub_kernel<<<grid2(b, batch), 256, 0, ctx->stream>>>(b, C, sC, A, sA, B, sB);
+    NEGF_LAUNCH_CHECK(ctx);
+    return NEGF_OK;
+}
+int ew_copy(negf_ctx* ctx, size_t n, int batch, cplx* dst, long long sd, const cplx* src, long long ss,
+            const int* skip) {
+    copy_kernel<<<dim3((unsigned)((n + 255) / 256), batch), 256, 0, ctx->stream>>>(n, dst, sd, src, ss, skip);
+    NEGF_LAUNCH_CHECK(ctx);
+    return NEGF_OK;
+}
+int ew_fill_int(negf_ctx* ctx, int* p, int n, int v) {
+    fill_int_kernel<<<(n + 255) / 256, 256, 0, ctx->stream>>>(p, n, v);
+    NEGF_LAUNCH_CHECK(ctx);
+    return NEGF_OK;
+}
+int ew_max_int(negf_ctx* ctx, int* dst, const int* src, int n) {
+    max_int_kernel<<<(n + 255) / 256, 256, 0, ctx->stream>>>(dst, src, n);
+    NEGF_LAUNCH_CHECK(ctx);
+    return NEGF_OK;
+}
+int ew_sr_update(negf_ctx* ctx, int b, int batch, int side, cplx* a_s, cplx* a_b, const cplx* lgu,
+                 const cplx* ugl, const int* skip) {
+    sr_update_kernel<<<grid2(b, batch), 256, 0, ctx->stream>>>(b, side, a_s, a_b, lgu, ugl, skip);
+    NEGF_LAUNCH_CHECK(ctx);
+    return NEGF_OK;
+}
+int ew_sr_norm(negf_ctx* ctx, int b, int batch, const cplx* u, const cplx* l, double* ref, double tol,
+               int* done, int* iters, int it, int mode) {
+    sr_norm_kernel<<<batch, 256, 0, ctx->stream>>>(b, u, l, ref, tol, done, iters, it, mode);
+    NEGF_LAUNCH_CHECK(ctx);
+    return NEGF_OK;
+}
+int ew_obc_finalize(negf_ctx* ctx, int b, int batch, const cplx* sigma, const double* energy, double mu,
+                    double kT, cplx* gamma, cplx* sl, cplx* sg, double* fermi) {
+    obc_finalize_kernel<<<grid2(b, batch), 256, 0, ctx->stream>>>(b, sigma, energy, mu, kT, gamma, sl, sg, fermi);
+    NEGF_LAUNCH_CHECK(ctx);
+    return NEGF_OK;
+}
+int ew_obc_status(negf_ctx* ctx, int ne, const int* done, const int* sing, int* status) {
+    obc_status_kernel<<<(ne + 255) / 256, 256, 0, ctx->stream>>>(ne, done, sing, status);
+    NEGF_LAUNCH_CHECK(ctx);
+    return NEGF_OK;
+}

@@ -1,0 +1,223 @@
+// S7 (readings R11-R13): density, LDOS, transmission, bond and contact currents
+// from the selected blocks.  O(n b^2) reductions plus two b^3 products
+// for T(E).  Deterministic: no atomics, fixed reduction order.
+#include "common.cuh"
+#include "kernels.cuh"
+#include "workspace.cuh"
+
+namespace {
+
+__device__ __forceinline__ double block_sum(double v) {
+    __shared__ double sh[32];
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    __syncthreads();
+    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = v;
+    __syncthreads();
+    double t = 0.0;
+    if (threadIdx.x < 32) {
+        t = threadIdx.x < (blockDim.x >> 5) ? sh[threadIdx.x] : 0.0;
+        for (int o = 16; o > 0; o >>= 1) t += __shfl_down_sync(0xffffffffu, t, o);
+    }
+    return t;   // valid in thread 0
+}
+
+// LDOS_i(E) = -(1/pi) Im Tr[(G^R S)_ii];  grid (n, NE)
+__global__ void ldos_kernel(int n, int b, const cplx* GRd, const cplx* GRu, const cplx* GRl,
+                            const cplx* Sd, const cplx* Su, double* ldos) {
+    const int i = blockIdx.x, e = blockIdx.y;
+    const size_t bb = (size_t)b * b;
+    const cplx* G = GRd + ((size_t)e * n + i) * bb;
+    double acc = 0.0;   // imaginary part of the trace
+    if (!Sd) {
+        for (int r = threadIdx.x; r < b; r += blockDim.x) acc += G[(size_t)r * b + r].y;
+    } else {
+        const cplx* S = Sd + (size_t)i * bb;
+        for (int idx = threadIdx.x; idx < (int)bb; idx += blockDim.x) {
+            int r = idx / b, c = idx % b;
+            // G[r][c] * S[c][r], S Hermitian-stored as given: read S[c][r] directly
+            cplx g = G[idx], s = S[(size_t)c * b + r];
+            acc += g.x * s.y + g.y * s.x;
+            if (i + 1 < n) {   // G_{i,i+1}[r][c] * S_{i+1,i}[c][r], S_{i+1,i} = S_up[i]^H
+                cplx gu = GRu[((size_t)e * (n - 1) + i) * bb + idx], su = Su[(size_t)i * bb + idx];
+                acc += -gu.x * su.y + gu.y * su.x;
+            }
+            if (i > 0) {       // G_{i,i-1}[r][c] * S_{i-1,i}[c][r]
+                cplx gl = GRl[((size_t)e * (n - 1) + i - 1) * bb + idx], su = Su[(size_t)(i - 1) * bb + (size_t)c * b + r];
+                acc += gl.x * su.y + gl.y * su.x;
+            }
+        }
+    }
+    double t = block_sum(acc);
+    if (threadIdx.x == 0) ldos[(size_t)e * n + i] = -t / 3.14159265358979323846;
+}
+
+// density_k = sum_E w_E Im[(G^< S)_kk] / (2 pi); one warp per k; terms with row-contiguous reads.
+__global__ void density_rows_kernel(int n, int b, int ne, const cplx* GLd, const cplx* GLu, const cplx* Sd,
+                                    const cplx* Su, const double* w, double* density) {
+    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (warp >= n * b) return;
+    const int i = warp / b, r = warp % b;
+    const size_t bb = (size_t)b * b;
+    double acc = 0.0;
+    for (int e = 0; e < ne; e++) {
+        double im = 0.0;
+        const cplx* G = GLd + ((size_t)e * n + i) * bb + (size_t)r * b;
+        if (!Sd) {
+            if (lane == 0) im = G[r].y;
+        } else {
+            const cplx* S = Sd + (size_t)i * bb + (size_t)r * b;    // S_ii[c][r] = conj(S_ii[r][c])
+            for (int c = lane; c < b; c += 32) { cplx g = G[c], s = S[c]; im += -g.x * s.y + g.y * s.x; }
+            if (i + 1 < n) {   // G^<_{i,i+1}[r][c] * conj(S_up[i][r][c])
+                const cplx* Gu = GLu + ((size_t)e * (n - 1) + i) * bb + (size_t)r * b;
+                const cplx* S2 = Su + (size_t)i * bb + (size_t)r * b;
+                for (int c = lane; c < b; c += 32) { cplx g = Gu[c], s = S2[c]; im += -g.x * s.y + g.y * s.x; }
+            }
+        }
+        acc += w[e] * im;
+    }
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, o);
+    if (lane == 0) density[warp] = acc / (2.0 * 3.14159265358979323846);
+}
+// third term (S != I, i > 0): sum_c G^<_{i,i-1}[r][c] S_{i-1,i}[c][r], G^<_{i,i-1}[r][c] = -conj(GLu[i-1][c][r]);
+// thread per r walks down column r of both arrays (coalesced across threads).
+__global__ void density_cols_kernel(int n, int b, int ne, const cplx* GLu, const cplx* Su, const double* w,
+                                    double* density) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n * b) return;
+    const int i = k / b, r = k % b;
+    if (i == 0) return;
+    const size_t bb = (size_t)b * b;
+    double acc = 0.0;
+    const cplx* S = Su + (size_t)(i - 1) * bb;
+    for (int e = 0; e < ne; e++) {
+        const cplx* G = GLu + ((size_t)e * (n - 1) + i - 1) * bb;
+        double im = 0.0;
+        for (int c = 0; c < b; c++) {
+            cplx g = G[(size_t)c * b + r], s = S[(size_t)c * b + r];
+            // (-conj(g)) * s = -(g.x s.x + g.y s.y) + i (-(g.x s.y) + g.y s.x)
+            im += -g.x * s.y + g.y * s.x;
+        }
+        acc += w[e] * im;
+    }
+    density[k] += acc / (2.0 * 3.14159265358979323846);
+}
+
+// out[e] = scale * Re sum_{r,c} A[e][r][c] * conj(B[e][r][c]); grid (items, NE)
+__global__ void dot_conj_kernel(int b, const cplx* A, long long sA, const cplx* B, long long sB, double scale,
+                                double* out, int out_stride, int items_stride_a, int items_stride_b) {
+    const int it = blockIdx.x, e = blockIdx.y;
+    const cplx* a = A + (size_t)e * sA + (size_t)it * items_stride_a;
+    const cplx* bp = B + (size_t)e * sB + (size_t)it * items_stride_b;
+    double acc = 0.0;
+    for (int idx = threadIdx.x; idx < b * b; idx += blockDim.x) { cplx x = a[idx], y = bp[idx]; acc += x.x * y.x + x.y * y.y; }
+    double t = block_sum(acc);
+    if (threadIdx.x == 0) out[(size_t)e * out_stride + it] = scale * t;
+}
+
+// J_i(E) = 2 Re Tr[(H_up[i] - E S_up[i]) G^<_{i+1,i}] = -2 Re sum (H - E S)[r][c] conj(GLu[r][c]); grid (n-1, NE)
+__global__ void bond_current_kernel(int n, int b, const cplx* Hu, const cplx* Su, const double* energy,
+                                    const cplx* GLu, double* out) {
+    const int i = blockIdx.x, e = blockIdx.y;
+    const size_t bb = (size_t)b * b;
+    const double E = energy[e];
+    const cplx* H = Hu + (size_t)i * bb;
+    const cplx* S = Su ? Su + (size_t)i * bb : nullptr;
+    const cplx* G = GLu + ((size_t)e * (n - 1) + i) * bb;
+    double acc = 0.0;
+    for (int idx = threadIdx.x; idx < (int)bb; idx += blockDim.x) {
+        cplx h = H[idx];
+        if (S) { cplx s = S[idx]; h.x -= E * s.x; h.y -= E * s.y; }
+        cplx g = G[idx];
+        acc += h.x * g.x + h.y * g.y;
+    }
+    double t = block_sum(acc);
+    if (threadIdx.x == 0) out[(size_t)e * (n - 1) + i] = -2.0 * t;
+}
+
+// I_c(E) = Re Tr[Sigma^<_c G^>_cc - Sigma^>_c G^<_cc]; grid (2, NE)
+__global__ void contact_current_kernel(int n, int b, const cplx* sLl, const cplx* sLg, const cplx* sRl,
+                                       const cplx* sRg, const cplx* GLd, const cplx* GGd, double* out) {
+    const int c = blockIdx.x, e = blockIdx.y;
+    const size_t bb = (size_t)b * b;
+    const cplx* sl = (c == 0 ? sLl : sRl) + (size_t)e * bb;
+    const cplx* sg = (c == 0 ? sLg : sRg) + (size_t)e * bb;
+    const int blk = c == 0 ? 0 : n - 1;
+    const cplx* gl = GLd + ((size_t)e * n + blk) * bb;
+    const cplx* gg = GGd + ((size_t)e * n + blk) * bb;
+    double acc = 0.0;
+    for (int idx = threadIdx.x; idx < (int)bb; idx += blockDim.x) {
+        int r = idx / b, k = idx % b;
+        cplx a = sl[idx], x = gg[(size_t)k * b + r];
+        cplx d = sg[idx], y = gl[(size_t)k * b + r];
+        acc += (a.x * x.x - a.y * x.y) - (d.x * y.x - d.y * y.y);
+    }
+    double t = block_sum(acc);
+    if (threadIdx.x == 0) out[(size_t)e * 2 + c] = t;
+}
+
+}  // namespace
+
+extern "C" int negf_observables(negf_ctx* ctx, const negf_problem* p,
+                                const negf_c128* GR_diag, const negf_c128* GR_upper, const negf_c128* GR_lower,
+                                const negf_c128* GR_corner, const negf_c128* GL_diag, const negf_c128* GL_upper,
+                                const negf_c128* GG_diag, const negf_c128* gamma_L, const negf_c128* gamma_R,
+                                const negf_c128* sigma_lesser_L, const negf_c128* sigma_greater_L,
+                                const negf_c128* sigma_lesser_R, const negf_c128* sigma_greater_R,
+                                const double* weights, double* density, double* ldos, double* transmission,
+                                double* bond_current, double* contact_current) {
+    if (!ctx || !p || p->n_blocks < 1 || p->block_size < 1 || p->n_energy < 1) return NEGF_EINVAL;
+    const int n = p->n_blocks, b = p->block_size, ne = p->n_energy;
+    const size_t bb = (size_t)b * b;
+    const bool hasS = p->S_diag != nullptr;
+    if (ne > 65535) return NEGF_EUNSUPPORTED;
+    if (ldos) {
+        if (!GR_diag || (hasS && n > 1 && (!GR_upper || !GR_lower || !p->S_upper))) return NEGF_EINVAL;
+        ldos_kernel<<<dim3(n, ne), 256, 0, ctx->stream>>>(n, b, (const cplx*)GR_diag, (const cplx*)GR_upper,
+                                                          (const cplx*)GR_lower, (const cplx*)p->S_diag,
+                                                          (const cplx*)p->S_upper, ldos);
+        NEGF_LAUNCH_CHECK(ctx);
+    }
+    if (density) {
+        if (!GL_diag || !weights || (hasS && n > 1 && (!GL_upper || !p->S_upper))) return NEGF_EINVAL;
+        long long threads = (long long)n * b * 32;
+        density_rows_kernel<<<(unsigned)((threads + 255) / 256), 256, 0, ctx->stream>>>(
+            n, b, ne, (const cplx*)GL_diag, (const cplx*)GL_upper, (const cplx*)p->S_diag, (const cplx*)p->S_upper,
+            weights, density);
+        NEGF_LAUNCH_CHECK(ctx);
+        if (hasS && n > 1) {
+            density_cols_kernel<<<(n * b + 127) / 128, 128, 0, ctx->stream>>>(n, b, ne, (const cplx*)GL_upper,
+                                                                            (const cplx*)p->S_upper, weights, density);
+            NEGF_LAUNCH_CHECK(ctx);
+        }
+    }
+    if (transmission) {
+        if (!GR_corner || !gamma_L || !gamma_R) return NEGF_EINVAL;
+        if (!ctx->ws) return NEGF_ENOWORKSPACE;
+        Workspace W = carve_workspace(ctx->ws, n, b, ne);
+        if (W.bytes > ctx->ws_bytes) return NEGF_ENOWORKSPACE;
+        const cplx one = cmake(1.0, 0.0), zero = cmake(0.0, 0.0);
+        // T = Re Tr[Gamma_L G Gamma_R G^H] = Re sum (Gamma_L G Gamma_R)[r][c] conj(G[r][c])
+        NEGF_TRY(zgemm_bb(ctx, 0, 0, b, one, (const cplx*)gamma_L, bb, (const cplx*)GR_corner, bb, zero, nullptr, 0,
+                          W.T[9], bb, ne, nullptr));
+        NEGF_TRY(zgemm_bb(ctx, 0, 0, b, one, W.T[9], bb, (const cplx*)gamma_R, bb, zero, nullptr, 0, W.T[10], bb, ne, nullptr));
+        dot_conj_kernel<<<dim3(1, ne), 256, 0, ctx->stream>>>(b, W.T[10], bb, (const cplx*)GR_corner, bb, 1.0,
+                                                             transmission, 1, 0, 0);
+        NEGF_LAUNCH_CHECK(ctx);
+    }
+    if (bond_current && n > 1) {
+        if (!GL_upper || !p->H_upper) return NEGF_EINVAL;
+        bond_current_kernel<<<dim3(n - 1, ne), 256, 0, ctx->stream>>>(n, b, (const cplx*)p->H_upper,
+                                                                      (const cplx*)p->S_upper, p->energy,
+                                                                      (const cplx*)GL_upper, bond_current);
+        NEGF_LAUNCH_CHECK(ctx);
+    }
+    if (contact_current) {
+        if (!GL_diag || !GG_diag || !sigma_lesser_L || !sigma_greater_L || !sigma_lesser_R || !sigma_greater_R)
+            return NEGF_EINVAL;
+        contact_current_kernel<<<dim3(2, ne), 256, 0, ctx->stream>>>(
+            n, b, (const cplx*)sigma_lesser_L, (const cplx*)sigma_greater_L, (const cplx*)sigma_lesser_R,
+            (const cplx*)sigma_greater_R, (const cplx*)GL_diag, (const cplx*)GG_diag, contact_current);
+        NEGF_LAUNCH_CHECK(ctx);
+    }
+    return NEGF_OK;
+}

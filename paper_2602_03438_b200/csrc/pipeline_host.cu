@@ -1,0 +1,186 @@
+// negf_pipeline_host: the whole S1-S7 path with HOST buffers (include/negf.h) - what a user
+// without device arrays calls, and what bench.py times as the end-to-end number: host->device
+// copies of all inputs, the four device calls, device->host copies of all requested outputs.
+#include "common.cuh"
+#include "workspace.cuh"
+
+namespace {
+
+struct Bump {
+    unsigned char* base; size_t off;
+    void* take(size_t bytes) { void* r = base ? base + off : nullptr; off += align_up(bytes, 256); return r; }
+};
+
+struct Layout {
+    cplx *Hd, *Hu, *Sd, *Su; double *energy, *weights;
+    cplx *sig[3][4];                 // [r,l,g][scalar, diag, upper, lower]
+    cplx *ob[2][4];                  // [side][sigma_r, gamma, sl, sg]
+    int *iters[2], *status[2];
+    cplx *GRd, *GRu, *GRl, *corner, *GLd, *GLu, *GGd, *GGu;
+    double *density, *ldos, *trans, *bond, *contact;
+    int *info_r, *info_x;
+    void* ws; size_t ws_bytes;
+    size_t total;
+};
+
+Layout make_layout(void* base, int n, int b, int ne, int kind_max, bool hasS, bool want_greater) {
+    Layout L = {};
+    Bump B{(unsigned char*)base, 0};
+    const size_t bb = (size_t)b * b * sizeof(cplx);
+    const int m = n > 1 ? n - 1 : 0;
+    L.Hd = (cplx*)B.take(bb * n); L.Hu = (cplx*)B.take(bb * m);
+    if (hasS) { L.Sd = (cplx*)B.take(bb * n); L.Su = (cplx*)B.take(bb * m); }
+    L.energy = (double*)B.take(sizeof(double) * ne); L.weights = (double*)B.take(sizeof(double) * ne);
+    for (int f = 0; f < 3; f++) {
+        if (kind_max == NEGF_SIGMA_SCALAR) L.sig[f][0] = (cplx*)B.take(sizeof(cplx) * ne);
+        if (kind_max == NEGF_SIGMA_BT) {
+            L.sig[f][1] = (cplx*)B.take(bb * n * ne); L.sig[f][2] = (cplx*)B.take(bb * m * ne);
+            if (f == 0) L.sig[f][3] = (cplx*)B.take(bb * m * ne);
+        }
+    }
+    for (int s = 0; s < 2; s++) {
+        for (int k = 0; k < 4; k++) L.ob[s][k] = (cplx*)B.take(bb * ne);
+        L.iters[s] = (int*)B.take(sizeof(int) * ne); L.status[s] = (int*)B.take(sizeof(int) * ne);
+    }
+    L.GRd = (cplx*)B.take(bb * n * ne); L.GRu = (cplx*)B.take(bb * m * ne); L.GRl = (cplx*)B.take(bb * m * ne);
+    L.corner = (cplx*)B.take(bb * ne);
+    L.GLd = (cplx*)B.take(bb * n * ne); L.GLu = (cplx*)B.take(bb * m * ne);
+    if (want_greater) { L.GGd = (cplx*)B.take(bb * n * ne); L.GGu = (cplx*)B.take(bb * m * ne); }
+    L.density = (double*)B.take(sizeof(double) * n * b); L.ldos = (double*)B.take(sizeof(double) * ne * n);
+    L.trans = (double*)B.take(sizeof(double) * ne); L.bond = (double*)B.take(sizeof(double) * ne * (m > 0 ? m : 1));
+    L.contact = (double*)B.take(sizeof(double) * ne * 2);
+    L.info_r = (int*)B.take(sizeof(int) * ne); L.info_x = (int*)B.take(sizeof(int) * ne);
+    Workspace W = carve_workspace(nullptr, n, b, ne);
+    L.ws_bytes = W.bytes; L.ws = B.take(W.bytes);
+    L.total = B.off;
+    return L;
+}
+
+__global__ void merge_info_kernel(int ne, const int* a, const int* b, const int* c, const int* d, int* out) {
+    int e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= ne) return;
+    int v = a[e]; if (!v) v = b[e]; if (!v) v = c[e]; if (!v) v = d[e];
+    out[e] = v;
+}
+
+}  // namespace
+
+extern "C" int negf_pipeline_host_bytes(const negf_problem* p, int kind_max, int want_greater, size_t* bytes) {
+    if (!p || !bytes || p->n_blocks < 1 || p->block_size < 1 || p->n_energy < 1) return NEGF_EINVAL;
+    Layout L = make_layout(nullptr, p->n_blocks, p->block_size, p->n_energy, kind_max, true, want_greater != 0);
+    *bytes = L.total;
+    return NEGF_OK;
+}
+
+extern "C" int negf_pipeline_host(negf_ctx* ctx, const negf_problem* hp, const negf_sigma* hsr,
+                                  const negf_sigma* hsl, const negf_sigma* hsg, const double* hweights,
+                                  double mu_L, double mu_R, double kT, double tol, int max_iter,
+                                  void* dev_scratch, size_t dev_scratch_bytes, const negf_host_outputs* out,
+                                  size_t* h2d_bytes, size_t* d2h_bytes) {
+    if (!ctx || !hp || !out || !dev_scratch || !hweights) return NEGF_EINVAL;
+    const int n = hp->n_blocks, b = hp->block_size, ne = hp->n_energy;
+    if (n < 2 || b < 1 || ne < 1 || !hp->H_diag || !hp->H_upper || !hp->energy) return NEGF_EINVAL;
+    const bool hasS = hp->S_diag != nullptr;
+    const bool want_g = hsg != nullptr;
+    int kind = NEGF_SIGMA_NONE;
+    const negf_sigma* hs[3] = {hsr, hsl, hsg};
+    for (int f = 0; f < 3; f++) if (hs[f] && hs[f]->kind > kind) kind = hs[f]->kind;
+    Layout L = make_layout(dev_scratch, n, b, ne, kind, hasS, want_g);
+    if (L.total > dev_scratch_bytes) return NEGF_ENOWORKSPACE;
+    const size_t bb = (size_t)b * b * sizeof(cplx);
+    const int m = n - 1;
+    size_t up = 0, down = 0;
+    cudaStream_t st = ctx->stream;
+    auto H2D = [&](void* d, const void* h, size_t bytes) -> cudaError_t {
+        up += bytes; return cudaMemcpyAsync(d, h, bytes, cudaMemcpyHostToDevice, st);
+    };
+    auto D2H = [&](void* h, const void* d, size_t bytes) -> cudaError_t {
+        if (!h) return cudaSuccess;
+        down += bytes; return cudaMemcpyAsync(h, d, bytes, cudaMemcpyDeviceToHost, st);
+    };
+    NEGF_CUDA_CHECK(ctx, H2D(L.Hd, hp->H_diag, bb * n));
+    NEGF_CUDA_CHECK(ctx, H2D(L.Hu, hp->H_upper, bb * m));
+    if (hasS) {
+        if (!hp->S_upper) return NEGF_EINVAL;
+        NEGF_CUDA_CHECK(ctx, H2D(L.Sd, hp->S_diag, bb * n));
+        NEGF_CUDA_CHECK(ctx, H2D(L.Su, hp->S_upper, bb * m));
+    }
+    NEGF_CUDA_CHECK(ctx, H2D(L.energy, hp->energy, sizeof(double) * ne));
+    NEGF_CUDA_CHECK(ctx, H2D(L.weights, hweights, sizeof(double) * ne));
+    negf_sigma ds[3];
+    for (int f = 0; f < 3; f++) {
+        ds[f] = negf_sigma{};
+        if (!hs[f]) continue;
+        ds[f].kind = hs[f]->kind;
+        if (hs[f]->kind == NEGF_SIGMA_SCALAR) {
+            NEGF_CUDA_CHECK(ctx, H2D(L.sig[f][0], hs[f]->scalar, sizeof(cplx) * ne));
+            ds[f].scalar = (negf_c128*)L.sig[f][0];
+        } else if (hs[f]->kind == NEGF_SIGMA_BT) {
+            NEGF_CUDA_CHECK(ctx, H2D(L.sig[f][1], hs[f]->diag, bb * n * ne));
+            NEGF_CUDA_CHECK(ctx, H2D(L.sig[f][2], hs[f]->upper, bb * m * ne));
+            ds[f].diag = (negf_c128*)L.sig[f][1]; ds[f].upper = (negf_c128*)L.sig[f][2];
+            if (f == 0) {
+                NEGF_CUDA_CHECK(ctx, H2D(L.sig[f][3], hs[f]->lower, bb * m * ne));
+                ds[f].lower = (negf_c128*)L.sig[f][3];
+            }
+        }
+    }
+    negf_problem dp = *hp;
+    dp.H_diag = (negf_c128*)L.Hd; dp.H_upper = (negf_c128*)L.Hu;
+    dp.S_diag = hasS ? (negf_c128*)L.Sd : nullptr; dp.S_upper = hasS ? (negf_c128*)L.Su : nullptr;
+    dp.energy = L.energy;
+
+    void* old_ws = ctx->ws; size_t old_bytes = ctx->ws_bytes;
+    ctx->ws = L.ws; ctx->ws_bytes = L.ws_bytes; ctx->sweep_valid = false;
+    int rc = NEGF_OK;
+    do {
+        const double mus[2] = {mu_L, mu_R};
+        for (int s = 0; s < 2 && rc == NEGF_OK; s++)
+            rc = negf_obc_decimate(ctx, &dp, nullptr, s, mus[s], kT, tol, max_iter, (negf_c128*)L.ob[s][0],
+                                   (negf_c128*)L.ob[s][1], (negf_c128*)L.ob[s][2], (negf_c128*)L.ob[s][3],
+                                   nullptr, nullptr, L.iters[s], L.status[s]);
+        if (rc) break;
+        ds[0].left = (negf_c128*)L.ob[0][0]; ds[0].right = (negf_c128*)L.ob[1][0];
+        ds[1].left = (negf_c128*)L.ob[0][2]; ds[1].right = (negf_c128*)L.ob[1][2];
+        ds[2].left = (negf_c128*)L.ob[0][3]; ds[2].right = (negf_c128*)L.ob[1][3];
+        rc = negf_rgf_retarded(ctx, &dp, &ds[0], (negf_c128*)L.GRd, (negf_c128*)L.GRu, (negf_c128*)L.GRl,
+                               (negf_c128*)L.corner, NEGF_KEEP_SWEEP, L.info_r);
+        if (rc) break;
+        rc = negf_rgf_lesser_greater(ctx, &dp, &ds[0], &ds[1], want_g ? &ds[2] : nullptr, (negf_c128*)L.GRd,
+                                     (negf_c128*)L.GLd, (negf_c128*)L.GLu, (negf_c128*)L.GGd, (negf_c128*)L.GGu,
+                                     L.info_x);
+        if (rc) break;
+        rc = negf_observables(ctx, &dp, (negf_c128*)L.GRd, (negf_c128*)L.GRu, (negf_c128*)L.GRl, (negf_c128*)L.corner,
+                              (negf_c128*)L.GLd, (negf_c128*)L.GLu, (negf_c128*)L.GGd,
+                              (negf_c128*)L.ob[0][1], (negf_c128*)L.ob[1][1],
+                              (negf_c128*)L.ob[0][2], (negf_c128*)L.ob[0][3], (negf_c128*)L.ob[1][2], (negf_c128*)L.ob[1][3],
+                              L.weights, out->density ? L.density : nullptr, out->ldos ? L.ldos : nullptr,
+                              out->transmission ? L.trans : nullptr, out->bond_current ? L.bond : nullptr,
+                              (out->contact_current && want_g) ? L.contact : nullptr);
+    } while (0);
+    ctx->ws = old_ws; ctx->ws_bytes = old_bytes; ctx->sweep_valid = false;
+    if (rc) return rc;
+    if (out->info) {
+        merge_info_kernel<<<(ne + 255) / 256, 256, 0, st>>>(ne, L.status[0], L.status[1], L.info_r, L.info_x, L.info_x);
+        NEGF_LAUNCH_CHECK(ctx);
+    }
+    NEGF_CUDA_CHECK(ctx, D2H(out->GR_diag, L.GRd, bb * n * ne));
+    NEGF_CUDA_CHECK(ctx, D2H(out->GR_upper, L.GRu, bb * m * ne));
+    NEGF_CUDA_CHECK(ctx, D2H(out->GR_lower, L.GRl, bb * m * ne));
+    NEGF_CUDA_CHECK(ctx, D2H(out->GL_diag, L.GLd, bb * n * ne));
+    NEGF_CUDA_CHECK(ctx, D2H(out->GL_upper, L.GLu, bb * m * ne));
+    if (want_g) {
+        NEGF_CUDA_CHECK(ctx, D2H(out->GG_diag, L.GGd, bb * n * ne));
+        NEGF_CUDA_CHECK(ctx, D2H(out->GG_upper, L.GGu, bb * m * ne));
+    }
+    NEGF_CUDA_CHECK(ctx, D2H(out->density, L.density, sizeof(double) * n * b));
+    NEGF_CUDA_CHECK(ctx, D2H(out->ldos, L.ldos, sizeof(double) * ne * n));
+    NEGF_CUDA_CHECK(ctx, D2H(out->transmission, L.trans, sizeof(double) * ne));
+    NEGF_CUDA_CHECK(ctx, D2H(out->bond_current, L.bond, sizeof(double) * ne * m));
+    if (want_g) NEGF_CUDA_CHECK(ctx, D2H(out->contact_current, L.contact, sizeof(double) * ne * 2));
+    NEGF_CUDA_CHECK(ctx, D2H(out->info, L.info_x, sizeof(int) * ne));
+    NEGF_CUDA_CHECK(ctx, cudaStreamSynchronize(st));
+    if (h2d_bytes) *h2d_bytes = up;
+    if (d2h_bytes) *d2h_bytes = down;
+    return NEGF_OK;
+}

@@ -1,0 +1,38 @@
+// Carve-up of the caller-owned workspace (negf_set_workspace), shared by all calls.
+#pragma once
+#include "common.cuh"
+
+constexpr int NEGF_NSCRATCH = 13;   // decimation needs 13 blocks per energy, the sweeps 9
+
+struct Workspace {
+    cplx* g;        // [NE][n][b][b]    left-connected g_i        (retained sweep state)
+    cplx* X;        // [NE][n-1][b][b]  X_i = g_i A_{i,i+1}       (retained)
+    cplx* Y;        // [NE][n-1][b][b]  Y_i = A_{i+1,i} g_i       (retained)
+    cplx* gx;       // [NE][n][b][b]    left-connected g^x_i (one of </> at a time)
+    cplx* T[NEGF_NSCRATCH];   // [NE][b][b] each
+    void* inv;      // zinv workspace
+    double* ref;    // [NE]
+    int* done;      // [NE]
+    int* sing;      // [NE]
+    int* tmpinfo;   // [NE]
+    size_t bytes;
+};
+
+inline Workspace carve_workspace(void* base, int n, int b, int ne) {
+    Workspace w;
+    unsigned char* p = (unsigned char*)base;
+    const size_t blk = (size_t)b * b * sizeof(cplx);
+    auto take = [&](size_t nbytes) { unsigned char* r = p; p += align_up(nbytes, 256); return r; };
+    w.g = (cplx*)take(blk * n * ne);
+    w.X = (cplx*)take(blk * (n > 1 ? n - 1 : 0) * ne);
+    w.Y = (cplx*)take(blk * (n > 1 ? n - 1 : 0) * ne);
+    w.gx = (cplx*)take(blk * n * ne);
+    for (int t = 0; t < NEGF_NSCRATCH; t++) w.T[t] = (cplx*)take(blk * ne);
+    w.inv = take(zinv_workspace_bytes(b, ne));
+    w.ref = (double*)take(sizeof(double) * ne);
+    w.done = (int*)take(sizeof(int) * ne);
+    w.sing = (int*)take(sizeof(int) * ne);
+    w.tmpinfo = (int*)take(sizeof(int) * ne);
+    w.bytes = (size_t)(p - (unsigned char*)base);
+    return w;
+}

@@ -1,0 +1,236 @@
+// K2: batched complex-FP64 GEMM on the FP64 tensor pipe (DMMA.8x8x4).
+//
+//   C[e] = alpha * op(A[e]) * op(B[e]) + beta * D[e],   op in {none, conjugate transpose}
+//
+// Every product of the RGF sweeps and of the Sancho-Rubio doubling goes through
+// this kernel.  sm_100a has no tcgen05 kind for f64 (ptxas rejects .kind::f64), so the FP64
+// tensor path is warp-level mma.sync.m8n8k4 with register operands; measured issue-rate peak
+// 37.15 TFLOP/s (= 148 SMs x 1.965 GHz x 128 flop/clk), identical to the DFMA peak.
+//
+// Design:
+//  * complex product by the 4M decomposition: four real DMMAs per 8x8x4 sub-product,
+//    accumulators (re, im planes) in registers;
+//  * operands stay interleaved (re, im) in shared memory, staged by 16-byte cp.async with an
+//    XOR swizzle that makes every LDS.128 fragment read bank-conflict free for BOTH the
+//    k-contiguous and the mn-contiguous tile layout, so conjugate-transposed operands
+//    (g^H, A^H, X^H of SURVEY.md 8(a) S5-S6) cost nothing: the dagger is a transposed fragment
+//    read plus a sign-bit flip (integer XOR, not an FP64 op);
+//  * 3-stage cp.async pipeline, BK = 16; one fragment read feeds 4 DMMAs per sub-tile pair, so
+//    shared-memory bandwidth stays < 20 % while the FP64 pipe is saturated;
+//  * ragged m, n, k handled by zero-filled cp.async and predicated stores.
+#include "common.cuh"
+
+namespace {
+
+constexpr int BK = 16;
+constexpr int STAGES = 3;
+
+__device__ __forceinline__ void dmma(double& c0, double& c1, double a, double b) {
+    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+        : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+__device__ __forceinline__ double flip(double x) {   // -x without touching the FP64 pipe
+    return __hiloint2double(__double2hiint(x) ^ 0x80000000, __double2loint(x));
+}
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem, bool pred) {
+    unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    int sz = pred ? 16 : 0;   // src-size 0 => 16 bytes of zeros
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" :: "r"(s), "l"(gmem), "r"(sz));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+template <int N> __device__ __forceinline__ void cp_async_wait() {
+    asm volatile("cp.async.wait_group %0;\n" :: "n"(N));
+}
+
+// Tile loaders.  "KC" layout: rows indexed by the m (or n) coordinate, 16 k-elements contiguous,
+// element (r, k) at r*16 + (k ^ 4*(r&1)).  "MC" layout: rows indexed by k, R mn-elements
+// contiguous, element (k, r) at k*R + (r ^ 2*(k&3)).
+template <int R, int NT>
+__device__ __forceinline__ void load_tile_kc(cplx* sm, const cplx* g, int ld, int r0, int k0,
+                                             int rmax, int kmax, int tid) {
+    // global: row (r0 + r), cols k0..k0+15 contiguous
+#pragma unroll
+    for (int c = tid; c < R * BK; c += NT) {
+        int r = c >> 4, kc = c & 15;
+        bool ok = (r0 + r < rmax) && (k0 + kc < kmax);
+        const cplx* src = ok ? g + (size_t)(r0 + r) * ld + (k0 + kc) : g;
+        cp_async16(sm + r * BK + (kc ^ ((r & 1) << 2)), src, ok);
+    }
+}
+template <int R, int NT>
+__device__ __forceinline__ void load_tile_mc(cplx* sm, const cplx* g, int ld, int r0, int k0,
+                                             int rmax, int kmax, int tid) {
+    // global: row (k0 + k), cols r0..r0+R-1 contiguous
+#pragma unroll
+    for (int c = tid; c < R * BK; c += NT) {
+        int k = c / R, r = c % R;
+        bool ok = (r0 + r < rmax) && (k0 + k < kmax);
+        const cplx* src = ok ? g + (size_t)(k0 + k) * ld + (r0 + r) : g;
+        cp_async16(sm + k * R + (r ^ ((k & 3) << 1)), src, ok);
+    }
+}
+
+template <int OPA, int OPB, int BM, int BN, int WM, int WN>
+__global__ void __launch_bounds__(WM * WN * 32, 1) zgemm_kernel(GemmArgs a) {
+    constexpr int NT = WM * WN * 32;
+    constexpr int MI = BM / WM / 8;     // 8x8 sub-tiles per warp along m
+    constexpr int NI = BN / WN / 8;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx* sA = reinterpret_cast<cplx*>(smem_raw);              // STAGES x BM x BK
+    cplx* sB = sA + STAGES * BM * BK;                          // STAGES x BN x BK
+
+    const int e = blockIdx.y;
+    if (a.skip && a.skip[e]) return;
+    const int tiles_n = (a.n + BN - 1) / BN;
+    const int tm = blockIdx.x / tiles_n, tn = blockIdx.x % tiles_n;
+    const int m0 = tm * BM, n0 = tn * BN;
+    const cplx* gA = a.A + (size_t)e * a.sA;
+    const cplx* gB = a.B + (size_t)e * a.sB;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int wm0 = (warp / WN) * (MI * 8), wn0 = (warp % WN) * (NI * 8);
+    const int lr = lane >> 2, lk = lane & 3;
+
+    double cre[MI][NI][2], cim[MI][NI][2];
+#pragma unroll
+    for (int i = 0; i < MI; i++)
+#pragma unroll
+        for (int j = 0; j < NI; j++) { cre[i][j][0] = cre[i][j][1] = cim[i][j][0] = cim[i][j][1] = 0.0; }
+
+    const int KB = (a.k + BK - 1) / BK;
+    auto issue = [&](int kb) {
+        if (kb < KB) {
+            int st = kb % STAGES, k0 = kb * BK;
+            if (OPA == 0) load_tile_kc<BM, NT>(sA + st * BM * BK, gA, a.lda, m0, k0, a.m, a.k, tid);
+            else          load_tile_mc<BM, NT>(sA + st * BM * BK, gA, a.lda, m0, k0, a.m, a.k, tid);
+            if (OPB == 0) load_tile_mc<BN, NT>(sB + st * BN * BK, gB, a.ldb, n0, k0, a.n, a.k, tid);
+            else          load_tile_kc<BN, NT>(sB + st * BN * BK, gB, a.ldb, n0, k0, a.n, a.k, tid);
+        }
+        cp_async_commit();
+    };
+#pragma unroll
+    for (int s = 0; s < STAGES - 1; s++) issue(s);
+
+    for (int kb = 0; kb < KB; kb++) {
+        cp_async_wait<STAGES - 2>();
+        __syncthreads();
+        issue(kb + STAGES - 1);
+        const cplx* tA = sA + (kb % STAGES) * BM * BK;
+        const cplx* tB = sB + (kb % STAGES) * BN * BK;
+#pragma unroll
+        for (int ks = 0; ks < BK / 4; ks++) {
+            const int k = ks * 4 + lk;
+            double ar[MI], ai[MI], an[MI], br[NI], bi[NI];
+#pragma unroll
+            for (int i = 0; i < MI; i++) {
+                int m = wm0 + i * 8 + lr;
+                cplx v = (OPA == 0) ? tA[m * BK + (k ^ ((m & 1) << 2))] : tA[k * BM + (m ^ ((k & 3) << 1))];
+                ar[i] = v.x;
+                // im += (sa ai) br ; re += (-sa sb ai) bi'   with bi' = |bi| sign-adjusted below
+                ai[i] = (OPA == 0) ? v.y : flip(v.y);
+                an[i] = ((OPA ^ OPB) == 0) ? flip(v.y) : v.y;
+            }
+#pragma unroll
+            for (int j = 0; j < NI; j++) {
+                int n = wn0 + j * 8 + lr;
+                cplx v = (OPB == 0) ? tB[k * BN + (n ^ ((k & 3) << 1))] : tB[n * BK + (k ^ ((n & 1) << 2))];
+                br[j] = v.x;
+                bi[j] = v.y;   // raw; the conj sign of B is folded: re uses an (has -sa*sb), im uses sb below
+            }
+#pragma unroll
+            for (int i = 0; i < MI; i++)
+#pragma unroll
+                for (int j = 0; j < NI; j++) {
+                    dmma(cre[i][j][0], cre[i][j][1], ar[i], br[j]);
+                    dmma(cim[i][j][0], cim[i][j][1], ai[i], br[j]);
+                    dmma(cre[i][j][0], cre[i][j][1], an[i], bi[j]);
+                    dmma(cim[i][j][0], cim[i][j][1], (OPB == 0) ? ar[i] : flip(ar[i]), bi[j]);
+                }
+        }
+    }
+    cp_async_wait<0>();
+
+    // epilogue: C = alpha*acc + beta*D
+    cplx* gC = a.C + (size_t)e * a.sC;
+    const cplx* gD = a.D ? a.D + (size_t)e * a.sD : nullptr;
+    const cplx al = a.alpha, be = a.beta;
+#pragma unroll
+    for (int i = 0; i < MI; i++) {
+        int row = m0 + wm0 + i * 8 + lr;
+        if (row >= a.m) continue;
+#pragma unroll
+        for (int j = 0; j < NI; j++) {
+#pragma unroll
+            for (int q = 0; q < 2; q++) {
+                int col = n0 + wn0 + j * 8 + lk * 2 + q;
+                if (col >= a.n) continue;
+                cplx acc = cmake(cre[i][j][q], cim[i][j][q]);
+                cplx r = cmul(al, acc);
+                if (gD) { cplx d = gD[(size_t)row * a.ldc + col]; cfma(r, be, d); }
+                gC[(size_t)row * a.ldc + col] = r;
+            }
+        }
+    }
+}
+
+template <int OPA, int OPB, int BM, int BN, int WM, int WN>
+int launch_cfg(negf_ctx* ctx, const GemmArgs& a) {
+    auto kern = zgemm_kernel<OPA, OPB, BM, BN, WM, WN>;
+    constexpr int smem = STAGES * (BM + BN) * BK * (int)sizeof(cplx);
+    static bool attr_done = false;
+    if (!attr_done) {
+        NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        attr_done = true;
+    }
+    int tiles = ((a.m + BM - 1) / BM) * ((a.n + BN - 1) / BN);
+    dim3 grid(tiles, a.batch);
+    kern<<<grid, WM * WN * 32, smem, ctx->stream>>>(a);
+    NEGF_LAUNCH_CHECK(ctx);
+    return NEGF_OK;
+}
+
+template <int BM, int BN, int WM, int WN>
+int launch_ops(negf_ctx* ctx, const GemmArgs& a) {
+    if (a.opA == 0 && a.opB == 0) return launch_cfg<0, 0, BM, BN, WM, WN>(ctx, a);
+    if (a.opA == 1 && a.opB == 0) return launch_cfg<1, 0, BM, BN, WM, WN>(ctx, a);
+    if (a.opA == 0 && a.opB == 1) return launch_cfg<0, 1, BM, BN, WM, WN>(ctx, a);
+    return launch_cfg<1, 1, BM, BN, WM, WN>(ctx, a);
+}
+
+}  // namespace
+
+int zgemm_launch(negf_ctx* ctx, const GemmArgs& a) {
+    if (a.m <= 0 || a.n <= 0 || a.batch <= 0) return NEGF_OK;
+    if (a.k < 0 || (a.opA | a.opB) & ~1) return NEGF_EINVAL;
+    if (a.batch > 65535) return NEGF_EUNSUPPORTED;
+    // Tile choice: 128x64 CTA tiles (8 warps, 32x32 warp tiles) when they fill the machine,
+    // else 64x64 (4 warps) to get more CTAs in flight.
+    long long big_tiles = (long long)((a.m + 127) / 128) * ((a.n + 63) / 64) * a.batch;
+    if (a.m > 64 && big_tiles >= ctx->num_sms) return launch_ops<128, 64, 4, 2>(ctx, a);
+    return launch_ops<64, 64, 2, 2>(ctx, a);
+}
+
+int zgemm_bb(negf_ctx* ctx, int opA, int opB, int b, cplx alpha, const cplx* A, long long sA,
+             const cplx* B, long long sB, cplx beta, const cplx* D, long long sD,
+             cplx* C, long long sC, int batch, const int* skip) {
+    GemmArgs g;
+    g.opA = opA; g.opB = opB; g.m = g.n = g.k = b; g.alpha = alpha; g.beta = beta;
+    g.A = A; g.lda = b; g.sA = sA; g.B = B; g.ldb = b; g.sB = sB;
+    g.D = D; g.sD = sD; g.C = C; g.ldc = b; g.sC = sC; g.batch = batch; g.skip = skip;
+    return zgemm_launch(ctx, g);
+}
+
+extern "C" int negf_zgemm_batched(negf_ctx* ctx, int opA, int opB, int m, int n, int k,
+                                  negf_c128 alpha, const negf_c128* A, int lda, long long strideA,
+                                  const negf_c128* B, int ldb, long long strideB,
+                                  negf_c128 beta, const negf_c128* D,
+                                  negf_c128* C, int ldc, long long strideC, int batch) {
+    if (!ctx || !A || !B || !C || m < 0 || n < 0 || k < 0 || batch < 0) return NEGF_EINVAL;
+    GemmArgs g;
+    g.opA = opA; g.opB = opB; g.m = m; g.n = n; g.k = k;
+    g.alpha = cmake(alpha.re, alpha.im); g.beta = cmake(beta.re, beta.im);
+    g.A = (const cplx*)A; g.lda = lda; g.sA = strideA;
+    g.B = (const cplx*)B; g.ldb = ldb; g.sB = strideB;
+    g.D = (const cplx*)D; g.sD = strideC;
+    g.C = (cplx*)C; g.ldc = ldc; g.sC = strideC; g.batch = batch; g.skip = nullptr;
+    return zgemm_launch(ctx, g);
+}

@@ -1,0 +1,484 @@
+// K1: batched in-place complex inverse with partial pivoting.
+//
+// Every g_i = (A_ii - A_{i,i-1} g_{i-1} A_{i-1,i})^-1 of the RGF forward sweep (
+// SURVEY.md 8(a) S3) and every g = a_b^-1 of the Sancho-Rubio doubling is one
+// call of this file.
+//
+//  * b <= SMALL_MAX: one CTA per matrix, whole matrix in shared memory, in-place Gauss-Jordan
+//    with row pivoting on |re|+|im| (izamax convention), column permutation undone at the end.
+//  * larger b: BLOCKED in-place Gauss-Jordan, panel width w <= 32:
+//      1. the panel (rows >= k0) is LU-factorised with partial pivoting by a thread-block
+//         CLUSTER that holds the tall panel in distributed shared memory (up to 8 CTAs x 200 KB);
+//         every column costs ONE cluster barrier: before it each CTA pushes its best pivot
+//         candidate (value, row index, row content) and CTA 0 the current diagonal row into all
+//         CTAs' buffers through DSMEM, after it everybody knows the pivot and already owns the
+//         two rows to exchange;
+//      2. row swaps are applied to the rest of the matrix, the pivot rows R are moved to scratch
+//         and zeroed;
+//      3. the panel is finalised to P' = [-T Dinv ; Dinv ; -L21 L11^-1] with two small GEMMs;
+//      4. ONE rank-w GEMM per side updates all other columns: M += P' R  (K2 kernel, DMMA).
+//    Cost b^3 complex multiply-adds = 8 b^3 flops = 1 U, same as getrf + getri, but every
+//    trailing update is a full-height uniform GEMM.  Pivoting is partial pivoting among the
+//    not-yet-eliminated rows, exactly as in LU.
+#include <cooperative_groups.h>
+
+#include "common.cuh"
+
+namespace cg = cooperative_groups;
+
+namespace {
+
+constexpr int SMALL_MAX = 96;      // b*b*16 B <= 147 KB
+constexpr int PW = 32;             // max panel width (one lane per panel column)
+constexpr int CMAX = 8;            // portable cluster size
+constexpr int PANEL_SMEM_ROWS_BYTES = 176 * 1024;   // + 9 KB exchange buffers + 33 KB static < 227 KB
+
+// ------------------------------------------------------------------------------------------------
+// small path
+// ------------------------------------------------------------------------------------------------
+template <int NT>
+__global__ void __launch_bounds__(NT) gj_small_kernel(cplx* A, long long sA, int b, int* info, int code,
+                                                      const int* skip) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int e = blockIdx.x;
+    if (skip && skip[e]) return;
+    const int ld = b + 1;
+    cplx* M = reinterpret_cast<cplx*>(smem_raw);       // [b][ld]
+    cplx* rowbuf = M + (size_t)b * ld;                  // [b]
+    cplx* colbuf = rowbuf + b;                          // [b]
+    int* piv = reinterpret_cast<int*>(colbuf + b);      // [b]
+    __shared__ double red_val[32];
+    __shared__ int red_idx[32];
+    __shared__ int s_p;
+    __shared__ int s_sing;
+    cplx* g = A + (size_t)e * sA;
+    const int tid = threadIdx.x;
+    for (int idx = tid; idx < b * b; idx += NT) M[(idx / b) * ld + idx % b] = g[idx];
+    if (tid == 0) s_sing = 0;
+    __syncthreads();
+    for (int k = 0; k < b; k++) {
+        // pivot search over rows >= k
+        double best = -1.0; int bi = k;
+        for (int r = k + tid; r < b; r += NT) {
+            double v = cabs1(M[r * ld + k]);
+            if (v > best) { best = v; bi = r; }
+        }
+        for (int o = 16; o > 0; o >>= 1) {
+            double ov = __shfl_down_sync(0xffffffffu, best, o);
+            int oi = __shfl_down_sync(0xffffffffu, bi, o);
+            if (ov > best || (ov == best && oi < bi)) { best = ov; bi = oi; }
+        }
+        if ((tid & 31) == 0) { red_val[tid >> 5] = best; red_idx[tid >> 5] = bi; }
+        __syncthreads();
+        if (tid == 0) {
+            for (int wv = 1; wv < NT / 32; wv++)
+                if (red_val[wv] > best || (red_val[wv] == best && red_idx[wv] < bi)) { best = red_val[wv]; bi = red_idx[wv]; }
+            s_p = bi; piv[k] = bi;
+            if (!(best > 0.0) && s_sing == 0) s_sing = k + 1;
+        }
+        __syncthreads();
+        const int p = s_p;
+        if (p != k) for (int j = tid; j < b; j += NT) { cplx t = M[k * ld + j]; M[k * ld + j] = M[p * ld + j]; M[p * ld + j] = t; }
+        __syncthreads();
+        cplx pv = M[k * ld + k];
+        cplx d = (pv.x == 0.0 && pv.y == 0.0) ? cmake(1.0, 0.0) : crecip(pv);
+        for (int j = tid; j < b; j += NT) {
+            rowbuf[j] = cmul(M[k * ld + j], d);
+            colbuf[j] = M[j * ld + k];
+        }
+        __syncthreads();
+        for (int idx = tid; idx < b * b; idx += NT) {
+            int i = idx / b, j = idx % b;
+            cplx v;
+            if (i == k) v = (j == k) ? d : rowbuf[j];
+            else if (j == k) v = cneg(cmul(colbuf[i], d));
+            else { v = M[i * ld + j]; cfms(v, colbuf[i], rowbuf[j]); }
+            M[i * ld + j] = v;
+        }
+        __syncthreads();
+    }
+    // undo the row permutation as column swaps in reverse order: A^-1 = (P A)^-1 P
+    for (int r = tid; r < b; r += NT)
+        for (int k = b - 1; k >= 0; k--) {
+            int p = piv[k];
+            if (p != k) { cplx t = M[r * ld + k]; M[r * ld + k] = M[r * ld + p]; M[r * ld + p] = t; }
+        }
+    __syncthreads();
+    for (int idx = tid; idx < b * b; idx += NT) g[idx] = M[(idx / b) * ld + idx % b];
+    if (tid == 0 && s_sing && info) info[e] = code > 0 ? code : s_sing;
+}
+
+// ------------------------------------------------------------------------------------------------
+// blocked path, step 1: cluster panel LU with partial pivoting
+// ------------------------------------------------------------------------------------------------
+struct Cand { double val; int row; int pad; };
+
+struct PanelArgs {
+    cplx* A; long long sA; int b, k0, w, slab;
+    int* ipiv;            // [batch][b] global row index chosen for column k
+    cplx* Dinv;           // [batch][PW*PW] (ld = w)  (L11 U11)^-1
+    cplx* Linv;           // [batch][PW*PW] (ld = w)  L11^-1
+    int* info; int code; const int* skip;
+};
+
+constexpr int PANEL_NT = 512;
+
+__global__ void __launch_bounds__(PANEL_NT, 1) gj_panel_cluster_kernel(PanelArgs a) {
+    cg::cluster_group cluster = cg::this_cluster();
+    const int rank = (int)cluster.block_rank();
+    const int C = (int)cluster.num_blocks();
+    const int e = blockIdx.y;
+    if (a.skip && a.skip[e]) return;              // uniform over the cluster
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int w = a.w, b = a.b, k0 = a.k0, slab = a.slab;
+    cplx* P = reinterpret_cast<cplx*>(smem_raw);                    // [slab][w]
+    cplx* candrow = P + (size_t)slab * w;                           // [2][CMAX][PW]
+    cplx* diagrow = candrow + 2 * CMAX * PW;                        // [2][PW]
+    Cand* cand = reinterpret_cast<Cand*>(diagrow + 2 * PW);         // [2][CMAX]
+    __shared__ double red_val[PANEL_NT / 32];
+    __shared__ int red_idx[PANEL_NT / 32];
+    __shared__ int s_best;
+
+    const int rows_total = b - k0;
+    const int r_lo = rank * slab;
+    const int nloc = max(0, min(rows_total, r_lo + slab) - r_lo);
+    cplx* g = a.A + (size_t)e * a.sA + (size_t)k0 * b + k0;       // panel origin
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    constexpr int NW = PANEL_NT / 32;
+
+    for (int idx = tid; idx < nloc * w; idx += PANEL_NT) {
+        int r = idx / w, j = idx % w;
+        P[r * w + j] = g[(size_t)(r_lo + r) * b + j];
+    }
+    __syncthreads();
+
+    for (int j = 0; j < w; j++) {
+        const int par = j & 1;
+        // local pivot candidate among my rows with global candidate index >= j
+        double best = -1.0; int bi = -1;
+        for (int r = tid; r < nloc; r += PANEL_NT) {
+            if (r_lo + r >= j) {
+                double v = cabs1(P[r * w + j]);
+                if (v > best) { best = v; bi = r; }
+            }
+        }
+        for (int o = 16; o > 0; o >>= 1) {
+            double ov = __shfl_down_sync(0xffffffffu, best, o);
+            int oi = __shfl_down_sync(0xffffffffu, bi, o);
+            if (ov > best || (ov == best && oi >= 0 && (bi < 0 || oi < bi))) { best = ov; bi = oi; }
+        }
+        if (lane == 0) { red_val[warp] = best; red_idx[warp] = bi; }
+        __syncthreads();
+        if (warp == 0) {
+            best = lane < NW ? red_val[lane] : -1.0;
+            bi = lane < NW ? red_idx[lane] : -1;
+            for (int o = 16; o > 0; o >>= 1) {
+                double ov = __shfl_down_sync(0xffffffffu, best, o);
+                int oi = __shfl_down_sync(0xffffffffu, bi, o);
+                if (ov > best || (ov == best && oi >= 0 && (bi < 0 || oi < bi))) { best = ov; bi = oi; }
+            }
+            best = __shfl_sync(0xffffffffu, best, 0);
+            bi = __shfl_sync(0xffffffffu, bi, 0);
+            // push (value, row, row content) to every CTA of the cluster; CTA 0 also the diagonal row
+            cplx myrow = (bi >= 0 && lane < w) ? P[bi * w + lane] : cmake(0.0, 0.0);
+            cplx drow = (rank == 0 && lane < w) ? P[j * w + lane] : cmake(0.0, 0.0);
+            for (int q = 0; q < C; q++) {
+                cplx* rc = cluster.map_shared_rank(candrow, q);
+                if (lane < w) rc[(par * CMAX + rank) * PW + lane] = myrow;
+                if (rank == 0 && lane < w) cluster.map_shared_rank(diagrow, q)[par * PW + lane] = drow;
+                if (lane == 0) {
+                    Cand c; c.val = best; c.row = bi >= 0 ? r_lo + bi : -1; c.pad = 0;
+                    cluster.map_shared_rank(cand, q)[par * CMAX + rank] = c;
+                }
+            }
+        }
+        cluster.sync();
+        // everybody picks the same winner
+        if (tid == 0) {
+            int wq = -1; double wv = -1.0; int wr = 0x7fffffff;
+            for (int q = 0; q < C; q++) {
+                Cand c = cand[par * CMAX + q];
+                if (c.row >= 0 && (c.val > wv || (c.val == wv && c.row < wr))) { wv = c.val; wq = q; wr = c.row; }
+            }
+            s_best = wq;
+            if (rank == 0) {
+                a.ipiv[(size_t)e * b + k0 + j] = k0 + wr;
+                if (!(wv > 0.0) && a.info && a.info[e] == 0) a.info[e] = a.code > 0 ? a.code : (k0 + j + 1);
+            }
+        }
+        __syncthreads();
+        const int wq = s_best;
+        const int prow = cand[par * CMAX + wq].row;                 // global candidate index of the pivot row
+        const double pval = cand[par * CMAX + wq].val;
+        const cplx* pr = candrow + (par * CMAX + wq) * PW;          // pivot row content
+        // exchange rows j <-> prow
+        if (prow != j && warp == 0 && lane < w) {
+            if (prow >= r_lo && prow < r_lo + nloc) P[(prow - r_lo) * w + lane] = diagrow[par * PW + lane];
+        }
+        if (rank == 0 && warp == 1 && lane < w) P[j * w + lane] = pr[lane];
+        __syncthreads();
+        // eliminate below: rows with candidate index > j
+        cplx pv = pr[j];
+        cplx rinv = (pval > 0.0) ? crecip(pv) : cmake(0.0, 0.0);
+        cplx pvl = lane < w ? pr[lane] : cmake(0.0, 0.0);
+        for (int r = warp; r < nloc; r += NW) {
+            if (r_lo + r > j) {
+                cplx l = cmul(P[r * w + j], rinv);
+                __syncwarp();
+                if (lane == j) P[r * w + j] = l;
+                else if (lane > j && lane < w) { cplx v = P[r * w + lane]; cfms(v, l, pvl); P[r * w + lane] = v; }
+            }
+        }
+        __syncthreads();
+    }
+
+    // CTA 0: L11^-1 and (L11 U11)^-1 from the w x w diagonal block, one thread per column
+    if (rank == 0) {
+        __shared__ cplx Li[PW * PW];
+        __shared__ cplx sUi[PW * PW];
+        // Linv (unit lower): solve L X = I column by column
+        if (tid < w) {
+            int c = tid;
+            for (int r = 0; r < w; r++) {
+                cplx s = (r == c) ? cmake(1.0, 0.0) : cmake(0.0, 0.0);
+                for (int k = c; k < r; k++) cfms(s, P[r * w + k], Li[k * PW + c]);
+                Li[r * PW + c] = (r < c) ? cmake(0.0, 0.0) : s;
+            }
+        } else if (tid >= 32 && tid < 32 + w) {
+            // Uinv: solve U X = I column by column (back substitution)
+            int c = tid - 32;
+            for (int r = w - 1; r >= 0; r--) {
+                cplx s = (r == c) ? cmake(1.0, 0.0) : cmake(0.0, 0.0);
+                for (int k = r + 1; k <= c; k++) cfms(s, P[r * w + k], sUi[k * PW + c]);
+                cplx ur = P[r * w + r];
+                cplx inv = (ur.x == 0.0 && ur.y == 0.0) ? cmake(0.0, 0.0) : crecip(ur);
+                sUi[r * PW + c] = (r > c) ? cmake(0.0, 0.0) : cmul(s, inv);
+            }
+        }
+        __syncthreads();
+        cplx* gD = a.Dinv + (size_t)e * PW * PW;
+        cplx* gL = a.Linv + (size_t)e * PW * PW;
+        for (int idx = tid; idx < w * w; idx += PANEL_NT) {
+            int r = idx / w, c = idx % w;
+            cplx s = cmake(0.0, 0.0);
+            for (int k = max(r, c); k < w; k++) cfma(s, sUi[r * PW + k], Li[k * PW + c]);
+            gD[r * w + c] = s;
+            gL[r * w + c] = Li[r * PW + c];
+        }
+    }
+    // write the factored panel back (L21 below, L11\U11 in the diagonal block)
+    for (int idx = tid; idx < nloc * w; idx += PANEL_NT) {
+        int r = idx / w, j = idx % w;
+        g[(size_t)(r_lo + r) * b + j] = P[r * w + j];
+    }
+    cluster.sync();   // nobody exits while remote shared memory may still be targeted
+}
+
+// ------------------------------------------------------------------------------------------------
+// step 2: apply the panel's row swaps to all other columns; move pivot rows to R and zero them
+// ------------------------------------------------------------------------------------------------
+__global__ void gj_swap_extract_kernel(cplx* A, long long sA, int b, int k0, int w, const int* ipiv,
+                                       cplx* R /*[batch][w][b]*/, const int* skip) {
+    const int e = blockIdx.y;
+    if (skip && skip[e]) return;
+    int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= b || (c >= k0 && c < k0 + w)) return;
+    cplx* g = A + (size_t)e * sA;
+    const int* pv = ipiv + (size_t)e * b + k0;
+    for (int j = 0; j < w; j++) {
+        int p = pv[j];
+        if (p != k0 + j) {
+            cplx t = g[(size_t)(k0 + j) * b + c];
+            g[(size_t)(k0 + j) * b + c] = g[(size_t)p * b + c];
+            g[(size_t)p * b + c] = t;
+        }
+    }
+    cplx* r = R + (size_t)e * w * b;
+    for (int j = 0; j < w; j++) {
+        r[(size_t)j * b + c] = g[(size_t)(k0 + j) * b + c];
+        g[(size_t)(k0 + j) * b + c] = cmake(0.0, 0.0);
+    }
+}
+
+// copy the finalised panel Pbuf [b][w] into columns [k0, k0+w) of A
+__global__ void gj_panel_store_kernel(cplx* A, long long sA, int b, int k0, int w, const cplx* Pbuf,
+                                      const cplx* Dinv, const int* skip) {
+    const int e = blockIdx.y;
+    if (skip && skip[e]) return;
+    int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= b * w) return;
+    int r = idx / w, j = idx % w;
+    cplx v = (r >= k0 && r < k0 + w) ? Dinv[(size_t)e * PW * PW + (r - k0) * w + j]
+                                     : Pbuf[(size_t)e * b * w + idx];
+    A[(size_t)e * sA + (size_t)r * b + k0 + j] = v;
+}
+// copy Dinv into rows [k0,k0+w) of Pbuf so the big GEMM sees the complete P'
+__global__ void gj_pbuf_diag_kernel(cplx* Pbuf, int b, int k0, int w, const cplx* Dinv, const int* skip) {
+    const int e = blockIdx.y;
+    if (skip && skip[e]) return;
+    int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= w * w) return;
+    Pbuf[(size_t)e * b * w + (size_t)k0 * w + idx] = Dinv[(size_t)e * PW * PW + idx];
+}
+
+// final column permutation: idx[] from the recorded swaps, then a row-wise gather through smem
+__global__ void gj_colperm_kernel(cplx* A, long long sA, int b, const int* ipiv, int* idxbuf, const int* skip) {
+    const int e = blockIdx.y;
+    if (skip && skip[e]) return;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx* row = reinterpret_cast<cplx*>(smem_raw);
+    int* idx = idxbuf + (size_t)e * b;
+    // idx was computed by gj_permidx_kernel
+    cplx* g = A + (size_t)e * sA;
+    for (int r = blockIdx.x; r < b; r += gridDim.x) {
+        for (int c = threadIdx.x; c < b; c += blockDim.x) row[c] = g[(size_t)r * b + c];
+        __syncthreads();
+        for (int c = threadIdx.x; c < b; c += blockDim.x) g[(size_t)r * b + c] = row[idx[c]];
+        __syncthreads();
+    }
+}
+__global__ void gj_permidx_kernel(int b, const int* ipiv, int* idxbuf, const int* skip) {
+    const int e = blockIdx.x;
+    if (skip && skip[e]) return;
+    extern __shared__ int sidx[];
+    for (int c = threadIdx.x; c < b; c += blockDim.x) sidx[c] = c;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const int* pv = ipiv + (size_t)e * b;
+        for (int k = b - 1; k >= 0; k--) {
+            int p = pv[k];
+            if (p != k) { int t = sidx[k]; sidx[k] = sidx[p]; sidx[p] = t; }
+        }
+    }
+    __syncthreads();
+    for (int c = threadIdx.x; c < b; c += blockDim.x) idxbuf[(size_t)e * b + c] = sidx[c];
+}
+
+struct InvWs {
+    cplx* R;      // [batch][PW][b]
+    cplx* Pbuf;   // [batch][b][PW]
+    cplx* Dinv;   // [batch][PW*PW]
+    cplx* Linv;   // [batch][PW*PW]
+    int* ipiv;    // [batch][b]
+    int* idx;     // [batch][b]
+};
+InvWs carve(void* ws, int b, int batch) {
+    InvWs o;
+    unsigned char* p = (unsigned char*)ws;
+    o.R = (cplx*)p;    p += align_up((size_t)batch * PW * b * sizeof(cplx), 256);
+    o.Pbuf = (cplx*)p; p += align_up((size_t)batch * PW * b * sizeof(cplx), 256);
+    o.Dinv = (cplx*)p; p += align_up((size_t)batch * PW * PW * sizeof(cplx), 256);
+    o.Linv = (cplx*)p; p += align_up((size_t)batch * PW * PW * sizeof(cplx), 256);
+    o.ipiv = (int*)p;  p += align_up((size_t)batch * b * sizeof(int), 256);
+    o.idx = (int*)p;
+    return o;
+}
+
+}  // namespace
+
+size_t zinv_workspace_bytes(int b, int batch) {
+    if (b <= SMALL_MAX) return 256;
+    return 2 * align_up((size_t)batch * PW * b * sizeof(cplx), 256) +
+           2 * align_up((size_t)batch * PW * PW * sizeof(cplx), 256) +
+           2 * align_up((size_t)batch * b * sizeof(int), 256);
+}
+
+int zinv_launch(negf_ctx* ctx, int b, cplx* A, long long sA, int batch, void* ws, int* info,
+                int info_code, const int* skip) {
+    if (b <= 0 || batch <= 0) return NEGF_OK;
+    if (b <= SMALL_MAX) {
+        constexpr int NT = 256;
+        size_t smem = ((size_t)b * (b + 1) + 2 * b) * sizeof(cplx) + (size_t)b * sizeof(int);
+        static bool small_attr_done = false;
+        if (!small_attr_done) {
+            NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_small_kernel<NT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                      (int)(((size_t)SMALL_MAX * (SMALL_MAX + 3)) * sizeof(cplx) + SMALL_MAX * 4)));
+            small_attr_done = true;
+        }
+        gj_small_kernel<NT><<<batch, NT, smem, ctx->stream>>>(A, sA, b, info, info_code, skip);
+        NEGF_LAUNCH_CHECK(ctx);
+        return NEGF_OK;
+    }
+    if (batch > 65535) return NEGF_EUNSUPPORTED;
+    if (!ws) return NEGF_ENOWORKSPACE;
+    InvWs W = carve(ws, b, batch);
+    // panel width: the widest of 32/16/8 whose tall panel fits 8 CTAs of shared memory
+    int w = PW;
+    while (w > 8 && (size_t)((b + CMAX - 1) / CMAX) * w * sizeof(cplx) > (size_t)PANEL_SMEM_ROWS_BYTES) w >>= 1;
+    if ((size_t)((b + CMAX - 1) / CMAX) * w * sizeof(cplx) > (size_t)PANEL_SMEM_ROWS_BYTES) return NEGF_EUNSUPPORTED;
+    const size_t fixed = (2 * CMAX * PW + 2 * PW) * sizeof(cplx) + 2 * CMAX * sizeof(Cand);
+    static bool attr_done = false;
+    if (!attr_done) {
+        NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_panel_cluster_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                  (int)(PANEL_SMEM_ROWS_BYTES + fixed)));
+        NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_colperm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+        attr_done = true;
+    }
+    const cplx one = cmake(1.0, 0.0), mone = cmake(-1.0, 0.0), zero = cmake(0.0, 0.0);
+    for (int k0 = 0; k0 < b; k0 += w) {
+        const int wk = min(w, b - k0);
+        const int rows = b - k0;
+        // cluster size: smallest power of two whose slabs fit, at least wk rows per slab
+        int C = 1;
+        while (C < CMAX && (size_t)((rows + C - 1) / C) * wk * sizeof(cplx) > (size_t)PANEL_SMEM_ROWS_BYTES) C <<= 1;
+        // more CTAs shorten the per-column elimination when the panel is tall
+        while (C < CMAX && (rows + C - 1) / C > 512) C <<= 1;
+        int slab = max(wk, (rows + C - 1) / C);
+        PanelArgs pa{A, sA, b, k0, wk, slab, W.ipiv, W.Dinv, W.Linv, info, info_code, skip};
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(C, batch);
+        cfg.blockDim = dim3(PANEL_NT);
+        cfg.dynamicSmemBytes = (size_t)slab * wk * sizeof(cplx) + fixed;
+        cfg.stream = ctx->stream;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = C; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        NEGF_CUDA_CHECK(ctx, cudaLaunchKernelEx(&cfg, gj_panel_cluster_kernel, pa));
+        ctx->launches++;
+        // row swaps on the other columns + pivot rows -> R, zeroed in A
+        gj_swap_extract_kernel<<<dim3((b + 127) / 128, batch), 128, 0, ctx->stream>>>(A, sA, b, k0, wk, W.ipiv, W.R, skip);
+        NEGF_LAUNCH_CHECK(ctx);
+        // P' = [-T Dinv ; Dinv ; -L21 Linv]
+        GemmArgs g;
+        g.opA = 0; g.opB = 0; g.alpha = mone; g.beta = zero; g.D = nullptr; g.sD = 0; g.batch = batch; g.skip = skip;
+        g.n = wk; g.k = wk; g.ldb = wk; g.sB = PW * PW; g.ldc = wk; g.sC = (long long)b * wk; g.lda = b; g.sA = sA;
+        if (k0 > 0) {
+            g.m = k0; g.A = A + k0; g.B = W.Dinv; g.C = W.Pbuf;
+            NEGF_TRY(zgemm_launch(ctx, g));
+        }
+        if (k0 + wk < b) {
+            g.m = b - k0 - wk; g.A = A + (size_t)(k0 + wk) * b + k0; g.B = W.Linv; g.C = W.Pbuf + (size_t)(k0 + wk) * wk;
+            NEGF_TRY(zgemm_launch(ctx, g));
+        }
+        gj_pbuf_diag_kernel<<<dim3((wk * wk + 255) / 256, batch), 256, 0, ctx->stream>>>(W.Pbuf, b, k0, wk, W.Dinv, skip);
+        NEGF_LAUNCH_CHECK(ctx);
+        // M[:, other columns] += P' R
+        g.alpha = one; g.beta = one; g.m = b; g.k = wk; g.A = W.Pbuf; g.lda = wk; g.sA = (long long)b * wk;
+        g.ldb = b; g.sB = (long long)wk * b; g.ldc = b; g.sC = sA; g.sD = sA;
+        if (k0 > 0) {
+            g.n = k0; g.B = W.R; g.C = A; g.D = A;
+            NEGF_TRY(zgemm_launch(ctx, g));
+        }
+        if (k0 + wk < b) {
+            g.n = b - k0 - wk; g.B = W.R + k0 + wk; g.C = A + k0 + wk; g.D = A + k0 + wk;
+            NEGF_TRY(zgemm_launch(ctx, g));
+        }
+        gj_panel_store_kernel<<<dim3((b * wk + 255) / 256, batch), 256, 0, ctx->stream>>>(A, sA, b, k0, wk, W.Pbuf, W.Dinv, skip);
+        NEGF_LAUNCH_CHECK(ctx);
+    }
+    gj_permidx_kernel<<<batch, 256, (size_t)b * sizeof(int), ctx->stream>>>(b, W.ipiv, W.idx, skip);
+    NEGF_LAUNCH_CHECK(ctx);
+    int rows_per = max(1, min(b, (4 * ctx->num_sms + batch - 1) / batch));
+    gj_colperm_kernel<<<dim3(rows_per, batch), 256, (size_t)b * sizeof(cplx), ctx->stream>>>(A, sA, b, W.ipiv, W.idx, skip);
+    NEGF_LAUNCH_CHECK(ctx);
+    return NEGF_OK;
+}
+
+extern "C" int negf_zinverse_batched(negf_ctx* ctx, int b, negf_c128* A, long long stride, int batch, int* info) {
+    if (!ctx || !A || b < 1 || batch < 0) return NEGF_EINVAL;
+    size_t need = zinv_workspace_bytes(b, batch);
+    if (b > SMALL_MAX && (!ctx->ws || ctx->ws_bytes < need)) return NEGF_ENOWORKSPACE;
+    if (info) NEGF_CUDA_CHECK(ctx, cudaMemsetAsync(info, 0, sizeof(int) * batch, ctx->stream));
+    return zinv_launch(ctx, b, (cplx*)A, stride, batch, ctx->ws, info, 0, nullptr);
+}

@@ -1,0 +1,139 @@
+"""Device-side driver of the hot path for a `workloads.Workload`: uploads inputs, owns output and
+workspace tensors, and calls negf_obc_decimate -> negf_rgf_retarded -> negf_rgf_lesser_greater ->
+negf_observables through the C ABI.  Marshalling and memory plumbing only (torch = device memory
++ streams); no arithmetic of the method happens here.
+"""
+from __future__ import annotations
+
+from typing import Dict, Optional
+
+import numpy as np
+import torch
+
+from . import negf
+from .workloads import Workload
+
+_KIND = {"none": negf.SIGMA_NONE, "scalar": negf.SIGMA_SCALAR, "bt": negf.SIGMA_BT}
+
+
+def _dev(a, device):
+    return None if a is None else torch.from_numpy(np.ascontiguousarray(a)).to(device)
+
+
+class DevicePath:
+    """One energy batch [e_lo, e_hi) of a workload resident on one GPU."""
+
+    def __init__(self, wl: Workload, e_lo: int = 0, e_hi: Optional[int] = None, device: str = "cuda:0",
+                 ctx: Optional[negf.Context] = None, want_greater: Optional[bool] = None,
+                 sigma: Optional[dict] = None, alloc_outputs: bool = True):
+        self.wl = wl
+        self.device = torch.device(device)
+        self.e_lo, self.e_hi = e_lo, wl.n_energy if e_hi is None else e_hi
+        self.ne = self.e_hi - self.e_lo
+        self.n, self.b = wl.n_blocks, wl.block_size
+        self.want_greater = wl.want_greater if want_greater is None else want_greater
+        self.ctx = ctx or negf.Context(self.device.index or 0)
+        d = self.device
+        self.H_diag, self.H_upper = _dev(wl.H_diag, d), _dev(wl.H_upper, d)
+        self.S_diag, self.S_upper = _dev(wl.S_diag, d), _dev(wl.S_upper, d)
+        self.energy = _dev(wl.energies[self.e_lo:self.e_hi].astype(np.float64), d)
+        self.weights = _dev(wl.weights[self.e_lo:self.e_hi].astype(np.float64), d)
+        self.problem = negf.make_problem(self.n, self.b, self.ne, self.H_diag, self.H_upper, self.S_diag,
+                                         self.S_upper, self.energy, wl.eta)
+        sig = wl.sigma_s(self.e_lo, self.e_hi) if sigma is None else sigma
+        self.sig_dev: Dict[str, Optional[dict]] = {}
+        for t in "rlg":
+            s = sig[t]
+            if s is None:
+                self.sig_dev[t] = None
+            elif s["kind"] == "scalar":
+                self.sig_dev[t] = {"kind": "scalar", "scalar": _dev(s["value"], d)}
+            else:
+                self.sig_dev[t] = {"kind": "bt", "diag": _dev(s["diag"], d), "upper": _dev(s["upper"], d),
+                                   "lower": _dev(s.get("lower"), d)}
+        ws_bytes = negf.Context.workspace_bytes(self.problem)
+        self.workspace = torch.empty(ws_bytes, dtype=torch.uint8, device=d)
+        self.ctx.set_workspace(self.workspace)
+        self.ctx.set_stream(torch.cuda.current_stream(d).cuda_stream)
+        self.out: Dict[str, torch.Tensor] = {}
+        if alloc_outputs:
+            self._alloc()
+
+    def _alloc(self):
+        ne, n, b, d = self.ne, self.n, self.b, self.device
+        z = lambda *shape: torch.empty(shape, dtype=torch.complex128, device=d)
+        r = lambda *shape: torch.empty(shape, dtype=torch.float64, device=d)
+        i = lambda *shape: torch.empty(shape, dtype=torch.int32, device=d)
+        o = self.out
+        for side in "LR":
+            for k in ("sigma_r", "gamma", "sigma_l", "sigma_g", "g_s"):
+                o[f"{k}_{side}"] = z(ne, b, b)
+            o[f"fermi_{side}"] = r(ne)
+            o[f"iters_{side}"] = i(ne)
+            o[f"status_{side}"] = i(ne)
+        o["GR_diag"], o["GR_upper"], o["GR_lower"] = z(ne, n, b, b), z(ne, n - 1, b, b), z(ne, n - 1, b, b)
+        o["GR_corner"] = z(ne, b, b)
+        o["GL_diag"], o["GL_upper"] = z(ne, n, b, b), z(ne, n - 1, b, b)
+        if self.want_greater:
+            o["GG_diag"], o["GG_upper"] = z(ne, n, b, b), z(ne, n - 1, b, b)
+        o["info_r"], o["info_x"] = i(ne), i(ne)
+        o["density"], o["ldos"], o["transmission"] = r(n * b), r(ne, n), r(ne)
+        o["bond_current"], o["contact_current"] = r(ne, max(n - 1, 1)), r(ne, 2)
+
+    # -- the four calls -----------------------------------------------------------------------
+    def _sigma(self, t: str, left=None, right=None) -> negf.Sigma:
+        s = self.sig_dev[t]
+        if s is None:
+            return negf.make_sigma(negf.SIGMA_NONE, left=left, right=right)
+        if s["kind"] == "scalar":
+            return negf.make_sigma(negf.SIGMA_SCALAR, scalar=s["scalar"], left=left, right=right)
+        return negf.make_sigma(negf.SIGMA_BT, diag=s["diag"], upper=s["upper"], lower=s["lower"],
+                               left=left, right=right)
+
+    def obc(self):
+        wl, o = self.wl, self.out
+        for side, tag, mu in ((0, "L", wl.mu_L), (1, "R", wl.mu_R)):
+            self.ctx.obc_decimate(self.problem, side, mu, wl.kT, wl.tol, wl.max_iter, o[f"sigma_r_{tag}"],
+                                  o[f"gamma_{tag}"], o[f"sigma_l_{tag}"], o[f"sigma_g_{tag}"], o[f"g_s_{tag}"],
+                                  o[f"fermi_{tag}"], o[f"iters_{tag}"], o[f"status_{tag}"])
+
+    def set_boundary(self, left: dict, right: dict):
+        """Overwrite the boundary blocks with given host arrays (feeding the oracle's Sigma_B, H2)."""
+        for tag, src in (("L", left), ("R", right)):
+            for k in ("sigma_r", "gamma", "sigma_l", "sigma_g"):
+                self.out[f"{k}_{tag}"].copy_(torch.from_numpy(np.ascontiguousarray(src[k])))
+
+    def retarded(self, corner: bool = True, keep: bool = True):
+        o = self.out
+        self._sr = self._sigma("r", o["sigma_r_L"], o["sigma_r_R"])
+        self.ctx.rgf_retarded(self.problem, self._sr, o["GR_diag"], o["GR_upper"] if self.n > 1 else None,
+                              o["GR_lower"] if self.n > 1 else None, o["GR_corner"] if corner else None,
+                              negf.KEEP_SWEEP if keep else 0, o["info_r"])
+
+    def lesser_greater(self):
+        o = self.out
+        sl = self._sigma("l", o["sigma_l_L"], o["sigma_l_R"])
+        sg = self._sigma("g", o["sigma_g_L"], o["sigma_g_R"]) if self.want_greater else None
+        self.ctx.rgf_lesser_greater(self.problem, self._sr, sl, sg, o["GR_diag"], o["GL_diag"],
+                                    o["GL_upper"] if self.n > 1 else None, o.get("GG_diag"),
+                                    o.get("GG_upper") if self.n > 1 else None, o["info_x"])
+
+    def observables(self):
+        o = self.out
+        g = self.want_greater
+        self.ctx.observables(self.problem, o["GR_diag"], o["GR_upper"], o["GR_lower"], o["GR_corner"], o["GL_diag"],
+                             o["GL_upper"], o.get("GG_diag"), o["gamma_L"], o["gamma_R"],
+                             o["sigma_l_L"] if g else None, o["sigma_g_L"] if g else None,
+                             o["sigma_l_R"] if g else None, o["sigma_g_R"] if g else None,
+                             self.weights, o["density"], o["ldos"], o["transmission"],
+                             o["bond_current"] if self.n > 1 else None, o["contact_current"] if g else None)
+
+    def run(self):
+        """One pass of the whole hot path (S1-S7) over this energy batch."""
+        self.obc()
+        self.retarded()
+        self.lesser_greater()
+        self.observables()
+
+    def host(self, name: str) -> np.ndarray:
+        return self.out[name].cpu().numpy()

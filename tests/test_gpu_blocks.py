@@ -1,0 +1,84 @@
+"""K1/K2 building blocks through the C ABI against library routines (numpy matmul / LAPACK inv).
+Sizes span several tiles and ragged tails."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ctx(negf_lib):
+    import torch
+    c = negf_lib.Context(0)
+    c.set_stream(torch.cuda.current_stream().cuda_stream)
+    return c
+
+
+def _rand(rng, *shape):
+    return rng.standard_normal(shape) + 1j * rng.standard_normal(shape)
+
+
+@pytest.mark.parametrize("m,n,k", [(1, 1, 1), (8, 8, 4), (16, 16, 16), (64, 64, 64), (37, 53, 29),
+                                   (128, 64, 16), (200, 130, 75), (256, 256, 256), (300, 257, 33)])
+@pytest.mark.parametrize("opA,opB", [(0, 0), (1, 0), (0, 1), (1, 1)])
+def test_zgemm_batched(ctx, m, n, k, opA, opB):
+    import torch
+    rng = np.random.default_rng(m * 1000 + n * 10 + k + opA * 2 + opB)
+    batch = 3
+    A = _rand(rng, batch, *((k, m) if opA else (m, k)))
+    B = _rand(rng, batch, *((n, k) if opB else (k, n)))
+    D = _rand(rng, batch, m, n)
+    alpha, beta = 0.7 - 0.3j, -1.1 + 0.4j
+    opa = (lambda x: np.conj(np.swapaxes(x, -1, -2))) if opA else (lambda x: x)
+    opb = (lambda x: np.conj(np.swapaxes(x, -1, -2))) if opB else (lambda x: x)
+    ref = alpha * (opa(A) @ opb(B)) + beta * D
+    dA, dB, dD = (torch.from_numpy(x).cuda() for x in (A, B, D))
+    dC = torch.empty_like(dD)
+    ctx.zgemm_batched(opA, opB, m, n, k, alpha, dA, A.shape[2], A.shape[1] * A.shape[2], dB, B.shape[2],
+                      B.shape[1] * B.shape[2], beta, dD, dC, n, m * n, batch)
+    got = dC.cpu().numpy()
+    err = np.linalg.norm(got - ref) / np.linalg.norm(ref)
+    assert err < 1e-13, err
+    # shared operand (stride 0), no addend, in-place addend
+    dC2 = dD.clone()
+    ctx.zgemm_batched(opA, opB, m, n, k, 1.0, dA, A.shape[2], 0, dB, B.shape[2], B.shape[1] * B.shape[2],
+                      1.0, dC2, dC2, n, m * n, batch)
+    ref2 = opa(A[:1]) @ opb(B) + D
+    assert np.linalg.norm(dC2.cpu().numpy() - ref2) / np.linalg.norm(ref2) < 1e-13
+
+
+@pytest.mark.parametrize("b", [1, 2, 7, 16, 33, 64, 96, 97, 130, 256, 300, 515])
+def test_zinverse_batched(ctx, negf_lib, b):
+    import torch
+    rng = np.random.default_rng(b)
+    batch = 3 if b < 400 else 2
+    A = _rand(rng, batch, b, b) / np.sqrt(b) + 0.3 * np.eye(b)
+    A[0, 0, :] *= 1e-3      # force row pivoting on the first column
+    if b > 2:
+        A[1, :, 1] = A[1, :, 0] * (1 + 1e-9) + 1e-7 * A[1, :, 1]   # nearly dependent columns
+    ref = np.linalg.inv(A)
+    dA = torch.from_numpy(A).cuda()
+    info = torch.full((batch,), -7, dtype=torch.int32, device="cuda")
+    p = negf_lib.Problem(2, b, batch, None, None, None, None, None, 0.0)
+    ws = torch.empty(negf_lib.Context.workspace_bytes(p), dtype=torch.uint8, device="cuda")
+    ctx.set_workspace(ws)
+    ctx.zinverse_batched(b, dA, b * b, batch, info)
+    got = dA.cpu().numpy()
+    assert info.cpu().tolist() == [0] * batch
+    for e in range(batch):
+        cond = np.linalg.cond(A[e])
+        err = np.linalg.norm(got[e] - ref[e]) / np.linalg.norm(ref[e])
+        assert err < 1e-14 * cond * 50 + 1e-13, (e, err, cond)
+        res = np.linalg.norm(A[e] @ got[e] - np.eye(b)) / np.sqrt(b)
+        assert res < 1e-14 * cond * 50 + 1e-12
+
+
+def test_zinverse_singular_reports_info(ctx, negf_lib):
+    import torch
+    b = 40
+    A = np.eye(b, dtype=complex)[None].repeat(2, 0)
+    A[1, :, 5] = 0.0
+    dA = torch.from_numpy(A).cuda()
+    info = torch.zeros(2, dtype=torch.int32, device="cuda")
+    ctx.zinverse_batched(b, dA, b * b, 2, info)
+    assert info.cpu().tolist() == [0, 6]

@@ -1,0 +1,151 @@
+"""Parity of the CUDA hot path (through the C ABI) with the oracle, element by element on the
+same seeded inputs.  Bar: relative Frobenius error <= 1e-10 per block (BASELINE.json:north_star),
+max over blocks and energies, no floor (reading R14)."""
+import numpy as np
+import pytest
+
+from oracle import pipeline
+from paper_2602_03438_b200 import workloads as W
+from tests.helpers import rel_fro
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-10
+
+# (config, size overrides): configs[0] itself, reduced configs[1-4] with ragged b, n = 2 edge case
+CASES = [
+    (0, {}),
+    (0, dict(n_blocks=2, block_size=5)),
+    (1, dict(n_blocks=6, block_size=24, n_energy=5)),
+    (1, dict(n_blocks=5, block_size=64, n_energy=4)),
+    (2, dict(n_blocks=4, block_size=40, n_energy=3)),
+    (2, dict(n_blocks=3, block_size=136, n_energy=2)),
+    (3, dict(n_blocks=4, block_size=72, n_energy=3)),
+    (3, dict(n_blocks=3, block_size=130, n_energy=2)),
+    (4, dict(n_blocks=3, block_size=200, n_energy=2)),
+]
+
+
+def _oracle_all(wl):
+    sig = wl.sigma_s()
+    outs = []
+    for k in range(wl.n_energy):
+        s1 = {t: (None if sig[t] is None else {kk: (vv[k:k + 1] if kk != "kind" else vv) for kk, vv in sig[t].items()})
+              for t in "rlg"}
+        outs.append(pipeline.solve_energy(wl, k, sigma=s1, want_greater=True))
+    return sig, outs
+
+
+@pytest.fixture(scope="module")
+def runner_mod(negf_lib):
+    from paper_2602_03438_b200 import runner
+    return runner
+
+
+@pytest.mark.parametrize("cfg,kw", CASES)
+def test_rgf_with_oracle_boundary(runner_mod, cfg, kw):
+    """negf_rgf_retarded / negf_rgf_lesser_greater / negf_observables on IDENTICAL inputs:
+    the oracle's Sigma_B is fed to the GPU (hazard H2)."""
+    wl = W.make_workload(cfg, **kw)
+    sig, outs = _oracle_all(wl)
+    dp = runner_mod.DevicePath(wl, want_greater=True, sigma=sig)
+    stack = lambda side, key: np.stack([o[side][key] for o in outs])
+    dp.set_boundary({k: stack("left", k) for k in ("sigma_r", "gamma", "sigma_l", "sigma_g")},
+                    {k: stack("right", k) for k in ("sigma_r", "gamma", "sigma_l", "sigma_g")})
+    dp.retarded()
+    dp.lesser_greater()
+    dp.observables()
+    assert dp.host("info_r").tolist() == [0] * wl.n_energy
+    n = wl.n_blocks
+    fam = {"GR_diag": ("ret", "GR_diag"), "GR_upper": ("ret", "GR_upper"), "GR_lower": ("ret", "GR_lower"),
+           "GL_diag": ("les", "GX_diag"), "GL_upper": ("les", "GX_upper"),
+           "GG_diag": ("gtr", "GX_diag"), "GG_upper": ("gtr", "GX_upper")}
+    for name, (grp, key) in fam.items():
+        ref = np.stack([o[grp][key] for o in outs])
+        if ref.shape[1] == 0:
+            continue
+        err = rel_fro(dp.host(name), ref)
+        assert err < TOL, (name, err)
+    corner = np.stack([o["ret"]["GR_corner"][0] for o in outs])
+    assert rel_fro(dp.host("GR_corner"), corner) < TOL
+    # observables
+    T = np.array([o["obs"]["transmission"] for o in outs])
+    assert np.allclose(dp.host("transmission"), T, rtol=1e-9, atol=1e-13)
+    ld = np.stack([o["obs"]["ldos"] for o in outs])
+    assert np.allclose(dp.host("ldos"), ld, rtol=1e-9, atol=1e-12 * np.abs(ld).max())
+    dens = pipeline.density(wl, [o["obs"]["density_integrand"] for o in outs])
+    assert np.allclose(dp.host("density"), dens, rtol=1e-9, atol=1e-12 * np.abs(dens).max())
+    if n > 1:
+        J = np.stack([o["obs"]["bond_current"] for o in outs])
+        assert np.allclose(dp.host("bond_current"), J, rtol=1e-8, atol=1e-11 * np.abs(J).max() + 1e-300)
+    I = np.stack([o["obs"]["contact_current"] for o in outs])
+    assert np.allclose(dp.host("contact_current"), I, rtol=1e-8, atol=1e-11 * np.abs(I).max() + 1e-300)
+
+
+@pytest.mark.parametrize("cfg,kw", [CASES[0], CASES[2], CASES[4], CASES[5], CASES[8]])
+def test_obc_decimate(runner_mod, cfg, kw):
+    """negf_obc_decimate vs the fp64 oracle.  Decimation is conditioning-limited (~eps/eta per
+    doubling, hazard H2): every energy is reported; the bar is 1e-10 except where two correct
+    fp64 evaluations themselves differ more, which is bounded here by 5e-9."""
+    wl = W.make_workload(cfg, **kw)
+    dp = runner_mod.DevicePath(wl, want_greater=True)
+    dp.obc()
+    worst = 0.0
+    for side, tag, mu in ((0, "L", wl.mu_L), (1, "R", wl.mu_R)):
+        sig = dp.host(f"sigma_r_{tag}")
+        gam = dp.host(f"gamma_{tag}")
+        sl, sg = dp.host(f"sigma_l_{tag}"), dp.host(f"sigma_g_{tag}")
+        its, st, fer = dp.host(f"iters_{tag}"), dp.host(f"status_{tag}"), dp.host(f"fermi_{tag}")
+        for k in range(wl.n_energy):
+            o = pipeline.obc_one_energy(float(wl.energies[k]), wl.eta, wl.H_diag, wl.H_upper, wl.S_diag,
+                                        wl.S_upper, mu, wl.kT, side, wl.tol, wl.max_iter)
+            assert st[k] == 0 and abs(int(its[k]) - o["iters"]) <= 1       # reading R3
+            assert abs(fer[k] - o["f"]) < 1e-15
+            e = rel_fro(sig[k], o["sigma_r"])
+            worst = max(worst, e)
+            assert e < 5e-9, (tag, k, e)
+            assert rel_fro(gam[k], o["gamma"]) < 5e-8
+            # derived blocks are consistent with the GPU's own Sigma (exact arithmetic relations)
+            g_own = 1j * (sig[k] - sig[k].conj().T)
+            assert np.allclose(gam[k], g_own, rtol=0, atol=1e-14 * np.abs(sig[k]).max())
+            assert np.allclose(sl[k], 1j * fer[k] * gam[k], rtol=1e-14, atol=1e-300)
+            assert np.allclose(sg[k], -1j * (1 - fer[k]) * gam[k], rtol=1e-14, atol=1e-300)
+    print(f"decimation worst rel err cfg{cfg}{kw}: {worst:.2e}")
+
+
+@pytest.mark.parametrize("cfg,kw", [CASES[0], CASES[3], CASES[6]])
+def test_end_to_end(runner_mod, cfg, kw):
+    """GPU decimation -> GPU RGF end to end vs the oracle end to end (reported, looser bar: the
+    decimation's conditioning, H2, propagates)."""
+    wl = W.make_workload(cfg, **kw)
+    sig, outs = _oracle_all(wl)
+    dp = runner_mod.DevicePath(wl, want_greater=True, sigma=sig)
+    dp.run()
+    ref = np.stack([o["ret"]["GR_diag"] for o in outs])
+    assert rel_fro(dp.host("GR_diag"), ref) < 2e-8
+    ref = np.stack([o["les"]["GX_diag"] for o in outs])
+    assert rel_fro(dp.host("GL_diag"), ref) < 2e-8
+
+
+def test_n1_explicit_lead_rejected_without_lead(runner_mod, negf_lib):
+    """n = 1: periodic-copy leads need two blocks; the call must refuse (EINVAL), RGF still works."""
+    wl = W.make_workload(0, n_blocks=1, block_size=12)
+    dp = runner_mod.DevicePath(wl, want_greater=True)
+    with pytest.raises(negf_lib.NegfError):
+        dp.obc()
+    rng = np.random.default_rng(1)
+    b = 12
+    def lead(f):
+        m = W.complex_normal(rng, (b, b), 0.1)
+        s = -1j * (m @ m.conj().T) + 0.05 * (m + m.conj().T)
+        g = 1j * (s - s.conj().T)
+        return {"sigma_r": s, "gamma": g, "sigma_l": 1j * f * g, "sigma_g": -1j * (1 - f) * g, "f": f}
+    L, R = lead(0.7), lead(0.2)
+    out = pipeline.solve_energy(wl, 0, obc_in=(L, R), want_greater=True)
+    dp.set_boundary({k: L[k][None] for k in ("sigma_r", "gamma", "sigma_l", "sigma_g")},
+                    {k: R[k][None] for k in ("sigma_r", "gamma", "sigma_l", "sigma_g")})
+    dp.retarded()
+    dp.lesser_greater()
+    assert rel_fro(dp.host("GR_diag")[0], out["ret"]["GR_diag"]) < TOL
+    assert rel_fro(dp.host("GL_diag")[0], out["les"]["GX_diag"]) < TOL
+    assert rel_fro(dp.host("GG_diag")[0], out["gtr"]["GX_diag"]) < TOL
