@@ -24,22 +24,37 @@ def lead_blocks(z, H_d, H_u, S_d=None, S_u=None):
     return a_d, a_u, a_l
 
 
-def sancho_rubio(a_d, a_u, a_l, side, tol=1e-12, max_iter=64):
+def _inv(m):
+    """LAPACK inverse in fp64; hand-written Gauss-Jordan (oracle/dense.py) in extended precision."""
+    if m.dtype == np.clongdouble:
+        from .dense import gauss_jordan_inverse
+        return gauss_jordan_inverse(m)
+    return np.linalg.inv(m)
+
+
+def sancho_rubio(a_d, a_u, a_l, side, tol=1e-12, max_iter=64, extended=False, cond_trace=None):
     """Surface Green's function g_s of the semi-infinite lead.
+    extended=True runs the SAME steps in 80-bit np.clongdouble (hazard H2: the fp64 doubling is
+    conditioning-limited at ~eps/eta per step; the extended run is the yardstick for that).
+    cond_trace: optional list that receives the 2-norm condition number of the inverted a_b of
+    every doubling and of the final a_s (diagnostic for the H2 error bound; no effect on results).
 
     side 0 = left lead (surface cell couples rightwards into the device): a_s <- a_s - l g u
     side 1 = right lead:                                                  a_s <- a_s - u g l
     Each doubling: g = a_d^-1; a_s update; a_d <- a_d - u g l - l g u; u <- -u g u; l <- -l g l.
     Stop AFTER the update when ||u||_F + ||l||_F <= tol (||a_u||_F + ||a_l||_F) (reading R3).
     Returns (g_s, iters, converged)."""
-    a_s = a_d.copy()
-    a_b = a_d.copy()
-    u = a_u.copy()
-    l = a_l.copy()
+    dt = np.clongdouble if extended else np.complex128
+    a_s = a_d.astype(dt)
+    a_b = a_d.astype(dt)
+    u = a_u.astype(dt)
+    l = a_l.astype(dt)
     ref = np.linalg.norm(a_u) + np.linalg.norm(a_l)
     iters, converged = 0, False
     for it in range(max_iter):
-        g = np.linalg.inv(a_b)
+        if cond_trace is not None:
+            cond_trace.append(float(np.linalg.cond(a_b.astype(np.complex128))))
+        g = _inv(a_b)
         gu = g @ u
         gl = g @ l
         lgu = l @ gu
@@ -52,7 +67,9 @@ def sancho_rubio(a_d, a_u, a_l, side, tol=1e-12, max_iter=64):
         if np.linalg.norm(u) + np.linalg.norm(l) <= tol * ref:
             converged = True
             break
-    return np.linalg.inv(a_s), iters, converged
+    if cond_trace is not None:
+        cond_trace.append(float(np.linalg.cond(a_s.astype(np.complex128))))
+    return _inv(a_s), iters, converged
 
 
 def boundary_self_energy(a_u, a_l, g_s, side):

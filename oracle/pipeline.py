@@ -20,11 +20,15 @@ def _slice_sigma(sig, k):
     return out
 
 
-def obc_one_energy(E, eta, H_diag, H_upper, S_diag, S_upper, mu, kT, side, tol=1e-12, max_iter=64):
+def obc_one_energy(E, eta, H_diag, H_upper, S_diag, S_upper, mu, kT, side, tol=1e-12, max_iter=64,
+                   extended=False, cond_trace=None):
     z = complex(E, eta)
     Hd, Hu, Sd, Su = obc.contact_blocks(H_diag, H_upper, S_diag, S_upper, side)
     a_d, a_u, a_l = obc.lead_blocks(z, Hd, Hu, Sd, Su)
-    g_s, iters, conv = obc.sancho_rubio(a_d, a_u, a_l, side, tol, max_iter)
+    g_s, iters, conv = obc.sancho_rubio(a_d, a_u, a_l, side, tol, max_iter, extended=extended,
+                                           cond_trace=cond_trace)
+    if extended:
+        a_u, a_l = a_u.astype(np.clongdouble), a_l.astype(np.clongdouble)
     sig = obc.boundary_self_energy(a_u, a_l, g_s, side)
     gam = obc.broadening(sig)
     f = obc.fermi(E, mu, kT)

@@ -107,3 +107,24 @@ def test_chain_band_centre_is_conditioning_limited():
     g, iters, conv = obc.sancho_rubio(a_d, a_u, a_l, 0, 1e-12, 64)
     assert conv
     assert abs(g[0, 0] - chain_surface_gf(z, 0.0, 1.0)) < 1e-3
+
+
+def test_extended_precision_decimation_is_the_yardstick():
+    """The 80-bit run of the same doubling reproduces the 1D closed form far better than fp64 where
+    fp64 is conditioning-limited (H2), which justifies using it to judge decimation parity."""
+    z = complex(0.013, 1e-6)
+    a_d, a_u, a_l = obc.lead_blocks(z, np.array([[0.0 + 0j]]), np.array([[-1.0 + 0j]]))
+    ref = chain_surface_gf(z, 0.0, 1.0)
+    g64, _, c64 = obc.sancho_rubio(a_d, a_u, a_l, 0)
+    g80, _, c80 = obc.sancho_rubio(a_d, a_u, a_l, 0, extended=True)
+    assert c64 and c80 and g80.dtype == np.clongdouble
+    e64, e80 = abs(g64[0, 0] - ref), abs(complex(g80[0, 0]) - ref)
+    assert e80 < 1e-12 and e80 <= e64
+    # and on a matrix lead: unitary-mixed chains
+    H_d, H_u, U, eps, t = W.chain_lead(6)
+    z = complex(0.1, 1e-6)
+    a_d, a_u, a_l = obc.lead_blocks(z, H_d, H_u)
+    gk = np.array([chain_surface_gf(z, eps[k], t[k]) for k in range(6)])
+    refm = (U * gk) @ U.conj().T
+    g80, _, _ = obc.sancho_rubio(a_d, a_u, a_l, 1, extended=True)
+    assert np.linalg.norm(g80.astype(np.complex128) - refm) / np.linalg.norm(refm) < 1e-11
