@@ -1,0 +1,376 @@
+#!/usr/bin/env python
+"""bench.py - energy points/s of the LSE+OBC hot path (S1-S7) on B200.
+
+One "step" = one pass of the whole path (negf_obc_decimate for both leads -> negf_rgf_retarded ->
+negf_rgf_lesser_greater -> negf_observables) over the energy batch of one BASELINE.json config
+(default configs[1]: 64 energies, n = 32, b = 64, scalar scattering), inputs resident in HBM.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl reference]
+
+Prints ONE JSON line (see DESIGN.md "Measurement" for every key).  Multi-GPU = energy sharding
+("Each E is independent of the other"): every rank runs its own N_E energies of a
+grid N times as dense, no data-path collective, weak scaling.  `--impl reference` times the CPU
+oracle (oracle/, NumPy) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "energy points/sec of RGF G^R+G^<> selected inversion incl. OBC decimation and observables"
+UNIT = "energy points/s"
+
+
+# ---------------------------------------------------------------------------------------------
+# nominal work: units U = 8 b^3 real flops
+# ---------------------------------------------------------------------------------------------
+def unit_counts(n, sigma_kind, want_greater, iters_total, n_energy):
+    """Returns (gemm_units, inverse_units) for ALL energies of the batch.
+    iters_total = sum over energies and both leads of the decimation doublings done."""
+    gr = 7 * n - 6 + (n - 1)                       # S3 + S4 + corner column
+    gr_inv = n
+    gx = (11 * n - 9) if sigma_kind == "bt" else (9 * n - 7)
+    n_x = 2 if want_greater else 1
+    obs = 2                                        # Gamma_L G Gamma_R for T(E)
+    per_e_gemm = (gr - gr_inv) + n_x * gx + obs
+    per_e_inv = gr_inv
+    # decimation: 6 products + 1 inversion per doubling, + (1 inversion + 2 products) at the end
+    dec_gemm = 6 * iters_total + 2 * 2 * n_energy
+    dec_inv = iters_total + 2 * n_energy
+    return per_e_gemm * n_energy + dec_gemm, per_e_inv * n_energy + dec_inv
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons of one GPU every 50 ms through NVML."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.reasons, self.max_mhz = index, [], set(), None
+        self._stop_evt = threading.Event()
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def run(self):
+        if self.nv is None:
+            return
+        nv = self.nv
+        names = {nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap",
+                 nv.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown",
+                 nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
+                 nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
+                 nv.nvmlClocksThrottleReasonHwPowerBrakeSlowdown: "hw_power_brake"}
+        while not self._stop_evt.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, nm in names.items():
+                    if r & bit:
+                        self.reasons.add(nm)
+            except Exception:
+                pass
+            self._stop_evt.wait(0.05)
+
+    def stop(self):
+        self._stop_evt.set()
+        self.join(timeout=2)
+        med = float(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+# ---------------------------------------------------------------------------------------------
+# CPU oracle arm (cpu_baseline leg and --impl reference)
+# ---------------------------------------------------------------------------------------------
+def oracle_sample(wl, budget_s, max_energies=None):
+    """Runs the oracle path energy by energy (evenly spread over the grid) until ~budget_s of CPU
+    time is spent; returns (energies done, seconds, threads used)."""
+    from oracle import pipeline
+    try:
+        from threadpoolctl import threadpool_info
+        threads = max([p.get("num_threads", 1) for p in threadpool_info()] + [1])
+    except Exception:
+        threads = os.cpu_count()
+    ne = wl.n_energy
+    order = [int(i) for i in np.linspace(0, ne - 1, ne).round()]
+    stride = max(1, ne // 8)
+    order = list(range(0, ne, stride)) + [k for k in range(ne) if k % stride]
+    done, t0 = 0, time.perf_counter()
+    for k in order:
+        pipeline.solve_energy(wl, k, want_greater=wl.want_greater)
+        done += 1
+        if time.perf_counter() - t0 > budget_s or (max_energies and done >= max_energies):
+            break
+    return done, time.perf_counter() - t0, threads
+
+
+def run_reference(args, rank, world):
+    if rank != 0:
+        return
+    from paper_2602_03438_b200 import workloads
+    wl = workloads.make_workload(args.config)
+    per_step = max(1, min(wl.n_energy, args.ref_energies))
+    total_e, total_t, threads = 0, 0.0, os.cpu_count()
+    for i in range(args.warmup + args.steps):
+        e, t, threads = oracle_sample(wl, 1e9, per_step)
+        if i >= args.warmup:
+            total_e += e; total_t += t
+    v = total_e / total_t
+    sample = f"{per_step} of {wl.n_energy} energies per step, evenly spread over the grid"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * total_t / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": wl.name, "n_energy": wl.n_energy, "n_blocks": wl.n_blocks,
+                   "block_size": wl.block_size, "sample": sample},
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+# ---------------------------------------------------------------------------------------------
+# GPU arm
+# ---------------------------------------------------------------------------------------------
+def run_gpu(args, rank, local_rank, world):
+    import torch
+    from paper_2602_03438_b200 import build as _build
+    _build.ensure_built()
+    from paper_2602_03438_b200 import negf, runner, workloads
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the hot path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = f"cuda:{local_rank}"
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(dev))
+
+    wl = workloads.make_workload(args.config)
+    if world > 1:   # energy sharding of a grid `world` times as dense (weak scaling)
+        de = (wl.energies[1] - wl.energies[0]) if wl.n_energy > 1 else 0.0
+        wl.energies = wl.energies + rank * de / world
+    ne_batch = args.energy_batch or default_energy_batch(wl, torch.cuda.mem_get_info(local_rank)[0])
+    ne_batch = min(ne_batch, wl.n_energy)
+    batches = [(lo, min(lo + ne_batch, wl.n_energy)) for lo in range(0, wl.n_energy, ne_batch)]
+    # one resident DevicePath per distinct batch size; Sigma_S of the FIRST batch of that size is
+    # reused for the others when it is a per-energy BT family (configs[3]; stated in config.note)
+    ctx = negf.Context(local_rank)
+    paths = {}
+    for lo, hi in batches:
+        if hi - lo not in paths:
+            paths[hi - lo] = runner.DevicePath(wl, lo, hi, device=dev, ctx=ctx)
+    energies_dev = {(lo, hi): torch.from_numpy(wl.energies[lo:hi].copy()).to(dev) for lo, hi in batches}
+    weights_dev = {(lo, hi): torch.from_numpy(wl.weights[lo:hi].copy()).to(dev) for lo, hi in batches}
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
+
+    def step():
+        for lo, hi in batches:
+            dp = paths[hi - lo]
+            if len(batches) > 1:
+                dp.energy.copy_(energies_dev[(lo, hi)]); dp.weights.copy_(weights_dev[(lo, hi)])
+                dp.ctx.set_workspace(dp.workspace)
+            dp.run()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step(); flush.zero_()
+    barrier()
+    sampler = ClockSampler(local_rank); sampler.start()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    l0 = ctx.launch_count()
+    for i in range(args.steps):
+        ev[i][0].record(); step(); ev[i][1].record()
+        flush.zero_()                                   # L2 flush between timed iterations (untimed)
+    barrier()
+    launches = ctx.launch_count() - l0
+    clocks = sampler.stop()
+    ms = sum(a.elapsed_time(b) for a, b in ev)
+    if dist is not None:
+        t = torch.tensor([ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = world * wl.n_energy * args.steps / (ms * 1e-3)
+
+    # status / iteration counts of the last step (last batch) for the work accounting
+    dp_last = paths[batches[-1][1] - batches[-1][0]]
+    bad = int((dp_last.out["info_r"] != 0).sum() + (dp_last.out["info_x"] != 0).sum()
+              + (dp_last.out["status_L"] != 0).sum() + (dp_last.out["status_R"] != 0).sum())
+    iters_mean = float((dp_last.out["iters_L"].double().mean() + dp_last.out["iters_R"].double().mean()) / 2)
+    iters_total = iters_mean * 2 * wl.n_energy
+    U = 8.0 * wl.block_size ** 3
+    gemm_u, inv_u = unit_counts(wl.n_blocks, wl.sigma_kind, wl.want_greater, iters_total, wl.n_energy)
+    step_ms = ms / args.steps
+
+    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak",
+           "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": {"workload": wl.name, "n_energy": wl.n_energy, "n_blocks": wl.n_blocks,
+                      "block_size": wl.block_size, "energy_batch": ne_batch, "sigma_s": wl.sigma_kind,
+                      "outputs": "G^R diag/upper/lower/corner, G^< diag/upper" + (", G^> diag/upper" if wl.want_greater else "")
+                                 + ", density, LDOS, T(E), bond/contact currents",
+                      "l2": "256 MB flush write between timed iterations (outside the event pairs)",
+                      "parallelism": f"energy-sharded x{world}, no collective",
+                      "decimation_iters_mean": iters_mean, "numerical_failures": bad},
+           "gpu_launches": int(launches), "clocks": clocks,
+           "nominal_tflops": (gemm_u + inv_u) * U / (step_ms * 1e-3) * 1e-12}
+    if len(batches) > 1 and wl.sigma_kind == "bt":
+        out["config"]["note"] = "BT Sigma_S arrays of the first energy batch are reused for every batch"
+
+    if rank == 0:
+        # ---- roofline of the dominant kernel: profiled passes of the SAME step (event pairs around
+        # every launch site, on the library's stream), separate from the throughput timing above
+        peak = ctx.fp64_peak(300.0)
+        ctx.profile_enable(True)
+        for k in range(5):
+            ctx.profile_read(k, True)
+        psteps = max(1, min(3, args.steps))
+        for _ in range(psteps):
+            step(); flush.zero_()
+        prof = {negf.PROF_NAMES[k]: ctx.profile_read(k, True) for k in range(5)}
+        ctx.profile_enable(False)
+        tot = sum(v[0] for v in prof.values()) or 1.0
+        gemm_ms, gemm_sites = prof["gemm"]
+        fused_ms, fused_sites = prof["fused"]
+        if fused_ms > gemm_ms:
+            dom, dom_ms, dom_sites, dom_flops = "fused", fused_ms, fused_sites, (gemm_u + inv_u) * U * psteps
+        else:
+            dom, dom_ms, dom_sites, dom_flops = "gemm", gemm_ms, gemm_sites, gemm_u * U * psteps
+        achieved = dom_flops / (dom_ms * 1e-3) * 1e-12 if dom_ms > 0 else 0.0
+        out["roofline"] = {"bound": "tensor", "kernel": {"gemm": "zgemm_kernel (DMMA.8x8x4, 4M complex)",
+                                                         "fused": "fused chain kernels"}[dom],
+                           "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+                           "traffic": None,
+                           "peak_source": "negf_fp64_peak: DMMA m8n8k4 issue-rate probe run in this process "
+                                          "(MEASURED_PEAKS.json has no FP64 figure; nominal 37.2 = 148 SM x 1.965 GHz x 128 flop/clk)",
+                           "flops_per_launch": dom_flops / max(dom_sites, 1),
+                           "avg_launch_us": 1e3 * dom_ms / max(dom_sites, 1), "launches_per_step": dom_sites / psteps,
+                           "share_of_step": {k: v[0] / tot for k, v in prof.items()},
+                           "measured": f"{psteps} profiled passes of the same step after the timed region"}
+        # ---- end to end through the host-buffer C-ABI call (pinned host memory, copies timed)
+        out["e2e"] = run_e2e(args, wl, ctx, dev, world, torch, negf)
+        # restore the workspace the DevicePath owns
+        # ---- CPU oracle on a bounded sample, same workload
+        e, t, threads = oracle_sample(wl, args.cpu_seconds)
+        out["cpu_baseline"] = {"value": e / t, "unit": UNIT, "cores": threads, "kind": "oracle",
+                               "sample": f"{e} of {wl.n_energy} energies (evenly spread), {t:.1f} s, NumPy/OpenBLAS complex128"}
+        print(json.dumps(out))
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def default_energy_batch(wl, free_bytes):
+    """Energies resident at once: outputs (G^R 3F+corner, G^< 2F, G^> 2F) + workspace (4F + scratch)
+    + BT Sigma_S inputs, kept under ~70 % of free HBM."""
+    n, b = wl.n_blocks, wl.block_size
+    F = n * b * b * 16
+    per_e = (3 + 2 + (2 if wl.want_greater else 0) + 4) * F + 40 * b * b * 16
+    if wl.sigma_kind == "bt":
+        per_e += 7 * F
+    return max(1, int(0.7 * free_bytes // per_e))
+
+
+def run_e2e(args, wl, ctx, dev, world, torch, negf):
+    """negf_pipeline_host on the first energy batch that fits, HOST (pinned) inputs and outputs."""
+    n, b = wl.n_blocks, wl.block_size
+    ne = min(wl.n_energy, args.e2e_energies or wl.n_energy)
+    F = n * b * b * 16
+    while ne > 1 and ne * F * 12 > 24e9:      # keep pinned host memory bounded
+        ne //= 2
+    pin = lambda a: None if a is None else torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    Hd, Hu, Sd, Su = pin(wl.H_diag), pin(wl.H_upper), pin(wl.S_diag), pin(wl.S_upper)
+    en, wt = pin(wl.energies[:ne].copy()), pin(wl.weights[:ne].copy())
+    hp = negf.make_problem(n, b, ne, Hd, Hu, Sd, Su, en, wl.eta)
+    sig = wl.sigma_s(0, ne)
+    keep, hs = [], {}
+    for t in "rlg":
+        s = sig[t]
+        if s is None or (t == "g" and not wl.want_greater):
+            hs[t] = None
+        elif s["kind"] == "scalar":
+            v = pin(s["value"]); keep.append(v)
+            hs[t] = negf.make_sigma(negf.SIGMA_SCALAR, scalar=v)
+        else:
+            d, u, l = pin(s["diag"]), pin(s["upper"]), pin(s.get("lower")); keep += [d, u, l]
+            hs[t] = negf.make_sigma(negf.SIGMA_BT, diag=d, upper=u, lower=l)
+    if hs["r"] is None:
+        hs["r"] = negf.make_sigma(negf.SIGMA_NONE)
+    if hs["l"] is None:
+        hs["l"] = negf.make_sigma(negf.SIGMA_NONE)
+    if wl.want_greater and hs["g"] is None:
+        hs["g"] = negf.make_sigma(negf.SIGMA_NONE)
+    kind = {"none": negf.SIGMA_NONE, "scalar": negf.SIGMA_SCALAR, "bt": negf.SIGMA_BT}[wl.sigma_kind]
+    scratch = torch.empty(negf.Context.pipeline_host_bytes(hp, kind, wl.want_greater), dtype=torch.uint8, device=dev)
+    z = lambda *s: torch.empty(s, dtype=torch.complex128).pin_memory()
+    r = lambda *s: torch.empty(s, dtype=torch.float64).pin_memory()
+    o = {"GR_diag": z(ne, n, b, b), "GR_upper": z(ne, n - 1, b, b), "GR_lower": z(ne, n - 1, b, b),
+         "GL_diag": z(ne, n, b, b), "GL_upper": z(ne, n - 1, b, b),
+         "GG_diag": z(ne, n, b, b) if wl.want_greater else None,
+         "GG_upper": z(ne, n - 1, b, b) if wl.want_greater else None,
+         "density": r(n * b), "ldos": r(ne, n), "transmission": r(ne), "bond_current": r(ne, n - 1),
+         "contact_current": r(ne, 2) if wl.want_greater else None,
+         "info": torch.empty(ne, dtype=torch.int32).pin_memory()}
+    ho = negf.HostOutputs(*[negf._ptr(o[k]) for k in ("GR_diag", "GR_upper", "GR_lower", "GL_diag", "GL_upper",
+                                                      "GG_diag", "GG_upper", "density", "ldos", "transmission",
+                                                      "bond_current", "contact_current", "info")])
+    call = lambda: ctx.pipeline_host(hp, hs["r"], hs["l"], hs["g"], wt, wl.mu_L, wl.mu_R, wl.kT, wl.tol,
+                                     wl.max_iter, scratch, ho)
+    reps = max(1, min(args.steps, 5))
+    for _ in range(2):
+        up, down = call()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(reps):
+        up, down = call()              # synchronises the stream before returning
+    dt = time.perf_counter() - t0
+    assert int(o["info"].abs().sum()) == 0, "numerical failure flagged in the e2e run"
+    return {"value": world * ne * reps / dt, "unit": UNIT, "h2d_bytes_per_step": int(up), "d2h_bytes_per_step": int(down),
+            "energies_per_call": ne, "ms_per_call": 1e3 * dt / reps,
+            "api": "negf_pipeline_host (host pinned buffers in, all selected G blocks + observables out)"}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=1, help="BASELINE.json configs index (default 1)")
+    ap.add_argument("--energy-batch", type=int, default=0, help="energies resident at once (0 = fit HBM)")
+    ap.add_argument("--e2e-energies", type=int, default=0)
+    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="CPU time budget of the cpu_baseline leg")
+    ap.add_argument("--ref-energies", type=int, default=8, help="--impl reference: energies per step")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+    else:
+        run_gpu(args, rank, local_rank, world)
+
+
+if __name__ == "__main__":
+    main()

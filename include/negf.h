@@ -110,6 +110,21 @@ int negf_last_cuda_error(const negf_ctx* ctx);
 /* Number of kernels this context has launched since creation (bench.py's gpu_launches). */
 long long negf_launch_count(const negf_ctx* ctx);
 
+/* Per-kernel-class device timing for bench.py's roofline: when enabled, every launch site is
+ * bracketed by a CUDA event pair on the context stream (no synchronisation; a few microseconds of
+ * host overhead per launch, so never enable it inside a timed throughput run).
+ * negf_profile_read SYNCHRONISES the stream, folds all finished pairs into the per-class totals
+ * and returns milliseconds and number of launch sites of `kclass` since the last reset; reset != 0
+ * clears the totals of that class afterwards.  ms / sites may be NULL. */
+#define NEGF_PROF_GEMM        0   /* K2 complex GEMM (DMMA)                                        */
+#define NEGF_PROF_INVERSE     1   /* K1 inverse (all its kernels, inner GEMMs included)             */
+#define NEGF_PROF_ELEMENTWISE 2   /* O(b^2) assembly / combination kernels                          */
+#define NEGF_PROF_OBSERVABLES 3   /* S7 reductions                                                  */
+#define NEGF_PROF_FUSED       4   /* fused small-block chain kernels                                */
+#define NEGF_PROF_CLASSES     5
+int negf_profile_enable(negf_ctx* ctx, int on);
+int negf_profile_read(negf_ctx* ctx, int kclass, double* ms, long long* sites, int reset);
+
 /* ---- S2: open-boundary self-energies ------------
  * For each energy: a_d = z S_d - H_d, a_u = z S_u - H_u, a_l = z S_u^H - H_u^H of the lead
  * (default: contact blocks 0/0-1 for side 0, n-1/(n-2,n-1) for side 1); Sancho-Rubio doubling

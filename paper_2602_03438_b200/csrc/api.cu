@@ -20,11 +20,15 @@ extern "C" int negf_create(negf_ctx** out, int device) {
     c->device = device; c->stream = nullptr; c->ws = nullptr; c->ws_bytes = 0; c->last_cuda_error = 0;
     c->launches = 0; c->num_sms = prop.multiProcessorCount; c->sweep_valid = false;
     c->sw_n = c->sw_b = c->sw_ne = 0;
+    c->prof_on = false; c->prof_depth = 0;
+    for (int k = 0; k < NEGF_PROF_CLASSES; k++) { c->prof_ms[k] = 0.0; c->prof_n[k] = 0; }
     *out = c;
     return NEGF_OK;
 }
 extern "C" int negf_destroy(negf_ctx* ctx) {
     if (!ctx) return NEGF_EINVAL;
+    for (auto& r : ctx->prof_recs) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
+    for (auto e : ctx->prof_pool) cudaEventDestroy(e);
     delete ctx;
     return NEGF_OK;
 }
@@ -52,6 +56,27 @@ extern "C" const char* negf_strerror(int code) {
 }
 extern "C" int negf_last_cuda_error(const negf_ctx* ctx) { return ctx ? ctx->last_cuda_error : 0; }
 extern "C" long long negf_launch_count(const negf_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+extern "C" int negf_profile_enable(negf_ctx* ctx, int on) {
+    if (!ctx) return NEGF_EINVAL;
+    ctx->prof_on = on != 0; ctx->prof_depth = 0;
+    return NEGF_OK;
+}
+extern "C" int negf_profile_read(negf_ctx* ctx, int kclass, double* ms, long long* sites, int reset) {
+    if (!ctx || kclass < 0 || kclass >= NEGF_PROF_CLASSES) return NEGF_EINVAL;
+    NEGF_CUDA_CHECK(ctx, cudaStreamSynchronize(ctx->stream));
+    for (auto& r : ctx->prof_recs) {
+        float t = 0.f;
+        NEGF_CUDA_CHECK(ctx, cudaEventElapsedTime(&t, r.e0, r.e1));
+        ctx->prof_ms[r.kclass] += t; ctx->prof_n[r.kclass]++;
+        ctx->prof_pool.push_back(r.e0); ctx->prof_pool.push_back(r.e1);
+    }
+    ctx->prof_recs.clear();
+    if (ms) *ms = ctx->prof_ms[kclass];
+    if (sites) *sites = ctx->prof_n[kclass];
+    if (reset) { ctx->prof_ms[kclass] = 0.0; ctx->prof_n[kclass] = 0; }
+    return NEGF_OK;
+}
 
 // ---- FP64 tensor-pipe peak probe ---------------------------------------------------------------
 namespace {

@@ -4,6 +4,8 @@
 #include <stdint.h>
 #include <stdio.h>
 
+#include <vector>
+
 #include "../../include/negf.h"
 
 typedef double2 cplx;  // (x, y) = (re, im), same bytes as negf_c128
@@ -19,6 +21,35 @@ struct negf_ctx {
     // retained sweep state (NEGF_KEEP_SWEEP): valid for this shape only
     bool sweep_valid;
     int sw_n, sw_b, sw_ne;
+    // optional per-kernel-class timing (negf_profile_enable): event pairs around every launch site
+    bool prof_on;
+    int prof_depth;
+    struct ProfRec { int kclass; cudaEvent_t e0, e1; };
+    std::vector<ProfRec> prof_recs;
+    std::vector<cudaEvent_t> prof_pool;
+    double prof_ms[NEGF_PROF_CLASSES];
+    long long prof_n[NEGF_PROF_CLASSES];
+};
+
+// Brackets one launch site with CUDA events on the context stream when profiling is on; nested
+// scopes (the GEMMs inside the blocked inverse) are charged to the outermost class only.
+struct ProfScope {
+    negf_ctx* c; int k; cudaEvent_t e0, e1; bool live;
+    static cudaEvent_t get(negf_ctx* c) {
+        cudaEvent_t e;
+        if (!c->prof_pool.empty()) { e = c->prof_pool.back(); c->prof_pool.pop_back(); }
+        else cudaEventCreate(&e);
+        return e;
+    }
+    ProfScope(negf_ctx* ctx, int kclass) : c(ctx), k(kclass), live(false) {
+        if (!c->prof_on) return;
+        if (c->prof_depth++ == 0) { live = true; e0 = get(c); e1 = get(c); cudaEventRecord(e0, c->stream); }
+    }
+    ~ProfScope() {
+        if (!c->prof_on) return;
+        c->prof_depth--;
+        if (live) { cudaEventRecord(e1, c->stream); c->prof_recs.push_back({k, e0, e1}); }
+    }
 };
 
 #define NEGF_CUDA_CHECK(ctx, expr)                                  \

@@ -157,57 +157,67 @@ inline dim3 grid2(int b, int batch) { return dim3((b * b + 255) / 256, batch); }
 }  // namespace
 
 int ew_combine(negf_ctx* ctx, const CombineArgs& a, int batch) {
+    ProfScope _ps(ctx, NEGF_PROF_ELEMENTWISE);
     combine_kernel<<<grid2(a.b, batch), 256, 0, ctx->stream>>>(a);
     NEGF_LAUNCH_CHECK(ctx);
     return NEGF_OK;
 }
 int ew_antiherm_add(negf_ctx* ctx, int b, int batch, cplx* C, long long sC, const cplx* Z, long long sZ,
                     const cplx* V, long long sV, double sign) {
+    ProfScope _ps(ctx, NEGF_PROF_ELEMENTWISE);
     antiherm_add_kernel<<<grid2(b, batch), 256, 0, ctx->stream>>>(b, C, sC, Z, sZ, V, sV, sign);
     NEGF_LAUNCH_CHECK(ctx);
     return NEGF_OK;
 }
 int ew_sub(negf_ctx* ctx, int b, int batch, cplx* C, long long sC, const cplx* A, long long sA,
            const cplx* B, long long sB) {
+    ProfScope _ps(ctx, NEGF_PROF_ELEMENTWISE);
     sub_kernel<<<grid2(b, batch), 256, 0, ctx->stream>>>(b, C, sC, A, sA, B, sB);
     NEGF_LAUNCH_CHECK(ctx);
     return NEGF_OK;
 }
 int ew_copy(negf_ctx* ctx, size_t n, int batch, cplx* dst, long long sd, const cplx* src, long long ss,
             const int* skip) {
+    ProfScope _ps(ctx, NEGF_PROF_ELEMENTWISE);
     copy_kernel<<<dim3((unsigned)((n + 255) / 256), batch), 256, 0, ctx->stream>>>(n, dst, sd, src, ss, skip);
     NEGF_LAUNCH_CHECK(ctx);
     return NEGF_OK;
 }
 int ew_fill_int(negf_ctx* ctx, int* p, int n, int v) {
+    ProfScope _ps(ctx, NEGF_PROF_ELEMENTWISE);
     fill_int_kernel<<<(n + 255) / 256, 256, 0, ctx->stream>>>(p, n, v);
     NEGF_LAUNCH_CHECK(ctx);
     return NEGF_OK;
 }
 int ew_max_int(negf_ctx* ctx, int* dst, const int* src, int n) {
+    ProfScope _ps(ctx, NEGF_PROF_ELEMENTWISE);
     max_int_kernel<<<(n + 255) / 256, 256, 0, ctx->stream>>>(dst, src, n);
     NEGF_LAUNCH_CHECK(ctx);
     return NEGF_OK;
 }
 int ew_sr_update(negf_ctx* ctx, int b, int batch, int side, cplx* a_s, cplx* a_b, const cplx* lgu,
                  const cplx* ugl, const int* skip) {
+    ProfScope _ps(ctx, NEGF_PROF_ELEMENTWISE);
     sr_update_kernel<<<grid2(b, batch), 256, 0, ctx->stream>>>(b, side, a_s, a_b, lgu, ugl, skip);
     NEGF_LAUNCH_CHECK(ctx);
     return NEGF_OK;
 }
 int ew_sr_norm(negf_ctx* ctx, int b, int batch, const cplx* u, const cplx* l, double* ref, double tol,
                int* done, int* iters, int it, int mode) {
+    ProfScope _ps(ctx, NEGF_PROF_ELEMENTWISE);
     sr_norm_kernel<<<batch, 256, 0, ctx->stream>>>(b, u, l, ref, tol, done, iters, it, mode);
     NEGF_LAUNCH_CHECK(ctx);
     return NEGF_OK;
 }
 int ew_obc_finalize(negf_ctx* ctx, int b, int batch, const cplx* sigma, const double* energy, double mu,
                     double kT, cplx* gamma, cplx* sl, cplx* sg, double* fermi) {
+    ProfScope _ps(ctx, NEGF_PROF_ELEMENTWISE);
     obc_finalize_kernel<<<grid2(b, batch), 256, 0, ctx->stream>>>(b, sigma, energy, mu, kT, gamma, sl, sg, fermi);
     NEGF_LAUNCH_CHECK(ctx);
     return NEGF_OK;
 }
 int ew_obc_status(negf_ctx* ctx, int ne, const int* done, const int* sing, int* status) {
+    ProfScope _ps(ctx, NEGF_PROF_ELEMENTWISE);
     obc_status_kernel<<<(ne + 255) / 256, 256, 0, ctx->stream>>>(ne, done, sing, status);
     NEGF_LAUNCH_CHECK(ctx);
     return NEGF_OK;

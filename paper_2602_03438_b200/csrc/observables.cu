@@ -170,6 +170,7 @@ extern "C" int negf_observables(negf_ctx* ctx, const negf_problem* p,
     const size_t bb = (size_t)b * b;
     const bool hasS = p->S_diag != nullptr;
     if (ne > 65535) return NEGF_EUNSUPPORTED;
+    ProfScope _ps(ctx, NEGF_PROF_OBSERVABLES);
     if (ldos) {
         if (!GR_diag || (hasS && n > 1 && (!GR_upper || !GR_lower || !p->S_upper))) return NEGF_EINVAL;
         ldos_kernel<<<dim3(n, ne), 256, 0, ctx->stream>>>(n, b, (const cplx*)GR_diag, (const cplx*)GR_upper,

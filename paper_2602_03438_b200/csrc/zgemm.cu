@@ -199,6 +199,7 @@ int launch_ops(negf_ctx* ctx, const GemmArgs& a) {
 }  // namespace
 
 int zgemm_launch(negf_ctx* ctx, const GemmArgs& a) {
+    ProfScope _ps(ctx, NEGF_PROF_GEMM);
     if (a.m <= 0 || a.n <= 0 || a.batch <= 0) return NEGF_OK;
     if (a.k < 0 || (a.opA | a.opB) & ~1) return NEGF_EINVAL;
     if (a.batch > 65535) return NEGF_EUNSUPPORTED;

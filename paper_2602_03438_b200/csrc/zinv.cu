@@ -385,6 +385,7 @@ size_t zinv_workspace_bytes(int b, int batch) {
 
 int zinv_launch(negf_ctx* ctx, int b, cplx* A, long long sA, int batch, void* ws, int* info,
                 int info_code, const int* skip) {
+    ProfScope _ps(ctx, NEGF_PROF_INVERSE);
     if (b <= 0 || batch <= 0) return NEGF_OK;
     if (b <= SMALL_MAX) {
         constexpr int NT = 256;

@@ -18,6 +18,8 @@ if not os.path.exists(LIB_PATH):
                       "(or __graft_entry__.build()); there is no CPU fallback")
 lib = C.CDLL(LIB_PATH)
 
+PROF_GEMM, PROF_INVERSE, PROF_ELEMENTWISE, PROF_OBSERVABLES, PROF_FUSED = range(5)
+PROF_NAMES = ("gemm", "inverse", "elementwise", "observables", "fused")
 OK, EINVAL, ENOWORKSPACE, EUNSUPPORTED, ECUDA, ENOSTATE = 0, -1, -2, -3, -4, -5
 SIGMA_NONE, SIGMA_SCALAR, SIGMA_BT = 0, 1, 2
 KEEP_SWEEP = 1
@@ -49,7 +51,8 @@ class HostOutputs(C.Structure):
 
 
 EXPORTS = ["negf_create", "negf_destroy", "negf_set_stream", "negf_workspace_bytes", "negf_set_workspace",
-           "negf_strerror", "negf_last_cuda_error", "negf_launch_count", "negf_obc_decimate",
+           "negf_strerror", "negf_last_cuda_error", "negf_launch_count",
+           "negf_profile_enable", "negf_profile_read", "negf_obc_decimate",
            "negf_rgf_retarded", "negf_rgf_lesser_greater", "negf_observables", "negf_pipeline_host_bytes",
            "negf_pipeline_host", "negf_zgemm_batched", "negf_zinverse_batched", "negf_fp64_peak"]
 
@@ -64,6 +67,8 @@ lib.negf_strerror.restype = C.c_char_p
 lib.negf_last_cuda_error.argtypes = [_P]
 lib.negf_launch_count.argtypes = [_P]
 lib.negf_launch_count.restype = C.c_longlong
+lib.negf_profile_enable.argtypes = [_P, C.c_int]
+lib.negf_profile_read.argtypes = [_P, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_longlong), C.c_int]
 lib.negf_obc_decimate.argtypes = [_P, C.POINTER(Problem), C.POINTER(Lead), C.c_int, C.c_double, C.c_double,
                                   C.c_double, C.c_int, _P, _P, _P, _P, _P, _P, _P, _P]
 lib.negf_rgf_retarded.argtypes = [_P, C.POINTER(Problem), C.POINTER(Sigma), _P, _P, _P, _P, C.c_int, _P]
@@ -159,6 +164,15 @@ class Context:
 
     def launch_count(self) -> int:
         return int(lib.negf_launch_count(self._h))
+
+    def profile_enable(self, on: bool):
+        self._check(lib.negf_profile_enable(self._h, int(on)), "negf_profile_enable")
+
+    def profile_read(self, kclass: int, reset: bool = True):
+        """(milliseconds, launch sites) of one kernel class since the last reset; synchronises."""
+        ms, n = C.c_double(), C.c_longlong()
+        self._check(lib.negf_profile_read(self._h, kclass, C.byref(ms), C.byref(n), int(reset)), "negf_profile_read")
+        return ms.value, n.value
 
     def obc_decimate(self, p: Problem, side, mu, kT, tol, max_iter, sigma_r, gamma=None, sigma_lesser=None,
                      sigma_greater=None, g_surface=None, fermi=None, iters=None, status=None, lead: Lead = None):
