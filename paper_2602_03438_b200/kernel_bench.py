@@ -1,0 +1,83 @@
+"""Micro-benchmarks of the K1/K2 building blocks through the C ABI:
+
+    python -m paper_2602_03438_b200.kernel_bench --kernel zgemm --b 1024 --batch 16 [--opA 0 --opB 1]
+    python -m paper_2602_03438_b200.kernel_bench --kernel zinv  --b 1024 --batch 16
+    python -m paper_2602_03438_b200.kernel_bench --kernel peak
+
+Prints one JSON line per run: achieved FP64 TFLOP/s (8 b^3 real flops per complex product or
+inversion, the unit U of SURVEY.md 8(d)) and the fraction of the DMMA issue-rate peak probed in
+the same process.  Timing: CUDA events on the library's stream, 3 warm-ups, operands rotated over
+several buffers so consecutive launches do not reuse L2 lines when the set is larger than L2.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+
+import torch
+
+from . import build as _build
+
+_build.ensure_built()
+from . import negf  # noqa: E402
+
+
+def _rand(shape, gen):
+    return torch.complex(torch.randn(shape, dtype=torch.float64, device="cuda", generator=gen),
+                         torch.randn(shape, dtype=torch.float64, device="cuda", generator=gen))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--kernel", default="zgemm", choices=["zgemm", "zinv", "peak"])
+    ap.add_argument("--b", type=int, default=1024)
+    ap.add_argument("--batch", type=int, default=16)
+    ap.add_argument("--opA", type=int, default=0)
+    ap.add_argument("--opB", type=int, default=0)
+    ap.add_argument("--reps", type=int, default=10)
+    ap.add_argument("--sets", type=int, default=2, help="operand sets rotated between launches")
+    args = ap.parse_args()
+    ctx = negf.Context(0)
+    st = torch.cuda.current_stream()
+    ctx.set_stream(st.cuda_stream)
+    peak = ctx.fp64_peak(200.0)
+    if args.kernel == "peak":
+        print(json.dumps({"kernel": "dmma_peak_probe", "tflops": peak}))
+        return
+    b, batch = args.b, args.batch
+    gen = torch.Generator(device="cuda"); gen.manual_seed(1)
+    flops = 8.0 * b ** 3 * batch
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if args.kernel == "zgemm":
+        sets = [(_rand((batch, b, b), gen), _rand((batch, b, b), gen), torch.empty(batch, b, b, dtype=torch.complex128, device="cuda"))
+                for _ in range(args.sets)]
+        run = lambda i: ctx.zgemm_batched(args.opA, args.opB, b, b, b, 1.0, sets[i][0], b, b * b, sets[i][1], b, b * b,
+                                          0.0, None, sets[i][2], b, b * b, batch)
+    else:
+        p = negf.Problem(2, b, batch, None, None, None, None, None, 0.0)
+        ws = torch.empty(negf.Context.workspace_bytes(p), dtype=torch.uint8, device="cuda")
+        ctx.set_workspace(ws)
+        eye = torch.eye(b, dtype=torch.complex128, device="cuda")
+        src = [_rand((batch, b, b), gen) / b ** 0.5 + 0.5 * eye for _ in range(args.sets)]
+        work = [s.clone() for s in src]
+        info = torch.zeros(batch, dtype=torch.int32, device="cuda")
+        run = lambda i: ctx.zinverse_batched(b, work[i], b * b, batch, info)
+    for i in range(3):
+        run(i % args.sets)
+    torch.cuda.synchronize()
+    times = []
+    for r in range(args.reps):
+        i = r % args.sets
+        if args.kernel == "zinv":
+            work[i].copy_(src[i])
+        e0.record(st); run(i); e1.record(st)
+        torch.cuda.synchronize()
+        times.append(e0.elapsed_time(e1))
+    ms = sorted(times)[len(times) // 2]
+    print(json.dumps({"kernel": args.kernel, "b": b, "batch": batch, "opA": args.opA, "opB": args.opB,
+                      "ms_median": ms, "ms_best": min(times), "tflops": flops / (ms * 1e-3) * 1e-12,
+                      "peak_tflops": peak, "frac": flops / (ms * 1e-3) * 1e-12 / peak}))
+
+
+if __name__ == "__main__":
+    main()
