@@ -34,77 +34,204 @@ constexpr int CMAX = 8;            // portable cluster size
 constexpr int PANEL_SMEM_ROWS_BYTES = 176 * 1024;   // + 9 KB exchange buffers + 33 KB static < 227 KB
 
 // ------------------------------------------------------------------------------------------------
-// small path
+// small path: REGISTER-resident Gauss-Jordan, one CTA of 8 warps per matrix (b <= 96).
+//   * warp w owns the columns j = w + 8 c (c < CB), lane l the rows i = l + 32 r (r < RB): the
+//     whole matrix lives in registers (RB x CB elements per thread);
+//   * the pivot search of column k is done by its owner warp alone with three redux.sync on the
+//     bit pattern of |re|+|im| (monotone for non-negative doubles), which then publishes the
+//     multiplier column, the pivot index and 1/pivot to shared memory;
+//   * ONE block barrier per column; the two rows that trade places travel inside each warp
+//     through a per-warp shared-memory line (no block-level traffic);
+//   * look-ahead: the owner of column k+1 updates that column first, searches its pivot and
+//     publishes it BEFORE finishing its update for column k, so the barrier of column k+1 never
+//     waits for a pivot search;
+//   * the rank-1 update runs out of registers at the DFMA rate (= the DMMA rate on sm_100).
+// Rows/columns >= b are padded with the identity and never reached.
 // ------------------------------------------------------------------------------------------------
-template <int NT>
-__global__ void __launch_bounds__(NT) gj_small_kernel(cplx* A, long long sA, int b, int* info, int code,
-                                                      const int* skip) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+constexpr int GJ_NW = 8;
+
+
+__device__ __forceinline__ cplx crecip_fast(cplx a) {      // pivots are O(1): no overflow guard needed
+    const double inv = 1.0 / fma(a.x, a.x, a.y * a.y);
+    return cmake(a.x * inv, -a.y * inv);
+}
+
+struct GjShared {            // pointers into the kernel's shared memory
+    cplx* colbuf;            // [2][NR]
+    cplx* wrow;              // this warp's [2][2][CB]
+    cplx* s_d; int* s_p; int* piv; int* s_sing;
+};
+
+// pivot search + publication of column kn, held in slot C of the calling (owner) warp
+template <int RB, int CB, int C>
+__device__ __forceinline__ void gj_owner(const cplx (&m)[RB][CB], const GjShared& sh, int kn, int b, int lane) {
+    constexpr int NR = RB * 32;
+    const int parn = kn & 1;
+    unsigned long long key = 0ull;
+    int bi = 0x7fffffff;
+#pragma unroll
+    for (int r = 0; r < RB; r++) {
+        const int i = lane + 32 * r;
+        sh.colbuf[parn * NR + i] = m[r][C];
+        if (i >= kn && i < b) {
+            const unsigned long long kq = (unsigned long long)__double_as_longlong(cabs1(m[r][C]));
+            if (bi == 0x7fffffff || kq > key) { key = kq; bi = i; }
+        }
+    }
+    const bool has = bi != 0x7fffffff;
+    const unsigned hi = __reduce_max_sync(0xffffffffu, has ? (unsigned)(key >> 32) : 0u);
+    const bool mh = has && (unsigned)(key >> 32) == hi;
+    const unsigned lo = __reduce_max_sync(0xffffffffu, mh ? (unsigned)key : 0u);
+    const bool ml = mh && (unsigned)key == lo;
+    const unsigned p = __reduce_min_sync(0xffffffffu, ml ? (unsigned)bi : 0x7fffffffu);
+    cplx pv = cmake(0.0, 0.0);
+#pragma unroll
+    for (int r = 0; r < RB; r++) if (lane + 32 * r == (int)p) pv = m[r][C];
+    pv.x = __shfl_sync(0xffffffffu, pv.x, p & 31);
+    pv.y = __shfl_sync(0xffffffffu, pv.y, p & 31);
+    const bool sing = (hi == 0u && lo == 0u);
+    if (lane == 0) {
+        sh.s_p[parn] = (int)p; sh.piv[kn] = (int)p;
+        sh.s_d[parn] = sing ? cmake(1.0, 0.0) : crecip_fast(pv);
+        if (sing && *sh.s_sing == 0) *sh.s_sing = kn + 1;
+    }
+}
+
+// Rank-1 update of column slot C: m[:, C] -= mult * sr.  The special rows/columns were prepared by
+// the caller so that this one formula is right everywhere (pivot row: m = 0, mult = -1 -> sr;
+// pivot column: m = 0, sr = 1/pivot -> -mult/pivot).
+template <int RB, int CB, int C>
+__device__ __forceinline__ void gj_update(cplx (&m)[RB][CB], const cplx (&mult)[RB], const cplx (&sr)[CB]) {
+#pragma unroll
+    for (int r = 0; r < RB; r++) cfms(m[r][C], mult[r], sr[C]);
+}
+
+template <int RB, int CB, int C>
+__device__ __forceinline__ void gj_update_rest(cplx (&m)[RB][CB], const cplx (&mult)[RB], const cplx (&sr)[CB], int done) {
+    if constexpr (C < CB) {
+        if (C != done) gj_update<RB, CB, C>(m, mult, sr);
+        gj_update_rest<RB, CB, C + 1>(m, mult, sr, done);
+    }
+}
+
+// all columns k = CK*8 + wk, wk < 8, then recurse to CK + 1
+template <int RB, int CB, int CK>
+__device__ __forceinline__ void gj_columns(cplx (&m)[RB][CB], const GjShared& sh, int b, int warp, int lane) {
+    if constexpr (CK < CB) {
+        constexpr int NR = RB * 32;
+        constexpr int CN = (CK + 1 < CB) ? CK + 1 : CK;
+#pragma unroll 1
+        for (int wk = 0; wk < GJ_NW; wk++) {
+            const int k = CK * GJ_NW + wk;
+            if (k >= b) break;
+            const int par = k & 1;
+            __syncthreads();
+            const int p = sh.s_p[par];
+            const cplx d = sh.s_d[par];
+            cplx* wr = sh.wrow + par * 2 * CB;
+            // the two rows that trade places, through this warp's shared-memory line
+#pragma unroll
+            for (int r = 0; r < RB; r++) {
+                const int i = lane + 32 * r;
+                if (i == p) {
+#pragma unroll
+                    for (int c = 0; c < CB; c++) wr[c] = m[r][c];
+                }
+                if (i == k && p != k) {
+#pragma unroll
+                    for (int c = 0; c < CB; c++) wr[CB + c] = m[r][c];
+                }
+            }
+            __syncwarp();
+            cplx mult[RB];
+#pragma unroll
+            for (int r = 0; r < RB; r++) {
+                const int i = lane + 32 * r;
+                mult[r] = sh.colbuf[par * NR + ((i == p) ? k : i)];   // row p inherits old row k's multiplier
+                if (i == p && p != k) {
+#pragma unroll
+                    for (int c = 0; c < CB; c++) m[r][c] = wr[CB + c];
+                }
+                if (i == k) {
+                    mult[r] = cmake(-1.0, 0.0);
+#pragma unroll
+                    for (int c = 0; c < CB; c++) m[r][c] = cmake(0.0, 0.0);
+                }
+            }
+            cplx sr[CB];
+#pragma unroll
+            for (int c = 0; c < CB; c++) sr[c] = cmul(wr[c], d);
+            if (warp == wk) {            // this warp's slot CK IS column k
+                sr[CK] = d;
+#pragma unroll
+                for (int r = 0; r < RB; r++) m[r][CK] = cmake(0.0, 0.0);
+            }
+            // look-ahead: the owner of column k+1 brings that column up to date and publishes it first
+            int done = -1;
+            if (k + 1 < b && warp == ((wk + 1) & (GJ_NW - 1))) {
+                if (wk < GJ_NW - 1) {
+                    gj_update<RB, CB, CK>(m, mult, sr);
+                    gj_owner<RB, CB, CK>(m, sh, k + 1, b, lane);
+                    done = CK;
+                } else if (CK + 1 < CB) {
+                    gj_update<RB, CB, CN>(m, mult, sr);
+                    gj_owner<RB, CB, CN>(m, sh, k + 1, b, lane);
+                    done = CN;
+                }
+            }
+            gj_update_rest<RB, CB, 0>(m, mult, sr, done);
+        }
+        gj_columns<RB, CB, CK + 1>(m, sh, b, warp, lane);
+    }
+}
+
+template <int RB, int CB>
+__global__ void __launch_bounds__(GJ_NW * 32) gj_reg_kernel(cplx* A, long long sA, int b, int* info, int code,
+                                                            const int* skip) {
+    constexpr int NR = RB * 32, NC = CB * GJ_NW;
     const int e = blockIdx.x;
     if (skip && skip[e]) return;
-    const int ld = b + 1;
-    cplx* M = reinterpret_cast<cplx*>(smem_raw);       // [b][ld]
-    cplx* rowbuf = M + (size_t)b * ld;                  // [b]
-    cplx* colbuf = rowbuf + b;                          // [b]
-    int* piv = reinterpret_cast<int*>(colbuf + b);      // [b]
-    __shared__ double red_val[32];
-    __shared__ int red_idx[32];
-    __shared__ int s_p;
+    __shared__ cplx colbuf[2 * NR];
+    __shared__ cplx wrow[GJ_NW][2 * 2 * CB];     // [warp][parity][pivot row | row k][slot]
+    __shared__ cplx s_d[2];
+    __shared__ int s_p[2];
+    __shared__ int piv[NC];
+    __shared__ int dest[NC];
     __shared__ int s_sing;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     cplx* g = A + (size_t)e * sA;
-    const int tid = threadIdx.x;
-    for (int idx = tid; idx < b * b; idx += NT) M[(idx / b) * ld + idx % b] = g[idx];
+    cplx m[RB][CB];
+#pragma unroll
+    for (int r = 0; r < RB; r++)
+#pragma unroll
+        for (int c = 0; c < CB; c++) {
+            const int i = lane + 32 * r, j = warp + GJ_NW * c;
+            m[r][c] = (i < b && j < b) ? g[(size_t)i * b + j] : cmake(i == j ? 1.0 : 0.0, 0.0);
+        }
     if (tid == 0) s_sing = 0;
     __syncthreads();
-    for (int k = 0; k < b; k++) {
-        // pivot search over rows >= k
-        double best = -1.0; int bi = k;
-        for (int r = k + tid; r < b; r += NT) {
-            double v = cabs1(M[r * ld + k]);
-            if (v > best) { best = v; bi = r; }
-        }
-        for (int o = 16; o > 0; o >>= 1) {
-            double ov = __shfl_down_sync(0xffffffffu, best, o);
-            int oi = __shfl_down_sync(0xffffffffu, bi, o);
-            if (ov > best || (ov == best && oi < bi)) { best = ov; bi = oi; }
-        }
-        if ((tid & 31) == 0) { red_val[tid >> 5] = best; red_idx[tid >> 5] = bi; }
-        __syncthreads();
-        if (tid == 0) {
-            for (int wv = 1; wv < NT / 32; wv++)
-                if (red_val[wv] > best || (red_val[wv] == best && red_idx[wv] < bi)) { best = red_val[wv]; bi = red_idx[wv]; }
-            s_p = bi; piv[k] = bi;
-            if (!(best > 0.0) && s_sing == 0) s_sing = k + 1;
-        }
-        __syncthreads();
-        const int p = s_p;
-        if (p != k) for (int j = tid; j < b; j += NT) { cplx t = M[k * ld + j]; M[k * ld + j] = M[p * ld + j]; M[p * ld + j] = t; }
-        __syncthreads();
-        cplx pv = M[k * ld + k];
-        cplx d = (pv.x == 0.0 && pv.y == 0.0) ? cmake(1.0, 0.0) : crecip(pv);
-        for (int j = tid; j < b; j += NT) {
-            rowbuf[j] = cmul(M[k * ld + j], d);
-            colbuf[j] = M[j * ld + k];
-        }
-        __syncthreads();
-        for (int idx = tid; idx < b * b; idx += NT) {
-            int i = idx / b, j = idx % b;
-            cplx v;
-            if (i == k) v = (j == k) ? d : rowbuf[j];
-            else if (j == k) v = cneg(cmul(colbuf[i], d));
-            else { v = M[i * ld + j]; cfms(v, colbuf[i], rowbuf[j]); }
-            M[i * ld + j] = v;
-        }
-        __syncthreads();
-    }
-    // undo the row permutation as column swaps in reverse order: A^-1 = (P A)^-1 P
-    for (int r = tid; r < b; r += NT)
-        for (int k = b - 1; k >= 0; k--) {
-            int p = piv[k];
-            if (p != k) { cplx t = M[r * ld + k]; M[r * ld + k] = M[r * ld + p]; M[r * ld + p] = t; }
-        }
+    GjShared sh{colbuf, wrow[warp], s_d, s_p, piv, &s_sing};
+    if (warp == 0) gj_owner<RB, CB, 0>(m, sh, 0, b, lane);
+    gj_columns<RB, CB, 0>(m, sh, b, warp, lane);
     __syncthreads();
-    for (int idx = tid; idx < b * b; idx += NT) g[idx] = M[(idx / b) * ld + idx % b];
+    // A^-1 = (P A)^-1 P: column j of the result is column src[j] of M, src = the recorded swaps
+    // applied in reverse order to the identity; every thread scatters its columns to src^-1.
+    if (tid == 0) {
+        for (int c = 0; c < b; c++) dest[c] = c;
+        for (int k = b - 1; k >= 0; k--) {
+            const int p = piv[k];
+            if (p != k) { int t = dest[k]; dest[k] = dest[p]; dest[p] = t; }
+        }
+        for (int c = 0; c < b; c++) piv[dest[c]] = c;     // piv now holds src^-1
+    }
+    __syncthreads();
+#pragma unroll
+    for (int r = 0; r < RB; r++)
+#pragma unroll
+        for (int c = 0; c < CB; c++) {
+            const int i = lane + 32 * r, j = warp + GJ_NW * c;
+            if (i < b && j < b) g[(size_t)i * b + piv[j]] = m[r][c];
+        }
     if (tid == 0 && s_sing && info) info[e] = code > 0 ? code : s_sing;
 }
 
@@ -388,15 +515,12 @@ int zinv_launch(negf_ctx* ctx, int b, cplx* A, long long sA, int batch, void* ws
     ProfScope _ps(ctx, NEGF_PROF_INVERSE);
     if (b <= 0 || batch <= 0) return NEGF_OK;
     if (b <= SMALL_MAX) {
-        constexpr int NT = 256;
-        size_t smem = ((size_t)b * (b + 1) + 2 * b) * sizeof(cplx) + (size_t)b * sizeof(int);
-        static bool small_attr_done = false;
-        if (!small_attr_done) {
-            NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_small_kernel<NT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                                      (int)(((size_t)SMALL_MAX * (SMALL_MAX + 3)) * sizeof(cplx) + SMALL_MAX * 4)));
-            small_attr_done = true;
-        }
-        gj_small_kernel<NT><<<batch, NT, smem, ctx->stream>>>(A, sA, b, info, info_code, skip);
+        if (b <= 16)      gj_reg_kernel<1, 2><<<batch, GJ_NW * 32, 0, ctx->stream>>>(A, sA, b, info, info_code, skip);
+        else if (b <= 32) gj_reg_kernel<1, 4><<<batch, GJ_NW * 32, 0, ctx->stream>>>(A, sA, b, info, info_code, skip);
+        else if (b <= 48) gj_reg_kernel<2, 6><<<batch, GJ_NW * 32, 0, ctx->stream>>>(A, sA, b, info, info_code, skip);
+        else if (b <= 64) gj_reg_kernel<2, 8><<<batch, GJ_NW * 32, 0, ctx->stream>>>(A, sA, b, info, info_code, skip);
+        else if (b <= 80) gj_reg_kernel<3, 10><<<batch, GJ_NW * 32, 0, ctx->stream>>>(A, sA, b, info, info_code, skip);
+        else              gj_reg_kernel<3, 12><<<batch, GJ_NW * 32, 0, ctx->stream>>>(A, sA, b, info, info_code, skip);
         NEGF_LAUNCH_CHECK(ctx);
         return NEGF_OK;
     }
