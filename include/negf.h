@@ -141,6 +141,20 @@ int negf_obc_decimate(negf_ctx* ctx, const negf_problem* p, const negf_lead* lea
                       negf_c128* sigma_lesser, negf_c128* sigma_greater,
                       negf_c128* g_surface, double* fermi, int* iters, int* status);
 
+/* Both leads in one call (K3, the energy-batch scheduler): for block sizes up to 128 the left and
+ * right decimations of all energies run as ONE batch of 2 N_E entries, so every launch carries
+ * twice the work; above that the two leads run one after the other.  Same results as two
+ * negf_obc_decimate calls.  Members of negf_obc_out as the like-named arguments above
+ * (sigma_r, iters, status required; the others may be NULL). */
+typedef struct {
+    negf_c128 *sigma_r, *gamma, *sigma_lesser, *sigma_greater, *g_surface;
+    double* fermi;
+    int *iters, *status;
+} negf_obc_out;
+int negf_obc_decimate_pair(negf_ctx* ctx, const negf_problem* p, const negf_lead* lead_L /* or NULL */,
+                           const negf_lead* lead_R /* or NULL */, double mu_L, double mu_R, double kT,
+                           double tol, int max_iter, const negf_obc_out* left, const negf_obc_out* right);
+
 /* ---- S1+S3+S4: retarded selected inversion ----------
  *   g_0 = A_00^-1; g_i = (A_ii - A_{i,i-1} g_{i-1} A_{i-1,i})^-1;
  *   G_{n-1,n-1} = g_{n-1}; X_i = g_i A_{i,i+1}; Y_i = A_{i+1,i} g_i;

@@ -123,6 +123,12 @@ struct GemmArgs {
     const int* skip;         // optional [batch] device mask: entry skipped when skip[e] != 0
 };
 int zgemm_launch(negf_ctx* ctx, const GemmArgs& a);
+// several independent products of identical shape / ops / batch in ONE launch (blockIdx.z = member)
+constexpr int NEGF_GEMM_GROUP_MAX = 4;
+struct GemmGroup { GemmArgs g[NEGF_GEMM_GROUP_MAX]; int ng; };
+int zgemm_launch_group(negf_ctx* ctx, const GemmGroup& grp);
+GemmArgs zgemm_bb_args(int opA, int opB, int b, cplx alpha, const cplx* A, long long sA, const cplx* B, long long sB,
+                       cplx beta, const cplx* D, long long sD, cplx* C, long long sC, int batch, const int* skip);
 // convenience: square b x b x b, contiguous blocks
 int zgemm_bb(negf_ctx* ctx, int opA, int opB, int b, cplx alpha, const cplx* A, long long sA,
              const cplx* B, long long sB, cplx beta, const cplx* D, long long sD,

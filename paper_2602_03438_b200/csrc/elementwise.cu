@@ -81,8 +81,8 @@ __global__ void max_int_kernel(int* dst, const int* src, int n) {
     if (i < n) { int a = dst[i], s = src[i]; if (a == 0) dst[i] = s; }
 }
 
-// a_s -= (side ? ugl : lgu) ; a_b -= ugl + lgu
-__global__ void sr_update_kernel(int b, int side, cplx* a_s, cplx* a_b, const cplx* lgu, const cplx* ugl,
+// a_s -= lgu ; a_b -= ugl + lgu ; g = new a_b (the next doubling inverts g in place)
+__global__ void sr_update_kernel(int b, cplx* a_s, cplx* a_b, cplx* g, const cplx* lgu, const cplx* ugl,
                                  const int* skip) {
     const int e = blockIdx.y;
     if (skip && skip[e]) return;
@@ -91,9 +91,40 @@ __global__ void sr_update_kernel(int b, int side, cplx* a_s, cplx* a_b, const cp
     size_t o = (size_t)e * b * b + idx;
     cplx x = lgu[o], y = ugl[o];
     cplx s = a_s[o], d = a_b[o];
-    cplx t = side ? y : x;
-    a_s[o] = csub(s, t);
-    a_b[o] = cmake(d.x - x.x - y.x, d.y - x.y - y.y);
+    a_s[o] = csub(s, x);
+    d = cmake(d.x - x.x - y.x, d.y - x.y - y.y);
+    a_b[o] = d; g[o] = d;
+}
+
+// small blocks: update + norms + convergence test of one doubling in ONE launch, one CTA per entry
+__global__ void __launch_bounds__(256) sr_step_kernel(int b, cplx* a_s, cplx* a_b, cplx* g, const cplx* lgu,
+                                                      const cplx* ugl, const cplx* un, const cplx* ln,
+                                                      const double* ref, double tol, int* done, int* iters, int it) {
+    const int e = blockIdx.x;
+    if (done[e]) return;
+    __shared__ double su[8], sl[8];
+    const size_t o = (size_t)e * b * b;
+    double au = 0.0, al = 0.0;
+    for (int i = threadIdx.x; i < b * b; i += 256) {
+        cplx x = lgu[o + i], y = ugl[o + i], s = a_s[o + i], d = a_b[o + i], u = un[o + i], l = ln[o + i];
+        a_s[o + i] = csub(s, x);
+        d = cmake(d.x - x.x - y.x, d.y - x.y - y.y);
+        a_b[o + i] = d; g[o + i] = d;
+        au += u.x * u.x + u.y * u.y;
+        al += l.x * l.x + l.y * l.y;
+    }
+    for (int q = 16; q > 0; q >>= 1) {
+        au += __shfl_down_sync(0xffffffffu, au, q);
+        al += __shfl_down_sync(0xffffffffu, al, q);
+    }
+    if ((threadIdx.x & 31) == 0) { su[threadIdx.x >> 5] = au; sl[threadIdx.x >> 5] = al; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        au = 0.0; al = 0.0;
+        for (int w = 0; w < 8; w++) { au += su[w]; al += sl[w]; }
+        iters[e] = it + 1;
+        if (sqrt(au) + sqrt(al) <= tol * ref[e]) done[e] = 1;
+    }
 }
 
 // ||u||_F + ||l||_F per energy.  mode 0: ref[e] = value.  mode 1: convergence test (reading R3).
@@ -147,9 +178,10 @@ __global__ void obc_finalize_kernel(int b, const cplx* sigma, const double* ener
     if (sg) sg[o + idx] = cmake((1.0 - f) * g.y, -(1.0 - f) * g.x);       // -i (1-f) g
 }
 
-__global__ void obc_status_kernel(int ne, const int* done, const int* sing, int* status) {
+__global__ void obc_status_kernel(int ne, const int* done, const int* sing, const int* it_in, int* status,
+                                  int* iters) {
     int e = blockIdx.x * blockDim.x + threadIdx.x;
-    if (e < ne) status[e] = sing[e] ? sing[e] : (done[e] ? 0 : -1);
+    if (e < ne) { status[e] = sing[e] ? sing[e] : (done[e] ? 0 : -1); iters[e] = it_in[e]; }
 }
 
 inline dim3 grid2(int b, int batch) { return dim3((b * b + 255) / 256, batch); }
@@ -195,10 +227,17 @@ int ew_max_int(negf_ctx* ctx, int* dst, const int* src, int n) {
     NEGF_LAUNCH_CHECK(ctx);
     return NEGF_OK;
 }
-int ew_sr_update(negf_ctx* ctx, int b, int batch, int side, cplx* a_s, cplx* a_b, const cplx* lgu,
+int ew_sr_step(negf_ctx* ctx, int b, int batch, cplx* a_s, cplx* a_b, cplx* g, const cplx* lgu, const cplx* ugl,
+               const cplx* un, const cplx* ln, const double* ref, double tol, int* done, int* iters, int it) {
+    ProfScope _ps(ctx, NEGF_PROF_ELEMENTWISE);
+    sr_step_kernel<<<batch, 256, 0, ctx->stream>>>(b, a_s, a_b, g, lgu, ugl, un, ln, ref, tol, done, iters, it);
+    NEGF_LAUNCH_CHECK(ctx);
+    return NEGF_OK;
+}
+int ew_sr_update(negf_ctx* ctx, int b, int batch, cplx* a_s, cplx* a_b, cplx* g, const cplx* lgu,
                  const cplx* ugl, const int* skip) {
     ProfScope _ps(ctx, NEGF_PROF_ELEMENTWISE);
-    sr_update_kernel<<<grid2(b, batch), 256, 0, ctx->stream>>>(b, side, a_s, a_b, lgu, ugl, skip);
+    sr_update_kernel<<<grid2(b, batch), 256, 0, ctx->stream>>>(b, a_s, a_b, g, lgu, ugl, skip);
     NEGF_LAUNCH_CHECK(ctx);
     return NEGF_OK;
 }
@@ -216,9 +255,9 @@ int ew_obc_finalize(negf_ctx* ctx, int b, int batch, const cplx* sigma, const do
     NEGF_LAUNCH_CHECK(ctx);
     return NEGF_OK;
 }
-int ew_obc_status(negf_ctx* ctx, int ne, const int* done, const int* sing, int* status) {
+int ew_obc_status(negf_ctx* ctx, int ne, const int* done, const int* sing, const int* it_in, int* status, int* iters) {
     ProfScope _ps(ctx, NEGF_PROF_ELEMENTWISE);
-    obc_status_kernel<<<(ne + 255) / 256, 256, 0, ctx->stream>>>(ne, done, sing, status);
+    obc_status_kernel<<<(ne + 255) / 256, 256, 0, ctx->stream>>>(ne, done, sing, it_in, status, iters);
     NEGF_LAUNCH_CHECK(ctx);
     return NEGF_OK;
 }

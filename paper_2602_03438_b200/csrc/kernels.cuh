@@ -26,10 +26,12 @@ int ew_copy(negf_ctx* ctx, size_t n_elems_per, int batch, cplx* dst, long long s
             long long ss, const int* skip);
 int ew_fill_int(negf_ctx* ctx, int* p, int n, int v);
 int ew_max_int(negf_ctx* ctx, int* dst, const int* src, int n);   // dst = dst ? dst : src
-int ew_sr_update(negf_ctx* ctx, int b, int batch, int side, cplx* a_s, cplx* a_b, const cplx* lgu,
+int ew_sr_update(negf_ctx* ctx, int b, int batch, cplx* a_s, cplx* a_b, cplx* g, const cplx* lgu,
                  const cplx* ugl, const int* skip);
+int ew_sr_step(negf_ctx* ctx, int b, int batch, cplx* a_s, cplx* a_b, cplx* g, const cplx* lgu, const cplx* ugl,
+               const cplx* un, const cplx* ln, const double* ref, double tol, int* done, int* iters, int it);
 int ew_sr_norm(negf_ctx* ctx, int b, int batch, const cplx* u, const cplx* l, double* ref, double tol,
                int* done, int* iters, int it, int mode);
 int ew_obc_finalize(negf_ctx* ctx, int b, int batch, const cplx* sigma, const double* energy, double mu,
                     double kT, cplx* gamma, cplx* sl, cplx* sg, double* fermi);
-int ew_obc_status(negf_ctx* ctx, int ne, const int* done, const int* sing, int* status);
+int ew_obc_status(negf_ctx* ctx, int ne, const int* done, const int* sing, const int* it_in, int* status, int* iters);

@@ -3,87 +3,156 @@
 // the algorithm is the one BASELINE.json:north_star names.  Energies that met the stopping rule
 // (reading R3) are masked out of every later launch through the device-side `done` flags, so the
 // host enqueues max_iter doublings without ever synchronising.
+//
+// Scheduling (K3): a right lead is the left-lead recursion with the roles of u and l exchanged
+// (a_s -= u g l, Sigma = a_u g_s a_l), so both leads of all energies run as ONE batch of 2 N_E
+// uniform entries when the blocks are small (b <= NEGF_PAIR_MAX_B); the two / four independent
+// products of a doubling share one grouped GEMM launch, and for small blocks the update, the
+// norms and the convergence test are one kernel: 4 launches per doubling.
 #include "common.cuh"
 #include "kernels.cuh"
 #include "workspace.cuh"
+
+namespace {
+
+struct LeadBlocks { const cplx *Hd, *Hu, *Sd, *Su; };
+
+int resolve_lead(const negf_problem* p, const negf_lead* lead, int side, LeadBlocks* out) {
+    const int n = p->n_blocks;
+    const size_t bb = (size_t)p->block_size * p->block_size;
+    if (lead) {
+        out->Hd = (const cplx*)lead->H_d; out->Hu = (const cplx*)lead->H_u;
+        out->Sd = (const cplx*)lead->S_d; out->Su = (const cplx*)lead->S_u;
+        return (out->Hd && out->Hu) ? NEGF_OK : NEGF_EINVAL;
+    }
+    if (n < 2 || !p->H_diag || !p->H_upper) return NEGF_EINVAL;   // periodic copies need two blocks (R2)
+    const cplx* HD = (const cplx*)p->H_diag; const cplx* HU = (const cplx*)p->H_upper;
+    const cplx* SD = (const cplx*)p->S_diag; const cplx* SU = (const cplx*)p->S_upper;
+    if (side == 0) { out->Hd = HD; out->Hu = HU; out->Sd = SD; out->Su = SU; }
+    else {
+        out->Hd = HD + bb * (n - 1); out->Hu = HU + bb * (n - 2);
+        out->Sd = SD ? SD + bb * (n - 1) : nullptr; out->Su = SU ? SU + bb * (n - 2) : nullptr;
+    }
+    return NEGF_OK;
+}
+
+// ns = 1 or 2 leads stacked in the batch dimension: entry s*ne + e.
+int obc_core(negf_ctx* ctx, const negf_problem* p, int ns, const LeadBlocks* lb, const int* sides, const double* mus,
+             double kT, double tol, int max_iter, const negf_obc_out* const* outs) {
+    const int n = p->n_blocks, b = p->block_size, ne = p->n_energy, nb = ns * ne;
+    const size_t bb = (size_t)b * b;
+    const long long sb = (long long)bb;
+    Workspace W = carve_workspace(ctx->ws, n, b, ne);
+    if (W.bytes > ctx->ws_bytes) return NEGF_ENOWORKSPACE;
+    cplx *a_s = W.T[0], *a_b = W.T[1], *U0 = W.T[2], *L0 = W.T[3];
+    cplx *ub[2] = {W.T[4], W.T[6]}, *lbuf[2] = {W.T[5], W.T[7]};
+    cplx *g = W.T[8], *gu = W.T[9], *gl = W.T[10], *lgu = W.T[11], *ugl = W.T[12];
+    const cplx one = cmake(1.0, 0.0), mone = cmake(-1.0, 0.0), zero = cmake(0.0, 0.0);
+
+    // lead blocks a_d, a_u, a_l for every energy; a right lead stores (u, l) exchanged
+    for (int s = 0; s < ns; s++) {
+        const size_t off = (size_t)s * ne * bb;
+        CombineArgs ca = {};
+        ca.b = b; ca.energy = p->energy; ca.eta = p->eta; ca.use_z = 1; ca.coef = -1.0; ca.sout = sb; ca.skip = nullptr;
+        ca.H = lb[s].Hd; ca.S = lb[s].Sd; ca.s_identity = lb[s].Sd ? 0 : 1; ca.dagger = 0; ca.out = a_s + off;
+        NEGF_TRY(ew_combine(ctx, ca, ne));
+        ca.H = lb[s].Hu; ca.S = lb[s].Su; ca.s_identity = 0;
+        ca.dagger = 0; ca.out = (sides[s] == 0 ? U0 : L0) + off;      // a_u
+        NEGF_TRY(ew_combine(ctx, ca, ne));
+        ca.dagger = 1; ca.out = (sides[s] == 0 ? L0 : U0) + off;      // a_l
+        NEGF_TRY(ew_combine(ctx, ca, ne));
+    }
+    NEGF_TRY(ew_copy(ctx, bb, nb, a_b, sb, a_s, sb, nullptr));
+    NEGF_TRY(ew_copy(ctx, bb, nb, g, sb, a_s, sb, nullptr));
+    NEGF_TRY(ew_fill_int(ctx, W.done, nb, 0));
+    NEGF_TRY(ew_fill_int(ctx, W.sing, nb, 0));
+    NEGF_TRY(ew_fill_int(ctx, W.its, nb, 0));
+    NEGF_TRY(ew_sr_norm(ctx, b, nb, U0, L0, W.ref, tol, W.done, W.its, 0, 0));
+
+    const bool fused_step = b <= NEGF_PAIR_MAX_B;
+    const cplx* u = U0; const cplx* l = L0;
+    for (int it = 0; it < max_iter; it++) {
+        const int* skip = W.done;
+        cplx* un = ub[it & 1]; cplx* ln = lbuf[it & 1];
+        NEGF_TRY(zinv_launch(ctx, b, g, sb, nb, W.inv, W.sing, it + 1, skip));            // g = a_b^-1
+        GemmGroup g1; g1.ng = 2;
+        g1.g[0] = zgemm_bb_args(0, 0, b, one, g, sb, u, sb, zero, nullptr, 0, gu, sb, nb, skip);    // g u
+        g1.g[1] = zgemm_bb_args(0, 0, b, one, g, sb, l, sb, zero, nullptr, 0, gl, sb, nb, skip);    // g l
+        NEGF_TRY(zgemm_launch_group(ctx, g1));
+        GemmGroup g2; g2.ng = 4;
+        g2.g[0] = zgemm_bb_args(0, 0, b, one, l, sb, gu, sb, zero, nullptr, 0, lgu, sb, nb, skip);  // l g u
+        g2.g[1] = zgemm_bb_args(0, 0, b, one, u, sb, gl, sb, zero, nullptr, 0, ugl, sb, nb, skip);  // u g l
+        g2.g[2] = zgemm_bb_args(0, 0, b, mone, u, sb, gu, sb, zero, nullptr, 0, un, sb, nb, skip);  // u <- -u g u
+        g2.g[3] = zgemm_bb_args(0, 0, b, mone, l, sb, gl, sb, zero, nullptr, 0, ln, sb, nb, skip);  // l <- -l g l
+        NEGF_TRY(zgemm_launch_group(ctx, g2));
+        if (fused_step) {
+            NEGF_TRY(ew_sr_step(ctx, b, nb, a_s, a_b, g, lgu, ugl, un, ln, W.ref, tol, W.done, W.its, it));
+        } else {
+            NEGF_TRY(ew_sr_update(ctx, b, nb, a_s, a_b, g, lgu, ugl, skip));
+            NEGF_TRY(ew_sr_norm(ctx, b, nb, un, ln, W.ref, tol, W.done, W.its, it, 1));
+        }
+        // a converged entry keeps its last (u, l) in whichever buffer; they are not used again
+        u = un; l = ln;
+    }
+    // g_s = a_s^-1 ; Sigma = a_l g_s a_u (in the exchanged storage of a right lead: a_u g_s a_l)
+    NEGF_TRY(zinv_launch(ctx, b, a_s, sb, nb, W.inv, W.sing, max_iter + 1, nullptr));
+    NEGF_TRY(zgemm_bb(ctx, 0, 0, b, one, a_s, sb, U0, sb, zero, nullptr, 0, gu, sb, nb, nullptr));
+    GemmGroup gs; gs.ng = ns;
+    for (int s = 0; s < ns; s++) {
+        const size_t off = (size_t)s * ne * bb;
+        gs.g[s] = zgemm_bb_args(0, 0, b, one, L0 + off, sb, gu + off, sb, zero, nullptr, 0, (cplx*)outs[s]->sigma_r, sb, ne, nullptr);
+    }
+    NEGF_TRY(zgemm_launch_group(ctx, gs));
+    for (int s = 0; s < ns; s++) {
+        const negf_obc_out* o = outs[s];
+        const size_t off = (size_t)s * ne * bb;
+        if (o->g_surface) NEGF_TRY(ew_copy(ctx, bb, ne, (cplx*)o->g_surface, sb, a_s + off, sb, nullptr));
+        NEGF_TRY(ew_obc_finalize(ctx, b, ne, (const cplx*)o->sigma_r, p->energy, mus[s], kT, (cplx*)o->gamma,
+                                 (cplx*)o->sigma_lesser, (cplx*)o->sigma_greater, o->fermi));
+        NEGF_TRY(ew_obc_status(ctx, ne, W.done + s * ne, W.sing + s * ne, W.its + s * ne, o->status, o->iters));
+    }
+    return NEGF_OK;
+}
+
+int check_common(const negf_ctx* ctx, const negf_problem* p, int max_iter) {
+    if (!ctx || !p) return NEGF_EINVAL;
+    if (p->n_blocks < 1 || p->block_size < 1 || p->n_energy < 1 || max_iter < 1 || !p->energy) return NEGF_EINVAL;
+    if ((p->S_diag == nullptr) != (p->S_upper == nullptr) && p->n_blocks > 1) return NEGF_EINVAL;
+    if (!ctx->ws) return NEGF_ENOWORKSPACE;
+    return NEGF_OK;
+}
+
+}  // namespace
 
 extern "C" int negf_obc_decimate(negf_ctx* ctx, const negf_problem* p, const negf_lead* lead, int side,
                                  double mu, double kT, double tol, int max_iter,
                                  negf_c128* sigma_r, negf_c128* gamma, negf_c128* sigma_lesser,
                                  negf_c128* sigma_greater, negf_c128* g_surface, double* fermi,
                                  int* iters, int* status) {
-    if (!ctx || !p || !sigma_r || !iters || !status) return NEGF_EINVAL;
+    if (!sigma_r || !iters || !status) return NEGF_EINVAL;
     if (side != 0 && side != 1) return NEGF_EINVAL;
-    const int n = p->n_blocks, b = p->block_size, ne = p->n_energy;
-    if (n < 1 || b < 1 || ne < 1 || max_iter < 1 || !p->energy) return NEGF_EINVAL;
-    if ((p->S_diag == nullptr) != (p->S_upper == nullptr) && n > 1) return NEGF_EINVAL;
-    const cplx *Hd, *Hu, *Sd, *Su;
-    const size_t bb = (size_t)b * b;
-    if (lead) {
-        Hd = (const cplx*)lead->H_d; Hu = (const cplx*)lead->H_u;
-        Sd = (const cplx*)lead->S_d; Su = (const cplx*)lead->S_u;
-        if (!Hd || !Hu) return NEGF_EINVAL;
-    } else {
-        if (n < 2 || !p->H_diag || !p->H_upper) return NEGF_EINVAL;   // periodic copies need two blocks (R2)
-        const cplx* HD = (const cplx*)p->H_diag; const cplx* HU = (const cplx*)p->H_upper;
-        const cplx* SD = (const cplx*)p->S_diag; const cplx* SU = (const cplx*)p->S_upper;
-        if (side == 0) { Hd = HD; Hu = HU; Sd = SD; Su = SU; }
-        else {
-            Hd = HD + bb * (n - 1); Hu = HU + bb * (n - 2);
-            Sd = SD ? SD + bb * (n - 1) : nullptr; Su = SU ? SU + bb * (n - 2) : nullptr;
-        }
-    }
-    if (!ctx->ws) return NEGF_ENOWORKSPACE;
-    Workspace W = carve_workspace(ctx->ws, n, b, ne);
-    if (W.bytes > ctx->ws_bytes) return NEGF_ENOWORKSPACE;
+    NEGF_TRY(check_common(ctx, p, max_iter));
+    LeadBlocks lb;
+    NEGF_TRY(resolve_lead(p, lead, side, &lb));
+    negf_obc_out o = {sigma_r, gamma, sigma_lesser, sigma_greater, g_surface, fermi, iters, status};
+    const negf_obc_out* po = &o;
+    return obc_core(ctx, p, 1, &lb, &side, &mu, kT, tol, max_iter, &po);
+}
 
-    cplx *a_s = W.T[0], *a_b = W.T[1], *U0 = W.T[2], *L0 = W.T[3];
-    cplx *ub[2] = {W.T[4], W.T[6]}, *lb[2] = {W.T[5], W.T[7]};
-    cplx *g = W.T[8], *gu = W.T[9], *gl = W.T[10], *lgu = W.T[11], *ugl = W.T[12];
-    const long long sb = (long long)bb;
-    const cplx one = cmake(1.0, 0.0), mone = cmake(-1.0, 0.0), zero = cmake(0.0, 0.0);
-
-    // lead blocks a_d, a_u, a_l for every energy
-    CombineArgs ca = {};
-    ca.b = b; ca.energy = p->energy; ca.eta = p->eta; ca.use_z = 1; ca.coef = -1.0; ca.sout = sb; ca.skip = nullptr;
-    ca.H = Hd; ca.S = Sd; ca.s_identity = Sd ? 0 : 1; ca.dagger = 0; ca.out = a_s;
-    NEGF_TRY(ew_combine(ctx, ca, ne));
-    NEGF_TRY(ew_copy(ctx, bb, ne, a_b, sb, a_s, sb, nullptr));
-    ca.H = Hu; ca.S = Su; ca.s_identity = 0; ca.dagger = 0; ca.out = U0;
-    NEGF_TRY(ew_combine(ctx, ca, ne));
-    ca.dagger = 1; ca.out = L0;
-    NEGF_TRY(ew_combine(ctx, ca, ne));
-    NEGF_TRY(ew_fill_int(ctx, W.done, ne, 0));
-    NEGF_TRY(ew_fill_int(ctx, W.sing, ne, 0));
-    NEGF_TRY(ew_fill_int(ctx, iters, ne, 0));
-    NEGF_TRY(ew_sr_norm(ctx, b, ne, U0, L0, W.ref, tol, W.done, iters, 0, 0));
-
-    const cplx* u = U0; const cplx* l = L0;
-    for (int it = 0; it < max_iter; it++) {
-        const int* skip = W.done;
-        cplx* un = ub[it & 1]; cplx* ln = lb[it & 1];
-        NEGF_TRY(ew_copy(ctx, bb, ne, g, sb, a_b, sb, skip));
-        NEGF_TRY(zinv_launch(ctx, b, g, sb, ne, W.inv, W.sing, it + 1, skip));
-        NEGF_TRY(zgemm_bb(ctx, 0, 0, b, one, g, sb, u, sb, zero, nullptr, 0, gu, sb, ne, skip));     // g u
-        NEGF_TRY(zgemm_bb(ctx, 0, 0, b, one, g, sb, l, sb, zero, nullptr, 0, gl, sb, ne, skip));     // g l
-        NEGF_TRY(zgemm_bb(ctx, 0, 0, b, one, l, sb, gu, sb, zero, nullptr, 0, lgu, sb, ne, skip));   // l g u
-        NEGF_TRY(zgemm_bb(ctx, 0, 0, b, one, u, sb, gl, sb, zero, nullptr, 0, ugl, sb, ne, skip));   // u g l
-        NEGF_TRY(ew_sr_update(ctx, b, ne, side, a_s, a_b, lgu, ugl, skip));
-        NEGF_TRY(zgemm_bb(ctx, 0, 0, b, mone, u, sb, gu, sb, zero, nullptr, 0, un, sb, ne, skip));   // u <- -u g u
-        NEGF_TRY(zgemm_bb(ctx, 0, 0, b, mone, l, sb, gl, sb, zero, nullptr, 0, ln, sb, ne, skip));   // l <- -l g l
-        NEGF_TRY(ew_sr_norm(ctx, b, ne, un, ln, W.ref, tol, W.done, iters, it, 1));
-        // a converged energy keeps its last (u, l) in whichever buffer; they are not used again
-        u = un; l = ln;
-    }
-    // g_s = a_s^-1 ; Sigma = a_l g_s a_u (left) | a_u g_s a_l (right)
-    NEGF_TRY(zinv_launch(ctx, b, a_s, sb, ne, W.inv, W.sing, max_iter + 1, nullptr));
-    if (g_surface) NEGF_TRY(ew_copy(ctx, bb, ne, (cplx*)g_surface, sb, a_s, sb, nullptr));
-    const cplx* first = side == 0 ? L0 : U0;
-    const cplx* last = side == 0 ? U0 : L0;
-    NEGF_TRY(zgemm_bb(ctx, 0, 0, b, one, a_s, sb, last, sb, zero, nullptr, 0, gu, sb, ne, nullptr));
-    NEGF_TRY(zgemm_bb(ctx, 0, 0, b, one, first, sb, gu, sb, zero, nullptr, 0, (cplx*)sigma_r, sb, ne, nullptr));
-    NEGF_TRY(ew_obc_finalize(ctx, b, ne, (const cplx*)sigma_r, p->energy, mu, kT, (cplx*)gamma,
-                             (cplx*)sigma_lesser, (cplx*)sigma_greater, fermi));
-    NEGF_TRY(ew_obc_status(ctx, ne, W.done, W.sing, status));
-    return NEGF_OK;
+extern "C" int negf_obc_decimate_pair(negf_ctx* ctx, const negf_problem* p, const negf_lead* lead_L,
+                                      const negf_lead* lead_R, double mu_L, double mu_R, double kT, double tol,
+                                      int max_iter, const negf_obc_out* left, const negf_obc_out* right) {
+    if (!left || !right || !left->sigma_r || !right->sigma_r || !left->iters || !right->iters ||
+        !left->status || !right->status) return NEGF_EINVAL;
+    NEGF_TRY(check_common(ctx, p, max_iter));
+    LeadBlocks lb[2];
+    NEGF_TRY(resolve_lead(p, lead_L, 0, &lb[0]));
+    NEGF_TRY(resolve_lead(p, lead_R, 1, &lb[1]));
+    const int sides[2] = {0, 1};
+    const double mus[2] = {mu_L, mu_R};
+    const negf_obc_out* outs[2] = {left, right};
+    if (negf_tmul(p->block_size) == 2) return obc_core(ctx, p, 2, lb, sides, mus, kT, tol, max_iter, outs);
+    // large blocks fill the machine on their own: one lead after the other, half the scratch
+    NEGF_TRY(obc_core(ctx, p, 1, &lb[0], &sides[0], &mus[0], kT, tol, max_iter, &outs[0]));
+    return obc_core(ctx, p, 1, &lb[1], &sides[1], &mus[1], kT, tol, max_iter, &outs[1]);
 }

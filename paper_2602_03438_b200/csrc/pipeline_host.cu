@@ -134,11 +134,11 @@ extern "C" int negf_pipeline_host(negf_ctx* ctx, const negf_problem* hp, const n
     ctx->ws = L.ws; ctx->ws_bytes = L.ws_bytes; ctx->sweep_valid = false;
     int rc = NEGF_OK;
     do {
-        const double mus[2] = {mu_L, mu_R};
-        for (int s = 0; s < 2 && rc == NEGF_OK; s++)
-            rc = negf_obc_decimate(ctx, &dp, nullptr, s, mus[s], kT, tol, max_iter, (negf_c128*)L.ob[s][0],
-                                   (negf_c128*)L.ob[s][1], (negf_c128*)L.ob[s][2], (negf_c128*)L.ob[s][3],
-                                   nullptr, nullptr, L.iters[s], L.status[s]);
+        negf_obc_out oo[2];
+        for (int s = 0; s < 2; s++)
+            oo[s] = negf_obc_out{(negf_c128*)L.ob[s][0], (negf_c128*)L.ob[s][1], (negf_c128*)L.ob[s][2],
+                                 (negf_c128*)L.ob[s][3], nullptr, nullptr, L.iters[s], L.status[s]};
+        rc = negf_obc_decimate_pair(ctx, &dp, nullptr, nullptr, mu_L, mu_R, kT, tol, max_iter, &oo[0], &oo[1]);
         if (rc) break;
         ds[0].left = (negf_c128*)L.ob[0][0]; ds[0].right = (negf_c128*)L.ob[1][0];
         ds[1].left = (negf_c128*)L.ob[0][2]; ds[1].right = (negf_c128*)L.ob[1][2];

@@ -3,6 +3,8 @@
 #include "common.cuh"
 
 constexpr int NEGF_NSCRATCH = 13;   // decimation needs 13 blocks per energy, the sweeps 9
+constexpr int NEGF_PAIR_MAX_B = 128; // up to this block size both leads are decimated in ONE batch of 2*NE entries
+inline int negf_tmul(int b) { return b <= NEGF_PAIR_MAX_B ? 2 : 1; }
 
 struct Workspace {
     cplx* g;        // [NE][n][b][b]    left-connected g_i        (retained sweep state)
@@ -15,6 +17,7 @@ struct Workspace {
     int* done;      // [NE]
     int* sing;      // [NE]
     int* tmpinfo;   // [NE]
+    int* its;       // [2 NE] doublings done
     size_t bytes;
 };
 
@@ -27,12 +30,14 @@ inline Workspace carve_workspace(void* base, int n, int b, int ne) {
     w.X = (cplx*)take(blk * (n > 1 ? n - 1 : 0) * ne);
     w.Y = (cplx*)take(blk * (n > 1 ? n - 1 : 0) * ne);
     w.gx = (cplx*)take(blk * n * ne);
-    for (int t = 0; t < NEGF_NSCRATCH; t++) w.T[t] = (cplx*)take(blk * ne);
-    w.inv = take(zinv_workspace_bytes(b, ne));
-    w.ref = (double*)take(sizeof(double) * ne);
-    w.done = (int*)take(sizeof(int) * ne);
-    w.sing = (int*)take(sizeof(int) * ne);
-    w.tmpinfo = (int*)take(sizeof(int) * ne);
+    const int tm = negf_tmul(b);
+    for (int t = 0; t < NEGF_NSCRATCH; t++) w.T[t] = (cplx*)take(blk * ne * tm);
+    w.inv = take(zinv_workspace_bytes(b, ne * tm));
+    w.ref = (double*)take(sizeof(double) * ne * 2);
+    w.done = (int*)take(sizeof(int) * ne * 2);
+    w.sing = (int*)take(sizeof(int) * ne * 2);
+    w.tmpinfo = (int*)take(sizeof(int) * ne * 2);
+    w.its = (int*)take(sizeof(int) * ne * 2);
     w.bytes = (size_t)(p - (unsigned char*)base);
     return w;
 }

@@ -70,8 +70,9 @@ __device__ __forceinline__ void load_tile_mc(cplx* sm, const cplx* g, int ld, in
     }
 }
 
-template <int OPA, int OPB, int BM, int BN, int WM, int WN>
-__global__ void __launch_bounds__(WM * WN * 32, 1) zgemm_kernel(GemmArgs a) {
+template <int OPA, int OPB, int BM, int BN, int WM, int WN, int MINB>
+__global__ void __launch_bounds__(WM * WN * 32, MINB) zgemm_kernel(const __grid_constant__ GemmGroup grp) {
+    const GemmArgs& a = grp.g[blockIdx.z];
     constexpr int NT = WM * WN * 32;
     constexpr int MI = BM / WM / 8;     // 8x8 sub-tiles per warp along m
     constexpr int NI = BN / WN / 8;
@@ -172,9 +173,10 @@ __global__ void __launch_bounds__(WM * WN * 32, 1) zgemm_kernel(GemmArgs a) {
     }
 }
 
-template <int OPA, int OPB, int BM, int BN, int WM, int WN>
-int launch_cfg(negf_ctx* ctx, const GemmArgs& a) {
-    auto kern = zgemm_kernel<OPA, OPB, BM, BN, WM, WN>;
+template <int OPA, int OPB, int BM, int BN, int WM, int WN, int MINB>
+int launch_cfg(negf_ctx* ctx, const GemmGroup& grp) {
+    const GemmArgs& a = grp.g[0];
+    auto kern = zgemm_kernel<OPA, OPB, BM, BN, WM, WN, MINB>;
     constexpr int smem = STAGES * (BM + BN) * BK * (int)sizeof(cplx);
     static bool attr_done = false;
     if (!attr_done) {
@@ -182,42 +184,64 @@ int launch_cfg(negf_ctx* ctx, const GemmArgs& a) {
         attr_done = true;
     }
     int tiles = ((a.m + BM - 1) / BM) * ((a.n + BN - 1) / BN);
-    dim3 grid(tiles, a.batch);
-    kern<<<grid, WM * WN * 32, smem, ctx->stream>>>(a);
+    dim3 grid(tiles, a.batch, grp.ng);
+    kern<<<grid, WM * WN * 32, smem, ctx->stream>>>(grp);
     NEGF_LAUNCH_CHECK(ctx);
     return NEGF_OK;
 }
 
-template <int BM, int BN, int WM, int WN>
-int launch_ops(negf_ctx* ctx, const GemmArgs& a) {
-    if (a.opA == 0 && a.opB == 0) return launch_cfg<0, 0, BM, BN, WM, WN>(ctx, a);
-    if (a.opA == 1 && a.opB == 0) return launch_cfg<1, 0, BM, BN, WM, WN>(ctx, a);
-    if (a.opA == 0 && a.opB == 1) return launch_cfg<0, 1, BM, BN, WM, WN>(ctx, a);
-    return launch_cfg<1, 1, BM, BN, WM, WN>(ctx, a);
+template <int BM, int BN, int WM, int WN, int MINB>
+int launch_ops(negf_ctx* ctx, const GemmGroup& grp) {
+    const GemmArgs& a = grp.g[0];
+    if (a.opA == 0 && a.opB == 0) return launch_cfg<0, 0, BM, BN, WM, WN, MINB>(ctx, grp);
+    if (a.opA == 1 && a.opB == 0) return launch_cfg<1, 0, BM, BN, WM, WN, MINB>(ctx, grp);
+    if (a.opA == 0 && a.opB == 1) return launch_cfg<0, 1, BM, BN, WM, WN, MINB>(ctx, grp);
+    return launch_cfg<1, 1, BM, BN, WM, WN, MINB>(ctx, grp);
 }
 
 }  // namespace
 
-int zgemm_launch(negf_ctx* ctx, const GemmArgs& a) {
+int zgemm_launch_group(negf_ctx* ctx, const GemmGroup& grp) {
     ProfScope _ps(ctx, NEGF_PROF_GEMM);
+    if (grp.ng < 1 || grp.ng > NEGF_GEMM_GROUP_MAX) return NEGF_EINVAL;
+    const GemmArgs& a = grp.g[0];
     if (a.m <= 0 || a.n <= 0 || a.batch <= 0) return NEGF_OK;
     if (a.k < 0 || (a.opA | a.opB) & ~1) return NEGF_EINVAL;
     if (a.batch > 65535) return NEGF_EUNSUPPORTED;
-    // Tile choice: 128x64 CTA tiles (8 warps, 32x32 warp tiles) when they fill the machine,
-    // else 64x64 (4 warps) to get more CTAs in flight.
-    long long big_tiles = (long long)((a.m + 127) / 128) * ((a.n + 63) / 64) * a.batch;
-    if (a.m > 64 && big_tiles >= ctx->num_sms) return launch_ops<128, 64, 4, 2>(ctx, a);
-    return launch_ops<64, 64, 2, 2>(ctx, a);
+    for (int i = 1; i < grp.ng; i++) {      // one grid serves every member: same shape, ops and batch
+        const GemmArgs& o = grp.g[i];
+        if (o.m != a.m || o.n != a.n || o.k != a.k || o.opA != a.opA || o.opB != a.opB || o.batch != a.batch)
+            return NEGF_EINVAL;
+    }
+    // Tile choice: the largest CTA tile that still gives every SM work.  128x64 (8 warps, 32x32 warp
+    // tiles, 1 CTA/SM) in the compute-bound regime; 64x64 (4 warps); 32x32 (4 warps of 16x16, up to
+    // 4 CTAs/SM) when the batch of small blocks would otherwise leave most SMs idle.
+    const long long per = (long long)a.batch * grp.ng;
+    const long long t128 = (long long)((a.m + 127) / 128) * ((a.n + 63) / 64) * per;
+    const long long t64 = (long long)((a.m + 63) / 64) * ((a.n + 63) / 64) * per;
+    if (a.m > 64 && t128 >= ctx->num_sms) return launch_ops<128, 64, 4, 2, 1>(ctx, grp);
+    if (t64 >= ctx->num_sms) return launch_ops<64, 64, 2, 2, 1>(ctx, grp);
+    return launch_ops<32, 32, 2, 2, 3>(ctx, grp);
 }
 
-int zgemm_bb(negf_ctx* ctx, int opA, int opB, int b, cplx alpha, const cplx* A, long long sA,
-             const cplx* B, long long sB, cplx beta, const cplx* D, long long sD,
-             cplx* C, long long sC, int batch, const int* skip) {
+int zgemm_launch(negf_ctx* ctx, const GemmArgs& a) {
+    GemmGroup grp;
+    grp.g[0] = a; grp.ng = 1;
+    return zgemm_launch_group(ctx, grp);
+}
+
+GemmArgs zgemm_bb_args(int opA, int opB, int b, cplx alpha, const cplx* A, long long sA, const cplx* B, long long sB,
+                       cplx beta, const cplx* D, long long sD, cplx* C, long long sC, int batch, const int* skip) {
     GemmArgs g;
     g.opA = opA; g.opB = opB; g.m = g.n = g.k = b; g.alpha = alpha; g.beta = beta;
     g.A = A; g.lda = b; g.sA = sA; g.B = B; g.ldb = b; g.sB = sB;
     g.D = D; g.sD = sD; g.C = C; g.ldc = b; g.sC = sC; g.batch = batch; g.skip = skip;
-    return zgemm_launch(ctx, g);
+    return g;
+}
+int zgemm_bb(negf_ctx* ctx, int opA, int opB, int b, cplx alpha, const cplx* A, long long sA,
+             const cplx* B, long long sB, cplx beta, const cplx* D, long long sD,
+             cplx* C, long long sC, int batch, const int* skip) {
+    return zgemm_launch(ctx, zgemm_bb_args(opA, opB, b, alpha, A, sA, B, sB, beta, D, sD, C, sC, batch, skip));
 }
 
 extern "C" int negf_zgemm_batched(negf_ctx* ctx, int opA, int opB, int m, int n, int k,

@@ -44,6 +44,11 @@ class Lead(C.Structure):
     _fields_ = [("H_d", C.c_void_p), ("H_u", C.c_void_p), ("S_d", C.c_void_p), ("S_u", C.c_void_p)]
 
 
+class ObcOut(C.Structure):
+    _fields_ = [(k, C.c_void_p) for k in
+                ("sigma_r", "gamma", "sigma_lesser", "sigma_greater", "g_surface", "fermi", "iters", "status")]
+
+
 class HostOutputs(C.Structure):
     _fields_ = [(k, C.c_void_p) for k in
                 ("GR_diag", "GR_upper", "GR_lower", "GL_diag", "GL_upper", "GG_diag", "GG_upper",
@@ -52,7 +57,7 @@ class HostOutputs(C.Structure):
 
 EXPORTS = ["negf_create", "negf_destroy", "negf_set_stream", "negf_workspace_bytes", "negf_set_workspace",
            "negf_strerror", "negf_last_cuda_error", "negf_launch_count",
-           "negf_profile_enable", "negf_profile_read", "negf_obc_decimate",
+           "negf_profile_enable", "negf_profile_read", "negf_obc_decimate", "negf_obc_decimate_pair",
            "negf_rgf_retarded", "negf_rgf_lesser_greater", "negf_observables", "negf_pipeline_host_bytes",
            "negf_pipeline_host", "negf_zgemm_batched", "negf_zinverse_batched", "negf_fp64_peak"]
 
@@ -71,6 +76,9 @@ lib.negf_profile_enable.argtypes = [_P, C.c_int]
 lib.negf_profile_read.argtypes = [_P, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_longlong), C.c_int]
 lib.negf_obc_decimate.argtypes = [_P, C.POINTER(Problem), C.POINTER(Lead), C.c_int, C.c_double, C.c_double,
                                   C.c_double, C.c_int, _P, _P, _P, _P, _P, _P, _P, _P]
+lib.negf_obc_decimate_pair.argtypes = [_P, C.POINTER(Problem), C.POINTER(Lead), C.POINTER(Lead), C.c_double,
+                                       C.c_double, C.c_double, C.c_double, C.c_int, C.POINTER(ObcOut),
+                                       C.POINTER(ObcOut)]
 lib.negf_rgf_retarded.argtypes = [_P, C.POINTER(Problem), C.POINTER(Sigma), _P, _P, _P, _P, C.c_int, _P]
 lib.negf_rgf_lesser_greater.argtypes = [_P, C.POINTER(Problem), C.POINTER(Sigma), C.POINTER(Sigma),
                                         C.POINTER(Sigma), _P, _P, _P, _P, _P, _P]
@@ -180,6 +188,16 @@ class Context:
                                           side, mu, kT, tol, max_iter, _ptr(sigma_r), _ptr(gamma),
                                           _ptr(sigma_lesser), _ptr(sigma_greater), _ptr(g_surface), _ptr(fermi),
                                           _ptr(iters), _ptr(status)), "negf_obc_decimate")
+
+    def obc_decimate_pair(self, p: Problem, mu_L, mu_R, kT, tol, max_iter, left: dict, right: dict,
+                          lead_L: Lead = None, lead_R: Lead = None):
+        """left / right: dicts with the keys of negf_obc_out (tensors or None)."""
+        keys = ("sigma_r", "gamma", "sigma_lesser", "sigma_greater", "g_surface", "fermi", "iters", "status")
+        oL = ObcOut(*[_ptr(left.get(k)) for k in keys])
+        oR = ObcOut(*[_ptr(right.get(k)) for k in keys])
+        ref = lambda s: C.byref(s) if s is not None else None
+        self._check(lib.negf_obc_decimate_pair(self._h, C.byref(p), ref(lead_L), ref(lead_R), mu_L, mu_R, kT, tol,
+                                               max_iter, C.byref(oL), C.byref(oR)), "negf_obc_decimate_pair")
 
     def rgf_retarded(self, p: Problem, sigma_r: Optional[Sigma], GR_diag, GR_upper=None, GR_lower=None,
                      GR_corner=None, flags=0, info=None):

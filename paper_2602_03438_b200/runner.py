@@ -90,8 +90,14 @@ class DevicePath:
         return negf.make_sigma(negf.SIGMA_BT, diag=s["diag"], upper=s["upper"], lower=s["lower"],
                                left=left, right=right)
 
-    def obc(self):
+    def obc(self, pair: bool = True):
         wl, o = self.wl, self.out
+        if pair:
+            d = lambda t: {"sigma_r": o[f"sigma_r_{t}"], "gamma": o[f"gamma_{t}"], "sigma_lesser": o[f"sigma_l_{t}"],
+                           "sigma_greater": o[f"sigma_g_{t}"], "g_surface": o[f"g_s_{t}"], "fermi": o[f"fermi_{t}"],
+                           "iters": o[f"iters_{t}"], "status": o[f"status_{t}"]}
+            self.ctx.obc_decimate_pair(self.problem, wl.mu_L, wl.mu_R, wl.kT, wl.tol, wl.max_iter, d("L"), d("R"))
+            return
         for side, tag, mu in ((0, "L", wl.mu_L), (1, "R", wl.mu_R)):
             self.ctx.obc_decimate(self.problem, side, mu, wl.kT, wl.tol, wl.max_iter, o[f"sigma_r_{tag}"],
                                   o[f"gamma_{tag}"], o[f"sigma_l_{tag}"], o[f"sigma_g_{tag}"], o[f"g_s_{tag}"],

@@ -177,3 +177,19 @@ def test_n1_explicit_lead_rejected_without_lead(runner_mod, negf_lib):
     assert rel_fro(dp.host("GR_diag")[0], out["ret"]["GR_diag"]) < TOL
     assert rel_fro(dp.host("GL_diag")[0], out["les"]["GX_diag"]) < TOL
     assert rel_fro(dp.host("GG_diag")[0], out["gtr"]["GX_diag"]) < TOL
+
+
+@pytest.mark.parametrize("cfg,kw", [CASES[2], CASES[5]])
+def test_obc_pair_equals_two_single_calls(runner_mod, cfg, kw):
+    """negf_obc_decimate_pair (both leads as one batch of 2 N_E entries, right lead stored with u and l
+    exchanged) against two negf_obc_decimate calls: the same arithmetic per entry, so bit-identical."""
+    wl = W.make_workload(cfg, **kw)
+    dp = runner_mod.DevicePath(wl, want_greater=True)
+    dp.obc(pair=True)
+    pair = {k: dp.host(k).copy() for k in dp.out if k.endswith(("_L", "_R"))}
+    for k in dp.out:
+        if k.endswith(("_L", "_R")):
+            dp.out[k].zero_()
+    dp.obc(pair=False)
+    for k, v in pair.items():
+        assert np.array_equal(v, dp.host(k)), k
