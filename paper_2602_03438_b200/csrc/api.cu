@@ -19,7 +19,7 @@ extern "C" int negf_create(negf_ctx** out, int device) {
     if (!c) return NEGF_EINVAL;
     c->device = device; c->stream = nullptr; c->ws = nullptr; c->ws_bytes = 0; c->last_cuda_error = 0;
     c->launches = 0; c->num_sms = prop.multiProcessorCount; c->sweep_valid = false;
-    c->sw_n = c->sw_b = c->sw_ne = 0;
+    c->sw_n = c->sw_b = c->sw_ne = 0; c->sw_assembled = false;
     c->prof_on = false; c->prof_depth = 0;
     for (int k = 0; k < NEGF_PROF_CLASSES; k++) { c->prof_ms[k] = 0.0; c->prof_n[k] = 0; }
     *out = c;

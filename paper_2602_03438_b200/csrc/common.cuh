@@ -21,6 +21,7 @@ struct negf_ctx {
     // retained sweep state (NEGF_KEEP_SWEEP): valid for this shape only
     bool sweep_valid;
     int sw_n, sw_b, sw_ne;
+    bool sw_assembled;
     // optional per-kernel-class timing (negf_profile_enable): event pairs around every launch site
     bool prof_on;
     int prof_depth;
@@ -121,6 +122,10 @@ struct GemmArgs {
     cplx* C; int ldc; long long sC;
     int batch;
     const int* skip;         // optional [batch] device mask: entry skipped when skip[e] != 0
+    // optional second batch dimension (the block index i of a family): entry (e, i), e < batch, i < batch2
+    int batch2;
+    long long sA2, sB2, sD2, sC2;
+    const cplx* alpha_vec;   // optional [batch]: entry e uses alpha * alpha_vec[e]
 };
 int zgemm_launch(negf_ctx* ctx, const GemmArgs& a);
 // several independent products of identical shape / ops / batch in ONE launch (blockIdx.z = member)

@@ -7,19 +7,20 @@
 
 namespace {
 
-__global__ void combine_kernel(CombineArgs a) {
+__global__ void combine_kernel(const __grid_constant__ CombineArgs a) {
     const int e = blockIdx.y;
     if (a.skip && a.skip[e]) return;
     const int b = a.b;
     const int idx = blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= b * b) return;
     const int r = idx / b, c = idx % b;
-    const int src = a.dagger ? c * b + r : idx;
+    const int fi = blockIdx.z;
+    const size_t src = (a.dagger ? c * b + r : idx);
     cplx v = cmake(0.0, 0.0);
     if (a.use_z) {
         cplx z = cmake(a.energy[e], a.eta);
         if (a.S) {
-            cplx s = a.S[src];
+            cplx s = a.S[src + (size_t)fi * a.fS];
             if (a.dagger) s = cconj(s);
             v = cmul(z, s);
         } else if (a.s_identity && r == c) {
@@ -27,13 +28,13 @@ __global__ void combine_kernel(CombineArgs a) {
         }
     }
     if (a.H) {
-        cplx h = a.H[src];
+        cplx h = a.H[src + (size_t)fi * a.fH];
         if (a.dagger) h = cconj(h);
         v = csub(v, h);
     }
     for (int t = 0; t < 3; t++) {
-        if (a.blk[t]) {
-            cplx x = a.blk[t][(size_t)e * a.sblk[t] + idx];
+        if (a.blk[t] && (a.nfam <= 1 || a.only[t] < 0 || a.only[t] == fi)) {
+            cplx x = a.blk[t][(size_t)e * a.sblk[t] + (a.only[t] < 0 ? (size_t)fi * a.fblk[t] : 0) + idx];
             v.x = fma(a.coef, x.x, v.x); v.y = fma(a.coef, x.y, v.y);
         }
     }
@@ -41,7 +42,7 @@ __global__ void combine_kernel(CombineArgs a) {
         cplx x = a.scalar[e];
         v.x = fma(a.coef, x.x, v.x); v.y = fma(a.coef, x.y, v.y);
     }
-    a.out[(size_t)e * a.sout + idx] = v;
+    a.out[(size_t)e * a.sout + (size_t)fi * a.fout + idx] = v;
 }
 
 // C = Z + sign * (V - V^H)
@@ -190,7 +191,9 @@ inline dim3 grid2(int b, int batch) { return dim3((b * b + 255) / 256, batch); }
 
 int ew_combine(negf_ctx* ctx, const CombineArgs& a, int batch) {
     ProfScope _ps(ctx, NEGF_PROF_ELEMENTWISE);
-    combine_kernel<<<grid2(a.b, batch), 256, 0, ctx->stream>>>(a);
+    dim3 grid = grid2(a.b, batch);
+    grid.z = a.nfam > 1 ? a.nfam : 1;
+    combine_kernel<<<grid, 256, 0, ctx->stream>>>(a);
     NEGF_LAUNCH_CHECK(ctx);
     return NEGF_OK;
 }

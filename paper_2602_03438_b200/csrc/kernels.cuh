@@ -15,6 +15,11 @@ struct CombineArgs {
     double coef;
     cplx* out; long long sout;
     const int* skip;
+    // family mode (nfam > 1): blockIdx.z = block index i; H, S, out and blk[t] advance by the strides
+    // below per i; blk[t] contributes only to block only[t] when only[t] >= 0 (boundary blocks).
+    int nfam;
+    long long fH, fS, fout, fblk[3];
+    int only[3];
 };
 int ew_combine(negf_ctx* ctx, const CombineArgs& a, int batch);
 // C = Z + sign * (V - V^H)   (Z may be NULL)

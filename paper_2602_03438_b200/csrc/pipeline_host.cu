@@ -50,7 +50,7 @@ Layout make_layout(void* base, int n, int b, int ne, int kind_max, bool hasS, bo
     L.trans = (double*)B.take(sizeof(double) * ne); L.bond = (double*)B.take(sizeof(double) * ne * (m > 0 ? m : 1));
     L.contact = (double*)B.take(sizeof(double) * ne * 2);
     L.info_r = (int*)B.take(sizeof(int) * ne); L.info_x = (int*)B.take(sizeof(int) * ne);
-    Workspace W = carve_workspace(nullptr, n, b, ne);
+    Workspace W = carve_workspace(nullptr, n, b, ne, hasS || kind_max == NEGF_SIGMA_BT);
     L.ws_bytes = W.bytes; L.ws = B.take(W.bytes);
     L.total = B.off;
     return L;

@@ -1,9 +1,18 @@
 // S1 + S3-S6: the RGF sweeps, all energies of the batch in lock-step
 // ("Each E is independent of the other"; "sequential in essence" along the
-// blocks).  Every sweep step is one batched launch of the K2 GEMM / K1 inverse
-// over the energy axis (K3: the energy-batch scheduler for the large-block regime).
-// The blocks of A = z S - H - Sigma^R are assembled per step into scratch and never stored as
-// a family (S1).
+// blocks).  K3, the energy-batch scheduler: every sweep step is one batched launch
+// of the K2 GEMM / K1 inverse over the energy axis, and everything that does NOT sit on the
+// sequential chain is hoisted out of it and batched over (energy x block index) in one launch:
+//   S4  X_i = g_i A_{i,i+1} for all i; then two launches per block (grouped Gu / Gl / corner, G_ii);
+//   S5  (small blocks or ballistic) g^x_i = W_i + Z_i g^x_{i-1} Z_i^H with W_i = g_i [..] g_i^H and
+//       Z_i = g_i A_{i,i-1} batched over i: two launches per block instead of four;
+//   S6  T2_i, Q_i = T2_i (G^R_{i+1,i+1})^H and P_i = g^x_i - Q_i X_i^H batched over i; then
+//       G^x_{i,i+1} = Q_i - X_i G^x_{i+1,i+1} and G^x_ii = P_i + X_i (G^x_{i,i+1})^H (same five
+//       products per block as the textbook form, two on the chain, no elementwise pass).
+// S1: with S = I and no block-tridiagonal Sigma^R_S the off-diagonal blocks of A are -H_{i,i+1}
+// and its dagger for every energy, so they are read straight from H (operand flags, alpha = -1)
+// and never materialised; otherwise the two off-diagonal families are assembled once per call.
+// The diagonal blocks are assembled straight into the g family and inverted in place.
 #include "common.cuh"
 #include "kernels.cuh"
 #include "workspace.cuh"
@@ -43,60 +52,65 @@ int check_sigma(const negf_sigma* s, int n, bool retarded) {
     return NEGF_EINVAL;
 }
 
-// A-block `which` (0 diag i, 1 upper i = A_{i,i+1}, 2 lower i = A_{i+1,i}) for all energies.
-int assemble_a(negf_ctx* ctx, const negf_problem* p, const negf_sigma* sr, const Shape& s, int which,
-               int i, cplx* out, long long sout) {
-    CombineArgs ca = {};
-    ca.b = s.b; ca.energy = p->energy; ca.eta = p->eta; ca.use_z = 1; ca.coef = -1.0;
-    ca.out = out; ca.sout = sout; ca.skip = nullptr;
-    const cplx* HD = (const cplx*)p->H_diag; const cplx* HU = (const cplx*)p->H_upper;
-    const cplx* SD = (const cplx*)p->S_diag; const cplx* SU = (const cplx*)p->S_upper;
-    int nb = 0;
-    if (which == 0) {
-        ca.H = HD + s.bb * i; ca.S = SD ? SD + s.bb * i : nullptr; ca.s_identity = SD ? 0 : 1; ca.dagger = 0;
-        if (sr) {
-            if (sr->kind == NEGF_SIGMA_SCALAR) ca.scalar = (const cplx*)sr->scalar;
-            if (sr->kind == NEGF_SIGMA_BT) { ca.blk[nb] = (const cplx*)sr->diag + s.bb * i; ca.sblk[nb] = s.sn; nb++; }
-            if (i == 0 && sr->left) { ca.blk[nb] = (const cplx*)sr->left; ca.sblk[nb] = s.sb; nb++; }
-            if (i == s.n - 1 && sr->right) { ca.blk[nb] = (const cplx*)sr->right; ca.sblk[nb] = s.sb; nb++; }
-        }
-    } else {
-        ca.H = HU + s.bb * i; ca.S = SU ? SU + s.bb * i : nullptr; ca.s_identity = 0; ca.dagger = (which == 2);
-        if (sr && sr->kind == NEGF_SIGMA_BT) {
-            ca.blk[0] = (const cplx*)(which == 1 ? sr->upper : sr->lower) + s.bb * i; ca.sblk[0] = s.sm;
-        }
-    }
-    return ew_combine(ctx, ca, s.ne);
+bool needs_assembly(const negf_problem* p, const negf_sigma* sr) {
+    return p->S_diag != nullptr || (sr && sr->kind == NEGF_SIGMA_BT);
 }
 
-// B-block of Sigma^x: which 0 = diag i, 1 = upper i.  *is_zero set when nothing contributes.
-int assemble_b(negf_ctx* ctx, const negf_sigma* sx, const Shape& s, int which, int i, cplx* out,
-               bool* is_zero) {
-    CombineArgs ca = {};
-    ca.b = s.b; ca.use_z = 0; ca.coef = 1.0; ca.out = out; ca.sout = s.sb; ca.skip = nullptr;
-    int nb = 0; bool any = false;
-    if (which == 0) {
-        if (sx->kind == NEGF_SIGMA_SCALAR) { ca.scalar = (const cplx*)sx->scalar; any = true; }
-        if (sx->kind == NEGF_SIGMA_BT) { ca.blk[nb] = (const cplx*)sx->diag + s.bb * i; ca.sblk[nb] = s.sn; nb++; }
-        if (i == 0 && sx->left) { ca.blk[nb] = (const cplx*)sx->left; ca.sblk[nb] = s.sb; nb++; }
-        if (i == s.n - 1 && sx->right) { ca.blk[nb] = (const cplx*)sx->right; ca.sblk[nb] = s.sb; nb++; }
-    } else {
-        if (sx->kind == NEGF_SIGMA_BT) { ca.blk[nb] = (const cplx*)sx->upper + s.bb * i; ca.sblk[nb] = s.sm; nb++; }
-    }
-    any = any || nb > 0;
-    *is_zero = !any;
-    if (!any && which == 1) return NEGF_OK;     // callers skip the products with a zero upper block
-    return ew_combine(ctx, ca, s.ne);
-}
+// A family of blocks as a GEMM operand: block i of energy e at p + e*se + i*si, read as op(.)
+struct Opnd { const cplx* p; long long se, si; int op; };
+inline Opnd dag(Opnd o) { o.op ^= 1; return o; }
 
 const cplx ONE = {1.0, 0.0}, MONE = {-1.0, 0.0}, ZERO = {0.0, 0.0};
+inline cplx real(double x) { return cmake(x, 0.0); }
+
+// C(ic + j) = alpha op(A(ia + j)) op(B(ib + j)) + beta D(id + j), j < cnt, for all energies
+GemmArgs gemm_fam(const Shape& s, cplx alpha, Opnd A, int ia, Opnd B, int ib, cplx beta, const Opnd* D, int id,
+                  Opnd C, int ic, int cnt) {
+    GemmArgs g = zgemm_bb_args(A.op, B.op, s.b, alpha, A.p + (size_t)ia * A.si, A.se, B.p + (size_t)ib * B.si, B.se, beta,
+                               D ? D->p + (size_t)id * D->si : nullptr, D ? D->se : 0,
+                               const_cast<cplx*>(C.p) + (size_t)ic * C.si, C.se, s.ne, nullptr);
+    g.batch2 = cnt; g.sA2 = A.si; g.sB2 = B.si; g.sD2 = D ? D->si : 0; g.sC2 = C.si;
+    return g;
+}
+inline GemmArgs gemm_one(const Shape& s, cplx alpha, Opnd A, int ia, Opnd B, int ib, cplx beta, const Opnd* D, int id,
+                         Opnd C, int ic) {
+    return gemm_fam(s, alpha, A, ia, B, ib, beta, D, id, C, ic, 1);
+}
+// families batched over (energy x i) can exceed the grid.y limit: split along i
+int launch_fam(negf_ctx* ctx, const Shape& s, cplx alpha, Opnd A, int ia, Opnd B, int ib, cplx beta, const Opnd* D,
+               int id, Opnd C, int ic, int cnt, const cplx* alpha_vec = nullptr) {
+    const int chunk = max(1, 65535 / s.ne);
+    for (int j = 0; j < cnt; j += chunk) {
+        GemmArgs g = gemm_fam(s, alpha, A, ia + j, B, ib + j, beta, D, id + j, C, ic + j, min(chunk, cnt - j));
+        g.alpha_vec = alpha_vec;
+        NEGF_TRY(zgemm_launch(ctx, g));
+    }
+    return NEGF_OK;
+}
+
+struct Fams {                // operand views of the workspace families and of A's off-diagonal blocks
+    Opnd g, X, Y, gx, Z, Q, AU, AL;
+    double sgn;              // AU / AL hold sgn * A_{i,i+1} / A_{i+1,i}
+};
+Fams make_fams(const negf_problem* p, const Shape& s, const Workspace& W, bool assembled) {
+    Fams f;
+    f.g = {W.g, s.sn, s.sb, 0}; f.gx = {W.gx, s.sn, s.sb, 0}; f.Q = {W.Q, s.sn, s.sb, 0};
+    f.X = {W.X, s.sm, s.sb, 0}; f.Y = {W.Y, s.sm, s.sb, 0}; f.Z = {W.Z, s.sm, s.sb, 0};
+    if (assembled) {
+        f.AU = {W.Aup, s.sm, s.sb, 0}; f.AL = {W.Alow, s.sm, s.sb, 0}; f.sgn = 1.0;
+    } else {                 // A_{i,i+1} = -H_{i,i+1}, A_{i+1,i} = -H_{i,i+1}^H for every energy
+        f.AU = {(const cplx*)p->H_upper, 0, s.sb, 0}; f.AL = {(const cplx*)p->H_upper, 0, s.sb, 1}; f.sgn = -1.0;
+    }
+    return f;
+}
 
 }  // namespace
 
 extern "C" int negf_workspace_bytes(const negf_problem* p, int kind_max, int flags, size_t* bytes) {
-    (void)kind_max; (void)flags;
+    (void)flags;
     if (!p || !bytes || p->n_blocks < 1 || p->block_size < 1 || p->n_energy < 1) return NEGF_EINVAL;
-    Workspace w = carve_workspace(nullptr, p->n_blocks, p->block_size, p->n_energy);
+    const bool assembled = p->S_diag != nullptr || kind_max == NEGF_SIGMA_BT;
+    Workspace w = carve_workspace(nullptr, p->n_blocks, p->block_size, p->n_energy, assembled);
     *bytes = w.bytes;
     return NEGF_OK;
 }
@@ -109,100 +123,184 @@ extern "C" int negf_rgf_retarded(negf_ctx* ctx, const negf_problem* p, const neg
     const Shape s = shape_of(p);
     NEGF_TRY(check_sigma(sigma_r, s.n, true));
     if (!ctx->ws) return NEGF_ENOWORKSPACE;
-    Workspace W = carve_workspace(ctx->ws, s.n, s.b, s.ne);
+    const bool assembled = needs_assembly(p, sigma_r);
+    Workspace W = carve_workspace(ctx->ws, s.n, s.b, s.ne, assembled);
     if (W.bytes > ctx->ws_bytes) return NEGF_ENOWORKSPACE;
     ctx->sweep_valid = false;
-    cplx* GRd = (cplx*)GR_diag_; cplx* GRu = (cplx*)GR_upper_; cplx* GRl = (cplx*)GR_lower_;
     const int b = s.b, ne = s.ne, n = s.n;
-    cplx *T0 = W.T[0], *T1 = W.T[1], *T2 = W.T[2], *T3 = W.T[3], *T4 = W.T[4], *T5 = W.T[5];
+    const Fams F = make_fams(p, s, W, assembled);
+    const Opnd GRd = {(const cplx*)GR_diag_, s.sn, s.sb, 0};
     NEGF_TRY(ew_fill_int(ctx, info, ne, 0));
 
-    // S3 forward: g_0 = A_00^-1 ; g_i = (A_ii - A_{i,i-1} g_{i-1} A_{i-1,i})^-1
-    for (int i = 0; i < n; i++) {
-        cplx* gi = W.g + s.bb * i;
-        if (i == 0) {
-            NEGF_TRY(assemble_a(ctx, p, sigma_r, s, 0, 0, gi, s.sn));
-        } else {
-            cplx* Yi = W.Y + s.bb * (i - 1);
-            NEGF_TRY(assemble_a(ctx, p, sigma_r, s, 0, i, T0, s.sb));
-            NEGF_TRY(assemble_a(ctx, p, sigma_r, s, 2, i - 1, T1, s.sb));      // A_{i,i-1}
-            NEGF_TRY(assemble_a(ctx, p, sigma_r, s, 1, i - 1, T2, s.sb));      // A_{i-1,i}
-            NEGF_TRY(zgemm_bb(ctx, 0, 0, b, ONE, T1, s.sb, W.g + s.bb * (i - 1), s.sn, ZERO, nullptr, 0,
-                              Yi, s.sm, ne, nullptr));                          // Y_{i-1} = A_{i,i-1} g_{i-1}
-            NEGF_TRY(zgemm_bb(ctx, 0, 0, b, MONE, Yi, s.sm, T2, s.sb, ONE, T0, s.sb, gi, s.sn, ne, nullptr));
+    // S1: diagonal blocks A_ii = z S_ii - H_ii - Sigma^R_ii for all i straight into the g family
+    {
+        CombineArgs ca = {};
+        ca.b = b; ca.energy = p->energy; ca.eta = p->eta; ca.use_z = 1; ca.coef = -1.0;
+        ca.H = (const cplx*)p->H_diag; ca.fH = s.sb;
+        ca.S = (const cplx*)p->S_diag; ca.fS = s.sb; ca.s_identity = p->S_diag ? 0 : 1;
+        ca.out = W.g; ca.sout = s.sn; ca.fout = s.sb; ca.nfam = n;
+        int nb = 0;
+        if (sigma_r) {
+            if (sigma_r->kind == NEGF_SIGMA_SCALAR) ca.scalar = (const cplx*)sigma_r->scalar;
+            if (sigma_r->kind == NEGF_SIGMA_BT) { ca.blk[nb] = (const cplx*)sigma_r->diag; ca.sblk[nb] = s.sn; ca.fblk[nb] = s.sb; ca.only[nb] = -1; nb++; }
+            if (sigma_r->left) { ca.blk[nb] = (const cplx*)sigma_r->left; ca.sblk[nb] = s.sb; ca.only[nb] = 0; nb++; }
+            if (sigma_r->right) { ca.blk[nb] = (const cplx*)sigma_r->right; ca.sblk[nb] = s.sb; ca.only[nb] = n - 1; nb++; }
         }
-        NEGF_TRY(zinv_launch(ctx, b, gi, s.sn, ne, W.inv, info, i + 1, nullptr));
+        if (n == 1) {   // a single launch slot (blockIdx.z = 0) must take both boundary blocks
+            ca.nfam = 1;
+        }
+        NEGF_TRY(ew_combine(ctx, ca, ne));
+    }
+    if (assembled && n > 1) {   // off-diagonal families, once per call
+        for (int which = 1; which <= 2; which++) {
+            CombineArgs ca = {};
+            ca.b = b; ca.energy = p->energy; ca.eta = p->eta; ca.use_z = 1; ca.coef = -1.0;
+            ca.H = (const cplx*)p->H_upper; ca.fH = s.sb; ca.S = (const cplx*)p->S_upper; ca.fS = s.sb; ca.s_identity = 0;
+            ca.dagger = (which == 2);
+            ca.out = which == 1 ? W.Aup : W.Alow; ca.sout = s.sm; ca.fout = s.sb; ca.nfam = n - 1;
+            if (sigma_r && sigma_r->kind == NEGF_SIGMA_BT) {
+                ca.blk[0] = (const cplx*)(which == 1 ? sigma_r->upper : sigma_r->lower);
+                ca.sblk[0] = s.sm; ca.fblk[0] = s.sb; ca.only[0] = -1;
+            }
+            if (n - 1 == 1) ca.nfam = 1;
+            NEGF_TRY(ew_combine(ctx, ca, ne));
+        }
+    }
+
+    // S3 forward: g_0 = A_00^-1 ; Y_{i-1} = A_{i,i-1} g_{i-1} ; g_i = (A_ii - Y_{i-1} A_{i-1,i})^-1
+    for (int i = 0; i < n; i++) {
+        if (i > 0) {
+            NEGF_TRY(zgemm_launch(ctx, gemm_one(s, real(F.sgn), F.AL, i - 1, F.g, i - 1, ZERO, nullptr, 0, F.Y, i - 1)));
+            NEGF_TRY(zgemm_launch(ctx, gemm_one(s, real(-F.sgn), F.Y, i - 1, F.AU, i - 1, ONE, &F.g, i, F.g, i)));
+        }
+        NEGF_TRY(zinv_launch(ctx, b, W.g + s.bb * i, s.sn, ne, W.inv, info, i + 1, nullptr));
     }
     // S4 backward
-    NEGF_TRY(ew_copy(ctx, s.bb, ne, GRd + s.bb * (n - 1), s.sn, W.g + s.bb * (n - 1), s.sn, nullptr));
-    cplx* col = T3; cplx* coln = T5;
-    if (GR_corner_) NEGF_TRY(ew_copy(ctx, s.bb, ne, col, s.sb, W.g + s.bb * (n - 1), s.sn, nullptr));
+    NEGF_TRY(ew_copy(ctx, s.bb, ne, (cplx*)GR_diag_ + s.bb * (n - 1), s.sn, W.g + s.bb * (n - 1), s.sn, nullptr));
+    if (n > 1) NEGF_TRY(launch_fam(ctx, s, real(F.sgn), F.g, 0, F.AU, 0, ZERO, nullptr, 0, F.X, 0, n - 1));   // X_i, all i
+    cplx* col = W.T[3]; cplx* coln = W.T[5];
+    if (GR_corner_) NEGF_TRY(ew_copy(ctx, s.bb, ne, n > 1 ? col : (cplx*)GR_corner_, s.sb, W.g + s.bb * (n - 1), s.sn, nullptr));
+    const Opnd GRu = GR_upper_ ? Opnd{(const cplx*)GR_upper_, s.sm, s.sb, 0} : Opnd{W.T[4], s.sb, 0, 0};
+    const Opnd GRl = {(const cplx*)GR_lower_, s.sm, s.sb, 0};
     for (int i = n - 2; i >= 0; i--) {
-        cplx* gi = W.g + s.bb * i; cplx* Xi = W.X + s.bb * i; cplx* Yi = W.Y + s.bb * i;
-        cplx* Gnext = GRd + s.bb * (i + 1);
-        NEGF_TRY(assemble_a(ctx, p, sigma_r, s, 1, i, T2, s.sb));                              // A_{i,i+1}
-        NEGF_TRY(zgemm_bb(ctx, 0, 0, b, ONE, gi, s.sn, T2, s.sb, ZERO, nullptr, 0, Xi, s.sm, ne, nullptr));
-        cplx* Gu = GRu ? GRu + s.bb * i : T4; long long sGu = GRu ? s.sm : s.sb;
-        NEGF_TRY(zgemm_bb(ctx, 0, 0, b, MONE, Xi, s.sm, Gnext, s.sn, ZERO, nullptr, 0, Gu, sGu, ne, nullptr));
-        if (GRl) NEGF_TRY(zgemm_bb(ctx, 0, 0, b, MONE, Gnext, s.sn, Yi, s.sm, ZERO, nullptr, 0,
-                                   GRl + s.bb * i, s.sm, ne, nullptr));
-        NEGF_TRY(zgemm_bb(ctx, 0, 0, b, MONE, Gu, sGu, Yi, s.sm, ONE, gi, s.sn, GRd + s.bb * i, s.sn, ne, nullptr));
-        if (GR_corner_) {
-            NEGF_TRY(zgemm_bb(ctx, 0, 0, b, MONE, Xi, s.sm, col, s.sb, ZERO, nullptr, 0, coln, s.sb, ne, nullptr));
+        GemmGroup grp; grp.ng = 0;
+        grp.g[grp.ng++] = gemm_one(s, MONE, F.X, i, GRd, i + 1, ZERO, nullptr, 0, GRu, GR_upper_ ? i : 0);   // G_{i,i+1}
+        if (GR_lower_) grp.g[grp.ng++] = gemm_one(s, MONE, GRd, i + 1, F.Y, i, ZERO, nullptr, 0, GRl, i);     // G_{i+1,i}
+        if (GR_corner_) {                                                                                     // G_{i,n-1}
+            cplx* dst = (i == 0) ? (cplx*)GR_corner_ : coln;
+            grp.g[grp.ng++] = gemm_one(s, MONE, F.X, i, Opnd{col, s.sb, 0, 0}, 0, ZERO, nullptr, 0, Opnd{dst, s.sb, 0, 0}, 0);
             cplx* t = col; col = coln; coln = t;
         }
+        NEGF_TRY(zgemm_launch_group(ctx, grp));
+        NEGF_TRY(zgemm_launch(ctx, gemm_one(s, MONE, GRu, GR_upper_ ? i : 0, F.Y, i, ONE, &F.g, i, GRd, i)));  // G_ii
     }
-    if (GR_corner_) NEGF_TRY(ew_copy(ctx, s.bb, ne, (cplx*)GR_corner_, s.sb, col, s.sb, nullptr));
-    if (flags & NEGF_KEEP_SWEEP) { ctx->sweep_valid = true; ctx->sw_n = n; ctx->sw_b = b; ctx->sw_ne = ne; }
+    if (flags & NEGF_KEEP_SWEEP) { ctx->sweep_valid = true; ctx->sw_n = n; ctx->sw_b = b; ctx->sw_ne = ne; ctx->sw_assembled = assembled; }
     return NEGF_OK;
 }
 
 namespace {
 
-// S5 + S6 for one of </>.  GXd [NE][n][b][b] required, GXu [NE][n-1][b][b] optional.
-int lesser_greater_one(negf_ctx* ctx, const negf_problem* p, const negf_sigma* sr, const negf_sigma* sx,
-                       const Shape& s, Workspace& W, const cplx* GRd, cplx* GXd, cplx* GXu) {
-    const int b = s.b, ne = s.ne, n = s.n;
-    cplx *T0 = W.T[0], *T1 = W.T[1], *T2 = W.T[2], *T3 = W.T[3], *T4 = W.T[4], *T5 = W.T[5],
-         *T6 = W.T[6], *T7 = W.T[7], *T8 = W.T[8];
-    bool zero_blk;
-    // S5 forward: g^x_0 = g_0 B_00 g_0^H
-    NEGF_TRY(assemble_b(ctx, sx, s, 0, 0, T0, &zero_blk));
-    NEGF_TRY(zgemm_bb(ctx, 0, 0, b, ONE, W.g, s.sn, T0, s.sb, ZERO, nullptr, 0, T1, s.sb, ne, nullptr));
-    NEGF_TRY(zgemm_bb(ctx, 0, 1, b, ONE, T1, s.sb, W.g, s.sn, ZERO, nullptr, 0, W.gx, s.sn, ne, nullptr));
-    for (int i = 1; i < n; i++) {
-        cplx* gi = W.g + s.bb * i; cplx* Yp = W.Y + s.bb * (i - 1);
-        NEGF_TRY(assemble_b(ctx, sx, s, 0, i, T0, &zero_blk));                    // B_ii
-        NEGF_TRY(assemble_a(ctx, p, sr, s, 2, i - 1, T1, s.sb));                  // A_{i,i-1}
-        NEGF_TRY(zgemm_bb(ctx, 0, 0, b, ONE, T1, s.sb, W.gx + s.bb * (i - 1), s.sn, ZERO, nullptr, 0,
-                          T2, s.sb, ne, nullptr));                                // A_{i,i-1} g^x_{i-1}
-        NEGF_TRY(zgemm_bb(ctx, 0, 1, b, ONE, T2, s.sb, T1, s.sb, ONE, T0, s.sb, T3, s.sb, ne, nullptr));
-        NEGF_TRY(assemble_b(ctx, sx, s, 1, i - 1, T4, &zero_blk));                // B_{i-1,i}
-        if (!zero_blk) {
-            // - Y B_up - B_low Y^H = -(W - W^H), W = Y_{i-1} B_{i-1,i}   (B_low = -B_up^H)
-            NEGF_TRY(zgemm_bb(ctx, 0, 0, b, ONE, Yp, s.sm, T4, s.sb, ZERO, nullptr, 0, T5, s.sb, ne, nullptr));
-            NEGF_TRY(ew_antiherm_add(ctx, b, ne, T3, s.sb, T3, s.sb, T5, s.sb, -1.0));
+// B_ii contribution of the boundary blocks at the two ends: gx_i (+)= g_i B g_i^H
+int add_boundary_w(negf_ctx* ctx, const Shape& s, const Fams& F, const Workspace& W, const cplx* bnd, int i, bool accumulate) {
+    if (!bnd) return NEGF_OK;
+    const Opnd Bn = {bnd, s.sb, 0, 0}, T = {W.T[0], s.sb, 0, 0};
+    NEGF_TRY(zgemm_launch(ctx, gemm_one(s, ONE, F.g, i, Bn, 0, ZERO, nullptr, 0, T, 0)));
+    return zgemm_launch(ctx, gemm_one(s, ONE, T, 0, dag(F.g), i, accumulate ? ONE : ZERO, accumulate ? &F.gx : nullptr, i, F.gx, i));
+}
+
+// S5, hoisted form: g^x_i = W_i + Z_i g^x_{i-1} Z_i^H
+int s5_hoisted(negf_ctx* ctx, const Shape& s, const Fams& F, const Workspace& W, const negf_sigma* sx) {
+    const int n = s.n, ne = s.ne, b = s.b;
+    bool have_w = false;     // interior W_i present in the gx family
+    if (sx->kind == NEGF_SIGMA_SCALAR) {
+        NEGF_TRY(launch_fam(ctx, s, ONE, F.g, 0, dag(F.g), 0, ZERO, nullptr, 0, F.gx, 0, n, (const cplx*)sx->scalar));
+        have_w = true;
+    } else if (sx->kind == NEGF_SIGMA_BT) {
+        const Opnd Sd = {(const cplx*)sx->diag, s.sn, s.sb, 0}, Su = {(const cplx*)sx->upper, s.sm, s.sb, 0};
+        // bracket_i = Sigma_ii - (V_i - V_i^H), V_i = Y_{i-1} Sigma_{i-1,i} (i >= 1), built in the gx family
+        NEGF_TRY(ew_copy(ctx, s.bb, ne, W.gx, s.sn, Sd.p, s.sn, nullptr));
+        if (n > 1) {
+            NEGF_TRY(launch_fam(ctx, s, ONE, F.Y, 0, Su, 0, ZERO, nullptr, 0, F.Q, 1, n - 1));
+            for (int i = 1; i < n; i++)
+                NEGF_TRY(ew_antiherm_add(ctx, b, ne, W.gx + s.bb * i, s.sn, Sd.p + s.bb * i, s.sn, W.Q + s.bb * i, s.sn, -1.0));
         }
-        NEGF_TRY(zgemm_bb(ctx, 0, 0, b, ONE, gi, s.sn, T3, s.sb, ZERO, nullptr, 0, T2, s.sb, ne, nullptr));
-        NEGF_TRY(zgemm_bb(ctx, 0, 1, b, ONE, T2, s.sb, gi, s.sn, ZERO, nullptr, 0, W.gx + s.bb * i, s.sn, ne, nullptr));
+        NEGF_TRY(launch_fam(ctx, s, ONE, F.g, 0, F.gx, 0, ZERO, nullptr, 0, F.Q, 0, n));
+        NEGF_TRY(launch_fam(ctx, s, ONE, F.Q, 0, dag(F.g), 0, ZERO, nullptr, 0, F.gx, 0, n));
+        have_w = true;
     }
+    bool first_set = have_w;
+    if (sx->left) { NEGF_TRY(add_boundary_w(ctx, s, F, W, (const cplx*)sx->left, 0, first_set)); first_set = true; }
+    if (n == 1 && sx->right) { NEGF_TRY(add_boundary_w(ctx, s, F, W, (const cplx*)sx->right, 0, first_set)); first_set = true; }
+    if (!first_set)          // g^x_0 = 0
+        NEGF_CUDA_CHECK(ctx, cudaMemset2DAsync(W.gx, (size_t)s.sn * sizeof(cplx), 0, s.bb * sizeof(cplx), ne, ctx->stream));
+    bool last_has_w = have_w;
+    if (n > 1 && sx->right) { NEGF_TRY(add_boundary_w(ctx, s, F, W, (const cplx*)sx->right, n - 1, have_w)); last_has_w = true; }
+    if (n == 1) return NEGF_OK;
+    NEGF_TRY(launch_fam(ctx, s, real(F.sgn), F.g, 1, F.AL, 0, ZERO, nullptr, 0, F.Z, 0, n - 1));      // Z_i = g_i A_{i,i-1}
+    const Opnd T = {W.T[1], s.sb, 0, 0};
+    for (int i = 1; i < n; i++) {
+        const bool w = (i == n - 1) ? last_has_w : have_w;
+        NEGF_TRY(zgemm_launch(ctx, gemm_one(s, ONE, F.Z, i - 1, F.gx, i - 1, ZERO, nullptr, 0, T, 0)));
+        NEGF_TRY(zgemm_launch(ctx, gemm_one(s, ONE, T, 0, dag(F.Z), i - 1, w ? ONE : ZERO, w ? &F.gx : nullptr, i, F.gx, i)));
+    }
+    return NEGF_OK;
+}
+
+// S5, textbook form (fewest products when Sigma^x_S is dense): g^x_i = g_i [B_ii + A g^x_{i-1} A^H - (V - V^H)] g_i^H
+int s5_textbook(negf_ctx* ctx, const Shape& s, const Fams& F, const Workspace& W, const negf_sigma* sx) {
+    const int n = s.n, ne = s.ne, b = s.b;
+    const Opnd T0 = {W.T[0], s.sb, 0, 0}, T2 = {W.T[2], s.sb, 0, 0}, T3 = {W.T[3], s.sb, 0, 0}, T5 = {W.T[5], s.sb, 0, 0};
+    for (int i = 0; i < n; i++) {
+        // B_ii into T0
+        CombineArgs ca = {};
+        ca.b = b; ca.use_z = 0; ca.coef = 1.0; ca.out = W.T[0]; ca.sout = s.sb;
+        int nb = 0;
+        if (sx->kind == NEGF_SIGMA_SCALAR) ca.scalar = (const cplx*)sx->scalar;
+        if (sx->kind == NEGF_SIGMA_BT) { ca.blk[nb] = (const cplx*)sx->diag + s.bb * i; ca.sblk[nb] = s.sn; nb++; }
+        if (i == 0 && sx->left) { ca.blk[nb] = (const cplx*)sx->left; ca.sblk[nb] = s.sb; nb++; }
+        if (i == n - 1 && sx->right) { ca.blk[nb] = (const cplx*)sx->right; ca.sblk[nb] = s.sb; nb++; }
+        NEGF_TRY(ew_combine(ctx, ca, ne));
+        const Opnd* M = &T0;
+        if (i > 0) {
+            NEGF_TRY(zgemm_launch(ctx, gemm_one(s, real(F.sgn), F.AL, i - 1, F.gx, i - 1, ZERO, nullptr, 0, T2, 0)));
+            NEGF_TRY(zgemm_launch(ctx, gemm_one(s, real(F.sgn), T2, 0, dag(F.AL), i - 1, ONE, &T0, 0, T3, 0)));
+            if (sx->kind == NEGF_SIGMA_BT) {
+                const Opnd Su = {(const cplx*)sx->upper, s.sm, s.sb, 0};
+                NEGF_TRY(zgemm_launch(ctx, gemm_one(s, ONE, F.Y, i - 1, Su, i - 1, ZERO, nullptr, 0, T5, 0)));
+                NEGF_TRY(ew_antiherm_add(ctx, b, ne, W.T[3], s.sb, W.T[3], s.sb, W.T[5], s.sb, -1.0));
+            }
+            M = &T3;
+        }
+        NEGF_TRY(zgemm_launch(ctx, gemm_one(s, ONE, F.g, i, *M, 0, ZERO, nullptr, 0, T2, 0)));
+        NEGF_TRY(zgemm_launch(ctx, gemm_one(s, ONE, T2, 0, dag(F.g), i, ZERO, nullptr, 0, F.gx, i)));
+    }
+    return NEGF_OK;
+}
+
+// S5 + S6 for one of </>.  GXd [NE][n][b][b] required, GXu [NE][n-1][b][b] optional.
+int lesser_greater_one(negf_ctx* ctx, const negf_problem* p, const negf_sigma* sx, const Shape& s, const Workspace& W,
+                       const Fams& F, const cplx* GRd_, cplx* GXd_, cplx* GXu_) {
+    (void)p;
+    const int ne = s.ne, n = s.n;
+    const bool dense_sx = sx->kind != NEGF_SIGMA_NONE;
+    if (dense_sx && s.b > NEGF_PAIR_MAX_B) NEGF_TRY(s5_textbook(ctx, s, F, W, sx));
+    else NEGF_TRY(s5_hoisted(ctx, s, F, W, sx));
     // S6 backward
-    NEGF_TRY(ew_copy(ctx, s.bb, ne, GXd + s.bb * (n - 1), s.sn, W.gx + s.bb * (n - 1), s.sn, nullptr));
+    NEGF_TRY(ew_copy(ctx, s.bb, ne, GXd_ + s.bb * (n - 1), s.sn, W.gx + s.bb * (n - 1), s.sn, nullptr));
+    if (n == 1) return NEGF_OK;
+    const Opnd GRd = {GRd_, s.sn, s.sb, 0}, GXd = {GXd_, s.sn, s.sb, 0};
+    const Opnd Qf = GXu_ ? Opnd{GXu_, s.sm, s.sb, 0} : Opnd{W.Q, s.sn, s.sb, 0};
+    // T2_i = -g^x_i A_{i+1,i}^H (+ g_i Sigma_{i,i+1}) into the Z family
+    NEGF_TRY(launch_fam(ctx, s, real(-F.sgn), F.gx, 0, dag(F.AL), 0, ZERO, nullptr, 0, F.Z, 0, n - 1));
+    if (sx->kind == NEGF_SIGMA_BT) {
+        const Opnd Su = {(const cplx*)sx->upper, s.sm, s.sb, 0};
+        NEGF_TRY(launch_fam(ctx, s, ONE, F.g, 0, Su, 0, ONE, &F.Z, 0, F.Z, 0, n - 1));
+    }
+    NEGF_TRY(launch_fam(ctx, s, ONE, F.Z, 0, dag(GRd), 1, ZERO, nullptr, 0, Qf, 0, n - 1));          // Q_i
+    NEGF_TRY(launch_fam(ctx, s, MONE, Qf, 0, dag(F.X), 0, ONE, &F.gx, 0, GXd, 0, n - 1));            // P_i
     for (int i = n - 2; i >= 0; i--) {
-        cplx* gi = W.g + s.bb * i; cplx* gxi = W.gx + s.bb * i; cplx* Xi = W.X + s.bb * i;
-        const cplx* GRn = GRd + s.bb * (i + 1); cplx* GXn = GXd + s.bb * (i + 1);
-        NEGF_TRY(assemble_a(ctx, p, sr, s, 2, i, T1, s.sb));                      // A_{i+1,i}
-        NEGF_TRY(zgemm_bb(ctx, 0, 1, b, MONE, gxi, s.sn, T1, s.sb, ZERO, nullptr, 0, T2, s.sb, ne, nullptr));
-        NEGF_TRY(assemble_b(ctx, sx, s, 1, i, T4, &zero_blk));                    // B_{i,i+1}
-        if (!zero_blk)
-            NEGF_TRY(zgemm_bb(ctx, 0, 0, b, ONE, gi, s.sn, T4, s.sb, ONE, T2, s.sb, T2, s.sb, ne, nullptr));
-        NEGF_TRY(zgemm_bb(ctx, 0, 1, b, ONE, T2, s.sb, GRn, s.sn, ZERO, nullptr, 0, T3, s.sb, ne, nullptr));  // Q
-        NEGF_TRY(zgemm_bb(ctx, 0, 0, b, ONE, Xi, s.sm, GXn, s.sn, ZERO, nullptr, 0, T5, s.sb, ne, nullptr));  // R
-        cplx* Gu = GXu ? GXu + s.bb * i : T6; long long sGu = GXu ? s.sm : s.sb;
-        NEGF_TRY(ew_sub(ctx, b, ne, Gu, sGu, T3, s.sb, T5, s.sb));                // G^x_{i,i+1} = Q - R
-        NEGF_TRY(zgemm_bb(ctx, 0, 1, b, ONE, Xi, s.sm, Gu, sGu, ZERO, nullptr, 0, T7, s.sb, ne, nullptr));    // V
-        NEGF_TRY(zgemm_bb(ctx, 0, 1, b, MONE, T5, s.sb, Xi, s.sm, ONE, gxi, s.sn, T8, s.sb, ne, nullptr));    // Z
-        NEGF_TRY(ew_antiherm_add(ctx, b, ne, GXd + s.bb * i, s.sn, T8, s.sb, T7, s.sb, 1.0));
+        NEGF_TRY(zgemm_launch(ctx, gemm_one(s, MONE, F.X, i, GXd, i + 1, ONE, &Qf, i, Qf, i)));     // G^x_{i,i+1}
+        NEGF_TRY(zgemm_launch(ctx, gemm_one(s, ONE, F.X, i, dag(Qf), i, ONE, &GXd, i, GXd, i)));    // G^x_ii
     }
     return NEGF_OK;
 }
@@ -222,13 +320,16 @@ extern "C" int negf_rgf_lesser_greater(negf_ctx* ctx, const negf_problem* p, con
     if (sigma_lesser && !GL_diag) return NEGF_EINVAL;
     if (sigma_greater && !GG_diag) return NEGF_EINVAL;
     if (!ctx->ws) return NEGF_ENOWORKSPACE;
-    Workspace W = carve_workspace(ctx->ws, s.n, s.b, s.ne);
+    const bool assembled = needs_assembly(p, sigma_r);
+    Workspace W = carve_workspace(ctx->ws, s.n, s.b, s.ne, assembled);
     if (W.bytes > ctx->ws_bytes) return NEGF_ENOWORKSPACE;
-    if (!ctx->sweep_valid || ctx->sw_n != s.n || ctx->sw_b != s.b || ctx->sw_ne != s.ne) return NEGF_ENOSTATE;
+    if (!ctx->sweep_valid || ctx->sw_n != s.n || ctx->sw_b != s.b || ctx->sw_ne != s.ne || ctx->sw_assembled != assembled)
+        return NEGF_ENOSTATE;
+    const Fams F = make_fams(p, s, W, assembled);
     NEGF_TRY(ew_fill_int(ctx, info, s.ne, 0));
     if (sigma_lesser)
-        NEGF_TRY(lesser_greater_one(ctx, p, sigma_r, sigma_lesser, s, W, (const cplx*)GR_diag, (cplx*)GL_diag, (cplx*)GL_upper));
+        NEGF_TRY(lesser_greater_one(ctx, p, sigma_lesser, s, W, F, (const cplx*)GR_diag, (cplx*)GL_diag, (cplx*)GL_upper));
     if (sigma_greater)
-        NEGF_TRY(lesser_greater_one(ctx, p, sigma_r, sigma_greater, s, W, (const cplx*)GR_diag, (cplx*)GG_diag, (cplx*)GG_upper));
+        NEGF_TRY(lesser_greater_one(ctx, p, sigma_greater, s, W, F, (const cplx*)GR_diag, (cplx*)GG_diag, (cplx*)GG_upper));
     return NEGF_OK;
 }

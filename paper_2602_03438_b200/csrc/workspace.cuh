@@ -11,6 +11,10 @@ struct Workspace {
     cplx* X;        // [NE][n-1][b][b]  X_i = g_i A_{i,i+1}       (retained)
     cplx* Y;        // [NE][n-1][b][b]  Y_i = A_{i+1,i} g_i       (retained)
     cplx* gx;       // [NE][n][b][b]    left-connected g^x_i (one of </> at a time)
+    cplx* Z;        // [NE][n-1][b][b]  Z_i = g_i A_{i,i-1} (S5), then T2_i (S6)
+    cplx* Q;        // [NE][n][b][b]    S5 temporaries, then Q_i when G^x_upper is not requested
+    cplx* Aup;      // [NE][n-1][b][b]  A_{i,i+1}, only when S != I or Sigma^R_S is BT   (retained)
+    cplx* Alow;     // [NE][n-1][b][b]  A_{i+1,i}, likewise                              (retained)
     cplx* T[NEGF_NSCRATCH];   // [NE][b][b] each
     void* inv;      // zinv workspace
     double* ref;    // [NE]
@@ -21,7 +25,8 @@ struct Workspace {
     size_t bytes;
 };
 
-inline Workspace carve_workspace(void* base, int n, int b, int ne) {
+// Aup / Alow sit at the END so that every other offset is independent of `assembled`.
+inline Workspace carve_workspace(void* base, int n, int b, int ne, bool assembled = false) {
     Workspace w;
     unsigned char* p = (unsigned char*)base;
     const size_t blk = (size_t)b * b * sizeof(cplx);
@@ -30,6 +35,8 @@ inline Workspace carve_workspace(void* base, int n, int b, int ne) {
     w.X = (cplx*)take(blk * (n > 1 ? n - 1 : 0) * ne);
     w.Y = (cplx*)take(blk * (n > 1 ? n - 1 : 0) * ne);
     w.gx = (cplx*)take(blk * n * ne);
+    w.Z = (cplx*)take(blk * (n > 1 ? n - 1 : 0) * ne);
+    w.Q = (cplx*)take(blk * n * ne);
     const int tm = negf_tmul(b);
     for (int t = 0; t < NEGF_NSCRATCH; t++) w.T[t] = (cplx*)take(blk * ne * tm);
     w.inv = take(zinv_workspace_bytes(b, ne * tm));
@@ -38,6 +45,11 @@ inline Workspace carve_workspace(void* base, int n, int b, int ne) {
     w.sing = (int*)take(sizeof(int) * ne * 2);
     w.tmpinfo = (int*)take(sizeof(int) * ne * 2);
     w.its = (int*)take(sizeof(int) * ne * 2);
+    w.Aup = w.Alow = nullptr;
+    if (assembled) {
+        w.Aup = (cplx*)take(blk * (n > 1 ? n - 1 : 0) * ne);
+        w.Alow = (cplx*)take(blk * (n > 1 ? n - 1 : 0) * ne);
+    }
     w.bytes = (size_t)(p - (unsigned char*)base);
     return w;
 }

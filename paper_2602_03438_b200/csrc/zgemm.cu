@@ -80,13 +80,13 @@ __global__ void __launch_bounds__(WM * WN * 32, MINB) zgemm_kernel(const __grid_
     cplx* sA = reinterpret_cast<cplx*>(smem_raw);              // STAGES x BM x BK
     cplx* sB = sA + STAGES * BM * BK;                          // STAGES x BN x BK
 
-    const int e = blockIdx.y;
+    const int e = blockIdx.y % a.batch, e2 = blockIdx.y / a.batch;
     if (a.skip && a.skip[e]) return;
     const int tiles_n = (a.n + BN - 1) / BN;
     const int tm = blockIdx.x / tiles_n, tn = blockIdx.x % tiles_n;
     const int m0 = tm * BM, n0 = tn * BN;
-    const cplx* gA = a.A + (size_t)e * a.sA;
-    const cplx* gB = a.B + (size_t)e * a.sB;
+    const cplx* gA = a.A + (size_t)e * a.sA + (size_t)e2 * a.sA2;
+    const cplx* gB = a.B + (size_t)e * a.sB + (size_t)e2 * a.sB2;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int wm0 = (warp / WN) * (MI * 8), wn0 = (warp % WN) * (NI * 8);
     const int lr = lane >> 2, lk = lane & 3;
@@ -151,9 +151,9 @@ __global__ void __launch_bounds__(WM * WN * 32, MINB) zgemm_kernel(const __grid_
     cp_async_wait<0>();
 
     // epilogue: C = alpha*acc + beta*D
-    cplx* gC = a.C + (size_t)e * a.sC;
-    const cplx* gD = a.D ? a.D + (size_t)e * a.sD : nullptr;
-    const cplx al = a.alpha, be = a.beta;
+    cplx* gC = a.C + (size_t)e * a.sC + (size_t)e2 * a.sC2;
+    const cplx* gD = a.D ? a.D + (size_t)e * a.sD + (size_t)e2 * a.sD2 : nullptr;
+    const cplx al = a.alpha_vec ? cmul(a.alpha, a.alpha_vec[e]) : a.alpha, be = a.beta;
 #pragma unroll
     for (int i = 0; i < MI; i++) {
         int row = m0 + wm0 + i * 8 + lr;
@@ -184,7 +184,7 @@ int launch_cfg(negf_ctx* ctx, const GemmGroup& grp) {
         attr_done = true;
     }
     int tiles = ((a.m + BM - 1) / BM) * ((a.n + BN - 1) / BN);
-    dim3 grid(tiles, a.batch, grp.ng);
+    dim3 grid(tiles, a.batch * a.batch2, grp.ng);
     kern<<<grid, WM * WN * 32, smem, ctx->stream>>>(grp);
     NEGF_LAUNCH_CHECK(ctx);
     return NEGF_OK;
@@ -207,16 +207,17 @@ int zgemm_launch_group(negf_ctx* ctx, const GemmGroup& grp) {
     const GemmArgs& a = grp.g[0];
     if (a.m <= 0 || a.n <= 0 || a.batch <= 0) return NEGF_OK;
     if (a.k < 0 || (a.opA | a.opB) & ~1) return NEGF_EINVAL;
-    if (a.batch > 65535) return NEGF_EUNSUPPORTED;
+    if (a.batch2 < 1 || (long long)a.batch * a.batch2 > 65535) return NEGF_EUNSUPPORTED;
     for (int i = 1; i < grp.ng; i++) {      // one grid serves every member: same shape, ops and batch
         const GemmArgs& o = grp.g[i];
-        if (o.m != a.m || o.n != a.n || o.k != a.k || o.opA != a.opA || o.opB != a.opB || o.batch != a.batch)
+        if (o.m != a.m || o.n != a.n || o.k != a.k || o.opA != a.opA || o.opB != a.opB || o.batch != a.batch ||
+            o.batch2 != a.batch2)
             return NEGF_EINVAL;
     }
     // Tile choice: the largest CTA tile that still gives every SM work.  128x64 (8 warps, 32x32 warp
     // tiles, 1 CTA/SM) in the compute-bound regime; 64x64 (4 warps); 32x32 (4 warps of 16x16, up to
     // 4 CTAs/SM) when the batch of small blocks would otherwise leave most SMs idle.
-    const long long per = (long long)a.batch * grp.ng;
+    const long long per = (long long)a.batch * a.batch2 * grp.ng;
     const long long t128 = (long long)((a.m + 127) / 128) * ((a.n + 63) / 64) * per;
     const long long t64 = (long long)((a.m + 63) / 64) * ((a.n + 63) / 64) * per;
     if (a.m > 64 && t128 >= ctx->num_sms) return launch_ops<128, 64, 4, 2, 1>(ctx, grp);
@@ -236,6 +237,7 @@ GemmArgs zgemm_bb_args(int opA, int opB, int b, cplx alpha, const cplx* A, long 
     g.opA = opA; g.opB = opB; g.m = g.n = g.k = b; g.alpha = alpha; g.beta = beta;
     g.A = A; g.lda = b; g.sA = sA; g.B = B; g.ldb = b; g.sB = sB;
     g.D = D; g.sD = sD; g.C = C; g.ldc = b; g.sC = sC; g.batch = batch; g.skip = skip;
+    g.batch2 = 1; g.sA2 = g.sB2 = g.sD2 = g.sC2 = 0; g.alpha_vec = nullptr;
     return g;
 }
 int zgemm_bb(negf_ctx* ctx, int opA, int opB, int b, cplx alpha, const cplx* A, long long sA,
@@ -257,5 +259,6 @@ extern "C" int negf_zgemm_batched(negf_ctx* ctx, int opA, int opB, int m, int n,
     g.B = (const cplx*)B; g.ldb = ldb; g.sB = strideB;
     g.D = (const cplx*)D; g.sD = strideC;
     g.C = (cplx*)C; g.ldc = ldc; g.sC = strideC; g.batch = batch; g.skip = nullptr;
+    g.batch2 = 1; g.sA2 = g.sB2 = g.sD2 = g.sC2 = 0; g.alpha_vec = nullptr;
     return zgemm_launch(ctx, g);
 }

@@ -567,6 +567,7 @@ int zinv_launch(negf_ctx* ctx, int b, cplx* A, long long sA, int batch, void* ws
         // P' = [-T Dinv ; Dinv ; -L21 Linv]
         GemmArgs g;
         g.opA = 0; g.opB = 0; g.alpha = mone; g.beta = zero; g.D = nullptr; g.sD = 0; g.batch = batch; g.skip = skip;
+        g.batch2 = 1; g.sA2 = g.sB2 = g.sD2 = g.sC2 = 0; g.alpha_vec = nullptr;
         g.n = wk; g.k = wk; g.ldb = wk; g.sB = PW * PW; g.ldc = wk; g.sC = (long long)b * wk; g.lda = b; g.sA = sA;
         if (k0 > 0) {
             g.m = k0; g.A = A + k0; g.B = W.Dinv; g.C = W.Pbuf;

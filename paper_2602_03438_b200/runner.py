@@ -51,7 +51,8 @@ class DevicePath:
             else:
                 self.sig_dev[t] = {"kind": "bt", "diag": _dev(s["diag"], d), "upper": _dev(s["upper"], d),
                                    "lower": _dev(s.get("lower"), d)}
-        ws_bytes = negf.Context.workspace_bytes(self.problem)
+        kind_r = _KIND[self.sig_dev['r']['kind']] if self.sig_dev['r'] is not None else negf.SIGMA_NONE
+        ws_bytes = negf.Context.workspace_bytes(self.problem, kind_r)
         self.workspace = torch.empty(ws_bytes, dtype=torch.uint8, device=d)
         self.ctx.set_workspace(self.workspace)
         self.ctx.set_stream(torch.cuda.current_stream(d).cuda_stream)
