@@ -402,28 +402,201 @@ __global__ void __launch_bounds__(PANEL_NT, 1) gj_panel_cluster_kernel(PanelArgs
 }
 
 // ------------------------------------------------------------------------------------------------
+// step 1, register-resident variant (tall panels up to 8 x 256 rows): every thread owns ONE row of
+// the width-32 panel in registers, a cluster of C CTAs covers the rows >= k0.  Per column: one
+// redux-based candidate per CTA, one DSMEM exchange (candidate value, row index, row content and
+// the current diagonal row) and one cluster barrier; the elimination runs out of registers.  The
+// kernel also finishes the panel in place: rows below the diagonal block leave as -L21 L11^-1,
+// the diagonal block as (L11 U11)^-1, so the trailing GEMM reads P' straight from A's columns.
+// ------------------------------------------------------------------------------------------------
+struct RegPanelSmem {
+    cplx candrow[2][CMAX][PW];
+    cplx diagrow[2][PW];
+    cplx rowstage[PW];
+    cplx drowstage[PW];
+    cplx Dm[PW * PW];      // factored diagonal block L11 \ U11
+    cplx Li[PW * PW];      // L11^-1 (every CTA gets a copy)
+    cplx Ui[PW * PW];      // U11^-1 (CTA 0)
+    unsigned long long red_key[8];
+    int red_row[8];
+    unsigned long long cand_key[2][CMAX];
+    int cand_row[2][CMAX];
+};
+
+template <int NT>
+__global__ void __launch_bounds__(NT) gj_panel_reg_kernel(PanelArgs a) {
+    cg::cluster_group cluster = cg::this_cluster();
+    const int rank = (int)cluster.block_rank();
+    const int C = (int)cluster.num_blocks();
+    const int e = blockIdx.y;
+    if (a.skip && a.skip[e]) return;              // uniform over the cluster
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    RegPanelSmem& S = *reinterpret_cast<RegPanelSmem*>(smem_raw);
+    const int w = a.w, b = a.b, k0 = a.k0;
+    const int rows_total = b - k0;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int gr = rank * NT + tid;               // candidate row index (global row k0 + gr)
+    const bool valid = gr < rows_total;
+    cplx* g = a.A + (size_t)e * a.sA + (size_t)k0 * b + k0;       // panel origin
+    cplx P[PW];
+#pragma unroll
+    for (int c = 0; c < PW; c++) P[c] = (valid && c < w) ? g[(size_t)gr * b + c] : cmake(0.0, 0.0);
+    constexpr int NONE = 0x7fffffff;
+
+#pragma unroll
+    for (int j = 0; j < PW; j++) {
+        if (j < w) {
+            const int par = j & 1;
+            // CTA candidate: largest |re|+|im| among my rows with index >= j (smallest row on ties)
+            const bool has = valid && gr >= j;
+            const unsigned long long key = has ? (unsigned long long)__double_as_longlong(cabs1(P[j])) : 0ull;
+            const unsigned hi = __reduce_max_sync(0xffffffffu, has ? (unsigned)(key >> 32) : 0u);
+            const bool mh = has && (unsigned)(key >> 32) == hi;
+            const unsigned lo = __reduce_max_sync(0xffffffffu, mh ? (unsigned)key : 0u);
+            const bool ml = mh && (unsigned)key == lo;
+            const unsigned wrow = __reduce_min_sync(0xffffffffu, ml ? (unsigned)gr : (unsigned)NONE);
+            if (lane == 0) { S.red_key[warp] = ((unsigned long long)hi << 32) | lo; S.red_row[warp] = (int)wrow; }
+            __syncthreads();
+            unsigned long long bk = 0ull; int br = NONE;
+#pragma unroll
+            for (int q = 0; q < NT / 32; q++) {
+                const unsigned long long k2 = S.red_key[q]; const int r2 = S.red_row[q];
+                if (r2 != NONE && (br == NONE || k2 > bk || (k2 == bk && r2 < br))) { bk = k2; br = r2; }
+            }
+            if (gr == br) {
+#pragma unroll
+                for (int c = 0; c < PW; c++) S.rowstage[c] = P[c];
+            }
+            if (rank == 0 && tid == j) {
+#pragma unroll
+                for (int c = 0; c < PW; c++) S.drowstage[c] = P[c];
+            }
+            __syncthreads();
+            if (warp == 0) {       // push (value, row, row content) to every CTA; CTA 0 also the diagonal row
+                const cplx myrow = S.rowstage[lane];
+                const cplx drow = S.drowstage[lane];
+                for (int q = 0; q < C; q++) {
+                    RegPanelSmem* R = cluster.map_shared_rank(&S, q);
+                    R->candrow[par][rank][lane] = myrow;
+                    if (rank == 0) R->diagrow[par][lane] = drow;
+                    if (lane == 0) { R->cand_key[par][rank] = bk; R->cand_row[par][rank] = br; }
+                }
+            }
+            cluster.sync();
+            // everybody picks the same winner
+            int wq = 0, prow = NONE; unsigned long long wk = 0ull;
+            for (int q = 0; q < C; q++) {
+                const unsigned long long k2 = S.cand_key[par][q]; const int r2 = S.cand_row[par][q];
+                if (r2 != NONE && (prow == NONE || k2 > wk || (k2 == wk && r2 < prow))) { wk = k2; prow = r2; wq = q; }
+            }
+            const bool sing = (prow == NONE) || wk == 0ull;
+            if (prow == NONE) prow = j;
+            if (rank == 0 && tid == 0) {
+                a.ipiv[(size_t)e * b + k0 + j] = k0 + prow;
+                if (sing && a.info && a.info[e] == 0) a.info[e] = a.code > 0 ? a.code : (k0 + j + 1);
+            }
+            const cplx* pr = S.candrow[par][wq];
+            // exchange rows j <-> prow
+            if (valid && gr == prow && prow != j) {
+#pragma unroll
+                for (int c = 0; c < PW; c++) P[c] = S.diagrow[par][c];
+            }
+            if (rank == 0 && tid == j && prow != j) {
+#pragma unroll
+                for (int c = 0; c < PW; c++) P[c] = pr[c];
+            }
+            // eliminate below
+            if (valid && gr > j) {
+                const cplx rinv = sing ? cmake(0.0, 0.0) : crecip(pr[j]);
+                const cplx l = cmul(P[j], rinv);
+                P[j] = l;
+#pragma unroll
+                for (int c = j + 1; c < PW; c++) cfms(P[c], l, pr[c]);
+            }
+        }
+    }
+
+    // CTA 0: L11^-1 and U11^-1 from the w x w diagonal block, one thread per column; then
+    // (L11 U11)^-1 = U11^-1 L11^-1; L11^-1 goes to every CTA of the cluster.
+    if (rank == 0) {
+        for (int idx = tid; idx < PW * PW; idx += NT) { S.Li[idx] = cmake(0.0, 0.0); S.Ui[idx] = cmake(0.0, 0.0); }
+        if (tid < w) {
+#pragma unroll
+            for (int c = 0; c < PW; c++) S.Dm[tid * PW + c] = P[c];
+        }
+        __syncthreads();
+        if (tid < w) {
+            const int c = tid;
+            for (int r = 0; r < w; r++) {
+                cplx s = (r == c) ? cmake(1.0, 0.0) : cmake(0.0, 0.0);
+                for (int k = c; k < r; k++) cfms(s, S.Dm[r * PW + k], S.Li[k * PW + c]);
+                S.Li[r * PW + c] = (r < c) ? cmake(0.0, 0.0) : s;
+            }
+        } else if (tid >= 32 && tid < 32 + w) {
+            const int c = tid - 32;
+            for (int r = w - 1; r >= 0; r--) {
+                cplx s = (r == c) ? cmake(1.0, 0.0) : cmake(0.0, 0.0);
+                for (int k = r + 1; k <= c; k++) cfms(s, S.Dm[r * PW + k], S.Ui[k * PW + c]);
+                const cplx ur = S.Dm[r * PW + r];
+                const cplx inv = (ur.x == 0.0 && ur.y == 0.0) ? cmake(0.0, 0.0) : crecip(ur);
+                S.Ui[r * PW + c] = (r > c) ? cmake(0.0, 0.0) : cmul(s, inv);
+            }
+        }
+        __syncthreads();
+        cplx* gD = a.Dinv + (size_t)e * PW * PW;
+        for (int idx = tid; idx < w * w; idx += NT) {
+            const int r = idx / w, c = idx % w;
+            cplx s = cmake(0.0, 0.0);
+            for (int k = max(r, c); k < w; k++) cfma(s, S.Ui[r * PW + k], S.Li[k * PW + c]);
+            gD[r * w + c] = s;
+            g[(size_t)r * b + c] = s;                       // diagonal block of P' in place
+        }
+        for (int idx = tid; idx < PW * PW; idx += NT) {
+            const cplx v = S.Li[idx];
+            for (int q = 1; q < C; q++) cluster.map_shared_rank(&S, q)->Li[idx] = v;
+        }
+    }
+    cluster.sync();
+    // rows below the diagonal block: P' = -L21 L11^-1, written in place
+    if (valid && gr >= w) {
+        cplx* out = g + (size_t)gr * b;
+#pragma unroll
+        for (int c = 0; c < PW; c++) {
+            if (c < w) {
+                cplx acc = cmake(0.0, 0.0);
+#pragma unroll
+                for (int k = c; k < PW; k++) cfms(acc, P[k], S.Li[k * PW + c]);    // Li[k][c] = 0 for k >= w
+                out[c] = acc;
+            }
+        }
+    }
+    cluster.sync();   // nobody exits while remote shared memory may still be targeted
+}
+
+// ------------------------------------------------------------------------------------------------
 // step 2: apply the panel's row swaps to all other columns; move pivot rows to R and zero them
 // ------------------------------------------------------------------------------------------------
-__global__ void gj_swap_extract_kernel(cplx* A, long long sA, int b, int k0, int w, const int* ipiv,
-                                       cplx* R /*[batch][w][b]*/, const int* skip) {
+// pivots p0 .. p0+np-1; columns [clo, chi) except [xlo, xhi)
+__global__ void gj_swap_extract_kernel(cplx* A, long long sA, int b, int p0, int np, int clo, int chi, int xlo,
+                                       int xhi, const int* ipiv, cplx* R /*[batch][np][b]*/, const int* skip) {
     const int e = blockIdx.y;
     if (skip && skip[e]) return;
-    int c = blockIdx.x * blockDim.x + threadIdx.x;
-    if (c >= b || (c >= k0 && c < k0 + w)) return;
+    int c = clo + blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= chi || (c >= xlo && c < xhi)) return;
     cplx* g = A + (size_t)e * sA;
-    const int* pv = ipiv + (size_t)e * b + k0;
-    for (int j = 0; j < w; j++) {
+    const int* pv = ipiv + (size_t)e * b + p0;
+    for (int j = 0; j < np; j++) {
         int p = pv[j];
-        if (p != k0 + j) {
-            cplx t = g[(size_t)(k0 + j) * b + c];
-            g[(size_t)(k0 + j) * b + c] = g[(size_t)p * b + c];
+        if (p != p0 + j) {
+            cplx t = g[(size_t)(p0 + j) * b + c];
+            g[(size_t)(p0 + j) * b + c] = g[(size_t)p * b + c];
             g[(size_t)p * b + c] = t;
         }
     }
-    cplx* r = R + (size_t)e * w * b;
-    for (int j = 0; j < w; j++) {
-        r[(size_t)j * b + c] = g[(size_t)(k0 + j) * b + c];
-        g[(size_t)(k0 + j) * b + c] = cmake(0.0, 0.0);
+    cplx* r = R + (size_t)e * np * b;
+    for (int j = 0; j < np; j++) {
+        r[(size_t)j * b + c] = g[(size_t)(p0 + j) * b + c];
+        g[(size_t)(p0 + j) * b + c] = cmake(0.0, 0.0);
     }
 }
 
@@ -481,7 +654,10 @@ __global__ void gj_permidx_kernel(int b, const int* ipiv, int* idxbuf, const int
     for (int c = threadIdx.x; c < b; c += blockDim.x) idxbuf[(size_t)e * b + c] = sidx[c];
 }
 
+constexpr int OUTER_NB = 128;      // outer block of the two-level blocked Gauss-Jordan
+
 struct InvWs {
+    cplx* Rout;   // [batch][OUTER_NB][b]  pivot rows of an outer block
     cplx* R;      // [batch][PW][b]
     cplx* Pbuf;   // [batch][b][PW]
     cplx* Dinv;   // [batch][PW*PW]
@@ -492,6 +668,7 @@ struct InvWs {
 InvWs carve(void* ws, int b, int batch) {
     InvWs o;
     unsigned char* p = (unsigned char*)ws;
+    o.Rout = (cplx*)p; p += align_up((size_t)batch * OUTER_NB * b * sizeof(cplx), 256);
     o.R = (cplx*)p;    p += align_up((size_t)batch * PW * b * sizeof(cplx), 256);
     o.Pbuf = (cplx*)p; p += align_up((size_t)batch * PW * b * sizeof(cplx), 256);
     o.Dinv = (cplx*)p; p += align_up((size_t)batch * PW * PW * sizeof(cplx), 256);
@@ -505,7 +682,8 @@ InvWs carve(void* ws, int b, int batch) {
 
 size_t zinv_workspace_bytes(int b, int batch) {
     if (b <= SMALL_MAX) return 256;
-    return 2 * align_up((size_t)batch * PW * b * sizeof(cplx), 256) +
+    return align_up((size_t)batch * OUTER_NB * b * sizeof(cplx), 256) +
+           2 * align_up((size_t)batch * PW * b * sizeof(cplx), 256) +
            2 * align_up((size_t)batch * PW * PW * sizeof(cplx), 256) +
            2 * align_up((size_t)batch * b * sizeof(int), 256);
 }
@@ -537,12 +715,66 @@ int zinv_launch(negf_ctx* ctx, int b, cplx* A, long long sA, int batch, void* ws
         NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_panel_cluster_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                                   (int)(PANEL_SMEM_ROWS_BYTES + fixed)));
         NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_colperm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+        NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_panel_reg_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(RegPanelSmem)));
+        NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_panel_reg_kernel<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(RegPanelSmem)));
         attr_done = true;
     }
     const cplx one = cmake(1.0, 0.0), mone = cmake(-1.0, 0.0), zero = cmake(0.0, 0.0);
-    for (int k0 = 0; k0 < b; k0 += w) {
-        const int wk = min(w, b - k0);
+    // Two-level blocking.  Inside an outer block K = [K0, K0 + nbk) the width-w panels are
+    // eliminated with their row swaps and rank-w updates restricted to the columns of K, so that
+    // those columns end up holding Q = E[:, K] of the accumulated transform E (identity outside the
+    // columns K); every other column then gets all nbk swaps at once and ONE rank-nbk update
+    // M[:, ~K] = (M with rows K zeroed)[:, ~K] + Q R, R = the pivot rows: a GEMM with k = 128.
+    for (int K0 = 0; K0 < b; K0 += OUTER_NB) {
+      const int nbk = min(OUTER_NB, b - K0), K1 = K0 + nbk;
+      for (int k0 = K0; k0 < K1; k0 += w) {
+        const int wk = min(w, K1 - k0);
         const int rows = b - k0;
+        const bool reg_panel = rows <= 2048;
+        GemmArgs g;
+        g.opA = 0; g.opB = 0; g.batch = batch; g.skip = skip;
+        g.batch2 = 1; g.sA2 = g.sB2 = g.sD2 = g.sC2 = 0; g.alpha_vec = nullptr;
+        cudaLaunchConfig_t cfg = {};
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.attrs = at; cfg.numAttrs = 1; cfg.stream = ctx->stream;
+        if (reg_panel) {
+            // one row per thread in registers; finishes P' (diagonal block and below) in place
+            const int NT = rows <= 1024 ? 128 : 256;
+            const int C = (rows + NT - 1) / NT;
+            PanelArgs pa{A, sA, b, k0, wk, 0, W.ipiv, W.Dinv, W.Linv, info, info_code, skip};
+            cfg.gridDim = dim3(C, batch); cfg.blockDim = dim3(NT); cfg.dynamicSmemBytes = sizeof(RegPanelSmem);
+            at[0].val.clusterDim.x = C;
+            if (NT == 128) NEGF_CUDA_CHECK(ctx, cudaLaunchKernelEx(&cfg, gj_panel_reg_kernel<128>, pa));
+            else           NEGF_CUDA_CHECK(ctx, cudaLaunchKernelEx(&cfg, gj_panel_reg_kernel<256>, pa));
+            ctx->launches++;
+            if (nbk > wk) {
+                gj_swap_extract_kernel<<<dim3((nbk + 127) / 128, batch), 128, 0, ctx->stream>>>(
+                    A, sA, b, k0, wk, K0, K1, k0, k0 + wk, W.ipiv, W.R, skip);
+                NEGF_LAUNCH_CHECK(ctx);
+            }
+            // rows above the panel: P' = -T Dinv, in place (each CTA reads exactly the rows it writes)
+            if (k0 > 0) {
+                g.alpha = mone; g.beta = zero; g.D = nullptr; g.sD = 0;
+                g.m = k0; g.n = wk; g.k = wk; g.A = A + k0; g.lda = b; g.sA = sA;
+                g.B = W.Dinv; g.ldb = wk; g.sB = PW * PW; g.C = A + k0; g.ldc = b; g.sC = sA;
+                NEGF_TRY(zgemm_launch(ctx, g));
+            }
+            // M[:, other columns of K] += P' R, P' read from the panel's own columns
+            g.alpha = one; g.beta = one; g.m = b; g.k = wk; g.A = A + k0; g.lda = b; g.sA = sA;
+            g.ldb = b; g.sB = (long long)wk * b; g.ldc = b; g.sC = sA; g.sD = sA;
+            if (k0 > K0) {
+                g.n = k0 - K0; g.B = W.R + K0; g.C = A + K0; g.D = A + K0;
+                NEGF_TRY(zgemm_launch(ctx, g));
+            }
+            if (k0 + wk < K1) {
+                g.n = K1 - k0 - wk; g.B = W.R + k0 + wk; g.C = A + k0 + wk; g.D = A + k0 + wk;
+                NEGF_TRY(zgemm_launch(ctx, g));
+            }
+            continue;
+        }
+        // cluster size: smallest power of two whose slabs fit, at least wk rows per slab
         // cluster size: smallest power of two whose slabs fit, at least wk rows per slab
         int C = 1;
         while (C < CMAX && (size_t)((rows + C - 1) / C) * wk * sizeof(cplx) > (size_t)PANEL_SMEM_ROWS_BYTES) C <<= 1;
@@ -550,24 +782,20 @@ int zinv_launch(negf_ctx* ctx, int b, cplx* A, long long sA, int batch, void* ws
         while (C < CMAX && (rows + C - 1) / C > 512) C <<= 1;
         int slab = max(wk, (rows + C - 1) / C);
         PanelArgs pa{A, sA, b, k0, wk, slab, W.ipiv, W.Dinv, W.Linv, info, info_code, skip};
-        cudaLaunchConfig_t cfg = {};
         cfg.gridDim = dim3(C, batch);
         cfg.blockDim = dim3(PANEL_NT);
         cfg.dynamicSmemBytes = (size_t)slab * wk * sizeof(cplx) + fixed;
-        cfg.stream = ctx->stream;
-        cudaLaunchAttribute at[1];
-        at[0].id = cudaLaunchAttributeClusterDimension;
-        at[0].val.clusterDim.x = C; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
-        cfg.attrs = at; cfg.numAttrs = 1;
+        at[0].val.clusterDim.x = C;
         NEGF_CUDA_CHECK(ctx, cudaLaunchKernelEx(&cfg, gj_panel_cluster_kernel, pa));
         ctx->launches++;
-        // row swaps on the other columns + pivot rows -> R, zeroed in A
-        gj_swap_extract_kernel<<<dim3((b + 127) / 128, batch), 128, 0, ctx->stream>>>(A, sA, b, k0, wk, W.ipiv, W.R, skip);
-        NEGF_LAUNCH_CHECK(ctx);
+        // row swaps on the other columns of K + pivot rows -> R, zeroed in A
+        if (nbk > wk) {
+            gj_swap_extract_kernel<<<dim3((nbk + 127) / 128, batch), 128, 0, ctx->stream>>>(
+                A, sA, b, k0, wk, K0, K1, k0, k0 + wk, W.ipiv, W.R, skip);
+            NEGF_LAUNCH_CHECK(ctx);
+        }
         // P' = [-T Dinv ; Dinv ; -L21 Linv]
-        GemmArgs g;
-        g.opA = 0; g.opB = 0; g.alpha = mone; g.beta = zero; g.D = nullptr; g.sD = 0; g.batch = batch; g.skip = skip;
-        g.batch2 = 1; g.sA2 = g.sB2 = g.sD2 = g.sC2 = 0; g.alpha_vec = nullptr;
+        g.alpha = mone; g.beta = zero; g.D = nullptr; g.sD = 0;
         g.n = wk; g.k = wk; g.ldb = wk; g.sB = PW * PW; g.ldc = wk; g.sC = (long long)b * wk; g.lda = b; g.sA = sA;
         if (k0 > 0) {
             g.m = k0; g.A = A + k0; g.B = W.Dinv; g.C = W.Pbuf;
@@ -579,19 +807,39 @@ int zinv_launch(negf_ctx* ctx, int b, cplx* A, long long sA, int batch, void* ws
         }
         gj_pbuf_diag_kernel<<<dim3((wk * wk + 255) / 256, batch), 256, 0, ctx->stream>>>(W.Pbuf, b, k0, wk, W.Dinv, skip);
         NEGF_LAUNCH_CHECK(ctx);
-        // M[:, other columns] += P' R
+        // M[:, other columns of K] += P' R
         g.alpha = one; g.beta = one; g.m = b; g.k = wk; g.A = W.Pbuf; g.lda = wk; g.sA = (long long)b * wk;
         g.ldb = b; g.sB = (long long)wk * b; g.ldc = b; g.sC = sA; g.sD = sA;
-        if (k0 > 0) {
-            g.n = k0; g.B = W.R; g.C = A; g.D = A;
+        if (k0 > K0) {
+            g.n = k0 - K0; g.B = W.R + K0; g.C = A + K0; g.D = A + K0;
             NEGF_TRY(zgemm_launch(ctx, g));
         }
-        if (k0 + wk < b) {
-            g.n = b - k0 - wk; g.B = W.R + k0 + wk; g.C = A + k0 + wk; g.D = A + k0 + wk;
+        if (k0 + wk < K1) {
+            g.n = K1 - k0 - wk; g.B = W.R + k0 + wk; g.C = A + k0 + wk; g.D = A + k0 + wk;
             NEGF_TRY(zgemm_launch(ctx, g));
         }
         gj_panel_store_kernel<<<dim3((b * wk + 255) / 256, batch), 256, 0, ctx->stream>>>(A, sA, b, k0, wk, W.Pbuf, W.Dinv, skip);
         NEGF_LAUNCH_CHECK(ctx);
+      }
+      if (nbk == b) break;       // a single outer block: nothing outside it
+      // all nbk swaps of this outer block on the columns outside K; pivot rows -> Rout, zeroed in A
+      gj_swap_extract_kernel<<<dim3((b + 127) / 128, batch), 128, 0, ctx->stream>>>(
+          A, sA, b, K0, nbk, 0, b, K0, K1, W.ipiv, W.Rout, skip);
+      NEGF_LAUNCH_CHECK(ctx);
+      // M[:, ~K] += Q R with Q = M[:, K] in place
+      GemmArgs g;
+      g.opA = 0; g.opB = 0; g.alpha = one; g.beta = one; g.batch = batch; g.skip = skip;
+      g.batch2 = 1; g.sA2 = g.sB2 = g.sD2 = g.sC2 = 0; g.alpha_vec = nullptr;
+      g.m = b; g.k = nbk; g.A = A + K0; g.lda = b; g.sA = sA;
+      g.ldb = b; g.sB = (long long)nbk * b; g.ldc = b; g.sC = sA; g.sD = sA;
+      if (K0 > 0) {
+          g.n = K0; g.B = W.Rout; g.C = A; g.D = A;
+          NEGF_TRY(zgemm_launch(ctx, g));
+      }
+      if (K1 < b) {
+          g.n = b - K1; g.B = W.Rout + K1; g.C = A + K1; g.D = A + K1;
+          NEGF_TRY(zgemm_launch(ctx, g));
+      }
     }
     gj_permidx_kernel<<<batch, 256, (size_t)b * sizeof(int), ctx->stream>>>(b, W.ipiv, W.idx, skip);
     NEGF_LAUNCH_CHECK(ctx);
