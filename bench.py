@@ -35,11 +35,15 @@ UNIT = "energy points/s"
 # nominal work: units U = 8 b^3 real flops
 # ---------------------------------------------------------------------------------------------
 def unit_counts(n, sigma_kind, want_greater, iters_total, n_energy):
-    """Returns (gemm_units, inverse_units) for ALL energies of the batch.
+    """Returns (gemm_units, inverse_units) for ALL energies of the batch: the SURVEY 8(d) nominal
+    count, lowered where the implementation executes fewer products (ballistic Sigma^<>: the
+    hoisted S5 needs 3(n-1)+4 products instead of 4n-2).  Never more than nominal.
     iters_total = sum over energies and both leads of the decimation doublings done."""
     gr = 7 * n - 6 + (n - 1)                       # S3 + S4 + corner column
     gr_inv = n
     gx = (11 * n - 9) if sigma_kind == "bt" else (9 * n - 7)
+    if sigma_kind == "none":
+        gx -= (4 * n - 2) - min(4 * n - 2, 3 * (n - 1) + 4)
     n_x = 2 if want_greater else 1
     obs = 2                                        # Gamma_L G Gamma_R for T(E)
     per_e_gemm = (gr - gr_inv) + n_x * gx + obs
@@ -162,9 +166,7 @@ def run_gpu(args, rank, local_rank, world):
         dist.init_process_group("nccl", device_id=torch.device(dev))
 
     wl = workloads.make_workload(args.config)
-    if world > 1:   # energy sharding of a grid `world` times as dense (weak scaling)
-        de = (wl.energies[1] - wl.energies[0]) if wl.n_energy > 1 else 0.0
-        wl.energies = wl.energies + rank * de / world
+    wl = workloads.shard_energies(wl, rank, world)   # grid `world` times as dense, every world-th point
     ne_batch = args.energy_batch or default_energy_batch(wl, torch.cuda.mem_get_info(local_rank)[0])
     ne_batch = min(ne_batch, wl.n_energy)
     ne_batch = -(-wl.n_energy // -(-wl.n_energy // ne_batch))     # equal batches: ceil(N_E / ceil(N_E / fit))

@@ -443,75 +443,84 @@ __global__ void __launch_bounds__(NT) gj_panel_reg_kernel(PanelArgs a) {
     for (int c = 0; c < PW; c++) P[c] = (valid && c < w) ? g[(size_t)gr * b + c] : cmake(0.0, 0.0);
     constexpr int NONE = 0x7fffffff;
 
+    // The column loop is deliberately NOT unrolled (a fully unrolled body is ~13k instructions that
+    // each run once: ncu showed 47 % of the stall cycles in instruction fetch); the register row
+    // is addressed with compile-time indices and the current column is picked by predication.
+#pragma unroll 1
+    for (int j = 0; j < w; j++) {
+        const int par = j & 1;
+        cplx pj = cmake(0.0, 0.0);
 #pragma unroll
-    for (int j = 0; j < PW; j++) {
-        if (j < w) {
-            const int par = j & 1;
-            // CTA candidate: largest |re|+|im| among my rows with index >= j (smallest row on ties)
-            const bool has = valid && gr >= j;
-            const unsigned long long key = has ? (unsigned long long)__double_as_longlong(cabs1(P[j])) : 0ull;
-            const unsigned hi = __reduce_max_sync(0xffffffffu, has ? (unsigned)(key >> 32) : 0u);
-            const bool mh = has && (unsigned)(key >> 32) == hi;
-            const unsigned lo = __reduce_max_sync(0xffffffffu, mh ? (unsigned)key : 0u);
-            const bool ml = mh && (unsigned)key == lo;
-            const unsigned wrow = __reduce_min_sync(0xffffffffu, ml ? (unsigned)gr : (unsigned)NONE);
-            if (lane == 0) { S.red_key[warp] = ((unsigned long long)hi << 32) | lo; S.red_row[warp] = (int)wrow; }
-            __syncthreads();
-            unsigned long long bk = 0ull; int br = NONE;
+        for (int c = 0; c < PW; c++) if (c == j) pj = P[c];
+        // CTA candidate: largest |re|+|im| among my rows with index >= j (smallest row on ties)
+        const bool has = valid && gr >= j;
+        const unsigned long long key = has ? (unsigned long long)__double_as_longlong(cabs1(pj)) : 0ull;
+        const unsigned hi = __reduce_max_sync(0xffffffffu, has ? (unsigned)(key >> 32) : 0u);
+        const bool mh = has && (unsigned)(key >> 32) == hi;
+        const unsigned lo = __reduce_max_sync(0xffffffffu, mh ? (unsigned)key : 0u);
+        const bool ml = mh && (unsigned)key == lo;
+        const unsigned wrow = __reduce_min_sync(0xffffffffu, ml ? (unsigned)gr : (unsigned)NONE);
+        if (lane == 0) { S.red_key[warp] = ((unsigned long long)hi << 32) | lo; S.red_row[warp] = (int)wrow; }
+        __syncthreads();
+        unsigned long long bk = 0ull; int br = NONE;
 #pragma unroll
-            for (int q = 0; q < NT / 32; q++) {
-                const unsigned long long k2 = S.red_key[q]; const int r2 = S.red_row[q];
-                if (r2 != NONE && (br == NONE || k2 > bk || (k2 == bk && r2 < br))) { bk = k2; br = r2; }
-            }
-            if (gr == br) {
+        for (int q = 0; q < NT / 32; q++) {
+            const unsigned long long k2 = S.red_key[q]; const int r2 = S.red_row[q];
+            if (r2 != NONE && (br == NONE || k2 > bk || (k2 == bk && r2 < br))) { bk = k2; br = r2; }
+        }
+        if (gr == br) {
 #pragma unroll
-                for (int c = 0; c < PW; c++) S.rowstage[c] = P[c];
-            }
-            if (rank == 0 && tid == j) {
+            for (int c = 0; c < PW; c++) S.rowstage[c] = P[c];
+        }
+        if (rank == 0 && tid == j) {
 #pragma unroll
-                for (int c = 0; c < PW; c++) S.drowstage[c] = P[c];
-            }
-            __syncthreads();
-            if (warp == 0) {       // push (value, row, row content) to every CTA; CTA 0 also the diagonal row
-                const cplx myrow = S.rowstage[lane];
-                const cplx drow = S.drowstage[lane];
-                for (int q = 0; q < C; q++) {
-                    RegPanelSmem* R = cluster.map_shared_rank(&S, q);
-                    R->candrow[par][rank][lane] = myrow;
-                    if (rank == 0) R->diagrow[par][lane] = drow;
-                    if (lane == 0) { R->cand_key[par][rank] = bk; R->cand_row[par][rank] = br; }
-                }
-            }
-            cluster.sync();
-            // everybody picks the same winner
-            int wq = 0, prow = NONE; unsigned long long wk = 0ull;
+            for (int c = 0; c < PW; c++) S.drowstage[c] = P[c];
+        }
+        __syncthreads();
+        if (warp == 0) {       // push (value, row, row content) to every CTA; CTA 0 also the diagonal row
+            const cplx myrow = S.rowstage[lane];
+            const cplx drow = S.drowstage[lane];
             for (int q = 0; q < C; q++) {
-                const unsigned long long k2 = S.cand_key[par][q]; const int r2 = S.cand_row[par][q];
-                if (r2 != NONE && (prow == NONE || k2 > wk || (k2 == wk && r2 < prow))) { wk = k2; prow = r2; wq = q; }
+                RegPanelSmem* R = cluster.map_shared_rank(&S, q);
+                R->candrow[par][rank][lane] = myrow;
+                if (rank == 0) R->diagrow[par][lane] = drow;
+                if (lane == 0) { R->cand_key[par][rank] = bk; R->cand_row[par][rank] = br; }
             }
-            const bool sing = (prow == NONE) || wk == 0ull;
-            if (prow == NONE) prow = j;
-            if (rank == 0 && tid == 0) {
-                a.ipiv[(size_t)e * b + k0 + j] = k0 + prow;
-                if (sing && a.info && a.info[e] == 0) a.info[e] = a.code > 0 ? a.code : (k0 + j + 1);
-            }
-            const cplx* pr = S.candrow[par][wq];
-            // exchange rows j <-> prow
-            if (valid && gr == prow && prow != j) {
+        }
+        cluster.sync();
+        // everybody picks the same winner
+        int wq = 0, prow = NONE; unsigned long long wk = 0ull;
+        for (int q = 0; q < C; q++) {
+            const unsigned long long k2 = S.cand_key[par][q]; const int r2 = S.cand_row[par][q];
+            if (r2 != NONE && (prow == NONE || k2 > wk || (k2 == wk && r2 < prow))) { wk = k2; prow = r2; wq = q; }
+        }
+        const bool sing = (prow == NONE) || wk == 0ull;
+        if (prow == NONE) prow = j;
+        if (rank == 0 && tid == 0) {
+            a.ipiv[(size_t)e * b + k0 + j] = k0 + prow;
+            if (sing && a.info && a.info[e] == 0) a.info[e] = a.code > 0 ? a.code : (k0 + j + 1);
+        }
+        const cplx* pr = S.candrow[par][wq];
+        // exchange rows j <-> prow
+        if (valid && gr == prow && prow != j) {
 #pragma unroll
-                for (int c = 0; c < PW; c++) P[c] = S.diagrow[par][c];
-            }
-            if (rank == 0 && tid == j && prow != j) {
+            for (int c = 0; c < PW; c++) P[c] = S.diagrow[par][c];
+        }
+        if (rank == 0 && tid == j && prow != j) {
 #pragma unroll
-                for (int c = 0; c < PW; c++) P[c] = pr[c];
-            }
-            // eliminate below
-            if (valid && gr > j) {
-                const cplx rinv = sing ? cmake(0.0, 0.0) : crecip(pr[j]);
-                const cplx l = cmul(P[j], rinv);
-                P[j] = l;
+            for (int c = 0; c < PW; c++) P[c] = pr[c];
+        }
+        // eliminate below
+        if (valid && gr > j) {
+            cplx mine = cmake(0.0, 0.0);
 #pragma unroll
-                for (int c = j + 1; c < PW; c++) cfms(P[c], l, pr[c]);
+            for (int c = 0; c < PW; c++) if (c == j) mine = P[c];
+            const cplx rinv = sing ? cmake(0.0, 0.0) : crecip(pr[j]);
+            const cplx l = cmul(mine, rinv);
+#pragma unroll
+            for (int c = 0; c < PW; c++) {
+                if (c == j) P[c] = l;
+                else if (c > j) cfms(P[c], l, pr[c]);
             }
         }
     }
@@ -560,14 +569,12 @@ __global__ void __launch_bounds__(NT) gj_panel_reg_kernel(PanelArgs a) {
     // rows below the diagonal block: P' = -L21 L11^-1, written in place
     if (valid && gr >= w) {
         cplx* out = g + (size_t)gr * b;
+#pragma unroll 1
+        for (int c = 0; c < w; c++) {
+            cplx acc = cmake(0.0, 0.0);
 #pragma unroll
-        for (int c = 0; c < PW; c++) {
-            if (c < w) {
-                cplx acc = cmake(0.0, 0.0);
-#pragma unroll
-                for (int k = c; k < PW; k++) cfms(acc, P[k], S.Li[k * PW + c]);    // Li[k][c] = 0 for k >= w
-                out[c] = acc;
-            }
+            for (int k = 0; k < PW; k++) cfms(acc, P[k], S.Li[k * PW + c]);    // Li[k][c] = 0 for k < c and k >= w
+            out[c] = acc;
         }
     }
     cluster.sync();   // nobody exits while remote shared memory may still be targeted

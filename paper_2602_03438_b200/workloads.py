@@ -215,3 +215,26 @@ def chain_lead(b: int, seed: int = 7):
     H_d = (q * eps) @ q.conj().T
     H_u = (q * (-t)) @ q.conj().T
     return H_d, H_u, q, eps, t
+
+
+def shard_energies(wl: Workload, rank: int, world: int) -> Workload:
+    """Energy sharding for multi-GPU runs ("Each E is independent of the other"): the
+    job's grid is `world` times as dense as the config's and rank r takes every world-th point
+    starting at r, so that every rank keeps N_E energies of the same range (weak scaling) and the
+    union over ranks is one uniform grid.  No data-path collective is needed; only the density
+    would be summed over ranks by a caller that wants the total."""
+    import copy
+    if world <= 1:
+        return wl
+    ne = wl.n_energy
+    if ne == 1:
+        lo, hi = float(wl.energies[0]), float(wl.energies[0]) + 1e-3 * world
+    else:
+        lo, hi = float(wl.energies[0]), float(wl.energies[-1])
+    dense = np.linspace(lo, hi, ne * world)
+    out = copy.copy(wl)
+    out.energies = np.ascontiguousarray(dense[rank::world])
+    w_dense = trapezoid_weights(dense)
+    out.weights = np.ascontiguousarray(w_dense[rank::world])
+    out.name = f"{wl.name}[rank {rank}/{world}]"
+    return out

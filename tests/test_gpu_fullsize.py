@@ -1,0 +1,133 @@
+"""Parity at BASELINE.json's full sizes, in the launch configuration bench.py times:
+configs[1] complete (64 energies, n = 32, b = 64) on sampled energies against the oracle plus the
+selected-block residual of Eq. 1 (SURVEY 8(c) pin P2) on EVERY energy; full block sizes of
+configs[2-4] (b = 256, 1024, 2048) at reduced n / N_E against the oracle where it finishes in seconds,
+else through the residual identities P2 / P3 that hold at any size."""
+import numpy as np
+import pytest
+
+from oracle import assemble, pipeline
+from paper_2602_03438_b200 import workloads as W
+from tests.helpers import rel_fro
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-10
+
+
+@pytest.fixture(scope="module")
+def runner_mod(negf_lib):
+    from paper_2602_03438_b200 import runner
+    return runner
+
+
+def _gpu_boundary(dp, k):
+    side = lambda t: {"sigma_r": dp.host(f"sigma_r_{t}")[k], "gamma": dp.host(f"gamma_{t}")[k],
+                      "sigma_l": dp.host(f"sigma_l_{t}")[k], "sigma_g": dp.host(f"sigma_g_{t}")[k]}
+    return side("L"), side("R")
+
+
+def _a_blocks(wl, dp, k, sig):
+    z = complex(float(wl.energies[k]), wl.eta)
+    sr = pipeline._slice_sigma(sig["r"], k) if sig["r"] is not None else None
+    return assemble.a_blocks(z, wl.H_diag, wl.H_upper, wl.S_diag, wl.S_upper, sr,
+                             dp.host("sigma_r_L")[k], dp.host("sigma_r_R")[k])
+
+
+def _residual_eq1(A, GRd, GRu, GRl):
+    """max_i || sum_j A_ij G_ji - I ||_F / sqrt(b) over the block rows (P2)."""
+    Ad, Au, Al = A
+    n, b = Ad.shape[0], Ad.shape[1]
+    worst = 0.0
+    for i in range(n):
+        r = Ad[i] @ GRd[i] - np.eye(b)
+        if i > 0:
+            r += Al[i - 1] @ GRu[i - 1]
+        if i < n - 1:
+            r += Au[i] @ GRl[i]
+        worst = max(worst, np.linalg.norm(r) / np.sqrt(b))
+    return worst
+
+
+def _residual_eq2(A, B, GRd, GRu, GRl, GXd, GXu):
+    """(A G^x)_ii = (Sigma^x G^A)_ii = sum_j B_ij (G^R_ij)^H over the BT pattern (P3, from Eq. 2 and
+    A G^R = I), with G^x_{i+1,i} = -(G^x_{i,i+1})^H and B_{i,i-1} = -B_{i-1,i}^H; relative to the
+    size of the terms."""
+    Ad, Au, Al = A
+    Bd, Bu = B
+    n = Ad.shape[0]
+    H = lambda x: np.conj(x.T)
+    worst = 0.0
+    for i in range(n):
+        lhs = Ad[i] @ GXd[i]
+        rhs = Bd[i] @ H(GRd[i])
+        scale = np.linalg.norm(Ad[i]) * np.linalg.norm(GXd[i])
+        if i > 0:
+            lhs = lhs + Al[i - 1] @ GXu[i - 1]
+            rhs = rhs - H(Bu[i - 1]) @ H(GRl[i - 1])
+        if i < n - 1:
+            lhs = lhs - Au[i] @ H(GXu[i])
+            rhs = rhs + Bu[i] @ H(GRu[i])
+        worst = max(worst, np.linalg.norm(lhs - rhs) / scale)
+    return worst
+
+
+def test_config1_full(runner_mod):
+    wl = W.make_workload(1)
+    sig = wl.sigma_s()
+    dp = runner_mod.DevicePath(wl, sigma=sig)
+    dp.run()
+    assert int(dp.out["info_r"].abs().sum()) == 0 and int(dp.out["status_L"].abs().sum()) == 0
+    GRd, GRu, GRl = dp.host("GR_diag"), dp.host("GR_upper"), dp.host("GR_lower")
+    worst = max(_residual_eq1(_a_blocks(wl, dp, k, sig), GRd[k], GRu[k], GRl[k]) for k in range(wl.n_energy))
+    print(f"config1 full: worst Eq.1 selected-block residual over 64 energies {worst:.2e}")
+    assert worst < 1e-9
+    for k in (0, 31, 63):
+        s1 = {t: (None if sig[t] is None else {kk: (vv[k:k + 1] if kk != "kind" else vv) for kk, vv in sig[t].items()})
+              for t in "rlg"}
+        o = pipeline.solve_energy(wl, k, sigma=s1, obc_in=_gpu_boundary(dp, k), want_greater=False)
+        for name, grp, key in (("GR_diag", "ret", "GR_diag"), ("GR_upper", "ret", "GR_upper"),
+                               ("GR_lower", "ret", "GR_lower"), ("GL_diag", "les", "GX_diag"),
+                               ("GL_upper", "les", "GX_upper")):
+            assert rel_fro(dp.host(name)[k], o[grp][key]) < TOL, (k, name)
+        assert abs(dp.host("transmission")[k] - o["obs"]["transmission"]) <= 1e-9 * abs(o["obs"]["transmission"]) + 1e-13
+
+
+@pytest.mark.parametrize("cfg,kw,vs_oracle", [
+    (2, dict(n_blocks=4, n_energy=2), True),          # b = 256, non-orthogonal S
+    (3, dict(n_blocks=3, n_energy=1), True),          # b = 1024, dense BT Sigma^{R,<,>}
+    (4, dict(n_blocks=3, n_energy=1), False),         # b = 2048: residual identities only
+])
+def test_full_block_sizes(runner_mod, cfg, kw, vs_oracle):
+    wl = W.make_workload(cfg, **kw)
+    sig = wl.sigma_s()
+    dp = runner_mod.DevicePath(wl, want_greater=True, sigma=sig)
+    dp.run()
+    assert int(dp.out["info_r"].abs().sum()) == 0
+    assert int(dp.out["status_L"].abs().sum()) == 0 and int(dp.out["status_R"].abs().sum()) == 0
+    GRd, GRu, GRl = dp.host("GR_diag"), dp.host("GR_upper"), dp.host("GR_lower")
+    for k in range(wl.n_energy):
+        A = _a_blocks(wl, dp, k, sig)
+        res = _residual_eq1(A, GRd[k], GRu[k], GRl[k])
+        print(f"cfg{cfg} b={wl.block_size} energy {k}: Eq.1 residual {res:.2e}")
+        assert res < 1e-9
+        # anti-Hermiticity of the diagonal G^<> blocks (P4)
+        for nm in ("GL_diag", "GG_diag"):
+            g = dp.host(nm)[k]
+            ah = max(np.linalg.norm(g[i] + np.conj(g[i].T)) / np.linalg.norm(g[i]) for i in range(wl.n_blocks))
+            assert ah < 1e-9, (nm, ah)
+        for tag, dn, un, key in (("l", "GL_diag", "GL_upper", "sigma_l"), ("g", "GG_diag", "GG_upper", "sigma_g")):
+            sx = pipeline._slice_sigma(sig[tag], k) if sig[tag] is not None else None
+            B = assemble.b_blocks(wl.n_blocks, wl.block_size, sx, dp.host(f"{key}_L")[k], dp.host(f"{key}_R")[k])
+            r2 = _residual_eq2(A, B, GRd[k], GRu[k], GRl[k], dp.host(dn)[k], dp.host(un)[k])
+            print(f"cfg{cfg} b={wl.block_size} energy {k}: Eq.2 residual ({tag}) {r2:.2e}")
+            assert r2 < 1e-9
+        if vs_oracle:
+            s1 = {t: (None if sig[t] is None else {kk: (vv[k:k + 1] if kk != "kind" else vv) for kk, vv in sig[t].items()})
+                  for t in "rlg"}
+            o = pipeline.solve_energy(wl, k, sigma=s1, obc_in=_gpu_boundary(dp, k), want_greater=True)
+            for name, grp, key in (("GR_diag", "ret", "GR_diag"), ("GR_upper", "ret", "GR_upper"),
+                                   ("GR_lower", "ret", "GR_lower"), ("GL_diag", "les", "GX_diag"),
+                                   ("GL_upper", "les", "GX_upper"), ("GG_diag", "gtr", "GX_diag"),
+                                   ("GG_upper", "gtr", "GX_upper")):
+                err = rel_fro(dp.host(name)[k], o[grp][key])
+                assert err < TOL, (cfg, k, name, err)
