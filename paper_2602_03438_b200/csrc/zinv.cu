@@ -48,7 +48,6 @@ constexpr int PANEL_SMEM_ROWS_BYTES = 176 * 1024;   // + 9 KB exchange buffers +
 //   * the rank-1 update runs out of registers at the DFMA rate (= the DMMA rate on sm_100).
 // Rows/columns >= b are padded with the identity and never reached.
 // ------------------------------------------------------------------------------------------------
-constexpr int GJ_NW = 8;
 
 
 __device__ __forceinline__ cplx crecip_fast(cplx a) {      // pivots are O(1): no overflow guard needed
@@ -64,7 +63,7 @@ struct GjShared {            // pointers into the kernel's shared memory
 
 // pivot search + publication of column kn, held in slot C of the calling (owner) warp
 template <int RB, int CB, int C>
-__device__ __forceinline__ void gj_owner(const cplx (&m)[RB][CB], const GjShared& sh, int kn, int b, int lane) {
+__device__ __forceinline__ void gj_owner(const cplx (&m)[RB][CB], unsigned used, const GjShared& sh, int kn, int b, int lane) {
     constexpr int NR = RB * 32;
     const int parn = kn & 1;
     unsigned long long key = 0ull;
@@ -73,7 +72,7 @@ __device__ __forceinline__ void gj_owner(const cplx (&m)[RB][CB], const GjShared
     for (int r = 0; r < RB; r++) {
         const int i = lane + 32 * r;
         sh.colbuf[parn * NR + i] = m[r][C];
-        if (i >= kn && i < b) {
+        if (!((used >> r) & 1u) && i < b) {
             const unsigned long long kq = (unsigned long long)__double_as_longlong(cabs1(m[r][C]));
             if (bi == 0x7fffffff || kq > key) { key = kq; bi = i; }
         }
@@ -114,9 +113,9 @@ __device__ __forceinline__ void gj_update_rest(cplx (&m)[RB][CB], const cplx (&m
     }
 }
 
-// all columns k = CK*8 + wk, wk < 8, then recurse to CK + 1
-template <int RB, int CB, int CK>
-__device__ __forceinline__ void gj_columns(cplx (&m)[RB][CB], const GjShared& sh, int b, int warp, int lane) {
+// all columns k = CK*NW + wk, wk < NW, then recurse to CK + 1
+template <int RB, int CB, int GJ_NW, int CK>
+__device__ __forceinline__ void gj_columns(cplx (&m)[RB][CB], unsigned& used, const GjShared& sh, int b, int warp, int lane) {
     if constexpr (CK < CB) {
         constexpr int NR = RB * 32;
         constexpr int CN = (CK + 1 < CB) ? CK + 1 : CK;
@@ -128,36 +127,23 @@ __device__ __forceinline__ void gj_columns(cplx (&m)[RB][CB], const GjShared& sh
             __syncthreads();
             const int p = sh.s_p[par];
             const cplx d = sh.s_d[par];
-            cplx* wr = sh.wrow + par * 2 * CB;
-            // the two rows that trade places, through this warp's shared-memory line
-#pragma unroll
-            for (int r = 0; r < RB; r++) {
-                const int i = lane + 32 * r;
-                if (i == p) {
-#pragma unroll
-                    for (int c = 0; c < CB; c++) wr[c] = m[r][c];
-                }
-                if (i == k && p != k) {
-#pragma unroll
-                    for (int c = 0; c < CB; c++) wr[CB + c] = m[r][c];
-                }
-            }
-            __syncwarp();
+            cplx* wr = sh.wrow + par * CB;
+            // IMPLICIT pivoting: rows never move.  The pivot row (physical row p) is broadcast inside
+            // each warp through its shared-memory line, marked as used, and turned into the scaled
+            // pivot row by the common update formula (m = 0, mult = -1).
             cplx mult[RB];
 #pragma unroll
             for (int r = 0; r < RB; r++) {
                 const int i = lane + 32 * r;
-                mult[r] = sh.colbuf[par * NR + ((i == p) ? k : i)];   // row p inherits old row k's multiplier
-                if (i == p && p != k) {
+                mult[r] = sh.colbuf[par * NR + i];
+                if (i == p) {
 #pragma unroll
-                    for (int c = 0; c < CB; c++) m[r][c] = wr[CB + c];
-                }
-                if (i == k) {
+                    for (int c = 0; c < CB; c++) { wr[c] = m[r][c]; m[r][c] = cmake(0.0, 0.0); }
                     mult[r] = cmake(-1.0, 0.0);
-#pragma unroll
-                    for (int c = 0; c < CB; c++) m[r][c] = cmake(0.0, 0.0);
+                    used |= 1u << r;
                 }
             }
+            __syncwarp();
             cplx sr[CB];
 #pragma unroll
             for (int c = 0; c < CB; c++) sr[c] = cmul(wr[c], d);
@@ -171,28 +157,28 @@ __device__ __forceinline__ void gj_columns(cplx (&m)[RB][CB], const GjShared& sh
             if (k + 1 < b && warp == ((wk + 1) & (GJ_NW - 1))) {
                 if (wk < GJ_NW - 1) {
                     gj_update<RB, CB, CK>(m, mult, sr);
-                    gj_owner<RB, CB, CK>(m, sh, k + 1, b, lane);
+                    gj_owner<RB, CB, CK>(m, used, sh, k + 1, b, lane);
                     done = CK;
                 } else if (CK + 1 < CB) {
                     gj_update<RB, CB, CN>(m, mult, sr);
-                    gj_owner<RB, CB, CN>(m, sh, k + 1, b, lane);
+                    gj_owner<RB, CB, CN>(m, used, sh, k + 1, b, lane);
                     done = CN;
                 }
             }
             gj_update_rest<RB, CB, 0>(m, mult, sr, done);
         }
-        gj_columns<RB, CB, CK + 1>(m, sh, b, warp, lane);
+        gj_columns<RB, CB, GJ_NW, CK + 1>(m, used, sh, b, warp, lane);
     }
 }
 
-template <int RB, int CB>
+template <int RB, int CB, int GJ_NW>
 __global__ void __launch_bounds__(GJ_NW * 32) gj_reg_kernel(cplx* A, long long sA, int b, int* info, int code,
                                                             const int* skip) {
     constexpr int NR = RB * 32, NC = CB * GJ_NW;
     const int e = blockIdx.x;
     if (skip && skip[e]) return;
     __shared__ cplx colbuf[2 * NR];
-    __shared__ cplx wrow[GJ_NW][2 * 2 * CB];     // [warp][parity][pivot row | row k][slot]
+    __shared__ cplx wrow[GJ_NW][2 * CB];         // [warp][parity][slot]: the pivot row of the current column
     __shared__ cplx s_d[2];
     __shared__ int s_p[2];
     __shared__ int piv[NC];
@@ -211,26 +197,21 @@ __global__ void __launch_bounds__(GJ_NW * 32) gj_reg_kernel(cplx* A, long long s
     if (tid == 0) s_sing = 0;
     __syncthreads();
     GjShared sh{colbuf, wrow[warp], s_d, s_p, piv, &s_sing};
-    if (warp == 0) gj_owner<RB, CB, 0>(m, sh, 0, b, lane);
-    gj_columns<RB, CB, 0>(m, sh, b, warp, lane);
+    unsigned used = 0u;              // bit r: my row lane + 32 r has been a pivot row
+    if (warp == 0) gj_owner<RB, CB, 0>(m, used, sh, 0, b, lane);
+    gj_columns<RB, CB, GJ_NW, 0>(m, used, sh, b, warp, lane);
     __syncthreads();
-    // A^-1 = (P A)^-1 P: column j of the result is column src[j] of M, src = the recorded swaps
-    // applied in reverse order to the identity; every thread scatters its columns to src^-1.
-    if (tid == 0) {
-        for (int c = 0; c < b; c++) dest[c] = c;
-        for (int k = b - 1; k >= 0; k--) {
-            const int p = piv[k];
-            if (p != k) { int t = dest[k]; dest[k] = dest[p]; dest[p] = t; }
-        }
-        for (int c = 0; c < b; c++) piv[dest[c]] = c;     // piv now holds src^-1
-    }
+    // With piv[k] = physical pivot row of column k the register array holds B[i][k] = X[i][piv[k]],
+    // X = Pi A^-1, Pi[piv[k]][k] = 1, so A^-1[r][piv[k]] = B[piv[r]][k]: every thread scatters its
+    // elements to row pinv[i], column piv[j].
+    if (tid < b) dest[piv[tid]] = tid;         // dest = pinv
     __syncthreads();
 #pragma unroll
     for (int r = 0; r < RB; r++)
 #pragma unroll
         for (int c = 0; c < CB; c++) {
             const int i = lane + 32 * r, j = warp + GJ_NW * c;
-            if (i < b && j < b) g[(size_t)i * b + piv[j]] = m[r][c];
+            if (i < b && j < b) g[(size_t)dest[i] * b + piv[j]] = m[r][c];
         }
     if (tid == 0 && s_sing && info) info[e] = code > 0 ? code : s_sing;
 }
@@ -402,29 +383,52 @@ __global__ void __launch_bounds__(PANEL_NT, 1) gj_panel_cluster_kernel(PanelArgs
 }
 
 // ------------------------------------------------------------------------------------------------
-// step 1, register-resident variant (tall panels up to 8 x 256 rows): every thread owns ONE row of
-// the width-32 panel in registers, a cluster of C CTAs covers the rows >= k0.  Per column: one
-// redux-based candidate per CTA, one DSMEM exchange (candidate value, row index, row content and
-// the current diagonal row) and one cluster barrier; the elimination runs out of registers.  The
-// kernel also finishes the panel in place: rows below the diagonal block leave as -L21 L11^-1,
-// the diagonal block as (L11 U11)^-1, so the trailing GEMM reads P' straight from A's columns.
+// step 1, register-resident variant (tall panels up to 8 x 256 rows).  Lane = panel column, every
+// warp keeps R consecutive rows of the width-32 panel in registers (one complex per lane and row),
+// 16 warps per CTA, a cluster of C CTAs covers the rows >= k0.  Per column: each warp's lane j
+// scans its R rows, redux picks the CTA candidate, ONE DSMEM exchange (candidate key, row index,
+// row content, current diagonal row) and ONE cluster barrier; the elimination is a shuffle
+// broadcast of the multiplier plus one complex FMA per row, out of registers.  The kernel also
+// finishes the panel in place: rows below the diagonal block leave as -L21 L11^-1, the diagonal
+// block as (L11 U11)^-1, so the trailing GEMM reads P' straight from A's columns.
+// (A first version with one ROW per thread needed ~1850 instructions per column and warp - the
+// column index had to be picked by predication - and was instruction-latency bound; this layout
+// needs ~300, see profiles/r01b_inverse.md.)
 // ------------------------------------------------------------------------------------------------
+constexpr int PNL_WARPS = 16;
+constexpr int PNL_NONE = 0x7fffffff;
+
 struct RegPanelSmem {
     cplx candrow[2][CMAX][PW];
     cplx diagrow[2][PW];
-    cplx rowstage[PW];
+    cplx wrows[PNL_WARPS][PW];   // every warp's candidate row of the current column
     cplx drowstage[PW];
     cplx Dm[PW * PW];      // factored diagonal block L11 \ U11
     cplx Li[PW * PW];      // L11^-1 (every CTA gets a copy)
     cplx Ui[PW * PW];      // U11^-1 (CTA 0)
-    unsigned long long red_key[8];
-    int red_row[8];
+    unsigned long long red_key[PNL_WARPS];
+    int red_row[PNL_WARPS];
     unsigned long long cand_key[2][CMAX];
     int cand_row[2][CMAX];
+    cplx Lrow[1];          // [PNL_WARPS * R][PW] follows (dynamic)
 };
 
-template <int NT>
-__global__ void __launch_bounds__(NT) gj_panel_reg_kernel(PanelArgs a) {
+// argmax of (key, smallest row) over the lanes that hold a candidate; every lane gets the result
+__device__ __forceinline__ void warp_best(unsigned long long key, int row, unsigned long long& bk, int& br) {
+    const bool has = row != PNL_NONE;
+    const unsigned hi = __reduce_max_sync(0xffffffffu, has ? (unsigned)(key >> 32) : 0u);
+    const bool mh = has && (unsigned)(key >> 32) == hi;
+    const unsigned lo = __reduce_max_sync(0xffffffffu, mh ? (unsigned)key : 0u);
+    const bool ml = mh && (unsigned)key == lo;
+    br = (int)__reduce_min_sync(0xffffffffu, ml ? (unsigned)row : (unsigned)PNL_NONE);
+    bk = ((unsigned long long)hi << 32) | lo;
+}
+
+inline size_t reg_panel_smem_bytes(int R) { return sizeof(RegPanelSmem) + (size_t)PNL_WARPS * R * PW * sizeof(cplx); }
+
+template <int R>
+__global__ void __launch_bounds__(PNL_WARPS * 32) gj_panel_reg_kernel(PanelArgs a) {
+    constexpr int NT = PNL_WARPS * 32;
     cg::cluster_group cluster = cg::this_cluster();
     const int rank = (int)cluster.block_rank();
     const int C = (int)cluster.num_blocks();
@@ -435,92 +439,93 @@ __global__ void __launch_bounds__(NT) gj_panel_reg_kernel(PanelArgs a) {
     const int w = a.w, b = a.b, k0 = a.k0;
     const int rows_total = b - k0;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int gr = rank * NT + tid;               // candidate row index (global row k0 + gr)
-    const bool valid = gr < rows_total;
+    const int row0 = (rank * PNL_WARPS + warp) * R;               // first candidate row of this warp
     cplx* g = a.A + (size_t)e * a.sA + (size_t)k0 * b + k0;       // panel origin
-    cplx P[PW];
+    cplx P[R];
 #pragma unroll
-    for (int c = 0; c < PW; c++) P[c] = (valid && c < w) ? g[(size_t)gr * b + c] : cmake(0.0, 0.0);
-    constexpr int NONE = 0x7fffffff;
+    for (int r = 0; r < R; r++)
+        P[r] = (row0 + r < rows_total && lane < w) ? g[(size_t)(row0 + r) * b + lane] : cmake(0.0, 0.0);
 
-    // The column loop is deliberately NOT unrolled (a fully unrolled body is ~13k instructions that
-    // each run once: ncu showed 47 % of the stall cycles in instruction fetch); the register row
-    // is addressed with compile-time indices and the current column is picked by predication.
 #pragma unroll 1
     for (int j = 0; j < w; j++) {
         const int par = j & 1;
-        cplx pj = cmake(0.0, 0.0);
+        // lane j scans its column over this warp's rows with index >= j (all lanes run the same code)
+        unsigned long long key = 0ull; int row = PNL_NONE;
 #pragma unroll
-        for (int c = 0; c < PW; c++) if (c == j) pj = P[c];
-        // CTA candidate: largest |re|+|im| among my rows with index >= j (smallest row on ties)
-        const bool has = valid && gr >= j;
-        const unsigned long long key = has ? (unsigned long long)__double_as_longlong(cabs1(pj)) : 0ull;
-        const unsigned hi = __reduce_max_sync(0xffffffffu, has ? (unsigned)(key >> 32) : 0u);
-        const bool mh = has && (unsigned)(key >> 32) == hi;
-        const unsigned lo = __reduce_max_sync(0xffffffffu, mh ? (unsigned)key : 0u);
-        const bool ml = mh && (unsigned)key == lo;
-        const unsigned wrow = __reduce_min_sync(0xffffffffu, ml ? (unsigned)gr : (unsigned)NONE);
-        if (lane == 0) { S.red_key[warp] = ((unsigned long long)hi << 32) | lo; S.red_row[warp] = (int)wrow; }
-        __syncthreads();
-        unsigned long long bk = 0ull; int br = NONE;
-#pragma unroll
-        for (int q = 0; q < NT / 32; q++) {
-            const unsigned long long k2 = S.red_key[q]; const int r2 = S.red_row[q];
-            if (r2 != NONE && (br == NONE || k2 > bk || (k2 == bk && r2 < br))) { bk = k2; br = r2; }
-        }
-        if (gr == br) {
-#pragma unroll
-            for (int c = 0; c < PW; c++) S.rowstage[c] = P[c];
-        }
-        if (rank == 0 && tid == j) {
-#pragma unroll
-            for (int c = 0; c < PW; c++) S.drowstage[c] = P[c];
-        }
-        __syncthreads();
-        if (warp == 0) {       // push (value, row, row content) to every CTA; CTA 0 also the diagonal row
-            const cplx myrow = S.rowstage[lane];
-            const cplx drow = S.drowstage[lane];
-            for (int q = 0; q < C; q++) {
-                RegPanelSmem* R = cluster.map_shared_rank(&S, q);
-                R->candrow[par][rank][lane] = myrow;
-                if (rank == 0) R->diagrow[par][lane] = drow;
-                if (lane == 0) { R->cand_key[par][rank] = bk; R->cand_row[par][rank] = br; }
+        for (int r = 0; r < R; r++) {
+            const int gr = row0 + r;
+            if (gr >= j && gr < rows_total) {
+                const unsigned long long kq = (unsigned long long)__double_as_longlong(cabs1(P[r]));
+                if (row == PNL_NONE || kq > key) { key = kq; row = gr; }
             }
         }
-        cluster.sync();
-        // everybody picks the same winner
-        int wq = 0, prow = NONE; unsigned long long wk = 0ull;
+        key = __shfl_sync(0xffffffffu, key, j);
+        row = __shfl_sync(0xffffffffu, row, j);
+        {   // this warp's candidate row (and the current diagonal row, if it lives here) go to shared memory
+            cplx v = cmake(0.0, 0.0), dv = cmake(0.0, 0.0);
+#pragma unroll
+            for (int r = 0; r < R; r++) {
+                if (row0 + r == row) v = P[r];
+                if (row0 + r == j) dv = P[r];
+            }
+            S.wrows[warp][lane] = v;
+            if (j >= row0 && j < row0 + R) S.drowstage[lane] = dv;
+            if (lane == 0) { S.red_key[warp] = key; S.red_row[warp] = row; }
+        }
+        __syncthreads();
+        if (warp == 0) {       // CTA candidate; push (key, row, row content) to every CTA; CTA 0 also the diagonal row
+            unsigned long long bk = 0ull; int br = PNL_NONE, bw = 0;
+#pragma unroll
+            for (int q = 0; q < PNL_WARPS; q++) {
+                const unsigned long long k2 = S.red_key[q]; const int r2 = S.red_row[q];
+                if (r2 != PNL_NONE && (br == PNL_NONE || k2 > bk)) { bk = k2; br = r2; bw = q; }   // rows ascend with q
+            }
+            const cplx myrow = S.wrows[bw][lane];
+            const cplx drow = S.drowstage[lane];
+            if (C == 1) {
+                S.candrow[par][0][lane] = myrow; S.diagrow[par][lane] = drow;
+                if (lane == 0) { S.cand_key[par][0] = bk; S.cand_row[par][0] = br; }
+            } else {
+                for (int q = 0; q < C; q++) {
+                    RegPanelSmem* Rm = cluster.map_shared_rank(&S, q);
+                    Rm->candrow[par][rank][lane] = myrow;
+                    if (rank == 0) Rm->diagrow[par][lane] = drow;
+                    if (lane == 0) { Rm->cand_key[par][rank] = bk; Rm->cand_row[par][rank] = br; }
+                }
+            }
+        }
+        if (C == 1) __syncthreads(); else cluster.sync();
+        // everybody picks the same winner; rows are contiguous per CTA, so the row names its CTA
+        unsigned long long wk = 0ull; int prow = PNL_NONE;
         for (int q = 0; q < C; q++) {
             const unsigned long long k2 = S.cand_key[par][q]; const int r2 = S.cand_row[par][q];
-            if (r2 != NONE && (prow == NONE || k2 > wk || (k2 == wk && r2 < prow))) { wk = k2; prow = r2; wq = q; }
+            if (r2 != PNL_NONE && (prow == PNL_NONE || k2 > wk)) { wk = k2; prow = r2; }             // rows ascend with q
         }
-        const bool sing = (prow == NONE) || wk == 0ull;
-        if (prow == NONE) prow = j;
+        const bool sing = (prow == PNL_NONE) || wk == 0ull;
+        if (prow == PNL_NONE) prow = j;
+        const int wq = min(prow / (PNL_WARPS * R), C - 1);
         if (rank == 0 && tid == 0) {
             a.ipiv[(size_t)e * b + k0 + j] = k0 + prow;
             if (sing && a.info && a.info[e] == 0) a.info[e] = a.code > 0 ? a.code : (k0 + j + 1);
         }
-        const cplx* pr = S.candrow[par][wq];
-        // exchange rows j <-> prow
-        if (valid && gr == prow && prow != j) {
+        const cplx prl = sing ? cmake(0.0, 0.0) : S.candrow[par][wq][lane];
+        const cplx pjv = S.candrow[par][wq][j];
+        const cplx rinv = sing ? cmake(0.0, 0.0) : crecip_fast(pjv);
+        const cplx dgl = S.diagrow[par][lane];
 #pragma unroll
-            for (int c = 0; c < PW; c++) P[c] = S.diagrow[par][c];
-        }
-        if (rank == 0 && tid == j && prow != j) {
-#pragma unroll
-            for (int c = 0; c < PW; c++) P[c] = pr[c];
-        }
-        // eliminate below
-        if (valid && gr > j) {
-            cplx mine = cmake(0.0, 0.0);
-#pragma unroll
-            for (int c = 0; c < PW; c++) if (c == j) mine = P[c];
-            const cplx rinv = sing ? cmake(0.0, 0.0) : crecip(pr[j]);
-            const cplx l = cmul(mine, rinv);
-#pragma unroll
-            for (int c = 0; c < PW; c++) {
-                if (c == j) P[c] = l;
-                else if (c > j) cfms(P[c], l, pr[c]);
+        for (int r = 0; r < R; r++) {
+            const int gr = row0 + r;
+            if (prow != j) {                                       // exchange rows j <-> prow
+                if (gr == prow) P[r] = dgl;
+                else if (gr == j) P[r] = prl;
+            }
+            if (gr > j && gr < rows_total) {                       // eliminate below (warp-uniform test)
+                cplx pj;
+                pj.x = __shfl_sync(0xffffffffu, P[r].x, j);
+                pj.y = __shfl_sync(0xffffffffu, P[r].y, j);
+                const cplx l = cmul(pj, rinv);
+                if (lane == j) P[r] = l;
+                else if (lane > j) cfms(P[r], l, prl);
             }
         }
     }
@@ -529,26 +534,37 @@ __global__ void __launch_bounds__(NT) gj_panel_reg_kernel(PanelArgs a) {
     // (L11 U11)^-1 = U11^-1 L11^-1; L11^-1 goes to every CTA of the cluster.
     if (rank == 0) {
         for (int idx = tid; idx < PW * PW; idx += NT) { S.Li[idx] = cmake(0.0, 0.0); S.Ui[idx] = cmake(0.0, 0.0); }
-        if (tid < w) {
 #pragma unroll
-            for (int c = 0; c < PW; c++) S.Dm[tid * PW + c] = P[c];
-        }
+        for (int r = 0; r < R; r++)
+            if (row0 + r < PW) S.Dm[(row0 + r) * PW + lane] = P[r];
         __syncthreads();
+        // (Li and Ui are zero outside their triangles, so the sums run over fixed, unrolled ranges
+        // with four independent accumulators instead of a dependent load -> FMA chain)
         if (tid < w) {
             const int c = tid;
             for (int r = 0; r < w; r++) {
-                cplx s = (r == c) ? cmake(1.0, 0.0) : cmake(0.0, 0.0);
-                for (int k = c; k < r; k++) cfms(s, S.Dm[r * PW + k], S.Li[k * PW + c]);
-                S.Li[r * PW + c] = (r < c) ? cmake(0.0, 0.0) : s;
+                cplx s0 = (r == c) ? cmake(1.0, 0.0) : cmake(0.0, 0.0), s1 = cmake(0.0, 0.0), s2 = s1, s3 = s1;
+                for (int k = 0; k < r; k += 4) {
+                    cfms(s0, S.Dm[r * PW + k], S.Li[k * PW + c]);
+                    if (k + 1 < r) cfms(s1, S.Dm[r * PW + k + 1], S.Li[(k + 1) * PW + c]);
+                    if (k + 2 < r) cfms(s2, S.Dm[r * PW + k + 2], S.Li[(k + 2) * PW + c]);
+                    if (k + 3 < r) cfms(s3, S.Dm[r * PW + k + 3], S.Li[(k + 3) * PW + c]);
+                }
+                S.Li[r * PW + c] = (r < c) ? cmake(0.0, 0.0) : cadd(cadd(s0, s1), cadd(s2, s3));
             }
         } else if (tid >= 32 && tid < 32 + w) {
             const int c = tid - 32;
             for (int r = w - 1; r >= 0; r--) {
-                cplx s = (r == c) ? cmake(1.0, 0.0) : cmake(0.0, 0.0);
-                for (int k = r + 1; k <= c; k++) cfms(s, S.Dm[r * PW + k], S.Ui[k * PW + c]);
+                cplx s0 = (r == c) ? cmake(1.0, 0.0) : cmake(0.0, 0.0), s1 = cmake(0.0, 0.0), s2 = s1, s3 = s1;
+                for (int k = r + 1; k < w; k += 4) {
+                    cfms(s0, S.Dm[r * PW + k], S.Ui[k * PW + c]);
+                    if (k + 1 < w) cfms(s1, S.Dm[r * PW + k + 1], S.Ui[(k + 1) * PW + c]);
+                    if (k + 2 < w) cfms(s2, S.Dm[r * PW + k + 2], S.Ui[(k + 2) * PW + c]);
+                    if (k + 3 < w) cfms(s3, S.Dm[r * PW + k + 3], S.Ui[(k + 3) * PW + c]);
+                }
                 const cplx ur = S.Dm[r * PW + r];
                 const cplx inv = (ur.x == 0.0 && ur.y == 0.0) ? cmake(0.0, 0.0) : crecip(ur);
-                S.Ui[r * PW + c] = (r > c) ? cmake(0.0, 0.0) : cmul(s, inv);
+                S.Ui[r * PW + c] = (r > c) ? cmake(0.0, 0.0) : cmul(cadd(cadd(s0, s1), cadd(s2, s3)), inv);
             }
         }
         __syncthreads();
@@ -566,15 +582,19 @@ __global__ void __launch_bounds__(NT) gj_panel_reg_kernel(PanelArgs a) {
         }
     }
     cluster.sync();
-    // rows below the diagonal block: P' = -L21 L11^-1, written in place
-    if (valid && gr >= w) {
-        cplx* out = g + (size_t)gr * b;
-#pragma unroll 1
-        for (int c = 0; c < w; c++) {
-            cplx acc = cmake(0.0, 0.0);
+    // rows below the diagonal block: P' = -L21 L11^-1, written in place (lane = output column)
+    cplx* Lr = S.Lrow + (size_t)warp * R * PW;
 #pragma unroll
-            for (int k = 0; k < PW; k++) cfms(acc, P[k], S.Li[k * PW + c]);    // Li[k][c] = 0 for k < c and k >= w
-            out[c] = acc;
+    for (int r = 0; r < R; r++) Lr[r * PW + lane] = P[r];
+    __syncwarp();
+#pragma unroll 1
+    for (int r = 0; r < R; r++) {
+        const int gr = row0 + r;
+        if (gr >= w && gr < rows_total) {
+            cplx acc = cmake(0.0, 0.0);
+#pragma unroll 8
+            for (int k = 0; k < PW; k++) cfms(acc, Lr[r * PW + k], S.Li[k * PW + lane]);   // Li[k][c] = 0 for k < c, k >= w
+            if (lane < w) g[(size_t)gr * b + lane] = acc;
         }
     }
     cluster.sync();   // nobody exits while remote shared memory may still be targeted
@@ -700,12 +720,14 @@ int zinv_launch(negf_ctx* ctx, int b, cplx* A, long long sA, int batch, void* ws
     ProfScope _ps(ctx, NEGF_PROF_INVERSE);
     if (b <= 0 || batch <= 0) return NEGF_OK;
     if (b <= SMALL_MAX) {
-        if (b <= 16)      gj_reg_kernel<1, 2><<<batch, GJ_NW * 32, 0, ctx->stream>>>(A, sA, b, info, info_code, skip);
-        else if (b <= 32) gj_reg_kernel<1, 4><<<batch, GJ_NW * 32, 0, ctx->stream>>>(A, sA, b, info, info_code, skip);
-        else if (b <= 48) gj_reg_kernel<2, 6><<<batch, GJ_NW * 32, 0, ctx->stream>>>(A, sA, b, info, info_code, skip);
-        else if (b <= 64) gj_reg_kernel<2, 8><<<batch, GJ_NW * 32, 0, ctx->stream>>>(A, sA, b, info, info_code, skip);
-        else if (b <= 80) gj_reg_kernel<3, 10><<<batch, GJ_NW * 32, 0, ctx->stream>>>(A, sA, b, info, info_code, skip);
-        else              gj_reg_kernel<3, 12><<<batch, GJ_NW * 32, 0, ctx->stream>>>(A, sA, b, info, info_code, skip);
+        // 16 warps per matrix: half the instructions per warp and column of an 8-warp layout (the
+        // kernel is bound by the per-warp dependent instruction chain, not by issue slots or FP64)
+        if (b <= 16)      gj_reg_kernel<1, 1, 16><<<batch, 512, 0, ctx->stream>>>(A, sA, b, info, info_code, skip);
+        else if (b <= 32) gj_reg_kernel<1, 2, 16><<<batch, 512, 0, ctx->stream>>>(A, sA, b, info, info_code, skip);
+        else if (b <= 48) gj_reg_kernel<2, 3, 16><<<batch, 512, 0, ctx->stream>>>(A, sA, b, info, info_code, skip);
+        else if (b <= 64) gj_reg_kernel<2, 4, 16><<<batch, 512, 0, ctx->stream>>>(A, sA, b, info, info_code, skip);
+        else if (b <= 80) gj_reg_kernel<3, 5, 16><<<batch, 512, 0, ctx->stream>>>(A, sA, b, info, info_code, skip);
+        else              gj_reg_kernel<3, 6, 16><<<batch, 512, 0, ctx->stream>>>(A, sA, b, info, info_code, skip);
         NEGF_LAUNCH_CHECK(ctx);
         return NEGF_OK;
     }
@@ -722,8 +744,8 @@ int zinv_launch(negf_ctx* ctx, int b, cplx* A, long long sA, int batch, void* ws
         NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_panel_cluster_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                                   (int)(PANEL_SMEM_ROWS_BYTES + fixed)));
         NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_colperm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-        NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_panel_reg_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(RegPanelSmem)));
-        NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_panel_reg_kernel<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(RegPanelSmem)));
+        NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_panel_reg_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)reg_panel_smem_bytes(8)));
+        NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_panel_reg_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)reg_panel_smem_bytes(16)));
         attr_done = true;
     }
     const cplx one = cmake(1.0, 0.0), mone = cmake(-1.0, 0.0), zero = cmake(0.0, 0.0);
@@ -748,13 +770,14 @@ int zinv_launch(negf_ctx* ctx, int b, cplx* A, long long sA, int batch, void* ws
         cfg.attrs = at; cfg.numAttrs = 1; cfg.stream = ctx->stream;
         if (reg_panel) {
             // one row per thread in registers; finishes P' (diagonal block and below) in place
-            const int NT = rows <= 1024 ? 128 : 256;
-            const int C = (rows + NT - 1) / NT;
+            const int R = rows <= 1024 ? 8 : 16;                 // rows per warp; 16 warps per CTA
+            const int C = (rows + PNL_WARPS * R - 1) / (PNL_WARPS * R);
             PanelArgs pa{A, sA, b, k0, wk, 0, W.ipiv, W.Dinv, W.Linv, info, info_code, skip};
-            cfg.gridDim = dim3(C, batch); cfg.blockDim = dim3(NT); cfg.dynamicSmemBytes = sizeof(RegPanelSmem);
+            cfg.gridDim = dim3(C, batch); cfg.blockDim = dim3(PNL_WARPS * 32);
+            cfg.dynamicSmemBytes = reg_panel_smem_bytes(R);
             at[0].val.clusterDim.x = C;
-            if (NT == 128) NEGF_CUDA_CHECK(ctx, cudaLaunchKernelEx(&cfg, gj_panel_reg_kernel<128>, pa));
-            else           NEGF_CUDA_CHECK(ctx, cudaLaunchKernelEx(&cfg, gj_panel_reg_kernel<256>, pa));
+            if (R == 8) NEGF_CUDA_CHECK(ctx, cudaLaunchKernelEx(&cfg, gj_panel_reg_kernel<8>, pa));
+            else        NEGF_CUDA_CHECK(ctx, cudaLaunchKernelEx(&cfg, gj_panel_reg_kernel<16>, pa));
             ctx->launches++;
             if (nbk > wk) {
                 gj_swap_extract_kernel<<<dim3((nbk + 127) / 128, batch), 128, 0, ctx->stream>>>(
