@@ -20,6 +20,12 @@ extern "C" int negf_create(negf_ctx** out, int device) {
     c->device = device; c->stream = nullptr; c->ws = nullptr; c->ws_bytes = 0; c->last_cuda_error = 0;
     c->launches = 0; c->num_sms = prop.multiProcessorCount; c->sweep_valid = false;
     c->sw_n = c->sw_b = c->sw_ne = 0; c->sw_assembled = false;
+    for (int k = 0; k < NEGF_NSIDE; k++) {
+        if (cudaStreamCreateWithFlags(&c->side[k], cudaStreamNonBlocking) != cudaSuccess ||
+            cudaEventCreateWithFlags(&c->ev_fork[k], cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&c->ev_join[k], cudaEventDisableTiming) != cudaSuccess) { delete c; return NEGF_ECUDA; }
+    }
+    if (cudaEventCreateWithFlags(&c->ev_aux, cudaEventDisableTiming) != cudaSuccess) { delete c; return NEGF_ECUDA; }
     c->prof_on = false; c->prof_depth = 0;
     for (int k = 0; k < NEGF_PROF_CLASSES; k++) { c->prof_ms[k] = 0.0; c->prof_n[k] = 0; }
     *out = c;
@@ -29,6 +35,8 @@ extern "C" int negf_destroy(negf_ctx* ctx) {
     if (!ctx) return NEGF_EINVAL;
     for (auto& r : ctx->prof_recs) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
     for (auto e : ctx->prof_pool) cudaEventDestroy(e);
+    for (int k = 0; k < NEGF_NSIDE; k++) { cudaStreamDestroy(ctx->side[k]); cudaEventDestroy(ctx->ev_fork[k]); cudaEventDestroy(ctx->ev_join[k]); }
+    cudaEventDestroy(ctx->ev_aux);
     delete ctx;
     return NEGF_OK;
 }

@@ -9,10 +9,15 @@
 #include "../../include/negf.h"
 
 typedef double2 cplx;  // (x, y) = (re, im), same bytes as negf_c128
+constexpr int NEGF_NSIDE = 2;
 
 struct negf_ctx {
     int device;
-    cudaStream_t stream;
+    cudaStream_t stream;          // the stream launches go to (the caller's, or temporarily a side stream)
+    // side streams for independent sub-chains inside ONE call (two-sided sweeps); every call forks
+    // them from the caller's stream and joins them back before it returns
+    cudaStream_t side[NEGF_NSIDE];
+    cudaEvent_t ev_fork[NEGF_NSIDE], ev_join[NEGF_NSIDE], ev_aux;
     void* ws;              // caller-owned workspace
     size_t ws_bytes;
     int last_cuda_error;
@@ -109,6 +114,31 @@ __device__ __forceinline__ cplx crecip(cplx a) {
 __device__ __forceinline__ double cabs1(cplx a) { return fabs(a.x) + fabs(a.y); }
 
 static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+// Fork / join of the side streams and redirection of ctx->stream (restored by the destructor on
+// every exit path).  main = the caller's stream as it was when the guard was built.
+struct StreamFork {
+    negf_ctx* c; cudaStream_t main;
+    explicit StreamFork(negf_ctx* ctx) : c(ctx), main(ctx->stream) {}
+    ~StreamFork() { c->stream = main; }
+    void use_main() { c->stream = main; }
+    void use_side(int k) { c->stream = c->side[k]; }
+    // side k starts after everything enqueued on `from` so far (default: main)
+    cudaError_t fork(int k) {
+        cudaError_t e = cudaEventRecord(c->ev_fork[k], main);
+        return e != cudaSuccess ? e : cudaStreamWaitEvent(c->side[k], c->ev_fork[k], 0);
+    }
+    // main continues after everything enqueued on side k so far
+    cudaError_t join(int k) {
+        cudaError_t e = cudaEventRecord(c->ev_join[k], c->side[k]);
+        return e != cudaSuccess ? e : cudaStreamWaitEvent(main, c->ev_join[k], 0);
+    }
+    // side k waits for everything enqueued on main so far (mid-call dependency)
+    cudaError_t side_waits_main(int k) {
+        cudaError_t e = cudaEventRecord(c->ev_aux, main);
+        return e != cudaSuccess ? e : cudaStreamWaitEvent(c->side[k], c->ev_aux, 0);
+    }
+};
 
 // ---- internal entry points (host side, enqueue on ctx->stream) --------------------------------
 // zgemm.cu

@@ -13,98 +13,9 @@
 // and its dagger for every energy, so they are read straight from H (operand flags, alpha = -1)
 // and never materialised; otherwise the two off-diagonal families are assembled once per call.
 // The diagonal blocks are assembled straight into the g family and inverted in place.
-#include "common.cuh"
-#include "kernels.cuh"
-#include "workspace.cuh"
+#include "rgf_common.cuh"
 
-namespace {
-
-struct Shape { int n, b, ne; size_t bb; long long sb, sn, sm; };   // sn = n*bb, sm = (n-1)*bb
-
-Shape shape_of(const negf_problem* p) {
-    Shape s;
-    s.n = p->n_blocks; s.b = p->block_size; s.ne = p->n_energy;
-    s.bb = (size_t)s.b * s.b; s.sb = (long long)s.bb; s.sn = (long long)s.bb * s.n;
-    s.sm = (long long)s.bb * (s.n - 1);
-    return s;
-}
-
-int check_problem(const negf_ctx* ctx, const negf_problem* p) {
-    if (!ctx || !p) return NEGF_EINVAL;
-    if (p->n_blocks < 1 || p->block_size < 1 || p->n_energy < 1) return NEGF_EINVAL;
-    if (!p->H_diag || !p->energy) return NEGF_EINVAL;
-    if (p->n_blocks > 1 && !p->H_upper) return NEGF_EINVAL;
-    if (p->n_blocks > 1 && ((p->S_diag == nullptr) != (p->S_upper == nullptr))) return NEGF_EINVAL;
-    if (p->n_energy > 65535) return NEGF_EUNSUPPORTED;
-    return NEGF_OK;
-}
-
-int check_sigma(const negf_sigma* s, int n, bool retarded) {
-    if (!s) return NEGF_OK;
-    if (s->kind == NEGF_SIGMA_NONE) return NEGF_OK;
-    if (s->kind == NEGF_SIGMA_SCALAR) return s->scalar ? NEGF_OK : NEGF_EINVAL;
-    if (s->kind == NEGF_SIGMA_BT) {
-        if (!s->diag) return NEGF_EINVAL;
-        if (n > 1 && !s->upper) return NEGF_EINVAL;
-        if (n > 1 && retarded && !s->lower) return NEGF_EINVAL;
-        return NEGF_OK;
-    }
-    return NEGF_EINVAL;
-}
-
-bool needs_assembly(const negf_problem* p, const negf_sigma* sr) {
-    return p->S_diag != nullptr || (sr && sr->kind == NEGF_SIGMA_BT);
-}
-
-// A family of blocks as a GEMM operand: block i of energy e at p + e*se + i*si, read as op(.)
-struct Opnd { const cplx* p; long long se, si; int op; };
-inline Opnd dag(Opnd o) { o.op ^= 1; return o; }
-
-const cplx ONE = {1.0, 0.0}, MONE = {-1.0, 0.0}, ZERO = {0.0, 0.0};
-inline cplx real(double x) { return cmake(x, 0.0); }
-
-// C(ic + j) = alpha op(A(ia + j)) op(B(ib + j)) + beta D(id + j), j < cnt, for all energies
-GemmArgs gemm_fam(const Shape& s, cplx alpha, Opnd A, int ia, Opnd B, int ib, cplx beta, const Opnd* D, int id,
-                  Opnd C, int ic, int cnt) {
-    GemmArgs g = zgemm_bb_args(A.op, B.op, s.b, alpha, A.p + (size_t)ia * A.si, A.se, B.p + (size_t)ib * B.si, B.se, beta,
-                               D ? D->p + (size_t)id * D->si : nullptr, D ? D->se : 0,
-                               const_cast<cplx*>(C.p) + (size_t)ic * C.si, C.se, s.ne, nullptr);
-    g.batch2 = cnt; g.sA2 = A.si; g.sB2 = B.si; g.sD2 = D ? D->si : 0; g.sC2 = C.si;
-    return g;
-}
-inline GemmArgs gemm_one(const Shape& s, cplx alpha, Opnd A, int ia, Opnd B, int ib, cplx beta, const Opnd* D, int id,
-                         Opnd C, int ic) {
-    return gemm_fam(s, alpha, A, ia, B, ib, beta, D, id, C, ic, 1);
-}
-// families batched over (energy x i) can exceed the grid.y limit: split along i
-int launch_fam(negf_ctx* ctx, const Shape& s, cplx alpha, Opnd A, int ia, Opnd B, int ib, cplx beta, const Opnd* D,
-               int id, Opnd C, int ic, int cnt, const cplx* alpha_vec = nullptr) {
-    const int chunk = max(1, 65535 / s.ne);
-    for (int j = 0; j < cnt; j += chunk) {
-        GemmArgs g = gemm_fam(s, alpha, A, ia + j, B, ib + j, beta, D, id + j, C, ic + j, min(chunk, cnt - j));
-        g.alpha_vec = alpha_vec;
-        NEGF_TRY(zgemm_launch(ctx, g));
-    }
-    return NEGF_OK;
-}
-
-struct Fams {                // operand views of the workspace families and of A's off-diagonal blocks
-    Opnd g, X, Y, gx, Z, Q, AU, AL;
-    double sgn;              // AU / AL hold sgn * A_{i,i+1} / A_{i+1,i}
-};
-Fams make_fams(const negf_problem* p, const Shape& s, const Workspace& W, bool assembled) {
-    Fams f;
-    f.g = {W.g, s.sn, s.sb, 0}; f.gx = {W.gx, s.sn, s.sb, 0}; f.Q = {W.Q, s.sn, s.sb, 0};
-    f.X = {W.X, s.sm, s.sb, 0}; f.Y = {W.Y, s.sm, s.sb, 0}; f.Z = {W.Z, s.sm, s.sb, 0};
-    if (assembled) {
-        f.AU = {W.Aup, s.sm, s.sb, 0}; f.AL = {W.Alow, s.sm, s.sb, 0}; f.sgn = 1.0;
-    } else {                 // A_{i,i+1} = -H_{i,i+1}, A_{i+1,i} = -H_{i,i+1}^H for every energy
-        f.AU = {(const cplx*)p->H_upper, 0, s.sb, 0}; f.AL = {(const cplx*)p->H_upper, 0, s.sb, 1}; f.sgn = -1.0;
-    }
-    return f;
-}
-
-}  // namespace
+using namespace rgfc;
 
 extern "C" int negf_workspace_bytes(const negf_problem* p, int kind_max, int flags, size_t* bytes) {
     (void)flags;
@@ -115,23 +26,11 @@ extern "C" int negf_workspace_bytes(const negf_problem* p, int kind_max, int fla
     return NEGF_OK;
 }
 
-extern "C" int negf_rgf_retarded(negf_ctx* ctx, const negf_problem* p, const negf_sigma* sigma_r,
-                                 negf_c128* GR_diag_, negf_c128* GR_upper_, negf_c128* GR_lower_,
-                                 negf_c128* GR_corner_, int flags, int* info) {
-    NEGF_TRY(check_problem(ctx, p));
-    if (!GR_diag_ || !info) return NEGF_EINVAL;
-    const Shape s = shape_of(p);
-    NEGF_TRY(check_sigma(sigma_r, s.n, true));
-    if (!ctx->ws) return NEGF_ENOWORKSPACE;
-    const bool assembled = needs_assembly(p, sigma_r);
-    Workspace W = carve_workspace(ctx->ws, s.n, s.b, s.ne, assembled);
-    if (W.bytes > ctx->ws_bytes) return NEGF_ENOWORKSPACE;
-    ctx->sweep_valid = false;
+// S1: the diagonal blocks of A into the g family (inverted in place later) and, when they depend on
+// the energy, the two off-diagonal families.
+int rgf_assemble(negf_ctx* ctx, const negf_problem* p, const negf_sigma* sigma_r, const Shape& s, const Workspace& W,
+                 bool assembled) {
     const int b = s.b, ne = s.ne, n = s.n;
-    const Fams F = make_fams(p, s, W, assembled);
-    const Opnd GRd = {(const cplx*)GR_diag_, s.sn, s.sb, 0};
-    NEGF_TRY(ew_fill_int(ctx, info, ne, 0));
-
     // S1: diagonal blocks A_ii = z S_ii - H_ii - Sigma^R_ii for all i straight into the g family
     {
         CombineArgs ca = {};
@@ -165,6 +64,33 @@ extern "C" int negf_rgf_retarded(negf_ctx* ctx, const negf_problem* p, const neg
             if (n - 1 == 1) ca.nfam = 1;
             NEGF_TRY(ew_combine(ctx, ca, ne));
         }
+    }
+
+    return NEGF_OK;
+}
+
+extern "C" int negf_rgf_retarded(negf_ctx* ctx, const negf_problem* p, const negf_sigma* sigma_r,
+                                 negf_c128* GR_diag_, negf_c128* GR_upper_, negf_c128* GR_lower_,
+                                 negf_c128* GR_corner_, int flags, int* info) {
+    NEGF_TRY(check_problem(ctx, p));
+    if (!GR_diag_ || !info) return NEGF_EINVAL;
+    const Shape s = shape_of(p);
+    NEGF_TRY(check_sigma(sigma_r, s.n, true));
+    if (!ctx->ws) return NEGF_ENOWORKSPACE;
+    const bool assembled = needs_assembly(p, sigma_r);
+    Workspace W = carve_workspace(ctx->ws, s.n, s.b, s.ne, assembled);
+    if (W.bytes > ctx->ws_bytes) return NEGF_ENOWORKSPACE;
+    ctx->sweep_valid = false;
+    const int b = s.b, ne = s.ne, n = s.n;
+    const Fams F = make_fams(p, s, W, assembled);
+    const Opnd GRd = {(const cplx*)GR_diag_, s.sn, s.sb, 0};
+    NEGF_TRY(ew_fill_int(ctx, info, ne, 0));
+
+    NEGF_TRY(rgf_assemble(ctx, p, sigma_r, s, W, assembled));
+    if (b <= NEGF_PAIR_MAX_B) {      // latency-bound regime: two-sided sweeps (rgf2.cu)
+        NEGF_TRY(rgf2_retarded(ctx, p, s, W, F, (cplx*)GR_diag_, (cplx*)GR_upper_, (cplx*)GR_lower_, (cplx*)GR_corner_, info));
+        if (flags & NEGF_KEEP_SWEEP) { ctx->sweep_valid = true; ctx->sw_n = n; ctx->sw_b = b; ctx->sw_ne = ne; ctx->sw_assembled = assembled; }
+        return NEGF_OK;
     }
 
     // S3 forward: g_0 = A_00^-1 ; Y_{i-1} = A_{i,i-1} g_{i-1} ; g_i = (A_ii - Y_{i-1} A_{i-1,i})^-1
@@ -327,9 +253,12 @@ extern "C" int negf_rgf_lesser_greater(negf_ctx* ctx, const negf_problem* p, con
         return NEGF_ENOSTATE;
     const Fams F = make_fams(p, s, W, assembled);
     NEGF_TRY(ew_fill_int(ctx, info, s.ne, 0));
+    const bool two_sided = s.b <= NEGF_PAIR_MAX_B;
     if (sigma_lesser)
-        NEGF_TRY(lesser_greater_one(ctx, p, sigma_lesser, s, W, F, (const cplx*)GR_diag, (cplx*)GL_diag, (cplx*)GL_upper));
+        NEGF_TRY(two_sided ? rgf2_lesser_greater_one(ctx, sigma_lesser, s, W, F, (const cplx*)GR_diag, (cplx*)GL_diag, (cplx*)GL_upper)
+                           : lesser_greater_one(ctx, p, sigma_lesser, s, W, F, (const cplx*)GR_diag, (cplx*)GL_diag, (cplx*)GL_upper));
     if (sigma_greater)
-        NEGF_TRY(lesser_greater_one(ctx, p, sigma_greater, s, W, F, (const cplx*)GR_diag, (cplx*)GG_diag, (cplx*)GG_upper));
+        NEGF_TRY(two_sided ? rgf2_lesser_greater_one(ctx, sigma_greater, s, W, F, (const cplx*)GR_diag, (cplx*)GG_diag, (cplx*)GG_upper)
+                           : lesser_greater_one(ctx, p, sigma_greater, s, W, F, (const cplx*)GR_diag, (cplx*)GG_diag, (cplx*)GG_upper));
     return NEGF_OK;
 }

@@ -16,7 +16,9 @@ struct Workspace {
     cplx* Aup;      // [NE][n-1][b][b]  A_{i,i+1}, only when S != I or Sigma^R_S is BT   (retained)
     cplx* Alow;     // [NE][n-1][b][b]  A_{i+1,i}, likewise                              (retained)
     cplx* T[NEGF_NSCRATCH];   // [NE][b][b] each
-    void* inv;      // zinv workspace
+    void* inv;      // zinv workspace (batch NE * tmul)
+    void* inv2;     // second zinv workspace (batch NE) for the chain that runs on a side stream
+    void* inv_side(bool side) const { return side ? inv2 : inv; }
     double* ref;    // [NE]
     int* done;      // [NE]
     int* sing;      // [NE]
@@ -40,6 +42,7 @@ inline Workspace carve_workspace(void* base, int n, int b, int ne, bool assemble
     const int tm = negf_tmul(b);
     for (int t = 0; t < NEGF_NSCRATCH; t++) w.T[t] = (cplx*)take(blk * ne * tm);
     w.inv = take(zinv_workspace_bytes(b, ne * tm));
+    w.inv2 = tm == 2 ? take(zinv_workspace_bytes(b, ne)) : w.inv;
     w.ref = (double*)take(sizeof(double) * ne * 2);
     w.done = (int*)take(sizeof(int) * ne * 2);
     w.sing = (int*)take(sizeof(int) * ne * 2);
