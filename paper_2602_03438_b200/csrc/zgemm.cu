@@ -221,7 +221,9 @@ int zgemm_launch_group(negf_ctx* ctx, const GemmGroup& grp) {
     const long long t128 = (long long)((a.m + 127) / 128) * ((a.n + 63) / 64) * per;
     const long long t64 = (long long)((a.m + 63) / 64) * ((a.n + 63) / 64) * per;
     if (a.m > 64 && t128 >= ctx->num_sms) return launch_ops<128, 64, 4, 2, 1>(ctx, grp);
-    if (t64 >= ctx->num_sms) return launch_ops<64, 64, 2, 2, 2>(ctx, grp);
+    // blocks up to 64 x 64: four 32x32 CTAs per product balance the SMs better than one 64x64 CTA
+    // (measured 5-7 % faster at b = 64 for 128 .. 512 products per launch)
+    if ((a.m > 64 || a.n > 64) && t64 >= ctx->num_sms) return launch_ops<64, 64, 2, 2, 2>(ctx, grp);
     return launch_ops<32, 32, 2, 2, 3>(ctx, grp);
 }
 
