@@ -97,16 +97,21 @@ __global__ void sr_update_kernel(int b, cplx* a_s, cplx* a_b, cplx* g, const cpl
     a_b[o] = d; g[o] = d;
 }
 
-// small blocks: update + norms + convergence test of one doubling in ONE launch, one CTA per entry
+// small blocks: update + norms + convergence test of one doubling in ONE launch.  SR_SPLIT CTAs per
+// entry (the kernel is latency-bound per thread, not bandwidth-bound); the partial sums of squares
+// go to acc[entry][SR_SPLIT][2] and the CTA that arrives last (ticket counter) adds them in a
+// fixed order (deterministic) and takes the decision.
+constexpr int SR_SPLIT = 8;
 __global__ void __launch_bounds__(256) sr_step_kernel(int b, cplx* a_s, cplx* a_b, cplx* g, const cplx* lgu,
                                                       const cplx* ugl, const cplx* un, const cplx* ln,
-                                                      const double* ref, double tol, int* done, int* iters, int it) {
-    const int e = blockIdx.x;
+                                                      const double* ref, double tol, int* done, int* iters, int it,
+                                                      double* acc, unsigned* ticket) {
+    const int e = blockIdx.y;
     if (done[e]) return;
     __shared__ double su[8], sl[8];
     const size_t o = (size_t)e * b * b;
     double au = 0.0, al = 0.0;
-    for (int i = threadIdx.x; i < b * b; i += 256) {
+    for (int i = blockIdx.x * 256 + threadIdx.x; i < b * b; i += 256 * SR_SPLIT) {
         cplx x = lgu[o + i], y = ugl[o + i], s = a_s[o + i], d = a_b[o + i], u = un[o + i], l = ln[o + i];
         a_s[o + i] = csub(s, x);
         d = cmake(d.x - x.x - y.x, d.y - x.y - y.y);
@@ -123,8 +128,17 @@ __global__ void __launch_bounds__(256) sr_step_kernel(int b, cplx* a_s, cplx* a_
     if (threadIdx.x == 0) {
         au = 0.0; al = 0.0;
         for (int w = 0; w < 8; w++) { au += su[w]; al += sl[w]; }
-        iters[e] = it + 1;
-        if (sqrt(au) + sqrt(al) <= tol * ref[e]) done[e] = 1;
+        volatile double* slot = acc + (size_t)e * 2 * SR_SPLIT;
+        slot[2 * blockIdx.x] = au; slot[2 * blockIdx.x + 1] = al;
+        __threadfence();
+        if (atomicAdd(&ticket[e], 1u) == SR_SPLIT - 1) {       // last CTA of this entry: fixed summation order
+            __threadfence();
+            double tu = 0.0, tl = 0.0;
+            for (int q = 0; q < SR_SPLIT; q++) { tu += slot[2 * q]; tl += slot[2 * q + 1]; }
+            iters[e] = it + 1;
+            if (sqrt(tu) + sqrt(tl) <= tol * ref[e]) done[e] = 1;
+            ticket[e] = 0u;
+        }
     }
 }
 
@@ -231,9 +245,11 @@ int ew_max_int(negf_ctx* ctx, int* dst, const int* src, int n) {
     return NEGF_OK;
 }
 int ew_sr_step(negf_ctx* ctx, int b, int batch, cplx* a_s, cplx* a_b, cplx* g, const cplx* lgu, const cplx* ugl,
-               const cplx* un, const cplx* ln, const double* ref, double tol, int* done, int* iters, int it) {
+               const cplx* un, const cplx* ln, const double* ref, double tol, int* done, int* iters, int it,
+               double* acc, unsigned* ticket) {
     ProfScope _ps(ctx, NEGF_PROF_ELEMENTWISE);
-    sr_step_kernel<<<batch, 256, 0, ctx->stream>>>(b, a_s, a_b, g, lgu, ugl, un, ln, ref, tol, done, iters, it);
+    sr_step_kernel<<<dim3(SR_SPLIT, batch), 256, 0, ctx->stream>>>(b, a_s, a_b, g, lgu, ugl, un, ln, ref, tol, done, iters, it,
+                                                                   acc, ticket);
     NEGF_LAUNCH_CHECK(ctx);
     return NEGF_OK;
 }

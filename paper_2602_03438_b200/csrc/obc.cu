@@ -67,6 +67,7 @@ int obc_core(negf_ctx* ctx, const negf_problem* p, int ns, const LeadBlocks* lb,
     NEGF_TRY(ew_fill_int(ctx, W.done, nb, 0));
     NEGF_TRY(ew_fill_int(ctx, W.sing, nb, 0));
     NEGF_TRY(ew_fill_int(ctx, W.its, nb, 0));
+    NEGF_CUDA_CHECK(ctx, cudaMemsetAsync(W.ticket, 0, sizeof(unsigned) * nb, ctx->stream));
     NEGF_TRY(ew_sr_norm(ctx, b, nb, U0, L0, W.ref, tol, W.done, W.its, 0, 0));
 
     const bool fused_step = b <= NEGF_PAIR_MAX_B;
@@ -86,7 +87,7 @@ int obc_core(negf_ctx* ctx, const negf_problem* p, int ns, const LeadBlocks* lb,
         g2.g[3] = zgemm_bb_args(0, 0, b, mone, l, sb, gl, sb, zero, nullptr, 0, ln, sb, nb, skip);  // l <- -l g l
         NEGF_TRY(zgemm_launch_group(ctx, g2));
         if (fused_step) {
-            NEGF_TRY(ew_sr_step(ctx, b, nb, a_s, a_b, g, lgu, ugl, un, ln, W.ref, tol, W.done, W.its, it));
+            NEGF_TRY(ew_sr_step(ctx, b, nb, a_s, a_b, g, lgu, ugl, un, ln, W.ref, tol, W.done, W.its, it, W.acc, W.ticket));
         } else {
             NEGF_TRY(ew_sr_update(ctx, b, nb, a_s, a_b, g, lgu, ugl, skip));
             NEGF_TRY(ew_sr_norm(ctx, b, nb, un, ln, W.ref, tol, W.done, W.its, it, 1));
