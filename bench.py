@@ -298,7 +298,7 @@ def run_gpu(args, rank, local_rank, world):
         out["roofline"] = {"bound": "tensor", "kernel": {"gemm": "zgemm_kernel (DMMA.8x8x4, 4M complex)",
                                                          "fused": "fused chain kernels"}[dom],
                            "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                           "traffic": None,
+                           "traffic": roofline_traffic(wl.name),
                            "peak_source": "negf_fp64_peak: DMMA m8n8k4 issue-rate probe run in this process "
                                           "(MEASURED_PEAKS.json has no FP64 figure; nominal 37.2 = 148 SM x 1.965 GHz x 128 flop/clk)",
                            "flops_per_launch": dom_flops / max(dom_sites, 1),
@@ -318,6 +318,20 @@ def run_gpu(args, rank, local_rank, world):
     if dist is not None:
         dist.barrier()
         dist.destroy_process_group()
+
+
+def roofline_traffic(workload):
+    """DRAM bytes per launch of the dominant kernel from the committed ncu capture of this workload
+    (profiles/roofline_traffic.csv), or None when none was taken."""
+    import csv
+    try:
+        with open(os.path.join(ROOT, "profiles", "roofline_traffic.csv")) as f:
+            for row in csv.DictReader(f):
+                if row["workload"] == workload:
+                    return float(row["bytes_per_launch"])
+    except OSError:
+        pass
+    return None
 
 
 def default_energy_batch(wl, free_bytes):

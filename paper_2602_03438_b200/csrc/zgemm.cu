@@ -23,7 +23,9 @@
 namespace {
 
 constexpr int BK = 16;
-constexpr int STAGES = 3;
+// pipeline depth.  Measured on configs[1] (b = 64, 32x32 tiles): 2 / 3 / 4 / 5 stages give 8.77 / 8.68 /
+// 8.80 / 9.47 ms per step - more stages cost CTAs per SM, which matters more than load latency.
+template <int BM> struct StagesFor { static constexpr int value = 3; };
 
 __device__ __forceinline__ void dmma(double& c0, double& c1, double a, double b) {
     asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
@@ -74,6 +76,7 @@ template <int OPA, int OPB, int BM, int BN, int WM, int WN, int MINB>
 __global__ void __launch_bounds__(WM * WN * 32, MINB) zgemm_kernel(const __grid_constant__ GemmGroup grp) {
     const GemmArgs& a = grp.g[blockIdx.z];
     constexpr int NT = WM * WN * 32;
+    constexpr int STAGES = StagesFor<BM>::value;
     constexpr int MI = BM / WM / 8;     // 8x8 sub-tiles per warp along m
     constexpr int NI = BN / WN / 8;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -177,7 +180,7 @@ template <int OPA, int OPB, int BM, int BN, int WM, int WN, int MINB>
 int launch_cfg(negf_ctx* ctx, const GemmGroup& grp) {
     const GemmArgs& a = grp.g[0];
     auto kern = zgemm_kernel<OPA, OPB, BM, BN, WM, WN, MINB>;
-    constexpr int smem = STAGES * (BM + BN) * BK * (int)sizeof(cplx);
+    constexpr int smem = StagesFor<BM>::value * (BM + BN) * BK * (int)sizeof(cplx);
     static bool attr_done = false;
     if (!attr_done) {
         NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
