@@ -335,14 +335,18 @@ def roofline_traffic(workload):
 
 
 def default_energy_batch(wl, free_bytes):
-    """Energies resident at once: outputs (G^R 3F+corner, G^< 2F, G^> 2F) + workspace (4F + scratch)
-    + BT Sigma_S inputs, kept under ~70 % of free HBM."""
+    """Energies resident at once: outputs (G^R 3F + corner, G^< 2F, G^> 2F) + workspace (g, X, Y, g^x, Z, Q =
+    6F, + 2F when the off-diagonal blocks of A are assembled, + 13 scratch blocks + K1 scratch) + BT Sigma_S
+    inputs (7F), kept under 85 % of free HBM."""
     n, b = wl.n_blocks, wl.block_size
-    F = n * b * b * 16
-    per_e = (3 + 2 + (2 if wl.want_greater else 0) + 4) * F + 40 * b * b * 16
+    blk = b * b * 16
+    F = n * blk
+    assembled = wl.S_diag is not None or wl.sigma_kind == "bt"
+    per_e = (3 + 2 + (2 if wl.want_greater else 0)) * F + 6 * blk          # outputs + boundary blocks
+    per_e += (6 + (2 if assembled else 0)) * F + 13 * blk * (2 if b <= 128 else 1) + (128 + 64) * b * 16
     if wl.sigma_kind == "bt":
         per_e += 7 * F
-    return max(1, int(0.7 * free_bytes // per_e))
+    return max(1, int(0.85 * free_bytes // per_e))
 
 
 def run_e2e(args, wl, ctx, dev, world, torch, negf):

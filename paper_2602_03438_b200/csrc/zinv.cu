@@ -770,7 +770,8 @@ int zinv_launch(negf_ctx* ctx, int b, cplx* A, long long sA, int batch, void* ws
         cfg.attrs = at; cfg.numAttrs = 1; cfg.stream = ctx->stream;
         if (reg_panel) {
             // one row per thread in registers; finishes P' (diagonal block and below) in place
-            const int R = rows <= 1024 ? 8 : 16;                 // rows per warp; 16 warps per CTA
+            // rows per warp (16 warps per CTA): up to 256 rows stay in ONE CTA (no cluster barrier)
+            const int R = (rows <= 128 || (rows > 256 && rows <= 1024)) ? 8 : 16;
             const int C = (rows + PNL_WARPS * R - 1) / (PNL_WARPS * R);
             PanelArgs pa{A, sA, b, k0, wk, 0, W.ipiv, W.Dinv, W.Linv, info, info_code, skip};
             cfg.gridDim = dim3(C, batch); cfg.blockDim = dim3(PNL_WARPS * 32);
