@@ -104,6 +104,12 @@ int negf_workspace_bytes(const negf_problem* p, int kind_max, int flags, size_t*
 /* Caller-owned device scratch (e.g. a torch tensor), 256-byte aligned. Retained sweep state
  * lives here; replacing the workspace drops it. */
 int negf_set_workspace(negf_ctx* ctx, void* dev_ptr, size_t bytes);
+/* Options.  NEGF_OPT_GRAPH_LOOPS (default 1): for block sizes up to 96 the Sancho-Rubio doublings of
+ * negf_obc_decimate[_pair] run as a cached device-driven WHILE graph (CUDA conditional node) that stops
+ * when every energy has converged; 0 = the plain host loop of max_iter masked doublings.  Same
+ * arithmetic and results either way. */
+#define NEGF_OPT_GRAPH_LOOPS 1
+int negf_set_option(negf_ctx* ctx, int option, int value);
 const char* negf_strerror(int code);
 /* cudaError_t of the last failing runtime call on this context (0 if none). */
 int negf_last_cuda_error(const negf_ctx* ctx);

@@ -26,8 +26,10 @@ extern "C" int negf_create(negf_ctx** out, int device) {
             cudaEventCreateWithFlags(&c->ev_join[k], cudaEventDisableTiming) != cudaSuccess) { delete c; return NEGF_ECUDA; }
     }
     if (cudaEventCreateWithFlags(&c->ev_aux, cudaEventDisableTiming) != cudaSuccess) { delete c; return NEGF_ECUDA; }
+    c->graph_loops = true; c->obc_exec = nullptr; c->obc_key_ws = nullptr; c->obc_key_b = c->obc_key_nb = c->obc_key_maxit = 0; c->obc_key_tol = 0.0;
     c->prof_on = false; c->prof_depth = 0;
     for (int k = 0; k < NEGF_PROF_CLASSES; k++) { c->prof_ms[k] = 0.0; c->prof_n[k] = 0; }
+    if (zgemm_prepare(c) != NEGF_OK) { delete c; return NEGF_ECUDA; }
     *out = c;
     return NEGF_OK;
 }
@@ -37,6 +39,7 @@ extern "C" int negf_destroy(negf_ctx* ctx) {
     for (auto e : ctx->prof_pool) cudaEventDestroy(e);
     for (int k = 0; k < NEGF_NSIDE; k++) { cudaStreamDestroy(ctx->side[k]); cudaEventDestroy(ctx->ev_fork[k]); cudaEventDestroy(ctx->ev_join[k]); }
     cudaEventDestroy(ctx->ev_aux);
+    if (ctx->obc_exec) cudaGraphExecDestroy(ctx->obc_exec);
     delete ctx;
     return NEGF_OK;
 }
@@ -50,6 +53,11 @@ extern "C" int negf_set_workspace(negf_ctx* ctx, void* p, size_t bytes) {
     if (p && ((uintptr_t)p & 255)) return NEGF_EINVAL;
     ctx->ws = p; ctx->ws_bytes = p ? bytes : 0; ctx->sweep_valid = false;
     return NEGF_OK;
+}
+extern "C" int negf_set_option(negf_ctx* ctx, int option, int value) {
+    if (!ctx) return NEGF_EINVAL;
+    if (option == NEGF_OPT_GRAPH_LOOPS) { ctx->graph_loops = value != 0; return NEGF_OK; }
+    return NEGF_EINVAL;
 }
 extern "C" const char* negf_strerror(int code) {
     switch (code) {

@@ -27,6 +27,10 @@ struct negf_ctx {
     bool sweep_valid;
     int sw_n, sw_b, sw_ne;
     bool sw_assembled;
+    // cached device-driven WHILE graph of the Sancho-Rubio doublings (small blocks, obc.cu)
+    bool graph_loops;             // negf_set_option(NEGF_OPT_GRAPH_LOOPS)
+    cudaGraphExec_t obc_exec;
+    const void* obc_key_ws; int obc_key_b, obc_key_nb, obc_key_maxit; double obc_key_tol;
     // optional per-kernel-class timing (negf_profile_enable): event pairs around every launch site
     bool prof_on;
     int prof_depth;
@@ -158,6 +162,7 @@ struct GemmArgs {
     const cplx* alpha_vec;   // optional [batch]: entry e uses alpha * alpha_vec[e]
 };
 int zgemm_launch(negf_ctx* ctx, const GemmArgs& a);
+int zgemm_prepare(negf_ctx* ctx);
 // several independent products of identical shape / ops / batch in ONE launch (blockIdx.z = member)
 constexpr int NEGF_GEMM_GROUP_MAX = 4;
 struct GemmGroup { GemmArgs g[NEGF_GEMM_GROUP_MAX]; int ng; };
@@ -174,5 +179,5 @@ size_t zinv_workspace_bytes(int b, int batch);
 // in-place inverse of A[e] (b x b, ld = b, stride sA); ws: zinv_workspace_bytes; info_code = value
 // written to info[e] on a zero pivot (>0), info untouched otherwise (caller zero-fills).
 int zinv_launch(negf_ctx* ctx, int b, cplx* A, long long sA, int batch, void* ws, int* info,
-                int info_code, const int* skip);
+                int info_code, const int* skip, const int* code_dev = nullptr);   // small path: code = *code_dev + info_code
 

@@ -105,9 +105,10 @@ constexpr int SR_SPLIT = 8;
 __global__ void __launch_bounds__(256) sr_step_kernel(int b, cplx* a_s, cplx* a_b, cplx* g, const cplx* lgu,
                                                       const cplx* ugl, const cplx* un, const cplx* ln,
                                                       const double* ref, double tol, int* done, int* iters, int it,
-                                                      double* acc, unsigned* ticket) {
+                                                      double* acc, unsigned* ticket, const int* it_dev) {
     const int e = blockIdx.y;
     if (done[e]) return;
+    if (it_dev) it += *it_dev;
     __shared__ double su[8], sl[8];
     const size_t o = (size_t)e * b * b;
     double au = 0.0, al = 0.0;
@@ -199,6 +200,20 @@ __global__ void obc_status_kernel(int ne, const int* done, const int* sing, cons
     if (e < ne) { status[e] = sing[e] ? sing[e] : (done[e] ? 0 : -1); iters[e] = it_in[e]; }
 }
 
+// loop condition of the decimation WHILE graph: two more doublings while any entry is active
+__global__ void sr_cond_kernel(cudaGraphConditionalHandle h, int nb, const int* done, int* it_dev, int max_iter) {
+    __shared__ int any;
+    if (threadIdx.x == 0) any = 0;
+    __syncthreads();
+    for (int e = threadIdx.x; e < nb; e += blockDim.x) if (!done[e]) any = 1;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const int it = *it_dev + 2;
+        *it_dev = it;
+        cudaGraphSetConditional(h, (any && it < max_iter) ? 1u : 0u);
+    }
+}
+
 inline dim3 grid2(int b, int batch) { return dim3((b * b + 255) / 256, batch); }
 
 }  // namespace
@@ -246,10 +261,15 @@ int ew_max_int(negf_ctx* ctx, int* dst, const int* src, int n) {
 }
 int ew_sr_step(negf_ctx* ctx, int b, int batch, cplx* a_s, cplx* a_b, cplx* g, const cplx* lgu, const cplx* ugl,
                const cplx* un, const cplx* ln, const double* ref, double tol, int* done, int* iters, int it,
-               double* acc, unsigned* ticket) {
+               double* acc, unsigned* ticket, const int* it_dev) {
     ProfScope _ps(ctx, NEGF_PROF_ELEMENTWISE);
     sr_step_kernel<<<dim3(SR_SPLIT, batch), 256, 0, ctx->stream>>>(b, a_s, a_b, g, lgu, ugl, un, ln, ref, tol, done, iters, it,
-                                                                   acc, ticket);
+                                                                   acc, ticket, it_dev);
+    NEGF_LAUNCH_CHECK(ctx);
+    return NEGF_OK;
+}
+int ew_sr_cond(negf_ctx* ctx, cudaGraphConditionalHandle h, int nb, const int* done, int* it_dev, int max_iter) {
+    sr_cond_kernel<<<1, 128, 0, ctx->stream>>>(h, nb, done, it_dev, max_iter);
     NEGF_LAUNCH_CHECK(ctx);
     return NEGF_OK;
 }

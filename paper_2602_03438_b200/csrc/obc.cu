@@ -71,11 +71,11 @@ int obc_core(negf_ctx* ctx, const negf_problem* p, int ns, const LeadBlocks* lb,
     NEGF_TRY(ew_sr_norm(ctx, b, nb, U0, L0, W.ref, tol, W.done, W.its, 0, 0));
 
     const bool fused_step = b <= NEGF_PAIR_MAX_B;
-    const cplx* u = U0; const cplx* l = L0;
-    for (int it = 0; it < max_iter; it++) {
+    // one doubling: reads (u, l), writes (un, ln); `it` is the host iteration index, or the offset
+    // added to the device counter it_dev inside the WHILE graph
+    auto doubling = [&](const cplx* u, const cplx* l, cplx* un, cplx* ln, int it, const int* it_dev) -> int {
         const int* skip = W.done;
-        cplx* un = ub[it & 1]; cplx* ln = lbuf[it & 1];
-        NEGF_TRY(zinv_launch(ctx, b, g, sb, nb, W.inv, W.sing, it + 1, skip));            // g = a_b^-1
+        NEGF_TRY(zinv_launch(ctx, b, g, sb, nb, W.inv, W.sing, it + 1, skip, it_dev));     // g = a_b^-1
         GemmGroup g1; g1.ng = 2;
         g1.g[0] = zgemm_bb_args(0, 0, b, one, g, sb, u, sb, zero, nullptr, 0, gu, sb, nb, skip);    // g u
         g1.g[1] = zgemm_bb_args(0, 0, b, one, g, sb, l, sb, zero, nullptr, 0, gl, sb, nb, skip);    // g l
@@ -87,13 +87,64 @@ int obc_core(negf_ctx* ctx, const negf_problem* p, int ns, const LeadBlocks* lb,
         g2.g[3] = zgemm_bb_args(0, 0, b, mone, l, sb, gl, sb, zero, nullptr, 0, ln, sb, nb, skip);  // l <- -l g l
         NEGF_TRY(zgemm_launch_group(ctx, g2));
         if (fused_step) {
-            NEGF_TRY(ew_sr_step(ctx, b, nb, a_s, a_b, g, lgu, ugl, un, ln, W.ref, tol, W.done, W.its, it, W.acc, W.ticket));
+            NEGF_TRY(ew_sr_step(ctx, b, nb, a_s, a_b, g, lgu, ugl, un, ln, W.ref, tol, W.done, W.its, it, W.acc, W.ticket, it_dev));
         } else {
             NEGF_TRY(ew_sr_update(ctx, b, nb, a_s, a_b, g, lgu, ugl, skip));
             NEGF_TRY(ew_sr_norm(ctx, b, nb, un, ln, W.ref, tol, W.done, W.its, it, 1));
         }
-        // a converged entry keeps its last (u, l) in whichever buffer; they are not used again
-        u = un; l = ln;
+        return NEGF_OK;
+    };
+    // Small blocks: the loop is a device-driven WHILE graph (CUDA conditional node): its body is two
+    // doublings (so the ping-pong buffers have fixed roles) plus a kernel that keeps the loop going
+    // while any entry is active - no masked launches after convergence, no host synchronisation.
+    // The graph is cached per (workspace, shape, tol, max_iter); profiling runs use the plain loop.
+    const bool use_graph = b <= 96 && (max_iter % 2 == 0) && !ctx->prof_on && ctx->graph_loops;
+    if (use_graph) {
+        int* it_dev = W.tmpinfo;
+        NEGF_TRY(ew_copy(ctx, bb, nb, ub[1], sb, U0, sb, nullptr));
+        NEGF_TRY(ew_copy(ctx, bb, nb, lbuf[1], sb, L0, sb, nullptr));
+        NEGF_TRY(ew_fill_int(ctx, it_dev, 1, 0));
+        const bool hit = ctx->obc_exec && ctx->obc_key_ws == ctx->ws && ctx->obc_key_b == b && ctx->obc_key_nb == nb &&
+                         ctx->obc_key_maxit == max_iter && ctx->obc_key_tol == tol;
+        if (!hit) {
+            if (ctx->obc_exec) { cudaGraphExecDestroy(ctx->obc_exec); ctx->obc_exec = nullptr; }
+            cudaGraph_t G = nullptr;
+            NEGF_CUDA_CHECK(ctx, cudaGraphCreate(&G, 0));
+            cudaGraphConditionalHandle h;
+            NEGF_CUDA_CHECK(ctx, cudaGraphConditionalHandleCreate(&h, G, 1, cudaGraphCondAssignDefault));
+            cudaGraphNodeParams np = {};
+            np.type = cudaGraphNodeTypeConditional;
+            np.conditional.handle = h; np.conditional.type = cudaGraphCondTypeWhile; np.conditional.size = 1;
+            cudaGraphNode_t node;
+            NEGF_CUDA_CHECK(ctx, cudaGraphAddNode(&node, G, nullptr, 0, &np));
+            cudaGraph_t body = np.conditional.phGraph_out[0];
+            // captured on a side stream: the caller's stream may be the legacy default stream, which cannot capture
+            StreamFork sf(ctx);
+            sf.use_side(0);
+            cudaError_t ce = cudaStreamBeginCaptureToGraph(ctx->stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed);
+            if (ce != cudaSuccess) { cudaGraphDestroy(G); ctx->last_cuda_error = (int)ce; return NEGF_ECUDA; }
+            int rc = doubling(ub[1], lbuf[1], ub[0], lbuf[0], 0, it_dev);
+            if (rc == NEGF_OK) rc = doubling(ub[0], lbuf[0], ub[1], lbuf[1], 1, it_dev);
+            if (rc == NEGF_OK) rc = ew_sr_cond(ctx, h, nb, W.done, it_dev, max_iter);
+            cudaGraph_t dummy = nullptr;
+            ce = cudaStreamEndCapture(ctx->stream, &dummy);
+            sf.use_main();
+            if (rc != NEGF_OK) { cudaGraphDestroy(G); return rc; }
+            if (ce != cudaSuccess) { cudaGraphDestroy(G); ctx->last_cuda_error = (int)ce; return NEGF_ECUDA; }
+            ce = cudaGraphInstantiate(&ctx->obc_exec, G, 0);
+            cudaGraphDestroy(G);
+            if (ce != cudaSuccess) { ctx->obc_exec = nullptr; ctx->last_cuda_error = (int)ce; return NEGF_ECUDA; }
+            ctx->obc_key_ws = ctx->ws; ctx->obc_key_b = b; ctx->obc_key_nb = nb; ctx->obc_key_maxit = max_iter; ctx->obc_key_tol = tol;
+        }
+        NEGF_CUDA_CHECK(ctx, cudaGraphLaunch(ctx->obc_exec, ctx->stream));
+    } else {
+        const cplx* u = U0; const cplx* l = L0;
+        for (int it = 0; it < max_iter; it++) {
+            cplx* un = ub[it & 1]; cplx* ln = lbuf[it & 1];
+            NEGF_TRY(doubling(u, l, un, ln, it, nullptr));
+            // a converged entry keeps its last (u, l) in whichever buffer; they are not used again
+            u = un; l = ln;
+        }
     }
     // g_s = a_s^-1 ; Sigma = a_l g_s a_u (in the exchanged storage of a right lead: a_u g_s a_l)
     NEGF_TRY(zinv_launch(ctx, b, a_s, sb, nb, W.inv, W.sing, max_iter + 1, nullptr));

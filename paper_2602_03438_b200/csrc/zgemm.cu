@@ -181,11 +181,6 @@ int launch_cfg(negf_ctx* ctx, const GemmGroup& grp) {
     const GemmArgs& a = grp.g[0];
     auto kern = zgemm_kernel<OPA, OPB, BM, BN, WM, WN, MINB>;
     constexpr int smem = StagesFor<BM>::value * (BM + BN) * BK * (int)sizeof(cplx);
-    static bool attr_done = false;
-    if (!attr_done) {
-        NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        attr_done = true;
-    }
     int tiles = ((a.m + BM - 1) / BM) * ((a.n + BN - 1) / BN);
     dim3 grid(tiles, a.batch * a.batch2, grp.ng);
     kern<<<grid, WM * WN * 32, smem, ctx->stream>>>(grp);
@@ -203,6 +198,26 @@ int launch_ops(negf_ctx* ctx, const GemmGroup& grp) {
 }
 
 }  // namespace
+
+namespace {
+template <int BM, int BN, int WM, int WN, int MINB>
+cudaError_t prepare_cfg() {
+    constexpr int smem = StagesFor<BM>::value * (BM + BN) * BK * (int)sizeof(cplx);
+    cudaError_t e = cudaFuncSetAttribute(zgemm_kernel<0, 0, BM, BN, WM, WN, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(zgemm_kernel<1, 0, BM, BN, WM, WN, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(zgemm_kernel<0, 1, BM, BN, WM, WN, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(zgemm_kernel<1, 1, BM, BN, WM, WN, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    return e;
+}
+}  // namespace
+
+// dynamic shared-memory limits of every instantiation, once per context (never inside a stream capture)
+int zgemm_prepare(negf_ctx* ctx) {
+    NEGF_CUDA_CHECK(ctx, (prepare_cfg<128, 64, 4, 2, 1>()));
+    NEGF_CUDA_CHECK(ctx, (prepare_cfg<64, 64, 2, 2, 2>()));
+    NEGF_CUDA_CHECK(ctx, (prepare_cfg<32, 32, 2, 2, 3>()));
+    return NEGF_OK;
+}
 
 int zgemm_launch_group(negf_ctx* ctx, const GemmGroup& grp) {
     ProfScope _ps(ctx, NEGF_PROF_GEMM);

@@ -173,7 +173,7 @@ __device__ __forceinline__ void gj_columns(cplx (&m)[RB][CB], unsigned& used, co
 
 template <int RB, int CB, int GJ_NW>
 __global__ void __launch_bounds__(GJ_NW * 32) gj_reg_kernel(cplx* A, long long sA, int b, int* info, int code,
-                                                            const int* skip) {
+                                                            const int* skip, const int* code_dev) {
     constexpr int NR = RB * 32, NC = CB * GJ_NW;
     const int e = blockIdx.x;
     if (skip && skip[e]) return;
@@ -213,7 +213,7 @@ __global__ void __launch_bounds__(GJ_NW * 32) gj_reg_kernel(cplx* A, long long s
             const int i = lane + 32 * r, j = warp + GJ_NW * c;
             if (i < b && j < b) g[(size_t)dest[i] * b + piv[j]] = m[r][c];
         }
-    if (tid == 0 && s_sing && info) info[e] = code > 0 ? code : s_sing;
+    if (tid == 0 && s_sing && info) info[e] = code_dev ? *code_dev + code : (code > 0 ? code : s_sing);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -716,18 +716,18 @@ size_t zinv_workspace_bytes(int b, int batch) {
 }
 
 int zinv_launch(negf_ctx* ctx, int b, cplx* A, long long sA, int batch, void* ws, int* info,
-                int info_code, const int* skip) {
+                int info_code, const int* skip, const int* code_dev) {
     ProfScope _ps(ctx, NEGF_PROF_INVERSE);
     if (b <= 0 || batch <= 0) return NEGF_OK;
     if (b <= SMALL_MAX) {
         // 16 warps per matrix: half the instructions per warp and column of an 8-warp layout (the
         // kernel is bound by the per-warp dependent instruction chain, not by issue slots or FP64)
-        if (b <= 16)      gj_reg_kernel<1, 1, 16><<<batch, 512, 0, ctx->stream>>>(A, sA, b, info, info_code, skip);
-        else if (b <= 32) gj_reg_kernel<1, 2, 16><<<batch, 512, 0, ctx->stream>>>(A, sA, b, info, info_code, skip);
-        else if (b <= 48) gj_reg_kernel<2, 3, 16><<<batch, 512, 0, ctx->stream>>>(A, sA, b, info, info_code, skip);
-        else if (b <= 64) gj_reg_kernel<2, 4, 16><<<batch, 512, 0, ctx->stream>>>(A, sA, b, info, info_code, skip);
-        else if (b <= 80) gj_reg_kernel<3, 5, 16><<<batch, 512, 0, ctx->stream>>>(A, sA, b, info, info_code, skip);
-        else              gj_reg_kernel<3, 6, 16><<<batch, 512, 0, ctx->stream>>>(A, sA, b, info, info_code, skip);
+        if (b <= 16)      gj_reg_kernel<1, 1, 16><<<batch, 512, 0, ctx->stream>>>(A, sA, b, info, info_code, skip, code_dev);
+        else if (b <= 32) gj_reg_kernel<1, 2, 16><<<batch, 512, 0, ctx->stream>>>(A, sA, b, info, info_code, skip, code_dev);
+        else if (b <= 48) gj_reg_kernel<2, 3, 16><<<batch, 512, 0, ctx->stream>>>(A, sA, b, info, info_code, skip, code_dev);
+        else if (b <= 64) gj_reg_kernel<2, 4, 16><<<batch, 512, 0, ctx->stream>>>(A, sA, b, info, info_code, skip, code_dev);
+        else if (b <= 80) gj_reg_kernel<3, 5, 16><<<batch, 512, 0, ctx->stream>>>(A, sA, b, info, info_code, skip, code_dev);
+        else              gj_reg_kernel<3, 6, 16><<<batch, 512, 0, ctx->stream>>>(A, sA, b, info, info_code, skip, code_dev);
         NEGF_LAUNCH_CHECK(ctx);
         return NEGF_OK;
     }

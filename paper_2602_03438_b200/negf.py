@@ -23,6 +23,7 @@ PROF_NAMES = ("gemm", "inverse", "elementwise", "observables", "fused")
 OK, EINVAL, ENOWORKSPACE, EUNSUPPORTED, ECUDA, ENOSTATE = 0, -1, -2, -3, -4, -5
 SIGMA_NONE, SIGMA_SCALAR, SIGMA_BT = 0, 1, 2
 KEEP_SWEEP = 1
+OPT_GRAPH_LOOPS = 1
 
 
 class c128(C.Structure):
@@ -56,7 +57,7 @@ class HostOutputs(C.Structure):
 
 
 EXPORTS = ["negf_create", "negf_destroy", "negf_set_stream", "negf_workspace_bytes", "negf_set_workspace",
-           "negf_strerror", "negf_last_cuda_error", "negf_launch_count",
+           "negf_set_option", "negf_strerror", "negf_last_cuda_error", "negf_launch_count",
            "negf_profile_enable", "negf_profile_read", "negf_obc_decimate", "negf_obc_decimate_pair",
            "negf_rgf_retarded", "negf_rgf_lesser_greater", "negf_observables", "negf_pipeline_host_bytes",
            "negf_pipeline_host", "negf_zgemm_batched", "negf_zinverse_batched", "negf_fp64_peak"]
@@ -67,6 +68,7 @@ lib.negf_destroy.argtypes = [_P]
 lib.negf_set_stream.argtypes = [_P, _P]
 lib.negf_workspace_bytes.argtypes = [C.POINTER(Problem), C.c_int, C.c_int, C.POINTER(C.c_size_t)]
 lib.negf_set_workspace.argtypes = [_P, _P, C.c_size_t]
+lib.negf_set_option.argtypes = [_P, C.c_int, C.c_int]
 lib.negf_strerror.argtypes = [C.c_int]
 lib.negf_strerror.restype = C.c_char_p
 lib.negf_last_cuda_error.argtypes = [_P]
@@ -169,6 +171,9 @@ class Context:
         self._ws = tensor
         self._check(lib.negf_set_workspace(self._h, _ptr(tensor), 0 if tensor is None else tensor.numel()),
                     "negf_set_workspace")
+
+    def set_option(self, option: int, value: int):
+        self._check(lib.negf_set_option(self._h, option, value), "negf_set_option")
 
     def launch_count(self) -> int:
         return int(lib.negf_launch_count(self._h))

@@ -193,3 +193,21 @@ def test_obc_pair_equals_two_single_calls(runner_mod, cfg, kw):
     dp.obc(pair=False)
     for k, v in pair.items():
         assert np.array_equal(v, dp.host(k)), k
+
+
+@pytest.mark.parametrize("cfg,kw", [CASES[0], CASES[3]])
+def test_obc_graph_loop_equals_host_loop(runner_mod, negf_lib, cfg, kw):
+    """The device-driven WHILE graph of the doublings (CUDA conditional node, default for b <= 96) and the
+    plain host loop of max_iter masked doublings run the same kernels on the same data: bit-identical."""
+    wl = W.make_workload(cfg, **kw)
+    dp = runner_mod.DevicePath(wl, want_greater=True)
+    dp.obc()
+    dp.obc()                                  # second call replays the cached graph
+    graph = {k: dp.host(k).copy() for k in dp.out if k.endswith(("_L", "_R"))}
+    assert int(dp.out["iters_L"].min()) > 5
+    dp.ctx.set_option(negf_lib.OPT_GRAPH_LOOPS, 0)
+    for k in graph:
+        dp.out[k].zero_()
+    dp.obc()
+    for k, v in graph.items():
+        assert np.array_equal(v, dp.host(k)), k
