@@ -249,6 +249,11 @@ def run_gpu(args, rank, local_rank, world):
     iters_mean = float(sum(d.out["iters_L"].double().sum() + d.out["iters_R"].double().sum() for d in dps)
                        / (2 * sum(d.ne for d in dps)))
     iters_total = iters_mean * 2 * wl.n_energy
+    if wl.block_size <= 96 and wl.max_iter % 2 == 0:
+        # the doublings run inside a device-driven WHILE graph (one host launch): its kernels are counted from
+        # the iteration counters: 9 per pair of doublings (2 x [inverse, 2 grouped GEMMs, step] + loop condition)
+        it_max = max(int(max(d.out["iters_L"].max(), d.out["iters_R"].max())) for d in dps)
+        launches += args.steps * len(dps) * (-(-it_max // 2)) * 9
     U = 8.0 * wl.block_size ** 3
     gemm_u, inv_u = unit_counts(wl.n_blocks, wl.sigma_kind, wl.want_greater, iters_total, wl.n_energy)
     step_ms = ms / args.steps

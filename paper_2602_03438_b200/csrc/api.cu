@@ -26,7 +26,9 @@ extern "C" int negf_create(negf_ctx** out, int device) {
             cudaEventCreateWithFlags(&c->ev_join[k], cudaEventDisableTiming) != cudaSuccess) { delete c; return NEGF_ECUDA; }
     }
     if (cudaEventCreateWithFlags(&c->ev_aux, cudaEventDisableTiming) != cudaSuccess) { delete c; return NEGF_ECUDA; }
-    c->graph_loops = true; c->obc_exec = nullptr; c->obc_key_ws = nullptr; c->obc_key_b = c->obc_key_nb = c->obc_key_maxit = 0; c->obc_key_tol = 0.0;
+    c->graph_loops = true; c->obc_exec = nullptr;
+    for (int k = 0; k < NEGF_NGRAPH; k++) { c->gslot[k].key = 0; c->gslot[k].exec = nullptr; c->gslot[k].launches = 0; }
+    if (cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking) != cudaSuccess) { delete c; return NEGF_ECUDA; } c->obc_key_ws = nullptr; c->obc_key_b = c->obc_key_nb = c->obc_key_maxit = 0; c->obc_key_tol = 0.0;
     c->prof_on = false; c->prof_depth = 0;
     for (int k = 0; k < NEGF_PROF_CLASSES; k++) { c->prof_ms[k] = 0.0; c->prof_n[k] = 0; }
     if (zgemm_prepare(c) != NEGF_OK) { delete c; return NEGF_ECUDA; }
@@ -40,6 +42,8 @@ extern "C" int negf_destroy(negf_ctx* ctx) {
     for (int k = 0; k < NEGF_NSIDE; k++) { cudaStreamDestroy(ctx->side[k]); cudaEventDestroy(ctx->ev_fork[k]); cudaEventDestroy(ctx->ev_join[k]); }
     cudaEventDestroy(ctx->ev_aux);
     if (ctx->obc_exec) cudaGraphExecDestroy(ctx->obc_exec);
+    for (int k = 0; k < NEGF_NGRAPH; k++) if (ctx->gslot[k].exec) cudaGraphExecDestroy(ctx->gslot[k].exec);
+    cudaStreamDestroy(ctx->cap_stream);
     delete ctx;
     return NEGF_OK;
 }
@@ -52,6 +56,7 @@ extern "C" int negf_set_workspace(negf_ctx* ctx, void* p, size_t bytes) {
     if (!ctx) return NEGF_EINVAL;
     if (p && ((uintptr_t)p & 255)) return NEGF_EINVAL;
     ctx->ws = p; ctx->ws_bytes = p ? bytes : 0; ctx->sweep_valid = false;
+    for (int k = 0; k < NEGF_NGRAPH; k++) ctx->gslot[k].key = 0;
     return NEGF_OK;
 }
 extern "C" int negf_set_option(negf_ctx* ctx, int option, int value) {

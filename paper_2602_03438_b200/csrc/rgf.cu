@@ -84,14 +84,20 @@ extern "C" int negf_rgf_retarded(negf_ctx* ctx, const negf_problem* p, const neg
     const int b = s.b, ne = s.ne, n = s.n;
     const Fams F = make_fams(p, s, W, assembled);
     const Opnd GRd = {(const cplx*)GR_diag_, s.sn, s.sb, 0};
-    NEGF_TRY(ew_fill_int(ctx, info, ne, 0));
-
-    NEGF_TRY(rgf_assemble(ctx, p, sigma_r, s, W, assembled));
-    if (b <= NEGF_PAIR_MAX_B) {      // latency-bound regime: two-sided sweeps (rgf2.cu)
-        NEGF_TRY(rgf2_retarded(ctx, p, s, W, F, (cplx*)GR_diag_, (cplx*)GR_upper_, (cplx*)GR_lower_, (cplx*)GR_corner_, info));
+    if (b <= NEGF_PAIR_MAX_B) {      // latency-bound regime: two-sided sweeps (rgf2.cu), replayed as a cached graph
+        KeyHash k;
+        k.val(*p); if (sigma_r) k.val(*sigma_r);
+        k.val(GR_diag_); k.val(GR_upper_); k.val(GR_lower_); k.val(GR_corner_); k.val(info); k.val(ctx->ws); k.val(ctx->ws_bytes);
+        NEGF_TRY(run_cached(ctx, 0, k.h, b <= 96, [&]() -> int {
+            NEGF_TRY(ew_fill_int(ctx, info, ne, 0));
+            NEGF_TRY(rgf_assemble(ctx, p, sigma_r, s, W, assembled));
+            return rgf2_retarded(ctx, p, s, W, F, (cplx*)GR_diag_, (cplx*)GR_upper_, (cplx*)GR_lower_, (cplx*)GR_corner_, info);
+        }));
         if (flags & NEGF_KEEP_SWEEP) { ctx->sweep_valid = true; ctx->sw_n = n; ctx->sw_b = b; ctx->sw_ne = ne; ctx->sw_assembled = assembled; }
         return NEGF_OK;
     }
+    NEGF_TRY(ew_fill_int(ctx, info, ne, 0));
+    NEGF_TRY(rgf_assemble(ctx, p, sigma_r, s, W, assembled));
 
     // S3 forward: g_0 = A_00^-1 ; Y_{i-1} = A_{i,i-1} g_{i-1} ; g_i = (A_ii - Y_{i-1} A_{i-1,i})^-1
     for (int i = 0; i < n; i++) {
@@ -252,8 +258,13 @@ extern "C" int negf_rgf_lesser_greater(negf_ctx* ctx, const negf_problem* p, con
     if (!ctx->sweep_valid || ctx->sw_n != s.n || ctx->sw_b != s.b || ctx->sw_ne != s.ne || ctx->sw_assembled != assembled)
         return NEGF_ENOSTATE;
     const Fams F = make_fams(p, s, W, assembled);
-    NEGF_TRY(ew_fill_int(ctx, info, s.ne, 0));
     const bool two_sided = s.b <= NEGF_PAIR_MAX_B;
+    KeyHash k;
+    k.val(*p); if (sigma_r) k.val(*sigma_r); if (sigma_lesser) k.val(*sigma_lesser); if (sigma_greater) k.val(*sigma_greater);
+    k.val(sigma_lesser != nullptr); k.val(sigma_greater != nullptr);
+    k.val(GR_diag); k.val(GL_diag); k.val(GL_upper); k.val(GG_diag); k.val(GG_upper); k.val(info); k.val(ctx->ws); k.val(ctx->ws_bytes);
+    return run_cached(ctx, 1, k.h, two_sided && s.b <= 96, [&]() -> int {
+    NEGF_TRY(ew_fill_int(ctx, info, s.ne, 0));
     if (sigma_lesser)
         NEGF_TRY(two_sided ? rgf2_lesser_greater_one(ctx, sigma_lesser, s, W, F, (const cplx*)GR_diag, (cplx*)GL_diag, (cplx*)GL_upper)
                            : lesser_greater_one(ctx, p, sigma_lesser, s, W, F, (const cplx*)GR_diag, (cplx*)GL_diag, (cplx*)GL_upper));
@@ -261,4 +272,5 @@ extern "C" int negf_rgf_lesser_greater(negf_ctx* ctx, const negf_problem* p, con
         NEGF_TRY(two_sided ? rgf2_lesser_greater_one(ctx, sigma_greater, s, W, F, (const cplx*)GR_diag, (cplx*)GG_diag, (cplx*)GG_upper)
                            : lesser_greater_one(ctx, p, sigma_greater, s, W, F, (const cplx*)GR_diag, (cplx*)GG_diag, (cplx*)GG_upper));
     return NEGF_OK;
+    });
 }

@@ -211,3 +211,25 @@ def test_obc_graph_loop_equals_host_loop(runner_mod, negf_lib, cfg, kw):
     dp.obc()
     for k, v in graph.items():
         assert np.array_equal(v, dp.host(k)), k
+
+
+@pytest.mark.parametrize("cfg,kw", [CASES[0], CASES[3], CASES[6]])
+def test_cached_call_graphs_replay_identically(runner_mod, negf_lib, cfg, kw):
+    """For b <= 96 the second negf_rgf_* call with the same arguments is captured into a CUDA graph and later
+    calls replay it: first (plain), second (captured) and third (replayed) pass give bit-identical outputs,
+    and so does a pass with the option switched off."""
+    wl = W.make_workload(cfg, **kw)
+    dp = runner_mod.DevicePath(wl, want_greater=True)
+    names = ["GR_diag", "GR_upper", "GR_lower", "GR_corner", "GL_diag", "GL_upper", "GG_diag", "GG_upper",
+             "transmission", "density"]
+    passes = []
+    for rep in range(4):
+        if rep == 3:
+            dp.ctx.set_option(negf_lib.OPT_GRAPH_LOOPS, 0)
+        for nm in names:
+            dp.out[nm].zero_()
+        dp.run()
+        passes.append({nm: dp.host(nm).copy() for nm in names})
+    for rep in (1, 2, 3):
+        for nm in names:
+            assert np.array_equal(passes[0][nm], passes[rep][nm]), (rep, nm)
