@@ -356,58 +356,22 @@ def default_energy_batch(wl, free_bytes):
 
 def run_e2e(args, wl, ctx, dev, world, torch, negf):
     """negf_pipeline_host on the first energy batch that fits, HOST (pinned) inputs and outputs."""
+    from paper_2602_03438_b200 import runner
     n, b = wl.n_blocks, wl.block_size
     ne = min(wl.n_energy, args.e2e_energies or wl.n_energy)
     F = n * b * b * 16
     while ne > 1 and ne * F * 12 > 24e9:      # keep pinned host memory bounded
         ne //= 2
-    pin = lambda a: None if a is None else torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
-    Hd, Hu, Sd, Su = pin(wl.H_diag), pin(wl.H_upper), pin(wl.S_diag), pin(wl.S_upper)
-    en, wt = pin(wl.energies[:ne].copy()), pin(wl.weights[:ne].copy())
-    hp = negf.make_problem(n, b, ne, Hd, Hu, Sd, Su, en, wl.eta)
-    sig = wl.sigma_s(0, ne)
-    keep, hs = [], {}
-    for t in "rlg":
-        s = sig[t]
-        if s is None or (t == "g" and not wl.want_greater):
-            hs[t] = None
-        elif s["kind"] == "scalar":
-            v = pin(s["value"]); keep.append(v)
-            hs[t] = negf.make_sigma(negf.SIGMA_SCALAR, scalar=v)
-        else:
-            d, u, l = pin(s["diag"]), pin(s["upper"]), pin(s.get("lower")); keep += [d, u, l]
-            hs[t] = negf.make_sigma(negf.SIGMA_BT, diag=d, upper=u, lower=l)
-    if hs["r"] is None:
-        hs["r"] = negf.make_sigma(negf.SIGMA_NONE)
-    if hs["l"] is None:
-        hs["l"] = negf.make_sigma(negf.SIGMA_NONE)
-    if wl.want_greater and hs["g"] is None:
-        hs["g"] = negf.make_sigma(negf.SIGMA_NONE)
-    kind = {"none": negf.SIGMA_NONE, "scalar": negf.SIGMA_SCALAR, "bt": negf.SIGMA_BT}[wl.sigma_kind]
-    scratch = torch.empty(negf.Context.pipeline_host_bytes(hp, kind, wl.want_greater), dtype=torch.uint8, device=dev)
-    z = lambda *s: torch.empty(s, dtype=torch.complex128).pin_memory()
-    r = lambda *s: torch.empty(s, dtype=torch.float64).pin_memory()
-    o = {"GR_diag": z(ne, n, b, b), "GR_upper": z(ne, n - 1, b, b), "GR_lower": z(ne, n - 1, b, b),
-         "GL_diag": z(ne, n, b, b), "GL_upper": z(ne, n - 1, b, b),
-         "GG_diag": z(ne, n, b, b) if wl.want_greater else None,
-         "GG_upper": z(ne, n - 1, b, b) if wl.want_greater else None,
-         "density": r(n * b), "ldos": r(ne, n), "transmission": r(ne), "bond_current": r(ne, n - 1),
-         "contact_current": r(ne, 2) if wl.want_greater else None,
-         "info": torch.empty(ne, dtype=torch.int32).pin_memory()}
-    ho = negf.HostOutputs(*[negf._ptr(o[k]) for k in ("GR_diag", "GR_upper", "GR_lower", "GL_diag", "GL_upper",
-                                                      "GG_diag", "GG_upper", "density", "ldos", "transmission",
-                                                      "bond_current", "contact_current", "info")])
-    call = lambda: ctx.pipeline_host(hp, hs["r"], hs["l"], hs["g"], wt, wl.mu_L, wl.mu_R, wl.kT, wl.tol,
-                                     wl.max_iter, scratch, ho)
+    hp = runner.HostPath(wl, ne, device=dev, ctx=ctx)
     reps = max(1, min(args.steps, 5))
     for _ in range(2):
-        up, down = call()
+        up, down = hp.run()
     torch.cuda.synchronize()
     t0 = time.perf_counter()
     for _ in range(reps):
-        up, down = call()              # synchronises the stream before returning
+        up, down = hp.run()            # synchronises the stream before returning
     dt = time.perf_counter() - t0
-    assert int(o["info"].abs().sum()) == 0, "numerical failure flagged in the e2e run"
+    assert int(hp.out["info"].abs().sum()) == 0, "numerical failure flagged in the e2e run"
     return {"value": world * ne * reps / dt, "unit": UNIT, "h2d_bytes_per_step": int(up), "d2h_bytes_per_step": int(down),
             "energies_per_call": ne, "ms_per_call": 1e3 * dt / reps,
             "api": "negf_pipeline_host (host pinned buffers in, all selected G blocks + observables out)"}

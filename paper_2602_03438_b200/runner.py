@@ -144,3 +144,57 @@ class DevicePath:
 
     def host(self, name: str) -> np.ndarray:
         return self.out[name].cpu().numpy()
+
+
+class HostPath:
+    """The whole path through negf_pipeline_host: HOST (pinned) inputs and outputs, host<->device copies
+    inside the call (what bench.py times as the end-to-end number)."""
+
+    def __init__(self, wl: Workload, n_energy: Optional[int] = None, device: str = "cuda:0",
+                 ctx: Optional[negf.Context] = None, want_greater: Optional[bool] = None):
+        self.wl = wl
+        self.device = torch.device(device)
+        self.ne = wl.n_energy if n_energy is None else min(n_energy, wl.n_energy)
+        self.n, self.b = wl.n_blocks, wl.block_size
+        self.want_greater = wl.want_greater if want_greater is None else want_greater
+        self.ctx = ctx or negf.Context(self.device.index or 0)
+        ne, n, b = self.ne, self.n, self.b
+        pin = lambda a: None if a is None else torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+        self._keep = [pin(wl.H_diag), pin(wl.H_upper), pin(wl.S_diag), pin(wl.S_upper),
+                      pin(wl.energies[:ne].astype(np.float64)), pin(wl.weights[:ne].astype(np.float64))]
+        Hd, Hu, Sd, Su, en, self.weights = self._keep
+        self.problem = negf.make_problem(n, b, ne, Hd, Hu, Sd, Su, en, wl.eta)
+        sig = wl.sigma_s(0, ne)
+        self.sig = {}
+        for t in "rlg":
+            s = sig[t]
+            if t == "g" and not self.want_greater:
+                self.sig[t] = None
+            elif s is None:
+                self.sig[t] = negf.make_sigma(negf.SIGMA_NONE)
+            elif s["kind"] == "scalar":
+                v = pin(s["value"]); self._keep.append(v)
+                self.sig[t] = negf.make_sigma(negf.SIGMA_SCALAR, scalar=v)
+            else:
+                d, u, l = pin(s["diag"]), pin(s["upper"]), pin(s.get("lower")); self._keep += [d, u, l]
+                self.sig[t] = negf.make_sigma(negf.SIGMA_BT, diag=d, upper=u, lower=l)
+        kind = _KIND[wl.sigma_kind]
+        self.scratch = torch.empty(negf.Context.pipeline_host_bytes(self.problem, kind, self.want_greater),
+                                   dtype=torch.uint8, device=self.device)
+        z = lambda *s: torch.empty(s, dtype=torch.complex128).pin_memory()
+        r = lambda *s: torch.empty(s, dtype=torch.float64).pin_memory()
+        g = self.want_greater
+        self.out = {"GR_diag": z(ne, n, b, b), "GR_upper": z(ne, n - 1, b, b), "GR_lower": z(ne, n - 1, b, b),
+                    "GL_diag": z(ne, n, b, b), "GL_upper": z(ne, n - 1, b, b),
+                    "GG_diag": z(ne, n, b, b) if g else None, "GG_upper": z(ne, n - 1, b, b) if g else None,
+                    "density": r(n * b), "ldos": r(ne, n), "transmission": r(ne), "bond_current": r(ne, n - 1),
+                    "contact_current": r(ne, 2) if g else None, "info": torch.empty(ne, dtype=torch.int32).pin_memory()}
+        self._ho = negf.HostOutputs(*[negf._ptr(self.out[k]) for k in
+                                      ("GR_diag", "GR_upper", "GR_lower", "GL_diag", "GL_upper", "GG_diag", "GG_upper",
+                                       "density", "ldos", "transmission", "bond_current", "contact_current", "info")])
+
+    def run(self):
+        """One synchronising call; returns (h2d_bytes, d2h_bytes)."""
+        wl = self.wl
+        return self.ctx.pipeline_host(self.problem, self.sig["r"], self.sig["l"], self.sig["g"], self.weights,
+                                      wl.mu_L, wl.mu_R, wl.kT, wl.tol, wl.max_iter, self.scratch, self._ho)
