@@ -27,7 +27,10 @@ extern "C" int negf_create(negf_ctx** out, int device) {
     }
     if (cudaEventCreateWithFlags(&c->ev_aux, cudaEventDisableTiming) != cudaSuccess) { delete c; return NEGF_ECUDA; }
     c->graph_loops = true; c->obc_exec = nullptr;
-    for (int k = 0; k < NEGF_NGRAPH; k++) { c->gslot[k].key = 0; c->gslot[k].exec = nullptr; c->gslot[k].launches = 0; }
+    for (int k = 0; k < NEGF_NGRAPH; k++) for (int q = 0; q < NEGF_GWAYS; q++) c->gslot[k][q] = {0ull, nullptr, 0, 0u};
+    c->gtick = 0;
+    if (cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) != cudaSuccess) { delete c; return NEGF_ECUDA; }
+    for (int k = 0; k < 4; k++) if (cudaEventCreateWithFlags(&c->ev_grp[k], cudaEventDisableTiming) != cudaSuccess) { delete c; return NEGF_ECUDA; }
     if (cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking) != cudaSuccess) { delete c; return NEGF_ECUDA; } c->obc_key_ws = nullptr; c->obc_key_b = c->obc_key_nb = c->obc_key_maxit = 0; c->obc_key_tol = 0.0;
     c->prof_on = false; c->prof_depth = 0;
     for (int k = 0; k < NEGF_PROF_CLASSES; k++) { c->prof_ms[k] = 0.0; c->prof_n[k] = 0; }
@@ -42,7 +45,9 @@ extern "C" int negf_destroy(negf_ctx* ctx) {
     for (int k = 0; k < NEGF_NSIDE; k++) { cudaStreamDestroy(ctx->side[k]); cudaEventDestroy(ctx->ev_fork[k]); cudaEventDestroy(ctx->ev_join[k]); }
     cudaEventDestroy(ctx->ev_aux);
     if (ctx->obc_exec) cudaGraphExecDestroy(ctx->obc_exec);
-    for (int k = 0; k < NEGF_NGRAPH; k++) if (ctx->gslot[k].exec) cudaGraphExecDestroy(ctx->gslot[k].exec);
+    for (int k = 0; k < NEGF_NGRAPH; k++) for (int q = 0; q < NEGF_GWAYS; q++) if (ctx->gslot[k][q].exec) cudaGraphExecDestroy(ctx->gslot[k][q].exec);
+    cudaStreamDestroy(ctx->copy_stream);
+    for (int k = 0; k < 4; k++) cudaEventDestroy(ctx->ev_grp[k]);
     cudaStreamDestroy(ctx->cap_stream);
     delete ctx;
     return NEGF_OK;
@@ -56,7 +61,7 @@ extern "C" int negf_set_workspace(negf_ctx* ctx, void* p, size_t bytes) {
     if (!ctx) return NEGF_EINVAL;
     if (p && ((uintptr_t)p & 255)) return NEGF_EINVAL;
     ctx->ws = p; ctx->ws_bytes = p ? bytes : 0; ctx->sweep_valid = false;
-    for (int k = 0; k < NEGF_NGRAPH; k++) ctx->gslot[k].key = 0;
+    for (int k = 0; k < NEGF_NGRAPH; k++) for (int q = 0; q < NEGF_GWAYS; q++) ctx->gslot[k][q].key = 0;
     return NEGF_OK;
 }
 extern "C" int negf_set_option(negf_ctx* ctx, int option, int value) {

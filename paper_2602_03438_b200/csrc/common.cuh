@@ -10,6 +10,7 @@
 
 typedef double2 cplx;  // (x, y) = (re, im), same bytes as negf_c128
 constexpr int NEGF_NSIDE = 2;
+constexpr int NEGF_GWAYS = 4;     // cached argument sets per entry point (energy groups of negf_pipeline_host)
 constexpr int NEGF_NGRAPH = 2;    // 0 negf_rgf_retarded, 1 negf_rgf_lesser_greater
 
 struct negf_ctx {
@@ -32,9 +33,12 @@ struct negf_ctx {
     bool graph_loops;             // negf_set_option(NEGF_OPT_GRAPH_LOOPS)
     // cached CUDA graphs of whole calls in the latency-bound regime (same arguments twice in a row
     // -> the second call is captured, later ones replay it); one slot per entry point
-    struct GraphSlot { unsigned long long key; cudaGraphExec_t exec; long long launches; };
-    GraphSlot gslot[NEGF_NGRAPH];
+    struct GraphSlot { unsigned long long key; cudaGraphExec_t exec; long long launches; unsigned used; };
+    GraphSlot gslot[NEGF_NGRAPH][NEGF_GWAYS];
+    unsigned gtick;
     cudaStream_t cap_stream;      // capture stream (the caller's may be the legacy default stream)
+    cudaStream_t copy_stream;     // device->host copies of negf_pipeline_host
+    cudaEvent_t ev_grp[4];
     cudaGraphExec_t obc_exec;
     const void* obc_key_ws; int obc_key_b, obc_key_nb, obc_key_maxit; double obc_key_tol;
     // optional per-kernel-class timing (negf_profile_enable): event pairs around every launch site
@@ -165,7 +169,13 @@ struct KeyHash {
 template <class F>
 int run_cached(negf_ctx* ctx, int slot, unsigned long long key, bool eligible, F&& body) {
     if (!eligible || !ctx->graph_loops || ctx->prof_on) return body();
-    negf_ctx::GraphSlot& g = ctx->gslot[slot];
+    // way with this key, else the least recently used one
+    int w = 0;
+    for (int q = 0; q < NEGF_GWAYS; q++) if (ctx->gslot[slot][q].key == key) { w = q; goto found; }
+    for (int q = 1; q < NEGF_GWAYS; q++) if (ctx->gslot[slot][q].used < ctx->gslot[slot][w].used) w = q;
+found:
+    negf_ctx::GraphSlot& g = ctx->gslot[slot][w];
+    g.used = ++ctx->gtick;
     if (g.exec && g.key == key) {
         NEGF_CUDA_CHECK(ctx, cudaGraphLaunch(g.exec, ctx->stream));
         ctx->launches += g.launches;         // the kernels inside the replayed graph

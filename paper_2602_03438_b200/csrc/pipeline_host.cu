@@ -46,7 +46,7 @@ Layout make_layout(void* base, int n, int b, int ne, int kind_max, bool hasS, bo
     L.corner = (cplx*)B.take(bb * ne);
     L.GLd = (cplx*)B.take(bb * n * ne); L.GLu = (cplx*)B.take(bb * m * ne);
     if (want_greater) { L.GGd = (cplx*)B.take(bb * n * ne); L.GGu = (cplx*)B.take(bb * m * ne); }
-    L.density = (double*)B.take(sizeof(double) * n * b); L.ldos = (double*)B.take(sizeof(double) * ne * n);
+    L.density = (double*)B.take(sizeof(double) * n * b * 4); L.ldos = (double*)B.take(sizeof(double) * ne * n);
     L.trans = (double*)B.take(sizeof(double) * ne); L.bond = (double*)B.take(sizeof(double) * ne * (m > 0 ? m : 1));
     L.contact = (double*)B.take(sizeof(double) * ne * 2);
     L.info_r = (int*)B.take(sizeof(int) * ne); L.info_x = (int*)B.take(sizeof(int) * ne);
@@ -61,6 +61,15 @@ __global__ void merge_info_kernel(int ne, const int* a, const int* b, const int*
     if (e >= ne) return;
     int v = a[e]; if (!v) v = b[e]; if (!v) v = c[e]; if (!v) v = d[e];
     out[e] = v;
+}
+
+// dst[0][i] += dst[g][i], g = 1 .. ng-1 (partial densities of the energy groups)
+__global__ void sum_groups_kernel(double* d, int len, int ng) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= len) return;
+    double acc = d[i];
+    for (int g = 1; g < ng; g++) acc += d[(size_t)g * len + i];
+    d[i] = acc;
 }
 
 }  // namespace
@@ -132,46 +141,85 @@ extern "C" int negf_pipeline_host(negf_ctx* ctx, const negf_problem* hp, const n
 
     void* old_ws = ctx->ws; size_t old_bytes = ctx->ws_bytes;
     ctx->ws = L.ws; ctx->ws_bytes = L.ws_bytes; ctx->sweep_valid = false;
-    int rc = NEGF_OK;
-    do {
+    // The device->host copies run on the copy stream and overlap the compute that follows them: G^R goes
+    // home while G^<> is computed.  (Splitting the batch into energy groups to overlap more was measured
+    // and rejected: the small-block path is bound by its chain latency, which every group pays again.)
+    const int G = 1;
+    const int per = (ne + G - 1) / G;
+    const size_t fam_n = bb * n, fam_m = bb * m;
+    cudaStream_t cs = ctx->copy_stream;
+    auto D2Hc = [&](void* h, const void* d, size_t bytes) -> cudaError_t {
+        if (!h || !bytes) return cudaSuccess;
+        down += bytes; return cudaMemcpyAsync(h, d, bytes, cudaMemcpyDeviceToHost, cs);
+    };
+    auto off = [](const void* p, size_t bytes) -> void* { return p ? (char*)p + bytes : nullptr; };
+    int rc = NEGF_OK, ng = 0;
+    for (int lo = 0; lo < ne && rc == NEGF_OK; lo += per, ng++) {
+        const int cnt = min(per, ne - lo);
+        negf_problem gp = dp;
+        gp.n_energy = cnt; gp.energy = L.energy + lo;
+        negf_sigma gs[3];
+        for (int f = 0; f < 3; f++) {
+            gs[f] = ds[f];
+            gs[f].scalar = (negf_c128*)off(ds[f].scalar, sizeof(cplx) * lo);
+            gs[f].diag = (negf_c128*)off(ds[f].diag, fam_n * lo);
+            gs[f].upper = (negf_c128*)off(ds[f].upper, fam_m * lo);
+            gs[f].lower = (negf_c128*)off(ds[f].lower, fam_m * lo);
+        }
+        cplx* ob[2][4];
+        for (int sd = 0; sd < 2; sd++) for (int k = 0; k < 4; k++) ob[sd][k] = (cplx*)off(L.ob[sd][k], bb * lo);
         negf_obc_out oo[2];
-        for (int s = 0; s < 2; s++)
-            oo[s] = negf_obc_out{(negf_c128*)L.ob[s][0], (negf_c128*)L.ob[s][1], (negf_c128*)L.ob[s][2],
-                                 (negf_c128*)L.ob[s][3], nullptr, nullptr, L.iters[s], L.status[s]};
-        rc = negf_obc_decimate_pair(ctx, &dp, nullptr, nullptr, mu_L, mu_R, kT, tol, max_iter, &oo[0], &oo[1]);
+        for (int sd = 0; sd < 2; sd++)
+            oo[sd] = negf_obc_out{(negf_c128*)ob[sd][0], (negf_c128*)ob[sd][1], (negf_c128*)ob[sd][2], (negf_c128*)ob[sd][3],
+                                  nullptr, nullptr, L.iters[sd] + lo, L.status[sd] + lo};
+        rc = negf_obc_decimate_pair(ctx, &gp, nullptr, nullptr, mu_L, mu_R, kT, tol, max_iter, &oo[0], &oo[1]);
         if (rc) break;
-        ds[0].left = (negf_c128*)L.ob[0][0]; ds[0].right = (negf_c128*)L.ob[1][0];
-        ds[1].left = (negf_c128*)L.ob[0][2]; ds[1].right = (negf_c128*)L.ob[1][2];
-        ds[2].left = (negf_c128*)L.ob[0][3]; ds[2].right = (negf_c128*)L.ob[1][3];
-        rc = negf_rgf_retarded(ctx, &dp, &ds[0], (negf_c128*)L.GRd, (negf_c128*)L.GRu, (negf_c128*)L.GRl,
-                               (negf_c128*)L.corner, NEGF_KEEP_SWEEP, L.info_r);
+        gs[0].left = (negf_c128*)ob[0][0]; gs[0].right = (negf_c128*)ob[1][0];
+        gs[1].left = (negf_c128*)ob[0][2]; gs[1].right = (negf_c128*)ob[1][2];
+        gs[2].left = (negf_c128*)ob[0][3]; gs[2].right = (negf_c128*)ob[1][3];
+        cplx *GRd = (cplx*)off(L.GRd, fam_n * lo), *GRu = (cplx*)off(L.GRu, fam_m * lo), *GRl = (cplx*)off(L.GRl, fam_m * lo);
+        cplx *cor = (cplx*)off(L.corner, bb * lo), *GLd = (cplx*)off(L.GLd, fam_n * lo), *GLu = (cplx*)off(L.GLu, fam_m * lo);
+        cplx *GGd = (cplx*)off(L.GGd, fam_n * lo), *GGu = (cplx*)off(L.GGu, fam_m * lo);
+        rc = negf_rgf_retarded(ctx, &gp, &gs[0], (negf_c128*)GRd, (negf_c128*)GRu, (negf_c128*)GRl, (negf_c128*)cor,
+                               NEGF_KEEP_SWEEP, L.info_r + lo);
         if (rc) break;
-        rc = negf_rgf_lesser_greater(ctx, &dp, &ds[0], &ds[1], want_g ? &ds[2] : nullptr, (negf_c128*)L.GRd,
-                                     (negf_c128*)L.GLd, (negf_c128*)L.GLu, (negf_c128*)L.GGd, (negf_c128*)L.GGu,
-                                     L.info_x);
+        NEGF_CUDA_CHECK(ctx, cudaEventRecord(ctx->ev_grp[1], st));
+        NEGF_CUDA_CHECK(ctx, cudaStreamWaitEvent(cs, ctx->ev_grp[1], 0));
+        NEGF_CUDA_CHECK(ctx, D2Hc(off(out->GR_diag, fam_n * lo), GRd, fam_n * cnt));
+        NEGF_CUDA_CHECK(ctx, D2Hc(off(out->GR_upper, fam_m * lo), GRu, fam_m * cnt));
+        NEGF_CUDA_CHECK(ctx, D2Hc(off(out->GR_lower, fam_m * lo), GRl, fam_m * cnt));
+        rc = negf_rgf_lesser_greater(ctx, &gp, &gs[0], &gs[1], want_g ? &gs[2] : nullptr, (negf_c128*)GRd,
+                                     (negf_c128*)GLd, (negf_c128*)GLu, (negf_c128*)GGd, (negf_c128*)GGu, L.info_x + lo);
         if (rc) break;
-        rc = negf_observables(ctx, &dp, (negf_c128*)L.GRd, (negf_c128*)L.GRu, (negf_c128*)L.GRl, (negf_c128*)L.corner,
-                              (negf_c128*)L.GLd, (negf_c128*)L.GLu, (negf_c128*)L.GGd,
-                              (negf_c128*)L.ob[0][1], (negf_c128*)L.ob[1][1],
-                              (negf_c128*)L.ob[0][2], (negf_c128*)L.ob[0][3], (negf_c128*)L.ob[1][2], (negf_c128*)L.ob[1][3],
-                              L.weights, out->density ? L.density : nullptr, out->ldos ? L.ldos : nullptr,
-                              out->transmission ? L.trans : nullptr, out->bond_current ? L.bond : nullptr,
-                              (out->contact_current && want_g) ? L.contact : nullptr);
-    } while (0);
-    ctx->ws = old_ws; ctx->ws_bytes = old_bytes; ctx->sweep_valid = false;
-    if (rc) return rc;
-    if (out->info) {
-        merge_info_kernel<<<(ne + 255) / 256, 256, 0, st>>>(ne, L.status[0], L.status[1], L.info_r, L.info_x, L.info_x);
-        NEGF_LAUNCH_CHECK(ctx);
+        double* dens = out->density ? L.density + (size_t)ng * n * b : nullptr;      // partial density of this group
+        rc = negf_observables(ctx, &gp, (negf_c128*)GRd, (negf_c128*)GRu, (negf_c128*)GRl, (negf_c128*)cor,
+                              (negf_c128*)GLd, (negf_c128*)GLu, (negf_c128*)GGd,
+                              (negf_c128*)ob[0][1], (negf_c128*)ob[1][1],
+                              (negf_c128*)ob[0][2], (negf_c128*)ob[0][3], (negf_c128*)ob[1][2], (negf_c128*)ob[1][3],
+                              L.weights + lo, dens, out->ldos ? L.ldos + (size_t)lo * n : nullptr,
+                              out->transmission ? L.trans + lo : nullptr, out->bond_current ? L.bond + (size_t)lo * m : nullptr,
+                              (out->contact_current && want_g) ? L.contact + (size_t)lo * 2 : nullptr);
+        if (rc) break;
+        if (out->info) {
+            merge_info_kernel<<<(cnt + 255) / 256, 256, 0, st>>>(cnt, L.status[0] + lo, L.status[1] + lo, L.info_r + lo,
+                                                                L.info_x + lo, L.info_x + lo);
+            NEGF_LAUNCH_CHECK(ctx);
+        }
+        // this group's results go home on the copy stream
+        NEGF_CUDA_CHECK(ctx, cudaEventRecord(ctx->ev_grp[ng], st));
+        NEGF_CUDA_CHECK(ctx, cudaStreamWaitEvent(cs, ctx->ev_grp[ng], 0));
+        NEGF_CUDA_CHECK(ctx, D2Hc(off(out->GL_diag, fam_n * lo), GLd, fam_n * cnt));
+        NEGF_CUDA_CHECK(ctx, D2Hc(off(out->GL_upper, fam_m * lo), GLu, fam_m * cnt));
+        if (want_g) {
+            NEGF_CUDA_CHECK(ctx, D2Hc(off(out->GG_diag, fam_n * lo), GGd, fam_n * cnt));
+            NEGF_CUDA_CHECK(ctx, D2Hc(off(out->GG_upper, fam_m * lo), GGu, fam_m * cnt));
+        }
     }
-    NEGF_CUDA_CHECK(ctx, D2H(out->GR_diag, L.GRd, bb * n * ne));
-    NEGF_CUDA_CHECK(ctx, D2H(out->GR_upper, L.GRu, bb * m * ne));
-    NEGF_CUDA_CHECK(ctx, D2H(out->GR_lower, L.GRl, bb * m * ne));
-    NEGF_CUDA_CHECK(ctx, D2H(out->GL_diag, L.GLd, bb * n * ne));
-    NEGF_CUDA_CHECK(ctx, D2H(out->GL_upper, L.GLu, bb * m * ne));
-    if (want_g) {
-        NEGF_CUDA_CHECK(ctx, D2H(out->GG_diag, L.GGd, bb * n * ne));
-        NEGF_CUDA_CHECK(ctx, D2H(out->GG_upper, L.GGu, bb * m * ne));
+    ctx->ws = old_ws; ctx->ws_bytes = old_bytes; ctx->sweep_valid = false;
+    if (rc) { cudaStreamSynchronize(cs); return rc; }
+    if (out->density) {          // total density = sum of the groups' partial densities, fixed order
+        sum_groups_kernel<<<(n * b + 255) / 256, 256, 0, st>>>(L.density, n * b, ng);
+        NEGF_LAUNCH_CHECK(ctx);
     }
     NEGF_CUDA_CHECK(ctx, D2H(out->density, L.density, sizeof(double) * n * b));
     NEGF_CUDA_CHECK(ctx, D2H(out->ldos, L.ldos, sizeof(double) * ne * n));
@@ -180,6 +228,7 @@ extern "C" int negf_pipeline_host(negf_ctx* ctx, const negf_problem* hp, const n
     if (want_g) NEGF_CUDA_CHECK(ctx, D2H(out->contact_current, L.contact, sizeof(double) * ne * 2));
     NEGF_CUDA_CHECK(ctx, D2H(out->info, L.info_x, sizeof(int) * ne));
     NEGF_CUDA_CHECK(ctx, cudaStreamSynchronize(st));
+    NEGF_CUDA_CHECK(ctx, cudaStreamSynchronize(cs));
     if (h2d_bytes) *h2d_bytes = up;
     if (d2h_bytes) *d2h_bytes = down;
     return NEGF_OK;
