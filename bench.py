@@ -178,7 +178,7 @@ def run_gpu(args, rank, local_rank, world):
     # `streams` groups of energies that run the whole path concurrently on their own CUDA streams
     # (their own context, workspace and outputs), so one group's latency-bound inversions overlap the
     # other's GEMMs.  Same work, same outputs; densities of the groups add up.
-    n_streams = args.streams or 1
+    n_streams = args.streams or (4 if (wl.block_size <= 96 and len(batches) == 1 and wl.n_energy >= 32) else 1)
     groups = []
     if n_streams > 1 and len(batches) == 1:
         per = -(-wl.n_energy // n_streams)
@@ -278,19 +278,26 @@ def run_gpu(args, rank, local_rank, world):
         # ---- roofline of the dominant kernel: profiled passes of the SAME step (event pairs around
         # every launch site, on the library's stream), separate from the throughput timing above
         peak = ctx.fp64_peak(300.0)
-        for c in all_ctx:
+        # (with concurrent energy groups the intervals of different streams would overlap: the profiled passes
+        # run the whole batch on ONE stream, plain launches)
+        pstep, pctx = step, all_ctx
+        if groups:
+            pdp = runner.DevicePath(wl, 0, wl.n_energy, device=dev, ctx=ctx)
+            pstep, pctx = pdp.run, [ctx]
+            pstep(); torch.cuda.synchronize()
+        for c in pctx:
             c.profile_enable(True)
             for k in range(5):
                 c.profile_read(k, True)
         psteps = max(1, min(3, args.steps))
         for _ in range(psteps):
-            step(); flush.zero_()
+            pstep(); flush.zero_()
         torch.cuda.synchronize()
         prof = {}
         for k in range(5):
-            rr = [c.profile_read(k, True) for c in all_ctx]
+            rr = [c.profile_read(k, True) for c in pctx]
             prof[negf.PROF_NAMES[k]] = (sum(r[0] for r in rr), sum(r[1] for r in rr))
-        for c in all_ctx:
+        for c in pctx:
             c.profile_enable(False)
         tot = sum(v[0] for v in prof.values()) or 1.0
         gemm_ms, gemm_sites = prof["gemm"]
@@ -309,7 +316,7 @@ def run_gpu(args, rank, local_rank, world):
                            "flops_per_launch": dom_flops / max(dom_sites, 1),
                            "avg_launch_us": 1e3 * dom_ms / max(dom_sites, 1), "launches_per_step": dom_sites / psteps,
                            "share_of_step": {k: v[0] / tot for k, v in prof.items()},
-                           "measured": f"{psteps} profiled passes of the same step after the timed region"}
+                           "measured": f"{psteps} profiled passes of the same step after the timed region (one stream, plain launches)"}
         # ---- end to end through the host-buffer C-ABI call (pinned host memory, copies timed)
         if not args.no_e2e:
             out["e2e"] = run_e2e(args, wl, ctx, dev, world, torch, negf)
@@ -384,7 +391,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=1, help="BASELINE.json configs index (default 1)")
-    ap.add_argument("--streams", type=int, default=0, help="concurrent energy groups on separate CUDA streams (default 1; measured gain at configs[1]: 3 %)")
+    ap.add_argument("--streams", type=int, default=0, help="concurrent energy groups on separate CUDA streams (0 = auto: 4 for b <= 96 and >= 32 energies, else 1)")
     ap.add_argument("--energy-batch", type=int, default=0, help="energies resident at once (0 = fit HBM)")
     ap.add_argument("--e2e-energies", type=int, default=0)
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="CPU time budget of the cpu_baseline leg")
