@@ -116,12 +116,14 @@ int negf_last_cuda_error(const negf_ctx* ctx);
 /* Number of kernels this context has launched since creation (bench.py's gpu_launches). */
 long long negf_launch_count(const negf_ctx* ctx);
 
-/* Per-kernel-class device timing for bench.py's roofline: when enabled, every launch site is
- * bracketed by a CUDA event pair on the context stream (no synchronisation; a few microseconds of
- * host overhead per launch, so never enable it inside a timed throughput run).
- * negf_profile_read SYNCHRONISES the stream, folds all finished pairs into the per-class totals
- * and returns milliseconds and number of launch sites of `kclass` since the last reset; reset != 0
- * clears the totals of that class afterwards.  ms / sites may be NULL. */
+/* Per-kernel-class device timing for bench.py's roofline: when enabled, one CUDA event is recorded on
+ * the context stream whenever the kernel class of the next launch differs from the previous one, so the
+ * consecutive launches of a class form one timed interval; the side streams and the call graphs are not
+ * used while profiling (every kernel runs on the caller's stream, plain launches), so intervals never
+ * overlap.  Never enable it inside a timed throughput run.
+ * negf_profile_read SYNCHRONISES the stream, folds all finished intervals into the per-class totals and
+ * returns milliseconds and number of kernel launches of `kclass` since the last reset; reset != 0 clears the
+ * totals of that class afterwards.  ms / sites may be NULL. */
 #define NEGF_PROF_GEMM        0   /* K2 complex GEMM (DMMA)                                        */
 #define NEGF_PROF_INVERSE     1   /* K1 inverse (all its kernels, inner GEMMs included)             */
 #define NEGF_PROF_ELEMENTWISE 2   /* O(b^2) assembly / combination kernels                          */

@@ -32,7 +32,7 @@ extern "C" int negf_create(negf_ctx** out, int device) {
     if (cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) != cudaSuccess) { delete c; return NEGF_ECUDA; }
     for (int k = 0; k < 4; k++) if (cudaEventCreateWithFlags(&c->ev_grp[k], cudaEventDisableTiming) != cudaSuccess) { delete c; return NEGF_ECUDA; }
     if (cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking) != cudaSuccess) { delete c; return NEGF_ECUDA; } c->obc_key_ws = nullptr; c->obc_key_b = c->obc_key_nb = c->obc_key_maxit = 0; c->obc_key_tol = 0.0;
-    c->prof_on = false; c->prof_depth = 0;
+    c->prof_on = false; c->prof_depth = 0; c->prof_last_class = -1; c->prof_last_event = nullptr;
     for (int k = 0; k < NEGF_PROF_CLASSES; k++) { c->prof_ms[k] = 0.0; c->prof_n[k] = 0; }
     if (zgemm_prepare(c) != NEGF_OK) { delete c; return NEGF_ECUDA; }
     *out = c;
@@ -40,8 +40,8 @@ extern "C" int negf_create(negf_ctx** out, int device) {
 }
 extern "C" int negf_destroy(negf_ctx* ctx) {
     if (!ctx) return NEGF_EINVAL;
-    for (auto& r : ctx->prof_recs) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
-    for (auto e : ctx->prof_pool) cudaEventDestroy(e);
+    for (auto& r : ctx->prof_recs) cudaEventDestroy(r.e0);
+    if (ctx->prof_last_event) cudaEventDestroy(ctx->prof_last_event);
     for (int k = 0; k < NEGF_NSIDE; k++) { cudaStreamDestroy(ctx->side[k]); cudaEventDestroy(ctx->ev_fork[k]); cudaEventDestroy(ctx->ev_join[k]); }
     cudaEventDestroy(ctx->ev_aux);
     if (ctx->obc_exec) cudaGraphExecDestroy(ctx->obc_exec);
@@ -83,21 +83,38 @@ extern "C" const char* negf_strerror(int code) {
 extern "C" int negf_last_cuda_error(const negf_ctx* ctx) { return ctx ? ctx->last_cuda_error : 0; }
 extern "C" long long negf_launch_count(const negf_ctx* ctx) { return ctx ? ctx->launches : 0; }
 
+namespace {
+// closes the open interval and folds every finished interval into the per-class totals (synchronises)
+int profile_fold(negf_ctx* ctx) {
+    if (ctx->prof_last_class >= 0) {
+        cudaEvent_t e;
+        NEGF_CUDA_CHECK(ctx, cudaEventCreate(&e));
+        NEGF_CUDA_CHECK(ctx, cudaEventRecord(e, ctx->stream));
+        ctx->prof_recs.push_back({ctx->prof_last_class, ctx->prof_last_event, e});
+        ctx->prof_last_class = -1; ctx->prof_last_event = e;      // e is destroyed below as the chain's tail
+    }
+    NEGF_CUDA_CHECK(ctx, cudaStreamSynchronize(ctx->stream));
+    for (auto& r : ctx->prof_recs) {
+        float t = 0.f;
+        NEGF_CUDA_CHECK(ctx, cudaEventElapsedTime(&t, r.e0, r.e1));
+        ctx->prof_ms[r.kclass] += t;
+    }
+    for (auto& r : ctx->prof_recs) cudaEventDestroy(r.e0);
+    ctx->prof_recs.clear();
+    if (ctx->prof_last_event) { cudaEventDestroy(ctx->prof_last_event); ctx->prof_last_event = nullptr; }
+    return NEGF_OK;
+}
+}  // namespace
+
 extern "C" int negf_profile_enable(negf_ctx* ctx, int on) {
     if (!ctx) return NEGF_EINVAL;
+    if (ctx->prof_on && !on) NEGF_TRY(profile_fold(ctx));
     ctx->prof_on = on != 0; ctx->prof_depth = 0;
     return NEGF_OK;
 }
 extern "C" int negf_profile_read(negf_ctx* ctx, int kclass, double* ms, long long* sites, int reset) {
     if (!ctx || kclass < 0 || kclass >= NEGF_PROF_CLASSES) return NEGF_EINVAL;
-    NEGF_CUDA_CHECK(ctx, cudaStreamSynchronize(ctx->stream));
-    for (auto& r : ctx->prof_recs) {
-        float t = 0.f;
-        NEGF_CUDA_CHECK(ctx, cudaEventElapsedTime(&t, r.e0, r.e1));
-        ctx->prof_ms[r.kclass] += t; ctx->prof_n[r.kclass]++;
-        ctx->prof_pool.push_back(r.e0); ctx->prof_pool.push_back(r.e1);
-    }
-    ctx->prof_recs.clear();
+    NEGF_TRY(profile_fold(ctx));
     if (ms) *ms = ctx->prof_ms[kclass];
     if (sites) *sites = ctx->prof_n[kclass];
     if (reset) { ctx->prof_ms[kclass] = 0.0; ctx->prof_n[kclass] = 0; }

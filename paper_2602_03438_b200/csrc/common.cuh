@@ -45,31 +45,30 @@ struct negf_ctx {
     bool prof_on;
     int prof_depth;
     struct ProfRec { int kclass; cudaEvent_t e0, e1; };
-    std::vector<ProfRec> prof_recs;
-    std::vector<cudaEvent_t> prof_pool;
+    std::vector<ProfRec> prof_recs;     // e1 of a record is e0 of the next one
+    int prof_last_class; cudaEvent_t prof_last_event;
     double prof_ms[NEGF_PROF_CLASSES];
     long long prof_n[NEGF_PROF_CLASSES];
 };
 
-// Brackets one launch site with CUDA events on the context stream when profiling is on; nested
-// scopes (the GEMMs inside the blocked inverse) are charged to the outermost class only.
+// Per-class device time when profiling is on: ONE event is recorded on the stream whenever the kernel
+// class of the next launch site differs from the previous one, so consecutive launches of a class form
+// one interval (two event records per launch would cost more than the small kernels they bracket).
+// Nested scopes (the GEMMs inside the blocked inverse) are charged to the outermost class.  While
+// profiling, the side streams are not used (StreamFork), so the intervals never overlap.
 struct ProfScope {
-    negf_ctx* c; int k; cudaEvent_t e0, e1; bool live;
-    static cudaEvent_t get(negf_ctx* c) {
-        cudaEvent_t e;
-        if (!c->prof_pool.empty()) { e = c->prof_pool.back(); c->prof_pool.pop_back(); }
-        else cudaEventCreate(&e);
-        return e;
-    }
-    ProfScope(negf_ctx* ctx, int kclass) : c(ctx), k(kclass), live(false) {
+    negf_ctx* c;
+    ProfScope(negf_ctx* ctx, int kclass) : c(ctx) {
         if (!c->prof_on) return;
-        if (c->prof_depth++ == 0) { live = true; e0 = get(c); e1 = get(c); cudaEventRecord(e0, c->stream); }
+        if (c->prof_depth++ == 0 && kclass != c->prof_last_class) {
+            cudaEvent_t e;
+            cudaEventCreate(&e);
+            cudaEventRecord(e, c->stream);
+            if (c->prof_last_class >= 0) c->prof_recs.push_back({c->prof_last_class, c->prof_last_event, e});
+            c->prof_last_class = kclass; c->prof_last_event = e;
+        }
     }
-    ~ProfScope() {
-        if (!c->prof_on) return;
-        c->prof_depth--;
-        if (live) { cudaEventRecord(e1, c->stream); c->prof_recs.push_back({k, e0, e1}); }
-    }
+    ~ProfScope() { if (c->prof_on) c->prof_depth--; }
 };
 
 #define NEGF_CUDA_CHECK(ctx, expr)                                  \
@@ -81,9 +80,15 @@ struct ProfScope {
         }                                                           \
     } while (0)
 
-#define NEGF_LAUNCH_CHECK(ctx)                                      \
+#define NEGF_COUNT_LAUNCH(ctx)                                      \
     do {                                                            \
         (ctx)->launches++;                                          \
+        if ((ctx)->prof_on && (ctx)->prof_last_class >= 0) (ctx)->prof_n[(ctx)->prof_last_class]++; \
+    } while (0)
+
+#define NEGF_LAUNCH_CHECK(ctx)                                      \
+    do {                                                            \
+        NEGF_COUNT_LAUNCH(ctx);                                     \
         cudaError_t _e = cudaGetLastError();                        \
         if (_e != cudaSuccess) {                                    \
             (ctx)->last_cuda_error = (int)_e;                       \
@@ -136,19 +141,22 @@ struct StreamFork {
     explicit StreamFork(negf_ctx* ctx) : c(ctx), main(ctx->stream) {}
     ~StreamFork() { c->stream = main; }
     void use_main() { c->stream = main; }
-    void use_side(int k) { c->stream = c->side[k]; }
+    void use_side(int k) { if (!c->prof_on) c->stream = c->side[k]; }
     // side k starts after everything enqueued on `from` so far (default: main)
     cudaError_t fork(int k) {
+        if (c->prof_on) return cudaSuccess;
         cudaError_t e = cudaEventRecord(c->ev_fork[k], main);
         return e != cudaSuccess ? e : cudaStreamWaitEvent(c->side[k], c->ev_fork[k], 0);
     }
     // main continues after everything enqueued on side k so far
     cudaError_t join(int k) {
+        if (c->prof_on) return cudaSuccess;
         cudaError_t e = cudaEventRecord(c->ev_join[k], c->side[k]);
         return e != cudaSuccess ? e : cudaStreamWaitEvent(main, c->ev_join[k], 0);
     }
     // side k waits for everything enqueued on main so far (mid-call dependency)
     cudaError_t side_waits_main(int k) {
+        if (c->prof_on) return cudaSuccess;
         cudaError_t e = cudaEventRecord(c->ev_aux, main);
         return e != cudaSuccess ? e : cudaStreamWaitEvent(c->side[k], c->ev_aux, 0);
     }

@@ -779,7 +779,7 @@ int zinv_launch(negf_ctx* ctx, int b, cplx* A, long long sA, int batch, void* ws
             at[0].val.clusterDim.x = C;
             if (R == 8) NEGF_CUDA_CHECK(ctx, cudaLaunchKernelEx(&cfg, gj_panel_reg_kernel<8>, pa));
             else        NEGF_CUDA_CHECK(ctx, cudaLaunchKernelEx(&cfg, gj_panel_reg_kernel<16>, pa));
-            ctx->launches++;
+            NEGF_COUNT_LAUNCH(ctx);
             if (nbk > wk) {
                 gj_swap_extract_kernel<<<dim3((nbk + 127) / 128, batch), 128, 0, ctx->stream>>>(
                     A, sA, b, k0, wk, K0, K1, k0, k0 + wk, W.ipiv, W.R, skip);
@@ -818,7 +818,7 @@ int zinv_launch(negf_ctx* ctx, int b, cplx* A, long long sA, int batch, void* ws
         cfg.dynamicSmemBytes = (size_t)slab * wk * sizeof(cplx) + fixed;
         at[0].val.clusterDim.x = C;
         NEGF_CUDA_CHECK(ctx, cudaLaunchKernelEx(&cfg, gj_panel_cluster_kernel, pa));
-        ctx->launches++;
+        NEGF_COUNT_LAUNCH(ctx);
         // row swaps on the other columns of K + pivot rows -> R, zeroed in A
         if (nbk > wk) {
             gj_swap_extract_kernel<<<dim3((nbk + 127) / 128, batch), 128, 0, ctx->stream>>>(
