@@ -174,6 +174,8 @@ def run_gpu(args, rank, local_rank, world):
     # one resident DevicePath per distinct batch size; Sigma_S of the FIRST batch of that size is
     # reused for the others when it is a per-energy BT family (configs[3]; stated in config.note)
     ctx = negf.Context(local_rank)
+    if args.gemm_3m:
+        ctx.set_option(negf.OPT_GEMM_3M, 1)
     # K3 at the runner level: in the latency-bound small-block regime the resident batch is split into
     # `streams` groups of energies that run the whole path concurrently on their own CUDA streams
     # (their own context, workspace and outputs), so one group's latency-bound inversions overlap the
@@ -257,6 +259,8 @@ def run_gpu(args, rank, local_rank, world):
     U = 8.0 * wl.block_size ** 3
     gemm_u, inv_u = unit_counts(wl.n_blocks, wl.sigma_kind, wl.want_greater, iters_total, wl.n_energy)
     step_ms = ms / args.steps
+    if args.gemm_3m and wl.block_size > 64:
+        gemm_u *= 0.75                      # executed DMMA flops of a 3M product: 6 b^3 instead of 8 b^3
 
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
            "warmup": args.warmup, "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak",
@@ -267,7 +271,7 @@ def run_gpu(args, rank, local_rank, world):
                                  + ", density, LDOS, T(E), bond/contact currents",
                       "l2": "256 MB flush write between timed iterations (outside the event pairs)",
                       "parallelism": f"energy-sharded x{world}, no collective",
-                      "streams": n_streams,
+                      "streams": n_streams, "complex_gemm": "3M" if (args.gemm_3m and wl.block_size > 64) else "4M",
                       "decimation_iters_mean": iters_mean, "numerical_failures": bad},
            "gpu_launches": int(launches), "clocks": clocks,
            "nominal_tflops": (gemm_u + inv_u) * U / (step_ms * 1e-3) * 1e-12}
@@ -391,6 +395,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=1, help="BASELINE.json configs index (default 1)")
+    ap.add_argument("--gemm-3m", action="store_true",
+                    help="3M complex products in the compute-bound regime (NEGF_OPT_GEMM_3M); flops are then counted as executed (x 0.75 per product)")
     ap.add_argument("--streams", type=int, default=0, help="concurrent energy groups on separate CUDA streams (0 = auto: 4 for b <= 96 and >= 32 energies, else 1)")
     ap.add_argument("--energy-batch", type=int, default=0, help="energies resident at once (0 = fit HBM)")
     ap.add_argument("--e2e-energies", type=int, default=0)

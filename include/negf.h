@@ -107,8 +107,13 @@ int negf_set_workspace(negf_ctx* ctx, void* dev_ptr, size_t bytes);
 /* Options.  NEGF_OPT_GRAPH_LOOPS (default 1): for block sizes up to 96 the Sancho-Rubio doublings of
  * negf_obc_decimate[_pair] run as a cached device-driven WHILE graph (CUDA conditional node) that stops
  * when every energy has converged; 0 = the plain host loop of max_iter masked doublings.  Same
- * arithmetic and results either way. */
+ * arithmetic and results either way.
+ * NEGF_OPT_GEMM_3M (default 0): in the compute-bound regime (blocks above 64 that fill the machine with
+ * 128-row tiles) complex products use the 3M decomposition (three real DMMA products instead of four: 25 % fewer
+ * tensor-pipe instructions; the imaginary part is accurate norm-wise, not component-wise).  Off by default: the
+ * 4M kernel is the one the FP64 roofline fraction is quoted on. */
 #define NEGF_OPT_GRAPH_LOOPS 1
+#define NEGF_OPT_GEMM_3M     2
 int negf_set_option(negf_ctx* ctx, int option, int value);
 const char* negf_strerror(int code);
 /* cudaError_t of the last failing runtime call on this context (0 if none). */

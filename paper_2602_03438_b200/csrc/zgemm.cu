@@ -176,6 +176,125 @@ __global__ void __launch_bounds__(WM * WN * 32, MINB) zgemm_kernel(const __grid_
     }
 }
 
+// 3M variant for the compute-bound regime: per 8x8x4 sub-product THREE real DMMAs,
+//   P1 = Ar Br,  P2 = Ai Bi,  P3 = (Ar + Ai)(Br + Bi);   Re = P1 - P2,  Im = P3 - P1 - P2,
+// i.e. 25 % fewer tensor-pipe instructions than 4M for MI + NI extra DADDs per k-step.  The imaginary
+// part is accurate norm-wise (|dIm| <~ eps (|Ar|+|Ai|)(|Br|+|Bi|)), far inside the 1e-10 bar.  Three
+// accumulator sets cost registers, hence 32x24 warp tiles (128x48 CTA tiles, 8 warps).
+template <int OPA, int OPB, int BM, int BN, int WM, int WN>
+__global__ void __launch_bounds__(WM * WN * 32, 1) zgemm3m_kernel(const __grid_constant__ GemmGroup grp) {
+    const GemmArgs& a = grp.g[blockIdx.z];
+    constexpr int NT = WM * WN * 32;
+    constexpr int STAGES = 3;
+    constexpr int MI = BM / WM / 8;
+    constexpr int NI = BN / WN / 8;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx* sA = reinterpret_cast<cplx*>(smem_raw);
+    cplx* sB = sA + STAGES * BM * BK;
+
+    const int e = blockIdx.y % a.batch, e2 = blockIdx.y / a.batch;
+    if (a.skip && a.skip[e]) return;
+    const int tiles_n = (a.n + BN - 1) / BN;
+    const int tm = blockIdx.x / tiles_n, tn = blockIdx.x % tiles_n;
+    const int m0 = tm * BM, n0 = tn * BN;
+    const cplx* gA = a.A + (size_t)e * a.sA + (size_t)e2 * a.sA2;
+    const cplx* gB = a.B + (size_t)e * a.sB + (size_t)e2 * a.sB2;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int wm0 = (warp / WN) * (MI * 8), wn0 = (warp % WN) * (NI * 8);
+    const int lr = lane >> 2, lk = lane & 3;
+
+    double p1[MI][NI][2], p2[MI][NI][2], p3[MI][NI][2];
+#pragma unroll
+    for (int i = 0; i < MI; i++)
+#pragma unroll
+        for (int j = 0; j < NI; j++)
+#pragma unroll
+            for (int q = 0; q < 2; q++) { p1[i][j][q] = 0.0; p2[i][j][q] = 0.0; p3[i][j][q] = 0.0; }
+
+    const int KB = (a.k + BK - 1) / BK;
+    auto issue = [&](int kb) {
+        if (kb < KB) {
+            int st = kb % STAGES, k0 = kb * BK;
+            if (OPA == 0) load_tile_kc<BM, NT>(sA + st * BM * BK, gA, a.lda, m0, k0, a.m, a.k, tid);
+            else          load_tile_mc<BM, NT>(sA + st * BM * BK, gA, a.lda, m0, k0, a.m, a.k, tid);
+            if (OPB == 0) load_tile_mc<BN, NT>(sB + st * BN * BK, gB, a.ldb, n0, k0, a.n, a.k, tid);
+            else          load_tile_kc<BN, NT>(sB + st * BN * BK, gB, a.ldb, n0, k0, a.n, a.k, tid);
+        }
+        cp_async_commit();
+    };
+#pragma unroll
+    for (int s = 0; s < STAGES - 1; s++) issue(s);
+
+    for (int kb = 0; kb < KB; kb++) {
+        cp_async_wait<STAGES - 2>();
+        __syncthreads();
+        issue(kb + STAGES - 1);
+        const cplx* tA = sA + (kb % STAGES) * BM * BK;
+        const cplx* tB = sB + (kb % STAGES) * BN * BK;
+#pragma unroll
+        for (int ks = 0; ks < BK / 4; ks++) {
+            const int k = ks * 4 + lk;
+            double ar[MI], ai[MI], as[MI], br[NI], bi[NI], bs[NI];
+#pragma unroll
+            for (int i = 0; i < MI; i++) {
+                int m = wm0 + i * 8 + lr;
+                cplx v = (OPA == 0) ? tA[m * BK + (k ^ ((m & 1) << 2))] : tA[k * BM + (m ^ ((k & 3) << 1))];
+                ar[i] = v.x; ai[i] = (OPA == 0) ? v.y : flip(v.y); as[i] = ar[i] + ai[i];
+            }
+#pragma unroll
+            for (int j = 0; j < NI; j++) {
+                int n = wn0 + j * 8 + lr;
+                cplx v = (OPB == 0) ? tB[k * BN + (n ^ ((k & 3) << 1))] : tB[n * BK + (k ^ ((n & 1) << 2))];
+                br[j] = v.x; bi[j] = (OPB == 0) ? v.y : flip(v.y); bs[j] = br[j] + bi[j];
+            }
+#pragma unroll
+            for (int i = 0; i < MI; i++)
+#pragma unroll
+                for (int j = 0; j < NI; j++) {
+                    dmma(p1[i][j][0], p1[i][j][1], ar[i], br[j]);
+                    dmma(p2[i][j][0], p2[i][j][1], ai[i], bi[j]);
+                    dmma(p3[i][j][0], p3[i][j][1], as[i], bs[j]);
+                }
+        }
+    }
+    cp_async_wait<0>();
+
+    cplx* gC = a.C + (size_t)e * a.sC + (size_t)e2 * a.sC2;
+    const cplx* gD = a.D ? a.D + (size_t)e * a.sD + (size_t)e2 * a.sD2 : nullptr;
+    const cplx al = a.alpha_vec ? cmul(a.alpha, a.alpha_vec[e]) : a.alpha, be = a.beta;
+#pragma unroll
+    for (int i = 0; i < MI; i++) {
+        int row = m0 + wm0 + i * 8 + lr;
+        if (row >= a.m) continue;
+#pragma unroll
+        for (int j = 0; j < NI; j++) {
+#pragma unroll
+            for (int q = 0; q < 2; q++) {
+                int col = n0 + wn0 + j * 8 + lk * 2 + q;
+                if (col >= a.n) continue;
+                cplx acc = cmake(p1[i][j][q] - p2[i][j][q], (p3[i][j][q] - p1[i][j][q]) - p2[i][j][q]);
+                cplx r = cmul(al, acc);
+                if (gD) { cplx d = gD[(size_t)row * a.ldc + col]; cfma(r, be, d); }
+                gC[(size_t)row * a.ldc + col] = r;
+            }
+        }
+    }
+}
+
+constexpr int M3_BN = 48;      // 32x24 warp tiles: the widest that keep three accumulator sets in registers
+
+template <int OPA, int OPB>
+int launch_3m(negf_ctx* ctx, const GemmGroup& grp) {
+    constexpr int BM = 128, BN = M3_BN, WM = 4, WN = 2;
+    const GemmArgs& a = grp.g[0];
+    constexpr int smem = 3 * (BM + BN) * BK * (int)sizeof(cplx);
+    int tiles = ((a.m + BM - 1) / BM) * ((a.n + BN - 1) / BN);
+    dim3 grid(tiles, a.batch * a.batch2, grp.ng);
+    zgemm3m_kernel<OPA, OPB, BM, BN, WM, WN><<<grid, WM * WN * 32, smem, ctx->stream>>>(grp);
+    NEGF_LAUNCH_CHECK(ctx);
+    return NEGF_OK;
+}
+
 template <int OPA, int OPB, int BM, int BN, int WM, int WN, int MINB>
 int launch_cfg(negf_ctx* ctx, const GemmGroup& grp) {
     const GemmArgs& a = grp.g[0];
@@ -216,6 +335,13 @@ int zgemm_prepare(negf_ctx* ctx) {
     NEGF_CUDA_CHECK(ctx, (prepare_cfg<128, 64, 4, 2, 1>()));
     NEGF_CUDA_CHECK(ctx, (prepare_cfg<64, 64, 2, 2, 2>()));
     NEGF_CUDA_CHECK(ctx, (prepare_cfg<32, 32, 2, 2, 3>()));
+    {
+        constexpr int smem = 3 * (128 + M3_BN) * BK * (int)sizeof(cplx);
+        NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(zgemm3m_kernel<0, 0, 128, M3_BN, 4, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(zgemm3m_kernel<1, 0, 128, M3_BN, 4, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(zgemm3m_kernel<0, 1, 128, M3_BN, 4, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(zgemm3m_kernel<1, 1, 128, M3_BN, 4, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    }
     return NEGF_OK;
 }
 
@@ -238,6 +364,12 @@ int zgemm_launch_group(negf_ctx* ctx, const GemmGroup& grp) {
     const long long per = (long long)a.batch * a.batch2 * grp.ng;
     const long long t128 = (long long)((a.m + 127) / 128) * ((a.n + 63) / 64) * per;
     const long long t64 = (long long)((a.m + 63) / 64) * ((a.n + 63) / 64) * per;
+    if (ctx->gemm_3m && a.m > 64 && t128 >= ctx->num_sms) {     // opt-in, compute-bound regime only
+        if (a.opA == 0 && a.opB == 0) return launch_3m<0, 0>(ctx, grp);
+        if (a.opA == 1 && a.opB == 0) return launch_3m<1, 0>(ctx, grp);
+        if (a.opA == 0 && a.opB == 1) return launch_3m<0, 1>(ctx, grp);
+        return launch_3m<1, 1>(ctx, grp);
+    }
     if (a.m > 64 && t128 >= ctx->num_sms) return launch_ops<128, 64, 4, 2, 1>(ctx, grp);
     // blocks up to 64 x 64: four 32x32 CTAs per product balance the SMs better than one 64x64 CTA
     // (measured 5-7 % faster at b = 64 for 128 .. 512 products per launch)

@@ -36,10 +36,13 @@ def main():
     ap.add_argument("--opB", type=int, default=0)
     ap.add_argument("--reps", type=int, default=10)
     ap.add_argument("--sets", type=int, default=2, help="operand sets rotated between launches")
+    ap.add_argument("--gemm-3m", action="store_true", help="NEGF_OPT_GEMM_3M (tflops still counted as 8 b^3 per product)")
     args = ap.parse_args()
     ctx = negf.Context(0)
     st = torch.cuda.current_stream()
     ctx.set_stream(st.cuda_stream)
+    if args.gemm_3m:
+        ctx.set_option(negf.OPT_GEMM_3M, 1)
     peak = ctx.fp64_peak(200.0)
     if args.kernel == "peak":
         print(json.dumps({"kernel": "dmma_peak_probe", "tflops": peak}))

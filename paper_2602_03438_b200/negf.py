@@ -24,6 +24,7 @@ OK, EINVAL, ENOWORKSPACE, EUNSUPPORTED, ECUDA, ENOSTATE = 0, -1, -2, -3, -4, -5
 SIGMA_NONE, SIGMA_SCALAR, SIGMA_BT = 0, 1, 2
 KEEP_SWEEP = 1
 OPT_GRAPH_LOOPS = 1
+OPT_GEMM_3M = 2
 
 
 class c128(C.Structure):

@@ -131,3 +131,36 @@ def test_full_block_sizes(runner_mod, cfg, kw, vs_oracle):
                                    ("GG_upper", "gtr", "GX_upper")):
                 err = rel_fro(dp.host(name)[k], o[grp][key])
                 assert err < TOL, (cfg, k, name, err)
+
+
+def test_gemm_3m_option(runner_mod, negf_lib):
+    """NEGF_OPT_GEMM_3M: 3M complex products in the compute-bound regime.  The building block stays inside
+    1e-13 norm-wise, the whole path (b = 1024, dense BT Sigma) inside the 1e-10 bar against the oracle."""
+    rng = np.random.default_rng(3)
+    import torch
+    ctx = negf_lib.Context(0)
+    ctx.set_stream(torch.cuda.current_stream().cuda_stream)
+    ctx.set_option(negf_lib.OPT_GEMM_3M, 1)
+    m = 512
+    for opA, opB in ((0, 0), (1, 0), (0, 1), (1, 1)):
+        A = rng.standard_normal((8, m, m)) + 1j * rng.standard_normal((8, m, m))
+        B = rng.standard_normal((8, m, m)) + 1j * rng.standard_normal((8, m, m))
+        h = lambda x: np.conj(np.swapaxes(x, -1, -2))
+        ref = (h(A) if opA else A) @ (h(B) if opB else B)
+        dA, dB = torch.from_numpy(A).cuda(), torch.from_numpy(B).cuda()
+        dC = torch.empty_like(dA)
+        ctx.zgemm_batched(opA, opB, m, m, m, 1.0, dA, m, m * m, dB, m, m * m, 0.0, None, dC, m, m * m, 8)
+        err = np.linalg.norm(dC.cpu().numpy() - ref) / np.linalg.norm(ref)
+        assert err < 1e-13, (opA, opB, err)
+    wl = W.make_workload(3, n_blocks=3, n_energy=1)
+    sig = wl.sigma_s()
+    dp = runner_mod.DevicePath(wl, want_greater=True, sigma=sig)
+    dp.ctx.set_option(negf_lib.OPT_GEMM_3M, 1)
+    dp.run()
+    assert int(dp.out["info_r"].abs().sum()) == 0
+    o = pipeline.solve_energy(wl, 0, sigma=sig, obc_in=_gpu_boundary(dp, 0), want_greater=True)
+    for name, grp, key in (("GR_diag", "ret", "GR_diag"), ("GR_upper", "ret", "GR_upper"), ("GL_diag", "les", "GX_diag"),
+                           ("GL_upper", "les", "GX_upper"), ("GG_diag", "gtr", "GX_diag")):
+        err = rel_fro(dp.host(name)[0], o[grp][key])
+        print(f"3M b=1024 {name}: {err:.2e}")
+        assert err < TOL, (name, err)
