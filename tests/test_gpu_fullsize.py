@@ -164,3 +164,25 @@ def test_gemm_3m_option(runner_mod, negf_lib):
         err = rel_fro(dp.host(name)[0], o[grp][key])
         print(f"3M b=1024 {name}: {err:.2e}")
         assert err < TOL, (name, err)
+
+
+def test_config1_full_against_dense_definition(runner_mod):
+    """The bench workload against the DEFINITION itself (dense inversion of the N = 2048 system)
+    for one energy of the grid, independent of the RGF oracle."""
+    from oracle import dense
+    wl = W.make_workload(1)
+    sig = wl.sigma_s()
+    dp = runner_mod.DevicePath(wl, sigma=sig)
+    dp.run()
+    k = 21
+    A = _a_blocks(wl, dp, k, sig)
+    B = assemble.b_blocks(wl.n_blocks, wl.block_size, pipeline._slice_sigma(sig["l"], k),
+                          dp.host("sigma_l_L")[k], dp.host("sigma_l_R")[k])
+    d = dense.dense_green(*A, B_list=[B])
+    tol = 5e-10            # the dense fp64 inverse itself carries eps * cond(A)
+    assert rel_fro(dp.host("GR_diag")[k], d["GR"][0]) < tol
+    assert rel_fro(dp.host("GR_upper")[k], d["GR"][1]) < tol
+    assert rel_fro(dp.host("GR_lower")[k], d["GR"][2]) < tol
+    assert rel_fro(dp.host("GR_corner")[k], d["GR_full"][:64, 31 * 64:]) < tol
+    assert rel_fro(dp.host("GL_diag")[k], d["GX"][0][0]) < tol
+    assert rel_fro(dp.host("GL_upper")[k], d["GX"][0][1]) < tol

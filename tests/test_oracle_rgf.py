@@ -172,3 +172,20 @@ def test_gauss_jordan_matches_lapack():
     rng = np.random.default_rng(3)
     M = rng.standard_normal((9, 9)) + 1j * rng.standard_normal((9, 9))
     assert np.allclose(dense.gauss_jordan_inverse(M), np.linalg.inv(M), rtol=1e-11, atol=1e-12)
+
+
+@pytest.mark.parametrize("k", [0, 37])
+def test_config1_full_size_rgf_equals_dense(k):
+    """P1 at the size bench.py times: configs[1] (n = 32, b = 64, N = 2048, scalar scattering), tier 1 against
+    the dense fp64 definition for two energies of the grid."""
+    wl = W.make_workload(1)
+    out = pipeline.solve_energy(wl, k, want_greater=False)
+    d = dense.dense_green(*out["A"], B_list=[out["BL"]])
+    r = out["ret"]
+    tol = 5e-10            # cond(A) ~ 1e3-1e4 at this size; both sides are fp64
+    assert rel_fro(r["GR_diag"], d["GR"][0]) < tol
+    assert rel_fro(r["GR_upper"], d["GR"][1]) < tol
+    assert rel_fro(r["GR_lower"], d["GR"][2]) < tol
+    assert rel_fro(r["GR_corner"][0], d["GR_full"][:64, 31 * 64:]) < tol
+    assert rel_fro(out["les"]["GX_diag"], d["GX"][0][0]) < tol
+    assert rel_fro(out["les"]["GX_upper"], d["GX"][0][1]) < tol
