@@ -216,6 +216,19 @@ int negf_observables(negf_ctx* ctx, const negf_problem* p,
                      double* density, double* ldos, double* transmission,
                      double* bond_current, double* contact_current);
 
+/* ---- Eq. 3: energy convolution of selected blocks ----------
+ * The step on the other side of the LSE in the paper's Fig. 1, for M1 = M2 = I and the element-wise product:
+ *   mode 0 (convolution)  Y[m] = scale * sum_k X1[m - k] (.) op(X2[k]),                  m = 0 .. 2 N_E - 2
+ *   mode 1 (correlation)  Y[m] = scale * sum_k X1[k] (.) op(X2[k - (m - (N_E - 1))])     (lag m - (N_E - 1))
+ * on a uniform grid of N_E <= 1024 energies, zero outside it; op = identity or complex conjugate (conj2),
+ * with the b x b blocks of X2 read transposed when transpose_block = b > 0 (elems_per_energy must then be a
+ * multiple of b*b).  X1, X2: [N_E][elems_per_energy] (any family of include/negf.h, energy slowest); Y:
+ * [2 N_E - 1][elems_per_energy].  Done by FFT along the energy axis in shared memory (radix 2, zero-padded
+ * to a power of two), the (E; i,j) -> (i,j; E) transposition of the paper happening in the tile load. */
+int negf_energy_convolve(negf_ctx* ctx, int n_energy, long long elems_per_energy, int transpose_block,
+                         const negf_c128* X1, const negf_c128* X2, int mode, int conj2, negf_c128 scale,
+                         negf_c128* Y);
+
 /* ---- whole path with HOST buffers (bench.py's end-to-end leg) ---------------------------------
  * All array arguments here are HOST pointers (pinned memory recommended).  Copies the inputs
  * to the device, runs negf_obc_decimate (both sides) -> negf_rgf_retarded ->

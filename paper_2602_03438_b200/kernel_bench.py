@@ -29,7 +29,7 @@ def _rand(shape, gen):
 
 def main():
     ap = argparse.ArgumentParser()
-    ap.add_argument("--kernel", default="zgemm", choices=["zgemm", "zinv", "peak"])
+    ap.add_argument("--kernel", default="zgemm", choices=["zgemm", "zinv", "peak", "econv"])
     ap.add_argument("--b", type=int, default=1024)
     ap.add_argument("--batch", type=int, default=16)
     ap.add_argument("--opA", type=int, default=0)
@@ -49,6 +49,32 @@ def main():
         return
     b, batch = args.b, args.batch
     gen = torch.Generator(device="cuda"); gen.manual_seed(1)
+    if args.kernel == "econv":
+        # Eq. 3 on a family of selected blocks: --batch energies, --b block size, 63 blocks (configs[1]-like);
+        # HBM-bound: (2 N_E + 2 N_E - 1) * 16 bytes per element, against MEASURED_PEAKS.json's copy bandwidth
+        ne, M = batch, 63 * b * b
+        X1, X2 = _rand((ne, M), gen), _rand((ne, M), gen)
+        Y = torch.empty(2 * ne - 1, M, dtype=torch.complex128, device="cuda")
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        for _ in range(3):
+            ctx.energy_convolve(ne, M, X1, X2, Y, mode=1, transpose_block=b)
+        torch.cuda.synchronize()
+        times = []
+        for _ in range(args.reps):
+            e0.record(st); ctx.energy_convolve(ne, M, X1, X2, Y, mode=1, transpose_block=b); e1.record(st)
+            torch.cuda.synchronize(); times.append(e0.elapsed_time(e1))
+        ms = sorted(times)[len(times) // 2]
+        nbytes = (4 * ne - 1) * M * 16.0
+        import os
+        peak_gbs = None
+        try:
+            peak_gbs = json.load(open(os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "MEASURED_PEAKS.json")))["hbm_gbs"]
+        except Exception:
+            peak_gbs = 6650.0     # fallback of the profiling recipe
+        gbs = nbytes / (ms * 1e-3) * 1e-9
+        print(json.dumps({"kernel": "econv", "n_energy": ne, "b": b, "elems_per_energy": M, "ms_median": ms,
+                          "algorithmic_GBps": gbs, "hbm_peak_GBps": peak_gbs, "frac": gbs / peak_gbs}))
+        return
     flops = 8.0 * b ** 3 * batch
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     if args.kernel == "zgemm":

@@ -60,7 +60,7 @@ class HostOutputs(C.Structure):
 EXPORTS = ["negf_create", "negf_destroy", "negf_set_stream", "negf_workspace_bytes", "negf_set_workspace",
            "negf_set_option", "negf_strerror", "negf_last_cuda_error", "negf_launch_count",
            "negf_profile_enable", "negf_profile_read", "negf_obc_decimate", "negf_obc_decimate_pair",
-           "negf_rgf_retarded", "negf_rgf_lesser_greater", "negf_observables", "negf_pipeline_host_bytes",
+           "negf_rgf_retarded", "negf_rgf_lesser_greater", "negf_observables", "negf_energy_convolve", "negf_pipeline_host_bytes",
            "negf_pipeline_host", "negf_zgemm_batched", "negf_zinverse_batched", "negf_fp64_peak"]
 
 _P = C.c_void_p
@@ -86,6 +86,7 @@ lib.negf_rgf_retarded.argtypes = [_P, C.POINTER(Problem), C.POINTER(Sigma), _P, 
 lib.negf_rgf_lesser_greater.argtypes = [_P, C.POINTER(Problem), C.POINTER(Sigma), C.POINTER(Sigma),
                                         C.POINTER(Sigma), _P, _P, _P, _P, _P, _P]
 lib.negf_observables.argtypes = [_P, C.POINTER(Problem)] + [_P] * 19
+lib.negf_energy_convolve.argtypes = [_P, C.c_int, C.c_longlong, C.c_int, _P, _P, C.c_int, C.c_int, c128, _P]
 lib.negf_pipeline_host_bytes.argtypes = [C.POINTER(Problem), C.c_int, C.c_int, C.POINTER(C.c_size_t)]
 lib.negf_pipeline_host.argtypes = [_P, C.POINTER(Problem), C.POINTER(Sigma), C.POINTER(Sigma), C.POINTER(Sigma),
                                    _P, C.c_double, C.c_double, C.c_double, C.c_double, C.c_int, _P, C.c_size_t,
@@ -227,6 +228,11 @@ class Context:
                 sigma_lesser_L, sigma_greater_L, sigma_lesser_R, sigma_greater_R, weights, density, ldos,
                 transmission, bond_current, contact_current]
         self._check(lib.negf_observables(self._h, C.byref(p), *[_ptr(a) for a in args]), "negf_observables")
+
+    def energy_convolve(self, n_energy, elems_per_energy, X1, X2, Y, mode=0, conj2=False, scale=1.0, transpose_block=0):
+        sc = complex(scale)
+        self._check(lib.negf_energy_convolve(self._h, n_energy, elems_per_energy, transpose_block, _ptr(X1), _ptr(X2),
+                                             mode, int(conj2), c128(sc.real, sc.imag), _ptr(Y)), "negf_energy_convolve")
 
     @staticmethod
     def pipeline_host_bytes(p: Problem, kind_max: int, want_greater: bool) -> int:
