@@ -383,7 +383,18 @@ def run_e2e(args, wl, ctx, dev, world, torch, negf):
         up, down = hp.run()            # synchronises the stream before returning
     dt = time.perf_counter() - t0
     assert int(hp.out["info"].abs().sum()) == 0, "numerical failure flagged in the e2e run"
-    return {"value": world * ne * reps / dt, "unit": UNIT, "h2d_bytes_per_step": int(up), "d2h_bytes_per_step": int(down),
+    # same call with the G block outputs NULL: only density, LDOS, T(E), currents and info cross PCIe on the way back
+    ho = runner.HostPath(wl, ne, device=dev, ctx=ctx, blocks=False)
+    for _ in range(2):
+        up_o, down_o = ho.run()
+    torch.cuda.synchronize()
+    t1 = time.perf_counter()
+    for _ in range(reps):
+        up_o, down_o = ho.run()
+    dt_o = time.perf_counter() - t1
+    obs_only = {"value": world * ne * reps / dt_o, "unit": UNIT, "h2d_bytes_per_step": int(up_o),
+                "d2h_bytes_per_step": int(down_o), "ms_per_call": 1e3 * dt_o / reps}
+    return {"value": world * ne * reps / dt, "observables_only": obs_only, "unit": UNIT, "h2d_bytes_per_step": int(up), "d2h_bytes_per_step": int(down),
             "energies_per_call": ne, "ms_per_call": 1e3 * dt / reps,
             "api": "negf_pipeline_host (host pinned buffers in, all selected G blocks + observables out)"}
 

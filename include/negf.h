@@ -224,7 +224,8 @@ int negf_observables(negf_ctx* ctx, const negf_problem* p,
  * with the b x b blocks of X2 read transposed when transpose_block = b > 0 (elems_per_energy must then be a
  * multiple of b*b).  X1, X2: [N_E][elems_per_energy] (any family of include/negf.h, energy slowest); Y:
  * [2 N_E - 1][elems_per_energy].  Done by FFT along the energy axis in shared memory (radix 2, zero-padded
- * to a power of two), the (E; i,j) -> (i,j; E) transposition of the paper happening in the tile load. */
+ * to a power of two L >= 2 N_E - 1), the (E; i,j) -> (i,j; E) transposition of the paper happening in the
+ * tile load.  NEGF_EUNSUPPORTED for N_E > 1024; X1, X2 and Y must not overlap. */
 int negf_energy_convolve(negf_ctx* ctx, int n_energy, long long elems_per_energy, int transpose_block,
                          const negf_c128* X1, const negf_c128* X2, int mode, int conj2, negf_c128 scale,
                          negf_c128* Y);

@@ -151,7 +151,8 @@ class HostPath:
     inside the call (what bench.py times as the end-to-end number)."""
 
     def __init__(self, wl: Workload, n_energy: Optional[int] = None, device: str = "cuda:0",
-                 ctx: Optional[negf.Context] = None, want_greater: Optional[bool] = None):
+                 ctx: Optional[negf.Context] = None, want_greater: Optional[bool] = None, blocks: bool = True):
+        """blocks=False: the G block outputs are NULL (only the observables come back to the host)."""
         self.wl = wl
         self.device = torch.device(device)
         self.ne = wl.n_energy if n_energy is None else min(n_energy, wl.n_energy)
@@ -181,7 +182,7 @@ class HostPath:
         kind = _KIND[wl.sigma_kind]
         self.scratch = torch.empty(negf.Context.pipeline_host_bytes(self.problem, kind, self.want_greater),
                                    dtype=torch.uint8, device=self.device)
-        z = lambda *s: torch.empty(s, dtype=torch.complex128).pin_memory()
+        z = lambda *s: torch.empty(s, dtype=torch.complex128).pin_memory() if blocks else None
         r = lambda *s: torch.empty(s, dtype=torch.float64).pin_memory()
         g = self.want_greater
         self.out = {"GR_diag": z(ne, n, b, b), "GR_upper": z(ne, n - 1, b, b), "GR_lower": z(ne, n - 1, b, b),
