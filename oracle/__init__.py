@@ -13,10 +13,13 @@ Tiers:
   obc.py          Sancho-Rubio decimation of the lead blocks.
   observables.py  density, LDOS, transmission, bond and contact currents (readings R11-R13).
   pipeline.py     the whole path for one workload, chaining the above (what bench.py times).
+  convolution.py  Eq. 3 for M1 = M2 = I: the discrete energy convolution / correlation
+                  of selected blocks as the written-out double sum.
 
 Pins (tests/test_oracle_*.py, all `-m "not gpu"`): tier 1 vs tier 0 on random tiny and
 config-shaped inputs; tier 0 fp64 vs extended precision; 1D-chain closed form for the
 decimation; integer transmission of a translation-invariant device; current conservation
 (PAPER.md:86); selected-block residuals of Eqs. 1-2; anti-Hermiticity; the corrected spectral
-identity; hand-solved 1x1/2x2 cases.  No function here is "parity unpinned".
+identity; hand-solved 1x1/2x2 cases; for the convolution a shifted delta, a polynomial product
+with binomial coefficients, np.convolve per element and an np.fft route.  No function here is "parity unpinned".
 """
