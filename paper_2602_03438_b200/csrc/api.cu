@@ -34,7 +34,7 @@ extern "C" int negf_create(negf_ctx** out, int device) {
     if (cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking) != cudaSuccess) { delete c; return NEGF_ECUDA; } c->obc_key_ws = nullptr; c->obc_key_b = c->obc_key_nb = c->obc_key_maxit = 0; c->obc_key_tol = 0.0;
     c->prof_on = false; c->prof_depth = 0; c->prof_last_class = -1; c->prof_last_event = nullptr;
     for (int k = 0; k < NEGF_PROF_CLASSES; k++) { c->prof_ms[k] = 0.0; c->prof_n[k] = 0; }
-    if (zgemm_prepare(c) != NEGF_OK) { delete c; return NEGF_ECUDA; }
+    if (zgemm_prepare(c) != NEGF_OK || zinv_prepare(c) != NEGF_OK || econv_prepare(c) != NEGF_OK) { delete c; return NEGF_ECUDA; }
     *out = c;
     return NEGF_OK;
 }

@@ -233,6 +233,8 @@ struct GemmArgs {
 };
 int zgemm_launch(negf_ctx* ctx, const GemmArgs& a);
 int zgemm_prepare(negf_ctx* ctx);
+int zinv_prepare(negf_ctx* ctx);      // shared-memory opt-ins of the K1 kernels (zinv.cu)
+int econv_prepare(negf_ctx* ctx);     // same for the energy-convolution kernels (econv.cu)
 // several independent products of identical shape / ops / batch in ONE launch (blockIdx.z = member)
 constexpr int NEGF_GEMM_GROUP_MAX = 4;
 struct GemmGroup { GemmArgs g[NEGF_GEMM_GROUP_MAX]; int ng; };

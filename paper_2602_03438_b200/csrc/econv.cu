@@ -103,6 +103,7 @@ template <int LOGL> struct EconvShape {
     static constexpr int TE = 1 << LT;
     static constexpr int NP = econv_npass(LOGL);
     static constexpr int NT = (L * TE) / 8;                  // one 8-point item per thread in a 3-stage pass
+    static constexpr size_t SMEM = ((size_t)2 * L * TE + L / 2) * sizeof(cplx);   // L >= 512: 64 - 144 KB
 };
 
 // Forward pass PS over the tile: its Q stages of the sub-transforms of size 2^LN, both operands.  The first
@@ -212,16 +213,23 @@ template <int LOGL>
 void econv_launch(const EconvArgs& a, cudaStream_t st) {
     using SH = EconvShape<LOGL>;
     const long long ctas = (a.M + SH::TE - 1) / SH::TE;
-    constexpr size_t smem = ((size_t)2 * SH::L * SH::TE + SH::L / 2) * sizeof(cplx);
-    static bool attr_done = false;                          // L >= 512: 64 - 144 KB
-    if (smem > 48 * 1024 && !attr_done) {
-        cudaFuncSetAttribute(econv_kernel<LOGL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        attr_done = true;
-    }
-    econv_kernel<LOGL><<<(unsigned)ctas, SH::NT, smem, st>>>(a);
+    econv_kernel<LOGL><<<(unsigned)ctas, SH::NT, SH::SMEM, st>>>(a);
+}
+
+template <int LOGL>
+cudaError_t econv_optin() {
+    return cudaFuncSetAttribute(econv_kernel<LOGL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)EconvShape<LOGL>::SMEM);
 }
 
 }  // namespace
+
+// shared-memory opt-in of the large transforms, once per context (= per device) at negf_create
+int econv_prepare(negf_ctx* ctx) {
+    NEGF_CUDA_CHECK(ctx, econv_optin<9>());
+    NEGF_CUDA_CHECK(ctx, econv_optin<10>());
+    NEGF_CUDA_CHECK(ctx, econv_optin<11>());
+    return NEGF_OK;
+}
 
 extern "C" int negf_energy_convolve(negf_ctx* ctx, int n_energy, long long elems_per_energy, int transpose_block,
                                     const negf_c128* X1, const negf_c128* X2, int mode, int conj2, negf_c128 scale,

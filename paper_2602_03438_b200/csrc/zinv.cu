@@ -220,6 +220,7 @@ __global__ void __launch_bounds__(GJ_NW * 32) gj_reg_kernel(cplx* A, long long s
 // blocked path, step 1: cluster panel LU with partial pivoting
 // ------------------------------------------------------------------------------------------------
 struct Cand { double val; int row; int pad; };
+constexpr size_t PANEL_SMEM_FIXED = (2 * CMAX * PW + 2 * PW) * sizeof(cplx) + 2 * CMAX * sizeof(Cand);
 
 struct PanelArgs {
     cplx* A; long long sA; int b, k0, w, slab;
@@ -715,6 +716,16 @@ size_t zinv_workspace_bytes(int b, int batch) {
            2 * align_up((size_t)batch * b * sizeof(int), 256);
 }
 
+// shared-memory opt-ins of the blocked path, once per context (= per device) at negf_create
+int zinv_prepare(negf_ctx* ctx) {
+    NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_panel_cluster_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                              (int)(PANEL_SMEM_ROWS_BYTES + PANEL_SMEM_FIXED)));
+    NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_colperm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+    NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_panel_reg_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)reg_panel_smem_bytes(8)));
+    NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_panel_reg_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)reg_panel_smem_bytes(16)));
+    return NEGF_OK;
+}
+
 int zinv_launch(negf_ctx* ctx, int b, cplx* A, long long sA, int batch, void* ws, int* info,
                 int info_code, const int* skip, const int* code_dev) {
     ProfScope _ps(ctx, NEGF_PROF_INVERSE);
@@ -738,16 +749,7 @@ int zinv_launch(negf_ctx* ctx, int b, cplx* A, long long sA, int batch, void* ws
     int w = PW;
     while (w > 8 && (size_t)((b + CMAX - 1) / CMAX) * w * sizeof(cplx) > (size_t)PANEL_SMEM_ROWS_BYTES) w >>= 1;
     if ((size_t)((b + CMAX - 1) / CMAX) * w * sizeof(cplx) > (size_t)PANEL_SMEM_ROWS_BYTES) return NEGF_EUNSUPPORTED;
-    const size_t fixed = (2 * CMAX * PW + 2 * PW) * sizeof(cplx) + 2 * CMAX * sizeof(Cand);
-    static bool attr_done = false;
-    if (!attr_done) {
-        NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_panel_cluster_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                                  (int)(PANEL_SMEM_ROWS_BYTES + fixed)));
-        NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_colperm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-        NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_panel_reg_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)reg_panel_smem_bytes(8)));
-        NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_panel_reg_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)reg_panel_smem_bytes(16)));
-        attr_done = true;
-    }
+    const size_t fixed = PANEL_SMEM_FIXED;
     const cplx one = cmake(1.0, 0.0), mone = cmake(-1.0, 0.0), zero = cmake(0.0, 0.0);
     // Two-level blocking.  Inside an outer block K = [K0, K0 + nbk) the width-w panels are
     // eliminated with their row swaps and rank-w updates restricted to the columns of K, so that

@@ -217,6 +217,81 @@ def chain_lead(b: int, seed: int = 7):
     return H_d, H_u, q, eps, t
 
 
+def make_phonon_workload(n_blocks: int, block_size: int, n_omega: int, periodic: bool = False,
+                         seed: int = 0, eta: float = 1e-4) -> Workload:
+    """Phonon-like inputs for the same Eqs. 1-2 (A "made of the Hamiltonian, dynamical,
+    or bare Coulomb matrices"): A(w) = (w^2 + i eta) I - Phi with the dynamical
+    matrix Phi of a network of unit masses and positive springs, block tridiagonal, real symmetric,
+    positive semi-definite (acoustic sum rule inside the device).  Mapping onto include/negf.h:
+    H := Phi, S := I, energy := w^2.  `periodic` repeats one cell and one inter-cell coupling, which makes
+    the device a piece of a perfect wire.  Inputs only; the frequencies sit inside the band."""
+    n, b = int(n_blocks), int(block_size)
+    rng = np.random.Generator(np.random.PCG64(np.random.SeedSequence([BASE_SEED, 201, seed, n, b])))
+    cells = 1 if periodic else n
+    K = rng.uniform(0.2, 1.0, size=(cells, b, b)) / max(b - 1, 1)
+    K = np.triu(K, 1)
+    K = K + np.swapaxes(K, -1, -2)                                 # springs inside a cell
+    C = rng.uniform(0.2, 1.0, size=(max(cells - 1, 1), b, b)) / b   # springs cell i (row) <-> cell i+1 (column)
+    if periodic:
+        K = np.repeat(K, n, axis=0)
+        C = np.repeat(C[:1], max(n - 1, 0), axis=0)
+        left = right = C[0] if n > 1 else C[0]
+    else:
+        C = C[:max(n - 1, 0)]
+        left = right = None
+    idx = np.arange(b)
+    Phi_d = -K.copy()
+    Phi_d[:, idx, idx] += K.sum(axis=2)
+    for i in range(n - 1):
+        Phi_d[i, idx, idx] += C[i].sum(axis=1)
+        Phi_d[i + 1, idx, idx] += C[i].sum(axis=0)
+    if periodic and n > 1:      # the springs to the lead cells, so that every cell of the wire is the same
+        Phi_d[0, idx, idx] += C[0].sum(axis=0)
+        Phi_d[n - 1, idx, idx] += C[0].sum(axis=1)
+    elif not periodic and n > 1:   # leads are periodic copies of the contact blocks (reading R2): tie them too
+        Phi_d[0, idx, idx] += C[0].sum(axis=0)
+        Phi_d[n - 1, idx, idx] += C[n - 2].sum(axis=1)
+    Phi_u = -C
+    wmax2 = 0.6 * float(np.max(np.linalg.eigvalsh(Phi_d[0])))
+    omega2 = np.linspace(0.05 * wmax2, wmax2, int(n_omega)) if n_omega > 1 else np.array([0.4 * wmax2])
+    return Workload(config=100, name=f"phonon[n={n},b={b},Nw={n_omega}]", n_blocks=n, block_size=b,
+                    energies=omega2, eta=eta, H_diag=np.ascontiguousarray(Phi_d.astype(np.complex128)),
+                    H_upper=np.ascontiguousarray(Phi_u.astype(np.complex128)), S_diag=None, S_upper=None,
+                    sigma_kind="none", want_lesser=True, want_greater=True, weights=trapezoid_weights(omega2))
+
+
+def make_coulomb_workload(n_blocks: int, block_size: int, n_omega: int, seed: int = 0):
+    """Screened-Coulomb-like inputs for the same Eqs. 1-2 (C = W, B = P):
+    W^R(w) = (V^-1 - P^R(w))^-1 with a block-tridiagonal Hermitian positive definite inverse bare
+    interaction V^-1 and block-tridiagonal polarisations P^R, P^<, P^> per frequency, P^> - P^< = P^R - P^A.
+    Mapping onto include/negf.h: H := -V^-1, S := I, energy := 0, eta := 0 (z = 0), Sigma := P, no leads.
+    Returns (workload, sigma) with sigma in the layout of Workload.sigma_s().  Inputs only."""
+    n, b, nw = int(n_blocks), int(block_size), int(n_omega)
+    rng = np.random.Generator(np.random.PCG64(np.random.SeedSequence([BASE_SEED, 202, seed, n, b])))
+    Vd = 0.3 * hermitian_blocks(rng, n, b, 1.0)
+    idx = np.arange(b)
+    Vd[:, idx, idx] += 2.0
+    Vu = 0.3 * complex_normal(rng, (max(n - 1, 0), b, b), 1.0) / np.sqrt(b)
+    wl = Workload(config=101, name=f"coulomb[n={n},b={b},Nw={nw}]", n_blocks=n, block_size=b,
+                  energies=np.zeros(nw), eta=0.0, H_diag=np.ascontiguousarray(-Vd), H_upper=np.ascontiguousarray(-Vu),
+                  S_diag=None, S_upper=None, sigma_kind="bt", want_lesser=True, want_greater=True,
+                  weights=np.ones(nw))
+    h = lambda a: np.conj(np.swapaxes(a, -1, -2))
+    var = 1e-2
+    sig = {k: {"kind": "bt", "diag": np.empty((nw, n, b, b), np.complex128),
+               "upper": np.empty((nw, max(n - 1, 0), b, b), np.complex128)} for k in "rlg"}
+    sig["r"]["lower"] = np.empty((nw, max(n - 1, 0), b, b), np.complex128)
+    for k in range(nw):
+        ld, gd, pd = (hermitian_blocks(rng, n, b, var) for _ in range(3))
+        lu, gu, pu = (complex_normal(rng, (max(n - 1, 0), b, b), var) / np.sqrt(b) for _ in range(3))
+        sig["l"]["diag"][k], sig["l"]["upper"][k] = 1j * ld, 1j * lu            # anti-Hermitian P^<
+        sig["g"]["diag"][k], sig["g"]["upper"][k] = -1j * gd, -1j * gu          # anti-Hermitian P^>
+        sig["r"]["diag"][k] = pd - 0.5j * (gd + ld)                             # P^R = Re + (P^> - P^<)/2
+        sig["r"]["upper"][k] = pu - 0.5j * (gu + lu)
+        sig["r"]["lower"][k] = h(pu) - 0.5j * (h(gu) + h(lu))
+    return wl, sig
+
+
 def shard_energies(wl: Workload, rank: int, world: int) -> Workload:
     """Energy sharding for multi-GPU runs ("Each E is independent of the other"): the
     job's grid is `world` times as dense as the config's and rank r takes every world-th point
