@@ -34,11 +34,11 @@ constexpr int CMAX = 8;            // portable cluster size
 constexpr int PANEL_SMEM_ROWS_BYTES = 176 * 1024;   // + 9 KB exchange buffers + 33 KB static < 227 KB
 
 // ------------------------------------------------------------------------------------------------
-// small path: REGISTER-resident Gauss-Jordan, one CTA of 8 warps per matrix (b <= 96).
-//   * warp w owns the columns j = w + 8 c (c < CB), lane l the rows i = l + 32 r (r < RB): the
+// small path: REGISTER-resident Gauss-Jordan, one CTA of 16 warps per matrix (b <= 96).
+//   * warp w owns the columns j = w + 16 c (c < CB), lane l the rows i = l + 32 r (r < RB): the
 //     whole matrix lives in registers (RB x CB elements per thread);
-//   * the pivot search of column k is done by its owner warp alone with three redux.sync on the
-//     bit pattern of |re|+|im| (monotone for non-negative doubles), which then publishes the
+//   * the pivot search of column k is done by its owner warp alone with one redux.sync on a 32-bit
+//     key made of the leading bits of |re|+|im| and the row, which then publishes the
 //     multiplier column, the pivot index and 1/pivot to shared memory;
 //   * ONE block barrier per column; the two rows that trade places travel inside each warp
 //     through a per-warp shared-memory line (no block-level traffic);
@@ -50,15 +50,25 @@ constexpr int PANEL_SMEM_ROWS_BYTES = 176 * 1024;   // + 9 KB exchange buffers +
 // ------------------------------------------------------------------------------------------------
 
 
-__device__ __forceinline__ cplx crecip_fast(cplx a) {      // pivots are O(1): no overflow guard needed
-    const double inv = 1.0 / fma(a.x, a.x, a.y * a.y);
-    return cmake(a.x * inv, -a.y * inv);
+// 1 / a for a pivot (O(1): no overflow guard needed).  The real reciprocal is the hardware's 20-bit
+// estimate refined by two Newton steps (2^-20 -> 2^-40 -> below one ulp): about 50 cycles of dependent
+// latency instead of the ~80 of the IEEE division sequence, on the critical chain of every column.
+__device__ __forceinline__ cplx crecip_fast(cplx a) {
+    const double x = fma(a.x, a.x, a.y * a.y);
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    double e = fma(-x, r, 1.0);
+    r = fma(r, e, r);
+    e = fma(-x, r, 1.0);
+    r = fma(r, e, r);
+    return cmake(a.x * r, -a.y * r);
 }
 
 struct GjShared {            // pointers into the kernel's shared memory
     cplx* colbuf;            // [2][NR]
     cplx* wrow;              // this warp's [2][2][CB]
     cplx* s_d; int* s_p; int* piv; int* s_sing;
+    cplx* rscale;            // [NR] pending scale 1/pivot of every row that has been a pivot row
 };
 
 // pivot search + publication of column kn, held in slot C of the calling (owner) warp
@@ -66,39 +76,37 @@ template <int RB, int CB, int C>
 __device__ __forceinline__ void gj_owner(const cplx (&m)[RB][CB], unsigned used, const GjShared& sh, int kn, int b, int lane) {
     constexpr int NR = RB * 32;
     const int parn = kn & 1;
-    unsigned long long key = 0ull;
-    int bi = 0x7fffffff;
+    // ONE 32-bit key per candidate: the top 25 bits of |re| + |im| (sign 0, exponent, 13 mantissa bits)
+    // above 7 bits of 127 - row, so a single redux.sync.max names the pivot: the largest candidate up
+    // to a relative 2^-13 (threshold pivoting; the growth bound changes by that factor), lowest row first
+    // among those.  Rows here are < 96.
+    unsigned key = 0u;
 #pragma unroll
     for (int r = 0; r < RB; r++) {
         const int i = lane + 32 * r;
         sh.colbuf[parn * NR + i] = m[r][C];
         if (!((used >> r) & 1u) && i < b) {
-            const unsigned long long kq = (unsigned long long)__double_as_longlong(cabs1(m[r][C]));
-            if (bi == 0x7fffffff || kq > key) { key = kq; bi = i; }
+            const unsigned hi = (unsigned)((unsigned long long)__double_as_longlong(cabs1(m[r][C])) >> 32);
+            key = max(key, (hi & 0xffffff80u) | (unsigned)(127 - i));
         }
     }
-    const bool has = bi != 0x7fffffff;
-    const unsigned hi = __reduce_max_sync(0xffffffffu, has ? (unsigned)(key >> 32) : 0u);
-    const bool mh = has && (unsigned)(key >> 32) == hi;
-    const unsigned lo = __reduce_max_sync(0xffffffffu, mh ? (unsigned)key : 0u);
-    const bool ml = mh && (unsigned)key == lo;
-    const unsigned p = __reduce_min_sync(0xffffffffu, ml ? (unsigned)bi : 0x7fffffffu);
-    cplx pv = cmake(0.0, 0.0);
+    const unsigned kmax = __reduce_max_sync(0xffffffffu, key);
+    const unsigned p = 127u - (kmax & 127u);
+    const bool sing = (kmax >> 7) == 0u;           // every candidate is zero (or denormal)
+    if (lane == (int)(p & 31u)) {        // the lane that holds the pivot inverts and publishes it
+        cplx pv = m[0][C];
 #pragma unroll
-    for (int r = 0; r < RB; r++) if (lane + 32 * r == (int)p) pv = m[r][C];
-    pv.x = __shfl_sync(0xffffffffu, pv.x, p & 31);
-    pv.y = __shfl_sync(0xffffffffu, pv.y, p & 31);
-    const bool sing = (hi == 0u && lo == 0u);
-    if (lane == 0) {
+        for (int r = 1; r < RB; r++) if ((int)(p >> 5) == r) pv = m[r][C];
         sh.s_p[parn] = (int)p; sh.piv[kn] = (int)p;
-        sh.s_d[parn] = sing ? cmake(1.0, 0.0) : crecip_fast(pv);
+        const cplx dn = sing ? cmake(1.0, 0.0) : crecip_fast(pv);
+        sh.s_d[parn] = dn; sh.rscale[p] = dn;
         if (sing && *sh.s_sing == 0) *sh.s_sing = kn + 1;
     }
 }
 
 // Rank-1 update of column slot C: m[:, C] -= mult * sr.  The special rows/columns were prepared by
-// the caller so that this one formula is right everywhere (pivot row: m = 0, mult = -1 -> sr;
-// pivot column: m = 0, sr = 1/pivot -> -mult/pivot).
+// the caller so that this one formula is right everywhere (pivot row: mult = 0, its scaling by 1/pivot
+// stays pending; pivot column: m = 0 (1 in the pivot row), sr = 1/pivot -> -mult/pivot).
 template <int RB, int CB, int C>
 __device__ __forceinline__ void gj_update(cplx (&m)[RB][CB], const cplx (&mult)[RB], const cplx (&sr)[CB]) {
 #pragma unroll
@@ -129,8 +137,12 @@ __device__ __forceinline__ void gj_columns(cplx (&m)[RB][CB], unsigned& used, co
             const cplx d = sh.s_d[par];
             cplx* wr = sh.wrow + par * CB;
             // IMPLICIT pivoting: rows never move.  The pivot row (physical row p) is broadcast inside
-            // each warp through its shared-memory line, marked as used, and turned into the scaled
-            // pivot row by the common update formula (m = 0, mult = -1).
+            // each warp through its shared-memory line and marked as used.  Its own scaling by 1/pivot
+            // is DEFERRED (rscale[p], applied once in the final scatter): the registers keep the
+            // unscaled row r_p, whose true value is d r_p.  Every later update of that row then needs
+            // true_mult / d = the register value itself as multiplier, which is what the column
+            // buffer holds, so pivoted and unpivoted rows run the same formula and the pivot row
+            // costs no register traffic here (mult = 0 for this column).
             cplx mult[RB];
 #pragma unroll
             for (int r = 0; r < RB; r++) {
@@ -138,8 +150,8 @@ __device__ __forceinline__ void gj_columns(cplx (&m)[RB][CB], unsigned& used, co
                 mult[r] = sh.colbuf[par * NR + i];
                 if (i == p) {
 #pragma unroll
-                    for (int c = 0; c < CB; c++) { wr[c] = m[r][c]; m[r][c] = cmake(0.0, 0.0); }
-                    mult[r] = cmake(-1.0, 0.0);
+                    for (int c = 0; c < CB; c++) wr[c] = m[r][c];
+                    mult[r] = cmake(0.0, 0.0);
                     used |= 1u << r;
                 }
             }
@@ -147,10 +159,10 @@ __device__ __forceinline__ void gj_columns(cplx (&m)[RB][CB], unsigned& used, co
             cplx sr[CB];
 #pragma unroll
             for (int c = 0; c < CB; c++) sr[c] = cmul(wr[c], d);
-            if (warp == wk) {            // this warp's slot CK IS column k
+            if (warp == wk) {            // this warp's slot CK IS column k: -mult d, and 1 (= d / d) in the pivot row
                 sr[CK] = d;
 #pragma unroll
-                for (int r = 0; r < RB; r++) m[r][CK] = cmake(0.0, 0.0);
+                for (int r = 0; r < RB; r++) m[r][CK] = cmake(lane + 32 * r == p ? 1.0 : 0.0, 0.0);
             }
             // look-ahead: the owner of column k+1 brings that column up to date and publishes it first
             int done = -1;
@@ -180,6 +192,7 @@ __global__ void __launch_bounds__(GJ_NW * 32) gj_reg_kernel(cplx* A, long long s
     __shared__ cplx colbuf[2 * NR];
     __shared__ cplx wrow[GJ_NW][2 * CB];         // [warp][parity][slot]: the pivot row of the current column
     __shared__ cplx s_d[2];
+    __shared__ cplx rscale[NR];
     __shared__ int s_p[2];
     __shared__ int piv[NC];
     __shared__ int dest[NC];
@@ -196,23 +209,26 @@ __global__ void __launch_bounds__(GJ_NW * 32) gj_reg_kernel(cplx* A, long long s
         }
     if (tid == 0) s_sing = 0;
     __syncthreads();
-    GjShared sh{colbuf, wrow[warp], s_d, s_p, piv, &s_sing};
+    GjShared sh{colbuf, wrow[warp], s_d, s_p, piv, &s_sing, rscale};
     unsigned used = 0u;              // bit r: my row lane + 32 r has been a pivot row
     if (warp == 0) gj_owner<RB, CB, 0>(m, used, sh, 0, b, lane);
     gj_columns<RB, CB, GJ_NW, 0>(m, used, sh, b, warp, lane);
     __syncthreads();
-    // With piv[k] = physical pivot row of column k the register array holds B[i][k] = X[i][piv[k]],
-    // X = Pi A^-1, Pi[piv[k]][k] = 1, so A^-1[r][piv[k]] = B[piv[r]][k]: every thread scatters its
-    // elements to row pinv[i], column piv[j].
+    // With piv[k] = physical pivot row of column k the register array (times the pending row scales)
+    // holds B[i][k] = X[i][piv[k]], X = Pi A^-1, Pi[piv[k]][k] = 1, so A^-1[r][piv[k]] = B[piv[r]][k]:
+    // every thread scatters its elements to row pinv[i], column piv[j].
     if (tid < b) dest[piv[tid]] = tid;         // dest = pinv
     __syncthreads();
 #pragma unroll
-    for (int r = 0; r < RB; r++)
+    for (int r = 0; r < RB; r++) {
+        const int i = lane + 32 * r;
+        const cplx rs = i < b ? rscale[i] : cmake(1.0, 0.0);
 #pragma unroll
         for (int c = 0; c < CB; c++) {
-            const int i = lane + 32 * r, j = warp + GJ_NW * c;
-            if (i < b && j < b) g[(size_t)dest[i] * b + piv[j]] = m[r][c];
+            const int j = warp + GJ_NW * c;
+            if (i < b && j < b) g[(size_t)dest[i] * b + piv[j]] = cmul(m[r][c], rs);
         }
+    }
     if (tid == 0 && s_sing && info) info[e] = code_dev ? *code_dev + code : (code > 0 ? code : s_sing);
 }
 
