@@ -261,7 +261,8 @@ int negf_zgemm_batched(negf_ctx* ctx, int opA, int opB, int m, int n, int k,
                        negf_c128 beta, const negf_c128* D,
                        negf_c128* C, int ldc, long long strideC, int batch);
 /* In-place inverse of `batch` dense b x b matrices (stride in elements), partial pivoting on
- * |re|+|im|; info[e] = 0 or (column+1) of the first zero pivot.  Uses the context workspace. */
+ * |re|+|im| (b <= 96: on its 25 leading bits, i.e. threshold pivoting at 1 - 2^-13); info[e] = 0 or
+ * (column+1) of the first zero pivot.  Uses the context workspace. */
 int negf_zinverse_batched(negf_ctx* ctx, int b, negf_c128* A, long long stride, int batch, int* info);
 /* Measures the FP64 DMMA (mma.sync m8n8k4) issue-rate peak of this GPU for about `ms`
  * milliseconds; SYNCHRONISES.  Writes TFLOP/s to *tflops (HOST pointer). */
