@@ -72,8 +72,84 @@ __device__ __forceinline__ void load_tile_mc(cplx* sm, const cplx* g, int ld, in
     }
 }
 
+// Per-thread state of one operand tile's loads, set up ONCE per CTA: the k-loop then only tests the k bound,
+// issues the cp.async of its slots at fixed shared-memory offsets and advances one pointer.  (At K = 64 the
+// tile loads' index arithmetic, redone for every k-block, was a third of the kernel's instructions.)
+//   KC (rows = the m or n coordinate, 16 k contiguous): slot i is row r_0 + i NT/16, column kc = tid & 15
+//   MC (rows = k, R mn-elements contiguous):            slot i is k-row k_0 + i NT/R, column r = tid % R
+template <int R, int NT, bool KC>
+struct TileLoader {
+    static constexpr int ITER = R * BK / NT;
+    static constexpr int RS = KC ? NT / BK : NT / R;     // rows between slots
+    static_assert(R * BK % NT == 0 && (KC ? (NT % BK == 0 && RS % 2 == 0) : (NT % R == 0)), "tile/thread shape");
+    const cplx* base;        // a valid address for the zero-filled copies
+    const cplx* ptr;         // slot 0 of the next k-block
+    long long slot_step;     // elements from slot i to slot i + 1
+    long long kstep;         // elements from one k-block to the next
+    unsigned soff;           // KC: shared-memory element offset of slot 0
+    unsigned okmask;         // KC: bit i = row of slot i exists; MC: bit 0 = column exists
+    int kin;                 // KC: kc; MC: k_0 (position inside the k-block)
+    int rcol;                // MC: r
+
+    __device__ __forceinline__ void init(const cplx* g, int ld, int r0, int rmax, int tid) {
+        base = g;
+        if (KC) {
+            const int kc = tid & (BK - 1), r = tid / BK;
+            kin = kc; rcol = 0;
+            ptr = g + (size_t)(r0 + r) * ld + kc;
+            slot_step = (long long)RS * ld; kstep = BK;
+            soff = r * BK + (kc ^ ((r & 1) << 2));
+            okmask = 0u;
+#pragma unroll
+            for (int i = 0; i < ITER; i++) okmask |= (r0 + r + i * RS < rmax ? 1u : 0u) << i;
+        } else {
+            const int r = tid % R, k = tid / R;
+            kin = k; rcol = r;
+            ptr = g + (size_t)k * ld + (r0 + r);
+            slot_step = (long long)RS * ld; kstep = (long long)BK * ld;
+            soff = 0u;
+            okmask = r0 + r < rmax ? 1u : 0u;
+        }
+    }
+    // loads of the k-block starting at k0 into the stage at sm; then points at the next k-block
+    __device__ __forceinline__ void issue(cplx* sm, int k0, int kmax) {
+        const cplx* p = ptr;
+        if (KC) {
+            const bool kok = k0 + kin < kmax;
+#pragma unroll
+            for (int i = 0; i < ITER; i++) {
+                const bool ok = kok && ((okmask >> i) & 1u);
+                cp_async16(sm + soff + i * RS * BK, ok ? p : base, ok);
+                p += slot_step;
+            }
+        } else {
+#pragma unroll
+            for (int i = 0; i < ITER; i++) {
+                const int k = kin + i * RS;
+                const bool ok = okmask && (k0 + k < kmax);
+                cp_async16(sm + k * R + (rcol ^ ((k & 3) << 1)), ok ? p : base, ok);
+                p += slot_step;
+            }
+        }
+        ptr += kstep;
+    }
+};
+
+// n / d for n < 2^31 without a division: d = the divisor, (mul, sh) from GemmDiv::set on the host
+__device__ __forceinline__ unsigned fastdiv(unsigned n, unsigned mul, unsigned sh) { return (__umulhi(n, mul) + n) >> sh; }
+
+struct GemmDiv {
+    unsigned tiles_n, tn_mul, tn_sh, batch, b_mul, b_sh;
+    static void magic(unsigned d, unsigned& mul, unsigned& sh) {
+        sh = 0; while ((1u << sh) < d) sh++;
+        mul = (unsigned)(((unsigned long long)((1ull << sh) - d) << 32) / d + 1);
+    }
+    void set(unsigned tn, unsigned bt) { tiles_n = tn; batch = bt; magic(tn, tn_mul, tn_sh); magic(bt, b_mul, b_sh); }
+};
+
 template <int OPA, int OPB, int BM, int BN, int WM, int WN, int MINB>
-__global__ void __launch_bounds__(WM * WN * 32, MINB) zgemm_kernel(const __grid_constant__ GemmGroup grp) {
+__global__ void __launch_bounds__(WM * WN * 32, MINB) zgemm_kernel(const __grid_constant__ GemmGroup grp,
+                                                                   const __grid_constant__ GemmDiv dv) {
     const GemmArgs& a = grp.g[blockIdx.z];
     constexpr int NT = WM * WN * 32;
     constexpr int STAGES = StagesFor<BM>::value;
@@ -83,10 +159,9 @@ __global__ void __launch_bounds__(WM * WN * 32, MINB) zgemm_kernel(const __grid_
     cplx* sA = reinterpret_cast<cplx*>(smem_raw);              // STAGES x BM x BK
     cplx* sB = sA + STAGES * BM * BK;                          // STAGES x BN x BK
 
-    const int e = blockIdx.y % a.batch, e2 = blockIdx.y / a.batch;
+    const unsigned e2 = fastdiv(blockIdx.y, dv.b_mul, dv.b_sh), e = blockIdx.y - e2 * dv.batch;
     if (a.skip && a.skip[e]) return;
-    const int tiles_n = (a.n + BN - 1) / BN;
-    const int tm = blockIdx.x / tiles_n, tn = blockIdx.x % tiles_n;
+    const unsigned tm = fastdiv(blockIdx.x, dv.tn_mul, dv.tn_sh), tn = blockIdx.x - tm * dv.tiles_n;
     const int m0 = tm * BM, n0 = tn * BN;
     const cplx* gA = a.A + (size_t)e * a.sA + (size_t)e2 * a.sA2;
     const cplx* gB = a.B + (size_t)e * a.sB + (size_t)e2 * a.sB2;
@@ -100,26 +175,32 @@ __global__ void __launch_bounds__(WM * WN * 32, MINB) zgemm_kernel(const __grid_
 #pragma unroll
         for (int j = 0; j < NI; j++) { cre[i][j][0] = cre[i][j][1] = cim[i][j][0] = cim[i][j][1] = 0.0; }
 
-    const int KB = (a.k + BK - 1) / BK;
-    auto issue = [&](int kb) {
-        if (kb < KB) {
-            int st = kb % STAGES, k0 = kb * BK;
-            if (OPA == 0) load_tile_kc<BM, NT>(sA + st * BM * BK, gA, a.lda, m0, k0, a.m, a.k, tid);
-            else          load_tile_mc<BM, NT>(sA + st * BM * BK, gA, a.lda, m0, k0, a.m, a.k, tid);
-            if (OPB == 0) load_tile_mc<BN, NT>(sB + st * BN * BK, gB, a.ldb, n0, k0, a.n, a.k, tid);
-            else          load_tile_kc<BN, NT>(sB + st * BN * BK, gB, a.ldb, n0, k0, a.n, a.k, tid);
+    const int KB = (a.k + BK - 1) / BK, kmax = a.k;
+    TileLoader<BM, NT, OPA == 0> ldA;
+    TileLoader<BN, NT, OPB != 0> ldB;
+    ldA.init(gA, a.lda, m0, a.m, tid);
+    ldB.init(gB, a.ldb, n0, a.n, tid);
+    int st_issue = 0, kb_issue = 0;          // stage and k-block of the next loads (issued in order)
+    auto issue = [&]() {
+        if (kb_issue < KB) {
+            ldA.issue(sA + st_issue * BM * BK, kb_issue * BK, kmax);
+            ldB.issue(sB + st_issue * BN * BK, kb_issue * BK, kmax);
         }
         cp_async_commit();
+        kb_issue++;
+        st_issue = st_issue + 1 == STAGES ? 0 : st_issue + 1;
     };
 #pragma unroll
-    for (int s = 0; s < STAGES - 1; s++) issue(s);
+    for (int s = 0; s < STAGES - 1; s++) issue();
 
+    int st = 0;
     for (int kb = 0; kb < KB; kb++) {
         cp_async_wait<STAGES - 2>();
         __syncthreads();
-        issue(kb + STAGES - 1);
-        const cplx* tA = sA + (kb % STAGES) * BM * BK;
-        const cplx* tB = sB + (kb % STAGES) * BN * BK;
+        issue();
+        const cplx* tA = sA + st * BM * BK;
+        const cplx* tB = sB + st * BN * BK;
+        st = st + 1 == STAGES ? 0 : st + 1;
 #pragma unroll
         for (int ks = 0; ks < BK / 4; ks++) {
             const int k = ks * 4 + lk;
@@ -153,25 +234,32 @@ __global__ void __launch_bounds__(WM * WN * 32, MINB) zgemm_kernel(const __grid_
     }
     cp_async_wait<0>();
 
-    // epilogue: C = alpha*acc + beta*D
-    cplx* gC = a.C + (size_t)e * a.sC + (size_t)e2 * a.sC2;
+    // epilogue: C = alpha*acc + beta*D; a thread holds two adjacent columns of each 8x8 sub-tile
+    const size_t eoff = (size_t)e * a.sC + (size_t)e2 * a.sC2;
+    cplx* gC = a.C + eoff;
     const cplx* gD = a.D ? a.D + (size_t)e * a.sD + (size_t)e2 * a.sD2 : nullptr;
     const cplx al = a.alpha_vec ? cmul(a.alpha, a.alpha_vec[e]) : a.alpha, be = a.beta;
+    const int col0 = n0 + wn0 + lk * 2, ncol = a.n;
 #pragma unroll
     for (int i = 0; i < MI; i++) {
-        int row = m0 + wm0 + i * 8 + lr;
+        const int row = m0 + wm0 + i * 8 + lr;
         if (row >= a.m) continue;
+        const size_t roff = (size_t)row * a.ldc + col0;
+        cplx* crow = gC + roff;
+        const cplx* drow = gD ? gD + roff : nullptr;
 #pragma unroll
         for (int j = 0; j < NI; j++) {
-#pragma unroll
-            for (int q = 0; q < 2; q++) {
-                int col = n0 + wn0 + j * 8 + lk * 2 + q;
-                if (col >= a.n) continue;
-                cplx acc = cmake(cre[i][j][q], cim[i][j][q]);
-                cplx r = cmul(al, acc);
-                if (gD) { cplx d = gD[(size_t)row * a.ldc + col]; cfma(r, be, d); }
-                gC[(size_t)row * a.ldc + col] = r;
+            const int col = col0 + j * 8;
+            if (col >= ncol) continue;
+            const bool two = col + 1 < ncol;
+            cplx r0 = cmul(al, cmake(cre[i][j][0], cim[i][j][0]));
+            cplx r1 = cmul(al, cmake(cre[i][j][1], cim[i][j][1]));
+            if (drow) {
+                cfma(r0, be, drow[j * 8]);
+                if (two) cfma(r1, be, drow[j * 8 + 1]);
             }
+            crow[j * 8] = r0;
+            if (two) crow[j * 8 + 1] = r1;
         }
     }
 }
@@ -300,9 +388,12 @@ int launch_cfg(negf_ctx* ctx, const GemmGroup& grp) {
     const GemmArgs& a = grp.g[0];
     auto kern = zgemm_kernel<OPA, OPB, BM, BN, WM, WN, MINB>;
     constexpr int smem = StagesFor<BM>::value * (BM + BN) * BK * (int)sizeof(cplx);
-    int tiles = ((a.m + BM - 1) / BM) * ((a.n + BN - 1) / BN);
+    const int tiles_n = (a.n + BN - 1) / BN;
+    int tiles = ((a.m + BM - 1) / BM) * tiles_n;
     dim3 grid(tiles, a.batch * a.batch2, grp.ng);
-    kern<<<grid, WM * WN * 32, smem, ctx->stream>>>(grp);
+    GemmDiv dv;
+    dv.set((unsigned)tiles_n, (unsigned)a.batch);
+    kern<<<grid, WM * WN * 32, smem, ctx->stream>>>(grp, dv);
     NEGF_LAUNCH_CHECK(ctx);
     return NEGF_OK;
 }
