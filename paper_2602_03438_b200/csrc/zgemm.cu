@@ -23,9 +23,12 @@
 namespace {
 
 constexpr int BK = 16;
-// pipeline depth.  Measured on configs[1] (b = 64, 32x32 tiles): 2 / 3 / 4 / 5 stages give 8.77 / 8.68 /
-// 8.80 / 9.47 ms per step - more stages cost CTAs per SM, which matters more than load latency.
+// pipeline depth.  Measured on configs[1] (b = 64, 32x32 tiles) with the first kernel (122 registers, at most
+// 4 CTAs/SM): 2 / 3 / 4 / 5 stages gave 8.77 / 8.68 / 8.80 / 9.47 ms per step - more stages cost CTAs per SM,
+// which matters more than load latency.  With the per-CTA load state (84-88 registers) two stages of the
+// 32x32 tiles let five CTAs share an SM: 6.63 -> 6.55 ms (six CTAs: 6.61).
 template <int BM> struct StagesFor { static constexpr int value = 3; };
+template <> struct StagesFor<32> { static constexpr int value = 2; };
 
 __device__ __forceinline__ void dmma(double& c0, double& c1, double a, double b) {
     asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
@@ -425,7 +428,7 @@ cudaError_t prepare_cfg() {
 int zgemm_prepare(negf_ctx* ctx) {
     NEGF_CUDA_CHECK(ctx, (prepare_cfg<128, 64, 4, 2, 1>()));
     NEGF_CUDA_CHECK(ctx, (prepare_cfg<64, 64, 2, 2, 2>()));
-    NEGF_CUDA_CHECK(ctx, (prepare_cfg<32, 32, 2, 2, 3>()));
+    NEGF_CUDA_CHECK(ctx, (prepare_cfg<32, 32, 2, 2, 5>()));
     {
         constexpr int smem = 3 * (128 + M3_BN) * BK * (int)sizeof(cplx);
         NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(zgemm3m_kernel<0, 0, 128, M3_BN, 4, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
@@ -465,7 +468,7 @@ int zgemm_launch_group(negf_ctx* ctx, const GemmGroup& grp) {
     // blocks up to 64 x 64: four 32x32 CTAs per product balance the SMs better than one 64x64 CTA
     // (measured 5-7 % faster at b = 64 for 128 .. 512 products per launch)
     if ((a.m > 64 || a.n > 64) && t64 >= ctx->num_sms) return launch_ops<64, 64, 2, 2, 2>(ctx, grp);
-    return launch_ops<32, 32, 2, 2, 3>(ctx, grp);
+    return launch_ops<32, 32, 2, 2, 5>(ctx, grp);
 }
 
 int zgemm_launch(negf_ctx* ctx, const GemmArgs& a) {
