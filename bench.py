@@ -384,6 +384,8 @@ def run_e2e(args, wl, ctx, dev, world, torch, negf):
     dt = time.perf_counter() - t0
     assert int(hp.out["info"].abs().sum()) == 0, "numerical failure flagged in the e2e run"
     # same call with the G block outputs NULL: only density, LDOS, T(E), currents and info cross PCIe on the way back
+    del hp                                   # its pinned buffers and device scratch first (configs[3-4] fill the box)
+    torch.cuda.empty_cache()
     ho = runner.HostPath(wl, ne, device=dev, ctx=ctx, blocks=False)
     for _ in range(2):
         up_o, down_o = ho.run()

@@ -273,7 +273,8 @@ __global__ void __launch_bounds__(WM * WN * 32, MINB) zgemm_kernel(const __grid_
 // part is accurate norm-wise (|dIm| <~ eps (|Ar|+|Ai|)(|Br|+|Bi|)), far inside the 1e-10 bar.  Three
 // accumulator sets cost registers, hence 32x24 warp tiles (128x48 CTA tiles, 8 warps).
 template <int OPA, int OPB, int BM, int BN, int WM, int WN>
-__global__ void __launch_bounds__(WM * WN * 32, 1) zgemm3m_kernel(const __grid_constant__ GemmGroup grp) {
+__global__ void __launch_bounds__(WM * WN * 32, 1) zgemm3m_kernel(const __grid_constant__ GemmGroup grp,
+                                                                  const __grid_constant__ GemmDiv dv) {
     const GemmArgs& a = grp.g[blockIdx.z];
     constexpr int NT = WM * WN * 32;
     constexpr int STAGES = 3;
@@ -283,10 +284,9 @@ __global__ void __launch_bounds__(WM * WN * 32, 1) zgemm3m_kernel(const __grid_c
     cplx* sA = reinterpret_cast<cplx*>(smem_raw);
     cplx* sB = sA + STAGES * BM * BK;
 
-    const int e = blockIdx.y % a.batch, e2 = blockIdx.y / a.batch;
+    const unsigned e2 = fastdiv(blockIdx.y, dv.b_mul, dv.b_sh), e = blockIdx.y - e2 * dv.batch;
     if (a.skip && a.skip[e]) return;
-    const int tiles_n = (a.n + BN - 1) / BN;
-    const int tm = blockIdx.x / tiles_n, tn = blockIdx.x % tiles_n;
+    const unsigned tm = fastdiv(blockIdx.x, dv.tn_mul, dv.tn_sh), tn = blockIdx.x - tm * dv.tiles_n;
     const int m0 = tm * BM, n0 = tn * BN;
     const cplx* gA = a.A + (size_t)e * a.sA + (size_t)e2 * a.sA2;
     const cplx* gB = a.B + (size_t)e * a.sB + (size_t)e2 * a.sB2;
@@ -302,26 +302,36 @@ __global__ void __launch_bounds__(WM * WN * 32, 1) zgemm3m_kernel(const __grid_c
 #pragma unroll
             for (int q = 0; q < 2; q++) { p1[i][j][q] = 0.0; p2[i][j][q] = 0.0; p3[i][j][q] = 0.0; }
 
-    const int KB = (a.k + BK - 1) / BK;
-    auto issue = [&](int kb) {
-        if (kb < KB) {
-            int st = kb % STAGES, k0 = kb * BK;
-            if (OPA == 0) load_tile_kc<BM, NT>(sA + st * BM * BK, gA, a.lda, m0, k0, a.m, a.k, tid);
-            else          load_tile_mc<BM, NT>(sA + st * BM * BK, gA, a.lda, m0, k0, a.m, a.k, tid);
-            if (OPB == 0) load_tile_mc<BN, NT>(sB + st * BN * BK, gB, a.ldb, n0, k0, a.n, a.k, tid);
-            else          load_tile_kc<BN, NT>(sB + st * BN * BK, gB, a.ldb, n0, k0, a.n, a.k, tid);
+    const int KB = (a.k + BK - 1) / BK, kmax = a.k;
+    // B tiles of 48 columns do not divide evenly over the threads in the mn-contiguous layout: old loaders there
+    constexpr bool FAST_B = (OPB != 0) ? (NT % BK == 0 && (NT / BK) % 2 == 0 && BN * BK % NT == 0) : (NT % BN == 0 && BN * BK % NT == 0);
+    TileLoader<BM, NT, OPA == 0> ldA;
+    ldA.init(gA, a.lda, m0, a.m, tid);
+    TileLoader<FAST_B ? BN : NT, NT, OPB != 0> ldB;
+    if (FAST_B) ldB.init(gB, a.ldb, n0, a.n, tid);
+    int st_issue = 0, kb_issue = 0;
+    auto issue = [&]() {
+        if (kb_issue < KB) {
+            ldA.issue(sA + st_issue * BM * BK, kb_issue * BK, kmax);
+            if (FAST_B) ldB.issue(sB + st_issue * BN * BK, kb_issue * BK, kmax);
+            else if (OPB == 0) load_tile_mc<BN, NT>(sB + st_issue * BN * BK, gB, a.ldb, n0, kb_issue * BK, a.n, a.k, tid);
+            else               load_tile_kc<BN, NT>(sB + st_issue * BN * BK, gB, a.ldb, n0, kb_issue * BK, a.n, a.k, tid);
         }
         cp_async_commit();
+        kb_issue++;
+        st_issue = st_issue + 1 == STAGES ? 0 : st_issue + 1;
     };
 #pragma unroll
-    for (int s = 0; s < STAGES - 1; s++) issue(s);
+    for (int s = 0; s < STAGES - 1; s++) issue();
 
+    int st = 0;
     for (int kb = 0; kb < KB; kb++) {
         cp_async_wait<STAGES - 2>();
         __syncthreads();
-        issue(kb + STAGES - 1);
-        const cplx* tA = sA + (kb % STAGES) * BM * BK;
-        const cplx* tB = sB + (kb % STAGES) * BN * BK;
+        issue();
+        const cplx* tA = sA + st * BM * BK;
+        const cplx* tB = sB + st * BN * BK;
+        st = st + 1 == STAGES ? 0 : st + 1;
 #pragma unroll
         for (int ks = 0; ks < BK / 4; ks++) {
             const int k = ks * 4 + lk;
@@ -353,21 +363,27 @@ __global__ void __launch_bounds__(WM * WN * 32, 1) zgemm3m_kernel(const __grid_c
     cplx* gC = a.C + (size_t)e * a.sC + (size_t)e2 * a.sC2;
     const cplx* gD = a.D ? a.D + (size_t)e * a.sD + (size_t)e2 * a.sD2 : nullptr;
     const cplx al = a.alpha_vec ? cmul(a.alpha, a.alpha_vec[e]) : a.alpha, be = a.beta;
+    const int col0 = n0 + wn0 + lk * 2, ncol = a.n;
 #pragma unroll
     for (int i = 0; i < MI; i++) {
-        int row = m0 + wm0 + i * 8 + lr;
+        const int row = m0 + wm0 + i * 8 + lr;
         if (row >= a.m) continue;
+        const size_t roff = (size_t)row * a.ldc + col0;
+        cplx* crow = gC + roff;
+        const cplx* drow = gD ? gD + roff : nullptr;
 #pragma unroll
         for (int j = 0; j < NI; j++) {
-#pragma unroll
-            for (int q = 0; q < 2; q++) {
-                int col = n0 + wn0 + j * 8 + lk * 2 + q;
-                if (col >= a.n) continue;
-                cplx acc = cmake(p1[i][j][q] - p2[i][j][q], (p3[i][j][q] - p1[i][j][q]) - p2[i][j][q]);
-                cplx r = cmul(al, acc);
-                if (gD) { cplx d = gD[(size_t)row * a.ldc + col]; cfma(r, be, d); }
-                gC[(size_t)row * a.ldc + col] = r;
+            const int col = col0 + j * 8;
+            if (col >= ncol) continue;
+            const bool two = col + 1 < ncol;
+            cplx r0 = cmul(al, cmake(p1[i][j][0] - p2[i][j][0], (p3[i][j][0] - p1[i][j][0]) - p2[i][j][0]));
+            cplx r1 = cmul(al, cmake(p1[i][j][1] - p2[i][j][1], (p3[i][j][1] - p1[i][j][1]) - p2[i][j][1]));
+            if (drow) {
+                cfma(r0, be, drow[j * 8]);
+                if (two) cfma(r1, be, drow[j * 8 + 1]);
             }
+            crow[j * 8] = r0;
+            if (two) crow[j * 8 + 1] = r1;
         }
     }
 }
@@ -379,9 +395,12 @@ int launch_3m(negf_ctx* ctx, const GemmGroup& grp) {
     constexpr int BM = 128, BN = M3_BN, WM = 4, WN = 2;
     const GemmArgs& a = grp.g[0];
     constexpr int smem = 3 * (BM + BN) * BK * (int)sizeof(cplx);
-    int tiles = ((a.m + BM - 1) / BM) * ((a.n + BN - 1) / BN);
+    const int tiles_n = (a.n + BN - 1) / BN;
+    int tiles = ((a.m + BM - 1) / BM) * tiles_n;
     dim3 grid(tiles, a.batch * a.batch2, grp.ng);
-    zgemm3m_kernel<OPA, OPB, BM, BN, WM, WN><<<grid, WM * WN * 32, smem, ctx->stream>>>(grp);
+    GemmDiv dv;
+    dv.set((unsigned)tiles_n, (unsigned)a.batch);
+    zgemm3m_kernel<OPA, OPB, BM, BN, WM, WN><<<grid, WM * WN * 32, smem, ctx->stream>>>(grp, dv);
     NEGF_LAUNCH_CHECK(ctx);
     return NEGF_OK;
 }
