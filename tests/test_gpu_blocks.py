@@ -47,8 +47,9 @@ def test_zgemm_batched(ctx, m, n, k, opA, opB):
     assert np.linalg.norm(dC2.cpu().numpy() - ref2) / np.linalg.norm(ref2) < 1e-13
 
 
-@pytest.mark.parametrize("b", [1, 2, 7, 16, 33, 64, 96, 97, 130, 256, 300, 515])
+@pytest.mark.parametrize("b", [1, 2, 7, 16, 33, 64, 96, 97, 130, 256, 300, 515, 1100, 2100])
 def test_zinverse_batched(ctx, negf_lib, b):
+    """2100 > 2048 rows: the first panels take the shared-memory cluster panel kernel instead of the register one."""
     import torch
     rng = np.random.default_rng(b)
     batch = 3 if b < 400 else 2
