@@ -479,24 +479,26 @@ __global__ void __launch_bounds__(PNL_WARPS * 32) gj_panel_reg_kernel(PanelArgs 
         key = __shfl_sync(0xffffffffu, key, j);
         row = __shfl_sync(0xffffffffu, row, j);
         {   // this warp's candidate row (and the current diagonal row, if it lives here) go to shared memory
-            cplx v = cmake(0.0, 0.0), dv = cmake(0.0, 0.0);
+            cplx v = cmake(0.0, 0.0);
 #pragma unroll
-            for (int r = 0; r < R; r++) {
+            for (int r = 0; r < R; r++)
                 if (row0 + r == row) v = P[r];
-                if (row0 + r == j) dv = P[r];
-            }
             S.wrows[warp][lane] = v;
-            if (j >= row0 && j < row0 + R) S.drowstage[lane] = dv;
+            if (j >= row0 && j < row0 + R) {           // warp-uniform: only the warp that holds row j
+                cplx dv = cmake(0.0, 0.0);
+#pragma unroll
+                for (int r = 0; r < R; r++)
+                    if (row0 + r == j) dv = P[r];
+                S.drowstage[lane] = dv;
+            }
             if (lane == 0) { S.red_key[warp] = key; S.red_row[warp] = row; }
         }
         __syncthreads();
         if (warp == 0) {       // CTA candidate; push (key, row, row content) to every CTA; CTA 0 also the diagonal row
-            unsigned long long bk = 0ull; int br = PNL_NONE, bw = 0;
-#pragma unroll
-            for (int q = 0; q < PNL_WARPS; q++) {
-                const unsigned long long k2 = S.red_key[q]; const int r2 = S.red_row[q];
-                if (r2 != PNL_NONE && (br == PNL_NONE || k2 > bk)) { bk = k2; br = r2; bw = q; }   // rows ascend with q
-            }
+            // lane q holds warp q's candidate; argmax by three redux.sync (ties: the smallest row, as rows ascend with q)
+            unsigned long long bk = 0ull; int br = PNL_NONE;
+            warp_best(lane < PNL_WARPS ? S.red_key[lane] : 0ull, lane < PNL_WARPS ? S.red_row[lane] : PNL_NONE, bk, br);
+            const int bw = br == PNL_NONE ? 0 : br / R - rank * PNL_WARPS;
             const cplx myrow = S.wrows[bw][lane];
             const cplx drow = S.drowstage[lane];
             if (C == 1) {
@@ -529,13 +531,18 @@ __global__ void __launch_bounds__(PNL_WARPS * 32) gj_panel_reg_kernel(PanelArgs 
         const cplx pjv = S.candrow[par][wq][j];
         const cplx rinv = sing ? cmake(0.0, 0.0) : crecip_fast(pjv);
         const cplx dgl = S.diagrow[par][lane];
+        // exchange rows j <-> prow: warp-uniform, only the (at most two) warps that hold one of them
+        if (prow != j && ((prow >= row0 && prow < row0 + R) || (j >= row0 && j < row0 + R))) {
 #pragma unroll
-        for (int r = 0; r < R; r++) {
-            const int gr = row0 + r;
-            if (prow != j) {                                       // exchange rows j <-> prow
+            for (int r = 0; r < R; r++) {
+                const int gr = row0 + r;
                 if (gr == prow) P[r] = dgl;
                 else if (gr == j) P[r] = prl;
             }
+        }
+#pragma unroll
+        for (int r = 0; r < R; r++) {
+            const int gr = row0 + r;
             if (gr > j && gr < rows_total) {                       // eliminate below (warp-uniform test)
                 cplx pj;
                 pj.x = __shfl_sync(0xffffffffu, P[r].x, j);
