@@ -443,6 +443,96 @@ __device__ __forceinline__ void warp_best(unsigned long long key, int row, unsig
 
 inline size_t reg_panel_smem_bytes(int R) { return sizeof(RegPanelSmem) + (size_t)PNL_WARPS * R * PW * sizeof(cplx); }
 
+// Triangular inverses of the factored w x w diagonal block S.Dm = L11 \\ U11 by one warp each, lane = column c,
+// the column held in registers: row r of the result needs rows k < r (k > r) of the same column, so the sums run
+// over registers and broadcast reads of the factor, fully unrolled (the entries outside the triangles come out
+// as exact zeros).  S.Li / S.Ui are zero-initialised by the caller.
+__device__ __noinline__ void panel_tri_lower(RegPanelSmem& S, int w, int lane) {     // L11^-1 (unit lower)
+    constexpr int H = PW / 2;
+    // rows 0 .. 15 of column `lane` in registers; then rows 16 .. 31, which read the first half back from
+    // shared memory (16 registers of column at a time keep the whole thing inside the register budget)
+    {
+        cplx li[H];
+#pragma unroll
+        for (int r = 0; r < H; r++) {
+            li[r] = cmake(0.0, 0.0);
+            if (r < w) {
+                cplx s0 = cmake(r == lane ? 1.0 : 0.0, 0.0), s1 = cmake(0.0, 0.0);
+#pragma unroll
+                for (int k = 0; k < r; k++) {
+                    if (k & 1) cfms(s1, S.Dm[r * PW + k], li[k]); else cfms(s0, S.Dm[r * PW + k], li[k]);
+                }
+                li[r] = cadd(s0, s1);
+                S.Li[r * PW + lane] = li[r];
+            }
+        }
+    }
+    __syncwarp();
+    cplx lj[H];
+#pragma unroll
+    for (int r = H; r < PW; r++) {
+        lj[r - H] = cmake(0.0, 0.0);
+        if (r < w) {
+            cplx s0 = cmake(r == lane ? 1.0 : 0.0, 0.0), s1 = cmake(0.0, 0.0);
+#pragma unroll
+            for (int k = 0; k < H; k++) {
+                if (k & 1) cfms(s1, S.Dm[r * PW + k], S.Li[k * PW + lane]); else cfms(s0, S.Dm[r * PW + k], S.Li[k * PW + lane]);
+            }
+#pragma unroll
+            for (int k = H; k < r; k++) {
+                if (k & 1) cfms(s1, S.Dm[r * PW + k], lj[k - H]); else cfms(s0, S.Dm[r * PW + k], lj[k - H]);
+            }
+            lj[r - H] = cadd(s0, s1);
+            S.Li[r * PW + lane] = lj[r - H];
+        }
+    }
+}
+__device__ __noinline__ void panel_tri_upper(RegPanelSmem& S, int w, int lane) {     // U11^-1
+    constexpr int H = PW / 2;
+    {
+        const cplx ur = S.Dm[lane * PW + lane];
+        S.drowstage[lane] = (lane >= w || (ur.x == 0.0 && ur.y == 0.0)) ? cmake(0.0, 0.0) : crecip(ur);
+    }
+    __syncwarp();
+    // rows 31 .. 16 first (registers), then rows 15 .. 0 with the upper half read back from shared memory;
+    // Dm[r][k] = 0 for k >= w and Ui is zero-initialised, so the fixed ranges are right for w < 32 too
+    {
+        cplx ui[H];
+#pragma unroll
+        for (int r = PW - 1; r >= H; r--) {
+            ui[r - H] = cmake(0.0, 0.0);
+            if (r < w) {
+                cplx s0 = cmake(r == lane ? 1.0 : 0.0, 0.0), s1 = cmake(0.0, 0.0);
+#pragma unroll
+                for (int k = r + 1; k < PW; k++) {
+                    if (k & 1) cfms(s1, S.Dm[r * PW + k], ui[k - H]); else cfms(s0, S.Dm[r * PW + k], ui[k - H]);
+                }
+                ui[r - H] = cmul(cadd(s0, s1), S.drowstage[r]);
+                S.Ui[r * PW + lane] = ui[r - H];
+            }
+        }
+    }
+    __syncwarp();
+    cplx uj[H];
+#pragma unroll
+    for (int r = H - 1; r >= 0; r--) {
+        uj[r] = cmake(0.0, 0.0);
+        if (r < w) {
+            cplx s0 = cmake(r == lane ? 1.0 : 0.0, 0.0), s1 = cmake(0.0, 0.0);
+#pragma unroll
+            for (int k = H; k < PW; k++) {
+                if (k & 1) cfms(s1, S.Dm[r * PW + k], S.Ui[k * PW + lane]); else cfms(s0, S.Dm[r * PW + k], S.Ui[k * PW + lane]);
+            }
+#pragma unroll
+            for (int k = r + 1; k < H; k++) {
+                if (k & 1) cfms(s1, S.Dm[r * PW + k], uj[k]); else cfms(s0, S.Dm[r * PW + k], uj[k]);
+            }
+            uj[r] = cmul(cadd(s0, s1), S.drowstage[r]);
+            S.Ui[r * PW + lane] = uj[r];
+        }
+    }
+}
+
 template <int R>
 __global__ void __launch_bounds__(PNL_WARPS * 32) gj_panel_reg_kernel(PanelArgs a) {
     constexpr int NT = PNL_WARPS * 32;
@@ -554,43 +644,24 @@ __global__ void __launch_bounds__(PNL_WARPS * 32) gj_panel_reg_kernel(PanelArgs 
         }
     }
 
-    // CTA 0: L11^-1 and U11^-1 from the w x w diagonal block, one thread per column; then
+    // every warp parks its rows in its own shared-memory lines now (read back for P' below), so that the
+    // panel registers are free during the triangular inverses
+    cplx* Lr = S.Lrow + (size_t)warp * R * PW;
+#pragma unroll
+    for (int r = 0; r < R; r++) Lr[r * PW + lane] = P[r];
+    __syncwarp();
+    // CTA 0: L11^-1 and U11^-1 from the w x w diagonal block, one warp each; then
     // (L11 U11)^-1 = U11^-1 L11^-1; L11^-1 goes to every CTA of the cluster.
     if (rank == 0) {
         for (int idx = tid; idx < PW * PW; idx += NT) { S.Li[idx] = cmake(0.0, 0.0); S.Ui[idx] = cmake(0.0, 0.0); }
 #pragma unroll
         for (int r = 0; r < R; r++)
-            if (row0 + r < PW) S.Dm[(row0 + r) * PW + lane] = P[r];
+            if (row0 + r < PW) S.Dm[(row0 + r) * PW + lane] = Lr[r * PW + lane];
         __syncthreads();
-        // (Li and Ui are zero outside their triangles, so the sums run over fixed, unrolled ranges
-        // with four independent accumulators instead of a dependent load -> FMA chain)
-        if (tid < w) {
-            const int c = tid;
-            for (int r = 0; r < w; r++) {
-                cplx s0 = (r == c) ? cmake(1.0, 0.0) : cmake(0.0, 0.0), s1 = cmake(0.0, 0.0), s2 = s1, s3 = s1;
-                for (int k = 0; k < r; k += 4) {
-                    cfms(s0, S.Dm[r * PW + k], S.Li[k * PW + c]);
-                    if (k + 1 < r) cfms(s1, S.Dm[r * PW + k + 1], S.Li[(k + 1) * PW + c]);
-                    if (k + 2 < r) cfms(s2, S.Dm[r * PW + k + 2], S.Li[(k + 2) * PW + c]);
-                    if (k + 3 < r) cfms(s3, S.Dm[r * PW + k + 3], S.Li[(k + 3) * PW + c]);
-                }
-                S.Li[r * PW + c] = (r < c) ? cmake(0.0, 0.0) : cadd(cadd(s0, s1), cadd(s2, s3));
-            }
-        } else if (tid >= 32 && tid < 32 + w) {
-            const int c = tid - 32;
-            for (int r = w - 1; r >= 0; r--) {
-                cplx s0 = (r == c) ? cmake(1.0, 0.0) : cmake(0.0, 0.0), s1 = cmake(0.0, 0.0), s2 = s1, s3 = s1;
-                for (int k = r + 1; k < w; k += 4) {
-                    cfms(s0, S.Dm[r * PW + k], S.Ui[k * PW + c]);
-                    if (k + 1 < w) cfms(s1, S.Dm[r * PW + k + 1], S.Ui[(k + 1) * PW + c]);
-                    if (k + 2 < w) cfms(s2, S.Dm[r * PW + k + 2], S.Ui[(k + 2) * PW + c]);
-                    if (k + 3 < w) cfms(s3, S.Dm[r * PW + k + 3], S.Ui[(k + 3) * PW + c]);
-                }
-                const cplx ur = S.Dm[r * PW + r];
-                const cplx inv = (ur.x == 0.0 && ur.y == 0.0) ? cmake(0.0, 0.0) : crecip(ur);
-                S.Ui[r * PW + c] = (r > c) ? cmake(0.0, 0.0) : cmul(cadd(cadd(s0, s1), cadd(s2, s3)), inv);
-            }
-        }
+        // triangular inverses by two warps (own functions, so that their register arrays do not weigh on the
+        // column loop's allocation)
+        if (warp == 0) panel_tri_lower(S, w, lane);
+        else if (warp == 1) panel_tri_upper(S, w, lane);
         __syncthreads();
         cplx* gD = a.Dinv + (size_t)e * PW * PW;
         for (int idx = tid; idx < w * w; idx += NT) {
@@ -607,10 +678,6 @@ __global__ void __launch_bounds__(PNL_WARPS * 32) gj_panel_reg_kernel(PanelArgs 
     }
     cluster.sync();
     // rows below the diagonal block: P' = -L21 L11^-1, written in place (lane = output column)
-    cplx* Lr = S.Lrow + (size_t)warp * R * PW;
-#pragma unroll
-    for (int r = 0; r < R; r++) Lr[r * PW + lane] = P[r];
-    __syncwarp();
 #pragma unroll 1
     for (int r = 0; r < R; r++) {
         const int gr = row0 + r;
