@@ -190,6 +190,7 @@ def run_gpu(args, rank, local_rank, world):
             with torch.cuda.stream(st):
                 gdp = runner.DevicePath(wl, lo, min(lo + per, wl.n_energy), device=dev, ctx=gctx)
             groups.append((gdp, st))
+            del gdp
         torch.cuda.synchronize()
     n_streams = max(1, len(groups))
     paths = {}
@@ -279,6 +280,7 @@ def run_gpu(args, rank, local_rank, world):
         out["config"]["note"] = "BT Sigma_S arrays of the first energy batch are reused for every batch"
 
     if rank == 0:
+        print(f"[bench] timed region: {step_ms:.3f} ms/step, {value:.4g} {UNIT}, {n_streams} stream(s)", file=sys.stderr, flush=True)
         # ---- roofline of the dominant kernel: profiled passes of the SAME step (event pairs around
         # every launch site, on the library's stream), separate from the throughput timing above
         peak = ctx.fp64_peak(300.0)
@@ -286,6 +288,12 @@ def run_gpu(args, rank, local_rank, world):
         # run the whole batch on ONE stream, plain launches)
         pstep, pctx = step, all_ctx
         if groups:
+            # the groups' buffers are released first: at large b a second resident copy of the batch does not fit
+            del dps
+            pctx = None
+            groups.clear(); all_ctx.clear()
+            import gc
+            gc.collect(); torch.cuda.empty_cache()
             pdp = runner.DevicePath(wl, 0, wl.n_energy, device=dev, ctx=ctx)
             pstep, pctx = pdp.run, [ctx]
             pstep(); torch.cuda.synchronize()
