@@ -114,6 +114,7 @@ int negf_set_workspace(negf_ctx* ctx, void* dev_ptr, size_t bytes);
  * 4M kernel is the one the FP64 roofline fraction is quoted on. */
 #define NEGF_OPT_GRAPH_LOOPS 1
 #define NEGF_OPT_GEMM_3M     2
+#define NEGF_OPT_INV_TENSOR  3
 int negf_set_option(negf_ctx* ctx, int option, int value);
 const char* negf_strerror(int code);
 /* cudaError_t of the last failing runtime call on this context (0 if none). */

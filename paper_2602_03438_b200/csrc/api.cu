@@ -26,7 +26,7 @@ extern "C" int negf_create(negf_ctx** out, int device) {
             cudaEventCreateWithFlags(&c->ev_join[k], cudaEventDisableTiming) != cudaSuccess) { delete c; return NEGF_ECUDA; }
     }
     if (cudaEventCreateWithFlags(&c->ev_aux, cudaEventDisableTiming) != cudaSuccess) { delete c; return NEGF_ECUDA; }
-    c->graph_loops = true; c->gemm_3m = false; c->obc_exec = nullptr;
+    c->graph_loops = true; c->gemm_3m = false; c->inv_tensor = 0; c->obc_exec = nullptr;
     for (int k = 0; k < NEGF_NGRAPH; k++) for (int q = 0; q < NEGF_GWAYS; q++) c->gslot[k][q] = {0ull, nullptr, 0, 0u};
     c->gtick = 0;
     if (cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) != cudaSuccess) { delete c; return NEGF_ECUDA; }
@@ -68,6 +68,7 @@ extern "C" int negf_set_option(negf_ctx* ctx, int option, int value) {
     if (!ctx) return NEGF_EINVAL;
     if (option == NEGF_OPT_GRAPH_LOOPS) { ctx->graph_loops = value != 0; return NEGF_OK; }
     if (option == NEGF_OPT_GEMM_3M) { ctx->gemm_3m = value != 0; return NEGF_OK; }
+    if (option == NEGF_OPT_INV_TENSOR) { ctx->inv_tensor = value; return NEGF_OK; }
     return NEGF_EINVAL;
 }
 extern "C" const char* negf_strerror(int code) {

@@ -32,6 +32,7 @@ struct negf_ctx {
     // cached device-driven WHILE graph of the Sancho-Rubio doublings (small blocks, obc.cu)
     bool graph_loops;             // negf_set_option(NEGF_OPT_GRAPH_LOOPS)
     bool gemm_3m;                 // negf_set_option(NEGF_OPT_GEMM_3M)
+    int inv_tensor;               // negf_set_option(NEGF_OPT_INV_TENSOR)
     // cached CUDA graphs of whole calls in the latency-bound regime (same arguments twice in a row
     // -> the second call is captured, later ones replay it); one slot per entry point
     struct GraphSlot { unsigned long long key; cudaGraphExec_t exec; long long launches; unsigned used; };

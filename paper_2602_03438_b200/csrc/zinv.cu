@@ -233,6 +233,311 @@ __global__ void __launch_bounds__(GJ_NW * 32) gj_reg_kernel(cplx* A, long long s
 }
 
 // ------------------------------------------------------------------------------------------------
+// small path, tensor-pipe variant: BLOCKED Gauss-Jordan inside one CTA (b <= 64), panel width 8.
+//   * the matrix (padded with the identity to N = 32 TM) lives in the DMMA accumulator layout of
+//     16 update warps (4 x 4 grid, warp tile 8 TM x 8 TM) AND as a copy in shared memory ("mirror",
+//     double-buffered), which is where the panel columns and the pivot rows are read from;
+//   * a 17th warp factorises the current 8-column panel on ALL N rows by in-place Gauss-Jordan with
+//     partial pivoting among the not yet used rows (lane = row, the 8 columns in registers, straight-
+//     line code: the pivot search + reciprocal of column j+1 are issued between the rank-1 updates of
+//     column j).  The 8 stored columns are the transform T (N x 8) of the panel;
+//   * all other columns then get ONE rank-8 update on the tensor pipe:
+//         C <- C (pivot rows zeroed) + T R,   R[j, :] = row p_j of the matrix before the panel,
+//     the panel columns themselves become T.  Two block barriers per panel instead of one per column.
+// Rows never move (implicit pivoting); the permutation is undone in the final scatter, as above.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void gjd_dmma(double& c0, double& c1, double a, double b) {
+    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+        : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+__device__ __forceinline__ double gjd_flip(double x) {
+    return __hiloint2double(__double2hiint(x) ^ 0x80000000, __double2loint(x));
+}
+
+constexpr int GJD_UW = 8;                      // update warps (2 x 4 grid); warp GJD_UW factorises the panels
+constexpr int GJD_NT = (GJD_UW + 1) * 32;      // 9 warps: at most 3 per scheduler partition -> up to 168 registers per thread
+template <int TM, int W> constexpr size_t gjd_smem_bytes() {
+    constexpr int N = 32 * TM, LD = N + 1;
+    return (size_t)2 * N * LD * sizeof(cplx) + (size_t)2 * N * W * sizeof(cplx) + 16 * sizeof(cplx) + (2 * N + 16 + 8 + 4) * sizeof(int);
+}
+
+// pivot of panel column C (global column k): p = row (warp-uniform), d = 1 / pivot (computed by every lane)
+template <int TM, int W, int C>
+__device__ __forceinline__ void gjd_search(const cplx (&x)[TM][W], unsigned used, int k, int b, int lane, int& p, cplx& d, int& sing_at) {
+    unsigned key = 0u;
+#pragma unroll
+    for (int r = 0; r < TM; r++) {
+        const int i = lane + 32 * r;
+        if (!((used >> r) & 1u) && ((i < b) == (k < b))) {
+            const unsigned hi = (unsigned)((unsigned long long)__double_as_longlong(cabs1(x[r][C])) >> 32);
+            key = max(key, (hi & 0xffffff80u) | (unsigned)(127 - i));
+        }
+    }
+    const unsigned kmax = __reduce_max_sync(0xffffffffu, key);
+    p = 127 - (int)(kmax & 127u);
+    const bool sing = (kmax >> 7) == 0u;
+    double vx = x[0][C].x, vy = x[0][C].y;
+#pragma unroll
+    for (int r = 1; r < TM; r++) if ((p >> 5) == r) { vx = x[r][C].x; vy = x[r][C].y; }
+    vx = __shfl_sync(0xffffffffu, vx, p & 31);
+    vy = __shfl_sync(0xffffffffu, vy, p & 31);
+    d = sing ? cmake(1.0, 0.0) : crecip_fast(cmake(vx, vy));
+    sing_at = (sing && sing_at == 0) ? k + 1 : sing_at;
+}
+
+// one Gauss-Jordan step of the panel (column J) + look-ahead search of column J+1
+template <int TM, int W, int J>
+__device__ __forceinline__ void gjd_panel_steps(cplx (&x)[TM][W], cplx (&rsc)[TM], unsigned& used, unsigned (&pm)[TM],
+                                                int& p, cplx& d, int& myp, int& sing_at, int k0, int b, int lane, cplx* prow_s) {
+    if constexpr (J < W) {
+        const int pl = p & 31, pr = p >> 5;
+        cplx* line = prow_s + (J & 1) * 8;
+#pragma unroll
+        for (int r = 0; r < TM; r++)
+            if (lane == pl && pr == r) {
+#pragma unroll
+                for (int c = 0; c < W; c++) line[c] = x[r][c];
+            }
+        myp = (lane == J) ? p : myp;
+#pragma unroll
+        for (int r = 0; r < TM; r++) if (pr == r) pm[r] |= 1u << pl;
+        __syncwarp();
+        // deferred scaling inside the panel: the registers of a pivot row keep the unscaled row (true value =
+        // rsc x register), so pivoted and unpivoted rows run the same update and the pivot row itself costs nothing
+        cplx mlt[TM];
+#pragma unroll
+        for (int r = 0; r < TM; r++) {
+            const bool isp = (lane == pl) && (pr == r);
+            const cplx t = cmul(x[r][J], d);
+            mlt[r] = isp ? cmake(0.0, 0.0) : t;
+            x[r][J] = isp ? cmake(1.0, 0.0) : cneg(t);
+            if (isp) { rsc[r] = d; used |= 1u << r; }
+        }
+        int pn = 0; cplx dn = cmake(1.0, 0.0);
+        if constexpr (J < W - 1) {
+            const cplx prn = line[J + 1];
+#pragma unroll
+            for (int r = 0; r < TM; r++) cfms(x[r][J + 1], mlt[r], prn);
+            gjd_search<TM, W, J + 1>(x, used, k0 + J + 1, b, lane, pn, dn, sing_at);
+        }
+#pragma unroll
+        for (int c = 0; c < W; c++) {
+            if (c == J || c == J + 1) continue;
+            const cplx prc = line[c];
+#pragma unroll
+            for (int r = 0; r < TM; r++) cfms(x[r][c], mlt[r], prc);
+        }
+        p = pn; d = dn;
+        gjd_panel_steps<TM, W, J + 1>(x, rsc, used, pm, p, d, myp, sing_at, k0, b, lane, prow_s);
+    }
+}
+
+__device__ __forceinline__ void gjd_bar_sync(int id, int count) { asm volatile("bar.sync %0, %1;" :: "r"(id), "r"(count) : "memory"); }
+__device__ __forceinline__ void gjd_bar_arrive(int id, int count) { __threadfence_block(); asm volatile("bar.arrive %0, %1;" :: "r"(id), "r"(count) : "memory"); }
+
+// Look-ahead: while the update warps apply panel K to the matrix, the panel warp already factorises
+// panel K+1.  For that the update warps FIRST bring the columns of panel K+1 up to date (one 8 x 8 row
+// tile per warp, accumulator taken from and written back to the mirror), signal the panel warp
+// (named barrier A) and only then update their own tiles (which repeats that tile bit for bit).
+// Named barriers: 1 = update warps only (mirror complete), 2/3 = T of panel K ready (panel warp
+// arrives, update warps wait), 4/5 = columns of panel K ready in the mirror (update warps arrive,
+// panel warp waits).  T, the pivot rows and their mask are double-buffered.
+// W = panel width (4 or 8): the narrow panel halves the sequential work of the panel warp per column
+// (W - 1 rank-1 column updates per step) at the price of twice as many update rounds.
+template <int TM, int W>
+__global__ void __launch_bounds__(GJD_NT, 1) gj_dmma_kernel(cplx* A, long long sA, int b, int* info, int code,
+                                                            const int* skip, const int* code_dev) {
+    // N = 32 TM rows; update warps in a 2 x 4 grid, warp tile (8 TR) x (8 TC) = TR x TC accumulator tiles
+    constexpr int N = 32 * TM, LD = N + 1, TR = 2 * TM, TC = TM, WC = 4, NRT = N / 8, UT = GJD_UW * 32;
+    constexpr int KS = W / 4, PPT = 8 / W;       // k-steps of a rank-W update; panels per 8-column tile
+    const int e = blockIdx.x;
+    if (skip && skip[e]) return;
+    extern __shared__ __align__(16) unsigned char gjd_smem[];
+    cplx* mir = (cplx*)gjd_smem;                 // [2][N][LD]
+    cplx* Tb = mir + 2 * N * LD;                 // [2][N][W]
+    cplx* prow_s = Tb + 2 * N * W;               // [2][8]
+    int* piv = (int*)(prow_s + 16);              // [N]
+    int* dest = piv + N;                         // [N]
+    int* prows = dest + N;                       // [2][8]
+    unsigned* pmask = (unsigned*)(prows + 16);   // [2][4]
+    int* s_sing = (int*)(pmask + 8);
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int g = lane >> 2, q = lane & 3, wr = (warp >> 2) & 1, wc = warp & 3;
+    const int row0 = 8 * TR * wr + g, col0 = 8 * TC * wc + 2 * q;     // + 8 tr, + 8 tc (+ h)
+    cplx* gA = A + (size_t)e * sA;
+    const int npanel = (b + W - 1) / W;
+    if (warp < GJD_UW) {
+#pragma unroll
+        for (int tr = 0; tr < TR; tr++)
+#pragma unroll
+            for (int tc = 0; tc < TC; tc++)
+#pragma unroll
+                for (int h = 0; h < 2; h++) {
+                    const int i = row0 + 8 * tr, j = col0 + 8 * tc + h;
+                    mir[i * LD + j] = (i < b && j < b) ? gA[(size_t)i * b + j] : cmake(i == j ? 1.0 : 0.0, 0.0);
+                }
+    }
+    if (tid == 0) *s_sing = 0;
+    __syncthreads();
+    if (warp == GJD_UW) {
+        // ---------------- panel warp ----------------
+        unsigned used = 0u;                      // bit r = my row lane + 32 r has been a pivot row
+        int sing_at = 0;
+#pragma unroll 1
+        for (int K = 0; K < npanel; K++) {
+            if (K > 0) gjd_bar_sync(4 + (K & 1), GJD_NT);
+            const cplx* mc = mir + (K & 1) * N * LD;
+            cplx x[TM][W], rsc[TM];
+            unsigned pm[TM];
+#pragma unroll
+            for (int r = 0; r < TM; r++) {
+                rsc[r] = cmake(1.0, 0.0); pm[r] = 0u;
+#pragma unroll
+                for (int c = 0; c < W; c++) x[r][c] = mc[(lane + 32 * r) * LD + W * K + c];
+            }
+            int p, myp = 0; cplx d;
+            gjd_search<TM, W, 0>(x, used, W * K, b, lane, p, d, sing_at);
+            gjd_panel_steps<TM, W, 0>(x, rsc, used, pm, p, d, myp, sing_at, W * K, b, lane, prow_s);
+            cplx* Tk = Tb + (K & 1) * N * W;
+#pragma unroll
+            for (int r = 0; r < TM; r++)
+#pragma unroll
+                for (int c = 0; c < W; c++) Tk[(lane + 32 * r) * W + c] = cmul(x[r][c], rsc[r]);
+            if (lane < W) { piv[W * K + lane] = myp; prows[(K & 1) * 8 + lane] = myp; }
+            if (lane == 0) {
+#pragma unroll
+                for (int r = 0; r < TM; r++) pmask[(K & 1) * 4 + r] = pm[r];
+            }
+            gjd_bar_arrive(2 + (K & 1), GJD_NT);
+        }
+        if (lane == 0 && sing_at) *s_sing = sing_at;
+    } else {
+        // ---------------- update warps ----------------
+        double cre[TR][TC][2], cim[TR][TC][2];
+#pragma unroll
+        for (int tr = 0; tr < TR; tr++)
+#pragma unroll
+            for (int tc = 0; tc < TC; tc++)
+#pragma unroll
+                for (int h = 0; h < 2; h++) {
+                    const cplx v = mir[(row0 + 8 * tr) * LD + col0 + 8 * tc + h];
+                    cre[tr][tc][h] = v.x; cim[tr][tc][h] = v.y;
+                }
+#pragma unroll 1
+        for (int Kc = 0; Kc < WC; Kc++) {
+#pragma unroll
+            for (int tcs = 0; tcs < TC; tcs++) {
+#pragma unroll
+                for (int hp = 0; hp < PPT; hp++) {
+                    const int K = (Kc * TC + tcs) * PPT + hp;
+                    if (K >= npanel) break;
+                    const bool more = K + 1 < npanel;
+                    const cplx* mc = mir + (K & 1) * N * LD;
+                    cplx* mn = mir + ((K + 1) & 1) * N * LD;
+                    const cplx* Tk = Tb + (K & 1) * N * W;
+                    const int* prk = prows + (K & 1) * 8;
+                    const unsigned* pmk = pmask + (K & 1) * 4;
+                    gjd_bar_sync(2 + (K & 1), GJD_NT);
+                    int pk[KS];
+#pragma unroll
+                    for (int ks = 0; ks < KS; ks++) pk[ks] = prk[4 * ks + q];
+                    if (more && warp < NRT) {
+                        // early tile: rows 8 warp .. + 7 of the 8-column tile that holds panel K+1
+                        const int cb = ((K + 1) / PPT) * 8;
+                        const int i = 8 * warp + g, j = cb + 2 * q;
+                        const bool isp = (pmk[i >> 5] >> (i & 31)) & 1u;
+                        cplx c0 = mc[i * LD + j], c1 = mc[i * LD + j + 1];
+                        if (isp) { c0 = cmake(0.0, 0.0); c1 = c0; }
+#pragma unroll
+                        for (int ks = 0; ks < KS; ks++) {
+                            const cplx ta = Tk[i * W + 4 * ks + q];
+                            const cplx tb = mc[pk[ks] * LD + cb + g];
+                            gjd_dmma(c0.x, c1.x, ta.x, tb.x);
+                            gjd_dmma(c0.y, c1.y, ta.x, tb.y);
+                            gjd_dmma(c0.x, c1.x, ta.y, gjd_flip(tb.y));
+                            gjd_dmma(c0.y, c1.y, ta.y, tb.x);
+                        }
+                        if (W == 8 || (q >> 1) == ((K + 1) & 1)) { mn[i * LD + j] = c0; mn[i * LD + j + 1] = c1; }
+                    }
+                    if (more) gjd_bar_arrive(4 + ((K + 1) & 1), GJD_NT);
+                    double are[TR][KS], aim[TR][KS], bre[TC][KS], bim[TC][KS], bni[TC][KS];
+#pragma unroll
+                    for (int ks = 0; ks < KS; ks++) {
+#pragma unroll
+                        for (int t = 0; t < TR; t++) {
+                            const cplx ta = Tk[(row0 + 8 * t) * W + 4 * ks + q];
+                            are[t][ks] = ta.x; aim[t][ks] = ta.y;
+                        }
+#pragma unroll
+                        for (int t = 0; t < TC; t++) {
+                            const cplx tb = mc[pk[ks] * LD + 8 * TC * wc + 8 * t + g];
+                            bre[t][ks] = tb.x; bim[t][ks] = tb.y; bni[t][ks] = gjd_flip(tb.y);
+                        }
+                    }
+#pragma unroll
+                    for (int tr = 0; tr < TR; tr++) {
+                        const int i = row0 + 8 * tr;
+                        if ((pmk[i >> 5] >> (i & 31)) & 1u) {
+#pragma unroll
+                            for (int tc = 0; tc < TC; tc++) { cre[tr][tc][0] = cre[tr][tc][1] = 0.0; cim[tr][tc][0] = cim[tr][tc][1] = 0.0; }
+                        }
+                    }
+#pragma unroll
+                    for (int tc = 0; tc < TC; tc++) {
+#pragma unroll
+                        for (int ks = 0; ks < KS; ks++)
+#pragma unroll
+                            for (int tr = 0; tr < TR; tr++) {
+                                gjd_dmma(cre[tr][tc][0], cre[tr][tc][1], are[tr][ks], bre[tc][ks]);
+                                gjd_dmma(cim[tr][tc][0], cim[tr][tc][1], are[tr][ks], bim[tc][ks]);
+                                gjd_dmma(cre[tr][tc][0], cre[tr][tc][1], aim[tr][ks], bni[tc][ks]);
+                                gjd_dmma(cim[tr][tc][0], cim[tr][tc][1], aim[tr][ks], bre[tc][ks]);
+                            }
+                        // my columns of panel K itself become T
+                        if (tc == tcs && wc == Kc && (W == 8 || (q >> 1) == hp)) {
+#pragma unroll
+                            for (int tr = 0; tr < TR; tr++)
+#pragma unroll
+                                for (int h = 0; h < 2; h++) {
+                                    const cplx t = Tk[(row0 + 8 * tr) * W + ((2 * q + h) & (W - 1))];
+                                    cre[tr][tc][h] = t.x; cim[tr][tc][h] = t.y;
+                                }
+                        }
+#pragma unroll
+                        for (int tr = 0; tr < TR; tr++)
+#pragma unroll
+                            for (int h = 0; h < 2; h++)
+                                mn[(row0 + 8 * tr) * LD + col0 + 8 * tc + h] = cmake(cre[tr][tc][h], cim[tr][tc][h]);
+                    }
+                    gjd_bar_sync(1, UT);
+                }
+            }
+        }
+        // as in gj_reg_kernel: the accumulators hold B[i][k] = X[i][piv[k]], X = Pi A^-1, so
+        // A^-1[pinv[i]][piv[j]] = B[i][j]; dest = pinv
+        if (tid < b) dest[piv[tid]] = tid;
+        gjd_bar_sync(1, UT);
+        cplx* ob = mir + ((npanel + 1) & 1) * N * LD;      // the buffer the last update read from: free now
+#pragma unroll
+        for (int tr = 0; tr < TR; tr++)
+#pragma unroll
+            for (int tc = 0; tc < TC; tc++)
+#pragma unroll
+                for (int h = 0; h < 2; h++) {
+                    const int i = row0 + 8 * tr, j = col0 + 8 * tc + h;
+                    if (i < b && j < b) ob[dest[i] * LD + piv[j]] = cmake(cre[tr][tc][h], cim[tr][tc][h]);
+                }
+    }
+    __syncthreads();
+    const cplx* ob = mir + ((npanel + 1) & 1) * N * LD;
+    for (int idx = tid; idx < b * b; idx += GJD_NT) {
+        const int i = idx / b, j = idx - i * b;
+        gA[idx] = ob[i * LD + j];
+    }
+    if (tid == 0 && *s_sing && info) info[e] = code_dev ? *code_dev + code : (code > 0 ? code : *s_sing);
+}
+
+// ------------------------------------------------------------------------------------------------
 // blocked path, step 1: cluster panel LU with partial pivoting
 // ------------------------------------------------------------------------------------------------
 struct Cand { double val; int row; int pad; };
@@ -810,6 +1115,10 @@ size_t zinv_workspace_bytes(int b, int batch) {
 int zinv_prepare(negf_ctx* ctx) {
     NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_panel_cluster_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                               (int)(PANEL_SMEM_ROWS_BYTES + PANEL_SMEM_FIXED)));
+    NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_dmma_kernel<1, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gjd_smem_bytes<1, 4>()));
+    NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_dmma_kernel<2, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gjd_smem_bytes<2, 4>()));
+    NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_dmma_kernel<1, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gjd_smem_bytes<1, 8>()));
+    NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_dmma_kernel<2, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gjd_smem_bytes<2, 8>()));
     NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_colperm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
     NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_panel_reg_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)reg_panel_smem_bytes(8)));
     NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_panel_reg_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)reg_panel_smem_bytes(16)));
@@ -820,6 +1129,17 @@ int zinv_launch(negf_ctx* ctx, int b, cplx* A, long long sA, int batch, void* ws
                 int info_code, const int* skip, const int* code_dev) {
     ProfScope _ps(ctx, NEGF_PROF_INVERSE);
     if (b <= 0 || batch <= 0) return NEGF_OK;
+    if (b <= 64 && ctx->inv_tensor) {
+        if (ctx->inv_tensor == 2) {
+            if (b <= 32) gj_dmma_kernel<1, 8><<<batch, GJD_NT, gjd_smem_bytes<1, 8>(), ctx->stream>>>(A, sA, b, info, info_code, skip, code_dev);
+            else         gj_dmma_kernel<2, 8><<<batch, GJD_NT, gjd_smem_bytes<2, 8>(), ctx->stream>>>(A, sA, b, info, info_code, skip, code_dev);
+        } else {
+            if (b <= 32) gj_dmma_kernel<1, 4><<<batch, GJD_NT, gjd_smem_bytes<1, 4>(), ctx->stream>>>(A, sA, b, info, info_code, skip, code_dev);
+            else         gj_dmma_kernel<2, 4><<<batch, GJD_NT, gjd_smem_bytes<2, 4>(), ctx->stream>>>(A, sA, b, info, info_code, skip, code_dev);
+        }
+        NEGF_LAUNCH_CHECK(ctx);
+        return NEGF_OK;
+    }
     if (b <= SMALL_MAX) {
         // 16 warps per matrix: half the instructions per warp and column of an 8-warp layout (the
         // kernel is bound by the per-warp dependent instruction chain, not by issue slots or FP64)

@@ -25,6 +25,7 @@ SIGMA_NONE, SIGMA_SCALAR, SIGMA_BT = 0, 1, 2
 KEEP_SWEEP = 1
 OPT_GRAPH_LOOPS = 1
 OPT_GEMM_3M = 2
+OPT_INV_TENSOR = 3
 
 
 class c128(C.Structure):
