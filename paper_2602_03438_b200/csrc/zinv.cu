@@ -254,11 +254,17 @@ __device__ __forceinline__ double gjd_flip(double x) {
     return __hiloint2double(__double2hiint(x) ^ 0x80000000, __double2loint(x));
 }
 
-constexpr int GJD_UW = 8;                      // update warps (2 x 4 grid); warp GJD_UW factorises the panels
-constexpr int GJD_NT = (GJD_UW + 1) * 32;      // 9 warps: at most 3 per scheduler partition -> up to 168 registers per thread
-template <int TM, int W> constexpr size_t gjd_smem_bytes() {
-    constexpr int N = 32 * TM, LD = N + 1;
-    return (size_t)2 * N * LD * sizeof(cplx) + (size_t)2 * N * W * sizeof(cplx) + 16 * sizeof(cplx) + (2 * N + 16 + 8 + 4) * sizeof(int);
+constexpr int GJD_UW = 8;                      // update warps (2 x 4 grid)
+// 11 hardware warps (at most 3 per scheduler partition -> up to 168 registers per thread): warp 0 factorises
+// the panels and has its scheduler partition to itself (warps 4 and 8 exit at once), because its dependent
+// FP64 chain would otherwise queue behind the DMMAs of the update warps on the shared FP64 pipe; the update
+// warps are the hardware warps 1-3, 5-7, 9-10.
+constexpr int GJD_NT = 11 * 32;
+constexpr int GJD_ACT = (GJD_UW + 1) * 32;     // threads that take part in the barriers
+constexpr int GJD_W = 4;                       // panel width = one k-step of DMMA.8x8x4
+template <int TM> constexpr size_t gjd_smem_bytes() {
+    constexpr int N = 32 * TM, LD = N + 1, W = GJD_W;
+    return (size_t)2 * N * LD * sizeof(cplx) + (size_t)4 * N * W * sizeof(cplx) + 16 * sizeof(cplx) + (4 * N + 16 + 4) * sizeof(int);
 }
 
 // pivot of panel column C (global column k): p = row (warp-uniform), d = 1 / pivot (computed by every lane)
@@ -285,10 +291,13 @@ __device__ __forceinline__ void gjd_search(const cplx (&x)[TM][W], unsigned used
     sing_at = (sing && sing_at == 0) ? k + 1 : sing_at;
 }
 
-// one Gauss-Jordan step of the panel (column J) + look-ahead search of column J+1
+// one Gauss-Jordan step of the panel (column J) + look-ahead search of column J+1.
+// Tt receives the coefficients AS APPLIED: row i gets  row_i += Tt[i][J] x (pivot row p_J as it is at step J),
+// Tt[p_J][J] = 1 / pivot (the pivot row is replaced by its scaled self); pjx[p_J] = J + 1.
 template <int TM, int W, int J>
-__device__ __forceinline__ void gjd_panel_steps(cplx (&x)[TM][W], cplx (&rsc)[TM], unsigned& used, unsigned (&pm)[TM],
-                                                int& p, cplx& d, int& myp, int& sing_at, int k0, int b, int lane, cplx* prow_s) {
+__device__ __forceinline__ void gjd_panel_steps(cplx (&x)[TM][W], cplx (&rsc)[TM], unsigned& used,
+                                                int& p, cplx& d, int& myp, int& sing_at, int k0, int b, int lane,
+                                                cplx* prow_s, cplx* Tt, int* pjx) {
     if constexpr (J < W) {
         const int pl = p & 31, pr = p >> 5;
         cplx* line = prow_s + (J & 1) * 8;
@@ -297,10 +306,9 @@ __device__ __forceinline__ void gjd_panel_steps(cplx (&x)[TM][W], cplx (&rsc)[TM
             if (lane == pl && pr == r) {
 #pragma unroll
                 for (int c = 0; c < W; c++) line[c] = x[r][c];
+                pjx[p] = J + 1;
             }
         myp = (lane == J) ? p : myp;
-#pragma unroll
-        for (int r = 0; r < TM; r++) if (pr == r) pm[r] |= 1u << pl;
         __syncwarp();
         // deferred scaling inside the panel: the registers of a pivot row keep the unscaled row (true value =
         // rsc x register), so pivoted and unpivoted rows run the same update and the pivot row itself costs nothing
@@ -311,6 +319,8 @@ __device__ __forceinline__ void gjd_panel_steps(cplx (&x)[TM][W], cplx (&rsc)[TM
             const cplx t = cmul(x[r][J], d);
             mlt[r] = isp ? cmake(0.0, 0.0) : t;
             x[r][J] = isp ? cmake(1.0, 0.0) : cneg(t);
+            const cplx tt = cmul(t, rsc[r]);                   // true coefficient of a row pivoted earlier in this panel
+            Tt[(lane + 32 * r) * W + J] = isp ? d : cneg(tt);
             if (isp) { rsc[r] = d; used |= 1u << r; }
         }
         int pn = 0; cplx dn = cmake(1.0, 0.0);
@@ -328,40 +338,59 @@ __device__ __forceinline__ void gjd_panel_steps(cplx (&x)[TM][W], cplx (&rsc)[TM
             for (int r = 0; r < TM; r++) cfms(x[r][c], mlt[r], prc);
         }
         p = pn; d = dn;
-        gjd_panel_steps<TM, W, J + 1>(x, rsc, used, pm, p, d, myp, sing_at, k0, b, lane, prow_s);
+        gjd_panel_steps<TM, W, J + 1>(x, rsc, used, p, d, myp, sing_at, k0, b, lane, prow_s, Tt, pjx);
     }
 }
 
 __device__ __forceinline__ void gjd_bar_sync(int id, int count) { asm volatile("bar.sync %0, %1;" :: "r"(id), "r"(count) : "memory"); }
 __device__ __forceinline__ void gjd_bar_arrive(int id, int count) { __threadfence_block(); asm volatile("bar.arrive %0, %1;" :: "r"(id), "r"(count) : "memory"); }
 
+// B operand of the rank-4 update for matrix column `col` (lane = (g: column, q: pivot index)): the pivot row
+// p_q AS IT IS WHEN IT IS USED, i.e. after the steps l < q of this panel have been applied to it:
+//   R~_q = R_q + sum_{l<q} Tt[p_q][l] R~_l      (lanes q = l are final after l rounds).
+// With this operand and the as-applied coefficients as A operand the DMMA accumulates, per element and in
+// the same order, exactly the updates of the unblocked elimination (bounded multipliers); the product
+// form T R with the original rows would go through the explicit inverse of the 4 x 4 pivot block instead.
+__device__ __forceinline__ cplx gjd_bfrag(const cplx* mc, int LD, const cplx* Tt, int pq, int col, int q, int lane) {
+    cplx v = mc[pq * LD + col];
+#pragma unroll
+    for (int l = 0; l < GJD_W - 1; l++) {
+        const int src = (lane & ~3) + l;
+        const double sx = __shfl_sync(0xffffffffu, v.x, src), sy = __shfl_sync(0xffffffffu, v.y, src);
+        if (q > l) cfma(v, Tt[pq * GJD_W + l], cmake(sx, sy));
+    }
+    return v;
+}
+
 // Look-ahead: while the update warps apply panel K to the matrix, the panel warp already factorises
 // panel K+1.  For that the update warps FIRST bring the columns of panel K+1 up to date (one 8 x 8 row
 // tile per warp, accumulator taken from and written back to the mirror), signal the panel warp
 // (named barrier A) and only then update their own tiles (which repeats that tile bit for bit).
-// Named barriers: 1 = update warps only (mirror complete), 2/3 = T of panel K ready (panel warp
+// Named barriers: 1 = update warps only (mirror complete), 2/3 = panel K factorised (panel warp
 // arrives, update warps wait), 4/5 = columns of panel K ready in the mirror (update warps arrive,
-// panel warp waits).  T, the pivot rows and their mask are double-buffered.
-// W = panel width (4 or 8): the narrow panel halves the sequential work of the panel warp per column
-// (W - 1 rank-1 column updates per step) at the price of twice as many update rounds.
-template <int TM, int W>
+// panel warp waits).  The panel outputs are double-buffered.
+template <int TM>
 __global__ void __launch_bounds__(GJD_NT, 1) gj_dmma_kernel(cplx* A, long long sA, int b, int* info, int code,
                                                             const int* skip, const int* code_dev) {
     // N = 32 TM rows; update warps in a 2 x 4 grid, warp tile (8 TR) x (8 TC) = TR x TC accumulator tiles
-    constexpr int N = 32 * TM, LD = N + 1, TR = 2 * TM, TC = TM, WC = 4, NRT = N / 8, UT = GJD_UW * 32;
-    constexpr int KS = W / 4, PPT = 8 / W;       // k-steps of a rank-W update; panels per 8-column tile
+    constexpr int N = 32 * TM, LD = N + 1, TR = 2 * TM, TC = TM, WC = 4, NRT = N / 8, UT = GJD_UW * 32, W = GJD_W;
+    constexpr int PPT = 8 / W;                   // panels per 8-column tile
     const int e = blockIdx.x;
     if (skip && skip[e]) return;
     extern __shared__ __align__(16) unsigned char gjd_smem[];
     cplx* mir = (cplx*)gjd_smem;                 // [2][N][LD]
-    cplx* Tb = mir + 2 * N * LD;                 // [2][N][W]
-    cplx* prow_s = Tb + 2 * N * W;               // [2][8]
+    cplx* Tb = mir + 2 * N * LD;                 // [2][N][W]  final panel columns (the transform T)
+    cplx* Ttb = Tb + 2 * N * W;                  // [2][N][W]  coefficients as applied
+    cplx* prow_s = Ttb + 2 * N * W;              // [2][8]
     int* piv = (int*)(prow_s + 16);              // [N]
     int* dest = piv + N;                         // [N]
-    int* prows = dest + N;                       // [2][8]
-    unsigned* pmask = (unsigned*)(prows + 16);   // [2][4]
-    int* s_sing = (int*)(pmask + 8);
-    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    int* pjxb = dest + N;                        // [2][N]  j + 1 for the j-th pivot row of the panel, else 0
+    int* prows = pjxb + 2 * N;                   // [2][8]
+    int* s_sing = prows + 16;
+    const int hw = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (hw == 4 || hw == 8) return;
+    const int warp = hw == 0 ? GJD_UW : hw - 1 - (hw > 4) - (hw > 8);    // 0..7 update warps, 8 = panel warp
+    const int tid = warp * 32 + lane;
     const int g = lane >> 2, q = lane & 3, wr = (warp >> 2) & 1, wc = warp & 3;
     const int row0 = 8 * TR * wr + g, col0 = 8 * TC * wc + 2 * q;     // + 8 tr, + 8 tc (+ h)
     cplx* gA = A + (size_t)e * sA;
@@ -378,37 +407,35 @@ __global__ void __launch_bounds__(GJD_NT, 1) gj_dmma_kernel(cplx* A, long long s
                 }
     }
     if (tid == 0) *s_sing = 0;
-    __syncthreads();
+    gjd_bar_sync(0, GJD_ACT);
     if (warp == GJD_UW) {
         // ---------------- panel warp ----------------
         unsigned used = 0u;                      // bit r = my row lane + 32 r has been a pivot row
         int sing_at = 0;
 #pragma unroll 1
         for (int K = 0; K < npanel; K++) {
-            if (K > 0) gjd_bar_sync(4 + (K & 1), GJD_NT);
+            if (K > 0) gjd_bar_sync(4 + (K & 1), GJD_ACT);
             const cplx* mc = mir + (K & 1) * N * LD;
+            int* pjx = pjxb + (K & 1) * N;
             cplx x[TM][W], rsc[TM];
-            unsigned pm[TM];
 #pragma unroll
             for (int r = 0; r < TM; r++) {
-                rsc[r] = cmake(1.0, 0.0); pm[r] = 0u;
+                rsc[r] = cmake(1.0, 0.0);
+                pjx[lane + 32 * r] = 0;
 #pragma unroll
                 for (int c = 0; c < W; c++) x[r][c] = mc[(lane + 32 * r) * LD + W * K + c];
             }
+            __syncwarp();
             int p, myp = 0; cplx d;
             gjd_search<TM, W, 0>(x, used, W * K, b, lane, p, d, sing_at);
-            gjd_panel_steps<TM, W, 0>(x, rsc, used, pm, p, d, myp, sing_at, W * K, b, lane, prow_s);
+            gjd_panel_steps<TM, W, 0>(x, rsc, used, p, d, myp, sing_at, W * K, b, lane, prow_s, Ttb + (K & 1) * N * W, pjx);
             cplx* Tk = Tb + (K & 1) * N * W;
 #pragma unroll
             for (int r = 0; r < TM; r++)
 #pragma unroll
                 for (int c = 0; c < W; c++) Tk[(lane + 32 * r) * W + c] = cmul(x[r][c], rsc[r]);
             if (lane < W) { piv[W * K + lane] = myp; prows[(K & 1) * 8 + lane] = myp; }
-            if (lane == 0) {
-#pragma unroll
-                for (int r = 0; r < TM; r++) pmask[(K & 1) * 4 + r] = pm[r];
-            }
-            gjd_bar_arrive(2 + (K & 1), GJD_NT);
+            gjd_bar_arrive(2 + (K & 1), GJD_ACT);
         }
         if (lane == 0 && sing_at) *s_sing = sing_at;
     } else {
@@ -435,49 +462,44 @@ __global__ void __launch_bounds__(GJD_NT, 1) gj_dmma_kernel(cplx* A, long long s
                     const cplx* mc = mir + (K & 1) * N * LD;
                     cplx* mn = mir + ((K + 1) & 1) * N * LD;
                     const cplx* Tk = Tb + (K & 1) * N * W;
-                    const int* prk = prows + (K & 1) * 8;
-                    const unsigned* pmk = pmask + (K & 1) * 4;
-                    gjd_bar_sync(2 + (K & 1), GJD_NT);
-                    int pk[KS];
-#pragma unroll
-                    for (int ks = 0; ks < KS; ks++) pk[ks] = prk[4 * ks + q];
-                    if (more && warp < NRT) {
-                        // early tile: rows 8 warp .. + 7 of the 8-column tile that holds panel K+1
+                    const cplx* Tt = Ttb + (K & 1) * N * W;
+                    const int* pjx = pjxb + (K & 1) * N;
+                    gjd_bar_sync(2 + (K & 1), GJD_ACT);
+                    const int pq = prows[(K & 1) * 8 + q];
+                    if (more) {
+                        // early tile: rows 8 warp .. + 7 of the 8-column tile that holds panel K+1 (all warps run the
+                        // shuffles of the operand; the warps beyond the last row tile only skip the product)
                         const int cb = ((K + 1) / PPT) * 8;
-                        const int i = 8 * warp + g, j = cb + 2 * q;
-                        const bool isp = (pmk[i >> 5] >> (i & 31)) & 1u;
-                        cplx c0 = mc[i * LD + j], c1 = mc[i * LD + j + 1];
-                        if (isp) { c0 = cmake(0.0, 0.0); c1 = c0; }
-#pragma unroll
-                        for (int ks = 0; ks < KS; ks++) {
-                            const cplx ta = Tk[i * W + 4 * ks + q];
-                            const cplx tb = mc[pk[ks] * LD + cb + g];
+                        const cplx tb = gjd_bfrag(mc, LD, Tt, pq, cb + g, q, lane);
+                        if (warp < NRT) {
+                            const int i = 8 * warp + g, j = cb + 2 * q;
+                            const int pj = pjx[i];
+                            cplx c0 = mc[i * LD + j], c1 = mc[i * LD + j + 1];
+                            if (pj) { c0 = cmake(0.0, 0.0); c1 = c0; }
+                            cplx ta = Tt[i * W + q];
+                            if (q < pj - 1) ta = cmake(0.0, 0.0);
                             gjd_dmma(c0.x, c1.x, ta.x, tb.x);
                             gjd_dmma(c0.y, c1.y, ta.x, tb.y);
                             gjd_dmma(c0.x, c1.x, ta.y, gjd_flip(tb.y));
                             gjd_dmma(c0.y, c1.y, ta.y, tb.x);
+                            if ((q >> 1) == ((K + 1) & 1)) { mn[i * LD + j] = c0; mn[i * LD + j + 1] = c1; }
                         }
-                        if (W == 8 || (q >> 1) == ((K + 1) & 1)) { mn[i * LD + j] = c0; mn[i * LD + j + 1] = c1; }
+                        gjd_bar_arrive(4 + ((K + 1) & 1), GJD_ACT);
                     }
-                    if (more) gjd_bar_arrive(4 + ((K + 1) & 1), GJD_NT);
-                    double are[TR][KS], aim[TR][KS], bre[TC][KS], bim[TC][KS], bni[TC][KS];
+                    double are[TR], aim[TR], bre[TC], bim[TC], bni[TC];
 #pragma unroll
-                    for (int ks = 0; ks < KS; ks++) {
-#pragma unroll
-                        for (int t = 0; t < TR; t++) {
-                            const cplx ta = Tk[(row0 + 8 * t) * W + 4 * ks + q];
-                            are[t][ks] = ta.x; aim[t][ks] = ta.y;
-                        }
-#pragma unroll
-                        for (int t = 0; t < TC; t++) {
-                            const cplx tb = mc[pk[ks] * LD + 8 * TC * wc + 8 * t + g];
-                            bre[t][ks] = tb.x; bim[t][ks] = tb.y; bni[t][ks] = gjd_flip(tb.y);
-                        }
+                    for (int t = 0; t < TC; t++) {
+                        const cplx tb = gjd_bfrag(mc, LD, Tt, pq, 8 * TC * wc + 8 * t + g, q, lane);
+                        bre[t] = tb.x; bim[t] = tb.y; bni[t] = gjd_flip(tb.y);
                     }
 #pragma unroll
                     for (int tr = 0; tr < TR; tr++) {
                         const int i = row0 + 8 * tr;
-                        if ((pmk[i >> 5] >> (i & 31)) & 1u) {
+                        const int pj = pjx[i];
+                        cplx ta = Tt[i * W + q];
+                        if (q < pj - 1) ta = cmake(0.0, 0.0);      // the steps before a pivot row's own are inside R~
+                        are[tr] = ta.x; aim[tr] = ta.y;
+                        if (pj) {
 #pragma unroll
                             for (int tc = 0; tc < TC; tc++) { cre[tr][tc][0] = cre[tr][tc][1] = 0.0; cim[tr][tc][0] = cim[tr][tc][1] = 0.0; }
                         }
@@ -485,16 +507,14 @@ __global__ void __launch_bounds__(GJD_NT, 1) gj_dmma_kernel(cplx* A, long long s
 #pragma unroll
                     for (int tc = 0; tc < TC; tc++) {
 #pragma unroll
-                        for (int ks = 0; ks < KS; ks++)
-#pragma unroll
-                            for (int tr = 0; tr < TR; tr++) {
-                                gjd_dmma(cre[tr][tc][0], cre[tr][tc][1], are[tr][ks], bre[tc][ks]);
-                                gjd_dmma(cim[tr][tc][0], cim[tr][tc][1], are[tr][ks], bim[tc][ks]);
-                                gjd_dmma(cre[tr][tc][0], cre[tr][tc][1], aim[tr][ks], bni[tc][ks]);
-                                gjd_dmma(cim[tr][tc][0], cim[tr][tc][1], aim[tr][ks], bre[tc][ks]);
-                            }
+                        for (int tr = 0; tr < TR; tr++) {
+                            gjd_dmma(cre[tr][tc][0], cre[tr][tc][1], are[tr], bre[tc]);
+                            gjd_dmma(cim[tr][tc][0], cim[tr][tc][1], are[tr], bim[tc]);
+                            gjd_dmma(cre[tr][tc][0], cre[tr][tc][1], aim[tr], bni[tc]);
+                            gjd_dmma(cim[tr][tc][0], cim[tr][tc][1], aim[tr], bre[tc]);
+                        }
                         // my columns of panel K itself become T
-                        if (tc == tcs && wc == Kc && (W == 8 || (q >> 1) == hp)) {
+                        if (tc == tcs && wc == Kc && (q >> 1) == hp) {
 #pragma unroll
                             for (int tr = 0; tr < TR; tr++)
 #pragma unroll
@@ -528,9 +548,9 @@ __global__ void __launch_bounds__(GJD_NT, 1) gj_dmma_kernel(cplx* A, long long s
                     if (i < b && j < b) ob[dest[i] * LD + piv[j]] = cmake(cre[tr][tc][h], cim[tr][tc][h]);
                 }
     }
-    __syncthreads();
+    gjd_bar_sync(0, GJD_ACT);
     const cplx* ob = mir + ((npanel + 1) & 1) * N * LD;
-    for (int idx = tid; idx < b * b; idx += GJD_NT) {
+    for (int idx = tid; idx < b * b; idx += GJD_ACT) {
         const int i = idx / b, j = idx - i * b;
         gA[idx] = ob[i * LD + j];
     }
@@ -1115,10 +1135,8 @@ size_t zinv_workspace_bytes(int b, int batch) {
 int zinv_prepare(negf_ctx* ctx) {
     NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_panel_cluster_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                               (int)(PANEL_SMEM_ROWS_BYTES + PANEL_SMEM_FIXED)));
-    NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_dmma_kernel<1, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gjd_smem_bytes<1, 4>()));
-    NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_dmma_kernel<2, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gjd_smem_bytes<2, 4>()));
-    NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_dmma_kernel<1, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gjd_smem_bytes<1, 8>()));
-    NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_dmma_kernel<2, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gjd_smem_bytes<2, 8>()));
+    NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_dmma_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gjd_smem_bytes<1>()));
+    NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_dmma_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gjd_smem_bytes<2>()));
     NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_colperm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
     NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_panel_reg_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)reg_panel_smem_bytes(8)));
     NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_panel_reg_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)reg_panel_smem_bytes(16)));
@@ -1129,14 +1147,9 @@ int zinv_launch(negf_ctx* ctx, int b, cplx* A, long long sA, int batch, void* ws
                 int info_code, const int* skip, const int* code_dev) {
     ProfScope _ps(ctx, NEGF_PROF_INVERSE);
     if (b <= 0 || batch <= 0) return NEGF_OK;
-    if (b <= 64 && ctx->inv_tensor) {
-        if (ctx->inv_tensor == 2) {
-            if (b <= 32) gj_dmma_kernel<1, 8><<<batch, GJD_NT, gjd_smem_bytes<1, 8>(), ctx->stream>>>(A, sA, b, info, info_code, skip, code_dev);
-            else         gj_dmma_kernel<2, 8><<<batch, GJD_NT, gjd_smem_bytes<2, 8>(), ctx->stream>>>(A, sA, b, info, info_code, skip, code_dev);
-        } else {
-            if (b <= 32) gj_dmma_kernel<1, 4><<<batch, GJD_NT, gjd_smem_bytes<1, 4>(), ctx->stream>>>(A, sA, b, info, info_code, skip, code_dev);
-            else         gj_dmma_kernel<2, 4><<<batch, GJD_NT, gjd_smem_bytes<2, 4>(), ctx->stream>>>(A, sA, b, info, info_code, skip, code_dev);
-        }
+    if (b > 8 && b <= 64 && ctx->inv_tensor) {
+        if (b <= 32) gj_dmma_kernel<1><<<batch, GJD_NT, gjd_smem_bytes<1>(), ctx->stream>>>(A, sA, b, info, info_code, skip, code_dev);
+        else         gj_dmma_kernel<2><<<batch, GJD_NT, gjd_smem_bytes<2>(), ctx->stream>>>(A, sA, b, info, info_code, skip, code_dev);
         NEGF_LAUNCH_CHECK(ctx);
         return NEGF_OK;
     }
