@@ -83,3 +83,61 @@ def test_zinverse_singular_reports_info(ctx, negf_lib):
     info = torch.zeros(2, dtype=torch.int32, device="cuda")
     ctx.zinverse_batched(b, dA, b * b, 2, info)
     assert info.cpu().tolist() == [0, 6]
+
+
+@pytest.mark.parametrize("b", [9, 12, 17, 24, 31, 32, 33, 40, 47, 56, 63, 64])
+def test_zinverse_tensor_and_register_kernels(negf_lib, b):
+    """8 < b <= 64 has two K1 kernels: the blocked one with rank-4 DMMA updates (NEGF_OPT_INV_TENSOR = 1, default) and the
+    register-resident unblocked one (0).  Both against LAPACK at the K1 bar; sizes cover both paddings (32 and 64 rows),
+    ragged last panels (b not a multiple of 4) and last tiles; the batch holds a matrix that needs pivoting at once, one
+    with nearly dependent columns and ill-conditioned ones (cond up to ~1e8), where the blocked kernel must stay
+    within a small factor of the unblocked one (the order of its updates is that of the unblocked elimination)."""
+    import torch
+    rng = np.random.default_rng(1000 + b)
+    batch = 6
+    A = _rand(rng, batch, b, b) / np.sqrt(b) + 0.3 * np.eye(b)
+    A[0, 0, :] *= 1e-3
+    A[1, :, 1] = A[1, :, 0] * (1 + 1e-9) + 1e-7 * A[1, :, 1]
+    for e, c in ((3, 1e4), (4, 1e6), (5, 1e8)):                    # graded singular values
+        u, _, vh = np.linalg.svd(_rand(rng, b, b))
+        A[e] = (u * np.logspace(0, -np.log10(c), b)) @ vh
+    ref = np.linalg.inv(A)
+    errs = {}
+    for opt in (1, 0):
+        c = negf_lib.Context(0)
+        c.set_stream(torch.cuda.current_stream().cuda_stream)
+        c.set_option(negf_lib.OPT_INV_TENSOR, opt)
+        dA = torch.from_numpy(A).cuda()
+        info = torch.full((batch,), -7, dtype=torch.int32, device="cuda")
+        c.zinverse_batched(b, dA, b * b, batch, info)
+        got = dA.cpu().numpy()
+        assert info.cpu().tolist() == [0] * batch
+        errs[opt] = [np.linalg.norm(got[e] - ref[e]) / np.linalg.norm(ref[e]) for e in range(batch)]
+        for e in range(batch):
+            cond = np.linalg.cond(A[e])
+            assert errs[opt][e] < 1e-14 * cond * 50 + 1e-13, (opt, e, errs[opt][e], cond)
+        c.close()
+    for e in range(batch):
+        assert errs[1][e] <= 8 * errs[0][e] + 1e-14, (e, errs[1][e], errs[0][e])
+
+
+@pytest.mark.parametrize("opt", [0, 1])
+@pytest.mark.parametrize("b,col", [(12, 0), (33, 32), (64, 63), (50, 17)])
+def test_zinverse_singular_both_kernels(negf_lib, opt, b, col):
+    """A zero column is reported as its 1-based index by either kernel; the other entries of the batch are untouched by it."""
+    import torch
+    c = negf_lib.Context(0)
+    c.set_stream(torch.cuda.current_stream().cuda_stream)
+    c.set_option(negf_lib.OPT_INV_TENSOR, opt)
+    rng = np.random.default_rng(b + col)
+    A = _rand(rng, 3, b, b) / np.sqrt(b) + 0.5 * np.eye(b)
+    A[1, :, col] = 0.0
+    ref0, ref2 = np.linalg.inv(A[0]), np.linalg.inv(A[2])
+    dA = torch.from_numpy(A).cuda()
+    info = torch.zeros(3, dtype=torch.int32, device="cuda")
+    c.zinverse_batched(b, dA, b * b, 3, info)
+    got = dA.cpu().numpy()
+    assert info.cpu().tolist() == [0, col + 1, 0]
+    assert np.linalg.norm(got[0] - ref0) / np.linalg.norm(ref0) < 1e-11
+    assert np.linalg.norm(got[2] - ref2) / np.linalg.norm(ref2) < 1e-11
+    c.close()
