@@ -112,10 +112,10 @@ int negf_set_workspace(negf_ctx* ctx, void* dev_ptr, size_t bytes);
  * 128-row tiles) complex products use the 3M decomposition (three real DMMA products instead of four: 25 % fewer
  * tensor-pipe instructions; the imaginary part is accurate norm-wise, not component-wise).  Off by default: the
  * 4M kernel is the one the FP64 roofline fraction is quoted on.
- * NEGF_OPT_INV_TENSOR (default 1): block sizes 9..64 are inverted by the blocked Gauss-Jordan kernel whose
+ * NEGF_OPT_INV_TENSOR (default 1): block sizes 17..64 are inverted by the blocked Gauss-Jordan kernel whose
  * rank-4 updates run on the FP64 tensor pipe (one CTA per matrix, same partial pivoting and the same order
  * of elimination updates per element as the unblocked kernel); 0 = the register-resident unblocked
- * Gauss-Jordan kernel for every block size up to 96 (the kernel 65..96 and 1..8 always use).  Set it
+ * Gauss-Jordan kernel for every block size up to 96 (the kernel 65..96 and 1..16 always use).  Set it
  * before the first call of a shape (cached call graphs keep the kernel they were captured with). */
 #define NEGF_OPT_GRAPH_LOOPS 1
 #define NEGF_OPT_GEMM_3M     2

@@ -1147,7 +1147,7 @@ int zinv_launch(negf_ctx* ctx, int b, cplx* A, long long sA, int batch, void* ws
                 int info_code, const int* skip, const int* code_dev) {
     ProfScope _ps(ctx, NEGF_PROF_INVERSE);
     if (b <= 0 || batch <= 0) return NEGF_OK;
-    if (b > 8 && b <= 64 && ctx->inv_tensor) {
+    if (b > 16 && b <= 64 && ctx->inv_tensor) {     // at b <= 16 the two kernels are level (15 us); the register one stays
         if (b <= 32) gj_dmma_kernel<1><<<batch, GJD_NT, gjd_smem_bytes<1>(), ctx->stream>>>(A, sA, b, info, info_code, skip, code_dev);
         else         gj_dmma_kernel<2><<<batch, GJD_NT, gjd_smem_bytes<2>(), ctx->stream>>>(A, sA, b, info, info_code, skip, code_dev);
         NEGF_LAUNCH_CHECK(ctx);

@@ -87,7 +87,7 @@ def test_zinverse_singular_reports_info(ctx, negf_lib):
 
 @pytest.mark.parametrize("b", [9, 12, 17, 24, 31, 32, 33, 40, 47, 56, 63, 64])
 def test_zinverse_tensor_and_register_kernels(negf_lib, b):
-    """8 < b <= 64 has two K1 kernels: the blocked one with rank-4 DMMA updates (NEGF_OPT_INV_TENSOR = 1, default) and the
+    """16 < b <= 64 has two K1 kernels (below, both options run the register kernel): the blocked one with rank-4 DMMA updates (NEGF_OPT_INV_TENSOR = 1, default) and the
     register-resident unblocked one (0).  Both against LAPACK at the K1 bar; sizes cover both paddings (32 and 64 rows),
     ragged last panels (b not a multiple of 4) and last tiles; the batch holds a matrix that needs pivoting at once, one
     with nearly dependent columns and ill-conditioned ones (cond up to ~1e8), where the blocked kernel must stay
