@@ -448,6 +448,7 @@ int zgemm_prepare(negf_ctx* ctx) {
     NEGF_CUDA_CHECK(ctx, (prepare_cfg<128, 64, 4, 2, 1>()));
     NEGF_CUDA_CHECK(ctx, (prepare_cfg<64, 64, 2, 2, 2>()));
     NEGF_CUDA_CHECK(ctx, (prepare_cfg<32, 32, 2, 2, 5>()));
+    NEGF_CUDA_CHECK(ctx, (prepare_cfg<16, 16, 2, 2, 6>()));
     {
         constexpr int smem = 3 * (128 + M3_BN) * BK * (int)sizeof(cplx);
         NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(zgemm3m_kernel<0, 0, 128, M3_BN, 4, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
@@ -487,6 +488,12 @@ int zgemm_launch_group(negf_ctx* ctx, const GemmGroup& grp) {
     // blocks up to 64 x 64: four 32x32 CTAs per product balance the SMs better than one 64x64 CTA
     // (measured 5-7 % faster at b = 64 for 128 .. 512 products per launch)
     if ((a.m > 64 || a.n > 64) && t64 >= ctx->num_sms) return launch_ops<64, 64, 2, 2, 2>(ctx, grp);
+    // launches of fewer than two 32x32 tiles per SM (the sequential chain steps: one b = 64 product per energy) are
+    // bound by the length of one warp's DMMA chain, not by the pipe: 16x16 tiles (4 warps of 8x8) quarter that chain.
+    // Measured on configs[1] with the threshold at 1 / 2 / 4 / always: 2 is best (5.97 -> 5.83 ms per step as 4
+    // energy groups, 6.41 -> 6.11 ms on one stream; always: 6.00 / 6.26 ms).
+    const long long t32 = (long long)((a.m + 31) / 32) * ((a.n + 31) / 32) * per;
+    if (t32 < 2LL * ctx->num_sms) return launch_ops<16, 16, 2, 2, 6>(ctx, grp);
     return launch_ops<32, 32, 2, 2, 5>(ctx, grp);
 }
 
