@@ -395,6 +395,7 @@ __global__ void __launch_bounds__(GJD_NT, 1) gj_dmma_kernel(cplx* A, long long s
     const int row0 = 8 * TR * wr + g, col0 = 8 * TC * wc + 2 * q;     // + 8 tr, + 8 tc (+ h)
     cplx* gA = A + (size_t)e * sA;
     const int npanel = (b + W - 1) / W;
+    double cre[TR][TC][2], cim[TR][TC][2];       // update warps: my accumulator tiles
     if (warp < GJD_UW) {
 #pragma unroll
         for (int tr = 0; tr < TR; tr++)
@@ -403,7 +404,9 @@ __global__ void __launch_bounds__(GJD_NT, 1) gj_dmma_kernel(cplx* A, long long s
 #pragma unroll
                 for (int h = 0; h < 2; h++) {
                     const int i = row0 + 8 * tr, j = col0 + 8 * tc + h;
-                    mir[i * LD + j] = (i < b && j < b) ? gA[(size_t)i * b + j] : cmake(i == j ? 1.0 : 0.0, 0.0);
+                    const cplx v = (i < b && j < b) ? gA[(size_t)i * b + j] : cmake(i == j ? 1.0 : 0.0, 0.0);
+                    cre[tr][tc][h] = v.x; cim[tr][tc][h] = v.y;
+                    mir[i * LD + j] = v;
                 }
     }
     if (tid == 0) *s_sing = 0;
@@ -440,16 +443,6 @@ __global__ void __launch_bounds__(GJD_NT, 1) gj_dmma_kernel(cplx* A, long long s
         if (lane == 0 && sing_at) *s_sing = sing_at;
     } else {
         // ---------------- update warps ----------------
-        double cre[TR][TC][2], cim[TR][TC][2];
-#pragma unroll
-        for (int tr = 0; tr < TR; tr++)
-#pragma unroll
-            for (int tc = 0; tc < TC; tc++)
-#pragma unroll
-                for (int h = 0; h < 2; h++) {
-                    const cplx v = mir[(row0 + 8 * tr) * LD + col0 + 8 * tc + h];
-                    cre[tr][tc][h] = v.x; cim[tr][tc][h] = v.y;
-                }
 #pragma unroll 1
         for (int Kc = 0; Kc < WC; Kc++) {
 #pragma unroll
@@ -537,23 +530,21 @@ __global__ void __launch_bounds__(GJD_NT, 1) gj_dmma_kernel(cplx* A, long long s
         // A^-1[pinv[i]][piv[j]] = B[i][j]; dest = pinv
         if (tid < b) dest[piv[tid]] = tid;
         gjd_bar_sync(1, UT);
-        cplx* ob = mir + ((npanel + 1) & 1) * N * LD;      // the buffer the last update read from: free now
 #pragma unroll
-        for (int tr = 0; tr < TR; tr++)
+        for (int tr = 0; tr < TR; tr++) {
+            const int i = row0 + 8 * tr;
+            if (i >= b) continue;
+            cplx* orow = gA + (size_t)dest[i] * b;
 #pragma unroll
             for (int tc = 0; tc < TC; tc++)
 #pragma unroll
                 for (int h = 0; h < 2; h++) {
-                    const int i = row0 + 8 * tr, j = col0 + 8 * tc + h;
-                    if (i < b && j < b) ob[dest[i] * LD + piv[j]] = cmake(cre[tr][tc][h], cim[tr][tc][h]);
+                    const int j = col0 + 8 * tc + h;
+                    if (j < b) orow[piv[j]] = cmake(cre[tr][tc][h], cim[tr][tc][h]);
                 }
+        }
     }
-    gjd_bar_sync(0, GJD_ACT);
-    const cplx* ob = mir + ((npanel + 1) & 1) * N * LD;
-    for (int idx = tid; idx < b * b; idx += GJD_ACT) {
-        const int i = idx / b, j = idx - i * b;
-        gA[idx] = ob[i * LD + j];
-    }
+    gjd_bar_sync(0, GJD_ACT);                    // the panel warp's singular flag
     if (tid == 0 && *s_sing && info) info[e] = code_dev ? *code_dev + code : (code > 0 ? code : *s_sing);
 }
 
