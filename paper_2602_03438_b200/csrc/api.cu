@@ -31,7 +31,7 @@ extern "C" int negf_create(negf_ctx** out, int device) {
     c->gtick = 0;
     if (cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) != cudaSuccess) { delete c; return NEGF_ECUDA; }
     for (int k = 0; k < 4; k++) if (cudaEventCreateWithFlags(&c->ev_grp[k], cudaEventDisableTiming) != cudaSuccess) { delete c; return NEGF_ECUDA; }
-    if (cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking) != cudaSuccess) { delete c; return NEGF_ECUDA; } c->obc_key_ws = nullptr; c->obc_key_b = c->obc_key_nb = c->obc_key_maxit = 0; c->obc_key_tol = 0.0;
+    if (cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking) != cudaSuccess) { delete c; return NEGF_ECUDA; } c->obc_key_ws = nullptr; c->obc_key_b = c->obc_key_n = c->obc_key_ne = c->obc_key_ns = c->obc_key_maxit = 0; c->obc_key_tol = 0.0;
     c->prof_on = false; c->prof_depth = 0; c->prof_last_class = -1; c->prof_last_event = nullptr;
     for (int k = 0; k < NEGF_PROF_CLASSES; k++) { c->prof_ms[k] = 0.0; c->prof_n[k] = 0; }
     if (zgemm_prepare(c) != NEGF_OK || zinv_prepare(c) != NEGF_OK || econv_prepare(c) != NEGF_OK) { delete c; return NEGF_ECUDA; }
@@ -60,8 +60,15 @@ extern "C" int negf_set_stream(negf_ctx* ctx, void* s) {
 extern "C" int negf_set_workspace(negf_ctx* ctx, void* p, size_t bytes) {
     if (!ctx) return NEGF_EINVAL;
     if (p && ((uintptr_t)p & 255)) return NEGF_EINVAL;
+    const bool same = p == ctx->ws && (p ? bytes : 0) == ctx->ws_bytes;
     ctx->ws = p; ctx->ws_bytes = p ? bytes : 0; ctx->sweep_valid = false;
     for (int k = 0; k < NEGF_NGRAPH; k++) for (int q = 0; q < NEGF_GWAYS; q++) ctx->gslot[k][q].key = 0;
+    // the decimation WHILE graph has workspace addresses baked in: a new workspace drops it (its key also
+    // holds every shape parameter the carve-up depends on, should the same address come back)
+    if (!same) {
+        if (ctx->obc_exec) { cudaGraphExecDestroy(ctx->obc_exec); ctx->obc_exec = nullptr; }
+        ctx->obc_key_ws = nullptr;
+    }
     return NEGF_OK;
 }
 extern "C" int negf_set_option(negf_ctx* ctx, int option, int value) {

@@ -42,7 +42,8 @@ struct negf_ctx {
     cudaStream_t copy_stream;     // device->host copies of negf_pipeline_host
     cudaEvent_t ev_grp[4];
     cudaGraphExec_t obc_exec;
-    const void* obc_key_ws; int obc_key_b, obc_key_nb, obc_key_maxit; double obc_key_tol;
+    // every pointer baked into that graph comes from carve_workspace(ws, n, b, ne) and the batch split ns x ne
+    const void* obc_key_ws; int obc_key_b, obc_key_n, obc_key_ne, obc_key_ns, obc_key_maxit; double obc_key_tol;
     // optional per-kernel-class timing (negf_profile_enable): event pairs around every launch site
     bool prof_on;
     int prof_depth;
@@ -231,6 +232,9 @@ struct GemmArgs {
     int batch2;
     long long sA2, sB2, sD2, sC2;
     const cplx* alpha_vec;   // optional [batch]: entry e uses alpha * alpha_vec[e]
+    // C overwrites A in place (C == A, n <= 64): only safe when ONE CTA owns all n columns of its rows, so the
+    // launcher must pick a tile with BN >= n (it rejects unflagged aliasing of C with A or B otherwise)
+    int c_aliases_a = 0;
 };
 int zgemm_launch(negf_ctx* ctx, const GemmArgs& a);
 int zgemm_prepare(negf_ctx* ctx);

@@ -97,14 +97,16 @@ int obc_core(negf_ctx* ctx, const negf_problem* p, int ns, const LeadBlocks* lb,
     // Small blocks: the loop is a device-driven WHILE graph (CUDA conditional node): its body is two
     // doublings (so the ping-pong buffers have fixed roles) plus a kernel that keeps the loop going
     // while any entry is active - no masked launches after convergence, no host synchronisation.
-    // The graph is cached per (workspace, shape, tol, max_iter); profiling runs use the plain loop.
+    // The graph is cached per (workspace, n, b, N_E, leads in the batch, tol, max_iter) - everything the baked-in
+    // workspace offsets depend on - and dropped by negf_set_workspace; profiling runs use the plain loop.
     const bool use_graph = b <= 96 && (max_iter % 2 == 0) && !ctx->prof_on && ctx->graph_loops;
     if (use_graph) {
         int* it_dev = W.tmpinfo;
         NEGF_TRY(ew_copy(ctx, bb, nb, ub[1], sb, U0, sb, nullptr));
         NEGF_TRY(ew_copy(ctx, bb, nb, lbuf[1], sb, L0, sb, nullptr));
         NEGF_TRY(ew_fill_int(ctx, it_dev, 1, 0));
-        const bool hit = ctx->obc_exec && ctx->obc_key_ws == ctx->ws && ctx->obc_key_b == b && ctx->obc_key_nb == nb &&
+        const bool hit = ctx->obc_exec && ctx->obc_key_ws == ctx->ws && ctx->obc_key_b == b && ctx->obc_key_n == n &&
+                         ctx->obc_key_ne == ne && ctx->obc_key_ns == ns &&
                          ctx->obc_key_maxit == max_iter && ctx->obc_key_tol == tol;
         if (!hit) {
             if (ctx->obc_exec) { cudaGraphExecDestroy(ctx->obc_exec); ctx->obc_exec = nullptr; }
@@ -134,7 +136,7 @@ int obc_core(negf_ctx* ctx, const negf_problem* p, int ns, const LeadBlocks* lb,
             ce = cudaGraphInstantiate(&ctx->obc_exec, G, 0);
             cudaGraphDestroy(G);
             if (ce != cudaSuccess) { ctx->obc_exec = nullptr; ctx->last_cuda_error = (int)ce; return NEGF_ECUDA; }
-            ctx->obc_key_ws = ctx->ws; ctx->obc_key_b = b; ctx->obc_key_nb = nb; ctx->obc_key_maxit = max_iter; ctx->obc_key_tol = tol;
+            ctx->obc_key_ws = ctx->ws; ctx->obc_key_b = b; ctx->obc_key_n = n; ctx->obc_key_ne = ne; ctx->obc_key_ns = ns; ctx->obc_key_maxit = max_iter; ctx->obc_key_tol = tol;
         }
         NEGF_CUDA_CHECK(ctx, cudaGraphLaunch(ctx->obc_exec, ctx->stream));
     } else {

@@ -23,7 +23,8 @@ struct Layout {
     size_t total;
 };
 
-Layout make_layout(void* base, int n, int b, int ne, int kind_max, bool hasS, bool want_greater) {
+// kinds[f] = kind of Sigma^{R,<,>}_S (each family gets the buffers of its OWN kind)
+Layout make_layout(void* base, int n, int b, int ne, const int* kinds, bool hasS, bool want_greater) {
     Layout L = {};
     Bump B{(unsigned char*)base, 0};
     const size_t bb = (size_t)b * b * sizeof(cplx);
@@ -32,8 +33,8 @@ Layout make_layout(void* base, int n, int b, int ne, int kind_max, bool hasS, bo
     if (hasS) { L.Sd = (cplx*)B.take(bb * n); L.Su = (cplx*)B.take(bb * m); }
     L.energy = (double*)B.take(sizeof(double) * ne); L.weights = (double*)B.take(sizeof(double) * ne);
     for (int f = 0; f < 3; f++) {
-        if (kind_max == NEGF_SIGMA_SCALAR) L.sig[f][0] = (cplx*)B.take(sizeof(cplx) * ne);
-        if (kind_max == NEGF_SIGMA_BT) {
+        if (kinds[f] == NEGF_SIGMA_SCALAR) L.sig[f][0] = (cplx*)B.take(sizeof(cplx) * ne);
+        if (kinds[f] == NEGF_SIGMA_BT) {
             L.sig[f][1] = (cplx*)B.take(bb * n * ne); L.sig[f][2] = (cplx*)B.take(bb * m * ne);
             if (f == 0) L.sig[f][3] = (cplx*)B.take(bb * m * ne);
         }
@@ -50,7 +51,7 @@ Layout make_layout(void* base, int n, int b, int ne, int kind_max, bool hasS, bo
     L.trans = (double*)B.take(sizeof(double) * ne); L.bond = (double*)B.take(sizeof(double) * ne * (m > 0 ? m : 1));
     L.contact = (double*)B.take(sizeof(double) * ne * 2);
     L.info_r = (int*)B.take(sizeof(int) * ne); L.info_x = (int*)B.take(sizeof(int) * ne);
-    Workspace W = carve_workspace(nullptr, n, b, ne, hasS || kind_max == NEGF_SIGMA_BT);
+    Workspace W = carve_workspace(nullptr, n, b, ne, hasS || kinds[0] == NEGF_SIGMA_BT);
     L.ws_bytes = W.bytes; L.ws = B.take(W.bytes);
     L.total = B.off;
     return L;
@@ -76,7 +77,8 @@ __global__ void sum_groups_kernel(double* d, int len, int ng) {
 
 extern "C" int negf_pipeline_host_bytes(const negf_problem* p, int kind_max, int want_greater, size_t* bytes) {
     if (!p || !bytes || p->n_blocks < 1 || p->block_size < 1 || p->n_energy < 1) return NEGF_EINVAL;
-    Layout L = make_layout(nullptr, p->n_blocks, p->block_size, p->n_energy, kind_max, true, want_greater != 0);
+    const int kinds[3] = {kind_max, kind_max, kind_max};      // an upper bound for any mix of kinds up to kind_max
+    Layout L = make_layout(nullptr, p->n_blocks, p->block_size, p->n_energy, kinds, true, want_greater != 0);
     *bytes = L.total;
     return NEGF_OK;
 }
@@ -91,10 +93,16 @@ extern "C" int negf_pipeline_host(negf_ctx* ctx, const negf_problem* hp, const n
     if (n < 2 || b < 1 || ne < 1 || !hp->H_diag || !hp->H_upper || !hp->energy) return NEGF_EINVAL;
     const bool hasS = hp->S_diag != nullptr;
     const bool want_g = hsg != nullptr;
-    int kind = NEGF_SIGMA_NONE;
+    int kinds[3] = {NEGF_SIGMA_NONE, NEGF_SIGMA_NONE, NEGF_SIGMA_NONE};
     const negf_sigma* hs[3] = {hsr, hsl, hsg};
-    for (int f = 0; f < 3; f++) if (hs[f] && hs[f]->kind > kind) kind = hs[f]->kind;
-    Layout L = make_layout(dev_scratch, n, b, ne, kind, hasS, want_g);
+    for (int f = 0; f < 3; f++) {
+        if (!hs[f]) continue;
+        kinds[f] = hs[f]->kind;
+        if (kinds[f] == NEGF_SIGMA_SCALAR && !hs[f]->scalar) return NEGF_EINVAL;
+        if (kinds[f] == NEGF_SIGMA_BT && (!hs[f]->diag || !hs[f]->upper || (f == 0 && !hs[f]->lower))) return NEGF_EINVAL;
+        if (kinds[f] < NEGF_SIGMA_NONE || kinds[f] > NEGF_SIGMA_BT) return NEGF_EINVAL;
+    }
+    Layout L = make_layout(dev_scratch, n, b, ne, kinds, hasS, want_g);
     if (L.total > dev_scratch_bytes) return NEGF_ENOWORKSPACE;
     const size_t bb = (size_t)b * b * sizeof(cplx);
     const int m = n - 1;
@@ -139,7 +147,12 @@ extern "C" int negf_pipeline_host(negf_ctx* ctx, const negf_problem* hp, const n
     dp.S_diag = hasS ? (negf_c128*)L.Sd : nullptr; dp.S_upper = hasS ? (negf_c128*)L.Su : nullptr;
     dp.energy = L.energy;
 
-    void* old_ws = ctx->ws; size_t old_bytes = ctx->ws_bytes;
+    // the four calls below run on the staging workspace; the caller's workspace comes back on EVERY exit path,
+    // after the copy stream has drained (it reads the staging buffers)
+    struct WsGuard {
+        negf_ctx* c; void* ws; size_t bytes;
+        ~WsGuard() { cudaStreamSynchronize(c->copy_stream); c->ws = ws; c->ws_bytes = bytes; c->sweep_valid = false; }
+    } ws_guard{ctx, ctx->ws, ctx->ws_bytes};
     ctx->ws = L.ws; ctx->ws_bytes = L.ws_bytes; ctx->sweep_valid = false;
     // The device->host copies run on the copy stream and overlap the compute that follows them: G^R goes
     // home while G^<> is computed.  (Splitting the batch into energy groups to overlap more was measured
@@ -215,8 +228,7 @@ extern "C" int negf_pipeline_host(negf_ctx* ctx, const negf_problem* hp, const n
             NEGF_CUDA_CHECK(ctx, D2Hc(off(out->GG_upper, fam_m * lo), GGu, fam_m * cnt));
         }
     }
-    ctx->ws = old_ws; ctx->ws_bytes = old_bytes; ctx->sweep_valid = false;
-    if (rc) { cudaStreamSynchronize(cs); return rc; }
+    if (rc) { cudaStreamSynchronize(st); return rc; }
     if (out->density) {          // total density = sum of the groups' partial densities, fixed order
         sum_groups_kernel<<<(n * b + 255) / 256, 256, 0, st>>>(L.density, n * b, ng);
         NEGF_LAUNCH_CHECK(ctx);

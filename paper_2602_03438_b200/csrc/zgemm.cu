@@ -473,6 +473,17 @@ int zgemm_launch_group(negf_ctx* ctx, const GemmGroup& grp) {
             o.batch2 != a.batch2)
             return NEGF_EINVAL;
     }
+    // In-place products.  C == A is safe only when one CTA owns all n columns of the rows it reads (every read of
+    // a CTA is complete before its first store: the last k-block's wait + barrier precede the epilogue), so the
+    // caller flags it and gets a tile with BN >= n; unflagged aliasing of C with an operand is rejected when
+    // more than one CTA would share the operand's rows / columns.
+    bool alias_a = false;
+    for (int i = 0; i < grp.ng; i++) {
+        const GemmArgs& o = grp.g[i];
+        if (o.c_aliases_a) { alias_a = true; if (o.n > 64 || o.opA != 0) return NEGF_EINVAL; continue; }
+        if ((const cplx*)o.C == o.A && o.n > 16) return NEGF_EINVAL;
+        if ((const cplx*)o.C == o.B && o.m > 16) return NEGF_EINVAL;
+    }
     // Tile choice: the largest CTA tile that still gives every SM work.  128x64 (8 warps, 32x32 warp
     // tiles, 1 CTA/SM) in the compute-bound regime; 64x64 (4 warps); 32x32 (4 warps of 16x16, up to
     // 4 CTAs/SM) when the batch of small blocks would otherwise leave most SMs idle.
@@ -493,8 +504,9 @@ int zgemm_launch_group(negf_ctx* ctx, const GemmGroup& grp) {
     // bound by the length of one warp's DMMA chain, not by the pipe: 16x16 tiles (4 warps of 8x8) quarter that chain.
     // Measured on configs[1] with the threshold at 1 / 2 / 4 / always: 2 is best (5.97 -> 5.83 ms per step as 4
     // energy groups, 6.41 -> 6.11 ms on one stream; always: 6.00 / 6.26 ms).
+    if (alias_a && a.n > 32) return launch_ops<64, 64, 2, 2, 2>(ctx, grp);
     const long long t32 = (long long)((a.m + 31) / 32) * ((a.n + 31) / 32) * per;
-    if (t32 < 2LL * ctx->num_sms) return launch_ops<16, 16, 2, 2, 6>(ctx, grp);
+    if (t32 < 2LL * ctx->num_sms && !(alias_a && a.n > 16)) return launch_ops<16, 16, 2, 2, 6>(ctx, grp);
     return launch_ops<32, 32, 2, 2, 5>(ctx, grp);
 }
 

@@ -229,7 +229,7 @@ __global__ void __launch_bounds__(GJ_NW * 32) gj_reg_kernel(cplx* A, long long s
             if (i < b && j < b) g[(size_t)dest[i] * b + piv[j]] = cmul(m[r][c], rs);
         }
     }
-    if (tid == 0 && s_sing && info) info[e] = code_dev ? *code_dev + code : (code > 0 ? code : s_sing);
+    if (tid == 0 && s_sing && info && info[e] == 0) info[e] = code_dev ? *code_dev + code : (code > 0 ? code : s_sing);   // first failure wins
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -545,7 +545,7 @@ __global__ void __launch_bounds__(GJD_NT, 1) gj_dmma_kernel(cplx* A, long long s
         }
     }
     gjd_bar_sync(0, GJD_ACT);                    // the panel warp's singular flag
-    if (tid == 0 && *s_sing && info) info[e] = code_dev ? *code_dev + code : (code > 0 ? code : *s_sing);
+    if (tid == 0 && *s_sing && info && info[e] == 0) info[e] = code_dev ? *code_dev + code : (code > 0 ? code : *s_sing);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -1206,7 +1206,9 @@ int zinv_launch(negf_ctx* ctx, int b, cplx* A, long long sA, int batch, void* ws
                 g.alpha = mone; g.beta = zero; g.D = nullptr; g.sD = 0;
                 g.m = k0; g.n = wk; g.k = wk; g.A = A + k0; g.lda = b; g.sA = sA;
                 g.B = W.Dinv; g.ldb = wk; g.sB = PW * PW; g.C = A + k0; g.ldc = b; g.sC = sA;
+                g.c_aliases_a = 1;         // tile with BN >= wk: one CTA owns all wk columns of its rows
                 NEGF_TRY(zgemm_launch(ctx, g));
+                g.c_aliases_a = 0;
             }
             // M[:, other columns of K] += P' R, P' read from the panel's own columns
             g.alpha = one; g.beta = one; g.m = b; g.k = wk; g.A = A + k0; g.lda = b; g.sA = sA;
@@ -1301,5 +1303,6 @@ extern "C" int negf_zinverse_batched(negf_ctx* ctx, int b, negf_c128* A, long lo
     size_t need = zinv_workspace_bytes(b, batch);
     if (b > SMALL_MAX && (!ctx->ws || ctx->ws_bytes < need)) return NEGF_ENOWORKSPACE;
     if (info) NEGF_CUDA_CHECK(ctx, cudaMemsetAsync(info, 0, sizeof(int) * batch, ctx->stream));
+    if (b > SMALL_MAX) ctx->sweep_valid = false;     // the scratch below overlays the retained sweep state
     return zinv_launch(ctx, b, (cplx*)A, stride, batch, ctx->ws, info, 0, nullptr);
 }
