@@ -68,6 +68,15 @@ typedef struct {
     const negf_c128* S_upper;  /* [n-1][b][b] S_{i,i+1}; S_{i+1,i} = S_{i,i+1}^H               */
     const double*    energy;   /* [N_E] real energies E                                         */
     double           eta;      /* z = E + i*eta multiplies S everywhere, leads included (R1)   */
+    /* Momentum (k-point) batching ("the momentum dependence is omitted for simplicity"; SURVEY.md
+     * 8(f) item 2): n_k > 1 makes H_diag / H_upper / S_diag / S_upper arrays of n_k devices, [n_k][n][b][b] and
+     * [n_k][n-1][b][b], and k_index [N_E] (DEVICE ints in [0, n_k)) names the device of every batch entry, so
+     * the batch axis is any list of (k, E) pairs: one lock-step batch of N_E entries, e.g. N_k x N_E' in k-major
+     * order with `energy` repeating the grid.  n_k <= 1 (or k_index NULL): one device, as above.  Every
+     * per-energy array of the calls below is per batch entry.  Sums over k (density, T) are the caller's:
+     * negf_observables folds weights[e] (= w_k w_E) into the density. */
+    int              n_k;
+    const int*       k_index;
 } negf_problem;
 
 /* One self-energy family: boundary blocks on the two contacts plus Sigma_S.
@@ -85,7 +94,8 @@ typedef struct {
 } negf_sigma;
 
 /* Optional explicit lead (overrides "periodic copies of the contact blocks", reading R2;
- * required when n_blocks == 1).  H_u/S_u couple a lead cell to its next cell on the right. */
+ * required when n_blocks == 1).  H_u/S_u couple a lead cell to its next cell on the right.
+ * With k-point batching (negf_problem.n_k > 1) every member is [n_k][b][b]. */
 typedef struct {
     const negf_c128* H_d;      /* [b][b] */
     const negf_c128* H_u;      /* [b][b] */
@@ -116,10 +126,23 @@ int negf_set_workspace(negf_ctx* ctx, void* dev_ptr, size_t bytes);
  * rank-4 updates run on the FP64 tensor pipe (one CTA per matrix, same partial pivoting and the same order
  * of elimination updates per element as the unblocked kernel); 0 = the register-resident unblocked
  * Gauss-Jordan kernel for every block size up to 96 (the kernel 65..96 and 1..16 always use).  Set it
- * before the first call of a shape (cached call graphs keep the kernel they were captured with). */
-#define NEGF_OPT_GRAPH_LOOPS 1
-#define NEGF_OPT_GEMM_3M     2
-#define NEGF_OPT_INV_TENSOR  3
+ * before the first call of a shape (cached call graphs keep the kernel they were captured with).
+ * NEGF_OPT_ENERGY_GROUPS (default 0 = automatic): number of concurrent energy groups (1..4) that
+ * negf_pipeline_device / negf_pipeline_host split the batch into.  K3, the energy-batch scheduler: in the
+ * latency-bound small-block regime every launch of the sequential chains leaves SMs idle, so the batch runs as
+ * groups of energies that walk the whole path S2-S7 concurrently on streams owned by the context (one group's
+ * inversions overlap another's products); same arithmetic per energy, same outputs.  Automatic = 4 groups for
+ * block sizes up to 96 with at least 32 energies, else 1 (at large blocks every launch fills the GPU).
+ * NEGF_OPT_INV_PANEL (default 1): panels of the blocked inverse (97 <= b <= 2048) are eliminated by the
+ * row-per-thread Gauss-Jordan kernel (all rows of the matrix, partial pivoting on the leading 32 bits of
+ * |re|+|im|); 0 = the first panel kernel (LU of the rows at and below the panel, lane = panel column), which
+ * larger blocks always use.  Same pivoting rule up to the key width, same results up to rounding. */
+#define NEGF_OPT_GRAPH_LOOPS   1
+#define NEGF_OPT_GEMM_3M       2
+#define NEGF_OPT_INV_TENSOR    3
+#define NEGF_OPT_ENERGY_GROUPS 4
+#define NEGF_OPT_INV_PANEL     5
+#define NEGF_MAX_ENERGY_GROUPS 4
 int negf_set_option(negf_ctx* ctx, int option, int value);
 const char* negf_strerror(int code);
 /* cudaError_t of the last failing runtime call on this context (0 if none). */
@@ -235,6 +258,28 @@ int negf_observables(negf_ctx* ctx, const negf_problem* p,
 int negf_energy_convolve(negf_ctx* ctx, int n_energy, long long elems_per_energy, int transpose_block,
                          const negf_c128* X1, const negf_c128* X2, int mode, int conj2, negf_c128 scale,
                          negf_c128* Y);
+
+/* ---- whole path with DEVICE buffers: S2 -> S7 in one call (Fig. 1 "LSE+OBC") --------
+ * negf_obc_decimate_pair -> negf_rgf_retarded (NEGF_KEEP_SWEEP) -> negf_rgf_lesser_greater -> negf_observables on
+ * one energy batch, all arrays DEVICE pointers owned by the caller.  This is the call the energy-batch scheduler
+ * (K3) sees the whole path through: it may split the batch into concurrent energy groups (NEGF_OPT_ENERGY_GROUPS),
+ * each on a stream and a slice of the workspace owned by the context; everything is forked from the context's
+ * stream and joined back to it before the call returns (asynchronous like the four calls, no host synchronisation).
+ * sigma_*: Sigma_S only (left / right members are ignored: the boundary blocks come from the decimation);
+ * sigma_greater NULL = no G^>.  Members of negf_device_outputs: left / right as negf_obc_out with sigma_r, gamma,
+ * sigma_lesser, sigma_greater, iters, status required; GR_diag, GL_diag, info_r, info_x required; GG_diag required
+ * when sigma_greater is given; the other pointers may be NULL (skipped).  Results are identical to the four calls
+ * made one after the other on the same batch (the density is summed over the groups in a fixed order). */
+typedef struct {
+    negf_obc_out left, right;
+    negf_c128 *GR_diag, *GR_upper, *GR_lower, *GR_corner, *GL_diag, *GL_upper, *GG_diag, *GG_upper;
+    double *density, *ldos, *transmission, *bond_current, *contact_current;
+    int *info_r, *info_x;
+} negf_device_outputs;
+int negf_pipeline_device(negf_ctx* ctx, const negf_problem* p,
+                         const negf_sigma* sigma_r, const negf_sigma* sigma_lesser, const negf_sigma* sigma_greater,
+                         const double* weights, double mu_L, double mu_R, double kT, double tol, int max_iter,
+                         const negf_device_outputs* out);
 
 /* ---- whole path with HOST buffers (bench.py's end-to-end leg) ---------------------------------
  * All array arguments here are HOST pointers (pinned memory recommended).  Copies the inputs

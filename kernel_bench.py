@@ -1,8 +1,8 @@
 """Micro-benchmarks of the K1/K2 building blocks through the C ABI:
 
-    python -m paper_2602_03438_b200.kernel_bench --kernel zgemm --b 1024 --batch 16 [--opA 0 --opB 1]
-    python -m paper_2602_03438_b200.kernel_bench --kernel zinv  --b 1024 --batch 16
-    python -m paper_2602_03438_b200.kernel_bench --kernel peak
+    python kernel_bench.py --kernel zgemm --b 1024 --batch 16 [--opA 0 --opB 1]
+    python kernel_bench.py --kernel zinv  --b 1024 --batch 16 [--inv-panel 0]
+    python kernel_bench.py --kernel peak
 
 Prints one JSON line per run: achieved FP64 TFLOP/s (8 b^3 real flops per complex product or
 inversion, the unit U of SURVEY.md 8(d)) and the fraction of the DMMA issue-rate peak probed in
@@ -16,10 +16,14 @@ import json
 
 import torch
 
-from . import build as _build
+import os
+import sys
+
+sys.path.insert(0, os.path.dirname(os.path.abspath(__file__)))
+from paper_2602_03438_b200 import build as _build  # noqa: E402
 
 _build.ensure_built()
-from . import negf  # noqa: E402
+from paper_2602_03438_b200 import negf  # noqa: E402
 
 
 def _rand(shape, gen):
@@ -36,6 +40,7 @@ def main():
     ap.add_argument("--opB", type=int, default=0)
     ap.add_argument("--reps", type=int, default=10)
     ap.add_argument("--sets", type=int, default=2, help="operand sets rotated between launches")
+    ap.add_argument("--inv-panel", type=int, default=1, help="NEGF_OPT_INV_PANEL (1 = row-per-thread Gauss-Jordan panel, 0 = first LU panel kernel)")
     ap.add_argument("--gemm-3m", action="store_true", help="NEGF_OPT_GEMM_3M (tflops still counted as 8 b^3 per product)")
     args = ap.parse_args()
     ctx = negf.Context(0)
@@ -43,6 +48,7 @@ def main():
     ctx.set_stream(st.cuda_stream)
     if args.gemm_3m:
         ctx.set_option(negf.OPT_GEMM_3M, 1)
+    ctx.set_option(negf.OPT_INV_PANEL, args.inv_panel)
     peak = ctx.fp64_peak(200.0)
     if args.kernel == "peak":
         print(json.dumps({"kernel": "dmma_peak_probe", "tflops": peak}))
@@ -68,7 +74,7 @@ def main():
         import os
         peak_gbs = None
         try:
-            peak_gbs = json.load(open(os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "MEASURED_PEAKS.json")))["hbm_gbs"]
+            peak_gbs = json.load(open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "MEASURED_PEAKS.json")))["hbm_gbs"]
         except Exception:
             peak_gbs = 6650.0     # fallback of the profiling recipe
         gbs = nbytes / (ms * 1e-3) * 1e-9

@@ -26,12 +26,14 @@ extern "C" int negf_create(negf_ctx** out, int device) {
             cudaEventCreateWithFlags(&c->ev_join[k], cudaEventDisableTiming) != cudaSuccess) { delete c; return NEGF_ECUDA; }
     }
     if (cudaEventCreateWithFlags(&c->ev_aux, cudaEventDisableTiming) != cudaSuccess) { delete c; return NEGF_ECUDA; }
-    c->graph_loops = true; c->gemm_3m = false; c->inv_tensor = 1; c->obc_exec = nullptr;
+    c->graph_loops = true; c->gemm_3m = false; c->inv_tensor = 1; c->inv_panel = 1; c->obc_exec = nullptr;
     for (int k = 0; k < NEGF_NGRAPH; k++) for (int q = 0; q < NEGF_GWAYS; q++) c->gslot[k][q] = {0ull, nullptr, 0, 0u};
     c->gtick = 0;
     if (cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) != cudaSuccess) { delete c; return NEGF_ECUDA; }
     for (int k = 0; k < 4; k++) if (cudaEventCreateWithFlags(&c->ev_grp[k], cudaEventDisableTiming) != cudaSuccess) { delete c; return NEGF_ECUDA; }
     if (cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking) != cudaSuccess) { delete c; return NEGF_ECUDA; } c->obc_key_ws = nullptr; c->obc_key_b = c->obc_key_n = c->obc_key_ne = c->obc_key_ns = c->obc_key_maxit = 0; c->obc_key_tol = 0.0;
+    c->energy_groups = 0; c->ev_grp_fork = nullptr;
+    for (int k = 0; k < NEGF_MAX_ENERGY_GROUPS; k++) { c->child[k] = nullptr; c->grp_stream[k] = nullptr; c->ev_grp_mid[k] = nullptr; }
     c->prof_on = false; c->prof_depth = 0; c->prof_last_class = -1; c->prof_last_event = nullptr;
     for (int k = 0; k < NEGF_PROF_CLASSES; k++) { c->prof_ms[k] = 0.0; c->prof_n[k] = 0; }
     if (zgemm_prepare(c) != NEGF_OK || zinv_prepare(c) != NEGF_OK || econv_prepare(c) != NEGF_OK) { delete c; return NEGF_ECUDA; }
@@ -49,6 +51,12 @@ extern "C" int negf_destroy(negf_ctx* ctx) {
     cudaStreamDestroy(ctx->copy_stream);
     for (int k = 0; k < 4; k++) cudaEventDestroy(ctx->ev_grp[k]);
     cudaStreamDestroy(ctx->cap_stream);
+    for (int k = 0; k < NEGF_MAX_ENERGY_GROUPS; k++) {
+        if (ctx->child[k]) negf_destroy(ctx->child[k]);
+        if (ctx->grp_stream[k]) cudaStreamDestroy(ctx->grp_stream[k]);
+        if (ctx->ev_grp_mid[k]) cudaEventDestroy(ctx->ev_grp_mid[k]);
+    }
+    if (ctx->ev_grp_fork) cudaEventDestroy(ctx->ev_grp_fork);
     delete ctx;
     return NEGF_OK;
 }
@@ -76,6 +84,11 @@ extern "C" int negf_set_option(negf_ctx* ctx, int option, int value) {
     if (option == NEGF_OPT_GRAPH_LOOPS) { ctx->graph_loops = value != 0; return NEGF_OK; }
     if (option == NEGF_OPT_GEMM_3M) { ctx->gemm_3m = value != 0; return NEGF_OK; }
     if (option == NEGF_OPT_INV_TENSOR) { ctx->inv_tensor = value; return NEGF_OK; }
+    if (option == NEGF_OPT_INV_PANEL) { ctx->inv_panel = value; return NEGF_OK; }
+    if (option == NEGF_OPT_ENERGY_GROUPS) {
+        if (value < 0 || value > NEGF_MAX_ENERGY_GROUPS) return NEGF_EINVAL;
+        ctx->energy_groups = value; return NEGF_OK;
+    }
     return NEGF_EINVAL;
 }
 extern "C" const char* negf_strerror(int code) {

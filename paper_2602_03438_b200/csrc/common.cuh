@@ -33,6 +33,7 @@ struct negf_ctx {
     bool graph_loops;             // negf_set_option(NEGF_OPT_GRAPH_LOOPS)
     bool gemm_3m;                 // negf_set_option(NEGF_OPT_GEMM_3M)
     int inv_tensor;               // negf_set_option(NEGF_OPT_INV_TENSOR)
+    int inv_panel;                // negf_set_option(NEGF_OPT_INV_PANEL)
     // cached CUDA graphs of whole calls in the latency-bound regime (same arguments twice in a row
     // -> the second call is captured, later ones replay it); one slot per entry point
     struct GraphSlot { unsigned long long key; cudaGraphExec_t exec; long long launches; unsigned used; };
@@ -41,6 +42,12 @@ struct negf_ctx {
     cudaStream_t cap_stream;      // capture stream (the caller's may be the legacy default stream)
     cudaStream_t copy_stream;     // device->host copies of negf_pipeline_host
     cudaEvent_t ev_grp[4];
+    // concurrent energy groups of negf_pipeline_device / _host (K3): child contexts (own side streams and
+    // graph caches), created on first use, each on its own stream
+    int energy_groups;            // negf_set_option(NEGF_OPT_ENERGY_GROUPS); 0 = automatic
+    negf_ctx* child[NEGF_MAX_ENERGY_GROUPS];
+    cudaStream_t grp_stream[NEGF_MAX_ENERGY_GROUPS];
+    cudaEvent_t ev_grp_fork, ev_grp_mid[NEGF_MAX_ENERGY_GROUPS];
     cudaGraphExec_t obc_exec;
     // every pointer baked into that graph comes from carve_workspace(ws, n, b, ne) and the batch split ns x ne
     const void* obc_key_ws; int obc_key_b, obc_key_n, obc_key_ne, obc_key_ns, obc_key_maxit; double obc_key_tol;

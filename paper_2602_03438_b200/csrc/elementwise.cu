@@ -16,11 +16,12 @@ __global__ void combine_kernel(const __grid_constant__ CombineArgs a) {
     const int r = idx / b, c = idx % b;
     const int fi = blockIdx.z;
     const size_t src = (a.dagger ? c * b + r : idx);
+    const size_t kk = a.kidx ? (size_t)a.kidx[e] : 0;
     cplx v = cmake(0.0, 0.0);
     if (a.use_z) {
         cplx z = cmake(a.energy[e], a.eta);
         if (a.S) {
-            cplx s = a.S[src + (size_t)fi * a.fS];
+            cplx s = a.S[src + (size_t)fi * a.fS + kk * a.kS];
             if (a.dagger) s = cconj(s);
             v = cmul(z, s);
         } else if (a.s_identity && r == c) {
@@ -28,7 +29,7 @@ __global__ void combine_kernel(const __grid_constant__ CombineArgs a) {
         }
     }
     if (a.H) {
-        cplx h = a.H[src + (size_t)fi * a.fH];
+        cplx h = a.H[src + (size_t)fi * a.fH + kk * a.kH];
         if (a.dagger) h = cconj(h);
         v = csub(v, h);
     }

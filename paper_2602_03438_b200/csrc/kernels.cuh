@@ -20,6 +20,9 @@ struct CombineArgs {
     int nfam;
     long long fH, fS, fout, fblk[3];
     int only[3];
+    // k-point batching: entry e reads H + kidx[e] * kH and S + kidx[e] * kS (kidx NULL: one device)
+    const int* kidx;
+    long long kH, kS;
 };
 int ew_combine(negf_ctx* ctx, const CombineArgs& a, int batch);
 // C = Z + sign * (V - V^H)   (Z may be NULL)

@@ -15,7 +15,7 @@
 
 namespace {
 
-struct LeadBlocks { const cplx *Hd, *Hu, *Sd, *Su; };
+struct LeadBlocks { const cplx *Hd, *Hu, *Sd, *Su; long long kd, ku; };   // kd / ku: strides between k-points
 
 int resolve_lead(const negf_problem* p, const negf_lead* lead, int side, LeadBlocks* out) {
     const int n = p->n_blocks;
@@ -23,11 +23,13 @@ int resolve_lead(const negf_problem* p, const negf_lead* lead, int side, LeadBlo
     if (lead) {
         out->Hd = (const cplx*)lead->H_d; out->Hu = (const cplx*)lead->H_u;
         out->Sd = (const cplx*)lead->S_d; out->Su = (const cplx*)lead->S_u;
+        out->kd = out->ku = (long long)bb;
         return (out->Hd && out->Hu) ? NEGF_OK : NEGF_EINVAL;
     }
     if (n < 2 || !p->H_diag || !p->H_upper) return NEGF_EINVAL;   // periodic copies need two blocks (R2)
     const cplx* HD = (const cplx*)p->H_diag; const cplx* HU = (const cplx*)p->H_upper;
     const cplx* SD = (const cplx*)p->S_diag; const cplx* SU = (const cplx*)p->S_upper;
+    out->kd = (long long)bb * n; out->ku = (long long)bb * (n - 1);
     if (side == 0) { out->Hd = HD; out->Hu = HU; out->Sd = SD; out->Su = SU; }
     else {
         out->Hd = HD + bb * (n - 1); out->Hu = HU + bb * (n - 2);
@@ -54,9 +56,11 @@ int obc_core(negf_ctx* ctx, const negf_problem* p, int ns, const LeadBlocks* lb,
         const size_t off = (size_t)s * ne * bb;
         CombineArgs ca = {};
         ca.b = b; ca.energy = p->energy; ca.eta = p->eta; ca.use_z = 1; ca.coef = -1.0; ca.sout = sb; ca.skip = nullptr;
+        ca.kidx = p->n_k > 1 ? p->k_index : nullptr;
         ca.H = lb[s].Hd; ca.S = lb[s].Sd; ca.s_identity = lb[s].Sd ? 0 : 1; ca.dagger = 0; ca.out = a_s + off;
+        ca.kH = ca.kS = lb[s].kd;
         NEGF_TRY(ew_combine(ctx, ca, ne));
-        ca.H = lb[s].Hu; ca.S = lb[s].Su; ca.s_identity = 0;
+        ca.H = lb[s].Hu; ca.S = lb[s].Su; ca.s_identity = 0; ca.kH = ca.kS = lb[s].ku;
         ca.dagger = 0; ca.out = (sides[s] == 0 ? U0 : L0) + off;      // a_u
         NEGF_TRY(ew_combine(ctx, ca, ne));
         ca.dagger = 1; ca.out = (sides[s] == 0 ? L0 : U0) + off;      // a_l
@@ -172,6 +176,7 @@ int check_common(const negf_ctx* ctx, const negf_problem* p, int max_iter) {
     if (!ctx || !p) return NEGF_EINVAL;
     if (p->n_blocks < 1 || p->block_size < 1 || p->n_energy < 1 || max_iter < 1 || !p->energy) return NEGF_EINVAL;
     if ((p->S_diag == nullptr) != (p->S_upper == nullptr) && p->n_blocks > 1) return NEGF_EINVAL;
+    if (p->n_k > 1 && !p->k_index) return NEGF_EINVAL;
     if (!ctx->ws) return NEGF_ENOWORKSPACE;
     return NEGF_OK;
 }

@@ -23,9 +23,10 @@ __device__ __forceinline__ double block_sum(double v) {
 
 // LDOS_i(E) = -(1/pi) Im Tr[(G^R S)_ii];  grid (n, NE)
 __global__ void ldos_kernel(int n, int b, const cplx* GRd, const cplx* GRu, const cplx* GRl,
-                            const cplx* Sd, const cplx* Su, double* ldos) {
+                            const cplx* Sd, const cplx* Su, const int* kidx, double* ldos) {
     const int i = blockIdx.x, e = blockIdx.y;
     const size_t bb = (size_t)b * b;
+    if (kidx && Sd) { Sd += (size_t)kidx[e] * n * bb; Su += (size_t)kidx[e] * (n - 1) * bb; }   // k-point batching
     const cplx* G = GRd + ((size_t)e * n + i) * bb;
     double acc = 0.0;   // imaginary part of the trace
     if (!Sd) {
@@ -52,8 +53,8 @@ __global__ void ldos_kernel(int n, int b, const cplx* GRd, const cplx* GRu, cons
 }
 
 // density_k = sum_E w_E Im[(G^< S)_kk] / (2 pi); one warp per k; terms with row-contiguous reads.
-__global__ void density_rows_kernel(int n, int b, int ne, const cplx* GLd, const cplx* GLu, const cplx* Sd,
-                                    const cplx* Su, const double* w, double* density) {
+__global__ void density_rows_kernel(int n, int b, int ne, const cplx* GLd, const cplx* GLu, const cplx* Sd0,
+                                    const cplx* Su0, const int* kidx, const double* w, double* density) {
     const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (warp >= n * b) return;
     const int i = warp / b, r = warp % b;
@@ -62,6 +63,8 @@ __global__ void density_rows_kernel(int n, int b, int ne, const cplx* GLd, const
     for (int e = 0; e < ne; e++) {
         double im = 0.0;
         const cplx* G = GLd + ((size_t)e * n + i) * bb + (size_t)r * b;
+        const cplx* Sd = Sd0; const cplx* Su = Su0;
+        if (kidx && Sd0) { Sd += (size_t)kidx[e] * n * bb; Su += (size_t)kidx[e] * (n - 1) * bb; }
         if (!Sd) {
             if (lane == 0) im = G[r].y;
         } else {
@@ -80,16 +83,16 @@ __global__ void density_rows_kernel(int n, int b, int ne, const cplx* GLd, const
 }
 // third term (S != I, i > 0): sum_c G^<_{i,i-1}[r][c] S_{i-1,i}[c][r], G^<_{i,i-1}[r][c] = -conj(GLu[i-1][c][r]);
 // thread per r walks down column r of both arrays (coalesced across threads).
-__global__ void density_cols_kernel(int n, int b, int ne, const cplx* GLu, const cplx* Su, const double* w,
-                                    double* density) {
+__global__ void density_cols_kernel(int n, int b, int ne, const cplx* GLu, const cplx* Su, const int* kidx,
+                                    const double* w, double* density) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= n * b) return;
     const int i = k / b, r = k % b;
     if (i == 0) return;
     const size_t bb = (size_t)b * b;
     double acc = 0.0;
-    const cplx* S = Su + (size_t)(i - 1) * bb;
     for (int e = 0; e < ne; e++) {
+        const cplx* S = Su + (size_t)(i - 1) * bb + (kidx ? (size_t)kidx[e] * (n - 1) * bb : 0);
         const cplx* G = GLu + ((size_t)e * (n - 1) + i - 1) * bb;
         double im = 0.0;
         for (int c = 0; c < b; c++) {
@@ -115,13 +118,14 @@ __global__ void dot_conj_kernel(int b, const cplx* A, long long sA, const cplx* 
 }
 
 // J_i(E) = 2 Re Tr[(H_up[i] - E S_up[i]) G^<_{i+1,i}] = -2 Re sum (H - E S)[r][c] conj(GLu[r][c]); grid (n-1, NE)
-__global__ void bond_current_kernel(int n, int b, const cplx* Hu, const cplx* Su, const double* energy,
+__global__ void bond_current_kernel(int n, int b, const cplx* Hu, const cplx* Su, const int* kidx, const double* energy,
                                     const cplx* GLu, double* out) {
     const int i = blockIdx.x, e = blockIdx.y;
     const size_t bb = (size_t)b * b;
     const double E = energy[e];
-    const cplx* H = Hu + (size_t)i * bb;
-    const cplx* S = Su ? Su + (size_t)i * bb : nullptr;
+    const size_t koff = kidx ? (size_t)kidx[e] * (n - 1) * bb : 0;
+    const cplx* H = Hu + (size_t)i * bb + koff;
+    const cplx* S = Su ? Su + (size_t)i * bb + koff : nullptr;
     const cplx* G = GLu + ((size_t)e * (n - 1) + i) * bb;
     double acc = 0.0;
     for (int idx = threadIdx.x; idx < (int)bb; idx += blockDim.x) {
@@ -171,11 +175,13 @@ extern "C" int negf_observables(negf_ctx* ctx, const negf_problem* p,
     const bool hasS = p->S_diag != nullptr;
     if (ne > 65535) return NEGF_EUNSUPPORTED;
     ProfScope _ps(ctx, NEGF_PROF_OBSERVABLES);
+    if (p->n_k > 1 && !p->k_index) return NEGF_EINVAL;
+    const int* kidx = p->n_k > 1 ? p->k_index : nullptr;        // k-point batching: S, H of the entry's own device
     if (ldos) {
         if (!GR_diag || (hasS && n > 1 && (!GR_upper || !GR_lower || !p->S_upper))) return NEGF_EINVAL;
         ldos_kernel<<<dim3(n, ne), 256, 0, ctx->stream>>>(n, b, (const cplx*)GR_diag, (const cplx*)GR_upper,
                                                           (const cplx*)GR_lower, (const cplx*)p->S_diag,
-                                                          (const cplx*)p->S_upper, ldos);
+                                                          (const cplx*)p->S_upper, kidx, ldos);
         NEGF_LAUNCH_CHECK(ctx);
     }
     if (density) {
@@ -183,11 +189,11 @@ extern "C" int negf_observables(negf_ctx* ctx, const negf_problem* p,
         long long threads = (long long)n * b * 32;
         density_rows_kernel<<<(unsigned)((threads + 255) / 256), 256, 0, ctx->stream>>>(
             n, b, ne, (const cplx*)GL_diag, (const cplx*)GL_upper, (const cplx*)p->S_diag, (const cplx*)p->S_upper,
-            weights, density);
+            kidx, weights, density);
         NEGF_LAUNCH_CHECK(ctx);
         if (hasS && n > 1) {
             density_cols_kernel<<<(n * b + 127) / 128, 128, 0, ctx->stream>>>(n, b, ne, (const cplx*)GL_upper,
-                                                                            (const cplx*)p->S_upper, weights, density);
+                                                                            (const cplx*)p->S_upper, kidx, weights, density);
             NEGF_LAUNCH_CHECK(ctx);
         }
     }
@@ -208,7 +214,7 @@ extern "C" int negf_observables(negf_ctx* ctx, const negf_problem* p,
     if (bond_current && n > 1) {
         if (!GL_upper || !p->H_upper) return NEGF_EINVAL;
         bond_current_kernel<<<dim3(n - 1, ne), 256, 0, ctx->stream>>>(n, b, (const cplx*)p->H_upper,
-                                                                      (const cplx*)p->S_upper, p->energy,
+                                                                      (const cplx*)p->S_upper, kidx, p->energy,
                                                                       (const cplx*)GL_upper, bond_current);
         NEGF_LAUNCH_CHECK(ctx);
     }

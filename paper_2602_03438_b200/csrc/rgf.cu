@@ -17,12 +17,14 @@
 
 using namespace rgfc;
 
+size_t path_workspace_bytes(int n, int b, int ne, bool assembled);   // pipeline_host.cu
+
 extern "C" int negf_workspace_bytes(const negf_problem* p, int kind_max, int flags, size_t* bytes) {
     (void)flags;
     if (!p || !bytes || p->n_blocks < 1 || p->block_size < 1 || p->n_energy < 1) return NEGF_EINVAL;
-    const bool assembled = p->S_diag != nullptr || kind_max == NEGF_SIGMA_BT;
-    Workspace w = carve_workspace(nullptr, p->n_blocks, p->block_size, p->n_energy, assembled);
-    *bytes = w.bytes;
+    const bool assembled = p->S_diag != nullptr || kind_max == NEGF_SIGMA_BT || p->n_k > 1;
+    // covers the four calls on the whole batch AND the per-group slices + partial densities of negf_pipeline_device
+    *bytes = path_workspace_bytes(p->n_blocks, p->block_size, p->n_energy, assembled);
     return NEGF_OK;
 }
 
@@ -37,6 +39,7 @@ int rgf_assemble(negf_ctx* ctx, const negf_problem* p, const negf_sigma* sigma_r
         ca.b = b; ca.energy = p->energy; ca.eta = p->eta; ca.use_z = 1; ca.coef = -1.0;
         ca.H = (const cplx*)p->H_diag; ca.fH = s.sb;
         ca.S = (const cplx*)p->S_diag; ca.fS = s.sb; ca.s_identity = p->S_diag ? 0 : 1;
+        ca.kidx = kidx_of(p); ca.kH = s.sn; ca.kS = s.sn;
         ca.out = W.g; ca.sout = s.sn; ca.fout = s.sb; ca.nfam = n;
         int nb = 0;
         if (sigma_r) {
@@ -55,6 +58,7 @@ int rgf_assemble(negf_ctx* ctx, const negf_problem* p, const negf_sigma* sigma_r
             CombineArgs ca = {};
             ca.b = b; ca.energy = p->energy; ca.eta = p->eta; ca.use_z = 1; ca.coef = -1.0;
             ca.H = (const cplx*)p->H_upper; ca.fH = s.sb; ca.S = (const cplx*)p->S_upper; ca.fS = s.sb; ca.s_identity = 0;
+            ca.kidx = kidx_of(p); ca.kH = s.sm; ca.kS = s.sm;
             ca.dagger = (which == 2);
             ca.out = which == 1 ? W.Aup : W.Alow; ca.sout = s.sm; ca.fout = s.sb; ca.nfam = n - 1;
             if (sigma_r && sigma_r->kind == NEGF_SIGMA_BT) {

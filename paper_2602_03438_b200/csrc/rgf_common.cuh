@@ -24,8 +24,12 @@ inline int check_problem(const negf_ctx* ctx, const negf_problem* p) {
     if (p->n_blocks > 1 && !p->H_upper) return NEGF_EINVAL;
     if (p->n_blocks > 1 && ((p->S_diag == nullptr) != (p->S_upper == nullptr))) return NEGF_EINVAL;
     if (p->n_energy > 65535) return NEGF_EUNSUPPORTED;
+    if (p->n_k > 1 && !p->k_index) return NEGF_EINVAL;
     return NEGF_OK;
 }
+
+// k-point batching (include/negf.h): device index per batch entry, or NULL for a single device
+inline const int* kidx_of(const negf_problem* p) { return p->n_k > 1 ? p->k_index : nullptr; }
 
 inline int check_sigma(const negf_sigma* s, int n, bool retarded) {
     if (!s) return NEGF_OK;
@@ -40,8 +44,10 @@ inline int check_sigma(const negf_sigma* s, int n, bool retarded) {
     return NEGF_EINVAL;
 }
 
+// the off-diagonal blocks of A are materialised per batch entry when they depend on it: S != I, a dense
+// Sigma^R_S, or k-point batching (H_{i,i+1} differs between the entries)
 inline bool needs_assembly(const negf_problem* p, const negf_sigma* sr) {
-    return p->S_diag != nullptr || (sr && sr->kind == NEGF_SIGMA_BT);
+    return p->S_diag != nullptr || (sr && sr->kind == NEGF_SIGMA_BT) || p->n_k > 1;
 }
 
 // A family of blocks as a GEMM operand: block i of energy e at p + e*se + i*si, read as op(.)

@@ -4,25 +4,31 @@
 // SURVEY.md 8(a) S3) and every g = a_b^-1 of the Sancho-Rubio doubling is one
 // call of this file.
 //
-//  * b <= SMALL_MAX: one CTA per matrix, whole matrix in shared memory, in-place Gauss-Jordan
-//    with row pivoting on |re|+|im| (izamax convention), column permutation undone at the end.
-//  * larger b: BLOCKED in-place Gauss-Jordan, panel width w <= 32:
-//      1. the panel (rows >= k0) is LU-factorised with partial pivoting by a thread-block
-//         CLUSTER that holds the tall panel in distributed shared memory (up to 8 CTAs x 200 KB);
-//         every column costs ONE cluster barrier: before it each CTA pushes its best pivot
-//         candidate (value, row index, row content) and CTA 0 the current diagonal row into all
-//         CTAs' buffers through DSMEM, after it everybody knows the pivot and already owns the
-//         two rows to exchange;
-//      2. row swaps are applied to the rest of the matrix, the pivot rows R are moved to scratch
-//         and zeroed;
-//      3. the panel is finalised to P' = [-T Dinv ; Dinv ; -L21 L11^-1] with two small GEMMs;
-//      4. ONE rank-w GEMM per side updates all other columns: M += P' R  (K2 kernel, DMMA).
-//    Cost b^3 complex multiply-adds = 8 b^3 flops = 1 U, same as getrf + getri, but every
-//    trailing update is a full-height uniform GEMM.  Pivoting is partial pivoting among the
-//    not-yet-eliminated rows, exactly as in LU.
+// Three regimes (zinv_launch at the end of the file picks one by block size):
+//  * b <= 16 and 64 < b <= 96 (and every b <= 96 with NEGF_OPT_INV_TENSOR = 0): gj_reg_kernel - unblocked
+//    Gauss-Jordan with the whole matrix in REGISTERS of one CTA of 16 warps, implicit threshold pivoting on a
+//    32-bit key, one block barrier per column, look-ahead of the next column's pivot search;
+//  * 16 < b <= 64: gj_dmma_kernel - blocked Gauss-Jordan in one CTA, panel width 4: one panel warp (alone on
+//    its scheduler partition) factorises panel K+1 while 8 update warps apply panel K to the whole matrix as
+//    a rank-4 update on the FP64 tensor pipe (DMMA.8x8x4), matrix in the accumulator layout + a shared copy;
+//  * b > 96: two-level BLOCKED in-place Gauss-Jordan (outer blocks of 128 columns, panels of 32):
+//      1. the panel is eliminated on ALL rows by gj_panel_rows_kernel (zinv_rows.cu: one matrix row per thread,
+//         cluster of up to 8 CTAs, one block + one cluster barrier per column), which leaves the transform columns
+//         P' = [-T D^-1 ; D^-1 ; -B D^-1] in place; blocks above 2048 rows (or NEGF_OPT_INV_PANEL = 0) use the first
+//         generation instead: LU of the rows at and below the panel by gj_panel_reg_kernel (lane = panel column)
+//         or gj_panel_cluster_kernel (panel in distributed shared memory), then P' from small GEMMs;
+//      2. the panel's row swaps are applied to the other columns of the outer block, the pivot rows R are
+//         moved to scratch and zeroed (gj_swap_extract_kernel);
+//      3. rank-32 update of the other columns of the outer block: M += P' R (K2, DMMA);
+//      4. after the 4 panels of an outer block: all 128 swaps on the columns outside it and ONE rank-128
+//         update M[:, ~K] += Q R, Q = the block's own columns read in place (87 % of the flops at b = 1024);
+//      5. the column permutation of the recorded swaps is undone at the end (gj_colperm_kernel).
+//    Cost b^3 complex multiply-adds = 8 b^3 flops = 1 U, same as getrf + getri.  Pivoting is partial pivoting
+//    among the not-yet-eliminated rows, exactly as in LU.
 #include <cooperative_groups.h>
 
 #include "common.cuh"
+#include "zinv_rows.cuh"
 
 namespace cg = cooperative_groups;
 
@@ -1098,6 +1104,7 @@ struct InvWs {
     cplx* Linv;   // [batch][PW*PW]
     int* ipiv;    // [batch][b]
     int* idx;     // [batch][b]
+    int2* moves;  // [ceil(b / PW)][batch][2 PW]  net row moves of every panel (zinv_rows.cu)
 };
 InvWs carve(void* ws, int b, int batch) {
     InvWs o;
@@ -1108,7 +1115,8 @@ InvWs carve(void* ws, int b, int batch) {
     o.Dinv = (cplx*)p; p += align_up((size_t)batch * PW * PW * sizeof(cplx), 256);
     o.Linv = (cplx*)p; p += align_up((size_t)batch * PW * PW * sizeof(cplx), 256);
     o.ipiv = (int*)p;  p += align_up((size_t)batch * b * sizeof(int), 256);
-    o.idx = (int*)p;
+    o.idx = (int*)p;   p += align_up((size_t)batch * b * sizeof(int), 256);
+    o.moves = (int2*)p;
     return o;
 }
 
@@ -1119,7 +1127,8 @@ size_t zinv_workspace_bytes(int b, int batch) {
     return align_up((size_t)batch * OUTER_NB * b * sizeof(cplx), 256) +
            2 * align_up((size_t)batch * PW * b * sizeof(cplx), 256) +
            2 * align_up((size_t)batch * PW * PW * sizeof(cplx), 256) +
-           2 * align_up((size_t)batch * b * sizeof(int), 256);
+           2 * align_up((size_t)batch * b * sizeof(int), 256) +
+           align_up((size_t)((b + PW - 1) / PW) * batch * 2 * PW * sizeof(int2), 256);
 }
 
 // shared-memory opt-ins of the blocked path, once per context (= per device) at negf_create
@@ -1184,6 +1193,28 @@ int zinv_launch(negf_ctx* ctx, int b, cplx* A, long long sA, int batch, void* ws
         at[0].id = cudaLaunchAttributeClusterDimension;
         at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
         cfg.attrs = at; cfg.numAttrs = 1; cfg.stream = ctx->stream;
+        if (gj_panel_rows_supported(b) && ctx->inv_panel) {
+            // Gauss-Jordan of the panel on ALL rows, one row per thread (zinv_rows.cu): leaves the complete transform
+            // columns [-T D^-1 ; D^-1 ; -B D^-1] in place and LAPACK-style pivots in ipiv
+            const long long mstride = (long long)batch * 2 * PW;
+            int2* mv = W.moves + (size_t)(k0 / PW) * mstride;
+            RowsArgs ra{A, sA, b, k0, wk, W.ipiv, info, info_code, skip, mv};
+            NEGF_TRY(gj_panel_rows_launch(ctx, ra, batch));
+            if (nbk > wk)      // the panel's exchanges on the other columns of K; pivot rows -> R, zeroed
+                NEGF_TRY(gj_moves_extract_launch(ctx, A, sA, b, batch, mv, mstride, 1, k0, wk, K0, K1, k0, k0 + wk, W.R, skip));
+            // M[:, other columns of K] += P' R, P' read from the panel's own columns
+            g.alpha = one; g.beta = one; g.m = b; g.k = wk; g.A = A + k0; g.lda = b; g.sA = sA;
+            g.ldb = b; g.sB = (long long)wk * b; g.ldc = b; g.sC = sA; g.sD = sA;
+            if (k0 > K0) {
+                g.n = k0 - K0; g.B = W.R + K0; g.C = A + K0; g.D = A + K0;
+                NEGF_TRY(zgemm_launch(ctx, g));
+            }
+            if (k0 + wk < K1) {
+                g.n = K1 - k0 - wk; g.B = W.R + k0 + wk; g.C = A + k0 + wk; g.D = A + k0 + wk;
+                NEGF_TRY(zgemm_launch(ctx, g));
+            }
+            continue;
+        }
         if (reg_panel) {
             // one row per thread in registers; finishes P' (diagonal block and below) in place
             // rows per warp (16 warps per CTA): up to 256 rows stay in ONE CTA (no cluster barrier)
@@ -1272,9 +1303,15 @@ int zinv_launch(negf_ctx* ctx, int b, cplx* A, long long sA, int batch, void* ws
       }
       if (nbk == b) break;       // a single outer block: nothing outside it
       // all nbk swaps of this outer block on the columns outside K; pivot rows -> Rout, zeroed in A
-      gj_swap_extract_kernel<<<dim3((b + 127) / 128, batch), 128, 0, ctx->stream>>>(
-          A, sA, b, K0, nbk, 0, b, K0, K1, W.ipiv, W.Rout, skip);
-      NEGF_LAUNCH_CHECK(ctx);
+      if (gj_panel_rows_supported(b) && ctx->inv_panel) {
+          const long long mstride = (long long)batch * 2 * PW;
+          NEGF_TRY(gj_moves_extract_launch(ctx, A, sA, b, batch, W.moves + (size_t)(K0 / PW) * mstride, mstride,
+                                           (nbk + PW - 1) / PW, K0, nbk, 0, b, K0, K1, W.Rout, skip));
+      } else {
+          gj_swap_extract_kernel<<<dim3((b + 127) / 128, batch), 128, 0, ctx->stream>>>(
+              A, sA, b, K0, nbk, 0, b, K0, K1, W.ipiv, W.Rout, skip);
+          NEGF_LAUNCH_CHECK(ctx);
+      }
       // M[:, ~K] += Q R with Q = M[:, K] in place
       GemmArgs g;
       g.opA = 0; g.opB = 0; g.alpha = one; g.beta = one; g.batch = batch; g.skip = skip;

@@ -26,6 +26,8 @@ KEEP_SWEEP = 1
 OPT_GRAPH_LOOPS = 1
 OPT_GEMM_3M = 2
 OPT_INV_TENSOR = 3
+OPT_ENERGY_GROUPS = 4
+OPT_INV_PANEL = 5
 
 
 class c128(C.Structure):
@@ -35,7 +37,8 @@ class c128(C.Structure):
 class Problem(C.Structure):
     _fields_ = [("n_blocks", C.c_int), ("block_size", C.c_int), ("n_energy", C.c_int),
                 ("H_diag", C.c_void_p), ("H_upper", C.c_void_p), ("S_diag", C.c_void_p),
-                ("S_upper", C.c_void_p), ("energy", C.c_void_p), ("eta", C.c_double)]
+                ("S_upper", C.c_void_p), ("energy", C.c_void_p), ("eta", C.c_double),
+                ("n_k", C.c_int), ("k_index", C.c_void_p)]
 
 
 class Sigma(C.Structure):
@@ -58,10 +61,17 @@ class HostOutputs(C.Structure):
                  "density", "ldos", "transmission", "bond_current", "contact_current", "info")]
 
 
+class DeviceOutputs(C.Structure):
+    _fields_ = [("left", ObcOut), ("right", ObcOut)] + [(k, C.c_void_p) for k in
+                ("GR_diag", "GR_upper", "GR_lower", "GR_corner", "GL_diag", "GL_upper", "GG_diag", "GG_upper",
+                 "density", "ldos", "transmission", "bond_current", "contact_current", "info_r", "info_x")]
+
+
 EXPORTS = ["negf_create", "negf_destroy", "negf_set_stream", "negf_workspace_bytes", "negf_set_workspace",
            "negf_set_option", "negf_strerror", "negf_last_cuda_error", "negf_launch_count",
            "negf_profile_enable", "negf_profile_read", "negf_obc_decimate", "negf_obc_decimate_pair",
-           "negf_rgf_retarded", "negf_rgf_lesser_greater", "negf_observables", "negf_energy_convolve", "negf_pipeline_host_bytes",
+           "negf_rgf_retarded", "negf_rgf_lesser_greater", "negf_observables", "negf_energy_convolve", "negf_pipeline_device",
+           "negf_pipeline_host_bytes",
            "negf_pipeline_host", "negf_zgemm_batched", "negf_zinverse_batched", "negf_fp64_peak"]
 
 _P = C.c_void_p
@@ -89,6 +99,8 @@ lib.negf_rgf_lesser_greater.argtypes = [_P, C.POINTER(Problem), C.POINTER(Sigma)
 lib.negf_observables.argtypes = [_P, C.POINTER(Problem)] + [_P] * 19
 lib.negf_energy_convolve.argtypes = [_P, C.c_int, C.c_longlong, C.c_int, _P, _P, C.c_int, C.c_int, c128, _P]
 lib.negf_pipeline_host_bytes.argtypes = [C.POINTER(Problem), C.c_int, C.c_int, C.POINTER(C.c_size_t)]
+lib.negf_pipeline_device.argtypes = [_P, C.POINTER(Problem), C.POINTER(Sigma), C.POINTER(Sigma), C.POINTER(Sigma), _P,
+                                     C.c_double, C.c_double, C.c_double, C.c_double, C.c_int, C.POINTER(DeviceOutputs)]
 lib.negf_pipeline_host.argtypes = [_P, C.POINTER(Problem), C.POINTER(Sigma), C.POINTER(Sigma), C.POINTER(Sigma),
                                    _P, C.c_double, C.c_double, C.c_double, C.c_double, C.c_int, _P, C.c_size_t,
                                    C.POINTER(HostOutputs), C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)]
@@ -122,9 +134,11 @@ def _ptr(t) -> Optional[int]:
     return int(t)
 
 
-def make_problem(n_blocks, block_size, n_energy, H_diag, H_upper, S_diag, S_upper, energy, eta) -> Problem:
+def make_problem(n_blocks, block_size, n_energy, H_diag, H_upper, S_diag, S_upper, energy, eta,
+                 n_k: int = 1, k_index=None) -> Problem:
+    """n_k > 1: H / S arrays are [n_k][...] and k_index [n_energy] (int32) names the device of every batch entry."""
     return Problem(n_blocks, block_size, n_energy, _ptr(H_diag), _ptr(H_upper), _ptr(S_diag), _ptr(S_upper),
-                   _ptr(energy), float(eta))
+                   _ptr(energy), float(eta), int(n_k), _ptr(k_index))
 
 
 def make_sigma(kind=SIGMA_NONE, scalar=None, diag=None, upper=None, lower=None, left=None, right=None) -> Sigma:
@@ -234,6 +248,13 @@ class Context:
         sc = complex(scale)
         self._check(lib.negf_energy_convolve(self._h, n_energy, elems_per_energy, transpose_block, _ptr(X1), _ptr(X2),
                                              mode, int(conj2), c128(sc.real, sc.imag), _ptr(Y)), "negf_energy_convolve")
+
+    def pipeline_device(self, p: Problem, sigma_r, sigma_lesser, sigma_greater, weights, mu_L, mu_R, kT, tol, max_iter,
+                        outputs: DeviceOutputs):
+        ref = lambda s: C.byref(s) if s is not None else None
+        self._check(lib.negf_pipeline_device(self._h, C.byref(p), ref(sigma_r), ref(sigma_lesser), ref(sigma_greater),
+                                             _ptr(weights), mu_L, mu_R, kT, tol, max_iter, C.byref(outputs)),
+                    "negf_pipeline_device")
 
     @staticmethod
     def pipeline_host_bytes(p: Problem, kind_max: int, want_greater: bool) -> int:

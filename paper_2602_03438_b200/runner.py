@@ -25,22 +25,39 @@ class DevicePath:
 
     def __init__(self, wl: Workload, e_lo: int = 0, e_hi: Optional[int] = None, device: str = "cuda:0",
                  ctx: Optional[negf.Context] = None, want_greater: Optional[bool] = None,
-                 sigma: Optional[dict] = None, alloc_outputs: bool = True):
+                 sigma: Optional[dict] = None, alloc_outputs: bool = True, kpoints=None, k_weights=None):
+        """kpoints: optional list of Workloads (one per momentum, same shape and energy grid as `wl`, e.g. from
+        workloads.make_kpoint_workloads): the batch then holds every (k, E) pair in k-major order, entry
+        j * N_E + e, as ONE lock-step batch (negf_problem.n_k / k_index); the quadrature weights become w_k w_E."""
         self.wl = wl
         self.device = torch.device(device)
         self.e_lo, self.e_hi = e_lo, wl.n_energy if e_hi is None else e_hi
-        self.ne = self.e_hi - self.e_lo
+        ne1 = self.e_hi - self.e_lo
+        self.n_k = 1 if kpoints is None else len(kpoints)
+        self.ne = ne1 * self.n_k
         self.n, self.b = wl.n_blocks, wl.block_size
         self.want_greater = wl.want_greater if want_greater is None else want_greater
         self.ctx = ctx or negf.Context(self.device.index or 0)
         d = self.device
-        self.H_diag, self.H_upper = _dev(wl.H_diag, d), _dev(wl.H_upper, d)
-        self.S_diag, self.S_upper = _dev(wl.S_diag, d), _dev(wl.S_upper, d)
-        self.energy = _dev(wl.energies[self.e_lo:self.e_hi].astype(np.float64), d)
-        self.weights = _dev(wl.weights[self.e_lo:self.e_hi].astype(np.float64), d)
+        devs = [wl] if kpoints is None else list(kpoints)
+        stack = lambda name: (None if getattr(devs[0], name) is None else
+                              np.concatenate([getattr(w, name) for w in devs]) if kpoints is not None else getattr(wl, name))
+        self.H_diag, self.H_upper = _dev(stack("H_diag"), d), _dev(stack("H_upper"), d)
+        self.S_diag, self.S_upper = _dev(stack("S_diag"), d), _dev(stack("S_upper"), d)
+        kw = np.ones(self.n_k) if k_weights is None else np.asarray(k_weights, dtype=np.float64)
+        self.energy = _dev(np.tile(wl.energies[self.e_lo:self.e_hi].astype(np.float64), self.n_k), d)
+        self.weights = _dev(np.concatenate([kw[j] * wl.weights[self.e_lo:self.e_hi].astype(np.float64)
+                                            for j in range(self.n_k)]), d)
+        self.k_index = None if kpoints is None else _dev(np.repeat(np.arange(self.n_k, dtype=np.int32), ne1), d)
         self.problem = negf.make_problem(self.n, self.b, self.ne, self.H_diag, self.H_upper, self.S_diag,
-                                         self.S_upper, self.energy, wl.eta)
-        sig = wl.sigma_s(self.e_lo, self.e_hi) if sigma is None else sigma
+                                         self.S_upper, self.energy, wl.eta, self.n_k, self.k_index)
+        if sigma is None:
+            per_k = [w.sigma_s(self.e_lo, self.e_hi) for w in devs]
+            sig = {t: (None if per_k[0][t] is None else
+                       {kk: (vv if kk == "kind" else np.concatenate([p[t][kk] for p in per_k]))
+                        for kk, vv in per_k[0][t].items()}) for t in "rlg"}
+        else:
+            sig = sigma
         self.sig_dev: Dict[str, Optional[dict]] = {}
         for t in "rlg":
             s = sig[t]
@@ -135,12 +152,31 @@ class DevicePath:
                              self.weights, o["density"], o["ldos"], o["transmission"],
                              o["bond_current"] if self.n > 1 else None, o["contact_current"] if g else None)
 
-    def run(self):
-        """One pass of the whole hot path (S1-S7) over this energy batch."""
+    def run_four_calls(self):
+        """One pass of the whole hot path (S1-S7) as the four C-ABI calls, one after the other on this context."""
         self.obc()
         self.retarded()
         self.lesser_greater()
         self.observables()
+
+    def run(self):
+        """One pass of the whole hot path (S1-S7) over this energy batch through negf_pipeline_device: the same
+        four steps, scheduled by the library (concurrent energy groups in the small-block regime)."""
+        o, wl, g = self.out, self.wl, self.want_greater
+        if not hasattr(self, "_dev_out"):
+            obc = lambda t: negf.ObcOut(*[negf._ptr(o[f"{k}_{t}"]) for k in
+                                          ("sigma_r", "gamma", "sigma_l", "sigma_g", "g_s", "fermi", "iters", "status")])
+            m = self.n > 1
+            self._dev_out = negf.DeviceOutputs(
+                obc("L"), obc("R"), negf._ptr(o["GR_diag"]), negf._ptr(o["GR_upper"] if m else None),
+                negf._ptr(o["GR_lower"] if m else None), negf._ptr(o["GR_corner"]), negf._ptr(o["GL_diag"]),
+                negf._ptr(o["GL_upper"] if m else None), negf._ptr(o.get("GG_diag")),
+                negf._ptr(o.get("GG_upper") if m else None), negf._ptr(o["density"]), negf._ptr(o["ldos"]),
+                negf._ptr(o["transmission"]), negf._ptr(o["bond_current"] if m else None),
+                negf._ptr(o["contact_current"] if g else None), negf._ptr(o["info_r"]), negf._ptr(o["info_x"]))
+        self._sr = self._sigma("r", o["sigma_r_L"], o["sigma_r_R"])
+        self.ctx.pipeline_device(self.problem, self._sigma("r"), self._sigma("l"), self._sigma("g") if g else None,
+                                 self.weights, wl.mu_L, wl.mu_R, wl.kT, wl.tol, wl.max_iter, self._dev_out)
 
     def host(self, name: str) -> np.ndarray:
         return self.out[name].cpu().numpy()
@@ -151,21 +187,34 @@ class HostPath:
     inside the call (what bench.py times as the end-to-end number)."""
 
     def __init__(self, wl: Workload, n_energy: Optional[int] = None, device: str = "cuda:0",
-                 ctx: Optional[negf.Context] = None, want_greater: Optional[bool] = None, blocks: bool = True):
-        """blocks=False: the G block outputs are NULL (only the observables come back to the host)."""
+                 ctx: Optional[negf.Context] = None, want_greater: Optional[bool] = None, blocks: bool = True,
+                 kpoints=None, k_weights=None):
+        """blocks=False: the G block outputs are NULL (only the observables come back to the host).
+        kpoints / k_weights: as for DevicePath (every (k, E) pair in k-major order as one batch)."""
         self.wl = wl
         self.device = torch.device(device)
-        self.ne = wl.n_energy if n_energy is None else min(n_energy, wl.n_energy)
+        ne1 = wl.n_energy if n_energy is None else min(n_energy, wl.n_energy)
+        self.n_k = 1 if kpoints is None else len(kpoints)
+        self.ne = ne1 * self.n_k
         self.n, self.b = wl.n_blocks, wl.block_size
         self.want_greater = wl.want_greater if want_greater is None else want_greater
         self.ctx = ctx or negf.Context(self.device.index or 0)
         ne, n, b = self.ne, self.n, self.b
         pin = lambda a: None if a is None else torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
-        self._keep = [pin(wl.H_diag), pin(wl.H_upper), pin(wl.S_diag), pin(wl.S_upper),
-                      pin(wl.energies[:ne].astype(np.float64)), pin(wl.weights[:ne].astype(np.float64))]
+        devs = [wl] if kpoints is None else list(kpoints)
+        stack = lambda name: (None if getattr(devs[0], name) is None else np.concatenate([getattr(w, name) for w in devs]))
+        kw = np.ones(self.n_k) if k_weights is None else np.asarray(k_weights, dtype=np.float64)
+        self._keep = [pin(stack("H_diag")), pin(stack("H_upper")), pin(stack("S_diag")), pin(stack("S_upper")),
+                      pin(np.tile(wl.energies[:ne1].astype(np.float64), self.n_k)),
+                      pin(np.concatenate([kw[j] * wl.weights[:ne1].astype(np.float64) for j in range(self.n_k)]))]
         Hd, Hu, Sd, Su, en, self.weights = self._keep
-        self.problem = negf.make_problem(n, b, ne, Hd, Hu, Sd, Su, en, wl.eta)
-        sig = wl.sigma_s(0, ne)
+        kidx = None if kpoints is None else np.repeat(np.arange(self.n_k, dtype=np.int32), ne1)
+        self._keep.append(kidx)
+        self.problem = negf.make_problem(n, b, ne, Hd, Hu, Sd, Su, en, wl.eta, self.n_k, kidx)
+        per_k = [w.sigma_s(0, ne1) for w in devs]
+        sig = {t: (None if per_k[0][t] is None else
+                   {kk: (vv if kk == "kind" else np.concatenate([p[t][kk] for p in per_k]))
+                    for kk, vv in per_k[0][t].items()}) for t in "rlg"}
         self.sig = {}
         for t in "rlg":
             s = sig[t]

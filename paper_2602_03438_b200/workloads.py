@@ -27,7 +27,7 @@ import numpy as np
 BASE_SEED = 26020343800
 
 # family ids for the child streams
-_F_HDIAG, _F_HUP, _F_SDIAG, _F_SUP, _F_OFFS, _F_SIG_L, _F_SIG_G, _F_SIG_P = range(8)
+_F_HDIAG, _F_HUP, _F_SDIAG, _F_SUP, _F_OFFS, _F_SIG_L, _F_SIG_G, _F_SIG_P, _F_KPT = range(9)
 
 
 def _rng(config: int, family: int, sub: int = 0) -> np.random.Generator:
@@ -290,6 +290,42 @@ def make_coulomb_workload(n_blocks: int, block_size: int, n_omega: int, seed: in
         sig["r"]["upper"][k] = pu - 0.5j * (gu + lu)
         sig["r"]["lower"][k] = h(pu) - 0.5j * (h(gu) + h(lu))
     return wl, sig
+
+
+def make_kpoint_workloads(config: int, n_k: int, transverse: float = 0.3, **size_overrides):
+    """Momentum-resolved inputs ("the momentum dependence is omitted for simplicity"; SURVEY.md 8(f)
+    item 2): the device of `make_workload(config, ...)` made periodic in one transverse direction with coupling
+    blocks V to the neighbouring transverse cell, Bloch-summed at n_k momenta k_j = -pi + 2 pi (j + 1/2) / n_k:
+        H_ii(k)     = H_ii     + e^{ik} V_ii + e^{-ik} V_ii^H              (Hermitian for every k)
+        H_{i,i+1}(k) = H_{i,i+1} + e^{ik} V+_i + e^{-ik} V-_i,   H_{i+1,i}(k) = H_{i,i+1}(k)^H
+    with V_ii ~ CN(0, 1)/sqrt(b), V+-_i ~ CN(0, 0.5)/sqrt(b), all scaled by `transverse`; for non-orthogonal configs
+    S(k) gets the same construction at a tenth of the overlap's own scale.  Returns (list of n_k Workloads that
+    share the energy grid, k values, k weights 1/n_k).  Inputs only."""
+    base = make_workload(config, **size_overrides)
+    n, b = base.n_blocks, base.block_size
+    rng = _rng(config, _F_KPT)
+    Vd = transverse * complex_normal(rng, (n, b, b), 1.0) / np.sqrt(b)
+    Vp = transverse * complex_normal(rng, (max(n - 1, 0), b, b), 0.5) / np.sqrt(b)
+    Vm = transverse * complex_normal(rng, (max(n - 1, 0), b, b), 0.5) / np.sqrt(b)
+    if base.S_diag is not None:
+        Td = 0.005 * complex_normal(rng, (n, b, b), 1.0) / np.sqrt(b)
+        Tp = 0.002 * complex_normal(rng, (max(n - 1, 0), b, b), 1.0) / np.sqrt(b)
+        Tm = 0.002 * complex_normal(rng, (max(n - 1, 0), b, b), 1.0) / np.sqrt(b)
+    h = lambda a: np.conj(np.swapaxes(a, -1, -2))
+    ks = -np.pi + 2.0 * np.pi * (np.arange(n_k) + 0.5) / n_k
+    out = []
+    import copy
+    for j, k in enumerate(ks):
+        ph = np.exp(1j * k)
+        wl = copy.copy(base)
+        wl.name = f"{base.name}[k{j}/{n_k}]"
+        wl.H_diag = np.ascontiguousarray(base.H_diag + ph * Vd + np.conj(ph) * h(Vd))
+        wl.H_upper = np.ascontiguousarray(base.H_upper + ph * Vp + np.conj(ph) * Vm)
+        if base.S_diag is not None:
+            wl.S_diag = np.ascontiguousarray(base.S_diag + ph * Td + np.conj(ph) * h(Td))
+            wl.S_upper = np.ascontiguousarray(base.S_upper + ph * Tp + np.conj(ph) * Tm)
+        out.append(wl)
+    return out, ks, np.full(n_k, 1.0 / n_k)
 
 
 def shard_energies(wl: Workload, rank: int, world: int) -> Workload:
