@@ -136,12 +136,28 @@ int negf_set_workspace(negf_ctx* ctx, void* dev_ptr, size_t bytes);
  * NEGF_OPT_INV_PANEL (default 1): panels of the blocked inverse (97 <= b <= 2048) are eliminated by the
  * row-per-thread Gauss-Jordan kernel (all rows of the matrix, partial pivoting on the leading 32 bits of
  * |re|+|im|); 0 = the first panel kernel (LU of the rows at and below the panel, lane = panel column), which
- * larger blocks always use.  Same pivoting rule up to the key width, same results up to rounding. */
+ * larger blocks always use.  Same pivoting rule up to the key width, same results up to rounding.
+ * NEGF_OPT_INV_LOOKAHEAD (default 1): the blocked inverse of blocks above 256 applies the rank-128 update of an
+ * outer block to the columns of the NEXT outer block first and to all other columns on a side stream of the
+ * context, while the caller's stream already eliminates the next block's panels; joined before the call
+ * returns.  0 = everything in order on the caller's stream.  Bit-identical results.
+ * NEGF_OPT_INV_OUTER (default 0 = automatic: 128 columns up to b = 1024, 256 above): width of the outer block of
+ * the blocked inverse, i.e. the k of its big trailing updates (a multiple of 32, at most 256).
+ * NEGF_OPT_FUSED_SMALL (default 1 = automatic: when N_E <= number of SMs; 2 = always; 0 = never): for block sizes
+ * up to 32 the whole chain of one energy runs in ONE thread block
+ * with every operand in shared memory: negf_obc_decimate[_pair] is one launch (one CTA per lead and energy walks the
+ * complete doubling loop), negf_rgf_retarded one launch (one CTA per energy, forward and backward sweep),
+ * negf_rgf_lesser_greater one launch (one CTA per energy and < / >).  0 = the batched lock-step launches used for
+ * larger blocks.  Same definitions, results equal to rounding.  Set it before negf_rgf_retarded: the retained
+ * sweep state of one regime is not valid for the other. */
 #define NEGF_OPT_GRAPH_LOOPS   1
 #define NEGF_OPT_GEMM_3M       2
 #define NEGF_OPT_INV_TENSOR    3
 #define NEGF_OPT_ENERGY_GROUPS 4
 #define NEGF_OPT_INV_PANEL     5
+#define NEGF_OPT_INV_LOOKAHEAD 6
+#define NEGF_OPT_INV_OUTER     7
+#define NEGF_OPT_FUSED_SMALL   8
 #define NEGF_MAX_ENERGY_GROUPS 4
 int negf_set_option(negf_ctx* ctx, int option, int value);
 const char* negf_strerror(int code);

@@ -41,6 +41,8 @@ def main():
     ap.add_argument("--reps", type=int, default=10)
     ap.add_argument("--sets", type=int, default=2, help="operand sets rotated between launches")
     ap.add_argument("--inv-panel", type=int, default=1, help="NEGF_OPT_INV_PANEL (1 = row-per-thread Gauss-Jordan panel, 0 = first LU panel kernel)")
+    ap.add_argument("--inv-lookahead", type=int, default=1, help="NEGF_OPT_INV_LOOKAHEAD")
+    ap.add_argument("--inv-outer", type=int, default=0, help="NEGF_OPT_INV_OUTER (0 = automatic)")
     ap.add_argument("--gemm-3m", action="store_true", help="NEGF_OPT_GEMM_3M (tflops still counted as 8 b^3 per product)")
     args = ap.parse_args()
     ctx = negf.Context(0)
@@ -49,6 +51,8 @@ def main():
     if args.gemm_3m:
         ctx.set_option(negf.OPT_GEMM_3M, 1)
     ctx.set_option(negf.OPT_INV_PANEL, args.inv_panel)
+    ctx.set_option(negf.OPT_INV_LOOKAHEAD, args.inv_lookahead)
+    ctx.set_option(negf.OPT_INV_OUTER, args.inv_outer)
     peak = ctx.fp64_peak(200.0)
     if args.kernel == "peak":
         print(json.dumps({"kernel": "dmma_peak_probe", "tflops": peak}))

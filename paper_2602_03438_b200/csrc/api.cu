@@ -19,7 +19,7 @@ extern "C" int negf_create(negf_ctx** out, int device) {
     if (!c) return NEGF_EINVAL;
     c->device = device; c->stream = nullptr; c->ws = nullptr; c->ws_bytes = 0; c->last_cuda_error = 0;
     c->launches = 0; c->num_sms = prop.multiProcessorCount; c->sweep_valid = false;
-    c->sw_n = c->sw_b = c->sw_ne = 0; c->sw_assembled = false;
+    c->sw_n = c->sw_b = c->sw_ne = 0; c->sw_assembled = false; c->sw_fused = false; c->fused_small = 1;
     for (int k = 0; k < NEGF_NSIDE; k++) {
         if (cudaStreamCreateWithFlags(&c->side[k], cudaStreamNonBlocking) != cudaSuccess ||
             cudaEventCreateWithFlags(&c->ev_fork[k], cudaEventDisableTiming) != cudaSuccess ||
@@ -32,11 +32,18 @@ extern "C" int negf_create(negf_ctx** out, int device) {
     if (cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) != cudaSuccess) { delete c; return NEGF_ECUDA; }
     for (int k = 0; k < 4; k++) if (cudaEventCreateWithFlags(&c->ev_grp[k], cudaEventDisableTiming) != cudaSuccess) { delete c; return NEGF_ECUDA; }
     if (cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking) != cudaSuccess) { delete c; return NEGF_ECUDA; } c->obc_key_ws = nullptr; c->obc_key_b = c->obc_key_n = c->obc_key_ne = c->obc_key_ns = c->obc_key_maxit = 0; c->obc_key_tol = 0.0;
+    c->inv_lookahead = 1; c->inv_outer = 0; c->inv_side = nullptr; c->ev_inv_main = c->ev_inv_side = nullptr;
+    // lowest priority: when both have CTAs pending, the caller's stream (the latency-bound panels) goes first
+    int prio_lo = 0, prio_hi = 0;
+    cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi);
+    if (cudaStreamCreateWithPriority(&c->inv_side, cudaStreamNonBlocking, prio_lo) != cudaSuccess ||
+        cudaEventCreateWithFlags(&c->ev_inv_main, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&c->ev_inv_side, cudaEventDisableTiming) != cudaSuccess) { delete c; return NEGF_ECUDA; }
     c->energy_groups = 0; c->ev_grp_fork = nullptr;
     for (int k = 0; k < NEGF_MAX_ENERGY_GROUPS; k++) { c->child[k] = nullptr; c->grp_stream[k] = nullptr; c->ev_grp_mid[k] = nullptr; }
     c->prof_on = false; c->prof_depth = 0; c->prof_last_class = -1; c->prof_last_event = nullptr;
     for (int k = 0; k < NEGF_PROF_CLASSES; k++) { c->prof_ms[k] = 0.0; c->prof_n[k] = 0; }
-    if (zgemm_prepare(c) != NEGF_OK || zinv_prepare(c) != NEGF_OK || econv_prepare(c) != NEGF_OK) { delete c; return NEGF_ECUDA; }
+    if (zgemm_prepare(c) != NEGF_OK || zinv_prepare(c) != NEGF_OK || econv_prepare(c) != NEGF_OK || fused_prepare(c) != NEGF_OK) { delete c; return NEGF_ECUDA; }
     *out = c;
     return NEGF_OK;
 }
@@ -57,6 +64,9 @@ extern "C" int negf_destroy(negf_ctx* ctx) {
         if (ctx->ev_grp_mid[k]) cudaEventDestroy(ctx->ev_grp_mid[k]);
     }
     if (ctx->ev_grp_fork) cudaEventDestroy(ctx->ev_grp_fork);
+    if (ctx->inv_side) cudaStreamDestroy(ctx->inv_side);
+    if (ctx->ev_inv_main) cudaEventDestroy(ctx->ev_inv_main);
+    if (ctx->ev_inv_side) cudaEventDestroy(ctx->ev_inv_side);
     delete ctx;
     return NEGF_OK;
 }
@@ -85,6 +95,9 @@ extern "C" int negf_set_option(negf_ctx* ctx, int option, int value) {
     if (option == NEGF_OPT_GEMM_3M) { ctx->gemm_3m = value != 0; return NEGF_OK; }
     if (option == NEGF_OPT_INV_TENSOR) { ctx->inv_tensor = value; return NEGF_OK; }
     if (option == NEGF_OPT_INV_PANEL) { ctx->inv_panel = value; return NEGF_OK; }
+    if (option == NEGF_OPT_INV_LOOKAHEAD) { ctx->inv_lookahead = value; return NEGF_OK; }
+    if (option == NEGF_OPT_INV_OUTER) { ctx->inv_outer = value; return NEGF_OK; }
+    if (option == NEGF_OPT_FUSED_SMALL) { ctx->fused_small = value; ctx->sweep_valid = false; return NEGF_OK; }
     if (option == NEGF_OPT_ENERGY_GROUPS) {
         if (value < 0 || value > NEGF_MAX_ENERGY_GROUPS) return NEGF_EINVAL;
         ctx->energy_groups = value; return NEGF_OK;

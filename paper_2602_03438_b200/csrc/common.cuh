@@ -29,11 +29,17 @@ struct negf_ctx {
     bool sweep_valid;
     int sw_n, sw_b, sw_ne;
     bool sw_assembled;
+    bool sw_fused;                // the retained state is the one-sided state of the resident small-block kernel
+    int fused_small;              // negf_set_option(NEGF_OPT_FUSED_SMALL)
     // cached device-driven WHILE graph of the Sancho-Rubio doublings (small blocks, obc.cu)
     bool graph_loops;             // negf_set_option(NEGF_OPT_GRAPH_LOOPS)
     bool gemm_3m;                 // negf_set_option(NEGF_OPT_GEMM_3M)
     int inv_tensor;               // negf_set_option(NEGF_OPT_INV_TENSOR)
     int inv_panel;                // negf_set_option(NEGF_OPT_INV_PANEL)
+    int inv_lookahead;            // negf_set_option(NEGF_OPT_INV_LOOKAHEAD)
+    int inv_outer;                // negf_set_option(NEGF_OPT_INV_OUTER); 0 = automatic
+    cudaStream_t inv_side;        // side stream of the blocked inverse's look-ahead (zinv.cu)
+    cudaEvent_t ev_inv_main, ev_inv_side;
     // cached CUDA graphs of whole calls in the latency-bound regime (same arguments twice in a row
     // -> the second call is captured, later ones replay it); one slot per entry point
     struct GraphSlot { unsigned long long key; cudaGraphExec_t exec; long long launches; unsigned used; };
@@ -247,6 +253,7 @@ int zgemm_launch(negf_ctx* ctx, const GemmArgs& a);
 int zgemm_prepare(negf_ctx* ctx);
 int zinv_prepare(negf_ctx* ctx);      // shared-memory opt-ins of the K1 kernels (zinv.cu)
 int econv_prepare(negf_ctx* ctx);     // same for the energy-convolution kernels (econv.cu)
+int fused_prepare(negf_ctx* ctx);     // same for the resident small-block kernels (fused_small.cu)
 // several independent products of identical shape / ops / batch in ONE launch (blockIdx.z = member)
 constexpr int NEGF_GEMM_GROUP_MAX = 4;
 struct GemmGroup { GemmArgs g[NEGF_GEMM_GROUP_MAX]; int ng; };

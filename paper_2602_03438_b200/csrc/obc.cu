@@ -12,6 +12,7 @@
 #include "common.cuh"
 #include "kernels.cuh"
 #include "workspace.cuh"
+#include "fused_small.cuh"
 
 namespace {
 
@@ -44,6 +45,19 @@ int obc_core(negf_ctx* ctx, const negf_problem* p, int ns, const LeadBlocks* lb,
     const int n = p->n_blocks, b = p->block_size, ne = p->n_energy, nb = ns * ne;
     const size_t bb = (size_t)b * b;
     const long long sb = (long long)bb;
+    if (fused_small_regime(ctx, b, ne)) {
+        // resident small-block regime: one CTA per (lead, energy) walks the whole doubling loop (fused_small.cu)
+        FusedObcArgs fa = {};
+        fa.b = b; fa.ne = ne; fa.ns = ns; fa.energy = p->energy; fa.eta = p->eta;
+        fa.kidx = p->n_k > 1 ? p->k_index : nullptr; fa.kT = kT; fa.tol = tol; fa.max_iter = max_iter;
+        for (int s = 0; s < ns; s++) {
+            const negf_obc_out* o = outs[s];
+            fa.lead[s] = FusedLead{lb[s].Hd, lb[s].Hu, lb[s].Sd, lb[s].Su, lb[s].kd, lb[s].ku, sides[s], mus[s],
+                                   (cplx*)o->sigma_r, (cplx*)o->gamma, (cplx*)o->sigma_lesser, (cplx*)o->sigma_greater,
+                                   (cplx*)o->g_surface, o->fermi, o->iters, o->status};
+        }
+        return fused_obc_launch(ctx, fa);
+    }
     Workspace W = carve_workspace(ctx->ws, n, b, ne);
     if (W.bytes > ctx->ws_bytes) return NEGF_ENOWORKSPACE;
     cplx *a_s = W.T[0], *a_b = W.T[1], *U0 = W.T[2], *L0 = W.T[3];
@@ -177,7 +191,7 @@ int check_common(const negf_ctx* ctx, const negf_problem* p, int max_iter) {
     if (p->n_blocks < 1 || p->block_size < 1 || p->n_energy < 1 || max_iter < 1 || !p->energy) return NEGF_EINVAL;
     if ((p->S_diag == nullptr) != (p->S_upper == nullptr) && p->n_blocks > 1) return NEGF_EINVAL;
     if (p->n_k > 1 && !p->k_index) return NEGF_EINVAL;
-    if (!ctx->ws) return NEGF_ENOWORKSPACE;
+    if (!ctx->ws && !fused_small_regime(ctx, p->block_size, p->n_energy)) return NEGF_ENOWORKSPACE;
     return NEGF_OK;
 }
 

@@ -10,6 +10,7 @@
 // partial densities in a fixed order.
 #include "common.cuh"
 #include "workspace.cuh"
+#include "fused_small.cuh"
 
 size_t path_workspace_bytes(int n, int b, int ne, bool assembled);
 
@@ -29,6 +30,7 @@ inline void group_range(int ne, int G, int g, int* lo, int* cnt) {
 int path_groups(const negf_ctx* ctx, int b, int ne) {
     if (ctx->prof_on) return 1;                     // per-class intervals must not overlap
     int G = ctx->energy_groups;
+    if (G == 0 && fused_small_regime(ctx, b, ne)) return 1;       // resident regime: one launch per call covers every energy
     if (G == 0) G = (b <= 96 && ne >= 32) ? NEGF_MAX_ENERGY_GROUPS : 1;
     return max(1, min(min(G, NEGF_MAX_ENERGY_GROUPS), ne));
 }
@@ -66,7 +68,7 @@ int ensure_children(negf_ctx* ctx, int G) {
         }
         negf_ctx* c = ctx->child[g];
         c->stream = ctx->grp_stream[g];
-        c->graph_loops = ctx->graph_loops; c->gemm_3m = ctx->gemm_3m; c->inv_tensor = ctx->inv_tensor; c->inv_panel = ctx->inv_panel;
+        c->graph_loops = ctx->graph_loops; c->gemm_3m = ctx->gemm_3m; c->inv_tensor = ctx->inv_tensor; c->inv_panel = ctx->inv_panel; c->inv_lookahead = ctx->inv_lookahead; c->inv_outer = ctx->inv_outer; c->fused_small = ctx->fused_small;
     }
     return NEGF_OK;
 }

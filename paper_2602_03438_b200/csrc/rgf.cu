@@ -14,6 +14,7 @@
 // and never materialised; otherwise the two off-diagonal families are assembled once per call.
 // The diagonal blocks are assembled straight into the g family and inverted in place.
 #include "rgf_common.cuh"
+#include "fused_small.cuh"
 
 using namespace rgfc;
 
@@ -73,6 +74,21 @@ int rgf_assemble(negf_ctx* ctx, const negf_problem* p, const negf_sigma* sigma_r
     return NEGF_OK;
 }
 
+namespace {
+FusedProblem fused_problem(const negf_problem* p, const negf_sigma* sr) {
+    FusedProblem P = {};
+    P.n = p->n_blocks; P.b = p->block_size; P.ne = p->n_energy;
+    P.Hd = (const cplx*)p->H_diag; P.Hu = (const cplx*)p->H_upper; P.Sd = (const cplx*)p->S_diag; P.Su = (const cplx*)p->S_upper;
+    P.energy = p->energy; P.eta = p->eta; P.kidx = kidx_of(p);
+    P.sr_kind = sr ? sr->kind : NEGF_SIGMA_NONE;
+    if (sr) {
+        P.sr_scalar = (const cplx*)sr->scalar; P.sr_diag = (const cplx*)sr->diag; P.sr_upper = (const cplx*)sr->upper;
+        P.sr_lower = (const cplx*)sr->lower; P.sr_left = (const cplx*)sr->left; P.sr_right = (const cplx*)sr->right;
+    }
+    return P;
+}
+}  // namespace
+
 extern "C" int negf_rgf_retarded(negf_ctx* ctx, const negf_problem* p, const negf_sigma* sigma_r,
                                  negf_c128* GR_diag_, negf_c128* GR_upper_, negf_c128* GR_lower_,
                                  negf_c128* GR_corner_, int flags, int* info) {
@@ -88,6 +104,15 @@ extern "C" int negf_rgf_retarded(negf_ctx* ctx, const negf_problem* p, const neg
     const int b = s.b, ne = s.ne, n = s.n;
     const Fams F = make_fams(p, s, W, assembled);
     const Opnd GRd = {(const cplx*)GR_diag_, s.sn, s.sb, 0};
+    if (fused_small_regime(ctx, b, ne)) {     // resident regime: one CTA per energy walks both sweeps
+        NEGF_TRY(ew_fill_int(ctx, info, ne, 0));
+        const FusedProblem P = fused_problem(p, sigma_r);
+        const FusedRetOut fo = {W.g, W.X, W.Y, (cplx*)GR_diag_, (cplx*)GR_upper_, (cplx*)GR_lower_, (cplx*)GR_corner_, info};
+        NEGF_TRY(fused_ret_launch(ctx, P, fo));
+        if (flags & NEGF_KEEP_SWEEP) { ctx->sweep_valid = true; ctx->sw_n = n; ctx->sw_b = b; ctx->sw_ne = ne; ctx->sw_assembled = assembled; ctx->sw_fused = true; }
+        return NEGF_OK;
+    }
+    ctx->sw_fused = false;
     if (b <= NEGF_PAIR_MAX_B) {      // latency-bound regime: two-sided sweeps (rgf2.cu), replayed as a cached graph
         KeyHash k;
         k.val(*p); if (sigma_r) k.val(*sigma_r);
@@ -262,6 +287,22 @@ extern "C" int negf_rgf_lesser_greater(negf_ctx* ctx, const negf_problem* p, con
     if (!ctx->sweep_valid || ctx->sw_n != s.n || ctx->sw_b != s.b || ctx->sw_ne != s.ne || ctx->sw_assembled != assembled)
         return NEGF_ENOSTATE;
     const Fams F = make_fams(p, s, W, assembled);
+    if (ctx->sw_fused) {            // state left by the resident small-block kernel: S5 + S6 in one launch, too
+        NEGF_TRY(ew_fill_int(ctx, info, s.ne, 0));
+        const FusedProblem P = fused_problem(p, sigma_r);
+        FusedLgArgs la = {};
+        la.g = W.g; la.X = W.X; la.Y = W.Y; la.GR_diag = (const cplx*)GR_diag;
+        const negf_sigma* sx[2] = {sigma_lesser, sigma_greater};
+        cplx* gxw[2] = {W.gx, W.Q};
+        cplx* od[2] = {(cplx*)GL_diag, (cplx*)GG_diag};
+        cplx* ou[2] = {(cplx*)GL_upper, (cplx*)GG_upper};
+        for (int q = 0; q < 2; q++) {
+            if (!sx[q]) continue;
+            la.x[la.nx++] = FusedLgOne{sx[q]->kind, (const cplx*)sx[q]->scalar, (const cplx*)sx[q]->diag, (const cplx*)sx[q]->upper,
+                                       (const cplx*)sx[q]->left, (const cplx*)sx[q]->right, gxw[q], od[q], ou[q]};
+        }
+        return la.nx ? fused_lg_launch(ctx, P, la) : NEGF_OK;
+    }
     const bool two_sided = s.b <= NEGF_PAIR_MAX_B;
     KeyHash k;
     k.val(*p); if (sigma_r) k.val(*sigma_r); if (sigma_lesser) k.val(*sigma_lesser); if (sigma_greater) k.val(*sigma_greater);

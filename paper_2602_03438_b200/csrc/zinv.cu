@@ -1094,10 +1094,21 @@ __global__ void gj_permidx_kernel(int b, const int* ipiv, int* idxbuf, const int
     for (int c = threadIdx.x; c < b; c += blockDim.x) idxbuf[(size_t)e * b + c] = sidx[c];
 }
 
-constexpr int OUTER_NB = 128;      // outer block of the two-level blocked Gauss-Jordan
+constexpr int OUTER_NB_MAX = 256;  // widest outer block of the two-level blocked Gauss-Jordan (sizes the scratch)
+// Outer block width: the rank-nb update of all other columns is a GEMM with k = nb, the rank-32 updates inside
+// the block grow with nb, and the look-ahead has more (shorter) stages with a small nb.  Measured (kernel_bench
+// --kernel zinv, ms per batched inverse, nb = 64 / 128 / 256): b = 256 batch 256: 3.19 / 3.29 / 3.89; b = 512
+// batch 32: 3.14 / 3.00 / 3.38; b = 1024 batch 8: 5.13 / 5.38 / 5.77; b = 2048 batch 8: 33.6 / 28.4 / 27.5.
+// NEGF_OPT_INV_OUTER overrides (multiple of 32, <= 256).
+inline int outer_nb(const negf_ctx* ctx, int b) {
+    if (ctx->inv_outer >= 32 && ctx->inv_outer <= OUTER_NB_MAX && ctx->inv_outer % 32 == 0) return ctx->inv_outer;
+    if (b > 1024) return 256;
+    if (b > 512) return 64;
+    return b > 256 ? 128 : 64;
+}
 
 struct InvWs {
-    cplx* Rout;   // [batch][OUTER_NB][b]  pivot rows of an outer block
+    cplx* Rout;   // [batch][OUTER_NB_MAX][b]  pivot rows of an outer block
     cplx* R;      // [batch][PW][b]
     cplx* Pbuf;   // [batch][b][PW]
     cplx* Dinv;   // [batch][PW*PW]
@@ -1109,7 +1120,7 @@ struct InvWs {
 InvWs carve(void* ws, int b, int batch) {
     InvWs o;
     unsigned char* p = (unsigned char*)ws;
-    o.Rout = (cplx*)p; p += align_up((size_t)batch * OUTER_NB * b * sizeof(cplx), 256);
+    o.Rout = (cplx*)p; p += align_up((size_t)batch * OUTER_NB_MAX * b * sizeof(cplx), 256);
     o.R = (cplx*)p;    p += align_up((size_t)batch * PW * b * sizeof(cplx), 256);
     o.Pbuf = (cplx*)p; p += align_up((size_t)batch * PW * b * sizeof(cplx), 256);
     o.Dinv = (cplx*)p; p += align_up((size_t)batch * PW * PW * sizeof(cplx), 256);
@@ -1124,7 +1135,7 @@ InvWs carve(void* ws, int b, int batch) {
 
 size_t zinv_workspace_bytes(int b, int batch) {
     if (b <= SMALL_MAX) return 256;
-    return align_up((size_t)batch * OUTER_NB * b * sizeof(cplx), 256) +
+    return align_up((size_t)batch * OUTER_NB_MAX * b * sizeof(cplx), 256) +
            2 * align_up((size_t)batch * PW * b * sizeof(cplx), 256) +
            2 * align_up((size_t)batch * PW * PW * sizeof(cplx), 256) +
            2 * align_up((size_t)batch * b * sizeof(int), 256) +
@@ -1179,6 +1190,12 @@ int zinv_launch(negf_ctx* ctx, int b, cplx* A, long long sA, int batch, void* ws
     // those columns end up holding Q = E[:, K] of the accumulated transform E (identity outside the
     // columns K); every other column then gets all nbk swaps at once and ONE rank-nbk update
     // M[:, ~K] = (M with rows K zeroed)[:, ~K] + Q R, R = the pivot rows: a GEMM with k = 128.
+    // look-ahead over the outer blocks (side stream): only where the inverse runs on the caller's own stream (b above
+    // the two-sided regime), outside profiling (intervals must not overlap) and with at least three outer blocks
+    const int OUTER_NB = outer_nb(ctx, b);
+    cudaStream_t main_stream = ctx->stream;
+    const bool lookahead = gj_panel_rows_supported(b) && ctx->inv_panel && ctx->inv_lookahead && !ctx->prof_on &&
+                           b > 2 * OUTER_NB && ctx->inv_side != nullptr;
     for (int K0 = 0; K0 < b; K0 += OUTER_NB) {
       const int nbk = min(OUTER_NB, b - K0), K1 = K0 + nbk;
       for (int k0 = K0; k0 < K1; k0 += w) {
@@ -1302,6 +1319,37 @@ int zinv_launch(negf_ctx* ctx, int b, cplx* A, long long sA, int batch, void* ws
         NEGF_LAUNCH_CHECK(ctx);
       }
       if (nbk == b) break;       // a single outer block: nothing outside it
+      if (lookahead) {
+          // Look-ahead: the columns of the NEXT outer block get this block's swaps and rank-128 update first, on the
+          // caller's stream; all other columns follow on a side stream while the caller's stream already eliminates
+          // the panels of the next block (latency-bound, few CTAs) - the two touch disjoint columns.
+          const long long mstride = (long long)batch * 2 * PW;
+          const int2* mv0 = W.moves + (size_t)(K0 / PW) * mstride;
+          const int nph = (nbk + PW - 1) / PW, K1n = min(K1 + OUTER_NB, b);
+          GemmArgs g;
+          g.opA = 0; g.opB = 0; g.alpha = one; g.beta = one; g.batch = batch; g.skip = skip;
+          g.batch2 = 1; g.sA2 = g.sB2 = g.sD2 = g.sC2 = 0; g.alpha_vec = nullptr;
+          g.m = b; g.k = nbk; g.A = A + K0; g.lda = b; g.sA = sA;
+          g.ldb = b; g.sB = (long long)nbk * b; g.ldc = b; g.sC = sA; g.sD = sA;
+          if (K0 > 0) NEGF_CUDA_CHECK(ctx, cudaStreamWaitEvent(main_stream, ctx->ev_inv_side, 0));   // the rest of block J-1
+          if (K1 < b) {
+              NEGF_TRY(gj_moves_extract_launch(ctx, A, sA, b, batch, mv0, mstride, nph, K0, nbk, K1, K1n, 0, 0, W.Rout, skip));
+              g.n = K1n - K1; g.B = W.Rout + K1; g.C = A + K1; g.D = A + K1;
+              NEGF_TRY(zgemm_launch(ctx, g));
+          }
+          NEGF_CUDA_CHECK(ctx, cudaEventRecord(ctx->ev_inv_main, main_stream));
+          NEGF_CUDA_CHECK(ctx, cudaStreamWaitEvent(ctx->inv_side, ctx->ev_inv_main, 0));
+          ctx->stream = ctx->inv_side;
+          int rc = gj_moves_extract_launch(ctx, A, sA, b, batch, mv0, mstride, nph, K0, nbk, 0, b, K0, K1n, W.Rout, skip);
+          if (rc == NEGF_OK && K0 > 0) { g.n = K0; g.B = W.Rout; g.C = A; g.D = A; rc = zgemm_launch(ctx, g); }
+          if (rc == NEGF_OK && K1n < b) { g.n = b - K1n; g.B = W.Rout + K1n; g.C = A + K1n; g.D = A + K1n; rc = zgemm_launch(ctx, g); }
+          cudaError_t ce = cudaEventRecord(ctx->ev_inv_side, ctx->inv_side);
+          ctx->stream = main_stream;
+          if (rc != NEGF_OK) return rc;
+          NEGF_CUDA_CHECK(ctx, ce);
+          if (K1 >= b) NEGF_CUDA_CHECK(ctx, cudaStreamWaitEvent(main_stream, ctx->ev_inv_side, 0));    // join before the epilogue
+          continue;
+      }
       // all nbk swaps of this outer block on the columns outside K; pivot rows -> Rout, zeroed in A
       if (gj_panel_rows_supported(b) && ctx->inv_panel) {
           const long long mstride = (long long)batch * 2 * PW;

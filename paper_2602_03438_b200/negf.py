@@ -28,6 +28,9 @@ OPT_GEMM_3M = 2
 OPT_INV_TENSOR = 3
 OPT_ENERGY_GROUPS = 4
 OPT_INV_PANEL = 5
+OPT_INV_LOOKAHEAD = 6
+OPT_INV_OUTER = 7
+OPT_FUSED_SMALL = 8
 
 
 class c128(C.Structure):

@@ -50,6 +50,7 @@ def decimation_rows(wl, dp):
 
 CASES = [("configs[0] full (1 energy, b = 16)", 0, {}),
          ("configs[1] full (64 energies, b = 64)", 1, {}),
+         ("configs[1]-shaped, b = 24, 12 energies (resident small-block kernel)", 1, dict(n_blocks=4, block_size=24, n_energy=12)),
          ("configs[2]-shaped, b = 136, 2 energies", 2, dict(n_blocks=3, block_size=136, n_energy=2)),
          ("configs[4]-shaped, b = 200, 2 energies", 4, dict(n_blocks=3, block_size=200, n_energy=2))]
 _report = {}

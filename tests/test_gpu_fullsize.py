@@ -226,7 +226,6 @@ def _compare_energy(wl, sig, dp, k, want_greater, tag, members=("mirror", "perm"
                       "sigma_l": blk(f"sigma_l_{t}"), "sigma_g": blk(f"sigma_g_{t}")}
     o = pipeline.solve_energy(wl, k, sigma=_one(sig, k), obc_in=(side("L"), side("R")), want_greater=want_greater)
     B_list = [o["BL"]] + ([o["BG"]] if want_greater else [])
-    ens = rgf_oracle_ensemble(o["A"], B_list, members=members, seed=k)
     fams = [("GR_diag", o["ret"]["GR_diag"], lambda m: m["GR_diag"]), ("GR_upper", o["ret"]["GR_upper"], lambda m: m["GR_upper"]),
             ("GR_lower", o["ret"]["GR_lower"], lambda m: m["GR_lower"]),
             ("GL_diag", o["les"]["GX_diag"], lambda m: m["GX"][0][0]), ("GL_upper", o["les"]["GX_upper"], lambda m: m["GX"][0][1])]
@@ -235,10 +234,12 @@ def _compare_energy(wl, sig, dp, k, want_greater, tag, members=("mirror", "perm"
     per_block = lambda x, ref: np.linalg.norm(x - ref, axis=(1, 2)) / np.linalg.norm(ref, axis=(1, 2))
     gnorm = float(np.linalg.norm(o["ret"]["GR_diag"], axis=(1, 2)).max())
     anorm = float(np.linalg.norm(o["A"][0], axis=(1, 2)).max())
+    errs = [float(per_block(blk(name), ref).max()) for name, ref, _ in fams]
+    # each member costs one more oracle run: evaluated only when a family misses the plain bar
+    ens = rgf_oracle_ensemble(o["A"], B_list, members=members, seed=k) if max(errs) > TOL else None
     bad = []
-    for name, ref, pick in fams:
-        e_gpu = float(per_block(blk(name), ref).max())
-        spread = max(float(per_block(pick(m), ref).max()) for m in ens)
+    for (name, ref, pick), e_gpu in zip(fams, errs):
+        spread = max(float(per_block(pick(m), ref).max()) for m in ens) if ens is not None else float("nan")
         ok = e_gpu <= TOL or e_gpu <= 2 * spread
         _rows.append(dict(tag=tag, k=k, E=float(wl.energies[k]), n=wl.n_blocks, b=wl.block_size, family=name, e_gpu=e_gpu,
                           spread=spread, cond_est=anorm * gnorm, label="conditioning-limited" if spread > TOL / 2 else "", ok=ok))
@@ -249,7 +250,8 @@ def _compare_energy(wl, sig, dp, k, want_greater, tag, members=("mirror", "perm"
           + ", ".join(f"{r['family']} {r['e_gpu']:.1e}/{r['spread']:.1e}" for r in _rows[-len(fams):]))
     assert not bad, (tag, k, bad)
     c = rel_fro(blk("GR_corner"), o["ret"]["GR_corner"][0])
-    assert c < max(TOL, 2 * _rows[-len(fams)]["spread"]), (tag, k, "GR_corner", c)
+    gr_spread = _rows[-len(fams)]["spread"]
+    assert c < max(TOL, 2 * (gr_spread if gr_spread == gr_spread else 0.0)), (tag, k, "GR_corner", c)
     T = o["obs"]["transmission"]
     assert abs(float(dp.out["transmission"][k]) - T) <= 1e-8 * abs(T) + 1e-13
 
@@ -265,7 +267,8 @@ def _write_fullchain_report():
                     "GPU err = max over the blocks of a family of the relative Frobenius error against the fp64 oracle fed "
                     "with the GPU's own boundary blocks; ensemble spread = the same measure between the oracle and exactly "
                     "equivalent fp64 evaluations of itself (mirrored chain, permuted blocks, both); cond est = max ||A_ii||_F "
-                    "max ||G_ii||_F.  Rule: GPU err <= 1e-10, else GPU err <= 2x spread.\n\n"
+                    "max ||G_ii||_F.  Rule: GPU err <= 1e-10, else GPU err <= 2x spread (the ensemble is evaluated only for "
+                    "energies where some family misses the plain bar; nan = not needed).\n\n"
                     "| config | n | b | energy | E | family | GPU err | ensemble spread | cond est | label | rule |\n"
                     "|---|---|---|---|---|---|---|---|---|---|---|\n")
             for r in _rows:
@@ -297,7 +300,7 @@ def test_config3_full_chain_length(runner_mod):
     assert int(dp.out["info_r"].abs().sum()) == 0 and int(dp.out["status_L"].abs().sum() + dp.out["status_R"].abs().sum()) == 0
     try:
         for k in range(3):
-            _compare_energy(wl, sig, dp, k, True, "configs[3]", members=("mirror", "perm"))
+            _compare_energy(wl, sig, dp, k, True, "configs[3]", members=("mirror+perm",))
     finally:
         _release(dp)
 

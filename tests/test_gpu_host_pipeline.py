@@ -32,8 +32,9 @@ def test_pipeline_host_matches_device_calls(negf_lib, cfg, kw):
     # and against the oracle end to end (looser: the decimation's conditioning, hazard H2)
     k = wl.n_energy // 2
     o = pipeline.solve_energy(wl, k, want_greater=True)
-    assert rel_fro(hp.out["GR_diag"].numpy()[k], o["ret"]["GR_diag"]) < 1e-6
-    assert rel_fro(hp.out["GL_diag"].numpy()[k], o["les"]["GX_diag"]) < 1e-6
+    d_sig = max(rel_fro(dp.host(f"sigma_r_{t}")[k], o[s]["sigma_r"]) for t, s in (("L", "left"), ("R", "right")))
+    assert rel_fro(hp.out["GR_diag"].numpy()[k], o["ret"]["GR_diag"]) <= 10 * d_sig + 1e-10
+    assert rel_fro(hp.out["GL_diag"].numpy()[k], o["les"]["GX_diag"]) <= 10 * d_sig + 1e-10
 
 
 @pytest.mark.parametrize("cfg,kw,groups", [(1, dict(n_blocks=6, block_size=24, n_energy=37), 0),     # automatic: 4 groups

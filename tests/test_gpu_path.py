@@ -136,18 +136,22 @@ def test_obc_decimate(runner_mod, cfg, kw):
 
 @pytest.mark.parametrize("cfg,kw", [CASES[0], CASES[3], CASES[6]])
 def test_end_to_end(runner_mod, cfg, kw):
-    """GPU decimation -> GPU RGF end to end vs the oracle end to end (reported, looser bar: the
-    decimation's conditioning, H2, propagates)."""
+    """GPU decimation -> GPU RGF end to end vs the oracle end to end.  The only difference between the two runs that is
+    not held to 1e-10 elsewhere is the boundary self-energy (conditioning-limited, H2), and G depends smoothly on it,
+    so the end-to-end error is bounded by a small multiple of the Sigma_B difference of the worst energy: bar
+    10 x max_E ||Sigma_B(GPU) - Sigma_B(oracle)|| / ||Sigma_B|| + 1e-10 (measured: 1.0x ... 3x that difference)."""
     wl = W.make_workload(cfg, **kw)
     sig, outs = _oracle_all(wl)
     dp = runner_mod.DevicePath(wl, want_greater=True, sigma=sig)
     dp.run()
+    d_sig = max(rel_fro(dp.host(f"sigma_r_{tag}")[k], outs[k][side]["sigma_r"])
+                for k in range(wl.n_energy) for tag, side in (("L", "left"), ("R", "right")))
     ref = np.stack([o["ret"]["GR_diag"] for o in outs])
     e1 = rel_fro(dp.host("GR_diag"), ref)
     ref = np.stack([o["les"]["GX_diag"] for o in outs])
     e2 = rel_fro(dp.host("GL_diag"), ref)
-    print(f"END-TO-END cfg{cfg}{kw}: GR_diag {e1:.2e}, GL_diag {e2:.2e} (fp64 oracle end to end)")
-    assert e1 < 1e-6 and e2 < 1e-6
+    print(f"END-TO-END cfg{cfg}{kw}: GR_diag {e1:.2e}, GL_diag {e2:.2e}, Sigma_B difference {d_sig:.2e} (fp64 oracle end to end)")
+    assert e1 <= 10 * d_sig + 1e-10 and e2 <= 10 * d_sig + 1e-10, (e1, e2, d_sig)
 
 
 def test_n1_explicit_lead_rejected_without_lead(runner_mod, negf_lib):
