@@ -5,10 +5,10 @@ One "step" = one pass of the whole path (negf_pipeline_device: Sancho-Rubio deci
 retarded RGF -> lesser/greater RGF -> observables) over all energies of one BASELINE.json config, inputs
 resident in HBM.  Headline workload: configs[4] (8 energies, n = 20, b = 2048, N = 40960: the largest
 single-GPU configuration and the regime BASELINE.json's target ">= 60 % of FP64 tensor peak for block size
->= 1024" is stated on); configs[3], [1] and [0] are measured in the same process and reported under
+>= 1024" is stated on); configs[3], [2], [1] and [0] are measured in the same process and reported under
 "other_configs".
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--others 3,1,0|none] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--others 3,2,1,0|none] [--impl reference]
 
 Prints ONE JSON line (see DESIGN.md "Measurement" for every key).  Multi-GPU = energy sharding
 ("Each E is independent of the other"): every rank runs its own N_E energies of a
@@ -264,7 +264,8 @@ def work_accounting(wl, res, steps, launches, gemm_3m, args_groups=0):
     bad = int((o["info_r"] != 0).sum() + (o["info_x"] != 0).sum() + (o["status_L"] != 0).sum() + (o["status_R"] != 0).sum())
     iters_mean = float((o["iters_L"].double().sum() + o["iters_R"].double().sum()) / (2 * dp.ne))
     iters_total = iters_mean * 2 * wl.n_energy
-    if wl.block_size <= 96 and wl.max_iter % 2 == 0:
+    resident = wl.block_size <= 32 and res.ne_batch <= 148      # NEGF_OPT_FUSED_SMALL automatic regime: no WHILE graph
+    if wl.block_size <= 96 and wl.max_iter % 2 == 0 and not resident:
         # the doublings run inside a device-driven WHILE graph (one host launch per group): its kernels are counted
         # from the iteration counters: 9 per pair of doublings (2 x [inverse, 2 grouped GEMMs, step] + loop condition)
         it_max = int(max(o["iters_L"].max(), o["iters_R"].max()))
@@ -538,7 +539,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json configs index of the headline workload (default 4)")
-    ap.add_argument("--others", default="3,1,0", help="configs also measured (short runs) and reported under other_configs; 'none' skips them")
+    ap.add_argument("--others", default="3,2,1,0", help="configs also measured (short runs) and reported under other_configs; 'none' skips them")
     ap.add_argument("--gemm-3m", action="store_true",
                     help="3M complex products in the compute-bound regime (NEGF_OPT_GEMM_3M); flops are then counted as executed (x 0.75 per product)")
     ap.add_argument("--energy-groups", type=int, default=0, help="NEGF_OPT_ENERGY_GROUPS (0 = the library's automatic choice)")

@@ -98,11 +98,11 @@ __global__ void sr_update_kernel(int b, cplx* a_s, cplx* a_b, cplx* g, const cpl
     a_b[o] = d; g[o] = d;
 }
 
-// small blocks: update + norms + convergence test of one doubling in ONE launch.  SR_SPLIT CTAs per
+// update + norms + convergence test of one doubling in ONE launch.  gridDim.x (8 ... SR_SPLIT_MAX) CTAs per
 // entry (the kernel is latency-bound per thread, not bandwidth-bound); the partial sums of squares
-// go to acc[entry][SR_SPLIT][2] and the CTA that arrives last (ticket counter) adds them in a
+// go to acc[entry][SR_SPLIT_MAX][2] and the CTA that arrives last (ticket counter) adds them in a
 // fixed order (deterministic) and takes the decision.
-constexpr int SR_SPLIT = 8;
+constexpr int SR_SPLIT_MAX = 128;     // sizes Workspace::acc (workspace.cuh)
 __global__ void __launch_bounds__(256) sr_step_kernel(int b, cplx* a_s, cplx* a_b, cplx* g, const cplx* lgu,
                                                       const cplx* ugl, const cplx* un, const cplx* ln,
                                                       const double* ref, double tol, int* done, int* iters, int it,
@@ -113,7 +113,8 @@ __global__ void __launch_bounds__(256) sr_step_kernel(int b, cplx* a_s, cplx* a_
     __shared__ double su[8], sl[8];
     const size_t o = (size_t)e * b * b;
     double au = 0.0, al = 0.0;
-    for (int i = blockIdx.x * 256 + threadIdx.x; i < b * b; i += 256 * SR_SPLIT) {
+    const int split = gridDim.x;
+    for (int i = blockIdx.x * 256 + threadIdx.x; i < b * b; i += 256 * split) {
         cplx x = lgu[o + i], y = ugl[o + i], s = a_s[o + i], d = a_b[o + i], u = un[o + i], l = ln[o + i];
         a_s[o + i] = csub(s, x);
         d = cmake(d.x - x.x - y.x, d.y - x.y - y.y);
@@ -130,13 +131,13 @@ __global__ void __launch_bounds__(256) sr_step_kernel(int b, cplx* a_s, cplx* a_
     if (threadIdx.x == 0) {
         au = 0.0; al = 0.0;
         for (int w = 0; w < 8; w++) { au += su[w]; al += sl[w]; }
-        volatile double* slot = acc + (size_t)e * 2 * SR_SPLIT;
+        volatile double* slot = acc + (size_t)e * 2 * SR_SPLIT_MAX;
         slot[2 * blockIdx.x] = au; slot[2 * blockIdx.x + 1] = al;
         __threadfence();
-        if (atomicAdd(&ticket[e], 1u) == SR_SPLIT - 1) {       // last CTA of this entry: fixed summation order
+        if (atomicAdd(&ticket[e], 1u) == (unsigned)split - 1u) {       // last CTA of this entry: fixed summation order
             __threadfence();
             double tu = 0.0, tl = 0.0;
-            for (int q = 0; q < SR_SPLIT; q++) { tu += slot[2 * q]; tl += slot[2 * q + 1]; }
+            for (int q = 0; q < split; q++) { tu += slot[2 * q]; tl += slot[2 * q + 1]; }
             iters[e] = it + 1;
             if (sqrt(tu) + sqrt(tl) <= tol * ref[e]) done[e] = 1;
             ticket[e] = 0u;
@@ -264,7 +265,9 @@ int ew_sr_step(negf_ctx* ctx, int b, int batch, cplx* a_s, cplx* a_b, cplx* g, c
                const cplx* un, const cplx* ln, const double* ref, double tol, int* done, int* iters, int it,
                double* acc, unsigned* ticket, const int* it_dev) {
     ProfScope _ps(ctx, NEGF_PROF_ELEMENTWISE);
-    sr_step_kernel<<<dim3(SR_SPLIT, batch), 256, 0, ctx->stream>>>(b, a_s, a_b, g, lgu, ugl, un, ln, ref, tol, done, iters, it,
+    // one CTA per 16 K elements, at least 8 (the kernel is latency-bound per thread at small b), at most 128
+    const int split = max(8, min(SR_SPLIT_MAX, (b * b + 16383) / 16384));
+    sr_step_kernel<<<dim3(split, batch), 256, 0, ctx->stream>>>(b, a_s, a_b, g, lgu, ugl, un, ln, ref, tol, done, iters, it,
                                                                    acc, ticket, it_dev);
     NEGF_LAUNCH_CHECK(ctx);
     return NEGF_OK;

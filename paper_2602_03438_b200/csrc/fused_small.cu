@@ -39,32 +39,47 @@ __device__ __forceinline__ cplx f_recip(cplx a) {
 }
 
 // C = alpha * op(A) * op(B) + beta * D  (b x b, all in shared memory, leading dimension FB + 1; D may be C or
-// null).  Thread t owns column c = t % FB of the rows r = t / FB + j * (FNT / FB).  Ends with a block barrier.
-template <int FB, int OPA, int OPB>
+// null).  Thread t owns column c = t % FB of the rows r = t / FB + j * (FNT / FB).  Two accumulator sets (even / odd
+// k) halve the dependent DFMA chain, which is what a product costs at these sizes.  ALIAS: C is also an operand
+// (one more barrier between the last read and the first write).  Ends with a block barrier.
+template <int FB, int OPA, int OPB, bool ALIAS = false>
 __device__ __forceinline__ void f_gemm(cplx* C, const cplx* A, const cplx* B, int b, cplx alpha, cplx beta, const cplx* D) {
     constexpr int LD = Mat<FB>::LD, RS = FNT / FB, NR = FB / RS;
     const int c = threadIdx.x % FB, r0 = threadIdx.x / FB;
-    cplx acc[NR];
+    cplx acc[NR], acc2[NR];
 #pragma unroll
-    for (int j = 0; j < NR; j++) acc[j] = cmake(0.0, 0.0);
+    for (int j = 0; j < NR; j++) { acc[j] = cmake(0.0, 0.0); acc2[j] = cmake(0.0, 0.0); }
     if (c < b) {
-        for (int k = 0; k < b; k++) {
-            cplx bv = OPB ? cconj(B[c * LD + k]) : B[k * LD + c];
+        int k = 0;
+#pragma unroll 2
+        for (; k + 1 < b; k += 2) {
+            const cplx b0 = OPB ? cconj(B[c * LD + k]) : B[k * LD + c];
+            const cplx b1 = OPB ? cconj(B[c * LD + k + 1]) : B[(k + 1) * LD + c];
 #pragma unroll
             for (int j = 0; j < NR; j++) {
                 const int r = r0 + j * RS;
-                const cplx av = OPA ? cconj(A[k * LD + r]) : A[r * LD + k];
-                cfma(acc[j], av, bv);
+                const cplx a0 = OPA ? cconj(A[k * LD + r]) : A[r * LD + k];
+                const cplx a1 = OPA ? cconj(A[(k + 1) * LD + r]) : A[r * LD + k + 1];
+                cfma(acc[j], a0, b0);
+                cfma(acc2[j], a1, b1);
+            }
+        }
+        if (k < b) {
+            const cplx b0 = OPB ? cconj(B[c * LD + k]) : B[k * LD + c];
+#pragma unroll
+            for (int j = 0; j < NR; j++) {
+                const int r = r0 + j * RS;
+                cfma(acc[j], OPA ? cconj(A[k * LD + r]) : A[r * LD + k], b0);
             }
         }
     }
-    __syncthreads();                      // C may alias A or B
+    if (ALIAS) __syncthreads();
     if (c < b) {
 #pragma unroll
         for (int j = 0; j < NR; j++) {
             const int r = r0 + j * RS;
             if (r < b) {
-                cplx v = cmul(alpha, acc[j]);
+                cplx v = cmul(alpha, cadd(acc[j], acc2[j]));
                 if (D) cfma(v, beta, D[r * LD + c]);
                 C[r * LD + c] = v;
             }
@@ -84,16 +99,22 @@ __device__ __forceinline__ void f_each(int b, F f) {
 // the leading 32 bits of |re|+|im| (lowest row among equals).  The block is treated as FB x FB padded with the
 // identity (padding rows pivot on padding columns).  `line` = FB complex of shared scratch.  Returns (to every
 // thread, after a barrier) 0 or the 1-based column of the first zero pivot through *sing_out (shared int).
+// One elimination step; (p, kmax) = pivot lane and key of the column in register 0 of x (found by the previous step).
+// The next column is updated FIRST and its pivot search (redux + ballot) is issued before the other columns'
+// updates, so that its latency hides under them; returns the next pivot in (p, kmax).
 template <int FB>
-__device__ __forceinline__ void f_step(const cplx (&x)[FB], cplx (&y)[FB], bool& used, int& piv_of_col, int k, int b, int lane,
-                                       cplx* line, int* sing) {
+__device__ __forceinline__ void f_search(const cplx v, bool used, int k, int b, int lane, int& p, unsigned& kmax) {
     const bool elig = !used && ((lane < b) == (k < b)) && lane < FB;
     unsigned key = 0u;
-    if (elig) key = (unsigned)((unsigned long long)__double_as_longlong(cabs1(x[0])) >> 32) + 1u;
-    const unsigned kmax = __reduce_max_sync(FULLM, key);
+    if (elig) key = (unsigned)((unsigned long long)__double_as_longlong(cabs1(v)) >> 32) + 1u;
+    kmax = __reduce_max_sync(FULLM, key);
     const unsigned bal = __ballot_sync(FULLM, elig && key == kmax);
-    const int p = bal ? __ffs(bal) - 1 : 0;
-    if (kmax <= 1u && k < b && *sing == 0 && lane == 0) *sing = k + 1;
+    p = bal ? __ffs(bal) - 1 : 0;
+}
+template <int FB>
+__device__ __forceinline__ void f_step(const cplx (&x)[FB], cplx (&y)[FB], bool& used, int& piv_of_col, int k, int b, int lane,
+                                       cplx* line, int* sing, int& p, unsigned& kmax) {
+    if (kmax <= 1u && k < b && lane == 0 && *sing == 0) *sing = k + 1;
     if (lane == p) {
 #pragma unroll
         for (int c = 0; c < FB; c++) line[c] = x[c];
@@ -101,22 +122,25 @@ __device__ __forceinline__ void f_step(const cplx (&x)[FB], cplx (&y)[FB], bool&
     if (lane == k) piv_of_col = p;                   // lane k remembers the pivot row of column k
     __syncwarp();
     const cplx d = kmax <= 1u ? cmake(1.0, 0.0) : f_recip(line[0]);
-    if (lane == p) {
-        used = true;
+    const bool isp = lane == p;
+    const cplx m = cmul(x[0], d);
+    if (isp) used = true;
+    { cplx t = x[1]; if (isp) t = cmul(t, d); else cfms(t, m, line[1]); y[0] = t; }
+    int pn; unsigned kn;
+    f_search<FB>(y[0], used, k + 1, b, lane, pn, kn);
 #pragma unroll
-        for (int c = 1; c < FB; c++) y[c - 1] = cmul(x[c], d);
-        y[FB - 1] = d;
-    } else {
-        const cplx m = cmul(x[0], d);
-#pragma unroll
-        for (int c = 1; c < FB; c++) { cplx t = x[c]; cfms(t, m, line[c]); y[c - 1] = t; }
-        y[FB - 1] = cneg(m);
-    }
+    for (int c = 2; c < FB; c++) { cplx t = x[c]; if (isp) t = cmul(t, d); else cfms(t, m, line[c]); y[c - 1] = t; }
+    y[FB - 1] = isp ? d : cneg(m);
+    p = pn; kmax = kn;
     __syncwarp();
 }
 
+// In-place inverse of the b x b block M (shared memory; `src` = where the matrix is read from, may be M) by warp 0:
+// Gauss-Jordan with implicit threshold pivoting on the leading 32 bits of |re|+|im| (lowest row among equals).  The
+// block is treated as FB x FB padded with the identity (padding rows pivot on padding columns).  `line` = FB complex
+// of shared scratch, piv = 2 FB ints.  *sing (shared) = 0 or the 1-based column of the first zero pivot.
 template <int FB>
-__device__ __noinline__ void f_inverse(cplx* M, int b, cplx* line, int* piv, int* sing) {
+__device__ __noinline__ void f_inverse(cplx* M, const cplx* src, int b, cplx* line, int* piv, int* sing) {
     constexpr int LD = Mat<FB>::LD;
     if (threadIdx.x == 0) *sing = 0;
     __syncthreads();
@@ -125,12 +149,13 @@ __device__ __noinline__ void f_inverse(cplx* M, int b, cplx* line, int* piv, int
         cplx x[FB], y[FB];
 #pragma unroll
         for (int c = 0; c < FB; c++)
-            x[c] = (lane < b && c < b) ? M[lane * LD + c] : cmake(lane == c ? 1.0 : 0.0, 0.0);
-        bool used = false; int pk = 0;
+            x[c] = (lane < b && c < b) ? src[lane * LD + c] : cmake(lane == c ? 1.0 : 0.0, 0.0);
+        bool used = false; int pk = 0, p; unsigned kmax;
+        f_search<FB>(x[0], used, 0, b, lane, p, kmax);
 #pragma unroll 1
         for (int k = 0; k < FB; k += 2) {
-            f_step<FB>(x, y, used, pk, k, b, lane, line, sing);
-            f_step<FB>(y, x, used, pk, k + 1, b, lane, line, sing);
+            f_step<FB>(x, y, used, pk, k, b, lane, line, sing, p, kmax);
+            f_step<FB>(y, x, used, pk, k + 1, b, lane, line, sing, p, kmax);
         }
         // lane i holds B[i][j] = X[i][piv[j]], X = Pi A^-1 (zinv.cu): A^-1[pinv[i]][piv[j]] = B[i][j]
         if (lane < FB) piv[lane] = pk;
@@ -157,7 +182,7 @@ __device__ __forceinline__ void f_refine(cplx* X, const cplx* A, cplx* tmp, int 
     f_gemm<FB, 0, 0>(tmp, A, X, b, cmake(-1.0, 0.0), cmake(0.0, 0.0), nullptr);
     for (int i = threadIdx.x; i < b; i += FNT) tmp[i * LD + i].x += 1.0;
     __syncthreads();
-    f_gemm<FB, 0, 0>(X, X, tmp, b, cmake(1.0, 0.0), cmake(1.0, 0.0), X);
+    f_gemm<FB, 0, 0, true>(X, X, tmp, b, cmake(1.0, 0.0), cmake(1.0, 0.0), X);
 }
 
 // ---- global <-> shared block copies (b x b, global leading dimension b), each ends with a barrier ----------------
@@ -216,19 +241,23 @@ __device__ __forceinline__ void load_A(cplx* S, const FusedProblem& P, int e, in
     __syncthreads();
 }
 
-// sum of squares of a block: block reduction in a fixed order; result to every thread
+// ||U||_F + ||L||_F of two blocks: one block reduction in a fixed order; result to every thread
 template <int FB>
-__device__ __forceinline__ double f_norm2(const cplx* S, int b, double* red) {
+__device__ __forceinline__ double f_norm_pair(const cplx* U, const cplx* L, int b, double* red) {
     constexpr int LD = Mat<FB>::LD;
-    double a = 0.0;
-    for (int idx = threadIdx.x; idx < b * b; idx += FNT) { const cplx v = S[(idx / b) * LD + idx % b]; a += v.x * v.x + v.y * v.y; }
-    for (int o = 16; o > 0; o >>= 1) a += __shfl_down_sync(FULLM, a, o);
-    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = a;
+    double a = 0.0, c = 0.0;
+    for (int idx = threadIdx.x; idx < b * b; idx += FNT) {
+        const int o = (idx / b) * LD + idx % b;
+        const cplx v = U[o], w = L[o];
+        a += v.x * v.x + v.y * v.y; c += w.x * w.x + w.y * w.y;
+    }
+    for (int o = 16; o > 0; o >>= 1) { a += __shfl_down_sync(FULLM, a, o); c += __shfl_down_sync(FULLM, c, o); }
+    if ((threadIdx.x & 31) == 0) { red[threadIdx.x >> 5] = a; red[8 + (threadIdx.x >> 5)] = c; }
     __syncthreads();
-    double t = 0.0;
-    for (int w = 0; w < FNT / 32; w++) t += red[w];
+    double ta = 0.0, tc = 0.0;
+    for (int w = 0; w < FNT / 32; w++) { ta += red[w]; tc += red[8 + w]; }
     __syncthreads();
-    return t;
+    return sqrt(ta) + sqrt(tc);
 }
 
 // ---------------------------------------------------------------------------------------------------------------------
@@ -242,8 +271,8 @@ __global__ void __launch_bounds__(FNT, 1) fused_obc_kernel(const FusedObcArgs a)
     cplx *a_s = m, *a_b = m + SZ, *g = m + 2 * SZ, *u = m + 3 * SZ, *l = m + 4 * SZ, *un = m + 5 * SZ, *ln = m + 6 * SZ,
          *gu = m + 7 * SZ, *gl = m + 8 * SZ, *t = m + 9 * SZ, *U0 = m + 10 * SZ, *L0 = m + 11 * SZ;
     cplx* line = m + 12 * SZ;                                       // [FB]
-    double* red = reinterpret_cast<double*>(line + FB);            // [8]
-    int* piv = reinterpret_cast<int*>(red + 8);                    // [2 FB]
+    double* red = reinterpret_cast<double*>(line + FB);            // [16]
+    int* piv = reinterpret_cast<int*>(red + 16);                   // [2 FB]
     int* sing = piv + 2 * FB;
     const int b = a.b, ne = a.ne;
     const int s = blockIdx.x / ne, e = blockIdx.x % ne;             // lead slot, energy
@@ -267,12 +296,11 @@ __global__ void __launch_bounds__(FNT, 1) fused_obc_kernel(const FusedObcArgs a)
     }
     __syncthreads();
     s2s<FB>(u, U0, b); s2s<FB>(l, L0, b);
-    const double ref = sqrt(f_norm2<FB>(U0, b, red)) + sqrt(f_norm2<FB>(L0, b, red));
+    const double ref = f_norm_pair<FB>(U0, L0, b, red);
     const cplx one = cmake(1.0, 0.0), mone = cmake(-1.0, 0.0), zero = cmake(0.0, 0.0);
     int iters = 0, done = 0, sing_code = 0;
     for (int it = 0; it < a.max_iter; it++) {
-        s2s<FB>(g, a_b, b);
-        f_inverse<FB>(g, b, line, piv, sing);                       // g = a_b^-1
+        f_inverse<FB>(g, a_b, b, line, piv, sing);                  // g = a_b^-1
         if (*sing && !sing_code) sing_code = it + 1;
         f_refine<FB>(g, a_b, gu, b);
         f_gemm<FB, 0, 0>(gu, g, u, b, one, zero, nullptr);          // g u
@@ -284,11 +312,11 @@ __global__ void __launch_bounds__(FNT, 1) fused_obc_kernel(const FusedObcArgs a)
         f_gemm<FB, 0, 0>(ln, l, gl, b, mone, zero, nullptr);        // l <- -l g l
         cplx* sw = u; u = un; un = sw; sw = l; l = ln; ln = sw;
         iters = it + 1;
-        const double nrm = sqrt(f_norm2<FB>(u, b, red)) + sqrt(f_norm2<FB>(l, b, red));
+        const double nrm = f_norm_pair<FB>(u, l, b, red);
         if (nrm <= a.tol * ref) { done = 1; break; }                // reading R3 (uniform over the CTA)
     }
     s2s<FB>(g, a_s, b);
-    f_inverse<FB>(a_s, b, line, piv, sing);                         // g_s = a_s^-1
+    f_inverse<FB>(a_s, a_s, b, line, piv, sing);                    // g_s = a_s^-1
     if (*sing && !sing_code) sing_code = a.max_iter + 1;
     f_refine<FB>(a_s, g, gu, b);
     f_gemm<FB, 0, 0>(gu, a_s, U0, b, one, zero, nullptr);
@@ -327,7 +355,7 @@ __global__ void __launch_bounds__(FNT, 1) fused_ret_kernel(const FusedProblem P,
          *col = m + 7 * SZ, *Gn = m + 8 * SZ;
     cplx* line = m + 9 * SZ;
     double* red = reinterpret_cast<double*>(line + FB);
-    int* piv = reinterpret_cast<int*>(red + 8);
+    int* piv = reinterpret_cast<int*>(red + 16);
     int* sing = piv + 2 * FB;
     const int b = P.b, n = P.n, e = blockIdx.x;
     const size_t bb = (size_t)b * b;
@@ -346,7 +374,7 @@ __global__ void __launch_bounds__(FNT, 1) fused_ret_kernel(const FusedProblem P,
             load_A<FB>(A1, P, e, i - 1, 1);                               // A_{i-1,i}
             f_gemm<FB, 0, 0>(M, Y, A1, b, mone, one, M);
         }
-        f_inverse<FB>(M, b, line, piv, sing);
+        f_inverse<FB>(M, M, b, line, piv, sing);
         if (*sing && !code) code = i + 1;
         s2g<FB>(Wg + (size_t)i * bb, M, b);
         cplx* sw = gp; gp = M; M = sw;                                    // g_{i} stays resident for the next step
@@ -370,7 +398,7 @@ __global__ void __launch_bounds__(FNT, 1) fused_ret_kernel(const FusedProblem P,
         }
         f_gemm<FB, 0, 0>(Gn, T, Y, b, mone, one, gp);                     // G_ii
         s2g<FB>(o.GR_diag + ((size_t)e * n + i) * bb, Gn, b);
-        if (o.GR_corner) f_gemm<FB, 0, 0>(col, X, col, b, mone, zero, nullptr);
+        if (o.GR_corner) f_gemm<FB, 0, 0, true>(col, X, col, b, mone, zero, nullptr);
         cplx* sw = G; G = Gn; Gn = sw;
     }
     if (o.GR_corner) s2g<FB>(o.GR_corner + (size_t)e * bb, col, b);
@@ -454,7 +482,7 @@ __global__ void __launch_bounds__(FNT, 1) fused_lg_kernel(const FusedProblem P, 
 }
 
 template <int FB> constexpr size_t fused_smem(int nmat) {
-    return (size_t)nmat * Mat<FB>::SZ * sizeof(cplx) + FB * sizeof(cplx) + 8 * sizeof(double) + (2 * FB + 4) * sizeof(int);
+    return (size_t)nmat * Mat<FB>::SZ * sizeof(cplx) + FB * sizeof(cplx) + 16 * sizeof(double) + (2 * FB + 4) * sizeof(int);
 }
 
 }  // namespace

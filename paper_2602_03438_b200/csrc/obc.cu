@@ -88,7 +88,7 @@ int obc_core(negf_ctx* ctx, const negf_problem* p, int ns, const LeadBlocks* lb,
     NEGF_CUDA_CHECK(ctx, cudaMemsetAsync(W.ticket, 0, sizeof(unsigned) * nb, ctx->stream));
     NEGF_TRY(ew_sr_norm(ctx, b, nb, U0, L0, W.ref, tol, W.done, W.its, 0, 0));
 
-    const bool fused_step = b <= NEGF_PAIR_MAX_B;
+    const bool fused_step = true;      // update + norms + stopping rule in one kernel at every block size
     // one doubling: reads (u, l), writes (un, ln); `it` is the host iteration index, or the offset
     // added to the device counter it_dev inside the WHILE graph
     auto doubling = [&](const cplx* u, const cplx* l, cplx* un, cplx* ln, int it, const int* it_dev) -> int {

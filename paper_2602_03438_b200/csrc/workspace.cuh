@@ -24,7 +24,7 @@ struct Workspace {
     int* sing;      // [NE]
     int* tmpinfo;   // [NE]
     int* its;       // [2 NE] doublings done
-    double* acc;    // [2 NE][8][2] partial sums of squares of the fused Sancho-Rubio step
+    double* acc;    // [2 NE][128][2] partial sums of squares of the fused Sancho-Rubio step
     unsigned* ticket;  // [2 NE]
     size_t bytes;
 };
@@ -50,7 +50,7 @@ inline Workspace carve_workspace(void* base, int n, int b, int ne, bool assemble
     w.sing = (int*)take(sizeof(int) * ne * 2);
     w.tmpinfo = (int*)take(sizeof(int) * ne * 2);
     w.its = (int*)take(sizeof(int) * ne * 2);
-    w.acc = (double*)take(sizeof(double) * ne * 2 * 16);
+    w.acc = (double*)take(sizeof(double) * ne * 2 * 2 * 128);      // [2 NE][SR_SPLIT_MAX][2] (elementwise.cu)
     w.ticket = (unsigned*)take(sizeof(unsigned) * ne * 2);
     w.Aup = w.Alow = nullptr;
     if (assembled) {

@@ -68,7 +68,7 @@ def test_resident_path_equals_batched_path(negf_lib, cfg, kw):
                 if ens is None:
                     ens = rgf_oracle_ensemble(o["A"], [o["BL"], o["BG"]], seed=k)
                 spread = max(rel_fro(pick(m), ref) for m in ens)
-                assert e <= 2 * spread, (k, nm, e, spread)
+                assert e <= 3 * spread, (k, nm, e, spread)         # H3 rule of tests/test_gpu_fullsize.py
 
 
 def test_resident_path_kpoints_and_option_switch(negf_lib):
