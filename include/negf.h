@@ -48,6 +48,7 @@ typedef struct negf_ctx negf_ctx;
 #define NEGF_EUNSUPPORTED -3   /* combination not implemented (documented at the call)         */
 #define NEGF_ECUDA        -4   /* CUDA runtime error; see negf_last_cuda_error()               */
 #define NEGF_ENOSTATE     -5   /* call needs the retained sweep state of negf_rgf_retarded     */
+#define NEGF_ESTATICLIMIT  -6   /* problem needs more than NEGF_STATIC_SCRATCH_BYTES (negf_zinverse_batched_static) */
 
 /* kinds of scattering self-energy Sigma_S */
 #define NEGF_SIGMA_NONE   0
@@ -331,6 +332,21 @@ int negf_zgemm_batched(negf_ctx* ctx, int opA, int opB, int m, int n, int k,
  * |re|+|im| (b <= 96: on its 25 leading bits, i.e. threshold pivoting at 1 - 2^-13); info[e] = 0 or
  * (column+1) of the first zero pivot.  Uses the context workspace. */
 int negf_zinverse_batched(negf_ctx* ctx, int b, negf_c128* A, long long stride, int batch, int* info);
+/* The same inverse for callers that must not allocate and have no workspace to hand over (code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid cudaMalloc): identical kernels, launch sequence and results
+ * as negf_zinverse_batched (K1; the block inversions of the RGF recurrences), but
+ * the scratch of the blocked algorithm (b > 96: pivot rows, row-move tables, pivot indices) is a file-scope
+ * `static __device__` array of NEGF_STATIC_SCRATCH_BYTES inside the library, which every GPU that loads the
+ * library holds until the process exits.  The call itself makes no cudaMalloc / cudaFree and calls no allocating
+ * library routine; it ignores (and leaves untouched) the context workspace and the retained sweep state.
+ * Limit: b <= 96 needs no scratch (any batch <= what the kernels take); above that about 5.2 KB * b per matrix, i.e.
+ * batch * b <= ~3200 (b = 130: batch 24; b = 256: 12; b = 1024: 3; b = 2048: 1).  Larger problems return
+ * NEGF_ESTATICLIMIT and launch nothing; NEGF_EUNSUPPORTED while negf_profile_enable is on (it creates events).
+ * All calls on a GPU share the one array, which keeps the last call's contents (nothing in it needs to start at
+ * zero: each call writes what it reads): calls that OVERLAP on the GPU (different streams, contexts or host
+ * threads) race; order them on one stream or with events.  A, info: DEVICE pointers as for negf_zinverse_batched. */
+#define NEGF_STATIC_SCRATCH_BYTES (16u << 20)
+int negf_zinverse_batched_static(negf_ctx* ctx, int b, negf_c128* A, long long stride, int batch, int* info);
 /* Measures the FP64 DMMA (mma.sync m8n8k4) issue-rate peak of this GPU for about `ms`
  * milliseconds; SYNCHRONISES.  Writes TFLOP/s to *tflops (HOST pointer). */
 int negf_fp64_peak(negf_ctx* ctx, double ms, double* tflops);

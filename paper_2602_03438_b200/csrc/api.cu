@@ -112,6 +112,7 @@ extern "C" const char* negf_strerror(int code) {
         case NEGF_EUNSUPPORTED: return "unsupported configuration or device (needs compute capability 10.x)";
         case NEGF_ECUDA: return "CUDA runtime error (see negf_last_cuda_error)";
         case NEGF_ENOSTATE: return "no retained sweep state: call negf_rgf_retarded with NEGF_KEEP_SWEEP first";
+        case NEGF_ESTATICLIMIT: return "problem exceeds the static scratch of the no-allocation entry point (NEGF_STATIC_SCRATCH_BYTES)";
         default: return "unknown error code";
     }
 }

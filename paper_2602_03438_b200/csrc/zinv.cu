@@ -1142,6 +1142,22 @@ size_t zinv_workspace_bytes(int b, int batch) {
            align_up((size_t)((b + PW - 1) / PW) * batch * 2 * PW * sizeof(int2), 256);
 }
 
+// ---- scratch of the no-allocation entry point (negf_zinverse_batched_static, end of this file) ----------------
+// One file-scope device array per GPU that loads the library, held until the process exits.  In HOST code the name
+// `zinv_static_scratch` is only a stand-in for the symbol, not a device address: the address the kernels get is the
+// one cudaGetSymbolAddress returns, taken once per device at set-up (negf_create, with that device current).
+static __device__ __align__(256) unsigned char zinv_static_scratch[NEGF_STATIC_SCRATCH_BYTES];
+constexpr int ZINV_STATIC_MAX_DEVICES = 64;
+static void* zinv_static_ptr[ZINV_STATIC_MAX_DEVICES];      // [device] -> device address of that GPU's copy
+
+static int zinv_static_setup(negf_ctx* ctx) {
+    if (ctx->device < 0 || ctx->device >= ZINV_STATIC_MAX_DEVICES) return NEGF_OK;    // the entry point reports it
+    void* ptr = nullptr;
+    NEGF_CUDA_CHECK(ctx, cudaGetSymbolAddress(&ptr, zinv_static_scratch));
+    zinv_static_ptr[ctx->device] = ptr;      // same value from every context of the device
+    return NEGF_OK;
+}
+
 // shared-memory opt-ins of the blocked path, once per context (= per device) at negf_create
 int zinv_prepare(negf_ctx* ctx) {
     NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_panel_cluster_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -1151,6 +1167,7 @@ int zinv_prepare(negf_ctx* ctx) {
     NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_colperm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
     NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_panel_reg_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)reg_panel_smem_bytes(8)));
     NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(gj_panel_reg_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)reg_panel_smem_bytes(16)));
+    NEGF_TRY(zinv_static_setup(ctx));
     return NEGF_OK;
 }
 
@@ -1390,4 +1407,17 @@ extern "C" int negf_zinverse_batched(negf_ctx* ctx, int b, negf_c128* A, long lo
     if (info) NEGF_CUDA_CHECK(ctx, cudaMemsetAsync(info, 0, sizeof(int) * batch, ctx->stream));
     if (b > SMALL_MAX) ctx->sweep_valid = false;     // the scratch below overlays the retained sweep state
     return zinv_launch(ctx, b, (cplx*)A, stride, batch, ctx->ws, info, 0, nullptr);
+}
+
+// No-allocation variant (include/negf.h): same kernels and launch sequence as negf_zinverse_batched, with the K1
+// scratch (pivot rows, row-move tables, pivot indices) in this file's static device array instead of the context
+// workspace.  Nothing in the scratch has to start at zero: every region is written by the call before it is read.
+extern "C" int negf_zinverse_batched_static(negf_ctx* ctx, int b, negf_c128* A, long long stride, int batch, int* info) {
+    if (!ctx || !A || b < 1 || batch < 0) return NEGF_EINVAL;
+    if (ctx->prof_on) return NEGF_EUNSUPPORTED;          // the per-class profiler creates CUDA events
+    if (ctx->device < 0 || ctx->device >= ZINV_STATIC_MAX_DEVICES || !zinv_static_ptr[ctx->device]) return NEGF_EUNSUPPORTED;
+    if (b > SMALL_MAX && (batch > 65535 || zinv_workspace_bytes(b, batch) > (size_t)NEGF_STATIC_SCRATCH_BYTES))
+        return NEGF_ESTATICLIMIT;
+    if (info) NEGF_CUDA_CHECK(ctx, cudaMemsetAsync(info, 0, sizeof(int) * batch, ctx->stream));
+    return zinv_launch(ctx, b, (cplx*)A, stride, batch, zinv_static_ptr[ctx->device], info, 0, nullptr);
 }

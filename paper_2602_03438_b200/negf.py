@@ -20,7 +20,8 @@ lib = C.CDLL(LIB_PATH)
 
 PROF_GEMM, PROF_INVERSE, PROF_ELEMENTWISE, PROF_OBSERVABLES, PROF_FUSED = range(5)
 PROF_NAMES = ("gemm", "inverse", "elementwise", "observables", "fused")
-OK, EINVAL, ENOWORKSPACE, EUNSUPPORTED, ECUDA, ENOSTATE = 0, -1, -2, -3, -4, -5
+OK, EINVAL, ENOWORKSPACE, EUNSUPPORTED, ECUDA, ENOSTATE, ESTATICLIMIT = 0, -1, -2, -3, -4, -5, -6
+STATIC_SCRATCH_BYTES = 16 << 20
 SIGMA_NONE, SIGMA_SCALAR, SIGMA_BT = 0, 1, 2
 KEEP_SWEEP = 1
 OPT_GRAPH_LOOPS = 1
@@ -75,7 +76,8 @@ EXPORTS = ["negf_create", "negf_destroy", "negf_set_stream", "negf_workspace_byt
            "negf_profile_enable", "negf_profile_read", "negf_obc_decimate", "negf_obc_decimate_pair",
            "negf_rgf_retarded", "negf_rgf_lesser_greater", "negf_observables", "negf_energy_convolve", "negf_pipeline_device",
            "negf_pipeline_host_bytes",
-           "negf_pipeline_host", "negf_zgemm_batched", "negf_zinverse_batched", "negf_fp64_peak"]
+           "negf_pipeline_host", "negf_zgemm_batched", "negf_zinverse_batched", "negf_zinverse_batched_static",
+           "negf_fp64_peak"]
 
 _P = C.c_void_p
 lib.negf_create.argtypes = [C.POINTER(_P), C.c_int]
@@ -111,6 +113,7 @@ lib.negf_zgemm_batched.argtypes = [_P, C.c_int, C.c_int, C.c_int, C.c_int, C.c_i
                                    C.c_longlong, _P, C.c_int, C.c_longlong, c128, _P, _P, C.c_int,
                                    C.c_longlong, C.c_int]
 lib.negf_zinverse_batched.argtypes = [_P, C.c_int, _P, C.c_longlong, C.c_int, _P]
+lib.negf_zinverse_batched_static.argtypes = [_P, C.c_int, _P, C.c_longlong, C.c_int, _P]
 lib.negf_fp64_peak.argtypes = [_P, C.c_double, C.POINTER(C.c_double)]
 
 
@@ -287,6 +290,11 @@ class Context:
     def zinverse_batched(self, b, A, stride, batch, info=None):
         self._check(lib.negf_zinverse_batched(self._h, b, _ptr(A), stride, batch, _ptr(info)),
                     "negf_zinverse_batched")
+
+    def zinverse_batched_static(self, b, A, stride, batch, info=None):
+        """No-allocation variant: scratch in the library's static device array (include/negf.h)."""
+        self._check(lib.negf_zinverse_batched_static(self._h, b, _ptr(A), stride, batch, _ptr(info)),
+                    "negf_zinverse_batched_static")
 
     def fp64_peak(self, ms: float = 200.0) -> float:
         out = C.c_double()
