@@ -88,6 +88,101 @@ __device__ __forceinline__ void f_gemm(cplx* C, const cplx* A, const cplx* B, in
     __syncthreads();
 }
 
+// ---- a PHASE of independent products ---------------------------------------------------------------------------------
+// The chains are sequential, but most steps hold two to four products that do not depend on each other (g u and g l;
+// l g u, u g l, u g u, l g l).  A phase runs NP of them at once: FNT / NP threads per product, each thread a
+// register tile of RB x CB outputs (every operand element read from shared memory serves RB or CB multiply-adds,
+// and the RB * CB independent accumulators hide the DFMA latency), ONE block barrier for all of them.
+//   C = alpha * A * op(B) + beta * D + eye * I      op = identity, or conjugate transpose where bit j of OPBMASK is set
+struct Job { cplx* C; const cplx* A; const cplx* B; const cplx* D; cplx alpha, beta; double eye; };
+__device__ __forceinline__ Job job(cplx* C, const cplx* A, const cplx* B, cplx alpha, const cplx* D = nullptr,
+                                   cplx beta = cplx{0.0, 0.0}, double eye = 0.0) {
+    Job j; j.C = C; j.A = A; j.B = B; j.D = D; j.alpha = alpha; j.beta = beta; j.eye = eye; return j;
+}
+template <int FB, int RB, int CB, int OPB>
+__device__ __forceinline__ void f_tile_mac(cplx (&acc)[RB][CB], const cplx* A, const cplx* B, int b, int rl, int cl) {
+    constexpr int LD = Mat<FB>::LD, TR = FB / RB, TC = FB / CB;
+    constexpr int KS = (RB * CB <= 2) ? 2 : 1;          // second accumulator set while the tile alone cannot hide the latency
+    cplx acc2[RB][CB];
+#pragma unroll
+    for (int i = 0; i < RB; i++)
+#pragma unroll
+        for (int j = 0; j < CB; j++) { acc[i][j] = cmake(0.0, 0.0); acc2[i][j] = cmake(0.0, 0.0); }
+    int k = 0;
+    if (KS == 2) {
+#pragma unroll 2
+        for (; k + 1 < b; k += 2) {
+            cplx a0[RB], a1[RB], b0[CB], b1[CB];
+#pragma unroll
+            for (int i = 0; i < RB; i++) { a0[i] = A[(rl + i * TR) * LD + k]; a1[i] = A[(rl + i * TR) * LD + k + 1]; }
+#pragma unroll
+            for (int j = 0; j < CB; j++) {
+                b0[j] = OPB ? cconj(B[(cl + j * TC) * LD + k]) : B[k * LD + cl + j * TC];
+                b1[j] = OPB ? cconj(B[(cl + j * TC) * LD + k + 1]) : B[(k + 1) * LD + cl + j * TC];
+            }
+#pragma unroll
+            for (int i = 0; i < RB; i++)
+#pragma unroll
+                for (int j = 0; j < CB; j++) { cfma(acc[i][j], a0[i], b0[j]); cfma(acc2[i][j], a1[i], b1[j]); }
+        }
+    }
+#pragma unroll 2
+    for (; k < b; k++) {
+        cplx a0[RB], b0[CB];
+#pragma unroll
+        for (int i = 0; i < RB; i++) a0[i] = A[(rl + i * TR) * LD + k];
+#pragma unroll
+        for (int j = 0; j < CB; j++) b0[j] = OPB ? cconj(B[(cl + j * TC) * LD + k]) : B[k * LD + cl + j * TC];
+#pragma unroll
+        for (int i = 0; i < RB; i++)
+#pragma unroll
+            for (int j = 0; j < CB; j++) cfma(acc[i][j], a0[i], b0[j]);
+    }
+    if (KS == 2) {
+#pragma unroll
+        for (int i = 0; i < RB; i++)
+#pragma unroll
+            for (int j = 0; j < CB; j++) acc[i][j] = cadd(acc[i][j], acc2[i][j]);
+    }
+}
+// ALIAS: some C of the phase is an operand (A or B) of a product of the phase: one more barrier before the stores
+// (D == C of the same product needs none: an element is read by the thread that writes it).  Ends with a barrier.
+template <int FB, int NP, unsigned OPBMASK = 0u, bool ALIAS = false>
+__device__ __forceinline__ void f_phase(const Job (&J)[NP], int b) {
+    constexpr int LD = Mat<FB>::LD, TP = FNT / NP, OPT = FB * FB / TP;      // threads per product, outputs per thread
+    static_assert(NP == 1 || NP == 2 || NP == 4, "products per phase");
+    constexpr int RB = OPT >= 8 ? 4 : (OPT >= 2 ? 2 : 1), CB = OPT / RB;
+    constexpr int TR = FB / RB, TC = FB / CB;
+    const int jn = threadIdx.x / TP, tl = threadIdx.x % TP;               // warp-uniform product index (TP >= 64)
+    const int cl = tl % TC, rl = tl / TC;
+    Job me = J[0];
+#pragma unroll
+    for (int q = 1; q < NP; q++) if (jn == q) me = J[q];
+    cplx acc[RB][CB];
+    const bool live = me.C != nullptr;                                     // a null C is an empty slot of the phase
+    if (live) {
+        if ((OPBMASK >> jn) & 1u) f_tile_mac<FB, RB, CB, 1>(acc, me.A, me.B, b, rl, cl);
+        else                      f_tile_mac<FB, RB, CB, 0>(acc, me.A, me.B, b, rl, cl);
+    }
+    if (ALIAS) __syncthreads();
+    if (live)
+#pragma unroll
+    for (int i = 0; i < RB; i++) {
+        const int r = rl + i * TR;
+#pragma unroll
+        for (int j = 0; j < CB; j++) {
+            const int c = cl + j * TC;
+            if (r < b && c < b) {
+                cplx v = cmul(me.alpha, acc[i][j]);
+                if (me.D) cfma(v, me.beta, me.D[r * LD + c]);
+                if (r == c) v.x += me.eye;
+                me.C[r * LD + c] = v;
+            }
+        }
+    }
+    __syncthreads();
+}
+
 // element-wise helpers over the b x b block (all threads), each ends with a barrier
 template <int FB, class F>
 __device__ __forceinline__ void f_each(int b, F f) {
@@ -95,78 +190,127 @@ __device__ __forceinline__ void f_each(int b, F f) {
     for (int idx = threadIdx.x; idx < b * b; idx += FNT) { const int r = idx / b, c = idx % b; f(r, c, r * LD + c); }
     __syncthreads();
 }
-// In-place inverse of the b x b block M (shared memory) by warp 0: Gauss-Jordan with implicit threshold pivoting on
-// the leading 32 bits of |re|+|im| (lowest row among equals).  The block is treated as FB x FB padded with the
-// identity (padding rows pivot on padding columns).  `line` = FB complex of shared scratch.  Returns (to every
-// thread, after a barrier) 0 or the 1-based column of the first zero pivot through *sing_out (shared int).
-// One elimination step; (p, kmax) = pivot lane and key of the column in register 0 of x (found by the previous step).
-// The next column is updated FIRST and its pivot search (redux + ballot) is issued before the other columns'
-// updates, so that its latency hides under them; returns the next pivot in (p, kmax).
-template <int FB>
-__device__ __forceinline__ void f_search(const cplx v, bool used, int k, int b, int lane, int& p, unsigned& kmax) {
-    const bool elig = !used && ((lane < b) == (k < b)) && lane < FB;
-    unsigned key = 0u;
-    if (elig) key = (unsigned)((unsigned long long)__double_as_longlong(cabs1(v)) >> 32) + 1u;
-    kmax = __reduce_max_sync(FULLM, key);
-    const unsigned bal = __ballot_sync(FULLM, elig && key == kmax);
-    p = bal ? __ffs(bal) - 1 : 0;
-}
-template <int FB>
-__device__ __forceinline__ void f_step(const cplx (&x)[FB], cplx (&y)[FB], bool& used, int& piv_of_col, int k, int b, int lane,
-                                       cplx* line, int* sing, int& p, unsigned& kmax) {
-    if (kmax <= 1u && k < b && lane == 0 && *sing == 0) *sing = k + 1;
-    if (lane == p) {
-#pragma unroll
-        for (int c = 0; c < FB; c++) line[c] = x[c];
-    }
-    if (lane == k) piv_of_col = p;                   // lane k remembers the pivot row of column k
-    __syncwarp();
-    const cplx d = kmax <= 1u ? cmake(1.0, 0.0) : f_recip(line[0]);
-    const bool isp = lane == p;
-    const cplx m = cmul(x[0], d);
-    if (isp) used = true;
-    { cplx t = x[1]; if (isp) t = cmul(t, d); else cfms(t, m, line[1]); y[0] = t; }
-    int pn; unsigned kn;
-    f_search<FB>(y[0], used, k + 1, b, lane, pn, kn);
-#pragma unroll
-    for (int c = 2; c < FB; c++) { cplx t = x[c]; if (isp) t = cmul(t, d); else cfms(t, m, line[c]); y[c - 1] = t; }
-    y[FB - 1] = isp ? d : cneg(m);
-    p = pn; kmax = kn;
-    __syncwarp();
-}
 
-// In-place inverse of the b x b block M (shared memory; `src` = where the matrix is read from, may be M) by warp 0:
-// Gauss-Jordan with implicit threshold pivoting on the leading 32 bits of |re|+|im| (lowest row among equals).  The
-// block is treated as FB x FB padded with the identity (padding rows pivot on padding columns).  `line` = FB complex
-// of shared scratch, piv = 2 FB ints.  *sing (shared) = 0 or the 1-based column of the first zero pivot.
+// ---- in-CTA inverse on all eight warps -------------------------------------------------------------------------------
+// Gauss-Jordan with implicit threshold pivoting on the leading 32 bits of |re|+|im| (lowest row among equals).
+// lane = matrix row; warp w holds the columns w, w + 8, ... in registers (2 at FB = 16, 4 at FB = 32).  Step k belongs
+// to warp k % 8, whose register 0 is column k (a warp rotates its registers by one after each step it owned, so the
+// step body is one piece of static code in a rolled loop).  As soon as its column is up to date the owner publishes
+// it in shared memory, runs the pivot search as ONE redux on a (magnitude, row) key while EVERY lane computes the
+// reciprocal of its own candidate, and the winning lane alone writes reciprocal and row index (two buffers, one block
+// barrier per step); every warp then forms its rows' multipliers and updates its own columns, the pivot row's
+// entries coming from lane p of the same warp by shuffle.  The next owner updates its pivot column first and
+// publishes before the rest of its update.  Only the b real columns are eliminated (no padding steps).
+struct FusedScratch {
+    cplx col[2][32];           // pivot column of the step as it is before the step, double-buffered
+    cplx dinv[2];              // 1 / pivot of the step
+    double red[16];            // norm reduction
+    int piv[64];               // [k] pivot row of column k; [32 + r] its inverse
+    int pcur[2];               // pivot row of the step (+ 256 if the pivot was zero), double-buffered
+    int sing;                  // 0 or 1-based column of the first zero pivot
+    int pad;
+};
+constexpr int IW = FNT / 32;   // warps of the inverse
+#ifdef FUSED_PROBE
+__device__ long long g_stamp[64];
+#define STAMP(i, cond, dep) do { if ((dep) == 0x7fffabcdu) __trap(); if ((cond) && lane == 0) g_stamp[i] = clock64(); } while (0)
+#else
+#define STAMP(i, cond, dep) do {} while (0)
+#endif
+// Pivot search of one column over the lanes of a warp with ONE redux: key = the leading 27 bits of |re|+|im| (+1, so
+// that an eligible zero still beats an ineligible lane) above 5 bits of 31 - lane, i.e. the largest candidate up to a
+// relative 2^-15, lowest row among equals.  Exactly one lane has key == kmax (the pivot lane); kmax >> 5 <= 1: zero pivot.
+__device__ __forceinline__ unsigned f_pivot_key(const cplx v, bool elig, int lane) {
+    unsigned key = 0u;
+    if (elig) key = ((((unsigned)((unsigned long long)__double_as_longlong(cabs1(v)) >> 32)) >> 5) + 1u) << 5 | (unsigned)(31 - lane);
+    return key;
+}
+__device__ __forceinline__ cplx f_shfl(cplx v, int src) {
+    return cmake(__shfl_sync(FULLM, v.x, src), __shfl_sync(FULLM, v.y, src));
+}
+// In-place inverse of the b x b block M (shared memory; `src` = where the matrix is read from, may be M).
+// sh->sing = 0 or the 1-based column of the first zero pivot.  Ends with a block barrier (the caller's previous phase
+// ended with one).
+// A warp here issues about one instruction every three cycles (two warps per scheduler, everything dependent), so
+// the time of a step is the number of instructions between the barrier and the next owner's publication: the pivot
+// row is NOT scaled when it is chosen (its 1 / pivot is applied once, when the result is stored - later steps update
+// an unscaled pivot row with the same formula as any other row), the winner of the redux writes the pivot itself,
+// and all bookkeeping sits behind the publication in program order.
 template <int FB>
-__device__ __noinline__ void f_inverse(cplx* M, const cplx* src, int b, cplx* line, int* piv, int* sing) {
-    constexpr int LD = Mat<FB>::LD;
-    if (threadIdx.x == 0) *sing = 0;
-    __syncthreads();
-    if (threadIdx.x < 32) {
-        const int lane = threadIdx.x;
-        cplx x[FB], y[FB];
+__device__ __noinline__ void f_inverse(cplx* M, const cplx* src, int b, FusedScratch* sh) {
+    constexpr int LD = Mat<FB>::LD, CPW = FB / IW;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const bool inb = lane < b;
+    cplx x[CPW];
 #pragma unroll
-        for (int c = 0; c < FB; c++)
-            x[c] = (lane < b && c < b) ? src[lane * LD + c] : cmake(lane == c ? 1.0 : 0.0, 0.0);
-        bool used = false; int pk = 0, p; unsigned kmax;
-        f_search<FB>(x[0], used, 0, b, lane, p, kmax);
-#pragma unroll 1
-        for (int k = 0; k < FB; k += 2) {
-            f_step<FB>(x, y, used, pk, k, b, lane, line, sing, p, kmax);
-            f_step<FB>(y, x, used, pk, k + 1, b, lane, line, sing, p, kmax);
+    for (int j = 0; j < CPW; j++) {
+        const int c = w + IW * j;
+        x[j] = (inb && c < b) ? src[lane * LD + c] : cmake(0.0, 0.0);
+    }
+    bool unused = inb;
+    int pk = 0, singk = 0;
+    cplx drow = cmake(1.0, 0.0);                           // 1 / pivot of the step this row was the pivot row of
+    // the owner of a step publishes its column as soon as the column is up to date, then the pivot: the lane whose key
+    // wins the redux writes its own reciprocal and its index (nobody else needs to learn them before the barrier)
+    auto publish = [&](int buf) {
+        sh->col[buf][lane] = x[0];
+        const unsigned key = f_pivot_key(x[0], unused, lane);
+        const unsigned kmax = __reduce_max_sync(FULLM, key);
+        const cplx rc = f_recip(x[0]);
+        if (key == kmax) {
+            const bool zero = (kmax >> 5) <= 1u;
+            sh->dinv[buf] = zero ? cmake(1.0, 0.0) : rc;
+            sh->pcur[buf] = lane | (zero ? 256 : 0);
         }
-        // lane i holds B[i][j] = X[i][piv[j]], X = Pi A^-1 (zinv.cu): A^-1[pinv[i]][piv[j]] = B[i][j]
-        if (lane < FB) piv[lane] = pk;
+        // the publisher only ARRIVES at the step's barrier (named barrier 1 + buf, all FNT threads): the other warps
+        // are released now, not after the rest of the publisher's update; it reads its own publication back
         __syncwarp();
-        if (lane < FB) piv[FB + piv[lane]] = lane;                  // pinv
-        __syncwarp();
-        if (lane < b) {
-            const int dr = piv[FB + lane];
+        asm volatile("bar.arrive %0, %1;" ::"r"(1 + buf), "n"(FNT) : "memory");
+    };
+    auto step = [&](int k, int buf) {
+        if (w != (k & (IW - 1))) asm volatile("bar.sync %0, %1;" ::"r"(1 + buf), "n"(FNT) : "memory");
+        const int pw = sh->pcur[buf];
+        const cplx d = sh->dinv[buf];
+        const cplx mr = cmul(sh->col[buf][lane], d);       // multiplier of this row
+        const int pp = pw & 255;
+        const bool isp = lane == pp;
+        auto upd = [&](cplx t) {
+            const cplx pr = f_shfl(t, pp);
+            if (!isp) cfms(t, mr, pr);
+            return t;
+        };
+        if (isp) unused = false;
+        if (w == (k & (IW - 1))) {                         // owner: update and rotate, the finished column goes to the back
 #pragma unroll
-            for (int c = 0; c < FB; c++)
-                if (c < b) M[dr * LD + piv[c]] = x[c];
+            for (int j = 1; j < CPW; j++) x[j - 1] = upd(x[j]);
+            x[CPW - 1] = isp ? cmake(1.0, 0.0) : cneg(mr);
+        } else {
+            x[0] = upd(x[0]);
+            if (w == ((k + 1) & (IW - 1)) && k + 1 < b) publish(buf ^ 1);      // next owner, before the rest of its update
+#pragma unroll
+            for (int j = 1; j < CPW; j++) x[j] = upd(x[j]);
+        }
+        if (isp) drow = d;
+        if (lane == k) pk = pp;                            // lane k remembers the pivot row of column k
+        if ((pw & 256) && !singk) singk = k + 1;
+    };
+    if (w == 0) publish(0);
+#pragma unroll 1
+    for (int k = 0; k < b; k += 2) {
+        step(k, 0);
+        if (k + 1 < b) step(k + 1, 1);
+    }
+    // lane i holds B[i][j] = X[i][piv[j]], X = Pi A^-1 (zinv.cu): A^-1[pinv[i]][piv[j]] = B[i][j]
+    if (w == 0 && inb) { sh->piv[lane] = pk; sh->piv[32 + pk] = lane; }
+    if (threadIdx.x == 0) sh->sing = singk;
+    __syncthreads();
+    const int rot = w < b ? (b - w + IW - 1) / IW : 0;    // steps this warp owned = rotations of its registers
+    if (inb) {
+        const int dr = sh->piv[32 + lane];
+#pragma unroll
+        for (int j = 0; j < CPW; j++) {
+            const int c = w + IW * ((j + rot) % CPW);
+            if (c < b) M[dr * LD + sh->piv[c]] = cmul(x[j], drow);
         }
     }
     __syncthreads();
@@ -178,11 +322,9 @@ __device__ __noinline__ void f_inverse(cplx* M, const cplx* src, int b, cplx* li
 // step brings it to the LU level for two products of 0.2 us.
 template <int FB>
 __device__ __forceinline__ void f_refine(cplx* X, const cplx* A, cplx* tmp, int b) {
-    constexpr int LD = Mat<FB>::LD;
-    f_gemm<FB, 0, 0>(tmp, A, X, b, cmake(-1.0, 0.0), cmake(0.0, 0.0), nullptr);
-    for (int i = threadIdx.x; i < b; i += FNT) tmp[i * LD + i].x += 1.0;
-    __syncthreads();
-    f_gemm<FB, 0, 0, true>(X, X, tmp, b, cmake(1.0, 0.0), cmake(1.0, 0.0), X);
+    const cplx one = cmake(1.0, 0.0), mone = cmake(-1.0, 0.0);
+    { const Job J[1] = {job(tmp, A, X, mone, nullptr, cmake(0.0, 0.0), 1.0)}; f_phase<FB, 1>(J, b); }
+    { const Job J[1] = {job(X, X, tmp, one, X, one)}; f_phase<FB, 1, 0u, true>(J, b); }
 }
 
 // ---- global <-> shared block copies (b x b, global leading dimension b), each ends with a barrier ----------------
@@ -241,13 +383,15 @@ __device__ __forceinline__ void load_A(cplx* S, const FusedProblem& P, int e, in
     __syncthreads();
 }
 
-// ||U||_F + ||L||_F of two blocks: one block reduction in a fixed order; result to every thread
-template <int FB>
-__device__ __forceinline__ double f_norm_pair(const cplx* U, const cplx* L, int b, double* red) {
+// ||U||_F + ||L||_F of two blocks: one block reduction in a fixed order; result to every thread.  each(o) runs once
+// per element offset o before the element is read (the caller's element-wise updates ride along).
+template <int FB, class F>
+__device__ __forceinline__ double f_norm_pair(const cplx* U, const cplx* L, int b, double* red, F each) {
     constexpr int LD = Mat<FB>::LD;
     double a = 0.0, c = 0.0;
     for (int idx = threadIdx.x; idx < b * b; idx += FNT) {
         const int o = (idx / b) * LD + idx % b;
+        each(o);                                             // element-wise work folded into the same pass
         const cplx v = U[o], w = L[o];
         a += v.x * v.x + v.y * v.y; c += w.x * w.x + w.y * w.y;
     }
@@ -270,10 +414,8 @@ __global__ void __launch_bounds__(FNT, 1) fused_obc_kernel(const FusedObcArgs a)
     cplx* m = reinterpret_cast<cplx*>(fsm);
     cplx *a_s = m, *a_b = m + SZ, *g = m + 2 * SZ, *u = m + 3 * SZ, *l = m + 4 * SZ, *un = m + 5 * SZ, *ln = m + 6 * SZ,
          *gu = m + 7 * SZ, *gl = m + 8 * SZ, *t = m + 9 * SZ, *U0 = m + 10 * SZ, *L0 = m + 11 * SZ;
-    cplx* line = m + 12 * SZ;                                       // [FB]
-    double* red = reinterpret_cast<double*>(line + FB);            // [16]
-    int* piv = reinterpret_cast<int*>(red + 16);                   // [2 FB]
-    int* sing = piv + 2 * FB;
+    FusedScratch* sh = reinterpret_cast<FusedScratch*>(m + 12 * SZ);
+    double* red = sh->red;
     const int b = a.b, ne = a.ne;
     const int s = blockIdx.x / ne, e = blockIdx.x % ne;             // lead slot, energy
     const FusedLead& L = a.lead[s];
@@ -296,31 +438,30 @@ __global__ void __launch_bounds__(FNT, 1) fused_obc_kernel(const FusedObcArgs a)
     }
     __syncthreads();
     s2s<FB>(u, U0, b); s2s<FB>(l, L0, b);
-    const double ref = f_norm_pair<FB>(U0, L0, b, red);
+    const double ref = f_norm_pair<FB>(U0, L0, b, red, [](int) {});
     const cplx one = cmake(1.0, 0.0), mone = cmake(-1.0, 0.0), zero = cmake(0.0, 0.0);
     int iters = 0, done = 0, sing_code = 0;
     for (int it = 0; it < a.max_iter; it++) {
-        f_inverse<FB>(g, a_b, b, line, piv, sing);                  // g = a_b^-1
-        if (*sing && !sing_code) sing_code = it + 1;
+        f_inverse<FB>(g, a_b, b, sh);                               // g = a_b^-1
+        if (sh->sing && !sing_code) sing_code = it + 1;
         f_refine<FB>(g, a_b, gu, b);
-        f_gemm<FB, 0, 0>(gu, g, u, b, one, zero, nullptr);          // g u
-        f_gemm<FB, 0, 0>(gl, g, l, b, one, zero, nullptr);          // g l
-        f_gemm<FB, 0, 0>(t, l, gu, b, one, zero, nullptr);          // l g u
-        f_each<FB>(b, [&](int, int, int o) { a_s[o] = csub(a_s[o], t[o]); a_b[o] = csub(a_b[o], t[o]); });
-        f_gemm<FB, 0, 0>(a_b, u, gl, b, mone, one, a_b);            // a_b -= u g l
-        f_gemm<FB, 0, 0>(un, u, gu, b, mone, zero, nullptr);        // u <- -u g u
-        f_gemm<FB, 0, 0>(ln, l, gl, b, mone, zero, nullptr);        // l <- -l g l
+        { const Job J[2] = {job(gu, g, u, one), job(gl, g, l, one)}; f_phase<FB, 2>(J, b); }          // g u, g l
+        { const Job J[4] = {job(t, l, gu, one),                                                      // l g u
+                            job(a_b, u, gl, mone, a_b, one),                                         // a_b -= u g l
+                            job(un, u, gu, mone), job(ln, l, gl, mone)};                             // -u g u, -l g l
+          f_phase<FB, 4>(J, b); }
         cplx* sw = u; u = un; un = sw; sw = l; l = ln; ln = sw;
         iters = it + 1;
-        const double nrm = f_norm_pair<FB>(u, l, b, red);
+        // a_s -= l g u, a_b -= l g u and the norms of the new u, l in one pass
+        const double nrm = f_norm_pair<FB>(u, l, b, red, [&](int o) { a_s[o] = csub(a_s[o], t[o]); a_b[o] = csub(a_b[o], t[o]); });
         if (nrm <= a.tol * ref) { done = 1; break; }                // reading R3 (uniform over the CTA)
     }
     s2s<FB>(g, a_s, b);
-    f_inverse<FB>(a_s, a_s, b, line, piv, sing);                    // g_s = a_s^-1
-    if (*sing && !sing_code) sing_code = a.max_iter + 1;
+    f_inverse<FB>(a_s, a_s, b, sh);                                 // g_s = a_s^-1
+    if (sh->sing && !sing_code) sing_code = a.max_iter + 1;
     f_refine<FB>(a_s, g, gu, b);
-    f_gemm<FB, 0, 0>(gu, a_s, U0, b, one, zero, nullptr);
-    f_gemm<FB, 0, 0>(t, L0, gu, b, one, zero, nullptr);             // Sigma^R (exchanged storage: a_u g_s a_l for a right lead)
+    { const Job J[1] = {job(gu, a_s, U0, one)}; f_phase<FB, 1>(J, b); }
+    { const Job J[1] = {job(t, L0, gu, one)}; f_phase<FB, 1>(J, b); }   // Sigma^R (exchanged storage: a_u g_s a_l for a right lead)
     // outputs
     const double xx = (a.energy[e] - L.mu) / a.kT;
     double f;
@@ -343,65 +484,169 @@ __global__ void __launch_bounds__(FNT, 1) fused_obc_kernel(const FusedObcArgs a)
     }
 }
 
+// ---- bulk-copy (TMA) staging of the next step's Hamiltonian blocks --------------------------------------------------
+// The blocks of H are contiguous b x b x 16 B in global memory: one `cp.async.bulk` per block (the 1D form of the TMA
+// unit, SASS UBLKCP) brings the NEXT step's H_ii and H_{i-1,i} into a staging area of shared memory while the CTA
+// inverts the current block; completion is an mbarrier transaction count, so no thread waits on a global load.
+__device__ __forceinline__ unsigned s_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(s_u32(bar)), "r"(count) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(s_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, unsigned long long* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(s_u32(dst)), "l"(src), "r"(bytes), "r"(s_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+    unsigned ok;
+    do {
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(ok) : "r"(s_u32(bar)), "r"(parity) : "memory");
+    } while (!ok);
+}
+
+// Blocks of A = z S - H - Sigma^R of sweep step i for batch entry e, from the staged H blocks: M = A_ii and, for i > 0,
+// U = A_{i-1,i}, A1 = A_{i,i-1} (the dagger of the upper arrays of H and S, written transposed).  S and the dense
+// Sigma^R_S families, where present, are read from global memory here.  No trailing barrier.
+template <int FB>
+__device__ __forceinline__ void assemble_step(cplx* M, cplx* A1, cplx* U, const FusedProblem& P, int e, int i,
+                                              const cplx* st_hd, const cplx* st_hu) {
+    constexpr int LD = Mat<FB>::LD;
+    const int b = P.b, n = P.n;
+    const size_t bb = (size_t)b * b;
+    const cplx z = cmake(P.energy[e], P.eta);
+    const size_t kk = P.kidx ? (size_t)P.kidx[e] : 0;
+    const cplx* Sd = P.Sd ? P.Sd + (kk * n + i) * bb : nullptr;
+    const cplx* Su = (P.Su && i > 0) ? P.Su + (kk * (n - 1) + i - 1) * bb : nullptr;
+    const bool bt = P.sr_kind == NEGF_SIGMA_BT;
+    const cplx* sgd = bt ? P.sr_diag + ((size_t)e * n + i) * bb : nullptr;
+    const cplx* sgu = (bt && i > 0) ? P.sr_upper + ((size_t)e * (n - 1) + i - 1) * bb : nullptr;
+    const cplx* sgl = (bt && i > 0) ? P.sr_lower + ((size_t)e * (n - 1) + i - 1) * bb : nullptr;
+    const cplx* bnd = (i == 0 && P.sr_left) ? P.sr_left + (size_t)e * bb : nullptr;
+    const cplx* bnd2 = (i == n - 1 && P.sr_right) ? P.sr_right + (size_t)e * bb : nullptr;
+    const cplx sc = P.sr_kind == NEGF_SIGMA_SCALAR ? P.sr_scalar[e] : cmake(0.0, 0.0);
+    for (int idx = threadIdx.x; idx < b * b; idx += FNT) {
+        const int r = idx / b, c = idx % b;
+        cplx v = Sd ? cmul(z, Sd[idx]) : (r == c ? z : cmake(0.0, 0.0));
+        v = csub(v, st_hd[idx]);
+        if (sgd) v = csub(v, sgd[idx]);
+        if (bnd) v = csub(v, bnd[idx]);
+        if (bnd2) v = csub(v, bnd2[idx]);
+        if (r == c) v = csub(v, sc);
+        M[r * LD + c] = v;
+        if (i > 0) {
+            const cplx hu = st_hu[idx];
+            cplx up = cmake(0.0, 0.0), lo = cmake(0.0, 0.0);
+            if (Su) { const cplx su = Su[idx]; up = cmul(z, su); lo = cmul(z, cconj(su)); }
+            up = csub(up, hu); lo = csub(lo, cconj(hu));
+            if (sgu) up = csub(up, sgu[idx]);
+            if (sgl) lo = csub(lo, sgl[c * b + r]);
+            U[r * LD + c] = up;
+            A1[c * LD + r] = lo;
+        }
+    }
+}
+template <int FB>
+__device__ __forceinline__ void s2g_nb(cplx* g, const cplx* S, int b) {       // shared -> global, no barrier
+    constexpr int LD = Mat<FB>::LD;
+    if (g) for (int idx = threadIdx.x; idx < b * b; idx += FNT) g[idx] = S[(idx / b) * LD + idx % b];
+}
+
 // ---------------------------------------------------------------------------------------------------------------------
 // S1 + S3 + S4: retarded sweeps, one CTA per energy
 // ---------------------------------------------------------------------------------------------------------------------
+// Forward step i: {Y_{i-1} = A_{i,i-1} g_{i-1}, X_{i-1} = g_{i-1} A_{i-1,i}} as one phase, M = A_ii - Y_{i-1} A_{i-1,i},
+// g_i = M^-1; H_{i+1,i+1} and H_{i,i+1} arrive by bulk copy meanwhile.  Backward step i: {G_{i,i+1} = -X_i G_{i+1,i+1},
+// G_{i+1,i} = -G_{i+1,i+1} Y_i, corner column} as one phase, G_ii = g_i - G_{i,i+1} Y_i; g, X, Y of step i - 1 are
+// loaded into registers before the products and parked in shared memory after them.
 template <int FB>
 __global__ void __launch_bounds__(FNT, 1) fused_ret_kernel(const FusedProblem P, const FusedRetOut o) {
-    constexpr int SZ = Mat<FB>::SZ;
+    constexpr int SZ = Mat<FB>::SZ, LD = Mat<FB>::LD, EPT = (FB * FB + FNT - 1) / FNT;
     extern __shared__ __align__(16) unsigned char fsm[];
     cplx* m = reinterpret_cast<cplx*>(fsm);
-    cplx *M = m, *gp = m + SZ, *A1 = m + 2 * SZ, *Y = m + 3 * SZ, *X = m + 4 * SZ, *G = m + 5 * SZ, *T = m + 6 * SZ,
-         *col = m + 7 * SZ, *Gn = m + 8 * SZ;
-    cplx* line = m + 9 * SZ;
-    double* red = reinterpret_cast<double*>(line + FB);
-    int* piv = reinterpret_cast<int*>(red + 16);
-    int* sing = piv + 2 * FB;
+    cplx *M = m, *gp = m + SZ, *A1 = m + 2 * SZ, *U = m + 3 * SZ, *Y = m + 4 * SZ, *X = m + 5 * SZ, *G = m + 6 * SZ,
+         *Gn = m + 7 * SZ, *col = m + 8 * SZ, *col2 = m + 9 * SZ;
+    FusedScratch* sh = reinterpret_cast<FusedScratch*>(m + 10 * SZ);
+    cplx* st_hd = reinterpret_cast<cplx*>(sh + 1);
+    cplx* st_hu = st_hd + FB * FB;
+    unsigned long long* bar = reinterpret_cast<unsigned long long*>(st_hu + FB * FB);
     const int b = P.b, n = P.n, e = blockIdx.x;
     const size_t bb = (size_t)b * b;
+    const unsigned blk_bytes = (unsigned)(bb * sizeof(cplx));
+    const size_t kk = P.kidx ? (size_t)P.kidx[e] : 0;
+    const cplx* Hd = P.Hd + kk * n * bb;
+    const cplx* Hu = P.Hu ? P.Hu + kk * (n - 1) * bb : nullptr;
     cplx* Wg = o.g + (size_t)e * n * bb;
     cplx* WX = o.X + (size_t)e * (n - 1) * bb;
     cplx* WY = o.Y + (size_t)e * (n - 1) * bb;
-    const cplx one = cmake(1.0, 0.0), mone = cmake(-1.0, 0.0), zero = cmake(0.0, 0.0);
+    const cplx one = cmake(1.0, 0.0), mone = cmake(-1.0, 0.0);
     int code = 0;
+    if (threadIdx.x == 0) mbar_init(bar, 1);
+    __syncthreads();
+    if (threadIdx.x == 0) { mbar_expect_tx(bar, blk_bytes); bulk_g2s(st_hd, Hd, blk_bytes, bar); }
+    unsigned parity = 0;
     // S3: g_0 = A_00^-1; Y_{i-1} = A_{i,i-1} g_{i-1}; g_i = (A_ii - Y_{i-1} A_{i-1,i})^-1
     for (int i = 0; i < n; i++) {
-        load_A<FB>(M, P, e, i, 0);
-        if (i > 0) {
-            load_A<FB>(A1, P, e, i - 1, 2);                               // A_{i,i-1}
-            f_gemm<FB, 0, 0>(Y, A1, gp, b, one, zero, nullptr);
-            s2g<FB>(WY + (size_t)(i - 1) * bb, Y, b);
-            load_A<FB>(A1, P, e, i - 1, 1);                               // A_{i-1,i}
-            f_gemm<FB, 0, 0>(M, Y, A1, b, mone, one, M);
+        mbar_wait(bar, parity); parity ^= 1u;
+        assemble_step<FB>(M, A1, U, P, e, i, st_hd, st_hu);
+        __syncthreads();                                                  // blocks assembled, staging area free
+        if (threadIdx.x == 0 && i + 1 < n) {
+            mbar_expect_tx(bar, 2 * blk_bytes);
+            bulk_g2s(st_hd, Hd + (size_t)(i + 1) * bb, blk_bytes, bar);
+            bulk_g2s(st_hu, Hu + (size_t)i * bb, blk_bytes, bar);
         }
-        f_inverse<FB>(M, M, b, line, piv, sing);
-        if (*sing && !code) code = i + 1;
-        s2g<FB>(Wg + (size_t)i * bb, M, b);
+        if (i > 0) {
+            { const Job J[2] = {job(Y, A1, gp, one), job(X, gp, U, one)}; f_phase<FB, 2>(J, b); }
+            s2g_nb<FB>(WY + (size_t)(i - 1) * bb, Y, b);
+            s2g_nb<FB>(WX + (size_t)(i - 1) * bb, X, b);
+            { const Job J[1] = {job(M, Y, U, mone, M, one)}; f_phase<FB, 1>(J, b); }
+        }
+        f_inverse<FB>(M, M, b, sh);
+        if (sh->sing && !code) code = i + 1;
+        s2g_nb<FB>(Wg + (size_t)i * bb, M, b);
         cplx* sw = gp; gp = M; M = sw;                                    // g_{i} stays resident for the next step
     }
-    // S4: G_{n-1,n-1} = g_{n-1}; X_i = g_i A_{i,i+1}; G_{i,i+1} = -X_i G_{i+1,i+1}; G_{i+1,i} = -G_{i+1,i+1} Y_i;
+    // S4: G_{n-1,n-1} = g_{n-1}; G_{i,i+1} = -X_i G_{i+1,i+1}; G_{i+1,i} = -G_{i+1,i+1} Y_i;
     //     G_ii = g_i - G_{i,i+1} Y_i; corner column G_{i,n-1} = -X_i G_{i+1,n-1}
-    s2s<FB>(G, gp, b);
-    s2g<FB>(o.GR_diag + ((size_t)e * n + n - 1) * bb, G, b);
-    if (o.GR_corner) s2s<FB>(col, gp, b);
-    for (int i = n - 2; i >= 0; i--) {
-        g2s<FB>(gp, Wg + (size_t)i * bb, b);
-        load_A<FB>(A1, P, e, i, 1);
-        f_gemm<FB, 0, 0>(X, gp, A1, b, one, zero, nullptr);
-        s2g<FB>(WX + (size_t)i * bb, X, b);
-        g2s<FB>(Y, WY + (size_t)i * bb, b);
-        f_gemm<FB, 0, 0>(T, X, G, b, mone, zero, nullptr);                // G_{i,i+1}
-        s2g<FB>(o.GR_upper ? o.GR_upper + ((size_t)e * (n - 1) + i) * bb : nullptr, T, b);
-        if (o.GR_lower) {
-            f_gemm<FB, 0, 0>(Gn, G, Y, b, mone, zero, nullptr);           // G_{i+1,i}
-            s2g<FB>(o.GR_lower + ((size_t)e * (n - 1) + i) * bb, Gn, b);
+    cplx rg[EPT], rx[EPT], ry[EPT];
+    auto issue = [&](int i) {
+#pragma unroll
+        for (int q = 0; q < EPT; q++) {
+            const int idx = threadIdx.x + q * FNT;
+            if (idx < b * b) { rg[q] = Wg[(size_t)i * bb + idx]; rx[q] = WX[(size_t)i * bb + idx]; ry[q] = WY[(size_t)i * bb + idx]; }
         }
-        f_gemm<FB, 0, 0>(Gn, T, Y, b, mone, one, gp);                     // G_ii
-        s2g<FB>(o.GR_diag + ((size_t)e * n + i) * bb, Gn, b);
-        if (o.GR_corner) f_gemm<FB, 0, 0, true>(col, X, col, b, mone, zero, nullptr);
-        cplx* sw = G; G = Gn; Gn = sw;
+    };
+    if (n > 1) issue(n - 2);              // every thread reads back the elements it stored itself
+    for (int idx = threadIdx.x; idx < b * b; idx += FNT) {
+        const int oo = (idx / b) * LD + idx % b;
+        const cplx v = gp[oo];
+        G[oo] = v; col[oo] = v;
+        o.GR_diag[((size_t)e * n + n - 1) * bb + idx] = v;
     }
-    if (o.GR_corner) s2g<FB>(o.GR_corner + (size_t)e * bb, col, b);
+    cplx *T = A1, *Gl = U;
+    for (int i = n - 2; i >= 0; i--) {
+#pragma unroll
+        for (int q = 0; q < EPT; q++) {
+            const int idx = threadIdx.x + q * FNT;
+            if (idx < b * b) { const int oo = (idx / b) * LD + idx % b; gp[oo] = rg[q]; X[oo] = rx[q]; Y[oo] = ry[q]; }
+        }
+        __syncthreads();
+        if (i > 0) issue(i - 1);
+        { const Job J[4] = {job(T, X, G, mone), job(o.GR_lower ? Gl : nullptr, G, Y, mone),
+                            job(o.GR_corner ? col2 : nullptr, X, col, mone), job(nullptr, X, G, mone)};
+          f_phase<FB, 4>(J, b); }
+        s2g_nb<FB>(o.GR_upper ? o.GR_upper + ((size_t)e * (n - 1) + i) * bb : nullptr, T, b);
+        if (o.GR_lower) s2g_nb<FB>(o.GR_lower + ((size_t)e * (n - 1) + i) * bb, Gl, b);
+        { const Job J[1] = {job(Gn, T, Y, mone, gp, one)}; f_phase<FB, 1>(J, b); }
+        s2g_nb<FB>(o.GR_diag + ((size_t)e * n + i) * bb, Gn, b);
+        cplx* sw = G; G = Gn; Gn = sw; sw = col; col = col2; col2 = sw;
+    }
+    __syncthreads();
+    if (o.GR_corner) s2g_nb<FB>(o.GR_corner + (size_t)e * bb, col, b);
     if (threadIdx.x == 0 && code && o.info[e] == 0) o.info[e] = code;
 }
 
@@ -482,16 +727,19 @@ __global__ void __launch_bounds__(FNT, 1) fused_lg_kernel(const FusedProblem P, 
 }
 
 template <int FB> constexpr size_t fused_smem(int nmat) {
-    return (size_t)nmat * Mat<FB>::SZ * sizeof(cplx) + FB * sizeof(cplx) + 16 * sizeof(double) + (2 * FB + 4) * sizeof(int);
+    return (size_t)nmat * Mat<FB>::SZ * sizeof(cplx) + sizeof(FusedScratch);
 }
+
+// retarded kernel: 10 blocks + scratch + staging area of two raw H blocks + the mbarrier
+template <int FB> constexpr size_t fused_smem_ret() { return fused_smem<FB>(10) + 2 * (size_t)FB * FB * sizeof(cplx) + 16; }
 
 }  // namespace
 
 int fused_prepare(negf_ctx* ctx) {
     NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(fused_obc_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fused_smem<16>(12)));
     NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(fused_obc_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fused_smem<32>(12)));
-    NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(fused_ret_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fused_smem<16>(9)));
-    NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(fused_ret_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fused_smem<32>(9)));
+    NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(fused_ret_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fused_smem_ret<16>()));
+    NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(fused_ret_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fused_smem_ret<32>()));
     NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(fused_lg_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fused_smem<16>(11)));
     NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(fused_lg_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fused_smem<32>(11)));
     return NEGF_OK;
@@ -508,8 +756,8 @@ int fused_obc_launch(negf_ctx* ctx, const FusedObcArgs& a) {
 
 int fused_ret_launch(negf_ctx* ctx, const FusedProblem& P, const FusedRetOut& o) {
     ProfScope _ps(ctx, NEGF_PROF_FUSED);
-    if (P.b <= 16) fused_ret_kernel<16><<<P.ne, FNT, fused_smem<16>(9), ctx->stream>>>(P, o);
-    else           fused_ret_kernel<32><<<P.ne, FNT, fused_smem<32>(9), ctx->stream>>>(P, o);
+    if (P.b <= 16) fused_ret_kernel<16><<<P.ne, FNT, fused_smem_ret<16>(), ctx->stream>>>(P, o);
+    else           fused_ret_kernel<32><<<P.ne, FNT, fused_smem_ret<32>(), ctx->stream>>>(P, o);
     NEGF_LAUNCH_CHECK(ctx);
     return NEGF_OK;
 }
