@@ -11,12 +11,20 @@
 //   fused_ret_kernel   S1+S3+S4: one CTA per energy, forward and backward retarded sweeps, the blocks of
 //                      A assembled on the fly from H, S, z and Sigma^R; g_i, X_i, Y_i go to the workspace in the
 //                      one-sided layout of rgf.cu (retained sweep state), the selected G^R blocks to the outputs;
-//   fused_lg_kernel    S5+S6: one CTA per (energy, < or >), textbook forward recursion and the compact backward form.
-// Building blocks inside the CTA: complex b x b x b products on the FP64 pipe out of shared memory (DFMA; at these
-// sizes a product is 100-400 ns and latency-, not pipe-bound) and a warp-resident Gauss-Jordan inverse with
-// implicit threshold pivoting (lane = row, the row in registers, the column being eliminated always in register 0
-// with the row rotated by one register per step - the scheme of zinv_rows.cu for one warp).
+//   fused_lg_kernel    S5+S6: one CTA per (energy, < or >), the hoisted forward recursion and the compact backward form
+//                      as a software pipeline of two phases per step.
+// Building blocks inside the CTA (all measured in-kernel with clock64, b = 16): a warp of these kernels issues about
+// one instruction every three cycles (two warps per scheduler, dependent code), so every block is built for a short
+// instruction path, not for pipe throughput:
+//   f_phase    two to four INDEPENDENT complex products of a chain step as 8 x 8 DMMA.8x8x4 tiles spread over the
+//              eight warps, one block barrier (a lone 16^3 product ~1000 cycles, four of them ~2000);
+//   f_inverse  Gauss-Jordan with implicit pivoting on all eight warps (lane = row, columns cyclic over the warps),
+//              ~450 cycles per column (first version, one warp: ~680);
+//   staging    the next step's H blocks by cp.async.bulk (TMA, completion on an mbarrier) in the retarded sweep,
+//              global -> registers -> shared memory one step ahead everywhere else.
 // Same arithmetic definitions as the batched path (obc.cu, rgf.cu); results agree to rounding, not to the bit.
+#include <type_traits>
+
 #include "common.cuh"
 #include "fused_small.cuh"
 
@@ -38,156 +46,106 @@ __device__ __forceinline__ cplx f_recip(cplx a) {
     return cmake(a.x * r, -a.y * r);
 }
 
-// C = alpha * op(A) * op(B) + beta * D  (b x b, all in shared memory, leading dimension FB + 1; D may be C or
-// null).  Thread t owns column c = t % FB of the rows r = t / FB + j * (FNT / FB).  Two accumulator sets (even / odd
-// k) halve the dependent DFMA chain, which is what a product costs at these sizes.  ALIAS: C is also an operand
-// (one more barrier between the last read and the first write).  Ends with a block barrier.
-template <int FB, int OPA, int OPB, bool ALIAS = false>
-__device__ __forceinline__ void f_gemm(cplx* C, const cplx* A, const cplx* B, int b, cplx alpha, cplx beta, const cplx* D) {
-    constexpr int LD = Mat<FB>::LD, RS = FNT / FB, NR = FB / RS;
-    const int c = threadIdx.x % FB, r0 = threadIdx.x / FB;
-    cplx acc[NR], acc2[NR];
-#pragma unroll
-    for (int j = 0; j < NR; j++) { acc[j] = cmake(0.0, 0.0); acc2[j] = cmake(0.0, 0.0); }
-    if (c < b) {
-        int k = 0;
-#pragma unroll 2
-        for (; k + 1 < b; k += 2) {
-            const cplx b0 = OPB ? cconj(B[c * LD + k]) : B[k * LD + c];
-            const cplx b1 = OPB ? cconj(B[c * LD + k + 1]) : B[(k + 1) * LD + c];
-#pragma unroll
-            for (int j = 0; j < NR; j++) {
-                const int r = r0 + j * RS;
-                const cplx a0 = OPA ? cconj(A[k * LD + r]) : A[r * LD + k];
-                const cplx a1 = OPA ? cconj(A[(k + 1) * LD + r]) : A[r * LD + k + 1];
-                cfma(acc[j], a0, b0);
-                cfma(acc2[j], a1, b1);
-            }
-        }
-        if (k < b) {
-            const cplx b0 = OPB ? cconj(B[c * LD + k]) : B[k * LD + c];
-#pragma unroll
-            for (int j = 0; j < NR; j++) {
-                const int r = r0 + j * RS;
-                cfma(acc[j], OPA ? cconj(A[k * LD + r]) : A[r * LD + k], b0);
-            }
-        }
-    }
-    if (ALIAS) __syncthreads();
-    if (c < b) {
-#pragma unroll
-        for (int j = 0; j < NR; j++) {
-            const int r = r0 + j * RS;
-            if (r < b) {
-                cplx v = cmul(alpha, cadd(acc[j], acc2[j]));
-                if (D) cfma(v, beta, D[r * LD + c]);
-                C[r * LD + c] = v;
-            }
-        }
-    }
-    __syncthreads();
-}
-
-// ---- a PHASE of independent products ---------------------------------------------------------------------------------
+// ---- a PHASE of independent products on the FP64 tensor pipe ---------------------------------------------------------
 // The chains are sequential, but most steps hold two to four products that do not depend on each other (g u and g l;
-// l g u, u g l, u g u, l g l).  A phase runs NP of them at once: FNT / NP threads per product, each thread a
-// register tile of RB x CB outputs (every operand element read from shared memory serves RB or CB multiply-adds,
-// and the RB * CB independent accumulators hide the DFMA latency), ONE block barrier for all of them.
-//   C = alpha * A * op(B) + beta * D + eye * I      op = identity, or conjugate transpose where bit j of OPBMASK is set
-struct Job { cplx* C; const cplx* A; const cplx* B; const cplx* D; cplx alpha, beta; double eye; };
-__device__ __forceinline__ Job job(cplx* C, const cplx* A, const cplx* B, cplx alpha, const cplx* D = nullptr,
-                                   cplx beta = cplx{0.0, 0.0}, double eye = 0.0) {
+// l g u, u g l, u g u, l g l).  A phase runs NP of them at once with ONE block barrier.  A warp here issues about one
+// instruction every three cycles (two warps per scheduler, dependent code), so what a product costs is its
+// instruction count: on the plain FP64 pipe a 16 x 16 x 16 complex product was ~250 instructions per thread
+// (1050 cycles); as DMMA.8x8x4 it is 8 x 8 output tiles of 4 k-steps x (2 LDS.128 + 4 DMMA): the interleaved
+// (re, im) element one lane loads IS its A (or B) fragment of both the real and the imaginary operand, and the four
+// accumulators rr, ii, ri, ir (re = rr - ii, im = ri + ir; conjugated B: re = rr + ii, im = ir - ri) are independent
+// chains.  Work units = (product, tile) spread over the eight warps; a lone 16 x 16 product splits every tile into its
+// real and imaginary half (two warps per tile).  k beyond b is loaded as zero; rows / columns beyond b are not stored.
+//   C = alpha * A * op(B) + beta * D + eye * I      alpha, beta real; op = identity, or conjugate transpose where bit
+//   j of OPBMASK is set; a null C is an empty slot of the phase
+struct Job { cplx* C; const cplx* A; const cplx* B; const cplx* D; double alpha, beta, eye; };
+__device__ __forceinline__ Job job(cplx* C, const cplx* A, const cplx* B, double alpha, const cplx* D = nullptr,
+                                   double beta = 0.0, double eye = 0.0) {
     Job j; j.C = C; j.A = A; j.B = B; j.D = D; j.alpha = alpha; j.beta = beta; j.eye = eye; return j;
 }
-template <int FB, int RB, int CB, int OPB>
-__device__ __forceinline__ void f_tile_mac(cplx (&acc)[RB][CB], const cplx* A, const cplx* B, int b, int rl, int cl) {
-    constexpr int LD = Mat<FB>::LD, TR = FB / RB, TC = FB / CB;
-    constexpr int KS = (RB * CB <= 2) ? 2 : 1;          // second accumulator set while the tile alone cannot hide the latency
-    cplx acc2[RB][CB];
-#pragma unroll
-    for (int i = 0; i < RB; i++)
-#pragma unroll
-        for (int j = 0; j < CB; j++) { acc[i][j] = cmake(0.0, 0.0); acc2[i][j] = cmake(0.0, 0.0); }
-    int k = 0;
-    if (KS == 2) {
+__device__ __forceinline__ void dmma884(double (&c)[2], double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};"
+                 : "+d"(c[0]), "+d"(c[1]) : "d"(a), "d"(b));
+}
+template <int Q, int N, class F>
+__device__ __forceinline__ void f_static_for(F&& f) {
+    if constexpr (Q < N) { f(std::integral_constant<int, Q>{}); f_static_for<Q + 1, N>(f); }
+}
+// One work unit: the 8 x 8 output tile (r0, c0) of one product; part (SPLIT only): 0 real half, 1 imaginary half.
+template <int FB, bool OPB, bool SPLIT>
+__device__ __forceinline__ void f_tile_mma(double (&acc)[4][2], const Job& me, int r0, int c0, int part, int b, int g, int t) {
+    constexpr int LD = Mat<FB>::LD;
+    const cplx* ap = me.A + (r0 + g) * LD + t;
+    const cplx* bp = OPB ? me.B + (c0 + g) * LD + t : me.B + t * LD + c0 + g;
+    constexpr int bstep = OPB ? 4 : 4 * LD;
+    const int ksteps = (b + 3) >> 2;
 #pragma unroll 2
-        for (; k + 1 < b; k += 2) {
-            cplx a0[RB], a1[RB], b0[CB], b1[CB];
+    for (int ks = 0; ks < ksteps; ks++) {
+        const bool in = 4 * ks + t < b;
+        const cplx a = in ? ap[4 * ks] : cmake(0.0, 0.0);
+        const cplx bv = in ? bp[ks * bstep] : cmake(0.0, 0.0);
+        if (!SPLIT || part == 0) { dmma884(acc[0], a.x, bv.x); dmma884(acc[1], a.y, bv.y); }
+        if (!SPLIT || part == 1) { dmma884(acc[2], a.x, bv.y); dmma884(acc[3], a.y, bv.x); }
+    }
+}
+template <int FB, bool OPB, bool SPLIT>
+__device__ __forceinline__ void f_tile_store(const double (&acc)[4][2], const Job& me, int r0, int c0, int part, int b, int g, int t) {
+    constexpr int LD = Mat<FB>::LD;
+    constexpr double cs = OPB ? -1.0 : 1.0;
+    const int r = r0 + g;
+    if (r >= b) return;
 #pragma unroll
-            for (int i = 0; i < RB; i++) { a0[i] = A[(rl + i * TR) * LD + k]; a1[i] = A[(rl + i * TR) * LD + k + 1]; }
-#pragma unroll
-            for (int j = 0; j < CB; j++) {
-                b0[j] = OPB ? cconj(B[(cl + j * TC) * LD + k]) : B[k * LD + cl + j * TC];
-                b1[j] = OPB ? cconj(B[(cl + j * TC) * LD + k + 1]) : B[(k + 1) * LD + cl + j * TC];
-            }
-#pragma unroll
-            for (int i = 0; i < RB; i++)
-#pragma unroll
-                for (int j = 0; j < CB; j++) { cfma(acc[i][j], a0[i], b0[j]); cfma(acc2[i][j], a1[i], b1[j]); }
+    for (int h = 0; h < 2; h++) {
+        const int c = c0 + 2 * t + h;
+        if (c < b) {
+            double re = me.alpha * (acc[0][h] - cs * acc[1][h]);
+            double im = me.alpha * (cs * acc[2][h] + acc[3][h]);
+            if (me.D) { const cplx dv = me.D[r * LD + c]; re = fma(me.beta, dv.x, re); im = fma(me.beta, dv.y, im); }
+            if (me.eye != 0.0 && r == c) re += me.eye;
+            if (!SPLIT) me.C[r * LD + c] = cmake(re, im);
+            else if (part == 0) me.C[r * LD + c].x = re;
+            else me.C[r * LD + c].y = im;
         }
-    }
-#pragma unroll 2
-    for (; k < b; k++) {
-        cplx a0[RB], b0[CB];
-#pragma unroll
-        for (int i = 0; i < RB; i++) a0[i] = A[(rl + i * TR) * LD + k];
-#pragma unroll
-        for (int j = 0; j < CB; j++) b0[j] = OPB ? cconj(B[(cl + j * TC) * LD + k]) : B[k * LD + cl + j * TC];
-#pragma unroll
-        for (int i = 0; i < RB; i++)
-#pragma unroll
-            for (int j = 0; j < CB; j++) cfma(acc[i][j], a0[i], b0[j]);
-    }
-    if (KS == 2) {
-#pragma unroll
-        for (int i = 0; i < RB; i++)
-#pragma unroll
-            for (int j = 0; j < CB; j++) acc[i][j] = cadd(acc[i][j], acc2[i][j]);
     }
 }
 // ALIAS: some C of the phase is an operand (A or B) of a product of the phase: one more barrier before the stores
 // (D == C of the same product needs none: an element is read by the thread that writes it).  Ends with a barrier.
+// The product a unit belongs to is resolved by a warp-uniform branch per product, so that alpha, beta, eye and a
+// null D fold into the code of that branch.
 template <int FB, int NP, unsigned OPBMASK = 0u, bool ALIAS = false>
 __device__ __forceinline__ void f_phase(const Job (&J)[NP], int b) {
-    constexpr int LD = Mat<FB>::LD, TP = FNT / NP, OPT = FB * FB / TP;      // threads per product, outputs per thread
+    constexpr int TD = FB / 8, T = TD * TD;                                // 8 x 8 tiles per product
+    constexpr bool SPLIT = NP * T < FNT / 32;                              // real / imaginary halves on different warps
+    constexpr int PARTS = SPLIT ? 2 : 1, U = NP * T * PARTS, NW = FNT / 32, UPW = (U + NW - 1) / NW;
     static_assert(NP == 1 || NP == 2 || NP == 4, "products per phase");
-    constexpr int RB = OPT >= 8 ? 4 : (OPT >= 2 ? 2 : 1), CB = OPT / RB;
-    constexpr int TR = FB / RB, TC = FB / CB;
-    const int jn = threadIdx.x / TP, tl = threadIdx.x % TP;               // warp-uniform product index (TP >= 64)
-    const int cl = tl % TC, rl = tl / TC;
-    Job me = J[0];
+    static_assert(U % NW == 0 && (T * PARTS) % NW == 0 || NW % (T * PARTS) == 0, "units per warp");
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, g = lane >> 2, t = lane & 3;
+    double acc[UPW][4][2];
 #pragma unroll
-    for (int q = 1; q < NP; q++) if (jn == q) me = J[q];
-    cplx acc[RB][CB];
-    const bool live = me.C != nullptr;                                     // a null C is an empty slot of the phase
-    if (live) {
-        if ((OPBMASK >> jn) & 1u) f_tile_mac<FB, RB, CB, 1>(acc, me.A, me.B, b, rl, cl);
-        else                      f_tile_mac<FB, RB, CB, 0>(acc, me.A, me.B, b, rl, cl);
-    }
-    if (ALIAS) __syncthreads();
-    if (live)
+    for (int i = 0; i < UPW; i++) {
 #pragma unroll
-    for (int i = 0; i < RB; i++) {
-        const int r = rl + i * TR;
-#pragma unroll
-        for (int j = 0; j < CB; j++) {
-            const int c = cl + j * TC;
-            if (r < b && c < b) {
-                cplx v = cmul(me.alpha, acc[i][j]);
-                if (me.D) cfma(v, me.beta, me.D[r * LD + c]);
-                if (r == c) v.x += me.eye;
-                me.C[r * LD + c] = v;
-            }
+        for (int q = 0; q < 4; q++) { acc[i][q][0] = 0.0; acc[i][q][1] = 0.0; }
+        const int u = w + NW * i, jn = u / (T * PARTS), tile = (u / PARTS) % T, part = u % PARTS;
+        const int r0 = (tile / TD) * 8, c0 = (tile % TD) * 8;
+        if (r0 < b && c0 < b) {
+            f_static_for<0, NP>([&](auto qc) {
+                constexpr int q = decltype(qc)::value;
+                if (jn == q && J[q].C != nullptr) f_tile_mma<FB, ((OPBMASK >> q) & 1u) != 0u, SPLIT>(acc[i], J[q], r0, c0, part, b, g, t);
+            });
         }
     }
-    __syncthreads();
-}
-
-// element-wise helpers over the b x b block (all threads), each ends with a barrier
-template <int FB, class F>
-__device__ __forceinline__ void f_each(int b, F f) {
-    constexpr int LD = Mat<FB>::LD;
-    for (int idx = threadIdx.x; idx < b * b; idx += FNT) { const int r = idx / b, c = idx % b; f(r, c, r * LD + c); }
+    if (ALIAS) __syncthreads();
+#pragma unroll
+    for (int i = 0; i < UPW; i++) {
+        const int u = w + NW * i, jn = u / (T * PARTS), tile = (u / PARTS) % T, part = u % PARTS;
+        const int r0 = (tile / TD) * 8, c0 = (tile % TD) * 8;
+        if (r0 < b && c0 < b) {
+            f_static_for<0, NP>([&](auto qc) {
+                constexpr int q = decltype(qc)::value;
+                if (jn == q && J[q].C != nullptr) f_tile_store<FB, ((OPBMASK >> q) & 1u) != 0u, SPLIT>(acc[i], J[q], r0, c0, part, b, g, t);
+            });
+        }
+    }
     __syncthreads();
 }
 
@@ -211,12 +169,6 @@ struct FusedScratch {
     int pad;
 };
 constexpr int IW = FNT / 32;   // warps of the inverse
-#ifdef FUSED_PROBE
-__device__ long long g_stamp[64];
-#define STAMP(i, cond, dep) do { if ((dep) == 0x7fffabcdu) __trap(); if ((cond) && lane == 0) g_stamp[i] = clock64(); } while (0)
-#else
-#define STAMP(i, cond, dep) do {} while (0)
-#endif
 // Pivot search of one column over the lanes of a warp with ONE redux: key = the leading 27 bits of |re|+|im| (+1, so
 // that an eligible zero still beats an ineligible lane) above 5 bits of 31 - lane, i.e. the largest candidate up to a
 // relative 2^-15, lowest row among equals.  Exactly one lane has key == kmax (the pivot lane); kmax >> 5 <= 1: zero pivot.
@@ -322,64 +274,15 @@ __device__ __noinline__ void f_inverse(cplx* M, const cplx* src, int b, FusedScr
 // step brings it to the LU level for two products of 0.2 us.
 template <int FB>
 __device__ __forceinline__ void f_refine(cplx* X, const cplx* A, cplx* tmp, int b) {
-    const cplx one = cmake(1.0, 0.0), mone = cmake(-1.0, 0.0);
-    { const Job J[1] = {job(tmp, A, X, mone, nullptr, cmake(0.0, 0.0), 1.0)}; f_phase<FB, 1>(J, b); }
-    { const Job J[1] = {job(X, X, tmp, one, X, one)}; f_phase<FB, 1, 0u, true>(J, b); }
+    { const Job J[1] = {job(tmp, A, X, -1.0, nullptr, 0.0, 1.0)}; f_phase<FB, 1>(J, b); }
+    { const Job J[1] = {job(X, X, tmp, 1.0, X, 1.0)}; f_phase<FB, 1, 0u, true>(J, b); }
 }
 
-// ---- global <-> shared block copies (b x b, global leading dimension b), each ends with a barrier ----------------
-template <int FB>
-__device__ __forceinline__ void g2s(cplx* S, const cplx* g, int b) {
-    constexpr int LD = Mat<FB>::LD;
-    for (int idx = threadIdx.x; idx < b * b; idx += FNT) S[(idx / b) * LD + idx % b] = g[idx];
-    __syncthreads();
-}
-template <int FB>
-__device__ __forceinline__ void s2g(cplx* g, const cplx* S, int b) {
-    constexpr int LD = Mat<FB>::LD;
-    if (g) for (int idx = threadIdx.x; idx < b * b; idx += FNT) g[idx] = S[(idx / b) * LD + idx % b];
-    __syncthreads();
-}
+// ---- shared -> shared block copy, ends with a barrier --------------------------------------------------------------
 template <int FB>
 __device__ __forceinline__ void s2s(cplx* D, const cplx* S, int b) {
     constexpr int LD = Mat<FB>::LD;
     for (int idx = threadIdx.x; idx < b * b; idx += FNT) { const int o = (idx / b) * LD + idx % b; D[o] = S[o]; }
-    __syncthreads();
-}
-
-// ---- blocks of A = z S - H - Sigma^R for batch entry e, assembled into shared memory --------------
-// which: 0 diagonal block i, 1 upper block A_{i,i+1}, 2 lower block A_{i+1,i}
-template <int FB>
-__device__ __forceinline__ void load_A(cplx* S, const FusedProblem& P, int e, int i, int which) {
-    constexpr int LD = Mat<FB>::LD;
-    const int b = P.b, n = P.n;
-    const size_t bb = (size_t)b * b;
-    const cplx z = cmake(P.energy[e], P.eta);
-    const size_t kk = P.kidx ? (size_t)P.kidx[e] : 0;
-    const cplx* H = which == 0 ? P.Hd + (kk * n + i) * bb : P.Hu + (kk * (n - 1) + i) * bb;
-    const cplx* Sm = which == 0 ? (P.Sd ? P.Sd + (kk * n + i) * bb : nullptr) : (P.Su ? P.Su + (kk * (n - 1) + i) * bb : nullptr);
-    const cplx* sg = nullptr;                       // dense Sigma^R_S block of this entry
-    if (P.sr_kind == NEGF_SIGMA_BT)
-        sg = which == 0 ? P.sr_diag + ((size_t)e * n + i) * bb
-                        : (which == 1 ? P.sr_upper : P.sr_lower) + ((size_t)e * (n - 1) + i) * bb;
-    const cplx* bnd = nullptr;
-    if (which == 0 && i == 0 && P.sr_left) bnd = P.sr_left + (size_t)e * bb;
-    const cplx* bnd2 = (which == 0 && i == n - 1 && P.sr_right) ? P.sr_right + (size_t)e * bb : nullptr;
-    const cplx sc = (which == 0 && P.sr_kind == NEGF_SIGMA_SCALAR) ? P.sr_scalar[e] : cmake(0.0, 0.0);
-    for (int idx = threadIdx.x; idx < b * b; idx += FNT) {
-        const int r = idx / b, c = idx % b;
-        const int src = which == 2 ? c * b + r : idx;            // lower block = dagger of the upper arrays of H and S
-        cplx h = H[src], v;
-        if (which == 2) h = cconj(h);
-        if (Sm) { cplx s = Sm[src]; if (which == 2) s = cconj(s); v = cmul(z, s); }
-        else v = (which == 0 && r == c) ? z : cmake(0.0, 0.0);
-        v = csub(v, h);
-        if (sg) v = csub(v, sg[idx]);
-        if (bnd) v = csub(v, bnd[idx]);
-        if (bnd2) v = csub(v, bnd2[idx]);
-        if (r == c) v = csub(v, sc);
-        S[r * LD + c] = v;
-    }
     __syncthreads();
 }
 
@@ -439,16 +342,15 @@ __global__ void __launch_bounds__(FNT, 1) fused_obc_kernel(const FusedObcArgs a)
     __syncthreads();
     s2s<FB>(u, U0, b); s2s<FB>(l, L0, b);
     const double ref = f_norm_pair<FB>(U0, L0, b, red, [](int) {});
-    const cplx one = cmake(1.0, 0.0), mone = cmake(-1.0, 0.0), zero = cmake(0.0, 0.0);
     int iters = 0, done = 0, sing_code = 0;
     for (int it = 0; it < a.max_iter; it++) {
         f_inverse<FB>(g, a_b, b, sh);                               // g = a_b^-1
         if (sh->sing && !sing_code) sing_code = it + 1;
         f_refine<FB>(g, a_b, gu, b);
-        { const Job J[2] = {job(gu, g, u, one), job(gl, g, l, one)}; f_phase<FB, 2>(J, b); }          // g u, g l
-        { const Job J[4] = {job(t, l, gu, one),                                                      // l g u
-                            job(a_b, u, gl, mone, a_b, one),                                         // a_b -= u g l
-                            job(un, u, gu, mone), job(ln, l, gl, mone)};                             // -u g u, -l g l
+        { const Job J[2] = {job(gu, g, u, 1.0), job(gl, g, l, 1.0)}; f_phase<FB, 2>(J, b); }          // g u, g l
+        { const Job J[4] = {job(t, l, gu, 1.0),                                                      // l g u
+                            job(a_b, u, gl, -1.0, a_b, 1.0),                                         // a_b -= u g l
+                            job(un, u, gu, -1.0), job(ln, l, gl, -1.0)};                             // -u g u, -l g l
           f_phase<FB, 4>(J, b); }
         cplx* sw = u; u = un; un = sw; sw = l; l = ln; ln = sw;
         iters = it + 1;
@@ -460,8 +362,8 @@ __global__ void __launch_bounds__(FNT, 1) fused_obc_kernel(const FusedObcArgs a)
     f_inverse<FB>(a_s, a_s, b, sh);                                 // g_s = a_s^-1
     if (sh->sing && !sing_code) sing_code = a.max_iter + 1;
     f_refine<FB>(a_s, g, gu, b);
-    { const Job J[1] = {job(gu, a_s, U0, one)}; f_phase<FB, 1>(J, b); }
-    { const Job J[1] = {job(t, L0, gu, one)}; f_phase<FB, 1>(J, b); }   // Sigma^R (exchanged storage: a_u g_s a_l for a right lead)
+    { const Job J[1] = {job(gu, a_s, U0, 1.0)}; f_phase<FB, 1>(J, b); }
+    { const Job J[1] = {job(t, L0, gu, 1.0)}; f_phase<FB, 1>(J, b); }   // Sigma^R (exchanged storage: a_u g_s a_l for a right lead)
     // outputs
     const double xx = (a.energy[e] - L.mu) / a.kT;
     double f;
@@ -583,7 +485,6 @@ __global__ void __launch_bounds__(FNT, 1) fused_ret_kernel(const FusedProblem P,
     cplx* Wg = o.g + (size_t)e * n * bb;
     cplx* WX = o.X + (size_t)e * (n - 1) * bb;
     cplx* WY = o.Y + (size_t)e * (n - 1) * bb;
-    const cplx one = cmake(1.0, 0.0), mone = cmake(-1.0, 0.0);
     int code = 0;
     if (threadIdx.x == 0) mbar_init(bar, 1);
     __syncthreads();
@@ -600,10 +501,10 @@ __global__ void __launch_bounds__(FNT, 1) fused_ret_kernel(const FusedProblem P,
             bulk_g2s(st_hu, Hu + (size_t)i * bb, blk_bytes, bar);
         }
         if (i > 0) {
-            { const Job J[2] = {job(Y, A1, gp, one), job(X, gp, U, one)}; f_phase<FB, 2>(J, b); }
+            { const Job J[2] = {job(Y, A1, gp, 1.0), job(X, gp, U, 1.0)}; f_phase<FB, 2>(J, b); }
             s2g_nb<FB>(WY + (size_t)(i - 1) * bb, Y, b);
             s2g_nb<FB>(WX + (size_t)(i - 1) * bb, X, b);
-            { const Job J[1] = {job(M, Y, U, mone, M, one)}; f_phase<FB, 1>(J, b); }
+            { const Job J[1] = {job(M, Y, U, -1.0, M, 1.0)}; f_phase<FB, 1>(J, b); }
         }
         f_inverse<FB>(M, M, b, sh);
         if (sh->sing && !code) code = i + 1;
@@ -636,12 +537,12 @@ __global__ void __launch_bounds__(FNT, 1) fused_ret_kernel(const FusedProblem P,
         }
         __syncthreads();
         if (i > 0) issue(i - 1);
-        { const Job J[4] = {job(T, X, G, mone), job(o.GR_lower ? Gl : nullptr, G, Y, mone),
-                            job(o.GR_corner ? col2 : nullptr, X, col, mone), job(nullptr, X, G, mone)};
+        { const Job J[4] = {job(T, X, G, -1.0), job(o.GR_lower ? Gl : nullptr, G, Y, -1.0),
+                            job(o.GR_corner ? col2 : nullptr, X, col, -1.0), job(nullptr, X, G, -1.0)};
           f_phase<FB, 4>(J, b); }
         s2g_nb<FB>(o.GR_upper ? o.GR_upper + ((size_t)e * (n - 1) + i) * bb : nullptr, T, b);
         if (o.GR_lower) s2g_nb<FB>(o.GR_lower + ((size_t)e * (n - 1) + i) * bb, Gl, b);
-        { const Job J[1] = {job(Gn, T, Y, mone, gp, one)}; f_phase<FB, 1>(J, b); }
+        { const Job J[1] = {job(Gn, T, Y, -1.0, gp, 1.0)}; f_phase<FB, 1>(J, b); }
         s2g_nb<FB>(o.GR_diag + ((size_t)e * n + i) * bb, Gn, b);
         cplx* sw = G; G = Gn; Gn = sw; sw = col; col = col2; col2 = sw;
     }
@@ -653,76 +554,161 @@ __global__ void __launch_bounds__(FNT, 1) fused_ret_kernel(const FusedProblem P,
 // ---------------------------------------------------------------------------------------------------------------------
 // S5 + S6: lesser / greater sweeps, one CTA per (energy, < or >)
 // ---------------------------------------------------------------------------------------------------------------------
+// Both sweeps are software-pipelined so that a step of the chain is TWO phases, each shared with the preparation of
+// the next step (which does not depend on the chain):
+//   S5  g^x_i = W_i + Z_i g^x_{i-1} Z_i^H,  Z_i = g_i A_{i,i-1},  W_i = g_i B'_i g_i^H,
+//       B'_i = B_ii - (V - V^H), V = Y_{i-1} B_{i-1,i}  (the hoisted form of rgf.cu, SURVEY 8(a) S5 regrouped):
+//       iteration j: {T = Z_j g^x_{j-1} | Z_{j+1} = g_{j+1} A_{j+1,j} | P = g_{j+1} B'_{j+1}},
+//                    {g^x_j = W_j + T Z_j^H | W_{j+1} = P g_{j+1}^H}
+//   S6  T2_i = -g^x_i A_{i+1,i}^H + g_i B_{i,i+1};  Q_i = T2_i (G^R_{i+1,i+1})^H;  P_i = g^x_i - Q_i X_i^H;
+//       G^x_{i,i+1} = Q_i - X_i G^x_{i+1,i+1};  G^x_ii = P_i + X_i (G^x_{i,i+1})^H:
+//       iteration i: {G^x_{i,i+1} | P_i | T2_{i-1}},  {G^x_ii | Q_{i-1}}
+// g, X, H_{i,i+1}, G^R and g^x of the next step travel global -> registers before the phases and registers -> shared
+// memory after them.  Dense (block-tridiagonal) Sigma^<> blocks are read where they are used (two more products per
+// step, not pipelined).
 template <int FB>
 __global__ void __launch_bounds__(FNT, 1) fused_lg_kernel(const FusedProblem P, const FusedLgArgs a) {
-    constexpr int SZ = Mat<FB>::SZ;
+    constexpr int SZ = Mat<FB>::SZ, LD = Mat<FB>::LD, EPT = (FB * FB + FNT - 1) / FNT;
     extern __shared__ __align__(16) unsigned char fsm[];
     cplx* m = reinterpret_cast<cplx*>(fsm);
-    cplx *gx = m, *gi = m + SZ, *A1 = m + 2 * SZ, *Bm = m + 3 * SZ, *T = m + 4 * SZ, *T2 = m + 5 * SZ, *Yp = m + 6 * SZ,
-         *X = m + 7 * SZ, *GX = m + 8 * SZ, *Q = m + 9 * SZ, *GR = m + 10 * SZ;
     const int b = P.b, n = P.n, e = blockIdx.x;
     const FusedLgOne& S = a.x[blockIdx.y];
     const size_t bb = (size_t)b * b;
     const cplx* Wg = a.g + (size_t)e * n * bb;
     const cplx* WX = a.X + (size_t)e * (n - 1) * bb;
     const cplx* WY = a.Y + (size_t)e * (n - 1) * bb;
+    const cplx* GRd = a.GR_diag + (size_t)e * n * bb;
     cplx* Wgx = S.gx + (size_t)e * n * bb;
-    const cplx one = cmake(1.0, 0.0), mone = cmake(-1.0, 0.0), zero = cmake(0.0, 0.0);
-    constexpr int LD = Mat<FB>::LD;
-    // S5: g^x_0 = g_0 B_00 g_0^H; g^x_i = g_i [B_ii + A_{i,i-1} g^x_{i-1} A_{i,i-1}^H - (V - V^H)] g_i^H, V = Y_{i-1} B_{i-1,i}
-    for (int i = 0; i < n; i++) {
+    const bool bt = S.kind == NEGF_SIGMA_BT;
+    const cplx z = cmake(P.energy[e], P.eta);
+    const size_t kk = P.kidx ? (size_t)P.kidx[e] : 0;
+    const cplx* Hu = P.Hu ? P.Hu + kk * (n - 1) * bb : nullptr;
+    const cplx* Su = P.Su ? P.Su + kk * (n - 1) * bb : nullptr;
+    const cplx* sgl = P.sr_kind == NEGF_SIGMA_BT ? P.sr_lower + (size_t)e * (n - 1) * bb : nullptr;
+    // element idx of a b x b block (global, dense) <-> offset in a shared block
+    auto soff = [&](int idx) { return (idx / b) * LD + idx % b; };
+    // A_{i+1,i} = z S_{i,i+1}^H - H_{i,i+1}^H - Sigma^R_{i+1,i}, written transposed from the raw upper block hu
+    auto put_lower = [&](cplx* A1, int i, const cplx (&hu)[EPT]) {
+#pragma unroll
+        for (int q = 0; q < EPT; q++) {
+            const int idx = threadIdx.x + q * FNT;
+            if (idx < b * b) {
+                const int r = idx / b, c = idx % b;
+                cplx lo = Su ? cmul(z, cconj(Su[(size_t)i * bb + idx])) : cmake(0.0, 0.0);
+                lo = csub(lo, cconj(hu[q]));
+                if (sgl) lo = csub(lo, sgl[(size_t)i * bb + c * b + r]);
+                A1[c * LD + r] = lo;
+            }
+        }
+    };
+    auto put = [&](cplx* D, const cplx (&v)[EPT]) {
+#pragma unroll
+        for (int q = 0; q < EPT; q++) { const int idx = threadIdx.x + q * FNT; if (idx < b * b) D[soff(idx)] = v[q]; }
+    };
+    auto get = [&](cplx (&v)[EPT], const cplx* g) {
+#pragma unroll
+        for (int q = 0; q < EPT; q++) { const int idx = threadIdx.x + q * FNT; if (idx < b * b) v[q] = g[idx]; }
+    };
+    // B_ii of this family: scalar * I + dense diagonal block + boundary blocks
+    auto put_B = [&](cplx* Bm, int i) {
         const cplx sc = S.kind == NEGF_SIGMA_SCALAR ? S.scalar[e] : cmake(0.0, 0.0);
-        const cplx* sd = S.kind == NEGF_SIGMA_BT ? S.diag + ((size_t)e * n + i) * bb : nullptr;
+        const cplx* sd = bt ? S.diag + ((size_t)e * n + i) * bb : nullptr;
         const cplx* bl = (i == 0 && S.left) ? S.left + (size_t)e * bb : nullptr;
         const cplx* br = (i == n - 1 && S.right) ? S.right + (size_t)e * bb : nullptr;
-        f_each<FB>(b, [&](int r, int c, int oo) {
-            const int idx = r * b + c;
-            cplx v = r == c ? sc : cmake(0.0, 0.0);
+        for (int idx = threadIdx.x; idx < b * b; idx += FNT) {
+            cplx v = (idx / b == idx % b) ? sc : cmake(0.0, 0.0);
             if (sd) v = cadd(v, sd[idx]);
             if (bl) v = cadd(v, bl[idx]);
             if (br) v = cadd(v, br[idx]);
-            Bm[oo] = v;
-        });
-        if (i > 0) {
-            load_A<FB>(A1, P, e, i - 1, 2);                               // A_{i,i-1}
-            f_gemm<FB, 0, 0>(T, A1, gx, b, one, zero, nullptr);
-            f_gemm<FB, 0, 1>(Bm, T, A1, b, one, one, Bm);                 // + A g^x A^H
-            if (S.kind == NEGF_SIGMA_BT) {
-                g2s<FB>(Yp, WY + (size_t)(i - 1) * bb, b);
-                g2s<FB>(T2, S.upper + ((size_t)e * (n - 1) + i - 1) * bb, b);
-                f_gemm<FB, 0, 0>(T, Yp, T2, b, one, zero, nullptr);       // V
-                f_each<FB>(b, [&](int r, int c, int oo) {
-                    const cplx v = T[oo], vt = T[c * LD + r];
-                    Bm[oo] = cmake(Bm[oo].x - (v.x - vt.x), Bm[oo].y - (v.y + vt.y));     // - (V - V^H)
-                });
+            Bm[soff(idx)] = v;
+        }
+    };
+    cplx r0[EPT], r1[EPT], r2[EPT], r3[EPT];
+    // ---------------- S5 ----------------
+    cplx *gx = m, *gxn = m + SZ, *Z = m + 2 * SZ, *Zn = m + 3 * SZ, *W = m + 4 * SZ, *Wn = m + 5 * SZ, *gin = m + 6 * SZ,
+         *A1n = m + 7 * SZ, *Bmn = m + 8 * SZ, *Pn = m + 9 * SZ, *T = m + 10 * SZ, *E1 = m + 11 * SZ, *E2 = m + 12 * SZ;
+    get(r0, Wg); put(gin, r0); put_B(Bmn, 0);
+    __syncthreads();
+    if (n > 1) { get(r0, Wg + bb); get(r1, Hu); }
+    { const Job J[1] = {job(Pn, gin, Bmn, 1.0)}; f_phase<FB, 1>(J, b); }
+    { const Job J[1] = {job(gx, Pn, gin, 1.0)}; f_phase<FB, 1, 1u>(J, b); }               // g^x_0 = g_0 B_00 g_0^H
+    s2g_nb<FB>(Wgx, gx, b);
+    for (int j = 0; j < n; j++) {
+        const bool nxt = j + 1 < n;
+        if (nxt) {
+            put(gin, r0); put_lower(A1n, j, r1); put_B(Bmn, j + 1);
+            if (bt) { get(r2, WY + (size_t)j * bb); get(r3, S.upper + ((size_t)e * (n - 1) + j) * bb); put(E1, r2); put(E2, r3); }
+        }
+        __syncthreads();
+        if (j + 2 < n) { get(r0, Wg + (size_t)(j + 2) * bb); get(r1, Hu + (size_t)(j + 1) * bb); }
+        if (nxt && bt) {                                                  // B'_{j+1} = B - (V - V^H), V = Y_j B_{j,j+1}
+            { const Job J[1] = {job(Pn, E1, E2, 1.0)}; f_phase<FB, 1>(J, b); }
+            for (int idx = threadIdx.x; idx < b * b; idx += FNT) {
+                const int r = idx / b, c = idx % b;
+                const cplx v = Pn[r * LD + c], vt = Pn[c * LD + r];
+                cplx& d = Bmn[r * LD + c];
+                d = cmake(d.x - (v.x - vt.x), d.y - (v.y + vt.y));
             }
+            __syncthreads();
         }
-        g2s<FB>(gi, Wg + (size_t)i * bb, b);
-        f_gemm<FB, 0, 0>(T, gi, Bm, b, one, zero, nullptr);
-        f_gemm<FB, 0, 1>(gx, T, gi, b, one, zero, nullptr);
-        s2g<FB>(Wgx + (size_t)i * bb, gx, b);
+        if (j == 0 && !nxt) break;
+        { const Job J[4] = {job(j > 0 ? T : nullptr, Z, gx, 1.0), job(nxt ? Zn : nullptr, gin, A1n, 1.0),
+                            job(nxt ? Pn : nullptr, gin, Bmn, 1.0), job(nullptr, gin, gin, 1.0)};
+          f_phase<FB, 4>(J, b); }
+        { const Job J[2] = {job(j > 0 ? gxn : nullptr, T, Z, 1.0, W, 1.0), job(nxt ? Wn : nullptr, Pn, gin, 1.0)};
+          f_phase<FB, 2, 3u>(J, b); }
+        if (j > 0) { s2g_nb<FB>(Wgx + (size_t)j * bb, gxn, b); cplx* sw = gx; gx = gxn; gxn = sw; }
+        { cplx* sw = Z; Z = Zn; Zn = sw; sw = W; W = Wn; Wn = sw; }
     }
-    // S6: G^x_{n-1,n-1} = g^x_{n-1};  T2 = -g^x_i A_{i+1,i}^H + g_i B_{i,i+1};  Q = T2 (G^R_{i+1,i+1})^H;
-    //     G^x_{i,i+1} = Q - X_i G^x_{i+1,i+1};  G^x_ii = g^x_i - Q X_i^H + X_i (G^x_{i,i+1})^H
-    s2s<FB>(GX, gx, b);
-    s2g<FB>(S.GX_diag + ((size_t)e * n + n - 1) * bb, GX, b);
+    // ---------------- S6 ----------------
+    // G^x_{n-1,n-1} = g^x_{n-1}
+    cplx *GXa = m + 9 * SZ, *GXb = m + 10 * SZ, *Xs = m + 2 * SZ, *GRn = m + 3 * SZ, *T2n = m + 4 * SZ, *Pm = m + 5 * SZ,
+         *Qn = m + 6 * SZ;
+    cplx* slotP[2] = {m + 7 * SZ, m + 8 * SZ};                           // A_{i,i-1} of the next step, then Q_{i-1}
+    cplx* gxs[2];                                                        // g^x_i lives in gxs[i & 1]
+    gxs[(n - 1) & 1] = gx; gxs[n & 1] = gxn;
+    __syncthreads();
+    for (int idx = threadIdx.x; idx < b * b; idx += FNT) {
+        const cplx v = gx[soff(idx)];
+        GXa[soff(idx)] = v;
+        S.GX_diag[((size_t)e * n + n - 1) * bb + idx] = v;
+    }
+    if (n > 1) {
+        // prologue: T2_{n-2}, Q_{n-2} (each thread reads back the g^x elements it stored itself)
+        get(r0, Wgx + (size_t)(n - 2) * bb); get(r1, Hu + (size_t)(n - 2) * bb); get(r2, GRd + (size_t)(n - 1) * bb);
+        get(r3, WX + (size_t)(n - 2) * bb);
+        put(gxs[(n - 2) & 1], r0); put_lower(slotP[(n - 1) & 1], n - 2, r1); put(GRn, r2);
+        if (bt) { get(r0, Wg + (size_t)(n - 2) * bb); get(r1, S.upper + ((size_t)e * (n - 1) + n - 2) * bb); put(E1, r0); put(E2, r1); }
+        __syncthreads();
+        { const Job J[1] = {job(T2n, gxs[(n - 2) & 1], slotP[(n - 1) & 1], -1.0)}; f_phase<FB, 1, 1u>(J, b); }
+        if (bt) { const Job J[1] = {job(T2n, E1, E2, 1.0, T2n, 1.0)}; f_phase<FB, 1>(J, b); }
+        if (n > 2) { get(r0, Wgx + (size_t)(n - 3) * bb); get(r1, Hu + (size_t)(n - 3) * bb); get(r2, GRd + (size_t)(n - 2) * bb); }
+        { const Job J[1] = {job(slotP[(n - 1) & 1], T2n, GRn, 1.0)}; f_phase<FB, 1, 1u>(J, b); }       // Q_{n-2}
+    }
     for (int i = n - 2; i >= 0; i--) {
-        g2s<FB>(gx, Wgx + (size_t)i * bb, b);
-        load_A<FB>(A1, P, e, i, 2);                                       // A_{i+1,i}
-        f_gemm<FB, 0, 1>(T2, gx, A1, b, mone, zero, nullptr);
-        if (S.kind == NEGF_SIGMA_BT) {
-            g2s<FB>(gi, Wg + (size_t)i * bb, b);
-            g2s<FB>(T, S.upper + ((size_t)e * (n - 1) + i) * bb, b);
-            f_gemm<FB, 0, 0>(T2, gi, T, b, one, one, T2);
+        cplx* Qi = slotP[(i + 1) & 1];
+        cplx* gxi = gxs[i & 1];
+        const bool nxt = i > 0;
+        // the registers hold X_i and, for the preparation of step i - 1, g^x_{i-1}, H_{i-1,i}, G^R_ii (loaded one step ago)
+        put(Xs, r3);
+        if (nxt) { put(gxs[(i - 1) & 1], r0); put_lower(slotP[i & 1], i - 1, r1); put(GRn, r2); }
+        __syncthreads();
+        if (i >= 1) get(r3, WX + (size_t)(i - 1) * bb);
+        if (i >= 2) { get(r0, Wgx + (size_t)(i - 2) * bb); get(r1, Hu + (size_t)(i - 2) * bb); get(r2, GRd + (size_t)(i - 1) * bb); }
+        { const Job J[4] = {job(Qn, Xs, GXa, -1.0, Qi, 1.0), job(Pm, Qi, Xs, -1.0, gxi, 1.0),
+                            job(nxt ? T2n : nullptr, gxs[(i - 1) & 1], slotP[i & 1], -1.0), job(nullptr, Xs, Xs, 1.0)};
+          f_phase<FB, 4, 6u>(J, b); }
+        s2g_nb<FB>(S.GX_upper ? S.GX_upper + ((size_t)e * (n - 1) + i) * bb : nullptr, Qn, b);
+        if (nxt && bt) {
+            cplx t0[EPT], t1[EPT];
+            get(t0, Wg + (size_t)(i - 1) * bb); get(t1, S.upper + ((size_t)e * (n - 1) + i - 1) * bb); put(E1, t0); put(E2, t1);
+            __syncthreads();
+            const Job J[1] = {job(T2n, E1, E2, 1.0, T2n, 1.0)}; f_phase<FB, 1>(J, b);
         }
-        g2s<FB>(GR, a.GR_diag + ((size_t)e * n + i + 1) * bb, b);
-        f_gemm<FB, 0, 1>(Q, T2, GR, b, one, zero, nullptr);
-        g2s<FB>(X, WX + (size_t)i * bb, b);
-        f_gemm<FB, 0, 1>(gx, Q, X, b, mone, one, gx);                     // P_i = g^x_i - Q X^H
-        f_gemm<FB, 0, 0>(Q, X, GX, b, mone, one, Q);                      // G^x_{i,i+1}
-        s2g<FB>(S.GX_upper ? S.GX_upper + ((size_t)e * (n - 1) + i) * bb : nullptr, Q, b);
-        f_gemm<FB, 0, 1>(GX, X, Q, b, one, one, gx);                      // G^x_ii
-        s2g<FB>(S.GX_diag + ((size_t)e * n + i) * bb, GX, b);
+        { const Job J[2] = {job(GXb, Xs, Qn, 1.0, Pm, 1.0), job(nxt ? slotP[i & 1] : nullptr, T2n, GRn, 1.0)};
+          f_phase<FB, 2, 3u>(J, b); }
+        s2g_nb<FB>(S.GX_diag + ((size_t)e * n + i) * bb, GXb, b);
+        cplx* sw = GXa; GXa = GXb; GXb = sw;
     }
 }
 
@@ -740,8 +726,8 @@ int fused_prepare(negf_ctx* ctx) {
     NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(fused_obc_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fused_smem<32>(12)));
     NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(fused_ret_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fused_smem_ret<16>()));
     NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(fused_ret_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fused_smem_ret<32>()));
-    NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(fused_lg_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fused_smem<16>(11)));
-    NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(fused_lg_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fused_smem<32>(11)));
+    NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(fused_lg_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fused_smem<16>(13)));
+    NEGF_CUDA_CHECK(ctx, cudaFuncSetAttribute(fused_lg_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fused_smem<32>(13)));
     return NEGF_OK;
 }
 
@@ -765,8 +751,8 @@ int fused_ret_launch(negf_ctx* ctx, const FusedProblem& P, const FusedRetOut& o)
 int fused_lg_launch(negf_ctx* ctx, const FusedProblem& P, const FusedLgArgs& a) {
     ProfScope _ps(ctx, NEGF_PROF_FUSED);
     const dim3 grid(P.ne, a.nx);
-    if (P.b <= 16) fused_lg_kernel<16><<<grid, FNT, fused_smem<16>(11), ctx->stream>>>(P, a);
-    else           fused_lg_kernel<32><<<grid, FNT, fused_smem<32>(11), ctx->stream>>>(P, a);
+    if (P.b <= 16) fused_lg_kernel<16><<<grid, FNT, fused_smem<16>(13), ctx->stream>>>(P, a);
+    else           fused_lg_kernel<32><<<grid, FNT, fused_smem<32>(13), ctx->stream>>>(P, a);
     NEGF_LAUNCH_CHECK(ctx);
     return NEGF_OK;
 }
