@@ -311,7 +311,7 @@ __device__ __forceinline__ double f_norm_pair(const cplx* U, const cplx* L, int 
 // S2: Sancho-Rubio decimation, one CTA per (lead, energy)
 // ---------------------------------------------------------------------------------------------------------------------
 template <int FB>
-__global__ void __launch_bounds__(FNT, 1) fused_obc_kernel(const FusedObcArgs a) {
+__global__ void __launch_bounds__(FNT, FB <= 16 ? 2 : 1) fused_obc_kernel(const FusedObcArgs a) {
     constexpr int LD = Mat<FB>::LD, SZ = Mat<FB>::SZ;
     extern __shared__ __align__(16) unsigned char fsm[];
     cplx* m = reinterpret_cast<cplx*>(fsm);
@@ -466,7 +466,7 @@ __device__ __forceinline__ void s2g_nb(cplx* g, const cplx* S, int b) {       //
 // G_{i+1,i} = -G_{i+1,i+1} Y_i, corner column} as one phase, G_ii = g_i - G_{i,i+1} Y_i; g, X, Y of step i - 1 are
 // loaded into registers before the products and parked in shared memory after them.
 template <int FB>
-__global__ void __launch_bounds__(FNT, 1) fused_ret_kernel(const FusedProblem P, const FusedRetOut o) {
+__global__ void __launch_bounds__(FNT, FB <= 16 ? 2 : 1) fused_ret_kernel(const FusedProblem P, const FusedRetOut o) {
     constexpr int SZ = Mat<FB>::SZ, LD = Mat<FB>::LD, EPT = (FB * FB + FNT - 1) / FNT;
     extern __shared__ __align__(16) unsigned char fsm[];
     cplx* m = reinterpret_cast<cplx*>(fsm);
@@ -567,7 +567,7 @@ __global__ void __launch_bounds__(FNT, 1) fused_ret_kernel(const FusedProblem P,
 // memory after them.  Dense (block-tridiagonal) Sigma^<> blocks are read where they are used (two more products per
 // step, not pipelined).
 template <int FB>
-__global__ void __launch_bounds__(FNT, 1) fused_lg_kernel(const FusedProblem P, const FusedLgArgs a) {
+__global__ void __launch_bounds__(FNT, FB <= 16 ? 2 : 1) fused_lg_kernel(const FusedProblem P, const FusedLgArgs a) {
     constexpr int SZ = Mat<FB>::SZ, LD = Mat<FB>::LD, EPT = (FB * FB + FNT - 1) / FNT;
     extern __shared__ __align__(16) unsigned char fsm[];
     cplx* m = reinterpret_cast<cplx*>(fsm);

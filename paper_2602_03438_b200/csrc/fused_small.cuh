@@ -3,13 +3,13 @@
 #include "common.cuh"
 
 constexpr int NEGF_FUSED_MAX_B = 32;      // whole chain of one energy in one CTA up to this block size
-// The resident kernels run one CTA per energy (one per SM: ~200 registers x 256 threads), each walking its chain
-// alone: a latency win while the batch fits one wave of CTAs; beyond that the batched lock-step launches, which
-// spread every step of every energy over all SMs, have the higher throughput.  NEGF_OPT_FUSED_SMALL: 0 never,
-// 1 automatic (b <= 32 and N_E <= number of SMs), 2 always for b <= 32.
+// The resident kernels run one CTA per energy, each walking its chain alone.  Up to b = 16 they win at every batch size
+// (two CTAs per SM; n = 32, 1184 energies: 6.4 ms against 8.9 ms for the batched lock-step launches, measured with one
+// CTA per SM); for 16 < b <= 32 (one CTA per SM, FP64-pipe-bound products) only while the batch fits one wave of CTAs
+// (148 energies: 2.9 against 3.1 ms; 296: 5.7 against 5.0 ms).  NEGF_OPT_FUSED_SMALL: 0 never, 1 automatic, 2 always for b <= 32.
 inline bool fused_small_regime(const negf_ctx* ctx, int b, int ne) {
     if (b > NEGF_FUSED_MAX_B || ctx->fused_small == 0) return false;
-    return ctx->fused_small >= 2 || ne <= ctx->num_sms;
+    return ctx->fused_small >= 2 || b <= 16 || ne <= ctx->num_sms;
 }
 
 // device + energy batch + retarded self-energy (what the blocks of A = z S - H - Sigma^R are assembled from)
