@@ -3,6 +3,7 @@
     python kernel_bench.py --kernel zgemm --b 1024 --batch 16 [--opA 0 --opB 1]
     python kernel_bench.py --kernel zinv  --b 1024 --batch 16 [--inv-panel 0]
     python kernel_bench.py --kernel peak
+    python kernel_bench.py --kernel chain --b 16 --n-blocks 8 --batch 1 [--fused 0]     # the four C-ABI calls, one by one
 
 Prints one JSON line per run: achieved FP64 TFLOP/s (8 b^3 real flops per complex product or
 inversion, the unit U of SURVEY.md 8(d)) and the fraction of the DMMA issue-rate peak probed in
@@ -31,20 +32,52 @@ def _rand(shape, gen):
                          torch.randn(shape, dtype=torch.float64, device="cuda", generator=gen))
 
 
+def chain(args):
+    """Latency of the path's C-ABI calls one by one (CUDA events around each call, median of --reps) on a configs[0]-
+    shaped (--batch 1) or configs[1]-shaped workload of block size --b: the view of the resident small-block regime
+    (fused_small.cu), where one call is one launch."""
+    from paper_2602_03438_b200 import runner, workloads
+    wl = workloads.make_workload(0 if args.batch == 1 else 1, n_blocks=args.n_blocks, block_size=args.b,
+                                 **({} if args.batch == 1 else {"n_energy": args.batch}))
+    dp = runner.DevicePath(wl, want_greater=True)
+    dp.ctx.set_option(negf.OPT_FUSED_SMALL, args.fused)
+    calls = [("obc_decimate_pair", dp.obc), ("rgf_retarded", dp.retarded), ("rgf_lesser_greater", dp.lesser_greater),
+             ("observables", dp.observables), ("pipeline_device", dp.run)]
+    for _ in range(3):
+        dp.run_four_calls(); dp.run()
+    torch.cuda.synchronize()
+    out = {"kernel": "chain", "workload": wl.name if hasattr(wl, "name") else "", "b": args.b, "n_blocks": args.n_blocks,
+           "n_energy": wl.n_energy, "fused_small": args.fused, "us_median": {}, "launches": {}}
+    for name, fn in calls:
+        ts = []
+        n0 = dp.ctx.launch_count()
+        for _ in range(args.reps):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); fn(); e1.record(); torch.cuda.synchronize()
+            ts.append(e0.elapsed_time(e1) * 1e3)
+        out["us_median"][name] = round(sorted(ts)[len(ts) // 2], 1)
+        out["launches"][name] = (dp.ctx.launch_count() - n0) // args.reps
+    print(json.dumps(out))
+
+
 def main():
     ap = argparse.ArgumentParser()
-    ap.add_argument("--kernel", default="zgemm", choices=["zgemm", "zinv", "peak", "econv"])
+    ap.add_argument("--kernel", default="zgemm", choices=["zgemm", "zinv", "peak", "econv", "chain"])
     ap.add_argument("--b", type=int, default=1024)
     ap.add_argument("--batch", type=int, default=16)
     ap.add_argument("--opA", type=int, default=0)
     ap.add_argument("--opB", type=int, default=0)
     ap.add_argument("--reps", type=int, default=10)
+    ap.add_argument("--n-blocks", type=int, default=8, help="--kernel chain: blocks of the device")
+    ap.add_argument("--fused", type=int, default=1, help="--kernel chain: NEGF_OPT_FUSED_SMALL (0 never, 1 automatic, 2 always for b <= 32)")
     ap.add_argument("--sets", type=int, default=2, help="operand sets rotated between launches")
     ap.add_argument("--inv-panel", type=int, default=1, help="NEGF_OPT_INV_PANEL (1 = row-per-thread Gauss-Jordan panel, 0 = first LU panel kernel)")
     ap.add_argument("--inv-lookahead", type=int, default=1, help="NEGF_OPT_INV_LOOKAHEAD")
     ap.add_argument("--inv-outer", type=int, default=0, help="NEGF_OPT_INV_OUTER (0 = automatic)")
     ap.add_argument("--gemm-3m", action="store_true", help="NEGF_OPT_GEMM_3M (tflops still counted as 8 b^3 per product)")
     args = ap.parse_args()
+    if args.kernel == "chain":
+        return chain(args)
     ctx = negf.Context(0)
     st = torch.cuda.current_stream()
     ctx.set_stream(st.cuda_stream)

@@ -202,15 +202,15 @@ __global__ void obc_status_kernel(int ne, const int* done, const int* sing, cons
     if (e < ne) { status[e] = sing[e] ? sing[e] : (done[e] ? 0 : -1); iters[e] = it_in[e]; }
 }
 
-// loop condition of the decimation WHILE graph: two more doublings while any entry is active
-__global__ void sr_cond_kernel(cudaGraphConditionalHandle h, int nb, const int* done, int* it_dev, int max_iter) {
+// loop condition of the decimation WHILE graph: `step` more doublings while any entry is active
+__global__ void sr_cond_kernel(cudaGraphConditionalHandle h, int nb, const int* done, int* it_dev, int max_iter, int step) {
     __shared__ int any;
     if (threadIdx.x == 0) any = 0;
     __syncthreads();
     for (int e = threadIdx.x; e < nb; e += blockDim.x) if (!done[e]) any = 1;
     __syncthreads();
     if (threadIdx.x == 0) {
-        const int it = *it_dev + 2;
+        const int it = *it_dev + step;
         *it_dev = it;
         cudaGraphSetConditional(h, (any && it < max_iter) ? 1u : 0u);
     }
@@ -272,8 +272,8 @@ int ew_sr_step(negf_ctx* ctx, int b, int batch, cplx* a_s, cplx* a_b, cplx* g, c
     NEGF_LAUNCH_CHECK(ctx);
     return NEGF_OK;
 }
-int ew_sr_cond(negf_ctx* ctx, cudaGraphConditionalHandle h, int nb, const int* done, int* it_dev, int max_iter) {
-    sr_cond_kernel<<<1, 128, 0, ctx->stream>>>(h, nb, done, it_dev, max_iter);
+int ew_sr_cond(negf_ctx* ctx, cudaGraphConditionalHandle h, int nb, const int* done, int* it_dev, int max_iter, int step) {
+    sr_cond_kernel<<<1, 128, 0, ctx->stream>>>(h, nb, done, it_dev, max_iter, step);
     NEGF_LAUNCH_CHECK(ctx);
     return NEGF_OK;
 }

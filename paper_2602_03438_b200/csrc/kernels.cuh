@@ -39,7 +39,7 @@ int ew_sr_update(negf_ctx* ctx, int b, int batch, cplx* a_s, cplx* a_b, cplx* g,
 int ew_sr_step(negf_ctx* ctx, int b, int batch, cplx* a_s, cplx* a_b, cplx* g, const cplx* lgu, const cplx* ugl,
                const cplx* un, const cplx* ln, const double* ref, double tol, int* done, int* iters, int it,
                double* acc /*[batch][8][2]*/, unsigned* ticket /*[batch], zero*/, const int* it_dev = nullptr);
-int ew_sr_cond(negf_ctx* ctx, cudaGraphConditionalHandle h, int nb, const int* done, int* it_dev, int max_iter);
+int ew_sr_cond(negf_ctx* ctx, cudaGraphConditionalHandle h, int nb, const int* done, int* it_dev, int max_iter, int step);
 int ew_sr_norm(negf_ctx* ctx, int b, int batch, const cplx* u, const cplx* l, double* ref, double tol,
                int* done, int* iters, int it, int mode);
 int ew_obc_finalize(negf_ctx* ctx, int b, int batch, const cplx* sigma, const double* energy, double mu,

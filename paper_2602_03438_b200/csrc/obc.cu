@@ -143,9 +143,13 @@ int obc_core(negf_ctx* ctx, const negf_problem* p, int ns, const LeadBlocks* lb,
             sf.use_side(0);
             cudaError_t ce = cudaStreamBeginCaptureToGraph(ctx->stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed);
             if (ce != cudaSuccess) { cudaGraphDestroy(G); ctx->last_cuda_error = (int)ce; return NEGF_ECUDA; }
-            int rc = doubling(ub[1], lbuf[1], ub[0], lbuf[0], 0, it_dev);
-            if (rc == NEGF_OK) rc = doubling(ub[0], lbuf[0], ub[1], lbuf[1], 1, it_dev);
-            if (rc == NEGF_OK) rc = ew_sr_cond(ctx, h, nb, W.done, it_dev, max_iter);
+            int rc = NEGF_OK;
+            const int dpb = 2;         // doublings per WHILE iteration (4 / 8 measured: 5.77 / 5.74 ms against 5.79 at configs[1])
+            for (int q = 0; q < dpb && rc == NEGF_OK; q += 2) {
+                rc = doubling(ub[1], lbuf[1], ub[0], lbuf[0], q, it_dev);
+                if (rc == NEGF_OK) rc = doubling(ub[0], lbuf[0], ub[1], lbuf[1], q + 1, it_dev);
+            }
+            if (rc == NEGF_OK) rc = ew_sr_cond(ctx, h, nb, W.done, it_dev, max_iter, dpb);
             cudaGraph_t dummy = nullptr;
             ce = cudaStreamEndCapture(ctx->stream, &dummy);
             sf.use_main();

@@ -114,3 +114,33 @@ def test_config0_latency(negf_lib):
     for nm, grp, key in (("GR_diag", "ret", "GR_diag"), ("GR_upper", "ret", "GR_upper"), ("GL_diag", "les", "GX_diag"),
                          ("GL_upper", "les", "GX_upper"), ("GG_diag", "gtr", "GX_diag")):
         assert rel_fro(dp.host(nm)[0], o[grp][key]) < 1e-10, nm
+
+
+@pytest.mark.parametrize("cfg,kw", [(0, {}), (1, dict(n_blocks=5, block_size=24, n_energy=4)),
+                                    (2, dict(n_blocks=4, block_size=17, n_energy=3)), (2, dict(n_blocks=2, block_size=9, n_energy=40)),
+                                    (3, dict(n_blocks=3, block_size=32, n_energy=2))])
+def test_resident_observables_equal_batched_kernels(negf_lib, cfg, kw):
+    """S7 of the resident regime is ONE launch (observables.cu:obs_small_kernel, blocks take roles); fed with the SAME G
+    blocks and boundary blocks it must reproduce the seven separate kernels of the batched path to summation order
+    (S != I exercises the three-term density and LDOS, configs[2])."""
+    from paper_2602_03438_b200 import runner
+    wl = W.make_workload(cfg, **kw)
+    fused = runner.DevicePath(wl, want_greater=True)
+    fused.run_four_calls()
+    plain = runner.DevicePath(wl, want_greater=True)
+    plain.ctx.set_option(negf_lib.OPT_FUSED_SMALL, 0)
+    plain.run_four_calls()                                   # sizes the workspace the batched T(E) needs
+    torch.cuda.synchronize()
+    for k, v in fused.out.items():
+        if k not in ("density", "ldos", "transmission", "bond_current", "contact_current"):
+            plain.out[k].copy_(v)
+    n0 = fused.ctx.launch_count()
+    fused.observables()
+    assert fused.ctx.launch_count() - n0 == 1
+    plain.observables()
+    torch.cuda.synchronize()
+    names = ["density", "ldos", "transmission", "contact_current"] + (["bond_current"] if wl.n_blocks > 1 else [])
+    for nm in names:
+        a, b = fused.host(nm), plain.host(nm)
+        scale = np.max(np.abs(b)) + 1e-300
+        assert np.max(np.abs(a - b)) <= 1e-12 * scale + 1e-13 * np.max(np.abs(fused.host("GL_diag"))), (nm, np.max(np.abs(a - b)), scale)
