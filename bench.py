@@ -264,7 +264,8 @@ def work_accounting(wl, res, steps, launches, gemm_3m, args_groups=0):
     bad = int((o["info_r"] != 0).sum() + (o["info_x"] != 0).sum() + (o["status_L"] != 0).sum() + (o["status_R"] != 0).sum())
     iters_mean = float((o["iters_L"].double().sum() + o["iters_R"].double().sum()) / (2 * dp.ne))
     iters_total = iters_mean * 2 * wl.n_energy
-    resident = wl.block_size <= 32 and res.ne_batch <= 148      # NEGF_OPT_FUSED_SMALL automatic regime: no WHILE graph
+    # NEGF_OPT_FUSED_SMALL automatic regime (fused_small.cuh:fused_small_regime): no WHILE graph
+    resident = wl.block_size <= 16 or (wl.block_size <= 32 and res.ne_batch <= 148)
     if wl.block_size <= 96 and wl.max_iter % 2 == 0 and not resident:
         # the doublings run inside a device-driven WHILE graph (one host launch per group): its kernels are counted
         # from the iteration counters: 9 per pair of doublings (2 x [inverse, 2 grouped GEMMs, step] + loop condition)
