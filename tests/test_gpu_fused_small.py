@@ -116,6 +116,26 @@ def test_config0_latency(negf_lib):
         assert rel_fro(dp.host(nm)[0], o[grp][key]) < 1e-10, nm
 
 
+@pytest.mark.parametrize("cfg,kw", [(0, {}), (1, dict(n_blocks=9, block_size=32, n_energy=150)),
+                                    (2, dict(n_blocks=5, block_size=17, n_energy=300)), (3, dict(n_blocks=4, block_size=31, n_energy=20))])
+def test_resident_path_is_bit_identical_run_to_run(negf_lib, cfg, kw):
+    """The resident kernels hand data between warps through named barriers, shuffles, an mbarrier and double-buffered
+    shared memory; every reduction has a fixed order.  A race would show as a run-to-run difference: twelve passes of
+    the whole path must reproduce the first one bit for bit (one wave and more than one wave of CTAs, every Sigma kind)."""
+    from paper_2602_03438_b200 import runner
+    wl = W.make_workload(cfg, **kw)
+    dp = runner.DevicePath(wl, want_greater=True)
+    dp.run(); torch.cuda.synchronize()
+    ref = {k: v.clone() for k, v in dp.out.items()}
+    for rep in range(12):
+        dp.run()
+        torch.cuda.synchronize()
+        for k, v in dp.out.items():
+            a = torch.view_as_real(v) if v.is_complex() else v
+            r = torch.view_as_real(ref[k]) if ref[k].is_complex() else ref[k]
+            assert torch.equal(torch.nan_to_num(a.double()), torch.nan_to_num(r.double())), (k, rep)
+
+
 @pytest.mark.parametrize("cfg,kw", [(0, {}), (1, dict(n_blocks=5, block_size=24, n_energy=4)),
                                     (2, dict(n_blocks=4, block_size=17, n_energy=3)), (2, dict(n_blocks=2, block_size=9, n_energy=40)),
                                     (3, dict(n_blocks=3, block_size=32, n_energy=2))])
