@@ -196,6 +196,22 @@ __global__ void __launch_bounds__(WM * WN * 32, MINB) zgemm_kernel(const __grid_
     };
 #pragma unroll
     for (int s = 0; s < STAGES - 1; s++) issue();
+    // beta D: the addend tile is read in the epilogue, after the last product - with one CTA per SM nothing overlaps
+    // that read (rank-k updates of the blocked inverse: k = 32 .. 256, the tile read is as long as 1-3 k-blocks).
+    // Ask L2 for this thread's 32-byte pieces of it now, behind the first operand loads.
+    if (BM >= 64 && a.D) {
+        const cplx* gDp = a.D + (size_t)e * a.sD + (size_t)e2 * a.sD2 + n0 + wn0 + lk * 2;
+#pragma unroll
+        for (int i = 0; i < MI; i++) {
+            const int row = m0 + wm0 + i * 8 + lr;
+            if (row < a.m) {
+#pragma unroll
+                for (int j = 0; j < NI; j++)
+                    if (n0 + wn0 + lk * 2 + j * 8 < a.n)
+                        asm volatile("prefetch.global.L2 [%0];" ::"l"(gDp + (size_t)row * a.ldc + j * 8));
+            }
+        }
+    }
 
     int st = 0;
     for (int kb = 0; kb < KB; kb++) {
