@@ -1100,10 +1100,13 @@ constexpr int OUTER_NB_MAX = 256;  // widest outer block of the two-level blocke
 // --kernel zinv, ms per batched inverse, nb = 64 / 128 / 256): b = 256 batch 256: 3.19 / 3.29 / 3.89; b = 512
 // batch 32: 3.14 / 3.00 / 3.38; b = 1024 batch 8: 5.13 / 5.38 / 5.77; b = 2048 batch 8: 33.6 / 28.4 / 27.5.
 // NEGF_OPT_INV_OUTER overrides (multiple of 32, <= 256).
-inline int outer_nb(const negf_ctx* ctx, int b) {
+// With the addend prefetch of K2 (zgemm.cu) re-measured, nb = 64 / 128 / 256: b = 256 batch 256: 2.92 / 3.02 / 3.37; b = 512
+// batch 32: 2.91 / 2.91 / 3.26; b = 1024 batch 8: 4.76 / 5.18 / 5.71, batch 32: 15.36 / 14.33 / 14.73 (a large batch fills the
+// machine without the look-ahead's many short stages); b = 2048 batch 8: 29.3 / 26.5 / 26.4.
+inline int outer_nb(const negf_ctx* ctx, int b, int batch) {
     if (ctx->inv_outer >= 32 && ctx->inv_outer <= OUTER_NB_MAX && ctx->inv_outer % 32 == 0) return ctx->inv_outer;
     if (b > 1024) return 256;
-    if (b > 512) return 64;
+    if (b > 512) return batch >= 16 ? 128 : 64;
     return b > 256 ? 128 : 64;
 }
 
@@ -1209,7 +1212,7 @@ int zinv_launch(negf_ctx* ctx, int b, cplx* A, long long sA, int batch, void* ws
     // M[:, ~K] = (M with rows K zeroed)[:, ~K] + Q R, R = the pivot rows: a GEMM with k = 128.
     // look-ahead over the outer blocks (side stream): only where the inverse runs on the caller's own stream (b above
     // the two-sided regime), outside profiling (intervals must not overlap) and with at least three outer blocks
-    const int OUTER_NB = outer_nb(ctx, b);
+    const int OUTER_NB = outer_nb(ctx, b, batch);
     cudaStream_t main_stream = ctx->stream;
     const bool lookahead = gj_panel_rows_supported(b) && ctx->inv_panel && ctx->inv_lookahead && !ctx->prof_on &&
                            b > 2 * OUTER_NB && ctx->inv_side != nullptr;
