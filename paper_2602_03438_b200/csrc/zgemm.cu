@@ -464,6 +464,7 @@ cudaError_t prepare_cfg() {
 int zgemm_prepare(negf_ctx* ctx) {
     NEGF_CUDA_CHECK(ctx, (prepare_cfg<128, 64, 4, 2, 1>()));
     NEGF_CUDA_CHECK(ctx, (prepare_cfg<64, 64, 2, 2, 2>()));
+    NEGF_CUDA_CHECK(ctx, (prepare_cfg<64, 64, 2, 4, 2>()));
     NEGF_CUDA_CHECK(ctx, (prepare_cfg<32, 32, 2, 2, 5>()));
     NEGF_CUDA_CHECK(ctx, (prepare_cfg<16, 16, 2, 2, 6>()));
     {
@@ -512,13 +513,14 @@ int zgemm_launch_group(negf_ctx* ctx, const GemmGroup& grp) {
         if (a.opA == 0 && a.opB == 1) return launch_3m<0, 1>(ctx, grp);
         return launch_3m<1, 1>(ctx, grp);
     }
-    // Compute-bound regime: 64x64 tiles, TWO CTAs of 4 warps per SM.  The 128x64 tile (8 warps, 243 registers) leaves one
+    // Compute-bound regime: 64x64 tiles, TWO CTAs per SM.  The 128x64 tile (8 warps, 243 registers) leaves one
     // CTA per SM, so nothing runs while it fills its pipeline, waits at its k-block barriers, reads the addend and stores
-    // its tile; two co-resident CTAs cover each other.  Measured (kernel_bench, fraction of the FP64 peak, 128x64 -> 64x64
+    // its tile; two co-resident CTAs cover each other (numbers below: 4 warps of 32x32 per CTA).  Measured (kernel_bench, fraction of the FP64 peak, 128x64 -> 64x64
     // x 2): b = 2048 batch 8: 92.4 -> 94.8 %; b = 1024 batch 32: 91.5 -> 94.3 %; b = 512 batch 32: 88.6 -> 91.7 %; b = 256
     // batch 512: 86.3 -> 91.0 %; b = 300 batch 40: 51.6 -> 64.7 %; blocked inverse b = 2048 batch 8: 26.4 -> 25.6 ms;
     // whole path configs[2] 1799 -> 1723 ms, configs[3] 13.37 -> 13.00 s, configs[4] 13.13 -> 12.77 s.
-    if (a.m > 64 && t64 >= 2LL * ctx->num_sms && !alias_a) return launch_ops<64, 64, 2, 2, 2>(ctx, grp);
+    // 8 warps of 32x16 per CTA (128 registers) measured another 0.3-0.7 points above 4 warps of 32x32 (230 registers).
+    if (a.m > 64 && t64 >= 2LL * ctx->num_sms && !alias_a) return launch_ops<64, 64, 2, 4, 2>(ctx, grp);
     if (a.m > 64 && t128 >= ctx->num_sms) return launch_ops<128, 64, 4, 2, 1>(ctx, grp);
     // blocks up to 64 x 64: four 32x32 CTAs per product balance the SMs better than one 64x64 CTA
     // (measured 5-7 % faster at b = 64 for 128 .. 512 products per launch)
