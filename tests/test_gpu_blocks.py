@@ -47,6 +47,32 @@ def test_zgemm_batched(ctx, m, n, k, opA, opB):
     assert np.linalg.norm(dC2.cpu().numpy() - ref2) / np.linalg.norm(ref2) < 1e-13
 
 
+@pytest.mark.parametrize("m,n,k,batch", [(200, 130, 75, 40), (129, 65, 17, 150), (300, 257, 33, 20), (70, 640, 130, 30),
+                                         (1030, 1000, 70, 2)])
+@pytest.mark.parametrize("opA,opB", [(0, 0), (1, 0), (0, 1), (1, 1)])
+def test_zgemm_compute_bound_tiles(ctx, m, n, k, batch, opA, opB):
+    """Launches with at least two 64 x 64 tiles per SM take the compute-bound tile configuration of K2 (two co-resident CTAs
+    of 8 warps per SM, addend tile prefetched into L2): ragged rows, columns and k, every operand orientation, with an
+    in-place addend (C == D), against NumPy at the K2 bar."""
+    import torch
+    assert ((m + 63) // 64) * ((n + 63) // 64) * batch >= 2 * 148
+    rng = np.random.default_rng(m * 7 + n * 3 + k + opA * 2 + opB)
+    A = _rand(rng, batch, *((k, m) if opA else (m, k)))
+    B = _rand(rng, batch, *((n, k) if opB else (k, n)))
+    D = _rand(rng, batch, m, n)
+    alpha, beta = -0.9 + 0.2j, 1.0
+    opa = (lambda x: np.conj(np.swapaxes(x, -1, -2))) if opA else (lambda x: x)
+    opb = (lambda x: np.conj(np.swapaxes(x, -1, -2))) if opB else (lambda x: x)
+    ref = alpha * (opa(A) @ opb(B)) + beta * D
+    dA, dB, dC = (torch.from_numpy(x).cuda() for x in (A, B, D))
+    ctx.zgemm_batched(opA, opB, m, n, k, alpha, dA, A.shape[2], A.shape[1] * A.shape[2], dB, B.shape[2],
+                      B.shape[1] * B.shape[2], beta, dC, dC, n, m * n, batch)
+    got = dC.cpu().numpy()
+    for e in (0, batch // 2, batch - 1):
+        assert np.linalg.norm(got[e] - ref[e]) / np.linalg.norm(ref[e]) < 1e-13, e
+    assert np.linalg.norm(got - ref) / np.linalg.norm(ref) < 1e-13
+
+
 @pytest.mark.parametrize("b", [1, 2, 7, 16, 33, 64, 96, 97, 130, 256, 300, 515, 1100, 2100])
 def test_zinverse_batched(ctx, negf_lib, b):
     """2100 > 2048 rows: the first panels take the shared-memory cluster panel kernel instead of the register one."""
