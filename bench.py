@@ -320,6 +320,8 @@ def run_gpu(args, rank, local_rank, world):
         ctx.set_option(negf.OPT_GEMM_3M, 1)
     if args.energy_groups:
         ctx.set_option(negf.OPT_ENERGY_GROUPS, args.energy_groups)
+    if args.pdl >= 0:
+        ctx.set_option(negf.OPT_PDL, args.pdl)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
     peak = ctx.fp64_peak(300.0)
     hbm_peak, hbm_src = measured_hbm_peak()
@@ -409,7 +411,7 @@ def roofline_entry(wl, prof, psteps, step_ms, gemm_u, inv_u, peak, hbm_peak, hbm
     achieved = dom_flops / (dom_ms * 1e-3) * 1e-12 if dom_ms > 0 else 0.0
     r = {"bound": "tensor", "kernel": {"gemm": "zgemm_kernel (DMMA.8x8x4, 4M complex)", "fused": "fused chain kernels"}[dom],
          "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-         "traffic": roofline_traffic(wl.name),
+         "traffic": roofline_traffic(wl.name)[0], "traffic_source": roofline_traffic(wl.name)[1],
          "peak_source": "negf_fp64_peak: DMMA m8n8k4 issue-rate probe run in this process "
                         "(MEASURED_PEAKS.json has no FP64 figure; nominal 37.2 = 148 SM x 1.965 GHz x 128 flop/clk)",
          "flops_per_launch": dom_flops / max(dom_sites, 1),
@@ -467,17 +469,17 @@ def measured_hbm_peak():
 
 
 def roofline_traffic(workload):
-    """DRAM bytes per launch of the dominant kernel from the committed ncu capture of this workload
-    (profiles/roofline_traffic.csv), or None when none was taken."""
+    """(DRAM bytes per launch of the dominant kernel, which launch and capture) from the committed ncu capture
+    of this workload (profiles/roofline_traffic.csv), or (None, None) when none was taken."""
     import csv
     try:
         with open(os.path.join(ROOT, "profiles", "roofline_traffic.csv")) as f:
             for row in csv.DictReader(f):
                 if row["workload"] == workload:
-                    return float(row["bytes_per_launch"])
+                    return float(row["bytes_per_launch"]), f'{row["kernel"]}: {row["source"]}'
     except OSError:
         pass
-    return None
+    return None, None
 
 
 def default_energy_batch(wl, free_bytes):
@@ -544,6 +546,7 @@ def main():
     ap.add_argument("--gemm-3m", action="store_true",
                     help="3M complex products in the compute-bound regime (NEGF_OPT_GEMM_3M); flops are then counted as executed (x 0.75 per product)")
     ap.add_argument("--energy-groups", type=int, default=0, help="NEGF_OPT_ENERGY_GROUPS (0 = the library's automatic choice)")
+    ap.add_argument("--pdl", type=int, default=-1, help="NEGF_OPT_PDL (-1 = the library's default)")
     ap.add_argument("--energy-batch", type=int, default=0, help="energies resident at once (0 = fit HBM)")
     ap.add_argument("--e2e-energies", type=int, default=0)
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="0 skips the cpu_baseline leg")

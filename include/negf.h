@@ -150,7 +150,15 @@ int negf_set_workspace(negf_ctx* ctx, void* dev_ptr, size_t bytes);
  * complete doubling loop), negf_rgf_retarded one launch (one CTA per energy, forward and backward sweep),
  * negf_rgf_lesser_greater one launch (one CTA per energy and < / >).  0 = the batched lock-step launches used for
  * larger blocks.  Same definitions, results equal to rounding.  Set it before negf_rgf_retarded: the retained
- * sweep state of one regime is not valid for the other. */
+ * sweep state of one regime is not valid for the other.
+ * NEGF_OPT_PDL (default 1; bit 0 = on, bit 1 = also inside the decimation WHILE graph): the kernels of the
+ * latency-bound chains (complex GEMM with tiles up to 32 x 32, the one-CTA inverse of 16 < b <= 64, the decimation
+ * step) are launched with CUDA's programmatic-stream-serialization attribute: their CTAs are placed while the previous
+ * kernel of the stream drains and block in griddepcontrol.wait until it has completed, which takes the launch gap out of
+ * the dependent chain (b = 64, 64 energies, one stream: negf_rgf_retarded 1.78 -> 1.71 ms, negf_rgf_lesser_greater 2.80 ->
+ * 2.69 ms).  Bit-identical results.  The concurrent energy groups of negf_pipeline_device / _host always run with 0:
+ * they already cover each other's gaps, and a waiting grid would only take SM slots from the other groups (measured
+ * 5.79 -> 6.12 ms per configs[1] step with it).  Changing the option drops the cached call graphs. */
 #define NEGF_OPT_GRAPH_LOOPS   1
 #define NEGF_OPT_GEMM_3M       2
 #define NEGF_OPT_INV_TENSOR    3
@@ -159,6 +167,7 @@ int negf_set_workspace(negf_ctx* ctx, void* dev_ptr, size_t bytes);
 #define NEGF_OPT_INV_LOOKAHEAD 6
 #define NEGF_OPT_INV_OUTER     7
 #define NEGF_OPT_FUSED_SMALL   8
+#define NEGF_OPT_PDL           9
 #define NEGF_MAX_ENERGY_GROUPS 4
 int negf_set_option(negf_ctx* ctx, int option, int value);
 const char* negf_strerror(int code);

@@ -41,13 +41,17 @@ def chain(args):
                                  **({} if args.batch == 1 else {"n_energy": args.batch}))
     dp = runner.DevicePath(wl, want_greater=True)
     dp.ctx.set_option(negf.OPT_FUSED_SMALL, args.fused)
+    if args.pdl >= 0:
+        dp.ctx.set_option(negf.OPT_PDL, args.pdl)
+    if args.energy_groups:
+        dp.ctx.set_option(negf.OPT_ENERGY_GROUPS, args.energy_groups)
     calls = [("obc_decimate_pair", dp.obc), ("rgf_retarded", dp.retarded), ("rgf_lesser_greater", dp.lesser_greater),
              ("observables", dp.observables), ("pipeline_device", dp.run)]
     for _ in range(3):
         dp.run_four_calls(); dp.run()
     torch.cuda.synchronize()
     out = {"kernel": "chain", "workload": wl.name if hasattr(wl, "name") else "", "b": args.b, "n_blocks": args.n_blocks,
-           "n_energy": wl.n_energy, "fused_small": args.fused, "us_median": {}, "launches": {}}
+           "n_energy": wl.n_energy, "fused_small": args.fused, "pdl": args.pdl, "energy_groups": args.energy_groups, "us_median": {}, "launches": {}}
     for name, fn in calls:
         ts = []
         n0 = dp.ctx.launch_count()
@@ -74,6 +78,8 @@ def main():
     ap.add_argument("--inv-panel", type=int, default=1, help="NEGF_OPT_INV_PANEL (1 = row-per-thread Gauss-Jordan panel, 0 = first LU panel kernel)")
     ap.add_argument("--inv-lookahead", type=int, default=1, help="NEGF_OPT_INV_LOOKAHEAD")
     ap.add_argument("--inv-outer", type=int, default=0, help="NEGF_OPT_INV_OUTER (0 = automatic)")
+    ap.add_argument("--pdl", type=int, default=-1, help="--kernel chain: NEGF_OPT_PDL (-1 = the library's default)")
+    ap.add_argument("--energy-groups", type=int, default=0, help="--kernel chain: NEGF_OPT_ENERGY_GROUPS (0 = automatic)")
     ap.add_argument("--gemm-3m", action="store_true", help="NEGF_OPT_GEMM_3M (tflops still counted as 8 b^3 per product)")
     args = ap.parse_args()
     if args.kernel == "chain":

@@ -1,6 +1,8 @@
 // Context management, error strings, the FP64 DMMA peak probe and the host-buffer pipeline
 // (include/negf.h).  No CPU fallback anywhere: negf_create fails unless a CUDA device of compute
 // capability 10.x is present.
+#include <stdlib.h>
+
 #include <new>
 
 #include "common.cuh"
@@ -30,8 +32,10 @@ extern "C" int negf_create(negf_ctx** out, int device) {
     for (int k = 0; k < NEGF_NGRAPH; k++) for (int q = 0; q < NEGF_GWAYS; q++) c->gslot[k][q] = {0ull, nullptr, 0, 0u};
     c->gtick = 0;
     if (cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) != cudaSuccess) { delete c; return NEGF_ECUDA; }
-    for (int k = 0; k < 4; k++) if (cudaEventCreateWithFlags(&c->ev_grp[k], cudaEventDisableTiming) != cudaSuccess) { delete c; return NEGF_ECUDA; }
+    for (int k = 0; k < NEGF_MAX_ENERGY_GROUPS; k++) if (cudaEventCreateWithFlags(&c->ev_grp[k], cudaEventDisableTiming) != cudaSuccess) { delete c; return NEGF_ECUDA; }
     if (cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking) != cudaSuccess) { delete c; return NEGF_ECUDA; } c->obc_key_ws = nullptr; c->obc_key_b = c->obc_key_n = c->obc_key_ne = c->obc_key_ns = c->obc_key_maxit = 0; c->obc_key_tol = 0.0;
+    c->pdl = NEGF_PDL_DEFAULT; c->in_while_body = false;
+    if (const char* ev = getenv("NEGF_PDL")) { const int v = atoi(ev); if (v >= 0 && v <= 3) c->pdl = v; }   // developer override
     c->inv_lookahead = 1; c->inv_outer = 0; c->inv_side = nullptr; c->ev_inv_main = c->ev_inv_side = nullptr;
     // lowest priority: when both have CTAs pending, the caller's stream (the latency-bound panels) goes first
     int prio_lo = 0, prio_hi = 0;
@@ -56,7 +60,7 @@ extern "C" int negf_destroy(negf_ctx* ctx) {
     if (ctx->obc_exec) cudaGraphExecDestroy(ctx->obc_exec);
     for (int k = 0; k < NEGF_NGRAPH; k++) for (int q = 0; q < NEGF_GWAYS; q++) if (ctx->gslot[k][q].exec) cudaGraphExecDestroy(ctx->gslot[k][q].exec);
     cudaStreamDestroy(ctx->copy_stream);
-    for (int k = 0; k < 4; k++) cudaEventDestroy(ctx->ev_grp[k]);
+    for (int k = 0; k < NEGF_MAX_ENERGY_GROUPS; k++) cudaEventDestroy(ctx->ev_grp[k]);
     cudaStreamDestroy(ctx->cap_stream);
     for (int k = 0; k < NEGF_MAX_ENERGY_GROUPS; k++) {
         if (ctx->child[k]) negf_destroy(ctx->child[k]);
@@ -97,6 +101,15 @@ extern "C" int negf_set_option(negf_ctx* ctx, int option, int value) {
     if (option == NEGF_OPT_INV_PANEL) { ctx->inv_panel = value; return NEGF_OK; }
     if (option == NEGF_OPT_INV_LOOKAHEAD) { ctx->inv_lookahead = value; return NEGF_OK; }
     if (option == NEGF_OPT_INV_OUTER) { ctx->inv_outer = value; return NEGF_OK; }
+    if (option == NEGF_OPT_PDL) {
+        if (value < 0 || value > 3) return NEGF_EINVAL;
+        if (value != ctx->pdl) {               // cached graphs hold the edges of the old setting
+            for (int k = 0; k < NEGF_NGRAPH; k++) for (int q = 0; q < NEGF_GWAYS; q++) ctx->gslot[k][q].key = 0;
+            if (ctx->obc_exec) { cudaGraphExecDestroy(ctx->obc_exec); ctx->obc_exec = nullptr; }
+            ctx->obc_key_ws = nullptr;
+        }
+        ctx->pdl = value; return NEGF_OK;
+    }
     if (option == NEGF_OPT_FUSED_SMALL) { ctx->fused_small = value; ctx->sweep_valid = false; return NEGF_OK; }
     if (option == NEGF_OPT_ENERGY_GROUPS) {
         if (value < 0 || value > NEGF_MAX_ENERGY_GROUPS) return NEGF_EINVAL;

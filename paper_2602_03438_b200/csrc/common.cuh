@@ -11,6 +11,7 @@
 typedef double2 cplx;  // (x, y) = (re, im), same bytes as negf_c128
 constexpr int NEGF_NSIDE = 2;
 constexpr int NEGF_GWAYS = 4;     // cached argument sets per entry point (energy groups of negf_pipeline_host)
+constexpr int NEGF_PDL_DEFAULT = 1;   // negf_set_option(NEGF_OPT_PDL) at negf_create
 constexpr int NEGF_NGRAPH = 2;    // 0 negf_rgf_retarded, 1 negf_rgf_lesser_greater
 
 struct negf_ctx {
@@ -38,6 +39,7 @@ struct negf_ctx {
     int inv_panel;                // negf_set_option(NEGF_OPT_INV_PANEL)
     int inv_lookahead;            // negf_set_option(NEGF_OPT_INV_LOOKAHEAD)
     int inv_outer;                // negf_set_option(NEGF_OPT_INV_OUTER); 0 = automatic
+    int pdl;                      // negf_set_option(NEGF_OPT_PDL): bit 0 = chain kernels, bit 1 = also inside the WHILE graph
     cudaStream_t inv_side;        // side stream of the blocked inverse's look-ahead (zinv.cu)
     cudaEvent_t ev_inv_main, ev_inv_side;
     // cached CUDA graphs of whole calls in the latency-bound regime (same arguments twice in a row
@@ -47,7 +49,7 @@ struct negf_ctx {
     unsigned gtick;
     cudaStream_t cap_stream;      // capture stream (the caller's may be the legacy default stream)
     cudaStream_t copy_stream;     // device->host copies of negf_pipeline_host
-    cudaEvent_t ev_grp[4];
+    cudaEvent_t ev_grp[NEGF_MAX_ENERGY_GROUPS];
     // concurrent energy groups of negf_pipeline_device / _host (K3): child contexts (own side streams and
     // graph caches), created on first use, each on its own stream
     int energy_groups;            // negf_set_option(NEGF_OPT_ENERGY_GROUPS); 0 = automatic
@@ -65,6 +67,8 @@ struct negf_ctx {
     int prof_last_class; cudaEvent_t prof_last_event;
     double prof_ms[NEGF_PROF_CLASSES];
     long long prof_n[NEGF_PROF_CLASSES];
+    bool in_while_body;           // the decimation WHILE graph's body is being captured
+    bool pdl_now() const { return !prof_on && (in_while_body ? (pdl & 2) != 0 : (pdl & 1) != 0); }
 };
 
 // Per-class device time when profiling is on: ONE event is recorded on the stream whenever the kernel
@@ -111,6 +115,27 @@ struct ProfScope {
             return NEGF_ECUDA;                                      \
         }                                                           \
     } while (0)
+
+// Programmatic dependent launch (sm_90+): a kernel of the latency-bound chains (K2 small tiles, the one-CTA
+// inverses, the decimation step) is launched with the programmatic-stream-serialization attribute, so its
+// CTAs are placed on the SMs while the previous kernel of the stream drains; it calls pdl_wait() before its
+// first global-memory access (returns when the previous kernel has completed and its writes are visible) and
+// pdl_trigger() right after (so at most one waiting kernel is resident behind the running one).  Both are
+// no-ops in a kernel launched without the attribute.  Only kernels that call pdl_wait() may be launched this way.
+#ifdef __CUDACC__
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+#endif
+template <class... KArgs, class... Args>
+inline cudaError_t launch_chain(negf_ctx* ctx, void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, Args&&... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = ctx->stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = (ctx->pdl_now() ? 1 : 0);
+    return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
+}
 
 #define NEGF_TRY(expr)                   \
     do {                                 \

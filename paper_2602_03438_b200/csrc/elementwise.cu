@@ -108,6 +108,8 @@ __global__ void __launch_bounds__(256) sr_step_kernel(int b, cplx* a_s, cplx* a_
                                                       const double* ref, double tol, int* done, int* iters, int it,
                                                       double* acc, unsigned* ticket, const int* it_dev) {
     const int e = blockIdx.y;
+    pdl_wait();                               // programmatic dependent launch (common.cuh)
+    pdl_trigger();
     if (done[e]) return;
     if (it_dev) it += *it_dev;
     __shared__ double su[8], sl[8];
@@ -267,8 +269,8 @@ int ew_sr_step(negf_ctx* ctx, int b, int batch, cplx* a_s, cplx* a_b, cplx* g, c
     ProfScope _ps(ctx, NEGF_PROF_ELEMENTWISE);
     // one CTA per 16 K elements, at least 8 (the kernel is latency-bound per thread at small b), at most 128
     const int split = max(8, min(SR_SPLIT_MAX, (b * b + 16383) / 16384));
-    sr_step_kernel<<<dim3(split, batch), 256, 0, ctx->stream>>>(b, a_s, a_b, g, lgu, ugl, un, ln, ref, tol, done, iters, it,
-                                                                   acc, ticket, it_dev);
+    NEGF_CUDA_CHECK(ctx, launch_chain(ctx, sr_step_kernel, dim3(split, batch), dim3(256), 0, b, a_s, a_b, g, lgu, ugl, un, ln, ref, tol,
+                                      done, iters, it, acc, ticket, it_dev));
     NEGF_LAUNCH_CHECK(ctx);
     return NEGF_OK;
 }

@@ -144,6 +144,7 @@ int obc_core(negf_ctx* ctx, const negf_problem* p, int ns, const LeadBlocks* lb,
             cudaError_t ce = cudaStreamBeginCaptureToGraph(ctx->stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed);
             if (ce != cudaSuccess) { cudaGraphDestroy(G); ctx->last_cuda_error = (int)ce; return NEGF_ECUDA; }
             int rc = NEGF_OK;
+            ctx->in_while_body = true;
             const int dpb = 2;         // doublings per WHILE iteration (4 / 8 measured: 5.77 / 5.74 ms against 5.79 at configs[1])
             for (int q = 0; q < dpb && rc == NEGF_OK; q += 2) {
                 rc = doubling(ub[1], lbuf[1], ub[0], lbuf[0], q, it_dev);
@@ -152,6 +153,7 @@ int obc_core(negf_ctx* ctx, const negf_problem* p, int ns, const LeadBlocks* lb,
             if (rc == NEGF_OK) rc = ew_sr_cond(ctx, h, nb, W.done, it_dev, max_iter, dpb);
             cudaGraph_t dummy = nullptr;
             ce = cudaStreamEndCapture(ctx->stream, &dummy);
+            ctx->in_while_body = false;
             sf.use_main();
             if (rc != NEGF_OK) { cudaGraphDestroy(G); return rc; }
             if (ce != cudaSuccess) { cudaGraphDestroy(G); ctx->last_cuda_error = (int)ce; return NEGF_ECUDA; }

@@ -69,6 +69,8 @@ int ensure_children(negf_ctx* ctx, int G) {
         negf_ctx* c = ctx->child[g];
         c->stream = ctx->grp_stream[g];
         c->graph_loops = ctx->graph_loops; c->gemm_3m = ctx->gemm_3m; c->inv_tensor = ctx->inv_tensor; c->inv_panel = ctx->inv_panel; c->inv_lookahead = ctx->inv_lookahead; c->inv_outer = ctx->inv_outer; c->fused_small = ctx->fused_small;
+        // concurrent groups cover each other's launch gaps; a waiting dependent grid would only take their SM slots
+        if (c->pdl != 0) negf_set_option(c, NEGF_OPT_PDL, 0);
     }
     return NEGF_OK;
 }

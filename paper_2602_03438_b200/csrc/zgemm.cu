@@ -164,6 +164,9 @@ __global__ void __launch_bounds__(WM * WN * 32, MINB) zgemm_kernel(const __grid_
     cplx* sB = sA + STAGES * BM * BK;                          // STAGES x BN x BK
 
     const unsigned e2 = fastdiv(blockIdx.y, dv.b_mul, dv.b_sh), e = blockIdx.y - e2 * dv.batch;
+    // programmatic dependent launch (common.cuh): nothing of the previous kernel is read above this line
+    pdl_wait();
+    pdl_trigger();
     if (a.skip && a.skip[e]) return;
     const unsigned tm = fastdiv(blockIdx.x, dv.tn_mul, dv.tn_sh), tn = blockIdx.x - tm * dv.tiles_n;
     const int m0 = tm * BM, n0 = tn * BN;
@@ -432,7 +435,9 @@ int launch_cfg(negf_ctx* ctx, const GemmGroup& grp) {
     dim3 grid(tiles, a.batch * a.batch2, grp.ng);
     GemmDiv dv;
     dv.set((unsigned)tiles_n, (unsigned)a.batch);
-    kern<<<grid, WM * WN * 32, smem, ctx->stream>>>(grp, dv);
+    // the small tiles are the latency-bound chain steps: programmatic dependent launch (common.cuh)
+    if (BM <= 32) NEGF_CUDA_CHECK(ctx, launch_chain(ctx, kern, grid, dim3(WM * WN * 32), (size_t)smem, grp, dv));
+    else kern<<<grid, WM * WN * 32, smem, ctx->stream>>>(grp, dv);
     NEGF_LAUNCH_CHECK(ctx);
     return NEGF_OK;
 }

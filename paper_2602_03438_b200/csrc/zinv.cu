@@ -382,6 +382,8 @@ __global__ void __launch_bounds__(GJD_NT, 1) gj_dmma_kernel(cplx* A, long long s
     constexpr int N = 32 * TM, LD = N + 1, TR = 2 * TM, TC = TM, WC = 4, NRT = N / 8, UT = GJD_UW * 32, W = GJD_W;
     constexpr int PPT = 8 / W;                   // panels per 8-column tile
     const int e = blockIdx.x;
+    pdl_wait();                                  // programmatic dependent launch (common.cuh)
+    pdl_trigger();
     if (skip && skip[e]) return;
     extern __shared__ __align__(16) unsigned char gjd_smem[];
     cplx* mir = (cplx*)gjd_smem;                 // [2][N][LD]
@@ -1179,8 +1181,8 @@ int zinv_launch(negf_ctx* ctx, int b, cplx* A, long long sA, int batch, void* ws
     ProfScope _ps(ctx, NEGF_PROF_INVERSE);
     if (b <= 0 || batch <= 0) return NEGF_OK;
     if (b > 16 && b <= 64 && ctx->inv_tensor) {     // at b <= 16 the two kernels are level (15 us); the register one stays
-        if (b <= 32) gj_dmma_kernel<1><<<batch, GJD_NT, gjd_smem_bytes<1>(), ctx->stream>>>(A, sA, b, info, info_code, skip, code_dev);
-        else         gj_dmma_kernel<2><<<batch, GJD_NT, gjd_smem_bytes<2>(), ctx->stream>>>(A, sA, b, info, info_code, skip, code_dev);
+        if (b <= 32) NEGF_CUDA_CHECK(ctx, launch_chain(ctx, gj_dmma_kernel<1>, dim3(batch), dim3(GJD_NT), gjd_smem_bytes<1>(), A, sA, b, info, info_code, skip, code_dev));
+        else         NEGF_CUDA_CHECK(ctx, launch_chain(ctx, gj_dmma_kernel<2>, dim3(batch), dim3(GJD_NT), gjd_smem_bytes<2>(), A, sA, b, info, info_code, skip, code_dev));
         NEGF_LAUNCH_CHECK(ctx);
         return NEGF_OK;
     }

@@ -32,6 +32,7 @@ OPT_INV_PANEL = 5
 OPT_INV_LOOKAHEAD = 6
 OPT_INV_OUTER = 7
 OPT_FUSED_SMALL = 8
+OPT_PDL = 9
 
 
 class c128(C.Structure):
