@@ -264,14 +264,17 @@ def work_accounting(wl, res, steps, launches, gemm_3m, args_groups=0):
     bad = int((o["info_r"] != 0).sum() + (o["info_x"] != 0).sum() + (o["status_L"] != 0).sum() + (o["status_R"] != 0).sum())
     iters_mean = float((o["iters_L"].double().sum() + o["iters_R"].double().sum()) / (2 * dp.ne))
     iters_total = iters_mean * 2 * wl.n_energy
-    # NEGF_OPT_FUSED_SMALL automatic regime (fused_small.cuh:fused_small_regime): no WHILE graph
-    resident = wl.block_size <= 16 or (wl.block_size <= 32 and res.ne_batch <= 148)
-    if wl.block_size <= 96 and wl.max_iter % 2 == 0 and not resident:
-        # the doublings run inside a device-driven WHILE graph (one host launch per group): its kernels are counted
-        # from the iteration counters: 9 per pair of doublings (2 x [inverse, 2 grouped GEMMs, step] + loop condition)
-        it_max = int(max(o["iters_L"].max(), o["iters_R"].max()))
-        groups = args_groups or (4 if res.ne_batch >= 32 else 1)
-        launches += steps * len(res.batches) * groups * (-(-it_max // 2)) * 9
+    # The doublings run inside a device-driven WHILE graph (one host launch per group and lead batch), except in the
+    # resident regime of NEGF_OPT_FUSED_SMALL: its kernels are counted from the iteration counters, body executions x
+    # kernels per body (negf_obc_graph_kernels: 9 for b <= 96 = 2 x [inverse, 2 grouped GEMMs, step] + loop condition;
+    # the ~300 launches of two blocked inverses above).  Both leads are one batch up to b = 128, two graph launches above.
+    resident = wl.block_size <= 16 or (wl.block_size <= 32 and res.ne_batch <= 148)     # fused_small.cuh:fused_small_regime
+    body = 0 if resident else res.ctx.obc_graph_kernels()
+    if body > 0:
+        itl, itr = int(o["iters_L"].max()), int(o["iters_R"].max())
+        execs = -(-max(itl, itr) // 2) if wl.block_size <= 128 else -(-itl // 2) + -(-itr // 2)
+        groups = args_groups or (4 if (wl.block_size <= 96 and res.ne_batch >= 32) else 1)
+        launches += steps * len(res.batches) * groups * execs * body
     gemm_u, inv_u = unit_counts(wl.n_blocks, wl.sigma_kind, wl.want_greater, iters_total, wl.n_energy)
     if gemm_3m and wl.block_size > 64:
         gemm_u *= 0.75                      # executed DMMA flops of a 3M product: 6 b^3 instead of 8 b^3
@@ -322,6 +325,8 @@ def run_gpu(args, rank, local_rank, world):
         ctx.set_option(negf.OPT_ENERGY_GROUPS, args.energy_groups)
     if args.pdl >= 0:
         ctx.set_option(negf.OPT_PDL, args.pdl)
+    if args.graph_loops >= 0:
+        ctx.set_option(negf.OPT_GRAPH_LOOPS, args.graph_loops)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
     peak = ctx.fp64_peak(300.0)
     hbm_peak, hbm_src = measured_hbm_peak()
@@ -546,6 +551,7 @@ def main():
     ap.add_argument("--gemm-3m", action="store_true",
                     help="3M complex products in the compute-bound regime (NEGF_OPT_GEMM_3M); flops are then counted as executed (x 0.75 per product)")
     ap.add_argument("--energy-groups", type=int, default=0, help="NEGF_OPT_ENERGY_GROUPS (0 = the library's automatic choice)")
+    ap.add_argument("--graph-loops", type=int, default=-1, help="NEGF_OPT_GRAPH_LOOPS (-1 = the library's default)")
     ap.add_argument("--pdl", type=int, default=-1, help="NEGF_OPT_PDL (-1 = the library's default)")
     ap.add_argument("--energy-batch", type=int, default=0, help="energies resident at once (0 = fit HBM)")
     ap.add_argument("--e2e-energies", type=int, default=0)

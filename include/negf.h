@@ -115,10 +115,13 @@ int negf_workspace_bytes(const negf_problem* p, int kind_max, int flags, size_t*
 /* Caller-owned device scratch (e.g. a torch tensor), 256-byte aligned. Retained sweep state
  * lives here; replacing the workspace drops it. */
 int negf_set_workspace(negf_ctx* ctx, void* dev_ptr, size_t bytes);
-/* Options.  NEGF_OPT_GRAPH_LOOPS (default 1): for block sizes up to 96 the Sancho-Rubio doublings of
- * negf_obc_decimate[_pair] run as a cached device-driven WHILE graph (CUDA conditional node) that stops
- * when every energy has converged; 0 = the plain host loop of max_iter masked doublings.  Same
- * arithmetic and results either way.
+/* Options.  NEGF_OPT_GRAPH_LOOPS (default 2): the Sancho-Rubio doublings of negf_obc_decimate[_pair] run as a
+ * cached device-driven WHILE graph (CUDA conditional node) that stops when every energy has converged; 1 = only
+ * for block sizes up to 96 (larger blocks: the host loop); 0 = the plain host loop of max_iter masked doublings
+ * everywhere (and no cached call graphs).  Above b = 96 one masked doubling is ~300 launches of kernels that exit at
+ * once (the blocked inverse), and the stopping rule is met after ~22 of max_iter = 64 doublings: the graph takes
+ * 27 000 of the 42 000 launches of a configs[4] step away (12.56 -> 12.47 s; configs[3] 12.78 -> 12.61 s, configs[2]
+ * 1665 -> 1637 ms).  Same arithmetic and results either way (bit-identical, tested).
  * NEGF_OPT_GEMM_3M (default 0): in the compute-bound regime (blocks above 64 that fill the machine with
  * 128-row tiles) complex products use the 3M decomposition (three real DMMA products instead of four: 25 % fewer
  * tensor-pipe instructions; the imaginary part is accurate norm-wise, not component-wise).  Off by default: the
@@ -158,7 +161,9 @@ int negf_set_workspace(negf_ctx* ctx, void* dev_ptr, size_t bytes);
  * the dependent chain (b = 64, 64 energies, one stream: negf_rgf_retarded 1.78 -> 1.71 ms, negf_rgf_lesser_greater 2.80 ->
  * 2.69 ms).  Bit-identical results.  The concurrent energy groups of negf_pipeline_device / _host always run with 0:
  * they already cover each other's gaps, and a waiting grid would only take SM slots from the other groups (measured
- * 5.79 -> 6.12 ms per configs[1] step with it).  Changing the option drops the cached call graphs. */
+ * 5.79 -> 6.12 ms per configs[1] step with it).  Changing the option drops the cached call graphs.
+ * The environment variable NEGF_PDL (0..3), read by negf_create, overrides the default (developer switch to run a whole
+ * test suite under one setting). */
 #define NEGF_OPT_GRAPH_LOOPS   1
 #define NEGF_OPT_GEMM_3M       2
 #define NEGF_OPT_INV_TENSOR    3
@@ -175,6 +180,11 @@ const char* negf_strerror(int code);
 int negf_last_cuda_error(const negf_ctx* ctx);
 /* Number of kernels this context has launched since creation (bench.py's gpu_launches). */
 long long negf_launch_count(const negf_ctx* ctx);
+/* Kernels in ONE execution of the body (two doublings + the loop condition) of the cached decimation WHILE graph of
+ * this context, or of its first energy group when the groups hold the graphs; 0 when no such graph exists.  The
+ * graph's kernels run on the device without host launches, so negf_launch_count does not see its iterations:
+ * bench.py multiplies this by the executed iterations it reads from the iteration counters. */
+long long negf_obc_graph_kernels(const negf_ctx* ctx);
 
 /* Per-kernel-class device timing for bench.py's roofline: when enabled, one CUDA event is recorded on
  * the context stream whenever the kernel class of the next launch differs from the previous one, so the

@@ -28,7 +28,7 @@ extern "C" int negf_create(negf_ctx** out, int device) {
             cudaEventCreateWithFlags(&c->ev_join[k], cudaEventDisableTiming) != cudaSuccess) { delete c; return NEGF_ECUDA; }
     }
     if (cudaEventCreateWithFlags(&c->ev_aux, cudaEventDisableTiming) != cudaSuccess) { delete c; return NEGF_ECUDA; }
-    c->graph_loops = true; c->gemm_3m = false; c->inv_tensor = 1; c->inv_panel = 1; c->obc_exec = nullptr;
+    c->graph_loops = NEGF_GRAPH_LOOPS_DEFAULT; c->gemm_3m = false; c->inv_tensor = 1; c->inv_panel = 1; c->obc_exec = nullptr; c->obc_body_launches = 0;
     for (int k = 0; k < NEGF_NGRAPH; k++) for (int q = 0; q < NEGF_GWAYS; q++) c->gslot[k][q] = {0ull, nullptr, 0, 0u};
     c->gtick = 0;
     if (cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) != cudaSuccess) { delete c; return NEGF_ECUDA; }
@@ -95,7 +95,11 @@ extern "C" int negf_set_workspace(negf_ctx* ctx, void* p, size_t bytes) {
 }
 extern "C" int negf_set_option(negf_ctx* ctx, int option, int value) {
     if (!ctx) return NEGF_EINVAL;
-    if (option == NEGF_OPT_GRAPH_LOOPS) { ctx->graph_loops = value != 0; return NEGF_OK; }
+    if (option == NEGF_OPT_GRAPH_LOOPS) {
+        if (value < 0 || value > 2) return NEGF_EINVAL;
+        if (value != ctx->graph_loops && ctx->obc_exec) { cudaGraphExecDestroy(ctx->obc_exec); ctx->obc_exec = nullptr; ctx->obc_key_ws = nullptr; }
+        ctx->graph_loops = value; return NEGF_OK;
+    }
     if (option == NEGF_OPT_GEMM_3M) { ctx->gemm_3m = value != 0; return NEGF_OK; }
     if (option == NEGF_OPT_INV_TENSOR) { ctx->inv_tensor = value; return NEGF_OK; }
     if (option == NEGF_OPT_INV_PANEL) { ctx->inv_panel = value; return NEGF_OK; }
@@ -131,6 +135,13 @@ extern "C" const char* negf_strerror(int code) {
 }
 extern "C" int negf_last_cuda_error(const negf_ctx* ctx) { return ctx ? ctx->last_cuda_error : 0; }
 extern "C" long long negf_launch_count(const negf_ctx* ctx) { return ctx ? ctx->launches : 0; }
+extern "C" long long negf_obc_graph_kernels(const negf_ctx* ctx) {
+    if (!ctx) return 0;
+    if (ctx->obc_exec) return ctx->obc_body_launches;
+    for (int k = 0; k < NEGF_MAX_ENERGY_GROUPS; k++)
+        if (ctx->child[k] && ctx->child[k]->obc_exec) return ctx->child[k]->obc_body_launches;
+    return 0;
+}
 
 namespace {
 // closes the open interval and folds every finished interval into the per-class totals (synchronises)

@@ -11,7 +11,8 @@
 typedef double2 cplx;  // (x, y) = (re, im), same bytes as negf_c128
 constexpr int NEGF_NSIDE = 2;
 constexpr int NEGF_GWAYS = 4;     // cached argument sets per entry point (energy groups of negf_pipeline_host)
-constexpr int NEGF_PDL_DEFAULT = 1;   // negf_set_option(NEGF_OPT_PDL) at negf_create
+constexpr int NEGF_PDL_DEFAULT = 1;
+constexpr int NEGF_GRAPH_LOOPS_DEFAULT = 2;   // negf_set_option(NEGF_OPT_GRAPH_LOOPS) at negf_create   // negf_set_option(NEGF_OPT_PDL) at negf_create
 constexpr int NEGF_NGRAPH = 2;    // 0 negf_rgf_retarded, 1 negf_rgf_lesser_greater
 
 struct negf_ctx {
@@ -33,7 +34,7 @@ struct negf_ctx {
     bool sw_fused;                // the retained state is the one-sided state of the resident small-block kernel
     int fused_small;              // negf_set_option(NEGF_OPT_FUSED_SMALL)
     // cached device-driven WHILE graph of the Sancho-Rubio doublings (small blocks, obc.cu)
-    bool graph_loops;             // negf_set_option(NEGF_OPT_GRAPH_LOOPS)
+    int graph_loops;              // negf_set_option(NEGF_OPT_GRAPH_LOOPS): 0 off, 1 = b <= 96, 2 = every block size
     bool gemm_3m;                 // negf_set_option(NEGF_OPT_GEMM_3M)
     int inv_tensor;               // negf_set_option(NEGF_OPT_INV_TENSOR)
     int inv_panel;                // negf_set_option(NEGF_OPT_INV_PANEL)
@@ -57,6 +58,7 @@ struct negf_ctx {
     cudaStream_t grp_stream[NEGF_MAX_ENERGY_GROUPS];
     cudaEvent_t ev_grp_fork, ev_grp_mid[NEGF_MAX_ENERGY_GROUPS];
     cudaGraphExec_t obc_exec;
+    long long obc_body_launches;  // kernels in one execution of that graph's body
     // every pointer baked into that graph comes from carve_workspace(ws, n, b, ne) and the batch split ns x ne
     const void* obc_key_ws; int obc_key_b, obc_key_n, obc_key_ne, obc_key_ns, obc_key_maxit; double obc_key_tol;
     // optional per-kernel-class timing (negf_profile_enable): event pairs around every launch site
@@ -295,5 +297,5 @@ size_t zinv_workspace_bytes(int b, int batch);
 // in-place inverse of A[e] (b x b, ld = b, stride sA); ws: zinv_workspace_bytes; info_code = value
 // written to info[e] on a zero pivot (>0), info untouched otherwise (caller zero-fills).
 int zinv_launch(negf_ctx* ctx, int b, cplx* A, long long sA, int batch, void* ws, int* info,
-                int info_code, const int* skip, const int* code_dev = nullptr);   // small path: code = *code_dev + info_code
+                int info_code, const int* skip, const int* code_dev = nullptr);   // code = *code_dev + info_code (small kernels and the row-per-thread panels)
 

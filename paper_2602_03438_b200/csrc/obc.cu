@@ -13,6 +13,7 @@
 #include "kernels.cuh"
 #include "workspace.cuh"
 #include "fused_small.cuh"
+#include "zinv_rows.cuh"
 
 namespace {
 
@@ -117,7 +118,11 @@ int obc_core(negf_ctx* ctx, const negf_problem* p, int ns, const LeadBlocks* lb,
     // while any entry is active - no masked launches after convergence, no host synchronisation.
     // The graph is cached per (workspace, n, b, N_E, leads in the batch, tol, max_iter) - everything the baked-in
     // workspace offsets depend on - and dropped by negf_set_workspace; profiling runs use the plain loop.
-    const bool use_graph = b <= 96 && (max_iter % 2 == 0) && !ctx->prof_on && ctx->graph_loops;
+    // Above b = 96 (NEGF_OPT_GRAPH_LOOPS = 2) the body holds the ~300 launches of two blocked inverses with their
+    // look-ahead side stream (a fork and join inside the capture); the zero-pivot code of the row-per-thread panels
+    // follows the device iteration counter, the first-generation panel kernels have no such argument.
+    const bool use_graph = (b <= 96 || (ctx->graph_loops >= 2 && gj_panel_rows_supported(b) && ctx->inv_panel)) &&
+                           (max_iter % 2 == 0) && !ctx->prof_on && ctx->graph_loops;
     if (use_graph) {
         int* it_dev = W.tmpinfo;
         NEGF_TRY(ew_copy(ctx, bb, nb, ub[1], sb, U0, sb, nullptr));
@@ -144,6 +149,7 @@ int obc_core(negf_ctx* ctx, const negf_problem* p, int ns, const LeadBlocks* lb,
             cudaError_t ce = cudaStreamBeginCaptureToGraph(ctx->stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed);
             if (ce != cudaSuccess) { cudaGraphDestroy(G); ctx->last_cuda_error = (int)ce; return NEGF_ECUDA; }
             int rc = NEGF_OK;
+            const long long launches0 = ctx->launches;
             ctx->in_while_body = true;
             const int dpb = 2;         // doublings per WHILE iteration (4 / 8 measured: 5.77 / 5.74 ms against 5.79 at configs[1])
             for (int q = 0; q < dpb && rc == NEGF_OK; q += 2) {
@@ -160,6 +166,7 @@ int obc_core(negf_ctx* ctx, const negf_problem* p, int ns, const LeadBlocks* lb,
             ce = cudaGraphInstantiate(&ctx->obc_exec, G, 0);
             cudaGraphDestroy(G);
             if (ce != cudaSuccess) { ctx->obc_exec = nullptr; ctx->last_cuda_error = (int)ce; return NEGF_ECUDA; }
+            ctx->obc_body_launches = ctx->launches - launches0;
             ctx->obc_key_ws = ctx->ws; ctx->obc_key_b = b; ctx->obc_key_n = n; ctx->obc_key_ne = ne; ctx->obc_key_ns = ns; ctx->obc_key_maxit = max_iter; ctx->obc_key_tol = tol;
         }
         NEGF_CUDA_CHECK(ctx, cudaGraphLaunch(ctx->obc_exec, ctx->stream));

@@ -1237,7 +1237,7 @@ int zinv_launch(negf_ctx* ctx, int b, cplx* A, long long sA, int batch, void* ws
             // columns [-T D^-1 ; D^-1 ; -B D^-1] in place and LAPACK-style pivots in ipiv
             const long long mstride = (long long)batch * 2 * PW;
             int2* mv = W.moves + (size_t)(k0 / PW) * mstride;
-            RowsArgs ra{A, sA, b, k0, wk, W.ipiv, info, info_code, skip, mv};
+            RowsArgs ra{A, sA, b, k0, wk, W.ipiv, info, info_code, skip, code_dev, mv};
             NEGF_TRY(gj_panel_rows_launch(ctx, ra, batch));
             if (nbk > wk)      // the panel's exchanges on the other columns of K; pivot rows -> R, zeroed
                 NEGF_TRY(gj_moves_extract_launch(ctx, A, sA, b, batch, mv, mstride, 1, k0, wk, K0, K1, k0, k0 + wk, W.R, skip));
@@ -1293,7 +1293,6 @@ int zinv_launch(negf_ctx* ctx, int b, cplx* A, long long sA, int batch, void* ws
             }
             continue;
         }
-        // cluster size: smallest power of two whose slabs fit, at least wk rows per slab
         // cluster size: smallest power of two whose slabs fit, at least wk rows per slab
         int C = 1;
         while (C < CMAX && (size_t)((rows + C - 1) / C) * wk * sizeof(cplx) > (size_t)PANEL_SMEM_ROWS_BYTES) C <<= 1;

@@ -122,7 +122,7 @@ __device__ __forceinline__ void rows_step(const cplx (&x)[RW], cplx (&y)[RW], bo
         S.partner[J] = q;
         if (rank == 0) {
             a.ipiv[(size_t)e * a.b + pj] = q;
-            if (sing && a.info && a.info[e] == 0) a.info[e] = a.code > 0 ? a.code : pj + 1;
+            if (sing && a.info && a.info[e] == 0) a.info[e] = a.code > 0 ? a.code + (a.code_dev ? *a.code_dev : 0) : pj + 1;
         }
     }
     // ---- elimination on all other columns of the panel; the eliminated column becomes the transform column

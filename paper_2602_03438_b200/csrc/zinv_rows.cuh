@@ -8,6 +8,7 @@ struct RowsArgs {
     int* ipiv;                 // [batch][b]: ipiv[k] = row exchanged with row k at step k (LAPACK style)
     int* info; int code;       // info[e] = code (or column + 1 when code <= 0) on a zero pivot, first failure wins
     const int* skip;           // optional [batch]: entry skipped when != 0
+    const int* code_dev;       // optional device int added to code (iteration counter of the decimation WHILE graph)
     // net effect of the panel's row exchanges as independent moves: moves[e][2 j] = (k0 + j, source row),
     // moves[e][2 j + 1] = (partner position of step j, source row): "position dst now holds what row src held
     // before the panel" (duplicates agree).  [batch][2 * 32] int2; lets the other columns be permuted in parallel

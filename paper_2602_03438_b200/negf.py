@@ -73,7 +73,7 @@ class DeviceOutputs(C.Structure):
 
 
 EXPORTS = ["negf_create", "negf_destroy", "negf_set_stream", "negf_workspace_bytes", "negf_set_workspace",
-           "negf_set_option", "negf_strerror", "negf_last_cuda_error", "negf_launch_count",
+           "negf_set_option", "negf_strerror", "negf_last_cuda_error", "negf_launch_count", "negf_obc_graph_kernels",
            "negf_profile_enable", "negf_profile_read", "negf_obc_decimate", "negf_obc_decimate_pair",
            "negf_rgf_retarded", "negf_rgf_lesser_greater", "negf_observables", "negf_energy_convolve", "negf_pipeline_device",
            "negf_pipeline_host_bytes",
@@ -92,6 +92,8 @@ lib.negf_strerror.restype = C.c_char_p
 lib.negf_last_cuda_error.argtypes = [_P]
 lib.negf_launch_count.argtypes = [_P]
 lib.negf_launch_count.restype = C.c_longlong
+lib.negf_obc_graph_kernels.argtypes = [_P]
+lib.negf_obc_graph_kernels.restype = C.c_longlong
 lib.negf_profile_enable.argtypes = [_P, C.c_int]
 lib.negf_profile_read.argtypes = [_P, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_longlong), C.c_int]
 lib.negf_obc_decimate.argtypes = [_P, C.POINTER(Problem), C.POINTER(Lead), C.c_int, C.c_double, C.c_double,
@@ -201,6 +203,9 @@ class Context:
 
     def launch_count(self) -> int:
         return int(lib.negf_launch_count(self._h))
+
+    def obc_graph_kernels(self) -> int:
+        return int(lib.negf_obc_graph_kernels(self._h))
 
     def profile_enable(self, on: bool):
         self._check(lib.negf_profile_enable(self._h, int(on)), "negf_profile_enable")

@@ -196,7 +196,7 @@ def test_obc_pair_equals_two_single_calls(runner_mod, cfg, kw):
 
 @pytest.mark.parametrize("cfg,kw", [CASES[0], CASES[3]])
 def test_obc_graph_loop_equals_host_loop(runner_mod, negf_lib, cfg, kw):
-    """The device-driven WHILE graph of the doublings (CUDA conditional node, default for b <= 96) and the
+    """The device-driven WHILE graph of the doublings (CUDA conditional node, default) and the
     plain host loop of max_iter masked doublings run the same kernels on the same data: bit-identical."""
     wl = W.make_workload(cfg, **kw)
     dp = runner_mod.DevicePath(wl, want_greater=True)
@@ -210,6 +210,33 @@ def test_obc_graph_loop_equals_host_loop(runner_mod, negf_lib, cfg, kw):
     dp.obc()
     for k, v in graph.items():
         assert np.array_equal(v, dp.host(k)), k
+
+
+@pytest.mark.parametrize("cfg,kw", [(2, dict(n_blocks=3, block_size=130, n_energy=3)),
+                                    (3, dict(n_blocks=3, block_size=300, n_energy=5)),
+                                    (4, dict(n_blocks=2, block_size=640, n_energy=2))])
+def test_obc_graph_loop_above_96_equals_host_loop(runner_mod, negf_lib, cfg, kw):
+    """NEGF_OPT_GRAPH_LOOPS = 2 (default): the WHILE graph also above b = 96, where its body holds the launches of two blocked
+    inverses (panels, row moves, rank-k updates, the look-ahead side stream forked and joined inside the capture).
+    Same kernels on the same data as the host loop of masked doublings: bit-identical, first and replayed launch."""
+    wl = W.make_workload(cfg, **kw)
+    dp = runner_mod.DevicePath(wl, want_greater=True)
+    dp.ctx.set_option(negf_lib.OPT_GRAPH_LOOPS, 1)           # graph only up to b = 96: the host loop here
+    dp.obc()
+    host = {k: dp.host(k).copy() for k in dp.out if k.endswith(("_L", "_R"))}
+    assert int(dp.out["iters_L"].min()) > 5 and dp.host("status_L").tolist() == [0] * wl.n_energy
+    n_host = dp.ctx.launch_count()
+    assert dp.ctx.obc_graph_kernels() == 0
+    dp.ctx.set_option(negf_lib.OPT_GRAPH_LOOPS, 2)           # the default
+    for rep in range(2):
+        for k in host:
+            dp.out[k].zero_()
+        n0 = dp.ctx.launch_count()
+        dp.obc()
+        for k, v in host.items():
+            assert np.array_equal(v, dp.host(k)), (rep, k)
+        assert dp.ctx.launch_count() - n0 < n_host // 4       # no masked doublings enqueued by the host
+    assert dp.ctx.obc_graph_kernels() > 50                    # two blocked inverses and their products per body
 
 
 @pytest.mark.parametrize("cfg,kw", [CASES[0], CASES[3], CASES[6]])
