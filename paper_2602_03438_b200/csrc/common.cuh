@@ -283,7 +283,9 @@ int econv_prepare(negf_ctx* ctx);     // same for the energy-convolution kernels
 int fused_prepare(negf_ctx* ctx);     // same for the resident small-block kernels (fused_small.cu)
 // several independent products of identical shape / ops / batch in ONE launch (blockIdx.z = member)
 constexpr int NEGF_GEMM_GROUP_MAX = 4;
-struct GemmGroup { GemmArgs g[NEGF_GEMM_GROUP_MAX]; int ng; };
+// ragged_n: the members may differ in n (and in B, C, D); the grid is laid out for the widest member and the CTAs
+// beyond a member's last column tile exit at once (the two rank-w updates of a panel of the blocked inverse)
+struct GemmGroup { GemmArgs g[NEGF_GEMM_GROUP_MAX]; int ng; int ragged_n = 0; };
 int zgemm_launch_group(negf_ctx* ctx, const GemmGroup& grp);
 GemmArgs zgemm_bb_args(int opA, int opB, int b, cplx alpha, const cplx* A, long long sA, const cplx* B, long long sB,
                        cplx beta, const cplx* D, long long sD, cplx* C, long long sC, int batch, const int* skip);

@@ -170,6 +170,7 @@ __global__ void __launch_bounds__(WM * WN * 32, MINB) zgemm_kernel(const __grid_
     if (a.skip && a.skip[e]) return;
     const unsigned tm = fastdiv(blockIdx.x, dv.tn_mul, dv.tn_sh), tn = blockIdx.x - tm * dv.tiles_n;
     const int m0 = tm * BM, n0 = tn * BN;
+    if (n0 >= a.n) return;                 // GemmGroup::ragged_n: this member has fewer column tiles than the grid
     const cplx* gA = a.A + (size_t)e * a.sA + (size_t)e2 * a.sA2;
     const cplx* gB = a.B + (size_t)e * a.sB + (size_t)e2 * a.sB2;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -308,6 +309,7 @@ __global__ void __launch_bounds__(WM * WN * 32, 1) zgemm3m_kernel(const __grid_c
     if (a.skip && a.skip[e]) return;
     const unsigned tm = fastdiv(blockIdx.x, dv.tn_mul, dv.tn_sh), tn = blockIdx.x - tm * dv.tiles_n;
     const int m0 = tm * BM, n0 = tn * BN;
+    if (n0 >= a.n) return;                 // GemmGroup::ragged_n: this member has fewer column tiles than the grid
     const cplx* gA = a.A + (size_t)e * a.sA + (size_t)e2 * a.sA2;
     const cplx* gB = a.B + (size_t)e * a.sB + (size_t)e2 * a.sB2;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -485,14 +487,20 @@ int zgemm_prepare(negf_ctx* ctx) {
 int zgemm_launch_group(negf_ctx* ctx, const GemmGroup& grp) {
     ProfScope _ps(ctx, NEGF_PROF_GEMM);
     if (grp.ng < 1 || grp.ng > NEGF_GEMM_GROUP_MAX) return NEGF_EINVAL;
+    if (grp.ragged_n) {                     // lay the grid out for the widest member: it goes first
+        int w = 0;
+        for (int i = 1; i < grp.ng; i++) if (grp.g[i].n > grp.g[w].n) w = i;
+        if (grp.g[w].n <= 0) return NEGF_OK;
+        if (w != 0) { GemmGroup h = grp; h.g[0] = grp.g[w]; h.g[w] = grp.g[0]; return zgemm_launch_group(ctx, h); }
+    }
     const GemmArgs& a = grp.g[0];
     if (a.m <= 0 || a.n <= 0 || a.batch <= 0) return NEGF_OK;
     if (a.k < 0 || (a.opA | a.opB) & ~1) return NEGF_EINVAL;
     if (a.batch2 < 1 || (long long)a.batch * a.batch2 > 65535) return NEGF_EUNSUPPORTED;
     for (int i = 1; i < grp.ng; i++) {      // one grid serves every member: same shape, ops and batch
         const GemmArgs& o = grp.g[i];
-        if (o.m != a.m || o.n != a.n || o.k != a.k || o.opA != a.opA || o.opB != a.opB || o.batch != a.batch ||
-            o.batch2 != a.batch2)
+        if (o.m != a.m || (o.n != a.n && !grp.ragged_n) || o.k != a.k || o.opA != a.opA || o.opB != a.opB ||
+            o.batch != a.batch || o.batch2 != a.batch2)
             return NEGF_EINVAL;
     }
     // In-place products.  C == A is safe only when one CTA owns all n columns of the rows it reads (every read of

@@ -1242,16 +1242,19 @@ int zinv_launch(negf_ctx* ctx, int b, cplx* A, long long sA, int batch, void* ws
             if (nbk > wk)      // the panel's exchanges on the other columns of K; pivot rows -> R, zeroed
                 NEGF_TRY(gj_moves_extract_launch(ctx, A, sA, b, batch, mv, mstride, 1, k0, wk, K0, K1, k0, k0 + wk, W.R, skip));
             // M[:, other columns of K] += P' R, P' read from the panel's own columns
+            // (the columns before and after the panel: ONE launch, two members of different widths)
             g.alpha = one; g.beta = one; g.m = b; g.k = wk; g.A = A + k0; g.lda = b; g.sA = sA;
             g.ldb = b; g.sB = (long long)wk * b; g.ldc = b; g.sC = sA; g.sD = sA;
+            GemmGroup upd; upd.ng = 0; upd.ragged_n = 1;
             if (k0 > K0) {
                 g.n = k0 - K0; g.B = W.R + K0; g.C = A + K0; g.D = A + K0;
-                NEGF_TRY(zgemm_launch(ctx, g));
+                upd.g[upd.ng++] = g;
             }
             if (k0 + wk < K1) {
                 g.n = K1 - k0 - wk; g.B = W.R + k0 + wk; g.C = A + k0 + wk; g.D = A + k0 + wk;
-                NEGF_TRY(zgemm_launch(ctx, g));
+                upd.g[upd.ng++] = g;
             }
+            if (upd.ng) NEGF_TRY(zgemm_launch_group(ctx, upd));
             continue;
         }
         if (reg_panel) {

@@ -3,6 +3,7 @@ same seeded inputs.  Bar: relative Frobenius error <= 1e-10 per block (BASELINE.
 max over blocks and energies, no floor (reading R14)."""
 import numpy as np
 import pytest
+import torch
 
 from oracle import pipeline
 from paper_2602_03438_b200 import workloads as W
@@ -237,6 +238,35 @@ def test_obc_graph_loop_above_96_equals_host_loop(runner_mod, negf_lib, cfg, kw)
             assert np.array_equal(v, dp.host(k)), (rep, k)
         assert dp.ctx.launch_count() - n0 < n_host // 4       # no masked doublings enqueued by the host
     assert dp.ctx.obc_graph_kernels() > 50                    # two blocked inverses and their products per body
+
+
+@pytest.mark.parametrize("cfg,kw", [(1, dict(n_blocks=4, block_size=64, n_energy=32)),
+                                    (2, dict(n_blocks=3, block_size=200, n_energy=16))])
+def test_obc_graph_loop_stops_at_convergence(runner_mod, negf_lib, cfg, kw):
+    """The WHILE graph ends when every entry has met the stopping rule (~24 doublings): raising max_iter from 64 to
+    1024 changes neither the iteration counts nor the time of the call.  A loop that ran on to max_iter (as the host
+    loop of masked doublings does, and as the graph does under ncu, which does not see the device-side condition:
+    profiles/r02e_bench_lines.md) would take several times as long with ~1000 masked doublings behind the ~24 real ones."""
+    import dataclasses
+    wl = W.make_workload(cfg, **kw)
+    times, its = {}, {}
+    for mi in (64, 1024):
+        dp = runner_mod.DevicePath(dataclasses.replace(wl, max_iter=mi), want_greater=True)
+        for _ in range(3):
+            dp.obc()
+        torch.cuda.synchronize()
+        ts = []
+        for _ in range(7):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); dp.obc(); e1.record()
+            torch.cuda.synchronize()
+            ts.append(e0.elapsed_time(e1))
+        times[mi] = sorted(ts)[3]
+        its[mi] = (dp.host("iters_L").copy(), dp.host("iters_R").copy())
+        assert dp.host("status_L").tolist() == [0] * wl.n_energy
+    assert np.array_equal(its[64][0], its[1024][0]) and np.array_equal(its[64][1], its[1024][1])
+    assert int(its[64][0].max()) < 40
+    assert times[1024] < 1.3 * times[64], times
 
 
 @pytest.mark.parametrize("cfg,kw", [CASES[0], CASES[3], CASES[6]])
