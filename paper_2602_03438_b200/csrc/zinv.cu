@@ -1105,6 +1105,9 @@ constexpr int OUTER_NB_MAX = 256;  // widest outer block of the two-level blocke
 // With the addend prefetch of K2 (zgemm.cu) re-measured, nb = 64 / 128 / 256: b = 256 batch 256: 2.92 / 3.02 / 3.37; b = 512
 // batch 32: 2.91 / 2.91 / 3.26; b = 1024 batch 8: 4.76 / 5.18 / 5.71, batch 32: 15.36 / 14.33 / 14.73 (a large batch fills the
 // machine without the look-ahead's many short stages); b = 2048 batch 8: 29.3 / 26.5 / 26.4.
+// Last build of round 2 (K2's two-CTA tiles, merged rank-32 updates), nb = 64 / 128 / 256: b = 256 batch 256: 2.60 / 2.63 / 2.83;
+// b = 512 batch 32: 2.71 / 2.65 / 2.81; b = 1024 batch 8: 4.45 / 5.03 / 5.13, batch 32: 13.30 / 12.65 / 12.78; b = 2048 batch 8:
+// 25.8 / 24.1 / 23.6: the table below still picks the best of each row.
 inline int outer_nb(const negf_ctx* ctx, int b, int batch) {
     if (ctx->inv_outer >= 32 && ctx->inv_outer <= OUTER_NB_MAX && ctx->inv_outer % 32 == 0) return ctx->inv_outer;
     if (b > 1024) return 256;
