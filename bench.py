@@ -508,10 +508,25 @@ def run_e2e(args, wl, ctx, dev, world, torch, negf):
     n, b = wl.n_blocks, wl.block_size
     ne = min(wl.n_energy, args.e2e_energies or wl.n_energy)
     F = n * b * b * 16
-    while ne > 1 and ne * F * 12 > 24e9:      # keep pinned host memory bounded
+    cap = 24e9                                # pinned host memory: at most 48 GB and 30 % of what the box has free
+    try:
+        import psutil
+        cap = min(48e9, 0.3 * psutil.virtual_memory().available)
+    except Exception:
+        pass
+    while ne > 1 and ne * F * 12 > cap:
         ne //= 2
-    hp = runner.HostPath(wl, ne, device=dev, ctx=ctx)
-    up, down = hp.run()
+    hp = None
+    while hp is None:
+        try:
+            hp = runner.HostPath(wl, ne, device=dev, ctx=ctx)
+            up, down = hp.run()
+        except (RuntimeError, MemoryError):   # pinned or device allocation refused: fewer energies per call
+            hp = None
+            gc.collect(); torch.cuda.empty_cache()
+            if ne == 1:
+                raise
+            ne //= 2
     torch.cuda.synchronize()
     t0 = time.perf_counter(); up, down = hp.run(); est = time.perf_counter() - t0
     reps = max(1, min(args.steps, 5, int(15.0 / max(est, 1e-4))))
